@@ -1,0 +1,206 @@
+"""CPU oracle for the FlashNav simulator step -- TEST INFRASTRUCTURE, not the product.
+
+Thin ctypes/NumPy binding over `fn_oracle.c` (plain fp64 C written from PAPER.md).  Only tests/,
+bench.py's cpu_baseline / --impl reference legs and __graft_entry__.smoke() may import this package.
+It imports nothing from `paper_2606_15846_b200` (the CUDA path) and that package never imports this.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+import numpy as np
+
+_DIR = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_DIR, "fn_oracle.c")
+_LIB = os.path.join(_DIR, "libfnoracle.so")
+_lib = None
+
+EPS_CELL = 1e-5     # near-tie margin in cell units (BASELINE.json north_star)
+
+
+def build(force: bool = False) -> str:
+    """Compile fn_oracle.c with gcc (no FMA contraction: the fp32 reset arithmetic is single-rounded)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        subprocess.check_call(["gcc", "-O2", "-std=c99", "-ffp-contract=off", "-fPIC", "-shared",
+                               "-o", _LIB, _SRC, "-lm"])
+    return _LIB
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(build())
+        _lib.fno_splitmix64.restype = C.c_uint64
+        _lib.fno_splitmix64.argtypes = [C.c_uint64, C.c_uint64]
+    return _lib
+
+
+def _p(a, t):
+    return None if a is None else a.ctypes.data_as(C.POINTER(t))
+
+
+def _f32(a):
+    return np.ascontiguousarray(a, np.float32)
+
+
+def _u8(a):
+    return np.ascontiguousarray(a, np.uint8)
+
+
+def splitmix64(sigma: int, c: int) -> int:
+    return int(lib().fno_splitmix64(C.c_uint64(sigma), C.c_uint64(c)))
+
+
+def motion(drive, lim, dt, states, actions):
+    states, actions, lim = _f32(states), _f32(actions), _f32(lim)
+    n = states.shape[1]
+    out = np.empty_like(states)
+    lib().fno_motion(C.c_int(drive), _p(lim, C.c_float), C.c_float(dt), C.c_int(n),
+                     _p(states, C.c_float), _p(actions, C.c_float), _p(out, C.c_float))
+    return out
+
+
+def goal_obs(x, y, psi, gx, gy):
+    x, y, psi, gx, gy = map(_f32, (x, y, psi, gx, gy))
+    n = x.shape[0]
+    out = np.empty((2, n), np.float32)
+    lib().fno_goal_obs(C.c_int(n), *[_p(a, C.c_float) for a in (x, y, psi, gx, gy)],
+                       _p(out[0], C.c_float), _p(out[1], C.c_float))
+    return out
+
+
+def reward_done(d_new, collision, forced, d_prev, ep_step, goal_tol=0.3, max_episode_steps=0,
+                r_success=10.0, r_collision=-10.0, c_progress=2.0):
+    """Updates d_prev (float32) and ep_step (int32) in place; returns reward, done."""
+    d_new, collision = _f32(d_new), _u8(collision)
+    forced = None if forced is None else _u8(forced)
+    assert d_prev.dtype == np.float32 and ep_step.dtype == np.int32
+    n = d_new.shape[0]
+    reward = np.empty(n, np.float32)
+    done = np.empty(n, np.uint8)
+    lib().fno_reward_done(C.c_int(n), _p(d_new, C.c_float), _p(collision, C.c_uint8),
+                          _p(forced, C.c_uint8), C.c_float(goal_tol), C.c_int(max_episode_steps),
+                          C.c_float(r_success), C.c_float(r_collision), C.c_float(c_progress),
+                          _p(d_prev, C.c_float), _p(ep_step, C.c_int32), _p(reward, C.c_float),
+                          _p(done, C.c_uint8))
+    return reward, done
+
+
+def collision(occ, res, footprint, x, y, psi, eps=EPS_CELL):
+    occ, fp = _u8(occ), _f32(footprint)
+    x, y, psi = map(_f32, (x, y, psi))
+    H, W = occ.shape
+    n = x.shape[0]
+    flag = np.empty(n, np.uint8)
+    amb = np.empty(n, np.uint8)
+    lib().fno_collision(_p(occ, C.c_uint8), C.c_int(H), C.c_int(W), C.c_float(res),
+                        C.c_int(fp.shape[0]), _p(fp, C.c_float), C.c_int(n), _p(x, C.c_float),
+                        _p(y, C.c_float), _p(psi, C.c_float), C.c_double(eps),
+                        _p(flag, C.c_uint8), _p(amb, C.c_uint8))
+    return flag, amb
+
+
+def collision_sampled(occ, res, footprint, h, x, y, psi):
+    occ, fp = _u8(occ), _f32(footprint)
+    x, y, psi = map(_f32, (x, y, psi))
+    H, W = occ.shape
+    n = x.shape[0]
+    flag = np.empty(n, np.uint8)
+    lib().fno_collision_sampled(_p(occ, C.c_uint8), C.c_int(H), C.c_int(W), C.c_float(res),
+                                C.c_int(fp.shape[0]), _p(fp, C.c_float), C.c_double(h), C.c_int(n),
+                                _p(x, C.c_float), _p(y, C.c_float), _p(psi, C.c_float),
+                                _p(flag, C.c_uint8))
+    return flag
+
+
+def ranges(occ, res, angles, max_range, x, y, psi, eps=EPS_CELL, sensor=None, want_visits=False):
+    """Returns ranges [n,B] f32, hit [n,B] i32, amb [n,B] u8 (, visits [n,B] i32)."""
+    occ, angles = _u8(occ), _f32(angles)
+    x, y, psi = map(_f32, (x, y, psi))
+    sensor = None if sensor is None else _f32(sensor)
+    H, W = occ.shape
+    n, B = x.shape[0], angles.shape[0]
+    r = np.empty((n, B), np.float32)
+    hit = np.empty((n, B), np.int32)
+    amb = np.empty((n, B), np.uint8)
+    vis = np.empty((n, B), np.int32) if want_visits else None
+    lib().fno_ranges(_p(occ, C.c_uint8), C.c_int(H), C.c_int(W), C.c_float(res), C.c_int(B),
+                     _p(angles, C.c_float), C.c_float(max_range), _p(sensor, C.c_float), C.c_int(n),
+                     _p(x, C.c_float), _p(y, C.c_float), _p(psi, C.c_float), C.c_double(eps),
+                     _p(r, C.c_float), _p(hit, C.c_int32), _p(amb, C.c_uint8), _p(vis, C.c_int32))
+    return (r, hit, amb, vis) if want_visits else (r, hit, amb)
+
+
+def ranges_fixed_step(occ, res, angles, max_range, delta, x, y, psi):
+    occ, angles = _u8(occ), _f32(angles)
+    x, y, psi = map(_f32, (x, y, psi))
+    H, W = occ.shape
+    n, B = x.shape[0], angles.shape[0]
+    r = np.empty((n, B), np.float32)
+    lib().fno_ranges_fixed_step(_p(occ, C.c_uint8), C.c_int(H), C.c_int(W), C.c_float(res),
+                                C.c_int(B), _p(angles, C.c_float), C.c_float(max_range),
+                                C.c_double(delta), C.c_int(n), _p(x, C.c_float), _p(y, C.c_float),
+                                _p(psi, C.c_float), _p(r, C.c_float))
+    return r
+
+
+def reset(occ, res, footprint, regions, goal_dist_min, goal_dist_max, mask, seeds, states, d_prev,
+          ep_step, eps=EPS_CELL):
+    """In place on states [8,n] f32, d_prev f32, ep_step i32 for masked envs. Returns amb, failed."""
+    occ, fp, mask = _u8(occ), _f32(footprint), _u8(mask)
+    seeds = np.ascontiguousarray(seeds, np.uint64)
+    assert states.dtype == np.float32 and states.flags.c_contiguous
+    assert d_prev.dtype == np.float32 and ep_step.dtype == np.int32
+    H, W = occ.shape
+    n = states.shape[1]
+    nreg = 0 if regions is None else int(regions.shape[0])
+    reg = None if regions is None else np.ascontiguousarray(regions, np.int32)
+    amb = np.empty(n, np.uint8)
+    failed = np.empty(n, np.uint8)
+    lib().fno_reset(_p(occ, C.c_uint8), C.c_int(H), C.c_int(W), C.c_float(res), C.c_int(fp.shape[0]),
+                    _p(fp, C.c_float), C.c_int(nreg), _p(reg, C.c_int32), C.c_float(goal_dist_min),
+                    C.c_float(goal_dist_max), C.c_int(n), _p(mask, C.c_uint8), _p(seeds, C.c_uint64),
+                    C.c_double(eps), _p(states, C.c_float), _p(d_prev, C.c_float),
+                    _p(ep_step, C.c_int32), _p(amb, C.c_uint8), _p(failed, C.c_uint8))
+    return amb, failed
+
+
+def ring_append(ring, capacity, head, obs_ranges, obs_goal, obs_vel, actions, reward, done):
+    obs_ranges, obs_goal, obs_vel, actions, reward = map(_f32, (obs_ranges, obs_goal, obs_vel,
+                                                                actions, reward))
+    done = _u8(done)
+    n, B = obs_ranges.shape
+    A = actions.shape[1]
+    assert ring.dtype == np.float32 and ring.flags.c_contiguous
+    lib().fno_ring_append(_p(ring, C.c_float), C.c_uint64(capacity), C.c_uint64(head), C.c_int(n),
+                          C.c_int(B), C.c_int(A), _p(obs_ranges, C.c_float), _p(obs_goal, C.c_float),
+                          _p(obs_vel, C.c_float), _p(actions, C.c_float), _p(reward, C.c_float),
+                          _p(done, C.c_uint8))
+
+
+def step(wl, states, actions, forced, d_prev, ep_step, want_hit=True):
+    """One whole vector step on a harness Workload-like object (fields only; no harness import).
+    states [8,n] f32 updated in place.  Returns dict(ranges, hit, collision, goal_obs, reward, done)."""
+    occ, fp, ang, lim = _u8(wl.occ), _f32(wl.footprint), _f32(wl.beam_angles), _f32(wl.vel_limits)
+    actions = _f32(actions)
+    forced = None if forced is None else _u8(forced)
+    assert states.dtype == np.float32 and states.flags.c_contiguous
+    H, W = occ.shape
+    n, B = states.shape[1], ang.shape[0]
+    r = np.empty((n, B), np.float32)
+    hit = np.empty((n, B), np.int32) if want_hit else None
+    col = np.empty(n, np.uint8)
+    gobs = np.empty((2, n), np.float32)
+    rew = np.empty(n, np.float32)
+    done = np.empty(n, np.uint8)
+    lib().fno_step(_p(occ, C.c_uint8), C.c_int(H), C.c_int(W), C.c_float(wl.resolution),
+                   C.c_int(fp.shape[0]), _p(fp, C.c_float), C.c_int(B), _p(ang, C.c_float),
+                   C.c_float(wl.max_range), C.c_int(wl.drive), _p(lim, C.c_float), C.c_float(wl.dt),
+                   C.c_float(wl.goal_tol), C.c_int(wl.max_episode_steps), C.c_float(wl.r_success),
+                   C.c_float(wl.r_collision), C.c_float(wl.c_progress), C.c_int(n),
+                   _p(states, C.c_float), _p(actions, C.c_float), _p(forced, C.c_uint8),
+                   _p(d_prev, C.c_float), _p(ep_step, C.c_int32), _p(r, C.c_float),
+                   _p(hit, C.c_int32), _p(col, C.c_uint8), _p(gobs, C.c_float), _p(rew, C.c_float),
+                   _p(done, C.c_uint8))
+    return dict(ranges=r, hit=hit, collision=col, goal_obs=gobs, reward=rew, done=done)

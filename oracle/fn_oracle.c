@@ -1,0 +1,542 @@
+/*
+ * fn_oracle.c -- CPU ORACLE for the FlashNav batched simulator step (arxiv/paper_2606_15846).
+ *
+ * TEST INFRASTRUCTURE ONLY.  Plain, slow, single-threaded, fp64 C.  Only tests/, bench.py's
+ * cpu_baseline / --impl reference legs and __graft_entry__.smoke() may load this library.  It shares
+ * no code, header, table or helper with the CUDA path under paper_2606_15846_b200/ and neither
+ * imports the other.
+ *
+ * What it computes (citations are PAPER.md lines; "SURVEY 8(c)" = /root/repo/SURVEY.md section 8(c),
+ * whose readings are restated in DESIGN.md "Readings of the paper"):
+ *   O1/O2  action clip + planar motion update for (v_x, w) / (v_x, v_y, w) body-frame commands
+ *          (integrator = exact constant-twist arc, reading G1).
+ *   O3     footprint collision: Eq. (2), taken to the limit of a zero footprint
+ *          sampling interval = closed polygon vs closed occupied cell; outside the map = collision.
+ *   O4     range sensing: PAPER.md:86 fixed-step beam samples taken to the limit of a zero step =
+ *          distance to the first occupied cell along the beam; no hit => max range.
+ *   O5     goal distance d and direction alpha relative to the robot.
+ *   O6     reward Eq. (1), PAPER.md:69-72 (r_success=10, r_collision=-10, c_1=2) and termination.
+ *   O7     reset of masked envs (PAPER.md:86, :199 say THAT envs are reset; the sampling rule is
+ *          reading G16 -- "parity unpinned" by the paper, pinned by invariants only).
+ *   O9     transition row for the replay ring (BASELINE.json config 5).
+ *   plus the paper's own two approximations as brute-force cross-checks:
+ *          fno_ranges_fixed_step and fno_collision_sampled (Eq. (2)).
+ *
+ * Conventions (reading G7): map-frame origin at the outer corner of cell (row 0, col 0); x grows with
+ * column, y with row; cell (i,j) = [j rho,(j+1) rho) x [i rho,(i+1) rho); linear index i*W + j;
+ * anything outside [0,W) x [0,H) is occupied (PAPER.md:123 for collision; reading G6 for beams).
+ * All inputs are fp32 and are widened exactly to fp64; outputs are rounded once to fp32.
+ *
+ * Pins (tests/test_oracle_*.py): motion -> closed-form arc / composition; ranges -> empty map, wall,
+ * single-cell slab closed form, the paper's fixed-step march, 90-degree symmetry; collision -> interval
+ * overlap, notch case, Eq. (2) sampling, point-in-polygon supersampling; reward ->
+ * Eq. (1) constants.  UNPINNED by the paper: reset distribution, goal tolerance, episode limit.
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+#define FNO_PI 3.14159265358979323846
+
+enum { FNO_DRIVE_DIFF = 0, FNO_DRIVE_OMNI = 1 };
+
+/* ------------------------------------------------------------------ map lookup (G6, G7) */
+
+static int occ_at(const uint8_t* occ, int H, int W, long i, long j) {
+    if (i < 0 || j < 0 || i >= H || j >= W) return 1;          /* outside the map => occupied */
+    return occ[(size_t)i * (size_t)W + (size_t)j] != 0;
+}
+
+static double wrap_pi(double a) {                               /* to [-pi, pi) (G4) */
+    double r = fmod(a + FNO_PI, 2.0 * FNO_PI);
+    if (r < 0.0) r += 2.0 * FNO_PI;
+    return r - FNO_PI;
+}
+
+/* ------------------------------------------------------------------ O1 + O2: clip and motion
+ * commands (v_x, w) [diff] or (v_x, v_y, w) [omni], body frame, "within the configured
+ * bounds".  Reading G1: the pose is advanced by the exact constant-twist SE(2) step
+ *   th = w dt,  A = sin(th)/th,  C = (1-cos th)/th = sin^2(th/2)/(th/2)
+ *   body displacement = dt (A v_x - C v_y, C v_x + A v_y),  p' = p + R(psi) * body displacement,
+ *   psi' = wrap(psi + th),  v' = clipped command.
+ * states: SoA planes [8][n] = x, y, psi, vx, vy, w, gx, gy.  actions: [n][A].
+ */
+void fno_motion(int drive, const float* lim /*[6]*/, float dt_f, int n,
+                const float* s_in, const float* actions, float* s_out) {
+    const int A = (drive == FNO_DRIVE_DIFF) ? 2 : 3;
+    const double dt = (double)dt_f;
+    for (int e = 0; e < n; ++e) {
+        double x = s_in[0 * n + e], y = s_in[1 * n + e], psi = s_in[2 * n + e];
+        double vx = actions[e * A + 0], vy = 0.0, w;
+        if (drive == FNO_DRIVE_DIFF) { w = actions[e * A + 1]; }
+        else { vy = actions[e * A + 1]; w = actions[e * A + 2]; }
+        /* O1: clamp each component to U's velocity limits */
+        vx = fmin(fmax(vx, (double)lim[0]), (double)lim[1]);
+        if (drive == FNO_DRIVE_OMNI) vy = fmin(fmax(vy, (double)lim[2]), (double)lim[3]);
+        w = fmin(fmax(w, (double)lim[4]), (double)lim[5]);
+        /* O2 */
+        double th = w * dt, Ac, Cc;
+        if (fabs(th) < 1e-8) { Ac = 1.0 - th * th / 6.0; Cc = th / 2.0; }
+        else { double sh = sin(0.5 * th); Ac = sin(th) / th; Cc = sh * sh / (0.5 * th); }
+        double bx = dt * (Ac * vx - Cc * vy), by = dt * (Cc * vx + Ac * vy);
+        double c = cos(psi), s = sin(psi);
+        s_out[0 * n + e] = (float)(x + c * bx - s * by);
+        s_out[1 * n + e] = (float)(y + s * bx + c * by);
+        s_out[2 * n + e] = (float)wrap_pi(psi + th);
+        s_out[3 * n + e] = (float)vx;
+        s_out[4 * n + e] = (float)vy;
+        s_out[5 * n + e] = (float)w;
+        s_out[6 * n + e] = s_in[6 * n + e];
+        s_out[7 * n + e] = s_in[7 * n + e];
+    }
+}
+
+/* ------------------------------------------------------------------ O5: goal observation
+ * d_t = goal distance, alpha_t = goal direction relative to the robot heading.
+ */
+void fno_goal_obs(int n, const float* x, const float* y, const float* psi,
+                  const float* gx, const float* gy, float* d_out, float* alpha_out) {
+    for (int e = 0; e < n; ++e) {
+        double dx = (double)gx[e] - (double)x[e], dy = (double)gy[e] - (double)y[e];
+        d_out[e] = (float)sqrt(dx * dx + dy * dy);
+        alpha_out[e] = (float)wrap_pi(atan2(dy, dx) - (double)psi[e]);
+    }
+}
+
+/* ------------------------------------------------------------------ O6: reward and termination
+ * Eq. (1): r = r_collision on collision; r_success when the goal is reached WITHOUT
+ * collision; c_1 (d_t - d_{t+1}) otherwise.  done = collision | reached | episode limit | forced.
+ * d_prev and ep_step are per-env episode state, updated in place (reading G17: d_prev is from the
+ * same episode; reset re-seeds it).
+ */
+void fno_reward_done(int n, const float* d_new, const uint8_t* collision, const uint8_t* forced,
+                     float goal_tol, int max_episode_steps, float r_success, float r_collision,
+                     float c_progress, float* d_prev, int32_t* ep_step, float* reward,
+                     uint8_t* done) {
+    for (int e = 0; e < n; ++e) {
+        int c = collision[e] != 0;
+        int reached = (double)d_new[e] < (double)goal_tol;
+        double r;
+        if (c) r = (double)r_collision;
+        else if (reached) r = (double)r_success;
+        else r = (double)c_progress * ((double)d_prev[e] - (double)d_new[e]);
+        int limit = (max_episode_steps > 0) && (ep_step[e] + 1 >= max_episode_steps);
+        reward[e] = (float)r;
+        done[e] = (uint8_t)(c || reached || limit || (forced && forced[e]));
+        d_prev[e] = d_new[e];
+        ep_step[e] += 1;
+    }
+}
+
+/* ------------------------------------------------------------------ O3: footprint collision
+ * Eq. (2): c = OR over footprint samples s of M(R(psi) s + p); a collision is
+ * detected if any sample lies in an occupied cell or outside the map.  The footprint "interior and
+ * boundary are sampled at a configured spatial resolution".  Taking the sampling
+ * interval to zero, the sample set becomes the closed polygon region, so
+ *   c = 1  iff  some occupied-or-outside cell's closed unit square meets the closed polygon region.
+ * Square vs simple polygon: they meet iff (some polygon edge meets the closed square) or (the
+ * square's centre is inside the polygon).  [If no edge meets the square, the square lies wholly
+ * inside or wholly outside the polygon, and its centre decides which.]
+ *
+ * Near-tie rule, margin eps in cell units: a cell ROBUSTLY intersects if an edge meets
+ * the square shrunk by eps per side or the centre is inside; it is ROBUSTLY disjoint if no edge meets
+ * the square grown by eps and the centre is outside.  The flag is ambiguous iff no occupied cell
+ * robustly intersects and some occupied cell is not robustly disjoint.
+ */
+
+/* closed segment P->Q vs closed box, by slab clipping of the segment parameter (Liang-Barsky) */
+static int seg_meets_box(double px, double py, double qx, double qy,
+                         double xlo, double xhi, double ylo, double yhi) {
+    double t0 = 0.0, t1 = 1.0;
+    double dx = qx - px, dy = qy - py;
+    double p[4] = { -dx, dx, -dy, dy };
+    double q[4] = { px - xlo, xhi - px, py - ylo, yhi - py };
+    for (int k = 0; k < 4; ++k) {
+        if (p[k] == 0.0) { if (q[k] < 0.0) return 0; }
+        else {
+            double r = q[k] / p[k];
+            if (p[k] < 0.0) { if (r > t1) return 0; if (r > t0) t0 = r; }
+            else            { if (r < t0) return 0; if (r < t1) t1 = r; }
+        }
+    }
+    return t0 <= t1;
+}
+
+/* even-odd crossing rule; polygon may be CW or CCW, collinear vertices allowed (G13) */
+static int point_in_poly(int V, const double* vx, const double* vy, double px, double py) {
+    int inside = 0;
+    for (int a = 0, b = V - 1; a < V; b = a++) {
+        if ((vy[a] > py) != (vy[b] > py)) {
+            double xc = (vx[b] - vx[a]) * (py - vy[a]) / (vy[b] - vy[a]) + vx[a];
+            if (px < xc) inside = !inside;
+        }
+    }
+    return inside;
+}
+
+#define FNO_MAX_V 256
+
+/* one pose -> flag (return value) and ambiguity (*amb) */
+static int collision_one(const uint8_t* occ, int H, int W, double rho, int V, const float* fp_xy,
+                         double x, double y, double psi, double eps, int* amb) {
+    double vx[FNO_MAX_V], vy[FNO_MAX_V];
+    double c = cos(psi), s = sin(psi);
+    double xmin = INFINITY, xmax = -INFINITY, ymin = INFINITY, ymax = -INFINITY;
+    for (int k = 0; k < V; ++k) {
+        double fx = fp_xy[2 * k], fy = fp_xy[2 * k + 1];
+        vx[k] = (x + c * fx - s * fy) / rho;                    /* cell units */
+        vy[k] = (y + s * fx + c * fy) / rho;
+        xmin = fmin(xmin, vx[k]); xmax = fmax(xmax, vx[k]);
+        ymin = fmin(ymin, vy[k]); ymax = fmax(ymax, vy[k]);
+    }
+    long j0 = (long)floor(xmin - eps), j1 = (long)floor(xmax + eps);
+    long i0 = (long)floor(ymin - eps), i1 = (long)floor(ymax + eps);
+    int flag = 0, robust = 0, near = 0;
+    for (long i = i0; i <= i1; ++i) for (long j = j0; j <= j1; ++j) {
+        if (!occ_at(occ, H, W, i, j)) continue;
+        double xl = (double)j, yl = (double)i;
+        int in_c = point_in_poly(V, vx, vy, xl + 0.5, yl + 0.5);
+        int e_exact = 0, e_shrunk = 0, e_grown = 0;
+        for (int a = 0, b = V - 1; a < V; b = a++) {
+            if (seg_meets_box(vx[b], vy[b], vx[a], vy[a], xl - eps, xl + 1 + eps, yl - eps, yl + 1 + eps)) {
+                e_grown = 1;
+                if (seg_meets_box(vx[b], vy[b], vx[a], vy[a], xl, xl + 1, yl, yl + 1)) e_exact = 1;
+                if (seg_meets_box(vx[b], vy[b], vx[a], vy[a], xl + eps, xl + 1 - eps, yl + eps, yl + 1 - eps)) e_shrunk = 1;
+            }
+        }
+        if (e_exact || in_c) flag = 1;
+        if (e_shrunk || in_c) robust = 1;
+        if (e_grown || in_c) near = 1;
+    }
+    if (amb) *amb = (!robust && near);
+    return flag;
+}
+
+void fno_collision(const uint8_t* occ, int H, int W, float res, int V, const float* fp_xy, int n,
+                   const float* x, const float* y, const float* psi, double eps,
+                   uint8_t* flag, uint8_t* amb) {
+    for (int e = 0; e < n; ++e) {
+        int a = 0;
+        flag[e] = (uint8_t)collision_one(occ, H, W, (double)res, V, fp_xy, x[e], y[e], psi[e], eps, &a);
+        if (amb) amb[e] = (uint8_t)a;
+    }
+}
+
+/* Eq. (2) exactly as the paper states it: sample the footprint interior and
+ * boundary at spacing h (metres, body frame), cache the point set, OR the occupancy of the cells the
+ * transformed samples fall in.  Cross-check only: sampled => exact always; exact-by-a-margin => sampled.
+ * Interior: body-frame lattice points inside the polygon; boundary: points every <= h along each edge.
+ */
+void fno_collision_sampled(const uint8_t* occ, int H, int W, float res, int V, const float* fp_xy,
+                           double h, int n, const float* x, const float* y, const float* psi,
+                           uint8_t* flag) {
+    double bx[FNO_MAX_V], by[FNO_MAX_V];
+    double xmin = INFINITY, xmax = -INFINITY, ymin = INFINITY, ymax = -INFINITY;
+    for (int k = 0; k < V; ++k) {
+        bx[k] = fp_xy[2 * k]; by[k] = fp_xy[2 * k + 1];
+        xmin = fmin(xmin, bx[k]); xmax = fmax(xmax, bx[k]);
+        ymin = fmin(ymin, by[k]); ymax = fmax(ymax, by[k]);
+    }
+    size_t cap = 1024, np_ = 0;
+    double* P = (double*)malloc(cap * 2 * sizeof(double));
+#define PUSH(px_, py_) do { if (np_ == cap) { cap *= 2; P = (double*)realloc(P, cap * 2 * sizeof(double)); } \
+                            P[2 * np_] = (px_); P[2 * np_ + 1] = (py_); ++np_; } while (0)
+    for (double yy = ymin; yy <= ymax; yy += h)
+        for (double xx = xmin; xx <= xmax; xx += h)
+            if (point_in_poly(V, bx, by, xx, yy)) PUSH(xx, yy);
+    for (int a = 0, b = V - 1; a < V; b = a++) {
+        double ex = bx[a] - bx[b], ey = by[a] - by[b];
+        int m = (int)ceil(sqrt(ex * ex + ey * ey) / h);
+        if (m < 1) m = 1;
+        for (int k = 0; k <= m; ++k) PUSH(bx[b] + ex * k / m, by[b] + ey * k / m);
+    }
+#undef PUSH
+    double rho = (double)res;
+    for (int e = 0; e < n; ++e) {
+        double c = cos((double)psi[e]), s = sin((double)psi[e]);
+        int f = 0;
+        for (size_t k = 0; k < np_ && !f; ++k) {
+            double wx = ((double)x[e] + c * P[2 * k] - s * P[2 * k + 1]) / rho;
+            double wy = ((double)y[e] + s * P[2 * k] + c * P[2 * k + 1]) / rho;
+            f = occ_at(occ, H, W, (long)floor(wy), (long)floor(wx));
+        }
+        flag[e] = (uint8_t)f;
+    }
+    free(P);
+}
+
+/* ------------------------------------------------------------------ O4: range sensing
+ * "Range sensing uses fixed-step samples along each beam."  With step Delta the range is
+ * the first sample distance whose cell is occupied; as Delta -> 0 this becomes
+ *   r = rho * inf{ t >= 0 : M(cell(o + t d)) = 1 },  capped at r_max,   no hit => r_max
+ * with o the sensor origin in cell units and d = (cos phi, sin phi), phi = psi + s_psi + theta_j.
+ * The infimum is found by walking the grid cell by cell (Amanatides-Woo): the next vertical /
+ * horizontal cell boundary along the beam is at parameter t_x = (b_x - o_x)/d_x, t_y = (b_y - o_y)/d_y,
+ * each computed DIRECTLY from the boundary coordinate (never accumulated); the smaller one is crossed
+ * first.  The first occupied (or outside-map) cell entered at t_hit < r_max/rho gives
+ *   range = t_hit * rho, hit = i*W + j  (-2 if that cell is outside the map);
+ * origin already in an occupied cell => range 0; otherwise range = r_max, hit = -1.
+ *
+ * Near-tie rule, eps in cells: a beam is ambiguous iff, up to and including the entry
+ * into the hit cell, it passes within eps of a lattice corner whose four surrounding cells do not all
+ * have the same occupancy, or |t_hit - r_max/rho| < eps (also: an occupied cell first entered within
+ * eps beyond r_max/rho), or the origin lies within eps of a cell edge separating different occupancy.
+ * sensor[3] = (s_x, s_y, s_psi) body-frame sensor placement (reading G8), NULL = 0.
+ * visits (optional, per beam): number of cells the walk entered (workload statistics only).
+ */
+static int corner_mixed(const uint8_t* occ, int H, int W, long cx, long cy) {
+    int a = occ_at(occ, H, W, cy - 1, cx - 1), b = occ_at(occ, H, W, cy - 1, cx);
+    int c = occ_at(occ, H, W, cy, cx - 1),     d = occ_at(occ, H, W, cy, cx);
+    return !(a == b && b == c && c == d);
+}
+
+static void ray_one(const uint8_t* occ, int H, int W, double rho, double ox, double oy, double phi,
+                    double T, double rmax, double eps, float* range, int32_t* hit, uint8_t* amb,
+                    int32_t* visits) {
+    double dx = cos(phi), dy = sin(phi);
+    long j = (long)floor(ox), i = (long)floor(oy);
+    int ambiguous = 0, nvis = 1;
+    /* origin within eps of an edge separating different occupancy */
+    {
+        int here = occ_at(occ, H, W, i, j);
+        double fx = ox - (double)j, fy = oy - (double)i;
+        if (fx < eps && occ_at(occ, H, W, i, j - 1) != here) ambiguous = 1;
+        if (1.0 - fx < eps && occ_at(occ, H, W, i, j + 1) != here) ambiguous = 1;
+        if (fy < eps && occ_at(occ, H, W, i - 1, j) != here) ambiguous = 1;
+        if (1.0 - fy < eps && occ_at(occ, H, W, i + 1, j) != here) ambiguous = 1;
+        if (here) {
+            *range = 0.0f;
+            *hit = (i >= 0 && j >= 0 && i < H && j < W) ? (int32_t)(i * W + j) : -2;
+            if (amb) *amb = (uint8_t)ambiguous;
+            if (visits) *visits = nvis;
+            return;
+        }
+    }
+    long sx = dx > 0.0 ? 1 : -1, sy = dy > 0.0 ? 1 : -1;
+    double bx = dx > 0.0 ? (double)(j + 1) : (double)j;         /* next vertical boundary   */
+    double by = dy > 0.0 ? (double)(i + 1) : (double)i;         /* next horizontal boundary */
+    double tx = dx != 0.0 ? (bx - ox) / dx : INFINITY;
+    double ty = dy != 0.0 ? (by - oy) / dy : INFINITY;
+    for (;;) {
+        double t;
+        int step_x = 0, step_y = 0;
+        if (tx < ty) { t = tx; step_x = 1; }
+        else if (ty < tx) { t = ty; step_y = 1; }
+        else { t = tx; step_x = step_y = 1; }                   /* exactly through a corner */
+        /* nearest lattice corner on the boundary line being crossed; perpendicular distance to the beam */
+        if (t < T + eps) {
+            if (step_x) {
+                double yc = oy + t * dy; long cy = (long)floor(yc + 0.5), cx = (long)bx;
+                double dist = fabs(((double)cx - ox) * dy - ((double)cy - oy) * dx);
+                if (dist < eps && corner_mixed(occ, H, W, cx, cy)) ambiguous = 1;
+            }
+            if (step_y) {
+                double xc = ox + t * dx; long cx = (long)floor(xc + 0.5), cy = (long)by;
+                double dist = fabs(((double)cx - ox) * dy - ((double)cy - oy) * dx);
+                if (dist < eps && corner_mixed(occ, H, W, cx, cy)) ambiguous = 1;
+            }
+        }
+        if (step_x) { j += sx; bx += (double)sx; tx = (bx - ox) / dx; }
+        if (step_y) { i += sy; by += (double)sy; ty = (by - oy) / dy; }
+        if (t >= T) {                                           /* cell entered at or beyond r_max */
+            if (t - T < eps && occ_at(occ, H, W, i, j)) ambiguous = 1;
+            *range = (float)rmax; *hit = -1;
+            break;
+        }
+        ++nvis;
+        if (occ_at(occ, H, W, i, j)) {
+            if (T - t < eps) ambiguous = 1;
+            *range = (float)(t * rho);
+            *hit = (i >= 0 && j >= 0 && i < H && j < W) ? (int32_t)(i * W + j) : -2;
+            break;
+        }
+    }
+    if (amb) *amb = (uint8_t)ambiguous;
+    if (visits) *visits = nvis;
+}
+
+void fno_ranges(const uint8_t* occ, int H, int W, float res, int B, const float* angles,
+                float max_range, const float* sensor /*[3] or NULL*/, int n,
+                const float* x, const float* y, const float* psi, double eps,
+                float* ranges /*[n][B]*/, int32_t* hit /*[n][B] or NULL*/,
+                uint8_t* amb /*[n][B] or NULL*/, int32_t* visits /*[n][B] or NULL*/) {
+    const double rho = (double)res, rmax = (double)max_range, T = rmax / rho;
+    const double s0 = sensor ? (double)sensor[0] : 0.0, s1 = sensor ? (double)sensor[1] : 0.0,
+                 s2 = sensor ? (double)sensor[2] : 0.0;
+    for (int e = 0; e < n; ++e) {
+        double c = cos((double)psi[e]), s = sin((double)psi[e]);
+        double ox = ((double)x[e] + c * s0 - s * s1) / rho;
+        double oy = ((double)y[e] + s * s0 + c * s1) / rho;
+        for (int b = 0; b < B; ++b) {
+            size_t k = (size_t)e * (size_t)B + (size_t)b;
+            double phi = (double)psi[e] + s2 + (double)angles[b];
+            int32_t h;
+            ray_one(occ, H, W, rho, ox, oy, phi, T, rmax, eps, &ranges[k], &h,
+                    amb ? &amb[k] : NULL, visits ? &visits[k] : NULL);
+            if (hit) hit[k] = h;
+        }
+    }
+}
+
+/* The paper's own definition: fixed-step samples along each beam, first sample at t = 0
+ * (reading G5), step `delta` metres; the range is the distance of the first sample that falls in an
+ * occupied (or outside-map) cell; no such sample below r_max => r_max.  Cross-check only.
+ */
+void fno_ranges_fixed_step(const uint8_t* occ, int H, int W, float res, int B, const float* angles,
+                           float max_range, double delta, int n, const float* x, const float* y,
+                           const float* psi, float* ranges) {
+    const double rho = (double)res, rmax = (double)max_range;
+    for (int e = 0; e < n; ++e) for (int b = 0; b < B; ++b) {
+        double phi = (double)psi[e] + (double)angles[b], dx = cos(phi), dy = sin(phi);
+        double r = rmax;
+        for (long k = 0; ; ++k) {
+            double t = (double)k * delta;
+            if (t >= rmax) break;
+            double px = ((double)x[e] + t * dx) / rho, py = ((double)y[e] + t * dy) / rho;
+            if (occ_at(occ, H, W, (long)floor(py), (long)floor(px))) { r = t; break; }
+        }
+        ranges[(size_t)e * B + b] = (float)r;
+    }
+}
+
+/* ------------------------------------------------------------------ O7: reset of masked envs
+ * PAPER.md:86 "When episodes end, only the corresponding environments are reset"; "their
+ * environments are reset to start new episodes".  The paper gives no sampling rule; this is reading
+ * G16 (BASELINE.json config 1: "Start poses uniform in free space, goals 3-8 m away"), PARITY UNPINNED.
+ *
+ * Random numbers: counter-based SplitMix64 (Steele, Lea, Flood 2014 finaliser): draw c of seed sigma is
+ *   z = sigma + (c+1) * 0x9E3779B97F4A7C15;  z = (z ^ z>>30) * 0xBF58476D1CE4E5B9;
+ *   z = (z ^ z>>27) * 0x94D049BB133111EB;    z ^ z>>31
+ * i.e. the (c+1)-th output of a SplitMix64 stream seeded with sigma.  Uniform u = (z >> 40) * 2^-24,
+ * exact in fp32.  Start attempt k = 0..255 uses draws 3k, 3k+1, 3k+2; goal attempt m = 0..255 uses
+ * draws 768+2m, 768+2m+1.  All fp32 operations below are single, separately rounded operations.
+ */
+uint64_t fno_splitmix64(uint64_t sigma, uint64_t c) {
+    uint64_t z = sigma + (c + 1u) * 0x9E3779B97F4A7C15ull;
+    z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+    z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+    return z ^ (z >> 31);
+}
+static float u24(uint64_t sigma, uint64_t c) {
+    return (float)(fno_splitmix64(sigma, c) >> 40) * 5.9604644775390625e-08f;   /* 2^-24 */
+}
+
+#define FNO_MAX_ATTEMPTS 256
+
+static int goal_cell_ok(const uint8_t* occ, int H, int W, long r0, long c0, long rh, long cw, long i, long j) {
+    if (i < r0 || j < c0 || i >= r0 + rh || j >= c0 + cw) return 0;
+    return !occ_at(occ, H, W, i, j);
+}
+
+/* states [8][n] updated in place for masked envs; d_prev/ep_step re-seeded; amb/fail optional. */
+void fno_reset(const uint8_t* occ, int H, int W, float res, int V, const float* fp_xy,
+               int n_regions, const int32_t* regions /*[n_regions][4] or NULL*/,
+               float goal_dist_min, float goal_dist_max, int n, const uint8_t* mask,
+               const uint64_t* seeds, double eps, float* states, float* d_prev, int32_t* ep_step,
+               uint8_t* amb /*[n] or NULL*/, uint8_t* failed /*[n] or NULL*/) {
+    const double rho = (double)res;
+    const float two_pi_f = 6.28318530717958647692f, pi_f = 3.14159265358979323846f;
+    const float dmin2 = goal_dist_min * goal_dist_min, dmax2 = goal_dist_max * goal_dist_max;
+    for (int e = 0; e < n; ++e) {
+        if (amb) amb[e] = 0;
+        if (failed) failed[e] = 0;
+        if (!mask[e]) continue;
+        long r0 = 0, c0 = 0, rh = H, cw = W;
+        if (n_regions > 0 && regions) {
+            const int32_t* R = regions + 4 * (e % n_regions);
+            r0 = R[0]; c0 = R[1]; rh = R[2]; cw = R[3];
+        }
+        const float X0 = (float)((double)c0 * rho), Xe = (float)((double)cw * rho);
+        const float Y0 = (float)((double)r0 * rho), Ye = (float)((double)rh * rho);
+        const uint64_t sigma = seeds[e];
+        int ambiguous = 0, fail = 0;
+        float x = 0, y = 0, psi = 0;
+        int ok = 0;
+        for (int k = 0; k < FNO_MAX_ATTEMPTS && !ok; ++k) {
+            x = fmaf(u24(sigma, 3u * k), Xe, X0);
+            y = fmaf(u24(sigma, 3u * k + 1u), Ye, Y0);
+            psi = fmaf(u24(sigma, 3u * k + 2u), two_pi_f, -pi_f);
+            int a = 0;
+            ok = !collision_one(occ, H, W, rho, V, fp_xy, x, y, psi, eps, &a);
+            ambiguous |= a;
+        }
+        if (!ok) fail = 1;
+        float gx = x, gy = y;
+        ok = 0;
+        for (int m = 0; m < FNO_MAX_ATTEMPTS && !ok; ++m) {
+            float a = fmaf(2.0f, u24(sigma, 768u + 2u * m), -1.0f);       /* exact */
+            float b = fmaf(2.0f, u24(sigma, 768u + 2u * m + 1u), -1.0f);
+            gx = fmaf(a, goal_dist_max, x);
+            gy = fmaf(b, goal_dist_max, y);
+            float ddx = gx - x, ddy = gy - y;
+            float p = ddx * ddx, q = ddy * ddy;
+            float d2 = p + q;
+            if (!(d2 >= dmin2 && d2 <= dmax2)) continue;
+            double cx = (double)gx / rho, cy = (double)gy / rho;
+            long j = (long)floor(cx), i = (long)floor(cy);
+            ok = goal_cell_ok(occ, H, W, r0, c0, rh, cw, i, j);
+            /* goal point within eps of a cell edge across which acceptability differs */
+            double fx = cx - (double)j, fy = cy - (double)i;
+            long dj0 = fx < eps ? -1 : 0, dj1 = (1.0 - fx) < eps ? 1 : 0;
+            long di0 = fy < eps ? -1 : 0, di1 = (1.0 - fy) < eps ? 1 : 0;
+            for (long di = di0; di <= di1; ++di) for (long dj = dj0; dj <= dj1; ++dj)
+                if (goal_cell_ok(occ, H, W, r0, c0, rh, cw, i + di, j + dj) != ok) ambiguous = 1;
+        }
+        if (!ok) fail = 1;
+        states[0 * n + e] = x;  states[1 * n + e] = y;  states[2 * n + e] = psi;
+        states[3 * n + e] = 0;  states[4 * n + e] = 0;  states[5 * n + e] = 0;
+        states[6 * n + e] = gx; states[7 * n + e] = gy;
+        double ex = (double)gx - (double)x, ey = (double)gy - (double)y;
+        d_prev[e] = (float)sqrt(ex * ex + ey * ey);
+        ep_step[e] = 0;
+        if (amb) amb[e] = (uint8_t)ambiguous;
+        if (failed) failed[e] = (uint8_t)fail;
+    }
+}
+
+/* ------------------------------------------------------------------ O9: replay-ring row
+ * PAPER.md:84 "transitions are written directly to a GPU-resident circular replay buffer";
+ * BASELINE.json config 5: "(obs, action, reward, done) in fp32".  Row layout (reading G18):
+ *   [ranges(B), d, alpha, v_x, v_y, w, action(A), reward, done]  with obs = the observation the action
+ * was chosen from.  slot = (head + e) mod capacity.
+ */
+void fno_ring_append(float* ring, uint64_t capacity, uint64_t head, int n, int B, int A,
+                     const float* obs_ranges /*[n][B]*/, const float* obs_goal /*[2][n]*/,
+                     const float* obs_vel /*[3][n]*/, const float* actions /*[n][A]*/,
+                     const float* reward, const uint8_t* done) {
+    const size_t row = (size_t)B + 5 + (size_t)A + 2;
+    for (int e = 0; e < n; ++e) {
+        float* r = ring + (size_t)((head + (uint64_t)e) % capacity) * row;
+        memcpy(r, obs_ranges + (size_t)e * B, (size_t)B * sizeof(float));
+        r[B + 0] = obs_goal[0 * n + e]; r[B + 1] = obs_goal[1 * n + e];
+        r[B + 2] = obs_vel[0 * n + e];  r[B + 3] = obs_vel[1 * n + e]; r[B + 4] = obs_vel[2 * n + e];
+        for (int a = 0; a < A; ++a) r[B + 5 + a] = actions[(size_t)e * A + a];
+        r[B + 5 + A] = reward[e];
+        r[B + 6 + A] = done[e] ? 1.0f : 0.0f;
+    }
+}
+
+/* ------------------------------------------------------------------ one whole vector step (3.2)
+ * actions -> O1/O2 motion -> O3 collision + O5 goal obs at the new pose -> O6 reward/done ->
+ * O4 ranges at the new pose.  Outputs are the PRE-reset (terminal) observations.
+ * The caller then applies fno_reset to done envs and recomputes only their observations (O8).
+ */
+void fno_step(const uint8_t* occ, int H, int W, float res, int V, const float* fp_xy, int B,
+              const float* angles, float max_range, int drive, const float* lim, float dt,
+              float goal_tol, int max_episode_steps, float r_success, float r_collision,
+              float c_progress, int n, float* states /*in/out [8][n]*/, const float* actions,
+              const uint8_t* forced, float* d_prev, int32_t* ep_step, float* ranges,
+              int32_t* hit, uint8_t* collision, float* goal_obs /*[2][n]*/, float* reward,
+              uint8_t* done) {
+    float* s2 = (float*)malloc((size_t)8 * n * sizeof(float));
+    fno_motion(drive, lim, dt, n, states, actions, s2);
+    memcpy(states, s2, (size_t)8 * n * sizeof(float));
+    free(s2);
+    const float *x = states, *y = states + n, *psi = states + 2 * n, *gx = states + 6 * n, *gy = states + 7 * n;
+    fno_collision(occ, H, W, res, V, fp_xy, n, x, y, psi, 0.0, collision, NULL);
+    fno_goal_obs(n, x, y, psi, gx, gy, goal_obs, goal_obs + n);
+    fno_reward_done(n, goal_obs, collision, forced, goal_tol, max_episode_steps, r_success,
+                    r_collision, c_progress, d_prev, ep_step, reward, done);
+    fno_ranges(occ, H, W, res, B, angles, max_range, NULL, n, x, y, psi, 0.0, ranges, hit, NULL, NULL);
+}

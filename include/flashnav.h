@@ -1,0 +1,139 @@
+/*
+ * flashnav.h -- C ABI of libflashnav: the batched navigation-simulator step of FlashNav
+ * (arxiv/paper_2606_15846), hand-written CUDA for sm_100a.
+ *
+ * One environment batch shares one occupancy bitmap; per step the library clips the
+ * commands and advances the planar pose for the robot's drive type, tests the (possibly
+ * nonconvex) footprint polygon against the map (Eq. (2) :118-123), computes goal
+ * distance/direction, reward and termination (Eq. (1)), casts the range
+ * beams, and on reset recomputes observations only for the environments that
+ * were reset.  DESIGN.md states the readings taken where the paper is silent.
+ *
+ * Conventions
+ *  - status: 0 = FN_OK, < 0 = error; fn_last_error() returns a thread-local message for the last error.
+ *  - `*_host` pointers are host memory, copied during the call (the caller may free them at once).
+ *  - `*_dev` pointers are caller-owned device memory on the current CUDA device; the library never
+ *    frees them and keeps them only where stated (fn_sim_bind_aux, fn_ring_attach).
+ *  - all work is enqueued on the CUDA stream given to fn_sim_create; calls return after enqueue and
+ *    never synchronise, except fn_get_counters and the *_host convenience entry points.
+ *  - argument errors are detected on the host before any launch; per-element problems (non-finite
+ *    action, reset attempts exhausted) never fault: they bump device counters (fn_get_counters).
+ *  - map frame: origin at the outer corner of cell (row 0, col 0); x grows with column, y with row;
+ *    cell (i, j) = [j rho, (j+1) rho) x [i rho, (i+1) rho); linear cell index = i*W + j; everything
+ *    outside the map is occupied.
+ *  - there is no CPU fallback: every entry point that computes fails with FN_ERR_CUDA without a device.
+ */
+#ifndef FLASHNAV_H_
+#define FLASHNAV_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum { FN_OK = 0, FN_ERR_INVALID_ARG = -1, FN_ERR_UNSUPPORTED = -2, FN_ERR_OOM = -3, FN_ERR_CUDA = -4 };
+enum { FN_DRIVE_DIFF = 0, FN_DRIVE_OMNI = 1 };
+enum { FN_MAX_VERTS = 64, FN_MAX_ATTEMPTS = 256 };
+enum { FN_N_COUNTERS = 8 };   /* rays cast, map words loaded, envs reset, reset failures,
+                                 non-finite actions, env steps, reserved, reserved */
+
+typedef struct fn_map fn_map;
+typedef struct fn_robot fn_robot;
+typedef struct fn_sim fn_sim;
+
+/* ---- map ("the environment batch shares an occupancy bitmap") -------------------
+ * bitmap_host: [H*W] row-major bytes, != 0 occupied.  The library bit-packs it (1 bit per cell) twice:
+ * row-packed (bits along columns) and column-packed (bits along rows), and uploads both.
+ * Errors: NULL pointers, H/W <= 0 or > 32768, resolution not finite or <= 0 -> FN_ERR_INVALID_ARG. */
+int fn_map_create(const uint8_t* bitmap_host, int H, int W, float resolution_m, fn_map** out);
+
+/* Optional sub-maps (BASELINE.json config 5: tiles of an atlas).  rects_host: [n][4] = row0, col0, h, w.
+ * Environment e belongs to region e % n; fn_reset samples its start and goal inside that rectangle.
+ * Beams and collision always see the whole map.  n = 0 clears the regions. */
+int fn_map_set_regions(fn_map* map, int n, const int32_t* rects_host);
+int fn_map_destroy(fn_map* map);
+
+/* ---- robot specification xi = (F, S, K, U) ----------------------------------------
+ * footprint_xy_host: [V][2] ordered polygon vertices, body frame, metres, CW or CCW, 3 <= V <= FN_MAX_VERTS.
+ * beam_angles_host:  [B] beam directions in the body frame, radians, B >= 1.
+ * drive_type: FN_DRIVE_DIFF commands (v_x, w); FN_DRIVE_OMNI commands (v_x, v_y, w).
+ * vel_limits_host:   [6] = vx_min, vx_max, vy_min, vy_max, w_min, w_max (min <= max). */
+int fn_robot_create(const float* footprint_xy_host, int V, const float* beam_angles_host, int B,
+                    float max_range_m, int drive_type, const float* vel_limits_host, fn_robot** out);
+/* sensor placement S in the body frame; default (0, 0, 0). */
+int fn_robot_set_sensor(fn_robot* robot, float sx_m, float sy_m, float spsi_rad);
+int fn_robot_destroy(fn_robot* robot);
+
+/* ---- task parameters (Eq. (1); defaults via fn_task_default) ---------------------- */
+typedef struct {
+    float goal_tol_m;          /* goal reached when d < goal_tol_m           (default 0.3) */
+    int   max_episode_steps;   /* 0 = no step limit                           (default 0)   */
+    float goal_dist_min_m;     /* reset: goal distance range                  (default 3)   */
+    float goal_dist_max_m;     /*                                             (default 8)   */
+    float r_success;           /* Eq. (1)                                     (default 10)  */
+    float r_collision;         /*                                             (default -10) */
+    float c_progress;          /* c_1                                         (default 2)   */
+} fn_task;
+void fn_task_default(fn_task* out);
+
+/* ---- simulator instance: n_envs environments on one map with one robot specification ----------------
+ * cuda_stream: a cudaStream_t (NULL = the default stream).  The map and robot must outlive the sim. */
+int fn_sim_create(const fn_map* map, const fn_robot* robot, int n_envs, const fn_task* task,
+                  void* cuda_stream, fn_sim** out);
+int fn_sim_destroy(fn_sim* sim);
+
+/* ---- one vector step -------------------------------------------------------------------
+ * states_dev:     [8][N] fp32 SoA planes x, y, psi, v_x, v_y, w, g_x, g_y; read and overwritten.
+ * actions_dev:    [N][A] fp32, A = 2 (v_x, w) or 3 (v_x, v_y, w); clipped to the limits.
+ * reset_mask_dev: [N] u8; in: forced-reset request, out: done = collision | goal reached | step limit | forced.
+ * out_ranges_dev: [N][B] fp32 metres; out_collision_dev: [N] u8; out_goal_obs_dev: [2][N] fp32 (d, alpha).
+ * Outputs are the PRE-reset observations ("Observations before reset are retained as next
+ * observations in replay").  Call fn_reset with the done mask afterwards. */
+int fn_step(fn_sim* sim, float* states_dev, const float* actions_dev, float dt, uint8_t* reset_mask_dev,
+            float* out_ranges_dev, uint8_t* out_collision_dev, float* out_goal_obs_dev);
+
+/* ---- reset of masked environments + selective observation recompute --------------
+ * mask_dev: [N] u8; seeds_dev: [N] u64 (one seed per env, read for masked envs only).
+ * Rewrites ONLY the masked envs' state planes and their rows of out_ranges_dev / out_goal_obs_dev. */
+int fn_reset(fn_sim* sim, float* states_dev, const uint8_t* mask_dev, const uint64_t* seeds_dev,
+             float* out_ranges_dev, float* out_goal_obs_dev);
+
+/* ---- optional outputs and hooks ---------------------------------------------------------------------------
+ * fn_sim_bind_aux: extra per-step outputs, retained until re-bound or destroy; either may be NULL.
+ *   out_hit_cell_dev [N][B] i32: linear cell index of the hit, -1 no hit, -2 outside the map.
+ *   out_reward_dev   [N] fp32: Eq. (1).
+ * fn_ring_attach: device replay ring (config 5).  Row = [ranges(B), d, alpha, v_x, v_y, w,
+ *   action(A), reward, done] fp32; fn_step appends one row per env at slot (head + e) mod capacity, with
+ *   obs = the observation the action was chosen from (the previous fn_step / fn_reset outputs).
+ * fn_observe_all: recompute ranges and goal obs of ALL envs from states ("Full batch").
+ * fn_get_counters: synchronises the stream and copies FN_N_COUNTERS u64 counters to host_out.
+ * fn_sim_count_words: 1 = also count 32-bit map words loaded by the beam kernel (slower; default 0). */
+int fn_sim_bind_aux(fn_sim* sim, int32_t* out_hit_cell_dev, float* out_reward_dev);
+int fn_ring_attach(fn_sim* sim, float* ring_dev, uint64_t capacity_transitions);
+int fn_observe_all(fn_sim* sim, const float* states_dev, float* out_ranges_dev, float* out_goal_obs_dev);
+int fn_get_counters(fn_sim* sim, uint64_t* host_out);
+int fn_sim_count_words(fn_sim* sim, int enable);
+/* episode state kept by the sim, copied to HOST arrays d_prev_host [N] fp32 and ep_step_host [N] i32
+ * (either may be NULL); synchronises the stream. */
+int fn_sim_episode_state(fn_sim* sim, float* d_prev_host, int32_t* ep_step_host);
+
+/* ---- end-to-end convenience: host buffers in, host buffers out -----------------------------------------
+ * Copies states/actions/mask (and seeds) host->device, runs fn_step (+ fn_reset of the done envs when
+ * seeds_host != NULL), copies states, ranges, collision, goal obs and the done mask back, synchronises.
+ * All pointers are HOST memory (pinned memory makes the copies asynchronous). */
+int fn_step_host(fn_sim* sim, float* states_host, const float* actions_host, float dt,
+                 uint8_t* reset_mask_host, const uint64_t* seeds_host, float* out_ranges_host,
+                 uint8_t* out_collision_host, float* out_goal_obs_host);
+
+/* ---- roofline microbenchmarks (same binary, same run): bytes/s of conflict-free ld.shared.u32 x2
+ * windows (kind 0), random-word ld.shared (kind 1) and L2-resident ld.global.nc (kind 2). */
+int fn_measure_peak(int kind, void* cuda_stream, double* out_bytes_per_s);
+
+const char* fn_last_error(void);
+const char* fn_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FLASHNAV_H_ */

@@ -1,0 +1,277 @@
+"""ctypes binding of libflashnav.so -- same names as include/flashnav.h, marshalling only."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_DIR = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_DIR, "libflashnav.so")
+_lib = None
+
+DRIVE_DIFF, DRIVE_OMNI = 0, 1
+N_COUNTERS = 8
+COUNTER_NAMES = ("rays_cast", "map_words_loaded", "envs_reset", "reset_failures", "nonfinite_actions",
+                 "env_steps", "reserved0", "reserved1")
+
+EXPORTED_SYMBOLS = (
+    "fn_map_create", "fn_map_set_regions", "fn_map_destroy", "fn_robot_create", "fn_robot_set_sensor",
+    "fn_robot_destroy", "fn_task_default", "fn_sim_create", "fn_sim_destroy", "fn_step", "fn_reset",
+    "fn_sim_bind_aux", "fn_ring_attach", "fn_observe_all", "fn_get_counters", "fn_sim_count_words",
+    "fn_sim_episode_state", "fn_step_host", "fn_measure_peak", "fn_last_error", "fn_version")
+
+
+class FlashNavError(RuntimeError):
+    pass
+
+
+class _Task(C.Structure):
+    _fields_ = [("goal_tol_m", C.c_float), ("max_episode_steps", C.c_int), ("goal_dist_min_m", C.c_float),
+                ("goal_dist_max_m", C.c_float), ("r_success", C.c_float), ("r_collision", C.c_float),
+                ("c_progress", C.c_float)]
+
+
+def library_path() -> str:
+    return _LIB_PATH
+
+
+def load_library():
+    """Loads libflashnav.so (built in-tree by paper_2606_15846_b200/build.py). Raises if absent."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_LIB_PATH):
+        raise FlashNavError(f"{_LIB_PATH} is missing: run `python -m paper_2606_15846_b200.build` "
+                            "(there is no CPU fallback)")
+    lib = C.CDLL(_LIB_PATH)
+    vp, i32, f32, u64 = C.c_void_p, C.c_int, C.c_float, C.c_uint64
+    sig = {
+        "fn_map_create": [vp, i32, i32, f32, C.POINTER(vp)],
+        "fn_map_set_regions": [vp, i32, vp],
+        "fn_map_destroy": [vp],
+        "fn_robot_create": [vp, i32, vp, i32, f32, i32, vp, C.POINTER(vp)],
+        "fn_robot_set_sensor": [vp, f32, f32, f32],
+        "fn_robot_destroy": [vp],
+        "fn_sim_create": [vp, vp, i32, C.POINTER(_Task), vp, C.POINTER(vp)],
+        "fn_sim_destroy": [vp],
+        "fn_step": [vp, vp, vp, f32, vp, vp, vp, vp],
+        "fn_reset": [vp, vp, vp, vp, vp, vp],
+        "fn_sim_bind_aux": [vp, vp, vp],
+        "fn_ring_attach": [vp, vp, u64],
+        "fn_observe_all": [vp, vp, vp, vp],
+        "fn_get_counters": [vp, vp],
+        "fn_sim_count_words": [vp, i32],
+        "fn_sim_episode_state": [vp, vp, vp],
+        "fn_step_host": [vp, vp, vp, f32, vp, vp, vp, vp, vp],
+        "fn_measure_peak": [i32, vp, C.POINTER(C.c_double)],
+    }
+    for name, argtypes in sig.items():
+        fn = getattr(lib, name)
+        fn.argtypes = argtypes
+        fn.restype = i32
+    lib.fn_task_default.argtypes = [C.POINTER(_Task)]
+    lib.fn_task_default.restype = None
+    lib.fn_last_error.restype = C.c_char_p
+    lib.fn_version.restype = C.c_char_p
+    _lib = lib
+    return lib
+
+
+def _check(rc: int, what: str):
+    if rc != 0:
+        msg = load_library().fn_last_error().decode("utf-8", "replace")
+        raise FlashNavError(f"{what} failed ({rc}): {msg}")
+
+
+def _np_ptr(a: np.ndarray):
+    return a.ctypes.data_as(C.c_void_p)
+
+
+def _dev_ptr(t, dtype, numel, name):
+    import torch
+    if t is None:
+        return None
+    if not isinstance(t, torch.Tensor) or not t.is_cuda:
+        raise FlashNavError(f"{name}: expected a CUDA tensor")
+    if t.dtype != dtype or not t.is_contiguous() or t.numel() != numel:
+        raise FlashNavError(f"{name}: expected contiguous {dtype} with {numel} elements, got {t.dtype} "
+                            f"{tuple(t.shape)} contiguous={t.is_contiguous()}")
+    return C.c_void_p(t.data_ptr())
+
+
+class Map:
+    """fn_map: a shared occupancy bitmap (uint8 [H, W], != 0 occupied)."""
+
+    def __init__(self, bitmap: np.ndarray, resolution: float):
+        lib = load_library()
+        bm = np.ascontiguousarray(bitmap, np.uint8)
+        if bm.ndim != 2:
+            raise FlashNavError("bitmap must be [H, W]")
+        self.H, self.W = int(bm.shape[0]), int(bm.shape[1])
+        self.resolution = float(np.float32(resolution))
+        h = C.c_void_p()
+        _check(lib.fn_map_create(_np_ptr(bm), self.H, self.W, C.c_float(resolution), C.byref(h)), "fn_map_create")
+        self._h = h
+
+    def set_regions(self, rects):
+        n = 0 if rects is None else int(len(rects))
+        arr = None if n == 0 else np.ascontiguousarray(rects, np.int32).reshape(n, 4)
+        _check(load_library().fn_map_set_regions(self._h, n, None if arr is None else _np_ptr(arr)), "fn_map_set_regions")
+
+    def close(self):
+        if getattr(self, "_h", None):
+            load_library().fn_map_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+class Robot:
+    """fn_robot: footprint polygon [V,2], beam angles [B], max range, drive type, velocity limits [6]."""
+
+    def __init__(self, footprint, beam_angles, max_range, drive, vel_limits):
+        lib = load_library()
+        fp = np.ascontiguousarray(footprint, np.float32).reshape(-1, 2)
+        ang = np.ascontiguousarray(beam_angles, np.float32).reshape(-1)
+        lim = np.ascontiguousarray(vel_limits, np.float32).reshape(-1)
+        if lim.shape[0] != 6:
+            raise FlashNavError("vel_limits must have 6 entries")
+        self.V, self.B, self.drive = int(fp.shape[0]), int(ang.shape[0]), int(drive)
+        self.A = 2 if self.drive == DRIVE_DIFF else 3
+        h = C.c_void_p()
+        _check(lib.fn_robot_create(_np_ptr(fp), self.V, _np_ptr(ang), self.B, C.c_float(max_range), self.drive,
+                                   _np_ptr(lim), C.byref(h)), "fn_robot_create")
+        self._h = h
+
+    def set_sensor(self, sx, sy, spsi):
+        _check(load_library().fn_robot_set_sensor(self._h, C.c_float(sx), C.c_float(sy), C.c_float(spsi)), "fn_robot_set_sensor")
+
+    def close(self):
+        if getattr(self, "_h", None):
+            load_library().fn_robot_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+class Sim:
+    """fn_sim: n_envs environments on one Map with one Robot; work goes to torch's current stream at creation."""
+
+    def __init__(self, map_: Map, robot: Robot, n_envs: int, goal_tol=0.3, max_episode_steps=0, goal_dist_min=3.0,
+                 goal_dist_max=8.0, r_success=10.0, r_collision=-10.0, c_progress=2.0, stream=None):
+        import torch
+        lib = load_library()
+        if not torch.cuda.is_available():
+            raise FlashNavError("no CUDA device: libflashnav has no CPU fallback")
+        self.map, self.robot, self.n = map_, robot, int(n_envs)
+        t = _Task(goal_tol, int(max_episode_steps), goal_dist_min, goal_dist_max, r_success, r_collision, c_progress)
+        self._stream = torch.cuda.current_stream() if stream is None else stream
+        h = C.c_void_p()
+        _check(lib.fn_sim_create(map_._h, robot._h, self.n, C.byref(t), C.c_void_p(self._stream.cuda_stream), C.byref(h)),
+               "fn_sim_create")
+        self._h = h
+        self._keep = []
+
+    # --- the four calls of the north star ------------------------------------------------------
+    def step(self, states, actions, dt, reset_mask, out_ranges, out_collision, out_goal_obs):
+        import torch
+        n, B, A = self.n, self.robot.B, self.robot.A
+        _check(load_library().fn_step(
+            self._h, _dev_ptr(states, torch.float32, 8 * n, "states"), _dev_ptr(actions, torch.float32, n * A, "actions"),
+            C.c_float(dt), _dev_ptr(reset_mask, torch.uint8, n, "reset_mask"),
+            _dev_ptr(out_ranges, torch.float32, n * B, "out_ranges"), _dev_ptr(out_collision, torch.uint8, n, "out_collision"),
+            _dev_ptr(out_goal_obs, torch.float32, 2 * n, "out_goal_obs")), "fn_step")
+
+    def reset(self, states, mask, seeds, out_ranges, out_goal_obs):
+        import torch
+        n, B = self.n, self.robot.B
+        if seeds.dtype not in (torch.int64, torch.uint64):
+            raise FlashNavError("seeds must be a 64-bit integer tensor")
+        _check(load_library().fn_reset(
+            self._h, _dev_ptr(states, torch.float32, 8 * n, "states"), _dev_ptr(mask, torch.uint8, n, "mask"),
+            _dev_ptr(seeds, seeds.dtype, n, "seeds"), _dev_ptr(out_ranges, torch.float32, n * B, "out_ranges"),
+            _dev_ptr(out_goal_obs, torch.float32, 2 * n, "out_goal_obs")), "fn_reset")
+
+    # --- hooks ----------------------------------------------------------------------------------------
+    def bind_aux(self, out_hit_cell=None, out_reward=None):
+        import torch
+        n, B = self.n, self.robot.B
+        self._keep = [out_hit_cell, out_reward]
+        _check(load_library().fn_sim_bind_aux(self._h, _dev_ptr(out_hit_cell, torch.int32, n * B, "out_hit_cell"),
+                                              _dev_ptr(out_reward, torch.float32, n, "out_reward")), "fn_sim_bind_aux")
+
+    def ring_row_floats(self):
+        return self.robot.B + 5 + self.robot.A + 2
+
+    def ring_attach(self, ring, capacity):
+        import torch
+        self._ring = ring
+        _check(load_library().fn_ring_attach(self._h, _dev_ptr(ring, torch.float32, capacity * self.ring_row_floats(), "ring")
+                                             if ring is not None else None, C.c_uint64(capacity)), "fn_ring_attach")
+
+    def observe_all(self, states, out_ranges, out_goal_obs=None):
+        import torch
+        n, B = self.n, self.robot.B
+        _check(load_library().fn_observe_all(
+            self._h, _dev_ptr(states, torch.float32, 8 * n, "states"), _dev_ptr(out_ranges, torch.float32, n * B, "out_ranges"),
+            _dev_ptr(out_goal_obs, torch.float32, 2 * n, "out_goal_obs")), "fn_observe_all")
+
+    def counters(self) -> dict:
+        out = np.zeros(N_COUNTERS, np.uint64)
+        _check(load_library().fn_get_counters(self._h, _np_ptr(out)), "fn_get_counters")
+        return {k: int(v) for k, v in zip(COUNTER_NAMES, out)}
+
+    def count_words(self, enable: bool):
+        _check(load_library().fn_sim_count_words(self._h, int(bool(enable))), "fn_sim_count_words")
+
+    def episode_state(self):
+        """Host copies of the sim's d_prev [N] f32 and ep_step [N] i32 (synchronises)."""
+        d = np.empty(self.n, np.float32)
+        e = np.empty(self.n, np.int32)
+        _check(load_library().fn_sim_episode_state(self._h, _np_ptr(d), _np_ptr(e)), "fn_sim_episode_state")
+        return d, e
+
+    def step_host(self, states, actions, dt, reset_mask, seeds, out_ranges, out_collision, out_goal_obs):
+        """End to end with HOST buffers (numpy arrays or pinned CPU tensors); copies inside the call."""
+        def hp(a, name):
+            if a is None:
+                return None
+            if isinstance(a, np.ndarray):
+                if not a.flags.c_contiguous:
+                    raise FlashNavError(f"{name}: not contiguous")
+                return C.c_void_p(a.ctypes.data)
+            if a.is_cuda or not a.is_contiguous():
+                raise FlashNavError(f"{name}: expected a contiguous CPU tensor")
+            return C.c_void_p(a.data_ptr())
+        _check(load_library().fn_step_host(self._h, hp(states, "states"), hp(actions, "actions"), C.c_float(dt),
+                                           hp(reset_mask, "reset_mask"), hp(seeds, "seeds"), hp(out_ranges, "out_ranges"),
+                                           hp(out_collision, "out_collision"), hp(out_goal_obs, "out_goal_obs")), "fn_step_host")
+
+    def close(self):
+        if getattr(self, "_h", None):
+            load_library().fn_sim_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def measure_peak(kind: int) -> float:
+    """bytes/s of kind 0 (smem conflict-free), 1 (smem random), 2 (L2-resident global)."""
+    import torch
+    out = C.c_double()
+    _check(load_library().fn_measure_peak(int(kind), C.c_void_p(torch.cuda.current_stream().cuda_stream), C.byref(out)),
+           "fn_measure_peak")
+    return float(out.value)

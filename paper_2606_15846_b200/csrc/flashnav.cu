@@ -1,0 +1,446 @@
+// flashnav.cu -- host side of the C ABI declared in include/flashnav.h.
+// Argument validation, bit-packing and upload of the map, launch configuration.  Every step of the
+// hot path runs in the kernels of fn_env.cuh / fn_beam.cuh; nothing here computes simulator results.
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <type_traits>
+#include <vector>
+
+#include "../../include/flashnav.h"
+#include "fn_beam.cuh"
+#include "fn_common.cuh"
+#include "fn_env.cuh"
+
+using namespace fn;
+
+static thread_local char g_err[512] = "";
+
+static int fail(int code, const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+#define FN_CUDA(call)                                                                        \
+    do {                                                                                     \
+        cudaError_t e_ = (call);                                                             \
+        if (e_ != cudaSuccess)                                                               \
+            return fail(e_ == cudaErrorMemoryAllocation ? FN_ERR_OOM : FN_ERR_CUDA, "%s: %s", \
+                        #call, cudaGetErrorString(e_));                                      \
+    } while (0)
+
+struct fn_map {
+    int H, W;
+    float res;
+    uint32_t* d_words;       // row-packed copy then column-packed copy, contiguous
+    size_t n_words;          // padded to a multiple of 4
+    MapDev dev;
+    int n_regions;
+    int4* d_regions;
+};
+
+struct fn_robot {
+    int V, B, drive;
+    float lim[6];
+    float rmax;
+    float sensor[3];
+    std::vector<float> angles;
+    std::vector<float> verts;
+    double2* d_beam_cs;
+    double2* d_verts;
+};
+
+struct fn_sim {
+    const fn_map* map;
+    const fn_robot* robot;
+    int n;
+    fn_task task;
+    cudaStream_t stream;
+    int num_sms;
+    // device state owned by the sim
+    PoseD* d_poses;
+    int* d_list;
+    int* d_count;
+    float* d_dprev;
+    int* d_epstep;
+    unsigned long long* d_counters;
+    // bound by the caller
+    int32_t* aux_hit;
+    float* aux_reward;
+    float* ring;
+    unsigned long long ring_cap, ring_head;
+    int count_words;
+    // beam-kernel launch configuration
+    bool use_smem;
+    size_t beam_smem;
+    int beam_grid;
+    // device staging for fn_step_host (lazily allocated)
+    float *stg_states, *stg_actions, *stg_ranges, *stg_gobs;
+    uint8_t *stg_mask, *stg_col;
+    unsigned long long* stg_seeds;
+};
+
+extern "C" const char* fn_last_error(void) { return g_err; }
+extern "C" const char* fn_version(void) { return "flashnav-b200 0.1 (sm_100a)"; }
+
+extern "C" void fn_task_default(fn_task* t) {
+    if (!t) return;
+    t->goal_tol_m = 0.3f; t->max_episode_steps = 0; t->goal_dist_min_m = 3.0f; t->goal_dist_max_m = 8.0f;
+    t->r_success = 10.0f; t->r_collision = -10.0f; t->c_progress = 2.0f;
+}
+
+// ------------------------------------------------------------------------------------------ map
+extern "C" int fn_map_create(const uint8_t* bitmap, int H, int W, float res, fn_map** out) {
+    if (!bitmap || !out) return fail(FN_ERR_INVALID_ARG, "fn_map_create: NULL argument");
+    if (H <= 0 || W <= 0 || H > 32768 || W > 32768) return fail(FN_ERR_INVALID_ARG, "fn_map_create: H, W must be in 1..32768");
+    if (!std::isfinite(res) || res <= 0.0f) return fail(FN_ERR_INVALID_ARG, "fn_map_create: resolution must be finite and > 0");
+    const int nwR = (W + 31) / 32, nwC = (H + 31) / 32;
+    const int sR = nwR + 2, sC = nwC + 2;
+    const size_t rowWords = (size_t)H * sR, colWords = (size_t)W * sC;
+    const size_t total = (rowWords + colWords + 3) / 4 * 4;
+    std::vector<uint32_t> words(total, 0u);
+    for (int i = 0; i < H; ++i)
+        for (int j = 0; j < W; ++j)
+            if (bitmap[(size_t)i * W + j]) {
+                words[(size_t)i * sR + 1 + (j >> 5)] |= 1u << (j & 31);
+                words[rowWords + (size_t)j * sC + 1 + (i >> 5)] |= 1u << (i & 31);
+            }
+    fn_map* m = new (std::nothrow) fn_map();
+    if (!m) return fail(FN_ERR_OOM, "fn_map_create: host allocation failed");
+    m->H = H; m->W = W; m->res = res; m->n_words = total; m->n_regions = 0; m->d_regions = nullptr; m->d_words = nullptr;
+    cudaError_t e = cudaMalloc(&m->d_words, total * sizeof(uint32_t));
+    if (e == cudaSuccess) e = cudaMemcpy(m->d_words, words.data(), total * sizeof(uint32_t), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) {
+        if (m->d_words) cudaFree(m->d_words);
+        delete m;
+        return fail(e == cudaErrorMemoryAllocation ? FN_ERR_OOM : FN_ERR_CUDA, "fn_map_create: %s", cudaGetErrorString(e));
+    }
+    m->dev.row = m->d_words; m->dev.col = m->d_words + rowWords;
+    m->dev.H = H; m->dev.W = W; m->dev.nwR = nwR; m->dev.nwC = nwC; m->dev.strideR = sR; m->dev.strideC = sC;
+    m->dev.rho = res; m->dev.inv_rho = 1.0 / (double)res;
+    *out = m;
+    return FN_OK;
+}
+
+extern "C" int fn_map_set_regions(fn_map* m, int n, const int32_t* rects) {
+    if (!m || n < 0 || (n > 0 && !rects)) return fail(FN_ERR_INVALID_ARG, "fn_map_set_regions: bad argument");
+    for (int k = 0; k < n; ++k) {
+        const int32_t* r = rects + 4 * k;
+        if (r[0] < 0 || r[1] < 0 || r[2] <= 0 || r[3] <= 0 || r[0] + r[2] > m->H || r[1] + r[3] > m->W)
+            return fail(FN_ERR_INVALID_ARG, "fn_map_set_regions: rect %d outside the map", k);
+    }
+    if (m->d_regions) { cudaFree(m->d_regions); m->d_regions = nullptr; }
+    m->n_regions = 0;
+    if (n > 0) {
+        FN_CUDA(cudaMalloc(&m->d_regions, (size_t)n * sizeof(int4)));
+        FN_CUDA(cudaMemcpy(m->d_regions, rects, (size_t)n * sizeof(int4), cudaMemcpyHostToDevice));
+        m->n_regions = n;
+    }
+    return FN_OK;
+}
+
+extern "C" int fn_map_destroy(fn_map* m) {
+    if (!m) return FN_OK;
+    if (m->d_words) cudaFree(m->d_words);
+    if (m->d_regions) cudaFree(m->d_regions);
+    delete m;
+    return FN_OK;
+}
+
+// ------------------------------------------------------------------------------------------ robot
+static int robot_upload(fn_robot* r) {
+    std::vector<double2> cs(r->B), vs(r->V);
+    for (int j = 0; j < r->B; ++j) {
+        const double a = (double)r->angles[j] + (double)r->sensor[2];
+        cs[j] = make_double2(std::cos(a), std::sin(a));
+    }
+    for (int k = 0; k < r->V; ++k) vs[k] = make_double2((double)r->verts[2 * k], (double)r->verts[2 * k + 1]);
+    FN_CUDA(cudaMemcpy(r->d_beam_cs, cs.data(), cs.size() * sizeof(double2), cudaMemcpyHostToDevice));
+    FN_CUDA(cudaMemcpy(r->d_verts, vs.data(), vs.size() * sizeof(double2), cudaMemcpyHostToDevice));
+    return FN_OK;
+}
+
+extern "C" int fn_robot_create(const float* fp, int V, const float* angles, int B, float rmax, int drive,
+                               const float* lim, fn_robot** out) {
+    if (!fp || !angles || !lim || !out) return fail(FN_ERR_INVALID_ARG, "fn_robot_create: NULL argument");
+    if (V < 3) return fail(FN_ERR_INVALID_ARG, "fn_robot_create: footprint needs >= 3 vertices");
+    if (V > FN_MAX_VERTS) return fail(FN_ERR_UNSUPPORTED, "fn_robot_create: V > FN_MAX_VERTS (%d)", FN_MAX_VERTS);
+    if (B < 1) return fail(FN_ERR_INVALID_ARG, "fn_robot_create: B must be >= 1");
+    if (!std::isfinite(rmax) || rmax <= 0.0f) return fail(FN_ERR_INVALID_ARG, "fn_robot_create: max range must be finite and > 0");
+    if (drive != FN_DRIVE_DIFF && drive != FN_DRIVE_OMNI) return fail(FN_ERR_INVALID_ARG, "fn_robot_create: unknown drive type");
+    for (int k = 0; k < 6; k += 2)
+        if (!std::isfinite(lim[k]) || !std::isfinite(lim[k + 1]) || lim[k] > lim[k + 1])
+            return fail(FN_ERR_INVALID_ARG, "fn_robot_create: velocity limits must be finite with min <= max");
+    for (int k = 0; k < 2 * V; ++k) if (!std::isfinite(fp[k])) return fail(FN_ERR_INVALID_ARG, "fn_robot_create: non-finite footprint vertex");
+    for (int j = 0; j < B; ++j) if (!std::isfinite(angles[j])) return fail(FN_ERR_INVALID_ARG, "fn_robot_create: non-finite beam angle");
+    fn_robot* r = new (std::nothrow) fn_robot();
+    if (!r) return fail(FN_ERR_OOM, "fn_robot_create: host allocation failed");
+    r->V = V; r->B = B; r->drive = drive; r->rmax = rmax;
+    std::memcpy(r->lim, lim, sizeof(r->lim));
+    r->sensor[0] = r->sensor[1] = r->sensor[2] = 0.0f;
+    r->angles.assign(angles, angles + B);
+    r->verts.assign(fp, fp + 2 * V);
+    r->d_beam_cs = nullptr; r->d_verts = nullptr;
+    cudaError_t e = cudaMalloc(&r->d_beam_cs, (size_t)B * sizeof(double2));
+    if (e == cudaSuccess) e = cudaMalloc(&r->d_verts, (size_t)V * sizeof(double2));
+    int st = (e == cudaSuccess) ? robot_upload(r) : fail(e == cudaErrorMemoryAllocation ? FN_ERR_OOM : FN_ERR_CUDA, "fn_robot_create: %s", cudaGetErrorString(e));
+    if (st != FN_OK) {
+        if (r->d_beam_cs) cudaFree(r->d_beam_cs);
+        if (r->d_verts) cudaFree(r->d_verts);
+        delete r;
+        return st;
+    }
+    *out = r;
+    return FN_OK;
+}
+
+extern "C" int fn_robot_set_sensor(fn_robot* r, float sx, float sy, float spsi) {
+    if (!r || !std::isfinite(sx) || !std::isfinite(sy) || !std::isfinite(spsi)) return fail(FN_ERR_INVALID_ARG, "fn_robot_set_sensor: bad argument");
+    r->sensor[0] = sx; r->sensor[1] = sy; r->sensor[2] = spsi;
+    return robot_upload(r);
+}
+
+extern "C" int fn_robot_destroy(fn_robot* r) {
+    if (!r) return FN_OK;
+    if (r->d_beam_cs) cudaFree(r->d_beam_cs);
+    if (r->d_verts) cudaFree(r->d_verts);
+    delete r;
+    return FN_OK;
+}
+
+static RobotDev robot_dev(const fn_robot* r, const fn_map* m) {
+    RobotDev d;
+    d.beam_cs = r->d_beam_cs; d.verts = r->d_verts; d.B = r->B; d.V = r->V; d.drive = r->drive;
+    d.A = r->drive == FN_DRIVE_DIFF ? 2 : 3;
+    for (int k = 0; k < 6; ++k) d.lim[k] = r->lim[k];
+    d.rmax = r->rmax;
+    d.T = (double)r->rmax / (double)m->res;
+    d.sx = r->sensor[0]; d.sy = r->sensor[1];
+    return d;
+}
+static TaskDev task_dev(const fn_task& t) {
+    TaskDev d;
+    d.goal_tol = t.goal_tol_m; d.max_episode_steps = t.max_episode_steps; d.dmin = t.goal_dist_min_m;
+    d.dmax = t.goal_dist_max_m; d.r_success = t.r_success; d.r_collision = t.r_collision; d.c_progress = t.c_progress;
+    return d;
+}
+
+// ------------------------------------------------------------------------------------------ sim
+template <bool S, bool C>
+static cudaError_t beam_config(size_t smem, int* blocks_per_sm) {
+    cudaError_t e = cudaFuncSetAttribute(beam_kernel<S, C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, beam_kernel<S, C>, 512, smem);
+}
+
+extern "C" int fn_sim_create(const fn_map* map, const fn_robot* robot, int n, const fn_task* task,
+                             void* stream, fn_sim** out) {
+    if (!map || !robot || !out) return fail(FN_ERR_INVALID_ARG, "fn_sim_create: NULL argument");
+    if (n <= 0) return fail(FN_ERR_INVALID_ARG, "fn_sim_create: n_envs must be > 0");
+    if ((long long)n * robot->B > (1ll << 40)) return fail(FN_ERR_UNSUPPORTED, "fn_sim_create: n_envs * B too large");
+    fn_sim* s = new (std::nothrow) fn_sim();
+    if (!s) return fail(FN_ERR_OOM, "fn_sim_create: host allocation failed");
+    std::memset(s, 0, sizeof(*s));
+    s->map = map; s->robot = robot; s->n = n; s->stream = (cudaStream_t)stream;
+    if (task) s->task = *task; else fn_task_default(&s->task);
+    if (!(s->task.goal_dist_min_m >= 0.0f) || !(s->task.goal_dist_max_m >= s->task.goal_dist_min_m)) {
+        delete s;
+        return fail(FN_ERR_INVALID_ARG, "fn_sim_create: goal distance range must satisfy 0 <= min <= max");
+    }
+    int dev = 0, max_optin = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&s->num_sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+    if (e == cudaSuccess) e = cudaMalloc(&s->d_poses, (size_t)n * sizeof(PoseD));
+    if (e == cudaSuccess) e = cudaMalloc(&s->d_list, (size_t)n * sizeof(int));
+    if (e == cudaSuccess) e = cudaMalloc(&s->d_count, sizeof(int));
+    if (e == cudaSuccess) e = cudaMalloc(&s->d_dprev, (size_t)n * sizeof(float));
+    if (e == cudaSuccess) e = cudaMalloc(&s->d_epstep, (size_t)n * sizeof(int));
+    if (e == cudaSuccess) e = cudaMalloc(&s->d_counters, kNCounters * sizeof(unsigned long long));
+    if (e == cudaSuccess) e = cudaMemsetAsync(s->d_dprev, 0, (size_t)n * sizeof(float), s->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(s->d_epstep, 0, (size_t)n * sizeof(int), s->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(s->d_counters, 0, kNCounters * sizeof(unsigned long long), s->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(s->d_poses, 0, (size_t)n * sizeof(PoseD), s->stream);
+    if (e == cudaSuccess) {
+        // stage the packed map in shared memory when both copies + the beam table fit, else read via L2
+        const size_t tab = (size_t)robot->B * sizeof(double2);
+        const size_t with_map = tab + map->n_words * sizeof(uint32_t);
+        s->use_smem = with_map <= (size_t)max_optin;
+        s->beam_smem = s->use_smem ? with_map : tab;
+        if (s->beam_smem > (size_t)max_optin) {
+            fn_sim_destroy(s);
+            return fail(FN_ERR_UNSUPPORTED, "fn_sim_create: beam table does not fit in shared memory (B too large)");
+        }
+        int bps = 0, bps2 = 0;
+        if (s->use_smem) { e = beam_config<true, false>(s->beam_smem, &bps); if (e == cudaSuccess) e = beam_config<true, true>(s->beam_smem, &bps2); }
+        else { e = beam_config<false, false>(s->beam_smem, &bps); if (e == cudaSuccess) e = beam_config<false, true>(s->beam_smem, &bps2); }
+        if (bps2 < bps) bps = bps2;
+        if (bps < 1) bps = 1;
+        s->beam_grid = s->num_sms * bps;
+    }
+    if (e != cudaSuccess) {
+        int code = e == cudaErrorMemoryAllocation ? FN_ERR_OOM : FN_ERR_CUDA;
+        fail(code, "fn_sim_create: %s", cudaGetErrorString(e));
+        fn_sim_destroy(s);
+        return code;
+    }
+    *out = s;
+    return FN_OK;
+}
+
+extern "C" int fn_sim_destroy(fn_sim* s) {
+    if (!s) return FN_OK;
+    cudaFree(s->d_poses); cudaFree(s->d_list); cudaFree(s->d_count); cudaFree(s->d_dprev);
+    cudaFree(s->d_epstep); cudaFree(s->d_counters);
+    cudaFree(s->stg_states); cudaFree(s->stg_actions); cudaFree(s->stg_ranges); cudaFree(s->stg_gobs);
+    cudaFree(s->stg_mask); cudaFree(s->stg_col); cudaFree(s->stg_seeds);
+    delete s;
+    return FN_OK;
+}
+
+static int ring_row_floats(const fn_sim* s) { return s->robot->B + 5 + (s->robot->drive == FN_DRIVE_DIFF ? 2 : 3) + 2; }
+
+static int launch_beams(fn_sim* s, const int* list, const int* count_dev, float* out_ranges, unsigned long long ring_head) {
+    BeamArgs b;
+    b.map = s->map->dev; b.robot = robot_dev(s->robot, s->map); b.poses = s->d_poses;
+    b.list = list; b.count_dev = count_dev; b.n_all = s->n; b.out_ranges = out_ranges; b.out_hit = s->aux_hit;
+    b.ring_obs = s->ring; b.ring_cap = s->ring_cap ? s->ring_cap : 1; b.ring_head = ring_head; b.ring_row = ring_row_floats(s);
+    b.counters = s->d_counters;
+    const dim3 grid(s->beam_grid), block(512);
+    if (s->use_smem) {
+        if (s->count_words) beam_kernel<true, true><<<grid, block, s->beam_smem, s->stream>>>(b);
+        else beam_kernel<true, false><<<grid, block, s->beam_smem, s->stream>>>(b);
+    } else {
+        if (s->count_words) beam_kernel<false, true><<<grid, block, s->beam_smem, s->stream>>>(b);
+        else beam_kernel<false, false><<<grid, block, s->beam_smem, s->stream>>>(b);
+    }
+    FN_CUDA(cudaGetLastError());
+    return FN_OK;
+}
+
+extern "C" int fn_step(fn_sim* s, float* states, const float* actions, float dt, uint8_t* reset_mask,
+                       float* out_ranges, uint8_t* out_collision, float* out_goal_obs) {
+    if (!s || !states || !actions || !reset_mask || !out_ranges || !out_collision || !out_goal_obs)
+        return fail(FN_ERR_INVALID_ARG, "fn_step: NULL argument");
+    if (!std::isfinite(dt) || dt < 0.0f) return fail(FN_ERR_INVALID_ARG, "fn_step: dt must be finite and >= 0");
+    EnvArgs a;
+    a.map = s->map->dev; a.robot = robot_dev(s->robot, s->map); a.task = task_dev(s->task);
+    a.n = s->n; a.dt = dt; a.states = states; a.actions = actions; a.reset_mask = reset_mask;
+    a.out_collision = out_collision; a.out_goal_obs = out_goal_obs; a.out_reward = s->aux_reward;
+    a.d_prev = s->d_dprev; a.ep_step = s->d_epstep; a.poses = s->d_poses;
+    a.ring = s->ring; a.ring_cap = s->ring_cap ? s->ring_cap : 1; a.ring_head = s->ring_head; a.ring_row = ring_row_floats(s);
+    a.counters = s->d_counters;
+    env_step_kernel<<<(s->n + 7) / 8, 256, 0, s->stream>>>(a);
+    FN_CUDA(cudaGetLastError());
+    if (s->ring) s->ring_head = (s->ring_head + (unsigned long long)s->n) % s->ring_cap;
+    return launch_beams(s, nullptr, nullptr, out_ranges, s->ring_head);
+}
+
+extern "C" int fn_reset(fn_sim* s, float* states, const uint8_t* mask, const uint64_t* seeds,
+                        float* out_ranges, float* out_goal_obs) {
+    if (!s || !states || !mask || !seeds || !out_ranges || !out_goal_obs)
+        return fail(FN_ERR_INVALID_ARG, "fn_reset: NULL argument");
+    compact_mask_kernel<<<1, 1024, 0, s->stream>>>(mask, s->n, s->d_list, s->d_count);
+    FN_CUDA(cudaGetLastError());
+    ResetArgs a;
+    a.map = s->map->dev; a.robot = robot_dev(s->robot, s->map); a.task = task_dev(s->task);
+    a.regions.rects = s->map->d_regions; a.regions.n = s->map->n_regions;
+    a.n = s->n; a.states = states; a.list = s->d_list; a.count_dev = s->d_count;
+    a.seeds = reinterpret_cast<const unsigned long long*>(seeds); a.out_goal_obs = out_goal_obs;
+    a.d_prev = s->d_dprev; a.ep_step = s->d_epstep; a.poses = s->d_poses;
+    a.ring = s->ring; a.ring_cap = s->ring_cap ? s->ring_cap : 1; a.ring_head = s->ring_head; a.ring_row = ring_row_floats(s);
+    a.counters = s->d_counters;
+    int grid = (s->n + 7) / 8;
+    if (grid > s->num_sms * 8) grid = s->num_sms * 8;
+    reset_kernel<<<grid, 256, 0, s->stream>>>(a);
+    FN_CUDA(cudaGetLastError());
+    return launch_beams(s, s->d_list, s->d_count, out_ranges, s->ring_head);
+}
+
+extern "C" int fn_observe_all(fn_sim* s, const float* states, float* out_ranges, float* out_goal_obs) {
+    if (!s || !states || !out_ranges) return fail(FN_ERR_INVALID_ARG, "fn_observe_all: NULL argument");
+    PoseArgs a;
+    a.map = s->map->dev; a.robot = robot_dev(s->robot, s->map); a.n = s->n; a.states = states;
+    a.out_goal_obs = out_goal_obs; a.poses = s->d_poses;
+    pose_from_state_kernel<<<(s->n + 255) / 256, 256, 0, s->stream>>>(a);
+    FN_CUDA(cudaGetLastError());
+    float* ring = s->ring;           // a test hook: never touches the ring
+    s->ring = nullptr;
+    int st = launch_beams(s, nullptr, nullptr, out_ranges, 0);
+    s->ring = ring;
+    return st;
+}
+
+extern "C" int fn_sim_bind_aux(fn_sim* s, int32_t* hit, float* reward) {
+    if (!s) return fail(FN_ERR_INVALID_ARG, "fn_sim_bind_aux: NULL sim");
+    s->aux_hit = hit; s->aux_reward = reward;
+    return FN_OK;
+}
+
+extern "C" int fn_ring_attach(fn_sim* s, float* ring, uint64_t cap) {
+    if (!s) return fail(FN_ERR_INVALID_ARG, "fn_ring_attach: NULL sim");
+    if (ring && cap < (uint64_t)s->n) return fail(FN_ERR_INVALID_ARG, "fn_ring_attach: capacity must be >= n_envs");
+    s->ring = ring; s->ring_cap = ring ? cap : 0; s->ring_head = 0;
+    return FN_OK;
+}
+
+extern "C" int fn_get_counters(fn_sim* s, uint64_t* host_out) {
+    if (!s || !host_out) return fail(FN_ERR_INVALID_ARG, "fn_get_counters: NULL argument");
+    FN_CUDA(cudaMemcpyAsync(host_out, s->d_counters, kNCounters * sizeof(unsigned long long), cudaMemcpyDeviceToHost, s->stream));
+    FN_CUDA(cudaStreamSynchronize(s->stream));
+    return FN_OK;
+}
+
+extern "C" int fn_sim_count_words(fn_sim* s, int enable) {
+    if (!s) return fail(FN_ERR_INVALID_ARG, "fn_sim_count_words: NULL sim");
+    s->count_words = enable != 0;
+    return FN_OK;
+}
+
+extern "C" int fn_sim_episode_state(fn_sim* s, float* d_prev, int32_t* ep_step) {
+    if (!s) return fail(FN_ERR_INVALID_ARG, "fn_sim_episode_state: NULL sim");
+    if (d_prev) FN_CUDA(cudaMemcpyAsync(d_prev, s->d_dprev, (size_t)s->n * sizeof(float), cudaMemcpyDeviceToHost, s->stream));
+    if (ep_step) FN_CUDA(cudaMemcpyAsync(ep_step, s->d_epstep, (size_t)s->n * sizeof(int), cudaMemcpyDeviceToHost, s->stream));
+    FN_CUDA(cudaStreamSynchronize(s->stream));
+    return FN_OK;
+}
+
+// ------------------------------------------------------------------------------------------ host buffers
+extern "C" int fn_step_host(fn_sim* s, float* states, const float* actions, float dt, uint8_t* mask,
+                            const uint64_t* seeds, float* out_ranges, uint8_t* out_collision, float* out_goal_obs) {
+    if (!s || !states || !actions || !mask || !out_ranges || !out_collision || !out_goal_obs)
+        return fail(FN_ERR_INVALID_ARG, "fn_step_host: NULL argument");
+    const size_t n = (size_t)s->n, B = (size_t)s->robot->B, A = s->robot->drive == FN_DRIVE_DIFF ? 2 : 3;
+    if (!s->stg_states) {
+        FN_CUDA(cudaMalloc(&s->stg_states, 8 * n * sizeof(float)));
+        FN_CUDA(cudaMalloc(&s->stg_actions, n * A * sizeof(float)));
+        FN_CUDA(cudaMalloc(&s->stg_ranges, n * B * sizeof(float)));
+        FN_CUDA(cudaMalloc(&s->stg_gobs, 2 * n * sizeof(float)));
+        FN_CUDA(cudaMalloc(&s->stg_mask, n));
+        FN_CUDA(cudaMalloc(&s->stg_col, n));
+        FN_CUDA(cudaMalloc(&s->stg_seeds, n * sizeof(unsigned long long)));
+    }
+    cudaStream_t st = s->stream;
+    FN_CUDA(cudaMemcpyAsync(s->stg_states, states, 8 * n * sizeof(float), cudaMemcpyHostToDevice, st));
+    FN_CUDA(cudaMemcpyAsync(s->stg_actions, actions, n * A * sizeof(float), cudaMemcpyHostToDevice, st));
+    FN_CUDA(cudaMemcpyAsync(s->stg_mask, mask, n, cudaMemcpyHostToDevice, st));
+    if (seeds) FN_CUDA(cudaMemcpyAsync(s->stg_seeds, seeds, n * sizeof(unsigned long long), cudaMemcpyHostToDevice, st));
+    int rc = fn_step(s, s->stg_states, s->stg_actions, dt, s->stg_mask, s->stg_ranges, s->stg_col, s->stg_gobs);
+    if (rc != FN_OK) return rc;
+    // the step's own (pre-reset) outputs go back first; the reset then overwrites the done rows
+    FN_CUDA(cudaMemcpyAsync(out_collision, s->stg_col, n, cudaMemcpyDeviceToHost, st));
+    FN_CUDA(cudaMemcpyAsync(mask, s->stg_mask, n, cudaMemcpyDeviceToHost, st));
+    if (seeds) {
+        rc = fn_reset(s, s->stg_states, s->stg_mask, reinterpret_cast<const uint64_t*>(s->stg_seeds), s->stg_ranges, s->stg_gobs);
+        if (rc != FN_OK) return rc;
+    }
+    FN_CUDA(cudaMemcpyAsync(states, s->stg_states, 8 * n * sizeof(float), cudaMemcpyDeviceToHost, st));
+    FN_CUDA(cudaMemcpyAsync(out_ranges, s->stg_ranges, n * B * sizeof(float), cudaMemcpyDeviceToHost, st));
+    FN_CUDA(cudaMemcpyAsync(out_goal_obs, s->stg_gobs, 2 * n * sizeof(float), cudaMemcpyDeviceToHost, st));
+    FN_CUDA(cudaStreamSynchronize(st));
+    return FN_OK;
+}

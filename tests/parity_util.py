@@ -1,0 +1,199 @@
+"""Teacher-forced parity of the CUDA path (through the C ABI) against the CPU oracle.
+
+Per step, the oracle is given the GPU's fp32 input state, action, forced mask and seeds; motion output
+is compared at 1e-5; sensing, collision, goal obs and reward are evaluated by the oracle AT THE GPU's
+fp32 post-motion pose (SURVEY.md 8(c) "Teacher forcing").  Tolerances are BASELINE.json north_star's:
+collision flags / hit cells / done flags / reset states bit-exact outside counted near-ties (oracle
+margin 1e-5 cell), ranges abs 1e-4 m, states 1e-5 relative (floor 1), psi modulo 2 pi.
+"""
+from __future__ import annotations
+
+import numpy as np
+import torch
+
+import oracle
+import paper_2606_15846_b200 as fn
+from harness import workloads as W
+
+TOL_RANGE = 1e-4
+TOL_STATE = 1e-5
+
+
+def make_sim(wl, n=None):
+    n = wl.n_envs if n is None else n
+    m = fn.Map(wl.occ, float(wl.resolution))
+    if wl.regions is not None:
+        m.set_regions(wl.regions)
+    r = fn.Robot(wl.footprint, wl.beam_angles, float(wl.max_range), wl.drive, wl.vel_limits)
+    s = fn.Sim(m, r, n, goal_tol=float(wl.goal_tol), max_episode_steps=wl.max_episode_steps,
+               goal_dist_min=float(wl.goal_dist_min), goal_dist_max=float(wl.goal_dist_max),
+               r_success=float(wl.r_success), r_collision=float(wl.r_collision), c_progress=float(wl.c_progress))
+    return m, r, s
+
+
+class Buffers:
+    def __init__(self, n, B, A, dev="cuda"):
+        self.states = torch.zeros(8, n, dtype=torch.float32, device=dev)
+        self.mask = torch.zeros(n, dtype=torch.uint8, device=dev)
+        self.ranges = torch.zeros(n, B, dtype=torch.float32, device=dev)
+        self.col = torch.zeros(n, dtype=torch.uint8, device=dev)
+        self.gobs = torch.zeros(2, n, dtype=torch.float32, device=dev)
+        self.hit = torch.zeros(n, B, dtype=torch.int32, device=dev)
+        self.reward = torch.zeros(n, dtype=torch.float32, device=dev)
+
+
+def ang_diff(a, b):
+    d = (a.astype(np.float64) - b.astype(np.float64) + np.pi) % (2 * np.pi) - np.pi
+    return np.abs(d)
+
+
+def close_state(got, ref):
+    return np.abs(got.astype(np.float64) - ref.astype(np.float64)) <= TOL_STATE * np.maximum(1.0, np.abs(ref.astype(np.float64)))
+
+
+class Report:
+    def __init__(self):
+        self.c = {}
+
+    def add(self, k, v=1):
+        self.c[k] = self.c.get(k, 0) + int(v)
+
+    def __repr__(self):
+        return "parity " + " ".join(f"{k}={v}" for k, v in sorted(self.c.items()))
+
+
+def check_observation(wl, rep, x, y, psi, g_ranges, g_hit, env_idx=None, tag="obs"):
+    """ranges / hit cells of the listed envs at fp32 poses (x, y, psi) vs the oracle."""
+    r, hit, amb = oracle.ranges(wl.occ, wl.resolution, wl.beam_angles, wl.max_range, x, y, psi)
+    ok = amb == 0
+    rep.add("beams", ok.size)
+    rep.add("beams_ambiguous", (~ok).sum())
+    bad_hit = ok & (g_hit != hit)
+    bad_r = ok & (np.abs(g_ranges.astype(np.float64) - r.astype(np.float64)) > TOL_RANGE)
+    if bad_hit.any() or bad_r.any():
+        e, b = np.nonzero(bad_hit | bad_r)
+        k = 0
+        raise AssertionError(
+            f"{tag}: {bad_hit.sum()} hit-cell and {bad_r.sum()} range mismatches outside near-ties; first: env "
+            f"{(env_idx[e[k]] if env_idx is not None else e[k])} beam {b[k]} pose=({x[e[k]]!r},{y[e[k]]!r},{psi[e[k]]!r}) "
+            f"gpu r={g_ranges[e[k], b[k]]!r} hit={g_hit[e[k], b[k]]} oracle r={r[e[k], b[k]]!r} hit={hit[e[k], b[k]]}")
+    # ambiguous beams must still be sane
+    assert np.all(np.isfinite(g_ranges)) and g_ranges.min() >= 0 and g_ranges.max() <= float(wl.max_range) + 1e-6
+
+
+def run_parity(wl, steps, n=None, subset=None, seed=0, forced=None, check_every=1):
+    """Free-running GPU trajectory, teacher-forced oracle check each `check_every` steps.
+    subset: number of envs (a fixed random sample) whose beams are checked; None = all."""
+    n = wl.n_envs if n is None else n
+    wl.n_envs = n
+    B, A = wl.n_beams, wl.action_dim
+    m, r, s = make_sim(wl, n)
+    buf = Buffers(n, B, A)
+    s.bind_aux(buf.hit, buf.reward)
+    actions = torch.from_numpy(W.action_tape(wl, steps, seed)).cuda()
+    seeds_np = W.seed_tape(wl, steps + 1, seed)
+    forced_np = W.forced_reset_tape(wl, steps, seed) if forced is None else forced
+    rng = np.random.default_rng(seed + 99)
+    sel = np.arange(n) if subset is None or subset >= n else np.sort(rng.choice(n, subset, replace=False))
+    rep = Report()
+
+    def do_reset(mask_np, seeds_row, tag):
+        pre = buf.states.cpu().numpy()
+        d_prev0, ep0 = s.episode_state()
+        seeds_t = torch.from_numpy(seeds_row.view(np.int64)).cuda()
+        mask_t = torch.from_numpy(mask_np).cuda()
+        keep_r = buf.ranges.clone()
+        s.reset(buf.states, mask_t, seeds_t, buf.ranges, buf.gobs)
+        torch.cuda.synchronize()
+        post = buf.states.cpu().numpy()
+        ref = pre.copy()
+        d_prev, ep = d_prev0.copy(), ep0.copy()
+        amb, failed = oracle.reset(wl.occ, wl.resolution, wl.footprint, wl.regions, wl.goal_dist_min,
+                                   wl.goal_dist_max, mask_np, seeds_row, ref, d_prev, ep)
+        okm = (mask_np != 0) & (amb == 0)
+        rep.add("resets", (mask_np != 0).sum())
+        rep.add("resets_ambiguous", ((mask_np != 0) & (amb != 0)).sum())
+        rep.add("reset_failures", failed.sum())
+        assert np.array_equal(post[:, mask_np == 0], pre[:, mask_np == 0]), f"{tag}: reset touched unmasked envs"
+        if not np.array_equal(post[:, okm], ref[:, okm]):
+            e = np.nonzero(okm & np.any(post != ref, axis=0))[0][0]
+            raise AssertionError(f"{tag}: reset state differs for env {e}: gpu {post[:, e]} oracle {ref[:, e]} seed {seeds_row[e]}")
+        gd, ge = s.episode_state()
+        assert np.array_equal(ge[okm], ep[okm]) and np.all(ge[mask_np == 0] == ep0[mask_np == 0])
+        assert np.allclose(gd[okm], d_prev[okm], atol=1e-5) and np.array_equal(gd[mask_np == 0], d_prev0[mask_np == 0])
+        # selective recompute: unmasked rows untouched, masked rows = observation at the new state
+        rg = buf.ranges.cpu().numpy()
+        assert np.array_equal(rg[mask_np == 0], keep_r.cpu().numpy()[mask_np == 0]), f"{tag}: recompute touched other rows"
+        idx = np.nonzero(okm)[0]
+        if subset is not None and idx.size > subset:
+            idx = idx[:subset]
+        if idx.size:
+            check_observation(wl, rep, post[0, idx], post[1, idx], post[2, idx], rg[idx], buf.hit.cpu().numpy()[idx],
+                              idx, tag + "/recompute")
+            g = buf.gobs.cpu().numpy()
+            og = oracle.goal_obs(post[0, idx], post[1, idx], post[2, idx], post[6, idx], post[7, idx])
+            assert np.all(close_state(g[0, idx], og[0])) and np.all(ang_diff(g[1, idx], og[1]) <= 1e-5)
+
+    do_reset(np.ones(n, np.uint8), seeds_np[0], "initial reset")
+
+    n_done = 0
+    for t in range(steps):
+        check = (t % check_every == 0) or t < 3
+        pre = buf.states.cpu().numpy() if check else None
+        d_prev0, ep0 = s.episode_state() if check else (None, None)
+        buf.mask.copy_(torch.from_numpy(forced_np[t]))
+        s.step(buf.states, actions[t], float(wl.dt), buf.mask, buf.ranges, buf.col, buf.gobs)
+        torch.cuda.synchronize()
+        done = buf.mask.cpu().numpy()
+        n_done += int(done.sum())
+        if check:
+            post = buf.states.cpu().numpy()
+            ref = oracle.motion(wl.drive, wl.vel_limits, wl.dt, pre, actions[t].cpu().numpy())
+            for p in (0, 1, 3, 4, 5, 6, 7):
+                assert np.all(close_state(post[p], ref[p])), f"step {t}: state plane {p} off by {np.abs(post[p] - ref[p]).max()}"
+            assert np.all(ang_diff(post[2], ref[2]) <= TOL_STATE * np.maximum(1, np.abs(ref[2]))), f"step {t}: psi"
+            x, y, psi = post[0], post[1], post[2]
+            flag, camb = oracle.collision(wl.occ, wl.resolution, wl.footprint, x, y, psi)
+            gcol = buf.col.cpu().numpy()
+            okc = camb == 0
+            rep.add("collision_checks", n)
+            rep.add("collision_ambiguous", (~okc).sum())
+            rep.add("collisions", int(flag.sum()))
+            if not np.array_equal(gcol[okc], flag[okc]):
+                e = np.nonzero(okc & (gcol != flag))[0][0]
+                raise AssertionError(f"step {t}: collision flag differs for env {e}: gpu {gcol[e]} oracle {flag[e]} pose {x[e]!r},{y[e]!r},{psi[e]!r}")
+            og = oracle.goal_obs(x, y, psi, post[6], post[7])
+            g = buf.gobs.cpu().numpy()
+            assert np.all(close_state(g[0], og[0])), f"step {t}: goal distance"
+            far = og[0] > 1e-3
+            assert np.all(ang_diff(g[1], og[1])[far] <= 1e-5), f"step {t}: goal direction"
+            # reward / done from the GPU's own d (so that the fp32 threshold decision is taken on the same bits)
+            d_prev, ep = d_prev0.copy(), ep0.copy()
+            rew, odone = oracle.reward_done(g[0], gcol, forced_np[t], d_prev, ep, float(wl.goal_tol), wl.max_episode_steps,
+                                            float(wl.r_success), float(wl.r_collision), float(wl.c_progress))
+            assert np.array_equal(done, odone), f"step {t}: done flags"
+            assert np.allclose(buf.reward.cpu().numpy(), rew, atol=1e-4), f"step {t}: reward"
+            gd, ge = s.episode_state()
+            assert np.array_equal(ge, ep) and np.array_equal(gd, d_prev)
+            check_observation(wl, rep, x[sel], y[sel], psi[sel], buf.ranges.cpu().numpy()[sel], buf.hit.cpu().numpy()[sel],
+                              sel, f"step {t}")
+        if done.any():
+            if check:
+                do_reset(done, seeds_np[t + 1], f"step {t} reset")
+            else:
+                s.reset(buf.states, buf.mask, torch.from_numpy(seeds_np[t + 1].view(np.int64)).cuda(), buf.ranges, buf.gobs)
+
+    # observation is a pure function of state: the incrementally maintained rows equal a full recompute
+    full_r = torch.empty_like(buf.ranges)
+    full_g = torch.empty_like(buf.gobs)
+    s.observe_all(buf.states, full_r, full_g)
+    torch.cuda.synchronize()
+    assert torch.equal(full_r, buf.ranges), "observe_all differs from incrementally maintained ranges"
+    assert torch.equal(full_g, buf.gobs), "observe_all differs from incrementally maintained goal obs"
+    rep.add("steps", steps)
+    rep.add("done_events", n_done)
+    cnt = s.counters()
+    rep.add("rays_cast", cnt["rays_cast"])
+    assert cnt["reset_failures"] == rep.c.get("reset_failures", 0) or check_every > 1
+    s.close(); r.close(); m.close()
+    return rep

@@ -1,0 +1,127 @@
+"""GPU parity tests proper: the CUDA path through the C ABI vs the CPU oracle (pytest -m gpu)."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def pu():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import oracle
+    oracle.build()
+    import parity_util
+    return parity_util
+
+
+def test_c1_tiny_full(pu):
+    from harness import workloads as W
+    wl = W.make_workload(1)
+    rep = pu.run_parity(wl, steps=100)
+    print(rep)
+    assert rep.c["beams_ambiguous"] < 1e-3 * rep.c["beams"]
+
+
+def test_c1_ragged_env_counts(pu):
+    # env counts that are not multiples of a warp/CTA; 1 env; beams not a multiple of 32
+    from harness import workloads as W
+    for n in (1, 7, 33):
+        wl = W.make_workload(1, n_envs=n)
+        wl.beam_angles = W.beam_table(45 + n, 270.0)
+        print(n, pu.run_parity(wl, steps=12, seed=n))
+
+
+def test_c2_rect_subset(pu):
+    from harness import workloads as W
+    wl = W.make_workload(2)
+    rep = pu.run_parity(wl, steps=30, subset=256, check_every=10)
+    print(rep)
+
+
+def test_c3_nonconvex_omni(pu):
+    from harness import workloads as W
+    wl = W.make_workload(3, n_envs=1024)
+    rep = pu.run_parity(wl, steps=30, subset=256, check_every=5)
+    print(rep)
+    assert rep.c["collisions"] > 0
+
+
+def test_c4_large_map_l2_path_forced_resets(pu):
+    from harness import workloads as W
+    wl = W.make_workload(4, n_envs=2048)
+    rep = pu.run_parity(wl, steps=20, subset=512, check_every=5)
+    print(rep)
+    assert rep.c["resets"] > 2048
+
+
+def test_c5_tiles_regions(pu):
+    from harness import workloads as W
+    wl = W.make_workload(5, n_envs=1024)
+    rep = pu.run_parity(wl, steps=20, subset=128, check_every=5)
+    print(rep)
+
+
+def test_tiny_maps_odd_sizes_and_no_border(pu):
+    # map sizes that are not multiples of 32, no border walls (beams and robots leave the map)
+    from harness import workloads as W
+    for size, seed in ((19, 1), (33, 2), (70, 3)):
+        wl = W.tiny_workload(size=size, n_envs=64, n_beams=41, seed=seed, max_range=2.0)
+        wl.occ[0, :] = wl.occ[-1, :] = 0
+        wl.occ[:, 0] = wl.occ[:, -1] = 0
+        wl.goal_dist_min, wl.goal_dist_max = np.float32(0.2), np.float32(0.6)
+        print(size, pu.run_parity(wl, steps=15, seed=seed))
+
+
+def test_axis_aligned_and_degenerate_beams(pu):
+    # beams exactly along the axes and diagonals from exactly representable poses (ties, long spans)
+    import torch
+    import oracle
+    import paper_2606_15846_b200 as fn
+    from harness import workloads as W
+    occ = np.zeros((200, 300), np.uint8)
+    occ[:, 280:] = 1
+    occ[150:, :] = 1
+    occ[:, :3] = 1
+    occ[:2, :] = 1
+    ang = np.array([0, np.pi / 2, np.pi, -np.pi / 2, np.pi / 4, -3 * np.pi / 4, 1e-7, np.pi / 2 + 1e-7], np.float32)
+    m = fn.Map(occ, 0.05)
+    r = fn.Robot(W.footprint_rect(0.2, 0.2), ang, 20.0, 0, [0, 1, 0, 0, -1, 1])
+    n = 8
+    s = fn.Sim(m, r, n)
+    st = torch.zeros(8, n, device="cuda")
+    # rows 1 and 3 sit exactly on lattice lines (legitimately ambiguous); the others do not
+    xs = np.array([5.025, 5.0, 7.5125, 1.0, 12.3, 5.0125, 9.9875, 3.3375], np.float32)
+    ys = np.array([5.025, 5.0, 2.5125, 6.0, 0.7, 3.7625, 6.2625, 1.1125], np.float32)
+    st[0] = torch.from_numpy(xs).cuda(); st[1] = torch.from_numpy(ys).cuda()
+    out = torch.zeros(n, len(ang), device="cuda")
+    hit = torch.zeros(n, len(ang), dtype=torch.int32, device="cuda")
+    s.bind_aux(hit, None)
+    s.observe_all(st, out)
+    torch.cuda.synchronize()
+    ro, ho, amb = oracle.ranges(occ, np.float32(0.05), ang, 20.0, xs, ys, np.zeros(n, np.float32))
+    ok = amb == 0
+    assert ok.sum() >= 40
+    assert np.allclose(out.cpu().numpy()[ok], ro[ok], atol=1e-4)
+    assert np.array_equal(hit.cpu().numpy()[ok], ho[ok])
+
+
+def test_argument_errors(pu):
+    import paper_2606_15846_b200 as fn
+    from harness import workloads as W
+    occ = np.zeros((8, 8), np.uint8)
+    with pytest.raises(fn.FlashNavError):
+        fn.Map(occ, 0.0)
+    with pytest.raises(fn.FlashNavError):
+        fn.Robot(W.footprint_rect(0.2, 0.2)[:2], [0.0], 1.0, 0, [0, 1, 0, 0, -1, 1])
+    with pytest.raises(fn.FlashNavError):
+        fn.Robot(W.footprint_rect(0.2, 0.2), [0.0], 1.0, 0, [1, 0, 0, 0, -1, 1])
+    with pytest.raises(fn.FlashNavError):
+        fn.Robot(W.footprint_rect(0.2, 0.2), [0.0], 1.0, 5, [0, 1, 0, 0, -1, 1])
+    m = fn.Map(occ, 0.05)
+    with pytest.raises(fn.FlashNavError):
+        m.set_regions([[0, 0, 9, 9]])
+    r = fn.Robot(W.footprint_rect(0.2, 0.2), [0.0], 1.0, 0, [0, 1, 0, 0, -1, 1])
+    with pytest.raises(fn.FlashNavError):
+        fn.Sim(m, r, 0)

@@ -1,0 +1,373 @@
+#!/usr/bin/env python
+"""bench.py -- env-steps/s and rays/s of the FlashNav simulator step on B200 (BASELINE.json metric).
+
+A "step" is one pass of the whole hot path over one batch: fn_step (clip + motion, footprint collision,
+goal obs / reward / done, beam casting for all envs) followed by fn_reset of the done envs (compaction,
+reset, observation recompute for those envs only).  Default workload: BASELINE.json configs[1]
+(C2: 512x512 map, 4096 envs, 720 beams over 270 deg, 10 m range, differential drive).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5] [--impl ours|reference]
+
+N > 1 (torchrun): environments are independent, so every rank runs its own batch on its own GPU with no
+data-path collective ("scaling": "weak"); value = total env-steps of all ranks / max-over-ranks time.
+--impl reference times the CPU oracle (oracle/) on the host cores on a bounded sample of the same
+workload; it is a deliberately slow program (parity and the roofline fraction are the headline).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from harness import workloads as W  # noqa: E402
+
+METRIC = "env_steps_per_s"
+UNIT = "env-steps/s"
+
+
+def workload_name(cfg):
+    return f"BASELINE.json configs[{cfg - 1}]"
+
+
+# --------------------------------------------------------------------------- reference arm = the oracle
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    import oracle
+    oracle.build()
+    wl = W.make_workload(args.config)
+    n = min(wl.n_envs, args.ref_envs)
+    wl.n_envs = n
+    st = np.zeros((8, n), np.float32)
+    dp = np.zeros(n, np.float32)
+    ep = np.zeros(n, np.int32)
+    seeds = W.seed_tape(wl, args.steps + args.warmup + 1)
+    act = W.action_tape(wl, args.steps + args.warmup)
+    oracle.reset(wl.occ, wl.resolution, wl.footprint, wl.regions, wl.goal_dist_min, wl.goal_dist_max,
+                 np.ones(n, np.uint8), seeds[0], st, dp, ep)
+
+    def one(t):
+        out = oracle.step(wl, st, act[t], None, dp, ep, want_hit=False)
+        done = out["done"]
+        if done.any():
+            oracle.reset(wl.occ, wl.resolution, wl.footprint, wl.regions, wl.goal_dist_min, wl.goal_dist_max,
+                         done, seeds[t + 1], st, dp, ep)
+            idx = np.nonzero(done)[0]
+            oracle.ranges(wl.occ, wl.resolution, wl.beam_angles, wl.max_range, st[0, idx], st[1, idx], st[2, idx], eps=0.0)
+        return int(done.sum())
+
+    for t in range(args.warmup):
+        one(t)
+    t0 = time.perf_counter()
+    resets = 0
+    for t in range(args.warmup, args.warmup + args.steps):
+        resets += one(t)
+    dt = time.perf_counter() - t0
+    v = n * args.steps / dt
+    sample = f"{n} of {W.make_workload(args.config).n_envs} envs x {args.steps} steps, single thread"
+    line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workload_name(args.config), "n_envs_sample": n, "beams": wl.n_beams},
+            "rays_per_s": (n * args.steps + resets) * wl.n_beams / dt,
+            "cpu_baseline": {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+            "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+# --------------------------------------------------------------------------- clocks sampling
+class ClockSampler:
+    Q = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
+        "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+
+    def __init__(self, gpu_index):
+        self.rows = []
+        self.proc = None
+        self.gpu = gpu_index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.gpu), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for ln in self.proc.stdout:
+            self.rows.append(ln.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, smax, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            f = [x.strip() for x in r.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); smax.append(float(f[1]))
+            except ValueError:
+                continue
+            for k, nm in enumerate(names):
+                if f[3 + k].lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(smax) if smax else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+# --------------------------------------------------------------------------- algorithmic bytes per beam
+def algorithmic_bytes_per_beam(wl, states_np, n_sample=128, seed=0):
+    """A_ray from the ORACLE's exact path, for the word shape the kernel uses:
+    one 32-bit word for the origin-cell test + one 64-bit window per line the beam visits along its minor
+    axis up to and including the hit line (+1 window per further 32 cells of a span longer than 32 cells)."""
+    import oracle
+    n = states_np.shape[1]
+    idx = np.random.default_rng(seed).choice(n, min(n, n_sample), replace=False)
+    x, y, psi = states_np[0, idx], states_np[1, idx], states_np[2, idx]
+    r, hit, amb = oracle.ranges(wl.occ, wl.resolution, wl.beam_angles, wl.max_range, x, y, psi, eps=0.0)
+    rho = np.float64(wl.resolution)
+    phi = psi[:, None].astype(np.float64) + wl.beam_angles[None, :].astype(np.float64)
+    dx, dy = np.cos(phi), np.sin(phi)
+    t = r.astype(np.float64) / rho
+    ox, oy = x[:, None] / rho, y[:, None] / rho
+    ex, ey = ox + t * dx, oy + t * dy
+    # entry point of the hit cell lies on its boundary: nudge inside along the beam to name the cell
+    ex, ey = ex + 1e-9 * dx, ey + 1e-9 * dy
+    major_x = np.abs(dx) >= np.abs(dy)
+    lines = np.where(major_x, np.abs(np.floor(ey) - np.floor(oy)), np.abs(np.floor(ex) - np.floor(ox))) + 1
+    slope = np.maximum(np.abs(dx), np.abs(dy)) / np.maximum(np.minimum(np.abs(dx), np.abs(dy)), 1e-12)
+    extra = np.where(slope > 32, np.floor(np.where(major_x, np.abs(ex - ox), np.abs(ey - oy)) / 32), 0)
+    windows = lines + extra
+    return float(4.0 + 8.0 * windows.mean()), float(windows.mean())
+
+
+# --------------------------------------------------------------------------- our arm
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    import paper_2606_15846_b200 as fn
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    fn.load_library()
+
+    wl = W.make_workload(args.config)
+    n, B, A = wl.n_envs, wl.n_beams, wl.action_dim
+    K, Wm = args.steps, args.warmup
+    tape_len = min(K + Wm, 256)
+    actions = torch.from_numpy(W.action_tape(wl, tape_len, seed=wl.seed + 17 * rank)).cuda()
+    seeds = torch.from_numpy(W.seed_tape(wl, tape_len + 1, seed=wl.seed + 17 * rank).view(np.int64)).cuda()
+    forced = torch.from_numpy(W.forced_reset_tape(wl, tape_len, seed=wl.seed + 17 * rank)).cuda()
+
+    m = fn.Map(wl.occ, float(wl.resolution))
+    if wl.regions is not None:
+        m.set_regions(wl.regions)
+    rb = fn.Robot(wl.footprint, wl.beam_angles, float(wl.max_range), wl.drive, wl.vel_limits)
+    sim = fn.Sim(m, rb, n, goal_tol=float(wl.goal_tol), max_episode_steps=wl.max_episode_steps,
+                 goal_dist_min=float(wl.goal_dist_min), goal_dist_max=float(wl.goal_dist_max))
+    states = torch.zeros(8, n, device="cuda")
+    mask = torch.ones(n, dtype=torch.uint8, device="cuda")
+    ranges = torch.zeros(n, B, device="cuda")
+    col = torch.zeros(n, dtype=torch.uint8, device="cuda")
+    gobs = torch.zeros(2, n, device="cuda")
+    ring = None
+    if wl.ring_capacity and args.ring:
+        ring = torch.zeros(wl.ring_capacity * sim.ring_row_floats(), device="cuda")
+        sim.ring_attach(ring, wl.ring_capacity)
+    sim.reset(states, mask, seeds[tape_len], ranges, gobs)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")     # > 126 MB L2
+
+    def step(t):
+        k = t % tape_len
+        mask.copy_(forced[k])
+        sim.step(states, actions[k], float(wl.dt), mask, ranges, col, gobs)
+        sim.reset(states, mask, seeds[k], ranges, gobs)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for t in range(Wm):
+        step(t)
+    barrier()
+    c0 = sim.counters()
+    sim.profile(True)
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    ev0 = [torch.cuda.Event(enable_timing=True) for _ in range(K)]
+    ev1 = [torch.cuda.Event(enable_timing=True) for _ in range(K)]
+    for k in range(K):
+        flush.fill_(k & 0xff)                      # L2 flush between timed iterations (outside the events)
+        ev0[k].record()
+        step(Wm + k)
+        ev1[k].record()
+    barrier()
+    clocks = sampler.stop() if rank == 0 else None
+    per_step_ms = np.array([ev0[k].elapsed_time(ev1[k]) for k in range(K)])
+    prof = sim.profile_read()
+    sim.profile(False)
+    c1 = sim.counters()
+    total_ms = float(per_step_ms.sum())
+
+    # steady state (no L2 flush, back to back): information only
+    s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    s0.record()
+    for k in range(K):
+        step(Wm + K + k)
+    s1.record()
+    barrier()
+    steady_ms = s0.elapsed_time(s1)
+
+    tmax = torch.tensor([total_ms, steady_ms], device="cuda", dtype=torch.float64)
+    rays = torch.tensor([float(c1["rays_cast"] - c0["rays_cast"]), float(c1["envs_reset"] - c0["envs_reset"])],
+                        device="cuda", dtype=torch.float64)
+    if world > 1:
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+        dist.all_reduce(rays, op=dist.ReduceOp.SUM)
+    total_ms, steady_ms = float(tmax[0]), float(tmax[1])
+    value = world * n * K / (total_ms * 1e-3)
+
+    out = None
+    if rank == 0:
+        # ---- roofline of the dominant kernel (full-batch beam kernel of fn_step), live CUDA events
+        beam_ms, beam_launches = prof["beam_step"]
+        env_ms, _ = prof["env_step"]
+        reset_ms, _ = prof["reset_path"]
+        st_np = states.cpu().numpy()
+        a_ray, windows = algorithmic_bytes_per_beam(wl, st_np)
+        smem_peak = fn.measure_peak(0)
+        l2_peak = fn.measure_peak(2)
+        use_smem = (wl.occ.shape[0] * ((wl.occ.shape[1] + 31) // 32 + 2) + wl.occ.shape[1] * ((wl.occ.shape[0] + 31) // 32 + 2)) * 4 \
+            + B * 16 <= 227 * 1024
+        peak = smem_peak if use_smem else l2_peak
+        beam_s = beam_ms * 1e-3 / max(1, beam_launches)
+        achieved = a_ray * n * B / beam_s
+        roofline = {"bound": "smem" if use_smem else "l2", "kernel": "fn::beam_kernel (fn_step, all envs)",
+                    "achieved": achieved / 1e9, "peak": peak / 1e9, "unit": "GB/s", "frac": achieved / peak,
+                    "peak_source": "fn_measure_peak in this run (conflict-free ld.shared / L2-resident ld.global.nc)",
+                    "algorithmic_bytes_per_beam": a_ray, "windows_per_beam": windows,
+                    "kernel_ms": beam_s * 1e3, "share_of_step": beam_ms / total_ms if world == 1 else None,
+                    "traffic": None, "smem_peak_GBps": smem_peak / 1e9, "l2_peak_GBps": l2_peak / 1e9,
+                    "issue": {"note": "kernel is issue-slot bound, see DESIGN.md / profiles", "beams_per_s": n * B / beam_s}}
+        # ---- oracle on the host cores, bounded sample of the same workload
+        cpu = None
+        if not args.no_cpu:
+            import oracle
+            oracle.build()
+            ns = min(n, args.ref_envs)
+            st = np.ascontiguousarray(st_np[:, :ns])
+            dp = np.zeros(ns, np.float32)
+            ep = np.zeros(ns, np.int32)
+            wl_s = W.make_workload(args.config, n_envs=ns)
+            act = W.action_tape(wl_s, args.cpu_steps)
+            t0 = time.perf_counter()
+            for t in range(args.cpu_steps):
+                oracle.step(wl_s, st, act[t], None, dp, ep, want_hit=False)
+            dtc = time.perf_counter() - t0
+            cpu = {"value": ns * args.cpu_steps / dtc, "unit": UNIT, "cores": 1, "kind": "oracle",
+                   "sample": f"{ns} of {n} envs x {args.cpu_steps} steps (fn_step part only, no resets), single thread",
+                   "rays_per_s": ns * args.cpu_steps * B / dtc, "host_cores_available": os.cpu_count()}
+        out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
+               "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+               "dtype": "f64+i64 fixed point (fp32 storage)", "data": "synthetic",
+               "config": {"workload": workload_name(args.config), "name": wl.name, "n_envs_per_gpu": n, "beams": B,
+                          "map": list(wl.occ.shape), "max_range_m": float(wl.max_range), "l2": "flushed between timed steps",
+                          "ring": bool(ring is not None)},
+               "rays_per_s": float(rays[0]) / (total_ms * 1e-3),
+               "useful_rays_per_s": world * n * B * K / (total_ms * 1e-3),
+               "reset_rate_per_step": float(rays[1]) / (world * n * K),
+               "steady_state": {"value": world * n * K / (steady_ms * 1e-3), "unit": UNIT, "ms_per_step": steady_ms / K,
+                                "note": "no L2 flush, K steps back to back"},
+               "kernel_ms_per_step": {"env_step": env_ms / K, "beam_step": beam_ms / K, "reset_path": reset_ms / K},
+               "ms_per_step_p50": float(np.median(per_step_ms)), "ms_per_step_p90": float(np.percentile(per_step_ms, 90)),
+               "roofline": roofline, "cpu_baseline": cpu, "clocks": clocks, "gpu_launches": 5 * K}
+
+    # ---- end to end through the public API with HOST buffers (copies inside the timed region)
+    hs = torch.empty(8, n, dtype=torch.float32).pin_memory()
+    ha = W.action_tape(wl, 8, seed=3)
+    ha_p = [torch.from_numpy(ha[k]).pin_memory() for k in range(8)]
+    hseed = [torch.from_numpy(W.seed_tape(wl, 8, seed=3)[k].view(np.int64)).pin_memory() for k in range(8)]
+    hm = torch.zeros(n, dtype=torch.uint8).pin_memory()
+    hr = torch.empty(n, B, dtype=torch.float32).pin_memory()
+    hc = torch.empty(n, dtype=torch.uint8).pin_memory()
+    hg = torch.empty(2, n, dtype=torch.float32).pin_memory()
+    hs.copy_(states)
+    Ke = max(3, min(K, args.e2e_steps))
+    for k in range(3):
+        hm.zero_()
+        sim.step_host(hs, ha_p[k % 8], float(wl.dt), hm, hseed[k % 8], hr, hc, hg)
+    barrier()
+    t0 = time.perf_counter()
+    for k in range(Ke):
+        hm.zero_()
+        sim.step_host(hs, ha_p[k % 8], float(wl.dt), hm, hseed[k % 8], hr, hc, hg)
+    barrier()
+    e2e_s = time.perf_counter() - t0
+    te = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
+    if world > 1:
+        dist.all_reduce(te, op=dist.ReduceOp.MAX)
+    if rank == 0:
+        h2d = 8 * n * 4 + n * A * 4 + n + n * 8
+        d2h = 8 * n * 4 + n * B * 4 + 2 * n * 4 + n + n
+        out["e2e"] = {"value": world * n * Ke / float(te[0]), "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                      "steps": Ke, "note": "fn_step_host: pinned host buffers, H2D + fn_step + fn_reset + D2H + sync per step"}
+        print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--config", type=int, default=2)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--ref-envs", type=int, default=4096, help="oracle sample size (envs)")
+    ap.add_argument("--cpu-steps", type=int, default=8, help="oracle steps in the cpu_baseline leg")
+    ap.add_argument("--e2e-steps", type=int, default=50)
+    ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--ring", type=int, default=1, help="attach the replay ring when the config has one (C5)")
+    args = ap.parse_args()
+    if args.warmup < 3:
+        args.warmup = 3
+    if args.impl == "reference":
+        if args.steps > 16:
+            args.steps = 16          # bounded: ~1.6 s per C2 step on one core
+        args.warmup = min(args.warmup, 1)
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

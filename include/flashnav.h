@@ -118,6 +118,13 @@ int fn_sim_count_words(fn_sim* sim, int enable);
  * (either may be NULL); synchronises the stream. */
 int fn_sim_episode_state(fn_sim* sim, float* d_prev_host, int32_t* ep_step_host);
 
+/* ---- live kernel timing (bench.py's roofline): when enabled, fn_step / fn_reset record CUDA events on
+ * the sim's stream around their kernels.  fn_sim_profile_read synchronises, adds up the elapsed times
+ * since the last read and clears them.  ms_out[4] / launches_out[4] = {env-step kernel, beam kernel of
+ * fn_step, whole fn_reset path (compaction + reset + beam kernels), reserved}. */
+int fn_sim_profile(fn_sim* sim, int enable);
+int fn_sim_profile_read(fn_sim* sim, double* ms_out, uint64_t* launches_out);
+
 /* ---- end-to-end convenience: host buffers in, host buffers out -----------------------------------------
  * Copies states/actions/mask (and seeds) host->device, runs fn_step (+ fn_reset of the done envs when
  * seeds_host != NULL), copies states, ranges, collision, goal obs and the done mask back, synchronises.

@@ -19,7 +19,7 @@ EXPORTED_SYMBOLS = (
     "fn_map_create", "fn_map_set_regions", "fn_map_destroy", "fn_robot_create", "fn_robot_set_sensor",
     "fn_robot_destroy", "fn_task_default", "fn_sim_create", "fn_sim_destroy", "fn_step", "fn_reset",
     "fn_sim_bind_aux", "fn_ring_attach", "fn_observe_all", "fn_get_counters", "fn_sim_count_words",
-    "fn_sim_episode_state", "fn_step_host", "fn_measure_peak", "fn_last_error", "fn_version")
+    "fn_sim_episode_state", "fn_sim_profile", "fn_sim_profile_read", "fn_step_host", "fn_measure_peak", "fn_last_error", "fn_version")
 
 
 class FlashNavError(RuntimeError):
@@ -63,6 +63,8 @@ def load_library():
         "fn_get_counters": [vp, vp],
         "fn_sim_count_words": [vp, i32],
         "fn_sim_episode_state": [vp, vp, vp],
+        "fn_sim_profile": [vp, i32],
+        "fn_sim_profile_read": [vp, vp, vp],
         "fn_step_host": [vp, vp, vp, f32, vp, vp, vp, vp, vp],
         "fn_measure_peak": [i32, vp, C.POINTER(C.c_double)],
     }
@@ -232,6 +234,17 @@ class Sim:
 
     def count_words(self, enable: bool):
         _check(load_library().fn_sim_count_words(self._h, int(bool(enable))), "fn_sim_count_words")
+
+    def profile(self, enable: bool):
+        _check(load_library().fn_sim_profile(self._h, int(bool(enable))), "fn_sim_profile")
+
+    def profile_read(self):
+        """dict kernel -> (total ms, launches) since the last read; synchronises."""
+        ms = np.zeros(4, np.float64)
+        ln = np.zeros(4, np.uint64)
+        _check(load_library().fn_sim_profile_read(self._h, _np_ptr(ms), _np_ptr(ln)), "fn_sim_profile_read")
+        return {"env_step": (float(ms[0]), int(ln[0])), "beam_step": (float(ms[1]), int(ln[1])),
+                "reset_path": (float(ms[2]), int(ln[2]))}
 
     def episode_state(self):
         """Host copies of the sim's d_prev [N] f32 and ep_step [N] i32 (synchronises)."""

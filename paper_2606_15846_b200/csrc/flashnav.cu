@@ -63,6 +63,7 @@ struct fn_sim {
     int num_sms;
     // device state owned by the sim
     PoseD* d_poses;
+    int* d_inside;
     int* d_list;
     int* d_count;
     float* d_dprev;
@@ -78,6 +79,10 @@ struct fn_sim {
     bool use_smem;
     size_t beam_smem;
     int beam_grid;
+    // live timing
+    int prof;
+    std::vector<cudaEvent_t>* ev;    // triples per fn_step (e0 env e1 beam e2), pairs per fn_reset
+    std::vector<int>* ev_kind;       // 0 = step triple start, 1 = reset pair start
     // device staging for fn_step_host (lazily allocated)
     float *stg_states, *stg_actions, *stg_ranges, *stg_gobs;
     uint8_t *stg_mask, *stg_col;
@@ -241,7 +246,7 @@ extern "C" int fn_sim_create(const fn_map* map, const fn_robot* robot, int n, co
                              void* stream, fn_sim** out) {
     if (!map || !robot || !out) return fail(FN_ERR_INVALID_ARG, "fn_sim_create: NULL argument");
     if (n <= 0) return fail(FN_ERR_INVALID_ARG, "fn_sim_create: n_envs must be > 0");
-    if ((long long)n * robot->B > (1ll << 40)) return fail(FN_ERR_UNSUPPORTED, "fn_sim_create: n_envs * B too large");
+    if ((long long)n * robot->B >= (1ll << 31)) return fail(FN_ERR_UNSUPPORTED, "fn_sim_create: n_envs * B must be < 2^31");
     fn_sim* s = new (std::nothrow) fn_sim();
     if (!s) return fail(FN_ERR_OOM, "fn_sim_create: host allocation failed");
     std::memset(s, 0, sizeof(*s));
@@ -256,6 +261,8 @@ extern "C" int fn_sim_create(const fn_map* map, const fn_robot* robot, int n, co
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&s->num_sms, cudaDevAttrMultiProcessorCount, dev);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
     if (e == cudaSuccess) e = cudaMalloc(&s->d_poses, (size_t)n * sizeof(PoseD));
+    if (e == cudaSuccess) e = cudaMalloc(&s->d_inside, (size_t)n * sizeof(int));
+    if (e == cudaSuccess) e = cudaMemsetAsync(s->d_inside, 0, (size_t)n * sizeof(int), s->stream);
     if (e == cudaSuccess) e = cudaMalloc(&s->d_list, (size_t)n * sizeof(int));
     if (e == cudaSuccess) e = cudaMalloc(&s->d_count, sizeof(int));
     if (e == cudaSuccess) e = cudaMalloc(&s->d_dprev, (size_t)n * sizeof(float));
@@ -294,8 +301,9 @@ extern "C" int fn_sim_create(const fn_map* map, const fn_robot* robot, int n, co
 
 extern "C" int fn_sim_destroy(fn_sim* s) {
     if (!s) return FN_OK;
-    cudaFree(s->d_poses); cudaFree(s->d_list); cudaFree(s->d_count); cudaFree(s->d_dprev);
+    cudaFree(s->d_poses); cudaFree(s->d_inside); cudaFree(s->d_list); cudaFree(s->d_count); cudaFree(s->d_dprev);
     cudaFree(s->d_epstep); cudaFree(s->d_counters);
+    if (s->ev) { for (cudaEvent_t e : *s->ev) cudaEventDestroy(e); delete s->ev; delete s->ev_kind; }
     cudaFree(s->stg_states); cudaFree(s->stg_actions); cudaFree(s->stg_ranges); cudaFree(s->stg_gobs);
     cudaFree(s->stg_mask); cudaFree(s->stg_col); cudaFree(s->stg_seeds);
     delete s;
@@ -306,16 +314,17 @@ static int ring_row_floats(const fn_sim* s) { return s->robot->B + 5 + (s->robot
 
 static int launch_beams(fn_sim* s, const int* list, const int* count_dev, float* out_ranges, unsigned long long ring_head) {
     BeamArgs b;
-    b.map = s->map->dev; b.robot = robot_dev(s->robot, s->map); b.poses = s->d_poses;
+    b.map = s->map->dev; b.robot = robot_dev(s->robot, s->map); b.poses = s->d_poses; b.pose_inside = s->d_inside; b.count_words = s->count_words;
     b.list = list; b.count_dev = count_dev; b.n_all = s->n; b.out_ranges = out_ranges; b.out_hit = s->aux_hit;
     b.ring_obs = s->ring; b.ring_cap = s->ring_cap ? s->ring_cap : 1; b.ring_head = ring_head; b.ring_row = ring_row_floats(s);
     b.counters = s->d_counters;
     const dim3 grid(s->beam_grid), block(512);
+    const bool aux = s->count_words || s->aux_hit;
     if (s->use_smem) {
-        if (s->count_words) beam_kernel<true, true><<<grid, block, s->beam_smem, s->stream>>>(b);
+        if (aux) beam_kernel<true, true><<<grid, block, s->beam_smem, s->stream>>>(b);
         else beam_kernel<true, false><<<grid, block, s->beam_smem, s->stream>>>(b);
     } else {
-        if (s->count_words) beam_kernel<false, true><<<grid, block, s->beam_smem, s->stream>>>(b);
+        if (aux) beam_kernel<false, true><<<grid, block, s->beam_smem, s->stream>>>(b);
         else beam_kernel<false, false><<<grid, block, s->beam_smem, s->stream>>>(b);
     }
     FN_CUDA(cudaGetLastError());
@@ -331,19 +340,34 @@ extern "C" int fn_step(fn_sim* s, float* states, const float* actions, float dt,
     a.map = s->map->dev; a.robot = robot_dev(s->robot, s->map); a.task = task_dev(s->task);
     a.n = s->n; a.dt = dt; a.states = states; a.actions = actions; a.reset_mask = reset_mask;
     a.out_collision = out_collision; a.out_goal_obs = out_goal_obs; a.out_reward = s->aux_reward;
-    a.d_prev = s->d_dprev; a.ep_step = s->d_epstep; a.poses = s->d_poses;
+    a.d_prev = s->d_dprev; a.ep_step = s->d_epstep; a.poses = s->d_poses; a.pose_inside = s->d_inside;
     a.ring = s->ring; a.ring_cap = s->ring_cap ? s->ring_cap : 1; a.ring_head = s->ring_head; a.ring_row = ring_row_floats(s);
     a.counters = s->d_counters;
+    cudaEvent_t e0 = nullptr, e1 = nullptr, e2 = nullptr;
+    if (s->prof) {
+        FN_CUDA(cudaEventCreate(&e0)); FN_CUDA(cudaEventCreate(&e1)); FN_CUDA(cudaEventCreate(&e2));
+        s->ev->push_back(e0); s->ev->push_back(e1); s->ev->push_back(e2); s->ev_kind->push_back(0);
+        FN_CUDA(cudaEventRecord(e0, s->stream));
+    }
     env_step_kernel<<<(s->n + 7) / 8, 256, 0, s->stream>>>(a);
     FN_CUDA(cudaGetLastError());
+    if (s->prof) FN_CUDA(cudaEventRecord(e1, s->stream));
     if (s->ring) s->ring_head = (s->ring_head + (unsigned long long)s->n) % s->ring_cap;
-    return launch_beams(s, nullptr, nullptr, out_ranges, s->ring_head);
+    int rc = launch_beams(s, nullptr, nullptr, out_ranges, s->ring_head);
+    if (s->prof && rc == FN_OK) FN_CUDA(cudaEventRecord(e2, s->stream));
+    return rc;
 }
 
 extern "C" int fn_reset(fn_sim* s, float* states, const uint8_t* mask, const uint64_t* seeds,
                         float* out_ranges, float* out_goal_obs) {
     if (!s || !states || !mask || !seeds || !out_ranges || !out_goal_obs)
         return fail(FN_ERR_INVALID_ARG, "fn_reset: NULL argument");
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    if (s->prof) {
+        FN_CUDA(cudaEventCreate(&e0)); FN_CUDA(cudaEventCreate(&e1));
+        s->ev->push_back(e0); s->ev->push_back(e1); s->ev_kind->push_back(1);
+        FN_CUDA(cudaEventRecord(e0, s->stream));
+    }
     compact_mask_kernel<<<1, 1024, 0, s->stream>>>(mask, s->n, s->d_list, s->d_count);
     FN_CUDA(cudaGetLastError());
     ResetArgs a;
@@ -351,21 +375,23 @@ extern "C" int fn_reset(fn_sim* s, float* states, const uint8_t* mask, const uin
     a.regions.rects = s->map->d_regions; a.regions.n = s->map->n_regions;
     a.n = s->n; a.states = states; a.list = s->d_list; a.count_dev = s->d_count;
     a.seeds = reinterpret_cast<const unsigned long long*>(seeds); a.out_goal_obs = out_goal_obs;
-    a.d_prev = s->d_dprev; a.ep_step = s->d_epstep; a.poses = s->d_poses;
+    a.d_prev = s->d_dprev; a.ep_step = s->d_epstep; a.poses = s->d_poses; a.pose_inside = s->d_inside;
     a.ring = s->ring; a.ring_cap = s->ring_cap ? s->ring_cap : 1; a.ring_head = s->ring_head; a.ring_row = ring_row_floats(s);
     a.counters = s->d_counters;
     int grid = (s->n + 7) / 8;
     if (grid > s->num_sms * 8) grid = s->num_sms * 8;
     reset_kernel<<<grid, 256, 0, s->stream>>>(a);
     FN_CUDA(cudaGetLastError());
-    return launch_beams(s, s->d_list, s->d_count, out_ranges, s->ring_head);
+    int rc = launch_beams(s, s->d_list, s->d_count, out_ranges, s->ring_head);
+    if (s->prof && rc == FN_OK) FN_CUDA(cudaEventRecord(e1, s->stream));
+    return rc;
 }
 
 extern "C" int fn_observe_all(fn_sim* s, const float* states, float* out_ranges, float* out_goal_obs) {
     if (!s || !states || !out_ranges) return fail(FN_ERR_INVALID_ARG, "fn_observe_all: NULL argument");
     PoseArgs a;
     a.map = s->map->dev; a.robot = robot_dev(s->robot, s->map); a.n = s->n; a.states = states;
-    a.out_goal_obs = out_goal_obs; a.poses = s->d_poses;
+    a.out_goal_obs = out_goal_obs; a.poses = s->d_poses; a.pose_inside = s->d_inside; a.pose_inside = s->d_inside;
     pose_from_state_kernel<<<(s->n + 255) / 256, 256, 0, s->stream>>>(a);
     FN_CUDA(cudaGetLastError());
     float* ring = s->ring;           // a test hook: never touches the ring
@@ -392,6 +418,35 @@ extern "C" int fn_get_counters(fn_sim* s, uint64_t* host_out) {
     if (!s || !host_out) return fail(FN_ERR_INVALID_ARG, "fn_get_counters: NULL argument");
     FN_CUDA(cudaMemcpyAsync(host_out, s->d_counters, kNCounters * sizeof(unsigned long long), cudaMemcpyDeviceToHost, s->stream));
     FN_CUDA(cudaStreamSynchronize(s->stream));
+    return FN_OK;
+}
+
+extern "C" int fn_sim_profile(fn_sim* s, int enable) {
+    if (!s) return fail(FN_ERR_INVALID_ARG, "fn_sim_profile: NULL sim");
+    if (!s->ev) { s->ev = new std::vector<cudaEvent_t>(); s->ev_kind = new std::vector<int>(); }
+    s->prof = enable != 0;
+    return FN_OK;
+}
+
+extern "C" int fn_sim_profile_read(fn_sim* s, double* ms_out, uint64_t* launches_out) {
+    if (!s || !ms_out || !launches_out) return fail(FN_ERR_INVALID_ARG, "fn_sim_profile_read: NULL argument");
+    for (int k = 0; k < 4; ++k) { ms_out[k] = 0.0; launches_out[k] = 0; }
+    if (!s->ev) return FN_OK;
+    FN_CUDA(cudaStreamSynchronize(s->stream));
+    size_t i = 0;
+    for (int kind : *s->ev_kind) {
+        float ms = 0.f;
+        if (kind == 0) {
+            FN_CUDA(cudaEventElapsedTime(&ms, (*s->ev)[i], (*s->ev)[i + 1])); ms_out[0] += ms; launches_out[0] += 1;
+            FN_CUDA(cudaEventElapsedTime(&ms, (*s->ev)[i + 1], (*s->ev)[i + 2])); ms_out[1] += ms; launches_out[1] += 1;
+            i += 3;
+        } else {
+            FN_CUDA(cudaEventElapsedTime(&ms, (*s->ev)[i], (*s->ev)[i + 1])); ms_out[2] += ms; launches_out[2] += 3;
+            i += 2;
+        }
+    }
+    for (cudaEvent_t e : *s->ev) cudaEventDestroy(e);
+    s->ev->clear(); s->ev_kind->clear();
     return FN_OK;
 }
 

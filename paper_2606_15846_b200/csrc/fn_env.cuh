@@ -90,20 +90,24 @@ struct EnvArgs {
     float* d_prev;
     int* ep_step;
     PoseD* poses;
+    int* pose_inside;
     float* ring;                 // or NULL
     unsigned long long ring_cap, ring_head;
     int ring_row;
     unsigned long long* counters;
 };
 
-__device__ __forceinline__ void write_pose(const MapDev& m, const RobotDev& rb, PoseD* out, float xf,
-                                           float yf, double c, double s) {
+__device__ __forceinline__ void write_pose(const MapDev& m, const RobotDev& rb, PoseD* out, int* inside,
+                                           float xf, float yf, double c, double s) {
     const double rho = (double)m.rho;
     PoseD p;
     p.ox = ((double)xf + c * rb.sx - s * rb.sy) / rho;
     p.oy = ((double)yf + s * rb.sx + c * rb.sy) / rho;
     p.c = c; p.s = s;
     *out = p;
+    // beams from here cannot leave the map: the beam kernel then skips its exit clipping
+    const double lo = rb.T + 1.0;
+    *inside = (p.ox >= lo && p.ox < (double)m.W - lo && p.oy >= lo && p.oy < (double)m.H - lo) ? 1 : 0;
 }
 
 __global__ void __launch_bounds__(256) env_step_kernel(EnvArgs a) {
@@ -161,7 +165,7 @@ __global__ void __launch_bounds__(256) env_step_kernel(EnvArgs a) {
         a.reset_mask[e] = done;
         a.d_prev[e] = d;
         a.ep_step[e] = es + 1;
-        write_pose(a.map, a.robot, &a.poses[e], xf, yf, c1, s1);
+        write_pose(a.map, a.robot, &a.poses[e], &a.pose_inside[e], xf, yf, c1, s1);
         if (a.ring) {
             // complete this step's row (its obs part was written when that observation was produced)
             const int B = a.robot.B;
@@ -230,6 +234,7 @@ struct ResetArgs {
     float* d_prev;
     int* ep_step;
     PoseD* poses;
+    int* pose_inside;
     float* ring;
     unsigned long long ring_cap, ring_head;
     int ring_row;
@@ -286,7 +291,7 @@ __global__ void __launch_bounds__(256) reset_kernel(ResetArgs a) {
             a.d_prev[e] = d;
             a.ep_step[e] = 0;
             if (a.out_goal_obs) { a.out_goal_obs[e] = d; a.out_goal_obs[n + e] = alpha; }
-            write_pose(a.map, a.robot, &a.poses[e], x, y, cp, sp);
+            write_pose(a.map, a.robot, &a.poses[e], &a.pose_inside[e], x, y, cp, sp);
             if (a.ring) {
                 float* row = a.ring + ((a.ring_head + (unsigned long long)e) % a.ring_cap) * (size_t)a.ring_row;
                 const int B = a.robot.B;
@@ -306,6 +311,7 @@ struct PoseArgs {
     const float* states;
     float* out_goal_obs;         // or NULL
     PoseD* poses;
+    int* pose_inside;
 };
 __global__ void __launch_bounds__(256) pose_from_state_kernel(PoseArgs a) {
     const int e = blockIdx.x * blockDim.x + threadIdx.x;
@@ -314,7 +320,7 @@ __global__ void __launch_bounds__(256) pose_from_state_kernel(PoseArgs a) {
     const float x = a.states[e], y = a.states[n + e], psi = a.states[2 * n + e];
     double s, c;
     sincos((double)psi, &s, &c);
-    write_pose(a.map, a.robot, &a.poses[e], x, y, c, s);
+    write_pose(a.map, a.robot, &a.poses[e], &a.pose_inside[e], x, y, c, s);
     if (a.out_goal_obs) {
         const double gdx = (double)a.states[6 * n + e] - (double)x, gdy = (double)a.states[7 * n + e] - (double)y;
         a.out_goal_obs[e] = (float)sqrt(gdx * gdx + gdy * gdy);

@@ -1,6 +1,6 @@
 // fn_peaks.cu -- roofline denominators measured in the same binary and run:
-//   kind 0: shared memory, conflict-free 64-bit windows read as two ld.shared.u32 per lane
-//   kind 1: shared memory, pseudo-random word per lane (bank conflicts as they fall)
+//   kind 0: shared memory, conflict-free 16-byte loads (512 contiguous bytes per warp instruction)
+//   kind 1: shared memory, pseudo-random 32-bit word per lane (bank conflicts as they fall)
 //   kind 2: L2-resident global memory, coalesced ld.global.nc 8-byte reads over a 32 MB buffer
 // Returns requested bytes per second (bytes = lanes x bytes per load, the same currency in which
 // the beam kernel's map traffic is counted).
@@ -21,17 +21,32 @@ __global__ void __launch_bounds__(1024, 2) smem_peak_kernel(int kind, unsigned* 
     __syncthreads();
     const uint32_t base = (uint32_t)__cvta_generic_to_shared(s_words);
     uint32_t acc = 0;
-    uint32_t idx = threadIdx.x * (kind == 0 ? 1u : 40503u);
-    for (int it = 0; it < kIters; ++it) {
+    if (kind == 0) {
+        // conflict-free: lane i of a warp reads the 16 bytes at 16*i (+ a per-warp, per-step offset),
+        // i.e. 512 contiguous bytes per warp instruction = 4 full 128-byte wavefronts
+        const uint32_t lane16 = base + (threadIdx.x & 31) * 16u;
+        for (int it = 0; it < kIters; ++it) {
+            const uint32_t a0 = lane16 + (((threadIdx.x >> 5) + it) & 7) * 4096u;   // moves every iteration
 #pragma unroll
-        for (int u = 0; u < kUnroll; ++u) {
-            const uint32_t w = (idx + (kind == 0 ? u * 1024u : acc * 0u + u * 7919u)) & (nwords - 2);
-            uint32_t a, b;
-            asm volatile("ld.shared.u32 %0, [%1];" : "=r"(a) : "r"(base + 4u * w));
-            asm volatile("ld.shared.u32 %0, [%1];" : "=r"(b) : "r"(base + 4u * w + 4u));
-            acc += a ^ b;
+            for (int u = 0; u < kUnroll; ++u) {
+                uint32_t x, y, z, w;
+                asm volatile("ld.volatile.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(x), "=r"(y), "=r"(z), "=r"(w)
+                             : "r"(a0 + u * 512u));
+                acc += x ^ y ^ z ^ w;
+            }
         }
-        idx = kind == 0 ? idx + 32u : idx * 1664525u + 1013904223u;
+    } else {
+        // one pseudo-random 32-bit word per lane per load (bank conflicts as they fall)
+        uint32_t idx = threadIdx.x * 40503u + 12345u;
+        for (int it = 0; it < kIters; ++it) {
+#pragma unroll
+            for (int u = 0; u < kUnroll; ++u) {
+                uint32_t x;
+                asm volatile("ld.volatile.shared.u32 %0, [%1];" : "=r"(x) : "r"(base + ((idx >> 8) & (nwords - 1)) * 4u));
+                acc += x;
+                idx = idx * 1664525u + 1013904223u;
+            }
+        }
     }
     if (acc == 0x12345678u) *sink = acc;
 }
@@ -78,7 +93,7 @@ extern "C" int fn_measure_peak(int kind, void* stream_v, double* out) {
             if (cudaEventSynchronize(e1) != cudaSuccess) { rc = FN_ERR_CUDA; break; }
             float ms = 0.f;
             cudaEventElapsedTime(&ms, e0, e1);
-            const double bytes = (double)grid * 1024.0 * kIters * kUnroll * 8.0;
+            const double bytes = (double)grid * 1024.0 * kIters * kUnroll * (kind == 0 ? 16.0 : 4.0);
             if (rep > 0 && bytes / (ms * 1e-3) > best) best = bytes / (ms * 1e-3);
         }
     } else {

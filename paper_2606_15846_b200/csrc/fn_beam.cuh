@@ -13,6 +13,7 @@
 //   * beams running towards lower u read the window downwards and use clz instead of ctz.
 #pragma once
 #include "fn_common.cuh"
+#include <type_traits>
 
 namespace fn {
 
@@ -113,6 +114,87 @@ __device__ __forceinline__ bool walk_lines(typename MS::addr_t wbase, const type
     }
 }
 
+// Hot loop in PTX for the shared-memory map and slopes M < 31 cells per line (span <= 32 cells, so one
+// window per line always suffices).  Per line: word address (shr, mad), two ld.shared, funnel shift,
+// (brev,) bfind.shiftamt = k, len = c1 - c0, hit = (k <= len) fused with the end-of-lines test into one
+// predicate and one branch, then the 64-bit fixed-point add and the line-pointer add: 14 (forward) /
+// 13 (backward) instructions.  Unrolled twice with the roles of the (c0, hi(Q)) registers swapped so
+// that "c0 := c1" costs nothing.  Returns true when the first occupied cell of the current line's
+// window lies inside the beam's span (k = its offset from c0); false when the lines are exhausted.
+template <bool kFwd>
+__device__ __forceinline__ bool fast_lines_smem(uint32_t& wbase, const uint32_t wend, const int lstep4,
+                                                uint32_t& qlo, int& qhi, const uint32_t mlo, const int mhi,
+                                                int& c0, int& k) {
+    int found, c0o, qho;
+#define FN_LINE(RC, RQ, EXIT)                                              \
+    "shr.s32 j, " RC ", 5;\n\t"                                            \
+    "mad.lo.s32 a, j, %12, %0;\n\t"                                        \
+    "ld.shared.u32 L, [a];\n\t"                                            \
+    "ld.shared.u32 H, [a+4];\n\t"                                          \
+    FN_SHIFT(RC)                                                           \
+    "bfind.shiftamt.u32 %4, x;\n\t"                                        \
+    "sub.s32 len, " RQ ", " RC ";\n\t"                                     \
+    "setp.le.u32 ph, %4, len;\n\t"                                         \
+    "setp.eq.or.u32 pe, %0, %8, ph;\n\t"                                   \
+    "@pe bra " EXIT ";\n\t"                                                \
+    "add.cc.u32 %1, %1, %10;\n\t"                                          \
+    "addc.s32 " RC ", " RQ ", %11;\n\t"                                    \
+    "add.s32 %0, %0, %9;\n\t"
+    if (kFwd) {
+#define FN_SHIFT(RC) "shf.r.wrap.b32 x, L, H, " RC ";\n\tbrev.b32 x, x;\n\t"
+        asm volatile(
+            "{\n\t"
+            ".reg .pred ph, pe;\n\t"
+            ".reg .b32 j, a, L, H, x, len, rc, rq;\n\t"
+            "mov.b32 rc, %2;\n\t"
+            "mov.b32 rq, %3;\n\t"
+            "FN_LA:\n\t" FN_LINE("rc", "rq", "FN_XA")
+            FN_LINE("rq", "rc", "FN_XB")
+            "bra FN_LA;\n\t"
+            "FN_XA:\n\t"
+            "mov.b32 %6, rc;\n\t"
+            "mov.b32 %7, rq;\n\t"
+            "bra FN_END;\n\t"
+            "FN_XB:\n\t"
+            "mov.b32 %6, rq;\n\t"
+            "mov.b32 %7, rc;\n\t"
+            "FN_END:\n\t"
+            "selp.s32 %5, 1, 0, ph;\n\t"
+            "}"
+            : "+r"(wbase), "+r"(qlo), "+r"(c0), "+r"(qhi), "=r"(k), "=r"(found), "=r"(c0o), "=r"(qho)
+            : "r"(wend), "r"(lstep4), "r"(mlo), "r"(mhi), "n"(4));
+#undef FN_SHIFT
+    } else {
+#define FN_SHIFT(RC) "shf.l.wrap.b32 x, L, H, " RC ";\n\t"
+        asm volatile(
+            "{\n\t"
+            ".reg .pred ph, pe;\n\t"
+            ".reg .b32 j, a, L, H, x, len, rc, rq;\n\t"
+            "mov.b32 rc, %2;\n\t"
+            "mov.b32 rq, %3;\n\t"
+            "FN_LA:\n\t" FN_LINE("rc", "rq", "FN_XA")
+            FN_LINE("rq", "rc", "FN_XB")
+            "bra FN_LA;\n\t"
+            "FN_XA:\n\t"
+            "mov.b32 %6, rc;\n\t"
+            "mov.b32 %7, rq;\n\t"
+            "bra FN_END;\n\t"
+            "FN_XB:\n\t"
+            "mov.b32 %6, rq;\n\t"
+            "mov.b32 %7, rc;\n\t"
+            "FN_END:\n\t"
+            "selp.s32 %5, 1, 0, ph;\n\t"
+            "}"
+            : "+r"(wbase), "+r"(qlo), "+r"(c0), "+r"(qhi), "=r"(k), "=r"(found), "=r"(c0o), "=r"(qho)
+            : "r"(wend), "r"(lstep4), "r"(mlo), "r"(mhi), "n"(-4));
+#undef FN_SHIFT
+    }
+#undef FN_LINE
+    c0 = c0o;
+    qhi = qho;
+    return found != 0;
+}
+
 // One beam.  (ox, oy) origin in cells, (dx, dy) unit direction, T = max range in cells; `inside` = the
 // r_max disc around the origin lies inside the map (no exit clipping needed).
 // Returns range in metres; *hit = linear cell index, -1 (no hit) or -2 (left the map).
@@ -172,8 +254,25 @@ __device__ __forceinline__ float cast_beam(const BeamMap<MS>& bm, const double o
     int cq = 0;
     long long qe = 0;
     typename MS::addr_t wfound = wbase;
-    const bool found = fu ? walk_lines<MS, true, kAux>(wbase, wend, lstep4, Qn, Mf, hi32(Q0), cend, cq, qe, wfound, words)
-                          : walk_lines<MS, false, kAux>(wbase, wend, lstep4, Qn, Mf, hi32(Q0), cend, cq, qe, wfound, words);
+    bool found;
+    if constexpr (std::is_same<MS, SmemSpace>::value && !kAux) {
+        if (hi32(Mf) < 31) {                                      // one window per line always suffices
+            uint32_t wb = wbase, qlo = (uint32_t)Qn;
+            int qhi = hi32(Qn), c0 = hi32(Q0), k;
+            found = fu ? fast_lines_smem<true>(wb, wend, lstep4, qlo, qhi, (uint32_t)Mf, hi32(Mf), c0, k)
+                       : fast_lines_smem<false>(wb, wend, lstep4, qlo, qhi, (uint32_t)Mf, hi32(Mf), c0, k);
+            cq = c0 + k;
+            const long long Qcur = ((long long)qhi << 32) | (long long)qlo;
+            qe = (k == 0 && wb != wbase) ? Qcur - Mf : ((long long)cq << 32);
+            wfound = wb;
+        } else {
+            found = fu ? walk_lines<MS, true, kAux>(wbase, wend, lstep4, Qn, Mf, hi32(Q0), cend, cq, qe, wfound, words)
+                       : walk_lines<MS, false, kAux>(wbase, wend, lstep4, Qn, Mf, hi32(Q0), cend, cq, qe, wfound, words);
+        }
+    } else {
+        found = fu ? walk_lines<MS, true, kAux>(wbase, wend, lstep4, Qn, Mf, hi32(Q0), cend, cq, qe, wfound, words)
+                   : walk_lines<MS, false, kAux>(wbase, wend, lstep4, Qn, Mf, hi32(Q0), cend, cq, qe, wfound, words);
+    }
     if (found && qe < Qend) {
         if (kAux) {
             const int cu = fu ? cq : Wq - 1 - cq;

@@ -177,6 +177,17 @@ def run_parity(wl, steps, n=None, subset=None, seed=0, forced=None, check_every=
             assert np.array_equal(ge, ep) and np.array_equal(gd, d_prev)
             check_observation(wl, rep, x[sel], y[sel], psi[sel], buf.ranges.cpu().numpy()[sel], buf.hit.cpu().numpy()[sel],
                               sel, f"step {t}")
+            # the production (non-instrumented) beam kernel must give bit-identical ranges
+            s.bind_aux(None, buf.reward)
+            fast = torch.empty_like(buf.ranges)
+            s.observe_all(buf.states, fast)
+            torch.cuda.synchronize()
+            s.bind_aux(buf.hit, buf.reward)
+            if not torch.equal(fast, buf.ranges):
+                bad = (fast != buf.ranges).nonzero()[0].tolist()
+                raise AssertionError(f"step {t}: fast beam kernel differs from instrumented one at env {bad[0]} beam {bad[1]}: "
+                                     f"{fast[bad[0], bad[1]].item()!r} vs {buf.ranges[bad[0], bad[1]].item()!r}")
+            rep.add("fast_path_checks", n * B)
         if done.any():
             if check:
                 do_reset(done, seeds_np[t + 1], f"step {t} reset")

@@ -272,8 +272,7 @@ def run_ours(args):
         a_ray, windows = algorithmic_bytes_per_beam(wl, st_np)
         smem_peak = fn.measure_peak(0)
         l2_peak = fn.measure_peak(2)
-        use_smem = (wl.occ.shape[0] * ((wl.occ.shape[1] + 31) // 32 + 2) + wl.occ.shape[1] * ((wl.occ.shape[0] + 31) // 32 + 2)) * 4 \
-            + B * 16 <= 227 * 1024
+        use_smem = sim.beam_config()["smem"]
         peak = smem_peak if use_smem else l2_peak
         beam_s = beam_ms * 1e-3 / max(1, beam_launches)
         achieved = a_ray * n * B / beam_s

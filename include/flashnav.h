@@ -44,7 +44,8 @@ typedef struct fn_sim fn_sim;
 
 /* ---- map ("the environment batch shares an occupancy bitmap") -------------------
  * bitmap_host: [H*W] row-major bytes, != 0 occupied.  The library bit-packs it (1 bit per cell) twice:
- * row-packed (bits along columns) and column-packed (bits along rows), and uploads both.
+ * row-packed (bits along columns) and column-packed (bits along rows), each with a frame of occupied
+ * cells around it ("outside the map is occupied"), and uploads both.
  * Errors: NULL pointers, H/W <= 0 or > 32768, resolution not finite or <= 0 -> FN_ERR_INVALID_ARG. */
 int fn_map_create(const uint8_t* bitmap_host, int H, int W, float resolution_m, fn_map** out);
 
@@ -124,6 +125,10 @@ int fn_sim_episode_state(fn_sim* sim, float* d_prev_host, int32_t* ep_step_host)
  * fn_step, whole fn_reset path (compaction + reset + beam kernels), reserved}. */
 int fn_sim_profile(fn_sim* sim, int enable);
 int fn_sim_profile_read(fn_sim* sim, double* ms_out, uint64_t* launches_out);
+
+/* ---- launch configuration of the beam kernel chosen at fn_sim_create (for reports): cfg_out[4] =
+ * {map staged in shared memory (1) or read through L1/L2 (0), grid size, CTA size, dynamic shared bytes}. */
+int fn_sim_beam_config(const fn_sim* sim, int* cfg_out);
 
 /* ---- end-to-end convenience: host buffers in, host buffers out -----------------------------------------
  * Copies states/actions/mask (and seeds) host->device, runs fn_step (+ fn_reset of the done envs when

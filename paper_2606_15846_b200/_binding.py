@@ -19,7 +19,7 @@ EXPORTED_SYMBOLS = (
     "fn_map_create", "fn_map_set_regions", "fn_map_destroy", "fn_robot_create", "fn_robot_set_sensor",
     "fn_robot_destroy", "fn_task_default", "fn_sim_create", "fn_sim_destroy", "fn_step", "fn_reset",
     "fn_sim_bind_aux", "fn_ring_attach", "fn_observe_all", "fn_get_counters", "fn_sim_count_words",
-    "fn_sim_episode_state", "fn_sim_profile", "fn_sim_profile_read", "fn_step_host", "fn_measure_peak", "fn_last_error", "fn_version")
+    "fn_sim_episode_state", "fn_sim_beam_config", "fn_sim_profile", "fn_sim_profile_read", "fn_step_host", "fn_measure_peak", "fn_last_error", "fn_version")
 
 
 class FlashNavError(RuntimeError):
@@ -63,6 +63,7 @@ def load_library():
         "fn_get_counters": [vp, vp],
         "fn_sim_count_words": [vp, i32],
         "fn_sim_episode_state": [vp, vp, vp],
+        "fn_sim_beam_config": [vp, vp],
         "fn_sim_profile": [vp, i32],
         "fn_sim_profile_read": [vp, vp, vp],
         "fn_step_host": [vp, vp, vp, f32, vp, vp, vp, vp, vp],
@@ -252,6 +253,11 @@ class Sim:
         e = np.empty(self.n, np.int32)
         _check(load_library().fn_sim_episode_state(self._h, _np_ptr(d), _np_ptr(e)), "fn_sim_episode_state")
         return d, e
+
+    def beam_config(self) -> dict:
+        cfg = np.zeros(4, np.int32)
+        _check(load_library().fn_sim_beam_config(self._h, _np_ptr(cfg)), "fn_sim_beam_config")
+        return {"smem": bool(cfg[0]), "grid": int(cfg[1]), "block": int(cfg[2]), "smem_bytes": int(cfg[3])}
 
     def step_host(self, states, actions, dt, reset_mask, seeds, out_ranges, out_collision, out_goal_obs):
         """End to end with HOST buffers (numpy arrays or pinned CPU tensors); copies inside the call."""

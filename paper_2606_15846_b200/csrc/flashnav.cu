@@ -62,8 +62,7 @@ struct fn_sim {
     cudaStream_t stream;
     int num_sms;
     // device state owned by the sim
-    PoseD* d_poses;
-    int* d_inside;
+    BeamPose* d_poses;
     int* d_list;
     int* d_count;
     float* d_dprev;
@@ -73,7 +72,8 @@ struct fn_sim {
     int32_t* aux_hit;
     float* aux_reward;
     float* ring;
-    unsigned long long ring_cap, ring_head;
+    unsigned long long ring_cap;
+    unsigned long long* d_ring_head;   // device: slot of env 0's pending ring row
     int count_words;
     // beam-kernel launch configuration
     bool use_smem;
@@ -103,17 +103,35 @@ extern "C" int fn_map_create(const uint8_t* bitmap, int H, int W, float res, fn_
     if (!bitmap || !out) return fail(FN_ERR_INVALID_ARG, "fn_map_create: NULL argument");
     if (H <= 0 || W <= 0 || H > 32768 || W > 32768) return fail(FN_ERR_INVALID_ARG, "fn_map_create: H, W must be in 1..32768");
     if (!std::isfinite(res) || res <= 0.0f) return fail(FN_ERR_INVALID_ARG, "fn_map_create: resolution must be finite and > 0");
+    // Layout (fn_common.cuh): per copy L + 4 lines of nw + 4 words; frame, guards, pads and the bits
+    // beyond a line's length are ones ("outside the map is occupied").
     const int nwR = (W + 31) / 32, nwC = (H + 31) / 32;
-    const int sR = nwR + 2, sC = nwC + 2;
-    const size_t rowWords = (size_t)H * sR, colWords = (size_t)W * sC;
+    const int sR = nwR + 4, sC = nwC + 4;
+    const size_t rowWords = (size_t)(H + 2 * kLineGuard) * sR, colWords = (size_t)(W + 2 * kLineGuard) * sC;
     const size_t total = (rowWords + colWords + 3) / 4 * 4;
-    std::vector<uint32_t> words(total, 0u);
-    for (int i = 0; i < H; ++i)
-        for (int j = 0; j < W; ++j)
-            if (bitmap[(size_t)i * W + j]) {
-                words[(size_t)i * sR + 1 + (j >> 5)] |= 1u << (j & 31);
-                words[rowWords + (size_t)j * sC + 1 + (i >> 5)] |= 1u << (i & 31);
+    std::vector<uint32_t> words(total, 0xffffffffu);
+    for (int i = 0; i < H; ++i) {
+        uint32_t* line = &words[(size_t)(i + kLineGuard) * sR + (kCellShift >> 5)];
+        for (int k = 0; k < nwR; ++k) {
+            uint32_t w = 0;
+            for (int b = 0; b < 32; ++b) {
+                const int j = 32 * k + b;
+                if (j >= W || bitmap[(size_t)i * W + j]) w |= 1u << b;
             }
+            line[k] = w;
+        }
+    }
+    for (int j = 0; j < W; ++j) {
+        uint32_t* line = &words[rowWords + (size_t)(j + kLineGuard) * sC + (kCellShift >> 5)];
+        for (int k = 0; k < nwC; ++k) {
+            uint32_t w = 0;
+            for (int b = 0; b < 32; ++b) {
+                const int i = 32 * k + b;
+                if (i >= H || bitmap[(size_t)i * W + j]) w |= 1u << b;
+            }
+            line[k] = w;
+        }
+    }
     fn_map* m = new (std::nothrow) fn_map();
     if (!m) return fail(FN_ERR_OOM, "fn_map_create: host allocation failed");
     m->H = H; m->W = W; m->res = res; m->n_words = total; m->n_regions = 0; m->d_regions = nullptr; m->d_words = nullptr;
@@ -260,9 +278,9 @@ extern "C" int fn_sim_create(const fn_map* map, const fn_robot* robot, int n, co
     cudaError_t e = cudaGetDevice(&dev);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&s->num_sms, cudaDevAttrMultiProcessorCount, dev);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
-    if (e == cudaSuccess) e = cudaMalloc(&s->d_poses, (size_t)n * sizeof(PoseD));
-    if (e == cudaSuccess) e = cudaMalloc(&s->d_inside, (size_t)n * sizeof(int));
-    if (e == cudaSuccess) e = cudaMemsetAsync(s->d_inside, 0, (size_t)n * sizeof(int), s->stream);
+    if (e == cudaSuccess) e = cudaMalloc(&s->d_poses, (size_t)n * sizeof(BeamPose));
+    if (e == cudaSuccess) e = cudaMalloc(&s->d_ring_head, sizeof(unsigned long long));
+    if (e == cudaSuccess) e = cudaMemsetAsync(s->d_ring_head, 0, sizeof(unsigned long long), s->stream);
     if (e == cudaSuccess) e = cudaMalloc(&s->d_list, (size_t)n * sizeof(int));
     if (e == cudaSuccess) e = cudaMalloc(&s->d_count, sizeof(int));
     if (e == cudaSuccess) e = cudaMalloc(&s->d_dprev, (size_t)n * sizeof(float));
@@ -271,7 +289,7 @@ extern "C" int fn_sim_create(const fn_map* map, const fn_robot* robot, int n, co
     if (e == cudaSuccess) e = cudaMemsetAsync(s->d_dprev, 0, (size_t)n * sizeof(float), s->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(s->d_epstep, 0, (size_t)n * sizeof(int), s->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(s->d_counters, 0, kNCounters * sizeof(unsigned long long), s->stream);
-    if (e == cudaSuccess) e = cudaMemsetAsync(s->d_poses, 0, (size_t)n * sizeof(PoseD), s->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(s->d_poses, 0xff, (size_t)n * sizeof(BeamPose), s->stream);
     if (e == cudaSuccess) {
         // stage the packed map in shared memory when both copies + the beam table fit, else read via L2
         const size_t tab = (size_t)robot->B * sizeof(double2);
@@ -301,7 +319,7 @@ extern "C" int fn_sim_create(const fn_map* map, const fn_robot* robot, int n, co
 
 extern "C" int fn_sim_destroy(fn_sim* s) {
     if (!s) return FN_OK;
-    cudaFree(s->d_poses); cudaFree(s->d_inside); cudaFree(s->d_list); cudaFree(s->d_count); cudaFree(s->d_dprev);
+    cudaFree(s->d_poses); cudaFree(s->d_ring_head); cudaFree(s->d_list); cudaFree(s->d_count); cudaFree(s->d_dprev);
     cudaFree(s->d_epstep); cudaFree(s->d_counters);
     if (s->ev) { for (cudaEvent_t e : *s->ev) cudaEventDestroy(e); delete s->ev; delete s->ev_kind; }
     cudaFree(s->stg_states); cudaFree(s->stg_actions); cudaFree(s->stg_ranges); cudaFree(s->stg_gobs);
@@ -312,11 +330,11 @@ extern "C" int fn_sim_destroy(fn_sim* s) {
 
 static int ring_row_floats(const fn_sim* s) { return s->robot->B + 5 + (s->robot->drive == FN_DRIVE_DIFF ? 2 : 3) + 2; }
 
-static int launch_beams(fn_sim* s, const int* list, const int* count_dev, float* out_ranges, unsigned long long ring_head) {
+static int launch_beams(fn_sim* s, const int* list, const int* count_dev, float* out_ranges) {
     BeamArgs b;
-    b.map = s->map->dev; b.robot = robot_dev(s->robot, s->map); b.poses = s->d_poses; b.pose_inside = s->d_inside; b.count_words = s->count_words;
+    b.map = s->map->dev; b.robot = robot_dev(s->robot, s->map); b.poses = s->d_poses; b.count_words = s->count_words;
     b.list = list; b.count_dev = count_dev; b.n_all = s->n; b.out_ranges = out_ranges; b.out_hit = s->aux_hit;
-    b.ring_obs = s->ring; b.ring_cap = s->ring_cap ? s->ring_cap : 1; b.ring_head = ring_head; b.ring_row = ring_row_floats(s);
+    b.ring_obs = s->ring; b.ring_cap = s->ring_cap ? s->ring_cap : 1; b.ring_head = s->d_ring_head; b.ring_row = ring_row_floats(s);
     b.counters = s->d_counters;
     const dim3 grid(s->beam_grid), block(512);
     const bool aux = s->count_words || s->aux_hit;
@@ -340,8 +358,8 @@ extern "C" int fn_step(fn_sim* s, float* states, const float* actions, float dt,
     a.map = s->map->dev; a.robot = robot_dev(s->robot, s->map); a.task = task_dev(s->task);
     a.n = s->n; a.dt = dt; a.states = states; a.actions = actions; a.reset_mask = reset_mask;
     a.out_collision = out_collision; a.out_goal_obs = out_goal_obs; a.out_reward = s->aux_reward;
-    a.d_prev = s->d_dprev; a.ep_step = s->d_epstep; a.poses = s->d_poses; a.pose_inside = s->d_inside;
-    a.ring = s->ring; a.ring_cap = s->ring_cap ? s->ring_cap : 1; a.ring_head = s->ring_head; a.ring_row = ring_row_floats(s);
+    a.d_prev = s->d_dprev; a.ep_step = s->d_epstep; a.poses = s->d_poses;
+    a.ring = s->ring; a.ring_cap = s->ring_cap ? s->ring_cap : 1; a.ring_head_dev = s->d_ring_head; a.ring_row = ring_row_floats(s);
     a.counters = s->d_counters;
     cudaEvent_t e0 = nullptr, e1 = nullptr, e2 = nullptr;
     if (s->prof) {
@@ -349,11 +367,14 @@ extern "C" int fn_step(fn_sim* s, float* states, const float* actions, float dt,
         s->ev->push_back(e0); s->ev->push_back(e1); s->ev->push_back(e2); s->ev_kind->push_back(0);
         FN_CUDA(cudaEventRecord(e0, s->stream));
     }
-    env_step_kernel<<<(s->n + 7) / 8, 256, 0, s->stream>>>(a);
+    env_step_kernel<<<(s->n + kEnvBlock - 1) / kEnvBlock, kEnvBlock, 0, s->stream>>>(a);
     FN_CUDA(cudaGetLastError());
     if (s->prof) FN_CUDA(cudaEventRecord(e1, s->stream));
-    if (s->ring) s->ring_head = (s->ring_head + (unsigned long long)s->n) % s->ring_cap;
-    int rc = launch_beams(s, nullptr, nullptr, out_ranges, s->ring_head);
+    if (s->ring) {
+        ring_advance_kernel<<<1, 1, 0, s->stream>>>(s->d_ring_head, (unsigned long long)s->n, s->ring_cap);
+        FN_CUDA(cudaGetLastError());
+    }
+    int rc = launch_beams(s, nullptr, nullptr, out_ranges);
     if (s->prof && rc == FN_OK) FN_CUDA(cudaEventRecord(e2, s->stream));
     return rc;
 }
@@ -375,14 +396,14 @@ extern "C" int fn_reset(fn_sim* s, float* states, const uint8_t* mask, const uin
     a.regions.rects = s->map->d_regions; a.regions.n = s->map->n_regions;
     a.n = s->n; a.states = states; a.list = s->d_list; a.count_dev = s->d_count;
     a.seeds = reinterpret_cast<const unsigned long long*>(seeds); a.out_goal_obs = out_goal_obs;
-    a.d_prev = s->d_dprev; a.ep_step = s->d_epstep; a.poses = s->d_poses; a.pose_inside = s->d_inside;
-    a.ring = s->ring; a.ring_cap = s->ring_cap ? s->ring_cap : 1; a.ring_head = s->ring_head; a.ring_row = ring_row_floats(s);
+    a.d_prev = s->d_dprev; a.ep_step = s->d_epstep; a.poses = s->d_poses;
+    a.ring = s->ring; a.ring_cap = s->ring_cap ? s->ring_cap : 1; a.ring_head_dev = s->d_ring_head; a.ring_row = ring_row_floats(s);
     a.counters = s->d_counters;
-    int grid = (s->n + 7) / 8;
+    int grid = (s->n + kResetWarps - 1) / kResetWarps;
     if (grid > s->num_sms * 8) grid = s->num_sms * 8;
-    reset_kernel<<<grid, 256, 0, s->stream>>>(a);
+    reset_kernel<<<grid, kResetWarps * 32, 0, s->stream>>>(a);
     FN_CUDA(cudaGetLastError());
-    int rc = launch_beams(s, s->d_list, s->d_count, out_ranges, s->ring_head);
+    int rc = launch_beams(s, s->d_list, s->d_count, out_ranges);
     if (s->prof && rc == FN_OK) FN_CUDA(cudaEventRecord(e1, s->stream));
     return rc;
 }
@@ -391,12 +412,12 @@ extern "C" int fn_observe_all(fn_sim* s, const float* states, float* out_ranges,
     if (!s || !states || !out_ranges) return fail(FN_ERR_INVALID_ARG, "fn_observe_all: NULL argument");
     PoseArgs a;
     a.map = s->map->dev; a.robot = robot_dev(s->robot, s->map); a.n = s->n; a.states = states;
-    a.out_goal_obs = out_goal_obs; a.poses = s->d_poses; a.pose_inside = s->d_inside; a.pose_inside = s->d_inside;
+    a.out_goal_obs = out_goal_obs; a.poses = s->d_poses;
     pose_from_state_kernel<<<(s->n + 255) / 256, 256, 0, s->stream>>>(a);
     FN_CUDA(cudaGetLastError());
     float* ring = s->ring;           // a test hook: never touches the ring
     s->ring = nullptr;
-    int st = launch_beams(s, nullptr, nullptr, out_ranges, 0);
+    int st = launch_beams(s, nullptr, nullptr, out_ranges);
     s->ring = ring;
     return st;
 }
@@ -410,7 +431,8 @@ extern "C" int fn_sim_bind_aux(fn_sim* s, int32_t* hit, float* reward) {
 extern "C" int fn_ring_attach(fn_sim* s, float* ring, uint64_t cap) {
     if (!s) return fail(FN_ERR_INVALID_ARG, "fn_ring_attach: NULL sim");
     if (ring && cap < (uint64_t)s->n) return fail(FN_ERR_INVALID_ARG, "fn_ring_attach: capacity must be >= n_envs");
-    s->ring = ring; s->ring_cap = ring ? cap : 0; s->ring_head = 0;
+    s->ring = ring; s->ring_cap = ring ? cap : 0;
+    FN_CUDA(cudaMemsetAsync(s->d_ring_head, 0, sizeof(unsigned long long), s->stream));
     return FN_OK;
 }
 
@@ -447,6 +469,12 @@ extern "C" int fn_sim_profile_read(fn_sim* s, double* ms_out, uint64_t* launches
     }
     for (cudaEvent_t e : *s->ev) cudaEventDestroy(e);
     s->ev->clear(); s->ev_kind->clear();
+    return FN_OK;
+}
+
+extern "C" int fn_sim_beam_config(const fn_sim* s, int* cfg) {
+    if (!s || !cfg) return fail(FN_ERR_INVALID_ARG, "fn_sim_beam_config: NULL argument");
+    cfg[0] = s->use_smem ? 1 : 0; cfg[1] = s->beam_grid; cfg[2] = 512; cfg[3] = (int)s->beam_smem;
     return FN_OK;
 }
 

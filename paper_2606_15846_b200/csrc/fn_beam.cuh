@@ -1,16 +1,27 @@
 // fn_beam.cuh -- range sensing: exact first-hit distance of each beam on the bit-packed map.
 //
 // Operation: r = rho * inf{t : cell(o + t d) occupied}, capped at
-// r_max, no hit => r_max.  The traversal is an exact grid walk organised by LINES instead of cells:
+// r_max, no hit => r_max; everything outside the map is occupied.
+//
+// The traversal is an exact grid walk organised by LINES instead of cells:
 //   * the beam's dominant axis is "u", the other "w"; the packing whose bits run along u is used
 //     (row-packed for |dx| >= |dy|, column-packed otherwise), so the beam stays in one line for
 //     M = |du/dw| >= 1 cells before it crosses into the next line;
-//   * per line the beam covers the cell span [floor(U_k), floor(U_{k+1})], U_{k+1} = U_k + M, tracked
-//     in 32.32 fixed point (exact integer adds; error < 2^-32 * lines, far below the 1e-5 cell margin);
-//   * the span's occupancy bits are read as one 64-bit window (two aligned 32-bit loads), funnel-
-//     shifted so that bit 0 is the span's first cell, and the first occupied cell is found with one
-//     count-leading/trailing-zeros -- no per-cell stepping;
-//   * beams running towards lower u read the window downwards and use clz instead of ctz.
+//   * line k is left at U_{k+1} = U_1 + k (+-M).  The crossing coordinate is carried as a double
+//     D = 2^20 + 64 + U (+1 for beams running towards higher u): in [2^20, 2^21) a double is a 20.32
+//     fixed-point number (ulp 2^-32 cell, far below the 1e-5 cell near-tie margin), its high word holds
+//     floor(U) in the low bits, and "U += M" is ONE DADD on the otherwise idle fp64 pipe;
+//   * per line ONE 64-bit window (two aligned 32-bit loads) is funnel-shifted by the low 5 bits of that
+//     high word so that it ends (forward beams) or starts (backward beams) at the line's exit cell, and
+//     ANDed with a per-beam constant mask of floor(M) + 2 bits that covers the cells the beam can have
+//     visited in the line: non-zero = candidate hit.  Forward and backward beams run the SAME
+//     instructions (the differences are per-lane constants), so a warp never serialises on direction;
+//   * on a candidate the exact span [entry cell, exit cell] is rebuilt, the first occupied cell in
+//     travel order is found with one clz/ctz, and the entry distance follows from the crossing
+//     coordinates; a candidate outside the exact span (one extra cell behind the entry) resumes the walk;
+//   * the map border is stored as occupied cells (fn_common.cuh), so leaving the map is an ordinary hit
+//     (index -2) and the hot loop has no clipping at all.
+// Beams within 1.9 deg of an axis (M >= 30.5, spans longer than one window) take a plain side path.
 #pragma once
 #include "fn_common.cuh"
 #include <type_traits>
@@ -18,287 +29,264 @@
 namespace fn {
 
 // Address spaces for the packed map: staged in shared memory, or read through L1/L2.
+// `base` addresses the start of the row copy MINUS the constant that the exponent bits of D's high
+// word add to the word offset (kMagicHi >> 5 words), so the hot loop never masks them off.
 struct SmemSpace {
     using addr_t = uint32_t;                                     // shared-window byte address
     static __device__ __forceinline__ uint32_t ld(addr_t a) {
         uint32_t v;
-        asm("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a));
+        asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a));
+        return v;
+    }
+    static __device__ __forceinline__ uint32_t ld4(addr_t a) {
+        uint32_t v;
+        asm volatile("ld.shared.u32 %0, [%1+4];" : "=r"(v) : "r"(a));
         return v;
     }
     static __device__ __forceinline__ addr_t addb(addr_t a, int bytes) { return a + (uint32_t)bytes; }
-    static __device__ __forceinline__ int diffb(addr_t a, addr_t b) { return (int)(a - b); }
+    static __device__ __forceinline__ long long diffb(addr_t a, addr_t b) { return (long long)(int)(a - b); }
 };
 struct GlobalSpace {
-    using addr_t = const uint32_t*;
-    static __device__ __forceinline__ uint32_t ld(addr_t a) { return __ldg(a); }
-    static __device__ __forceinline__ addr_t addb(addr_t a, int bytes) {
-        return reinterpret_cast<addr_t>(reinterpret_cast<const char*>(a) + bytes);
+    using addr_t = unsigned long long;                           // global byte address
+    static __device__ __forceinline__ uint32_t ld(addr_t a) {
+        uint32_t v;
+        asm volatile("ld.global.nc.u32 %0, [%1];" : "=r"(v) : "l"(a));
+        return v;
     }
-    static __device__ __forceinline__ int diffb(addr_t a, addr_t b) {
-        return (int)(reinterpret_cast<const char*>(a) - reinterpret_cast<const char*>(b));
+    static __device__ __forceinline__ uint32_t ld4(addr_t a) {
+        uint32_t v;
+        asm volatile("ld.global.nc.u32 %0, [%1+4];" : "=r"(v) : "l"(a));
+        return v;
     }
+    static __device__ __forceinline__ addr_t addb(addr_t a, int bytes) { return a + (unsigned long long)(long long)bytes; }
+    static __device__ __forceinline__ long long diffb(addr_t a, addr_t b) { return (long long)(a - b); }
 };
 
 template <class MS>
 struct BeamMap {
-    typename MS::addr_t row, col;
-    int H, W, nwR, nwC, strideR, strideC;
+    typename MS::addr_t base;        // start of the row copy (true address)
+    int H, W, stride4R, stride4C;    // line strides in bytes
 };
 
-constexpr double kFix = 4294967296.0;          // 2^32
-constexpr double kMaxSlope = 1048576.0;        // 2^20 cells per line: beyond any map
+constexpr unsigned kExpOff = (kMagicHi >> 5) << 2;               // byte offset added by D's exponent bits
+constexpr double kSlowSlope = 30.5;                              // spans of floor(M) + 2 <= 32 cells fit one window
 
-__device__ __forceinline__ int bfind32(uint32_t x) {            // msb position, -1 if x == 0 (SASS FLO.U32)
-    int r;
-    asm("bfind.u32 %0, %1;" : "=r"(r) : "r"(x));
+__device__ __forceinline__ double rcp64h(double x) {             // MUFU.RCP64H: ~20-bit reciprocal
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
     return r;
 }
-__device__ __forceinline__ int hi32(long long q) { return (int)(q >> 32); }
+__device__ __forceinline__ unsigned hiw(double d) { return (unsigned)__double2hiint(d); }
 
-// The 64-bit occupancy window that starts at forward cell c0 of the current line, normalised so that
-// the FIRST cell of the span sits at bit 31 and later cells at lower bits: bfind then names the first
-// occupied cell as k = 31 - p.  Both words are at ascending addresses (a, a + 4) in either direction.
-template <class MS, bool kFwd, bool kAux>
-__device__ __forceinline__ int window_msb(typename MS::addr_t wbase, int c0, uint32_t& words) {
-    const int j4 = (c0 >> 5) << 2;
-    typename MS::addr_t a = MS::addb(wbase, kFwd ? j4 : -j4);
-    const uint32_t L = MS::ld(a), Hh = MS::ld(MS::addb(a, 4));
-    if (kAux) words += 2;
-    return bfind32(kFwd ? __brev(__funnelshift_r(L, Hh, c0)) : __funnelshift_l(L, Hh, c0));
+struct BeamHit {
+    float r;
+    int hit;
+};
+
+// Entry distance of a hit -> range in metres (fp32 is ample: tolerance 1e-4 m on <= tens of metres).
+__device__ __forceinline__ float range_from_du(double dU, double adu, float rho) {
+    return __fdividef((float)dU * rho, (float)adu);
 }
 
-// Walks the lines of one beam.  Returns true with (cq, qe) = forward cell and 32.32 entry coordinate of
-// the first occupied cell met, false if the lines up to the end pointer hold none.
-template <class MS, bool kFwd, bool kAux>
-__device__ __forceinline__ bool walk_lines(typename MS::addr_t wbase, const typename MS::addr_t wend,
-                                           const int lstep4, long long Qn, const long long Mf, int c0,
-                                           const int cend, int& cq, long long& qe, typename MS::addr_t& wfound,
-                                           uint32_t& words) {
-    bool first = true;
-    for (;;) {
-        int p;
-        for (;;) {                                               // hot loop: one window per line
-            const int c1 = hi32(Qn);
-            p = window_msb<MS, kFwd, kAux>(wbase, c0, words);
-            if (p >= c0 + 31 - c1) break;                        // first occupied cell lies inside the span
-            if (wbase == wend) return false;
-            c0 = c1;
-            Qn += Mf;
-            wbase = MS::addb(wbase, lstep4);
-            first = false;
-        }
-        const int c1 = hi32(Qn);
-        if (p >= 0) {
-            const int k = 31 - p;
-            cq = c0 + k;
-            qe = (k == 0 && !first) ? Qn - Mf : ((long long)cq << 32);
-            wfound = wbase;
-            return true;
-        }
-        // span longer than one window with an empty first window: scan the rest of it
-        const int cl = min(c1, cend);
-        for (int cc = c0 + 32; cc <= cl; cc += 32) {
-            const int p2 = window_msb<MS, kFwd, kAux>(wbase, cc, words);
-            if (p2 >= 0 && cc + 31 - p2 <= cl) {
-                cq = cc + 31 - p2;
-                qe = (long long)cq << 32;
-                wfound = wbase;
-                return true;
-            }
-        }
-        if (wbase == wend) return false;
-        c0 = c1;
-        Qn += Mf;
-        wbase = MS::addb(wbase, lstep4);
-        first = false;
-    }
-}
-
-// Hot loop in PTX for the shared-memory map and slopes M < 31 cells per line (span <= 32 cells, so one
-// window per line always suffices).  Per line: word address (shr, mad), two ld.shared, funnel shift,
-// (brev,) bfind.shiftamt = k, len = c1 - c0, hit = (k <= len) fused with the end-of-lines test into one
-// predicate and one branch, then the 64-bit fixed-point add and the line-pointer add: 14 (forward) /
-// 13 (backward) instructions.  Unrolled twice with the roles of the (c0, hi(Q)) registers swapped so
-// that "c0 := c1" costs nothing.  Returns true when the first occupied cell of the current line's
-// window lies inside the beam's span (k = its offset from c0); false when the lines are exhausted.
-template <bool kFwd>
-__device__ __forceinline__ bool fast_lines_smem(uint32_t& wbase, const uint32_t wend, const int lstep4,
-                                                uint32_t& qlo, int& qhi, const uint32_t mlo, const int mhi,
-                                                int& c0, int& k) {
-    int found, c0o, qho;
-#define FN_LINE(RC, RQ, EXIT)                                              \
-    "shr.s32 j, " RC ", 5;\n\t"                                            \
-    "mad.lo.s32 a, j, %12, %0;\n\t"                                        \
-    "ld.shared.u32 L, [a];\n\t"                                            \
-    "ld.shared.u32 H, [a+4];\n\t"                                          \
-    FN_SHIFT(RC)                                                           \
-    "bfind.shiftamt.u32 %4, x;\n\t"                                        \
-    "sub.s32 len, " RQ ", " RC ";\n\t"                                     \
-    "setp.le.u32 ph, %4, len;\n\t"                                         \
-    "setp.eq.or.u32 pe, %0, %8, ph;\n\t"                                   \
-    "@pe bra " EXIT ";\n\t"                                                \
-    "add.cc.u32 %1, %1, %10;\n\t"                                          \
-    "addc.s32 " RC ", " RQ ", %11;\n\t"                                    \
-    "add.s32 %0, %0, %9;\n\t"
-    if (kFwd) {
-#define FN_SHIFT(RC) "shf.r.wrap.b32 x, L, H, " RC ";\n\tbrev.b32 x, x;\n\t"
-        asm volatile(
-            "{\n\t"
-            ".reg .pred ph, pe;\n\t"
-            ".reg .b32 j, a, L, H, x, len, rc, rq;\n\t"
-            "mov.b32 rc, %2;\n\t"
-            "mov.b32 rq, %3;\n\t"
-            "FN_LA:\n\t" FN_LINE("rc", "rq", "FN_XA")
-            FN_LINE("rq", "rc", "FN_XB")
-            "bra FN_LA;\n\t"
-            "FN_XA:\n\t"
-            "mov.b32 %6, rc;\n\t"
-            "mov.b32 %7, rq;\n\t"
-            "bra FN_END;\n\t"
-            "FN_XB:\n\t"
-            "mov.b32 %6, rq;\n\t"
-            "mov.b32 %7, rc;\n\t"
-            "FN_END:\n\t"
-            "selp.s32 %5, 1, 0, ph;\n\t"
-            "}"
-            : "+r"(wbase), "+r"(qlo), "+r"(c0), "+r"(qhi), "=r"(k), "=r"(found), "=r"(c0o), "=r"(qho)
-            : "r"(wend), "r"(lstep4), "r"(mlo), "r"(mhi), "n"(4));
-#undef FN_SHIFT
-    } else {
-#define FN_SHIFT(RC) "shf.l.wrap.b32 x, L, H, " RC ";\n\t"
-        asm volatile(
-            "{\n\t"
-            ".reg .pred ph, pe;\n\t"
-            ".reg .b32 j, a, L, H, x, len, rc, rq;\n\t"
-            "mov.b32 rc, %2;\n\t"
-            "mov.b32 rq, %3;\n\t"
-            "FN_LA:\n\t" FN_LINE("rc", "rq", "FN_XA")
-            FN_LINE("rq", "rc", "FN_XB")
-            "bra FN_LA;\n\t"
-            "FN_XA:\n\t"
-            "mov.b32 %6, rc;\n\t"
-            "mov.b32 %7, rq;\n\t"
-            "bra FN_END;\n\t"
-            "FN_XB:\n\t"
-            "mov.b32 %6, rq;\n\t"
-            "mov.b32 %7, rc;\n\t"
-            "FN_END:\n\t"
-            "selp.s32 %5, 1, 0, ph;\n\t"
-            "}"
-            : "+r"(wbase), "+r"(qlo), "+r"(c0), "+r"(qhi), "=r"(k), "=r"(found), "=r"(c0o), "=r"(qho)
-            : "r"(wend), "r"(lstep4), "r"(mlo), "r"(mhi), "n"(-4));
-#undef FN_SHIFT
-    }
-#undef FN_LINE
-    c0 = c0o;
-    qhi = qho;
-    return found != 0;
-}
-
-// One beam.  (ox, oy) origin in cells, (dx, dy) unit direction, T = max range in cells; `inside` = the
-// r_max disc around the origin lies inside the map (no exit clipping needed).
-// Returns range in metres; *hit = linear cell index, -1 (no hit) or -2 (left the map).
-template <class MS, bool kAux>
-__device__ __forceinline__ float cast_beam(const BeamMap<MS>& bm, const double ox, const double oy,
-                                           const double dx, const double dy, double T, const bool inside,
-                                           const float rho, const float rmax, int* hit, uint32_t& words) {
-    const int jx = __double2int_rd(ox), iy = __double2int_rd(oy);
-    if ((unsigned)jx >= (unsigned)bm.W || (unsigned)iy >= (unsigned)bm.H) { *hit = -2; return 0.0f; }
-    {
-        const uint32_t w0 = MS::ld(MS::addb(bm.row, (iy * bm.strideR + 1 + (jx >> 5)) << 2));
-        if (kAux) ++words;
-        if ((w0 >> (jx & 31)) & 1u) { *hit = iy * bm.W + jx; return 0.0f; }
-    }
-    const bool mx = fabs(dx) >= fabs(dy);                         // dominant axis is x
-    const double ou = mx ? ox : oy, ow = mx ? oy : ox;
-    const double du = mx ? dx : dy, dw = mx ? dy : dx;
+// ---- side path: beams nearly parallel to an axis (or exactly parallel: dw == 0).  Plain per-line walk
+// over 32-bit words; at most T / 30 + 2 lines of up to T cells each.
+template <class MS>
+__device__ __noinline__ BeamHit cast_beam_slow(const BeamMap<MS> bm, const BeamOrient o, const bool mx,
+                                               const double du, const double dw, const double T,
+                                               const float rho, const float rmax) {
     const double adu = fabs(du), adw = fabs(dw);
     const bool fu = du >= 0.0, fw = dw >= 0.0;
+    const double ou = o.ouM - (kMagic + (double)kCellShift);
+    const double f = fw ? 0.5 + o.h : 0.5 - o.h;
     const int Wu = mx ? bm.W : bm.H, Hw = mx ? bm.H : bm.W;
-    const int nw = mx ? bm.nwR : bm.nwC, stride = mx ? bm.strideR : bm.strideC;
-    const int l0 = mx ? iy : jx;
-    const int Wq = nw << 5;
-
-    // slope M = |du/dw| by one Newton step on the fp32 reciprocal (relative error ~1e-14), capped
-    double M;
-    {
-        const double r0 = (double)__frcp_rn((float)adw);
-        const double r1 = r0 * (2.0 - adw * r0);
-        M = (adw * kMaxSlope > adu) ? adu * r1 : kMaxSlope;
-    }
-    bool exit_hit = false;
-    if (!inside) {                                                // does the beam leave the map before r_max?
-        const double tu = (fu ? (double)Wu - ou : ou) / adu;
-        const double tw = adw > 0.0 ? (fw ? (double)Hw - ow : ow) / adw : INFINITY;
-        const double te = fmin(tu, tw);
-        if (te < T) { T = te; exit_hit = true; }
-    }
-    const double l0d = (double)l0;
-    const double tf = l0d - ow;                                   // in (-1, 0]
-    const double f = fw ? tf + 1.0 : -tf;                         // distance to the first line boundary
-    const double q0s = (fu ? ou : (double)Wq - ou) * kFix;        // forward coordinate, 32.32 scaled
-    const double Ms = M * kFix;
-    int lend = __double2int_rd(ow + T * dw);
-    lend = max(0, min(Hw - 1, lend));
-    const long long Q0 = __double2ll_rd(q0s);
-    const long long Qn = __double2ll_rd(q0s + f * Ms);            // U_1
-    const long long Mf = __double2ll_rd(Ms);
-    const long long Qend = __double2ll_rd(q0s + (T * kFix) * adu);
-    const int cend = min(hi32(Qend), fu ? Wu - 1 : Wq - 1);
-
-    const int stride4 = stride << 2;
-    const int lstep4 = fw ? stride4 : -stride4;
-    typename MS::addr_t line0 = MS::addb(mx ? bm.row : bm.col, l0 * stride4);
-    typename MS::addr_t wbase = MS::addb(line0, fu ? 4 : (nw - 1) << 2);
-    typename MS::addr_t wend = MS::addb(wbase, (lend - l0) * stride4);
-    int cq = 0;
-    long long qe = 0;
-    typename MS::addr_t wfound = wbase;
-    bool found;
-    if constexpr (std::is_same<MS, SmemSpace>::value && !kAux) {
-        if (hi32(Mf) < 31) {                                      // one window per line always suffices
-            uint32_t wb = wbase, qlo = (uint32_t)Qn;
-            int qhi = hi32(Qn), c0 = hi32(Q0), k;
-            found = fu ? fast_lines_smem<true>(wb, wend, lstep4, qlo, qhi, (uint32_t)Mf, hi32(Mf), c0, k)
-                       : fast_lines_smem<false>(wb, wend, lstep4, qlo, qhi, (uint32_t)Mf, hi32(Mf), c0, k);
-            cq = c0 + k;
-            const long long Qcur = ((long long)qhi << 32) | (long long)qlo;
-            qe = (k == 0 && wb != wbase) ? Qcur - Mf : ((long long)cq << 32);
-            wfound = wb;
+    const int stride4 = mx ? bm.stride4R : bm.stride4C;
+    const double M = adw > 0.0 ? adu / adw : INFINITY;
+    const double Tu = T * adu;                                    // travel along u at the range limit
+    typename MS::addr_t line = MS::addb(bm.base, (int)o.line_off);
+    int l = o.l0;
+    double E = ou;                                                // entry coordinate of the current line
+    for (int k = 0;; ++k) {
+        double X = fu ? ou + (f + (double)k) * M : ou - (f + (double)k) * M;        // exit coordinate
+        if (!(X > -1.0)) X = -0.5;                                // clamp into the frame cells (also NaN/inf)
+        if (!(X < (double)Wu + 1.0)) X = (double)Wu + 0.5;
+        const bool last = !(fabs(X - ou) < Tu);                   // the range limit lies in this line
+        const int ce = __double2int_rd(E), cx = __double2int_rd(X);
+        int c = ce, found = 0;
+        if (fu) {
+            while (c <= cx) {
+                const int q = c + kCellShift;
+                const uint32_t w = MS::ld(MS::addb(line, (q >> 5) << 2)) >> (q & 31);
+                if (w) { c += __ffs(w) - 1; found = c <= cx; break; }
+                c += 32 - (q & 31);
+            }
         } else {
-            found = fu ? walk_lines<MS, true, kAux>(wbase, wend, lstep4, Qn, Mf, hi32(Q0), cend, cq, qe, wfound, words)
-                       : walk_lines<MS, false, kAux>(wbase, wend, lstep4, Qn, Mf, hi32(Q0), cend, cq, qe, wfound, words);
+            while (c >= cx) {
+                const int q = c + kCellShift;
+                const uint32_t w = MS::ld(MS::addb(line, (q >> 5) << 2)) << (31 - (q & 31));
+                if (w) { c -= __clz(w); found = c >= cx; break; }
+                c -= (q & 31) + 1;
+            }
         }
-    } else {
-        found = fu ? walk_lines<MS, true, kAux>(wbase, wend, lstep4, Qn, Mf, hi32(Q0), cend, cq, qe, wfound, words)
-                   : walk_lines<MS, false, kAux>(wbase, wend, lstep4, Qn, Mf, hi32(Q0), cend, cq, qe, wfound, words);
-    }
-    if (found && qe < Qend) {
-        if (kAux) {
-            const int cu = fu ? cq : Wq - 1 - cq;
-            const int line = l0 + MS::diffb(wfound, wbase) / stride4;
-            *hit = mx ? line * bm.W + cu : cu * bm.W + line;
+        if (found) {
+            double dU;
+            if (c == ce) dU = fabs(E - ou);                       // entered through the line boundary (or origin)
+            else dU = fu ? (double)c - ou : ou - (double)(c + 1);
+            if (!(dU < Tu)) break;
+            BeamHit h;
+            h.r = range_from_du(dU, adu, rho);
+            const bool outside = (unsigned)c >= (unsigned)Wu || (unsigned)l >= (unsigned)Hw;
+            h.hit = outside ? -2 : (mx ? l * bm.W + c : c * bm.W + l);
+            return h;
         }
-        const long long dq = qe - Q0;
-        return (float)(dq > 0 ? dq : 0) * (float)((double)rho / (adu * kFix));
+        if (last) break;
+        E = X;
+        l += fw ? 1 : -1;
+        line = MS::addb(line, fw ? stride4 : -stride4);
     }
-    if (exit_hit) { *hit = -2; return (float)(T * (double)rho); }
-    *hit = -1;
-    return rmax;
+    BeamHit h;
+    h.r = rmax; h.hit = -1;
+    return h;
+}
+
+// ---- hot loop for the shared-memory map, in PTX so that exactly one induction variable per quantity
+// survives: per line  shr (word index), mad (address), 2 x ld.shared, shf.r.wrap (window), and + setp
+// (candidate), setp.eq.or (last line), bra, add.f64 (crossing coordinate), add (line pointer) = 11 PTX
+// instructions, 10 in SASS (and + setp fuse into one LOP3; the loop is rotated so the adds lead).  Leaves with x != 0 (candidate in the
+// line wb, th = high word of D) or x == 0 (wb == wend: lines exhausted).
+__device__ __forceinline__ void hot_lines_smem(double& D, uint32_t& wb, const double Md, const int lstep,
+                                               const uint32_t wend, const uint32_t mask, uint32_t& x, uint32_t& th) {
+    // rotated loop: the increments lead, so the loop variables themselves are the values at the exit
+    D -= Md;
+    wb -= (uint32_t)lstep;
+    asm volatile(
+        "{\n\t"
+        ".reg .pred ph, pc;\n\t"
+        ".reg .b32 j, a, L, H, lo, hi;\n\t"
+        "FN_LOOP:\n\t"
+        "add.f64 %0, %0, %3;\n\t"
+        "add.s32 %1, %1, %4;\n\t"
+        "mov.b64 {lo, hi}, %0;\n\t"
+        "shr.u32 j, hi, 5;\n\t"
+        "mad.lo.u32 a, j, 4, %1;\n\t"
+        "ld.shared.u32 L, [a];\n\t"
+        "ld.shared.u32 H, [a+4];\n\t"
+        "shf.r.wrap.b32 %2, L, H, hi;\n\t"
+        "and.b32 %2, %2, %6;\n\t"
+        "setp.eq.u32 ph, %2, 0;\n\t"
+        "setp.ne.and.u32 pc, %1, %5, ph;\n\t"
+        "@pc bra FN_LOOP;\n\t"
+        "}"
+        : "+d"(D), "+r"(wb), "=r"(x)
+        : "d"(Md), "r"(lstep), "r"(wend), "r"(mask));
+    th = hiw(D);
+}
+
+// ---- one beam.  pose = the env's BeamPose (global memory), cs = (cos, sin) of the beam's body-frame angle.
+// kAux additionally names the hit cell (linear index, -1 no hit, -2 outside the map) and counts 32-bit
+// map words loaded.
+template <class MS, bool kAux>
+__device__ __forceinline__ float cast_beam(const BeamMap<MS>& bm, const BeamPose* __restrict__ pose,
+                                           const double2 cs, const double T, const float rho, const float rmax,
+                                           int* hit, uint32_t& words) {
+    const double2 pcs = *reinterpret_cast<const double2*>(&pose->c);
+    const double dx = pcs.x * cs.x - pcs.y * cs.y, dy = pcs.y * cs.x + pcs.x * cs.y;
+    const bool mx = fabs(dx) >= fabs(dy);                         // dominant axis is x
+    const BeamOrient o = pose->o[mx ? 0 : 1];
+    const double du = mx ? dx : dy, dw = mx ? dy : dx;
+    const double adu = fabs(du), adw = fabs(dw);
+    // slope M = |du / dw| >= 1: one Newton step on the 20-bit reciprocal (relative error ~2^-40)
+    const double r0 = rcp64h(adw);
+    const double r1 = fma(fma(-adw, r0, 1.0), r0, r0);
+    const double M = adu * r1;
+    if (!(M < kSlowSlope)) {                                      // also dw == 0 (M = inf or NaN)
+        const BeamHit h = cast_beam_slow<MS>(bm, o, mx, du, dw, T, rho, rmax);
+        if (kAux) { *hit = h.hit; words += 8; }
+        return h.r;
+    }
+    const unsigned su = hiw(du) & 0x80000000u, sw = hiw(dw) & 0x80000000u;   // sign bits: set = backward
+    const unsigned fu1 = (su >> 31) ^ 1u;                         // 1 for beams towards higher u
+    // signed slope, distance f to the first line boundary (f = 0.5 + h forward in w, 0.5 - h backward)
+    const double Md = __hiloint2double((int)(hiw(M) ^ su), __double2loint(M));
+    const double f = __hiloint2double((int)(hiw(o.h) ^ sw), __double2loint(o.h)) + 0.5;
+    // D_0 = 2^20 + 64 + U_1 (+ 1 forward): the "+ 1" is one unit of the integer field of the high word
+    const double D0 = fma(f, Md, o.ouM);
+    double D = __hiloint2double((int)(hiw(D0) + fu1), __double2loint(D0));
+    // candidate mask: floor(M) + 2 cells ending (forward) / starting (backward) at the exit cell
+    const unsigned sh = 30u - hiw(M + kMagic);                    // low 5 bits = 30 - floor(M)
+    const uint32_t mask = su ? __funnelshift_r(0xffffffffu, 0u, sh) : __funnelshift_l(0u, 0xffffffffu, sh);
+    // lines: at most floor(T |dw|) + 2 (the frame stops every beam that would leave the map earlier)
+    const int nl = __double2loint(fma(T, adw, 2.0 + 4503599627370496.0));
+    const int stride4 = mx ? bm.stride4R : bm.stride4C;
+    const int lstep = sw ? -stride4 : stride4;
+    // forward beams read the window that ENDS at the exit cell: words (t >> 5) - 1 and t >> 5
+    const typename MS::addr_t wb0 =
+        MS::addb(bm.base, (int)(o.line_off - kExpOff) - (int)(fu1 << 2));
+    const typename MS::addr_t wend = MS::addb(wb0, (nl - 1) * lstep);
+    typename MS::addr_t wb = wb0;
+
+    float r = rmax;
+    int hcell = -1;
+    for (;;) {
+        uint32_t x, th;
+        if constexpr (std::is_same<MS, SmemSpace>::value && !kAux) {
+            hot_lines_smem(D, wb, Md, lstep, wend, mask, x, th);
+        } else {
+            for (;;) {                                            // hot loop: one window per line
+                th = hiw(D);
+                const typename MS::addr_t a = MS::addb(wb, (int)((th >> 5) << 2));
+                x = __funnelshift_r(MS::ld(a), MS::ld4(a), th) & mask;
+                if (kAux) words += 2;
+                if (x != 0u || wb == wend) break;
+                D += Md;
+                wb = MS::addb(wb, lstep);
+            }
+        }
+        if (x == 0u) break;                                       // lines exhausted: no hit
+        // exact span of this line: entry cell ce (origin cell in the first line), exit cell cx
+        const bool first = wb == wb0;
+        const int cx = (int)(th - kMagicHi - fu1);                // floor(U_{k+1}) + 64
+        const double Dp = D - Md;
+        const int ce = first ? o.cu0 + kCellShift : (int)(hiw(Dp) - kMagicHi - fu1);
+        const unsigned n = 31u - (unsigned)abs(cx - ce);
+        const uint32_t xe = x & (su ? __funnelshift_r(0xffffffffu, 0u, n) : __funnelshift_l(0u, 0xffffffffu, n));
+        if (xe != 0u) {
+            // first occupied cell in travel order: lowest bit forward, highest bit backward
+            const int c = su ? cx + (31 - __clz(xe)) : cx - 31 + (__ffs(xe) - 1);
+            double dU;
+            if (c == ce) dU = first ? 0.0 : fabs(Dp - (o.ouM + (double)fu1));          // through the line boundary
+            else dU = fabs((double)(c + (int)(su >> 31)) - (o.ouM - kMagic));          // through the cell's u-face
+            if (dU < T * adu) {
+                r = range_from_du(dU, adu, rho);
+                if (kAux) {
+                    const int k = (int)(MS::diffb(wb, wb0) / lstep);                   // lines crossed so far
+                    const int lw = sw ? o.l0 - k : o.l0 + k, cu = c - kCellShift;
+                    const int Wu = mx ? bm.W : bm.H, Hw = mx ? bm.H : bm.W;
+                    const bool outside = (unsigned)cu >= (unsigned)Wu || (unsigned)lw >= (unsigned)Hw;
+                    hcell = outside ? -2 : (mx ? lw * bm.W + cu : cu * bm.W + lw);
+                }
+            }
+            break;                                                // later lines are farther away
+        }
+        if (wb == wend) break;
+        D += Md;
+        wb = MS::addb(wb, lstep);
+    }
+    if (kAux) *hit = hcell;
+    return r;
 }
 
 struct BeamArgs {
     MapDev map;
     RobotDev robot;
-    const PoseD* poses;          // [N]
-    const int* pose_inside;      // [N] 1 = the r_max disc around the sensor lies inside the map
+    const BeamPose* poses;       // [N]
     const int* list;             // compacted env indices or NULL (= all envs)
     const int* count_dev;        // number of listed envs (device) or NULL
     int n_all;                   // number of envs when list == NULL
     float* out_ranges;           // [N][B]
     int* out_hit;                // [N][B] or NULL            (kAux only)
     float* ring_obs;             // ring base or NULL: also write ranges into the env's pending ring row
-    unsigned long long ring_cap, ring_head;   // pending row of env e = (ring_head + e) % ring_cap
+    unsigned long long ring_cap;
+    const unsigned long long* ring_head;      // device: pending row of env e = (*ring_head + e) % ring_cap
     int ring_row;                // floats per ring row
     int count_words;             // (kAux only)
     unsigned long long* counters;
@@ -317,14 +305,14 @@ __global__ void __launch_bounds__(512, 2) beam_kernel(BeamArgs a) {
     const unsigned total = (unsigned)n_env * (unsigned)B;
     const int warps_per_cta = blockDim.x >> 5;
     if ((unsigned)blockIdx.x * warps_per_cta * 32u >= total) return;      // nothing for this CTA: skip staging
-    const int rowWords = a.map.H * a.map.strideR, colWords = a.map.W * a.map.strideC;
+    const int mapWords = (a.map.H + 2 * kLineGuard) * a.map.strideR + (a.map.W + 2 * kLineGuard) * a.map.strideC;
     double2* s_tab = reinterpret_cast<double2*>(smem_raw);
     uint32_t* s_map = reinterpret_cast<uint32_t*>(smem_raw + (size_t)B * sizeof(double2));
     for (int i = threadIdx.x; i < B; i += blockDim.x) s_tab[i] = a.robot.beam_cs[i];
     if (kSmem) {
-        const uint4* src = reinterpret_cast<const uint4*>(a.map.row);      // row and col are contiguous
+        const uint4* src = reinterpret_cast<const uint4*>(a.map.row);      // row and col copies are contiguous
         uint4* dst = reinterpret_cast<uint4*>(s_map);
-        const int n4 = (rowWords + colWords + 3) / 4;
+        const int n4 = (mapWords + 3) / 4;
         int i = threadIdx.x;
         for (; i + 3 * (int)blockDim.x < n4; i += 4 * blockDim.x) {         // 4 loads in flight per thread
             const uint4 v0 = __ldg(src + i), v1 = __ldg(src + i + blockDim.x);
@@ -337,15 +325,10 @@ __global__ void __launch_bounds__(512, 2) beam_kernel(BeamArgs a) {
 
     using MS = typename std::conditional<kSmem, SmemSpace, GlobalSpace>::type;
     BeamMap<MS> bm;
-    if constexpr (kSmem) {
-        bm.row = (uint32_t)__cvta_generic_to_shared(s_map);
-        bm.col = bm.row + 4u * (uint32_t)rowWords;
-    } else {
-        bm.row = a.map.row;
-        bm.col = a.map.col;
-    }
-    bm.H = a.map.H; bm.W = a.map.W; bm.nwR = a.map.nwR; bm.nwC = a.map.nwC;
-    bm.strideR = a.map.strideR; bm.strideC = a.map.strideC;
+    if constexpr (kSmem) bm.base = (uint32_t)__cvta_generic_to_shared(s_map);
+    else bm.base = (unsigned long long)__cvta_generic_to_global(a.map.row);
+    bm.H = a.map.H; bm.W = a.map.W; bm.stride4R = a.map.strideR << 2; bm.stride4C = a.map.strideC << 2;
+    const unsigned long long ring_head = a.ring_obs ? *a.ring_head : 0ull;
 
     const int lane = threadIdx.x & 31;
     const unsigned warp0 = blockIdx.x * warps_per_cta + (threadIdx.x >> 5);
@@ -359,18 +342,17 @@ __global__ void __launch_bounds__(512, 2) beam_kernel(BeamArgs a) {
         while (j >= (unsigned)B) { j -= B; ++le; }
         if (le < (unsigned)n_env) {
             const int e = a.list ? a.list[le] : (int)le;
-            const PoseD p = a.poses[e];
-            const bool inside = a.pose_inside[e] != 0;
-            const double2 cs = s_tab[j];
-            const double dx = p.c * cs.x - p.s * cs.y, dy = p.s * cs.x + p.c * cs.y;
-            int hit;
-            const float r = cast_beam<MS, kAux>(bm, p.ox, p.oy, dx, dy, a.robot.T, inside, a.map.rho,
-                                                a.robot.rmax, &hit, words);
+            const BeamPose* pose = a.poses + e;
+            const int state = pose->state;
+            float r = 0.0f;
+            int hit = -2;
+            if (state == 0) r = cast_beam<MS, kAux>(bm, pose, s_tab[j], a.robot.T, a.map.rho, a.robot.rmax, &hit, words);
+            else if (kAux) { if (state == 1) hit = pose->o[0].l0 * a.map.W + pose->o[0].cu0; ++words; }
             const size_t o = (size_t)e * B + j;
             a.out_ranges[o] = r;
             if (kAux && a.out_hit) a.out_hit[o] = hit;
             if (a.ring_obs) {
-                const unsigned long long slot = (a.ring_head + (unsigned long long)e) % a.ring_cap;
+                const unsigned long long slot = (ring_head + (unsigned long long)e) % a.ring_cap;
                 a.ring_obs[slot * a.ring_row + j] = r;
             }
             ++rays;

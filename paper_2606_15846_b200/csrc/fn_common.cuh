@@ -12,23 +12,43 @@ constexpr int kNCounters = 8;
 enum Counter { kRays = 0, kWords = 1, kResets = 2, kResetFail = 3, kNonFinite = 4, kEnvSteps = 5 };
 
 // Bit-packed map, two orientations.  A "line" is one row of the row-packed copy (bits run along
-// columns) or one column of the column-packed copy (bits run along rows).  Each line is
-//   [1 pad word][nw data words][1 pad word]   (32-bit words, bit b of word k = cell 32k + b, pads = 0)
-// so that a 64-bit window starting at any data word can be read with two aligned 32-bit loads.
+// columns) or one column of the column-packed copy (bits run along rows).  "Outside the map is
+// occupied" is stored physically, so no kernel clips a beam against the map border:
+//   * a copy holds L + 4 lines: physical line p = l + 2; lines l = -2, -1, L, L+1 are all ones
+//     (l = -1 and L are the frame the beams hit; the outer two are guards for look-ahead reads);
+//   * a line is [2 pad words][nw data words][2 pad words] of 32 bits, pads all ones; data bit b of
+//     word k is cell 32k + b, bits at or beyond the line's length are ones.  So cell u sits at bit
+//     (u + 64) & 31 of physical word (u + 64) >> 5, for u in [-64, 32 nw + 64).
 struct MapDev {
-    const uint32_t* row;     // [H][strideR]
-    const uint32_t* col;     // [W][strideC]
+    const uint32_t* row;     // [H + 4][strideR]
+    const uint32_t* col;     // [W + 4][strideC]   (directly after the row copy)
     int H, W;
     int nwR, nwC;            // data words per line: ceil(W/32), ceil(H/32)
-    int strideR, strideC;    // nw + 2
+    int strideR, strideC;    // nw + 4
     float rho;               // metres per cell
     double inv_rho;          // 1 / (double)rho
 };
+constexpr int kCellShift = 64;     // cell u is stored at bit position u + kCellShift of its line
+constexpr int kLineGuard = 2;      // physical line = l + kLineGuard
 
-// Per-env sensing pose, written by the env/reset kernels, read by the beam kernel.
-struct __align__(32) PoseD {
-    double ox, oy;           // sensor origin in cell units
+// Per-env sensing pose, written by the env/reset/pose kernels, read by the beam kernel.  The beam
+// kernel walks along the beam's dominant axis "u" (minor axis "w"); both choices are prepared here:
+// o[0]: u = x (row-packed copy, line = row), o[1]: u = y (column-packed copy, line = column).
+constexpr double kMagic = 1048576.0;            // 2^20: a double D in [2^20, 2^21) has ulp 2^-32, its
+constexpr unsigned kMagicHi = 0x41300000u;      // high word is kMagicHi + floor(D - 2^20)
+struct __align__(16) BeamOrient {
+    double ouM;              // origin along u, in cells, + kCellShift + kMagic
+    double h;                // 0.5 - frac(origin along w): first line boundary at f = 0.5 +- h
+    int cu0;                 // floor(origin along u)
+    unsigned line_off;       // byte offset of the origin's line from the start of the row copy
+    int l0;                  // floor(origin along w) = line index
+    int pad_;
+};
+struct __align__(32) BeamPose {
     double c, s;             // cos/sin of the heading
+    BeamOrient o[2];
+    int state;               // 0 = origin in a free cell, 1 = in an occupied cell, 2 = outside the map
+    int pad_[3];
 };
 
 struct RobotDev {
@@ -81,7 +101,7 @@ __device__ __forceinline__ double wrap_pi(double a) {
 // occupancy of cell (i, j) from the row-packed copy in global memory; outside the map = occupied
 __device__ __forceinline__ bool occ_global(const MapDev& m, int i, int j) {
     if ((unsigned)i >= (unsigned)m.H || (unsigned)j >= (unsigned)m.W) return true;
-    uint32_t w = __ldg(m.row + (size_t)i * m.strideR + 1 + (j >> 5));
+    uint32_t w = __ldg(m.row + (size_t)(i + kLineGuard) * m.strideR + ((j + kCellShift) >> 5));
     return (w >> (j & 31)) & 1u;
 }
 

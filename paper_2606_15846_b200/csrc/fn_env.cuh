@@ -1,77 +1,175 @@
 // fn_env.cuh -- per-environment kernels: S1 clip + motion, S3 footprint collision, S4 goal obs /
-// reward / done, S5 reset, S6 compaction of the reset mask.  One warp per environment.
-// fp64 throughout for the geometry (per-env work is ~0.1 % of the beam work; B200 runs fp64 at half
-// rate), so every decision sits far inside the 1e-5 cell near-tie margin of the parity contract.
+// reward / done, S5 reset, S6 compaction of the reset mask.
+// Geometry is fp64 (per-env work is ~1 % of the beam work; B200 runs fp64 at half rate), so every
+// discrete decision sits ~10 orders of magnitude inside the 1e-5 cell near-tie margin of the parity
+// contract.  The scalar math runs one THREAD per env (a warp-uniform fp64 instruction still occupies
+// the fp64 pipe for the whole warp, so redundant lanes are not free); only the exact polygon test of
+// the few envs whose footprint window holds occupied cells is warp-cooperative.
 #pragma once
 #include "fn_common.cuh"
 
 namespace fn {
 
 // ---------------------------------------------------------------- S3: footprint collision
-// Closed polygon vs closed occupied cell (the zero-sampling-interval limit of Eq. (2),
-// PAPER.md:118-123): a cell collides iff some polygon edge meets its closed square, or the
-// square's centre lies inside the polygon.  Edge vs square by the separating-axis test
-// (axes x, y and the edge normal), centre by the even-odd crossing rule -- no divisions.
-__device__ __forceinline__ bool cell_meets_polygon(int V, const double* vx, const double* vy, int j, int i) {
-    const double xl = (double)j, xh = xl + 1.0, yl = (double)i, yh = yl + 1.0;
-    const double cx = xl + 0.5, cy = yl + 0.5;
-    bool inside = false;
-    double px = vx[V - 1], py = vy[V - 1];
-    for (int a = 0; a < V; ++a) {
-        const double qx = vx[a], qy = vy[a];
-        if (!(fmax(px, qx) < xl || fmin(px, qx) > xh || fmax(py, qy) < yl || fmin(py, qy) > yh)) {
-            const double ex = qx - px, ey = qy - py;
-            const double a0 = ex * (yl - py), a1 = ex * (yh - py);
-            const double b0 = ey * (xl - px), b1 = ey * (xh - px);
-            const double f00 = a0 - b0, f10 = a0 - b1, f01 = a1 - b0, f11 = a1 - b1;
-            const double mn = fmin(fmin(f00, f10), fmin(f01, f11));
-            const double mxv = fmax(fmax(f00, f10), fmax(f01, f11));
-            if (mn <= 0.0 && mxv >= 0.0) return true;
-        }
-        if ((qy > cy) != (py > cy)) {
-            const double ey = py - qy;
-            const double t = (px - qx) * (cy - qy) - (cx - qx) * ey;   // sign(ey) * (x_cross - cx)
-            if (ey > 0.0 ? t > 0.0 : t < 0.0) inside = !inside;
-        }
-        px = qx; py = qy;
-    }
-    return inside;
+// Closed polygon vs closed occupied cell = the zero-sampling-interval limit of Eq. (2)
+// (PAPER.md:118-123); anything outside the map is occupied.
+//
+// Two stages.  (1) per thread: transform the vertices, take the bounding window of cells; a window
+// that leaves the map collides at once; otherwise read the window's rows of occupancy bits -- no
+// occupied cell in the window = no collision (the common case).  (2) warp-cooperative, only for
+// windows holding occupied cells: one lane per window row builds the exact set of cells of that row
+// that the closed polygon meets, as a bit mask, and ANDs it with the row's occupancy bits:
+//   cells met by the polygon = cells some edge passes through  U  cells whose centre is inside
+// (a cell no edge passes through lies wholly inside or wholly outside).  Per row, an edge clipped to
+// the strip y in [i, i+1] covers the cells floor(x_a)..floor(x_b) of its x-extent; the centres inside
+// follow from the even-odd rule on the line y = i + 1/2 (each crossing toggles the cells to its left).
+// Cost: O(V) per row whatever the number of occupied cells.
+
+struct Window {
+    int i0, i1, j0, j1;      // inclusive cell ranges (rows, columns)
+    int status;              // 0 = free (no occupied cell in the window), 1 = collides (leaves the map /
+};                           //     non-finite), 2 = occupied cells in the window: exact test needed
+
+// occupancy bits of row i, columns jb .. jb+31 (bit b = cell jb + b), from the row-packed copy
+__device__ __forceinline__ uint32_t row_bits(const MapDev& m, int i, int jb) {
+    const int q = jb + kCellShift;
+    const uint32_t* p = m.row + (size_t)(i + kLineGuard) * m.strideR + (q >> 5);
+    return __funnelshift_r(__ldg(p), __ldg(p + 1), q);
+}
+__device__ __forceinline__ uint32_t low_bits(int n) {           // n in [0, 32] -> n low bits set
+    return n >= 32 ? 0xffffffffu : ((1u << n) - 1u);
 }
 
-// Warp-cooperative: all lanes pass the same pose; svx/svy are this warp's shared scratch [kMaxVerts].
-// Lanes transform the vertices, reduce the bounding window, then stride over its cells; only
-// occupied (or outside-map) cells pay for the polygon test.  Returns the same flag on every lane.
-__device__ bool warp_collision(const MapDev& m, const RobotDev& rb, double x, double y, double c,
-                               double s, double* svx, double* svy) {
-    const int lane = lane_id();
-    const double rho = (double)m.rho;
+// stage 1, one thread per pose
+__device__ __forceinline__ Window footprint_window(const MapDev& m, const RobotDev& rb, double x, double y,
+                                                   double c, double s) {
+    const double inv = m.inv_rho;
     double xmin = INFINITY, xmax = -INFINITY, ymin = INFINITY, ymax = -INFINITY;
-    __syncwarp();
-    for (int k = lane; k < rb.V; k += 32) {
+    for (int k = 0; k < rb.V; ++k) {
         const double2 f = rb.verts[k];
-        const double wx = (x + c * f.x - s * f.y) / rho, wy = (y + s * f.x + c * f.y) / rho;
-        svx[k] = wx; svy[k] = wy;
+        const double wx = (x + c * f.x - s * f.y) * inv, wy = (y + s * f.x + c * f.y) * inv;
         xmin = fmin(xmin, wx); xmax = fmax(xmax, wx);
         ymin = fmin(ymin, wy); ymax = fmax(ymax, wy);
     }
-    xmin = warp_min(xmin); xmax = warp_max(xmax); ymin = warp_min(ymin); ymax = warp_max(ymax);
+    Window w;
+    w.i0 = w.i1 = w.j0 = w.j1 = 0;
+    w.status = 1;
+    // NaN-safe: a footprint reaching outside the map meets the (occupied) outside at once
+    if (!(xmin >= 0.0 && ymin >= 0.0 && xmax < (double)m.W && ymax < (double)m.H)) return w;
+    w.j0 = __double2int_rd(xmin); w.j1 = __double2int_rd(xmax);
+    w.i0 = __double2int_rd(ymin); w.i1 = __double2int_rd(ymax);
+    uint32_t any = 0;
+    for (int jb = w.j0; jb <= w.j1; jb += 32) {
+        const uint32_t cm = low_bits(w.j1 - jb + 1);
+        for (int i = w.i0; i <= w.i1; ++i) any |= row_bits(m, i, jb) & cm;
+    }
+    w.status = any ? 2 : 0;
+    return w;
+}
+
+// stage 2, warp-cooperative: every lane passes the SAME pose and window; sv = this warp's shared
+// scratch [3][kMaxVerts] doubles (vertex x, vertex y, edge dx/dy).  Returns the flag on every lane.
+__device__ __noinline__ bool warp_collision_exact(const MapDev& m, const RobotDev& rb, double x, double y,
+                                                  double c, double s, int i0, int i1, int j0, int j1,
+                                                  double* sv) {
+    const int lane = lane_id();
+    const int V = rb.V;
+    double* vx = sv;
+    double* vy = sv + kMaxVerts;
+    double* sl = sv + 2 * kMaxVerts;
+    const double inv = m.inv_rho;
     __syncwarp();
-    if (!(isfinite(xmin) && isfinite(xmax) && isfinite(ymin) && isfinite(ymax))) return true;
-    // a footprint reaching outside the map collides with the (occupied) outside at once
-    if (xmin < 0.0 || ymin < 0.0 || xmax >= (double)m.W || ymax >= (double)m.H) return true;
-    const int j0 = __double2int_rd(xmin), j1 = __double2int_rd(xmax);
-    const int i0 = __double2int_rd(ymin), i1 = __double2int_rd(ymax);
-    const int ncols = j1 - j0 + 1, total = ncols * (i1 - i0 + 1);
-    bool found = false;
-    for (int base = 0; base < total; base += 32) {
-        const int n = base + lane;
-        if (n < total) {
-            const int i = i0 + n / ncols, j = j0 + n % ncols;
-            if (occ_global(m, i, j)) found = cell_meets_polygon(rb.V, svx, svy, j, i);
+    for (int k = lane; k < V; k += 32) {
+        const double2 f = rb.verts[k];
+        vx[k] = (x + c * f.x - s * f.y) * inv;
+        vy[k] = (y + s * f.x + c * f.y) * inv;
+    }
+    __syncwarp();
+    for (int k = lane; k < V; k += 32) {                           // edge k: vertex k -> k+1
+        const int k1 = k + 1 == V ? 0 : k + 1;
+        const double dy = vy[k1] - vy[k];
+        sl[k] = dy != 0.0 ? (vx[k1] - vx[k]) / dy : 0.0;
+    }
+    __syncwarp();
+    const int rows = i1 - i0 + 1;
+    for (int r0 = 0; r0 < rows; r0 += 32) {
+        const int i = i0 + r0 + lane;
+        const bool active = i <= i1;
+        const double ylo_s = (double)i, yhi_s = ylo_s + 1.0, yc = ylo_s + 0.5;
+        bool found = false;
+        for (int jb = j0; jb <= j1 && !found; jb += 32) {
+            const uint32_t cm = low_bits(j1 - jb + 1);
+            const uint32_t occ = active ? (row_bits(m, i, jb) & cm) : 0u;
+            uint32_t touch = 0, inside = 0;
+            if (occ) {
+                for (int k = 0; k < V; ++k) {
+                    const int k1 = k + 1 == V ? 0 : k + 1;
+                    const double px = vx[k], py = vy[k], qx = vx[k1], qy = vy[k1], sk = sl[k];
+                    const double elo = fmin(py, qy), ehi = fmax(py, qy);
+                    if (ehi >= ylo_s && elo <= yhi_s) {            // the edge meets the closed strip
+                        const double exlo = fmin(px, qx), exhi = fmax(px, qx);
+                        double xa = exlo, xb = exhi;
+                        if (py != qy) {
+                            const double x1 = px + (fmax(elo, ylo_s) - py) * sk, x2 = px + (fmin(ehi, yhi_s) - py) * sk;
+                            xa = fmax(fmin(x1, x2), exlo); xb = fmin(fmax(x1, x2), exhi);
+                        }
+                        const int ca = max(__double2int_rd(xa) - jb, 0), cb = min(__double2int_rd(xb) - jb, 31);
+                        if (ca <= cb) touch |= low_bits(cb + 1) & ~low_bits(ca);
+                    }
+                    if ((py > yc) != (qy > yc)) {                   // crosses the centre line: cells with
+                        const double xc = px + (yc - py) * sk;      // centre j + 1/2 < xc lie to its left
+                        const int nleft = __double2int_ru(xc - 0.5) - jb;
+                        inside ^= low_bits(min(max(nleft, 0), 32));
+                    }
+                }
+            }
+            found = (occ & (touch | inside)) != 0u;
         }
         if (__any_sync(0xffffffffu, found)) return true;
     }
     return false;
+}
+
+// Resolves the exact test for every lane whose window needs it (status 2), one pose at a time with
+// the whole warp cooperating.  All 32 lanes must call; returns this lane's collision flag.
+__device__ __forceinline__ bool resolve_collisions(const MapDev& m, const RobotDev& rb, const Window& w,
+                                                   double x, double y, double c, double s, double* sv) {
+    bool col = w.status == 1;
+    unsigned need = __ballot_sync(0xffffffffu, w.status == 2);
+    while (need) {
+        const int src = __ffs(need) - 1;
+        need &= need - 1;
+        const double bx = __shfl_sync(0xffffffffu, x, src), by = __shfl_sync(0xffffffffu, y, src);
+        const double bc = __shfl_sync(0xffffffffu, c, src), bs = __shfl_sync(0xffffffffu, s, src);
+        const int i0 = __shfl_sync(0xffffffffu, w.i0, src), i1 = __shfl_sync(0xffffffffu, w.i1, src);
+        const int j0 = __shfl_sync(0xffffffffu, w.j0, src), j1 = __shfl_sync(0xffffffffu, w.j1, src);
+        const bool r = warp_collision_exact(m, rb, bx, by, bc, bs, i0, i1, j0, j1, sv);
+        if (lane_id() == src) col = r;
+    }
+    return col;
+}
+
+// ---------------------------------------------------------------- sensing pose for the beam kernel
+// BeamPose (fn_common.cuh): sensor origin in cells and, for both choices of the dominant axis, the
+// origin's fixed-point coordinate, the offset to the first line boundary and the address of the
+// origin's line.
+__device__ __forceinline__ void write_pose(const MapDev& m, const RobotDev& rb, BeamPose* out,
+                                           float xf, float yf, double c, double s) {
+    const double ox = ((double)xf + c * rb.sx - s * rb.sy) * m.inv_rho;
+    const double oy = ((double)yf + s * rb.sx + c * rb.sy) * m.inv_rho;
+    BeamPose p;
+    p.c = c; p.s = s;
+    p.pad_[0] = p.pad_[1] = p.pad_[2] = 0;
+    const bool in = ox >= 0.0 && ox < (double)m.W && oy >= 0.0 && oy < (double)m.H;   // false for NaN
+    const int jx = in ? __double2int_rd(ox) : 0, iy = in ? __double2int_rd(oy) : 0;
+    p.state = !in ? 2 : (occ_global(m, iy, jx) ? 1 : 0);
+    const double fx = ox - (double)jx, fy = oy - (double)iy;
+    const unsigned rowBytes = (unsigned)(m.H + 2 * kLineGuard) * (unsigned)m.strideR * 4u;
+    p.o[0].ouM = ox + ((double)kCellShift + kMagic); p.o[0].h = 0.5 - fy; p.o[0].cu0 = jx; p.o[0].l0 = iy;
+    p.o[0].line_off = (unsigned)(iy + kLineGuard) * (unsigned)m.strideR * 4u; p.o[0].pad_ = 0;
+    p.o[1].ouM = oy + ((double)kCellShift + kMagic); p.o[1].h = 0.5 - fx; p.o[1].cu0 = iy; p.o[1].l0 = jx;
+    p.o[1].line_off = rowBytes + (unsigned)(jx + kLineGuard) * (unsigned)m.strideC * 4u; p.o[1].pad_ = 0;
+    *out = p;
 }
 
 // ---------------------------------------------------------------- S1 + S3 + S4: the env step
@@ -89,40 +187,30 @@ struct EnvArgs {
     float* out_reward;           // or NULL
     float* d_prev;
     int* ep_step;
-    PoseD* poses;
-    int* pose_inside;
+    BeamPose* poses;
     float* ring;                 // or NULL
-    unsigned long long ring_cap, ring_head;
+    unsigned long long ring_cap;
+    const unsigned long long* ring_head_dev;   // device: slot of env 0's pending row
     int ring_row;
     unsigned long long* counters;
 };
 
-__device__ __forceinline__ void write_pose(const MapDev& m, const RobotDev& rb, PoseD* out, int* inside,
-                                           float xf, float yf, double c, double s) {
-    const double rho = (double)m.rho;
-    PoseD p;
-    p.ox = ((double)xf + c * rb.sx - s * rb.sy) / rho;
-    p.oy = ((double)yf + s * rb.sx + c * rb.sy) / rho;
-    p.c = c; p.s = s;
-    *out = p;
-    // beams from here cannot leave the map: the beam kernel then skips its exit clipping
-    const double lo = rb.T + 1.0;
-    *inside = (p.ox >= lo && p.ox < (double)m.W - lo && p.oy >= lo && p.oy < (double)m.H - lo) ? 1 : 0;
-}
+constexpr int kEnvBlock = 32;    // one warp per CTA: N/32 CTAs spread the (serial) exact tests over the SMs
 
-__global__ void __launch_bounds__(256) env_step_kernel(EnvArgs a) {
-    __shared__ double s_vx[8][kMaxVerts], s_vy[8][kMaxVerts];
-    const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int e = blockIdx.x * 8 + wib;
-    if (e >= a.n) return;
+__global__ void __launch_bounds__(kEnvBlock) env_step_kernel(EnvArgs a) {
+    __shared__ double s_scratch[3 * kMaxVerts];
+    const int e = blockIdx.x * kEnvBlock + threadIdx.x;
     const int n = a.n;
+    const bool live = e < n;
+    const int el = live ? e : n - 1;                               // idle lanes shadow the last env, write nothing
     // ---- S1: clip ("within the configured bounds") and exact constant-twist step
-    const double x = a.states[0 * n + e], y = a.states[1 * n + e], psi = a.states[2 * n + e];
-    const float gxf = a.states[6 * n + e], gyf = a.states[7 * n + e];
+    const double x = a.states[0 * n + el], y = a.states[1 * n + el], psi = a.states[2 * n + el];
+    const float gxf = a.states[6 * n + el], gyf = a.states[7 * n + el];
     const int A = a.robot.A;
-    float avx = a.actions[(size_t)e * A], avy = 0.0f, aw;
-    if (a.robot.drive == 0) aw = a.actions[(size_t)e * A + 1];
-    else { avy = a.actions[(size_t)e * A + 1]; aw = a.actions[(size_t)e * A + 2]; }
+    float avx = a.actions[(size_t)el * A], avy = 0.0f, aw;
+    if (a.robot.drive == 0) aw = a.actions[(size_t)el * A + 1];
+    else { avy = a.actions[(size_t)el * A + 1]; aw = a.actions[(size_t)el * A + 2]; }
+    const float raw0 = avx, raw1 = a.robot.drive == 0 ? aw : avy, raw2 = aw;
     const bool bad = !(isfinite(avx) && isfinite(avy) && isfinite(aw));
     avx = fminf(fmaxf(avx, a.robot.lim[0]), a.robot.lim[1]);
     if (a.robot.drive != 0) avy = fminf(fmaxf(avy, a.robot.lim[2]), a.robot.lim[3]);
@@ -142,43 +230,51 @@ __global__ void __launch_bounds__(256) env_step_kernel(EnvArgs a) {
     double s1, c1;
     sincos((double)psif, &s1, &c1);
     // ---- S3
-    const bool col = warp_collision(a.map, a.robot, (double)xf, (double)yf, c1, s1, s_vx[wib], s_vy[wib]);
+    Window win = footprint_window(a.map, a.robot, (double)xf, (double)yf, c1, s1);
+    if (!live) win.status = 0;
+    const bool col = resolve_collisions(a.map, a.robot, win, (double)xf, (double)yf, c1, s1, s_scratch);
+    if (!live) return;
     // ---- S4: goal obs, reward Eq. (1), done
     const double gdx = (double)gxf - (double)xf, gdy = (double)gyf - (double)yf;
     const float d = (float)sqrt(gdx * gdx + gdy * gdy);
     const float alpha = (float)wrap_pi(atan2(gdy, gdx) - (double)psif);
-    if (lane == 0) {
-        const float dp = a.d_prev[e];
-        const int es = a.ep_step[e];
-        const bool reached = d < a.task.goal_tol;
-        const float r = col ? a.task.r_collision
-                            : reached ? a.task.r_success
-                                      : (float)((double)a.task.c_progress * ((double)dp - (double)d));
-        const bool limit = a.task.max_episode_steps > 0 && es + 1 >= a.task.max_episode_steps;
-        const bool forced = a.reset_mask[e] != 0;
-        const uint8_t done = (col || reached || limit || forced) ? 1 : 0;
-        a.states[0 * n + e] = xf; a.states[1 * n + e] = yf; a.states[2 * n + e] = psif;
-        a.states[3 * n + e] = avx; a.states[4 * n + e] = avy; a.states[5 * n + e] = aw;
-        a.out_collision[e] = col ? 1 : 0;
-        a.out_goal_obs[e] = d; a.out_goal_obs[n + e] = alpha;
-        if (a.out_reward) a.out_reward[e] = r;
-        a.reset_mask[e] = done;
-        a.d_prev[e] = d;
-        a.ep_step[e] = es + 1;
-        write_pose(a.map, a.robot, &a.poses[e], &a.pose_inside[e], xf, yf, c1, s1);
-        if (a.ring) {
-            // complete this step's row (its obs part was written when that observation was produced)
-            const int B = a.robot.B;
-            float* row = a.ring + ((a.ring_head + (unsigned long long)e) % a.ring_cap) * (size_t)a.ring_row;
-            for (int k = 0; k < A; ++k) row[B + 5 + k] = a.actions[(size_t)e * A + k];
-            row[B + 5 + A] = r;
-            row[B + 6 + A] = done ? 1.0f : 0.0f;
-            // and start the next step's row with the new goal obs and velocities
-            float* nxt = a.ring + ((a.ring_head + (unsigned long long)n + (unsigned long long)e) % a.ring_cap) * (size_t)a.ring_row;
-            nxt[B] = d; nxt[B + 1] = alpha; nxt[B + 2] = avx; nxt[B + 3] = avy; nxt[B + 4] = aw;
-        }
-        if (bad) atomicAdd(&a.counters[kNonFinite], 1ull);
+    const float dp = a.d_prev[e];
+    const int es = a.ep_step[e];
+    const bool reached = d < a.task.goal_tol;
+    const float r = col ? a.task.r_collision
+                        : reached ? a.task.r_success
+                                  : (float)((double)a.task.c_progress * ((double)dp - (double)d));
+    const bool limit = a.task.max_episode_steps > 0 && es + 1 >= a.task.max_episode_steps;
+    const bool forced = a.reset_mask[e] != 0;
+    const uint8_t done = (col || reached || limit || forced) ? 1 : 0;
+    a.states[0 * n + e] = xf; a.states[1 * n + e] = yf; a.states[2 * n + e] = psif;
+    a.states[3 * n + e] = avx; a.states[4 * n + e] = avy; a.states[5 * n + e] = aw;
+    a.out_collision[e] = col ? 1 : 0;
+    a.out_goal_obs[e] = d; a.out_goal_obs[n + e] = alpha;
+    if (a.out_reward) a.out_reward[e] = r;
+    a.reset_mask[e] = done;
+    a.d_prev[e] = d;
+    a.ep_step[e] = es + 1;
+    write_pose(a.map, a.robot, &a.poses[e], xf, yf, c1, s1);
+    if (a.ring) {
+        // complete this step's row (its obs part was written when that observation was produced)
+        const int B = a.robot.B;
+        const unsigned long long head = *a.ring_head_dev;
+        float* row = a.ring + ((head + (unsigned long long)e) % a.ring_cap) * (size_t)a.ring_row;
+        row[B + 5] = raw0; row[B + 6] = raw1;
+        if (A == 3) row[B + 7] = raw2;
+        row[B + 5 + A] = r;
+        row[B + 6 + A] = done ? 1.0f : 0.0f;
+        // and start the next step's row with the new goal obs and velocities
+        float* nxt = a.ring + ((head + (unsigned long long)n + (unsigned long long)e) % a.ring_cap) * (size_t)a.ring_row;
+        nxt[B] = d; nxt[B + 1] = alpha; nxt[B + 2] = avx; nxt[B + 3] = avy; nxt[B + 4] = aw;
     }
+    if (bad) atomicAdd(&a.counters[kNonFinite], 1ull);
+}
+
+// advances the replay ring's head by n rows (one thread), after the env-step kernel of fn_step
+__global__ void ring_advance_kernel(unsigned long long* head, unsigned long long n, unsigned long long cap) {
+    *head = (*head + n) % cap;
 }
 
 // ---------------------------------------------------------------- S6: ordered compaction of a u8 mask
@@ -210,6 +306,8 @@ __global__ void __launch_bounds__(1024) compact_mask_kernel(const uint8_t* mask,
 
 // ---------------------------------------------------------------- S5: reset of the listed envs
 // Reading G16: counter-based SplitMix64 draws, first accepted attempt in attempt order.
+// One warp per listed env; the 32 lanes evaluate 32 consecutive attempts at once and the first
+// accepted one in ATTEMPT order wins (ballot + ffs), so the result equals the sequential rule.
 __device__ __forceinline__ unsigned long long splitmix64_at(unsigned long long sigma, unsigned long long c) {
     unsigned long long z = sigma + (c + 1ull) * 0x9E3779B97F4A7C15ull;
     z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
@@ -233,67 +331,100 @@ struct ResetArgs {
     float* out_goal_obs;
     float* d_prev;
     int* ep_step;
-    PoseD* poses;
-    int* pose_inside;
+    BeamPose* poses;
     float* ring;
-    unsigned long long ring_cap, ring_head;
+    unsigned long long ring_cap;
+    const unsigned long long* ring_head_dev;
     int ring_row;
     unsigned long long* counters;
 };
 
-__global__ void __launch_bounds__(256) reset_kernel(ResetArgs a) {
-    __shared__ double s_vx[8][kMaxVerts], s_vy[8][kMaxVerts];
+constexpr int kResetWarps = 4;
+
+__global__ void __launch_bounds__(kResetWarps * 32) reset_kernel(ResetArgs a) {
+    __shared__ double s_scratch[kResetWarps][3 * kMaxVerts];
     const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int count = *a.count_dev;
     const int n = a.n;
     const double rho = (double)a.map.rho;
     const float two_pi_f = 6.28318530717958647692f, pi_f = 3.14159265358979323846f;
     const float dmin2 = __fmul_rn(a.task.dmin, a.task.dmin), dmax2 = __fmul_rn(a.task.dmax, a.task.dmax);
-    for (int li = blockIdx.x * 8 + wib; li < count; li += gridDim.x * 8) {
+    for (int li = blockIdx.x * kResetWarps + wib; li < count; li += gridDim.x * kResetWarps) {
         const int e = a.list[li];
         int r0 = 0, c0 = 0, rh = a.map.H, cw = a.map.W;
         if (a.regions.n > 0) { const int4 R = a.regions.rects[e % a.regions.n]; r0 = R.x; c0 = R.y; rh = R.z; cw = R.w; }
         const float X0 = (float)((double)c0 * rho), Xe = (float)((double)cw * rho);
         const float Y0 = (float)((double)r0 * rho), Ye = (float)((double)rh * rho);
         const unsigned long long sigma = a.seeds[e];
+        // ---- start pose: attempts k = 0..255, 32 at a time
         float x = 0.f, y = 0.f, psi = 0.f;
         double sp = 0.0, cp = 1.0;
         bool ok = false;
-        for (int k = 0; k < kMaxAttempts && !ok; ++k) {
-            x = __fmaf_rn(u24_at(sigma, 3ull * k), Xe, X0);
-            y = __fmaf_rn(u24_at(sigma, 3ull * k + 1ull), Ye, Y0);
-            psi = __fmaf_rn(u24_at(sigma, 3ull * k + 2ull), two_pi_f, -pi_f);
-            sincos((double)psi, &sp, &cp);
-            ok = !warp_collision(a.map, a.robot, (double)x, (double)y, cp, sp, s_vx[wib], s_vy[wib]);
+        for (int chunk = 0; chunk < kMaxAttempts / 32 && !ok; ++chunk) {
+            const unsigned long long k = (unsigned long long)(chunk * 32 + lane);
+            const float xk = __fmaf_rn(u24_at(sigma, 3ull * k), Xe, X0);
+            const float yk = __fmaf_rn(u24_at(sigma, 3ull * k + 1ull), Ye, Y0);
+            const float pk = __fmaf_rn(u24_at(sigma, 3ull * k + 2ull), two_pi_f, -pi_f);
+            double sk, ck;
+            sincos((double)pk, &sk, &ck);
+            const Window w = footprint_window(a.map, a.robot, (double)xk, (double)yk, ck, sk);
+            const unsigned free_m = __ballot_sync(0xffffffffu, w.status == 0);
+            unsigned cand = free_m | __ballot_sync(0xffffffffu, w.status == 2);
+            int src = 31;                                          // exhausted: keep the last candidate
+            while (cand) {
+                const int t = __ffs(cand) - 1;
+                cand &= cand - 1;
+                bool acc = (free_m >> t) & 1u;
+                if (!acc) {
+                    const double bx = __shfl_sync(0xffffffffu, (double)xk, t), by = __shfl_sync(0xffffffffu, (double)yk, t);
+                    const double bc = __shfl_sync(0xffffffffu, ck, t), bs = __shfl_sync(0xffffffffu, sk, t);
+                    const int i0 = __shfl_sync(0xffffffffu, w.i0, t), i1 = __shfl_sync(0xffffffffu, w.i1, t);
+                    const int j0 = __shfl_sync(0xffffffffu, w.j0, t), j1 = __shfl_sync(0xffffffffu, w.j1, t);
+                    acc = !warp_collision_exact(a.map, a.robot, bx, by, bc, bs, i0, i1, j0, j1, s_scratch[wib]);
+                }
+                if (acc) { ok = true; src = t; break; }
+            }
+            x = __shfl_sync(0xffffffffu, xk, src); y = __shfl_sync(0xffffffffu, yk, src);
+            psi = __shfl_sync(0xffffffffu, pk, src);
+            sp = __shfl_sync(0xffffffffu, sk, src); cp = __shfl_sync(0xffffffffu, ck, src);
         }
         bool fail = !ok;
+        // ---- goal: attempts m = 0..255, 32 at a time
         float gx = x, gy = y;
         ok = false;
-        for (int m = 0; m < kMaxAttempts && !ok; ++m) {
+        for (int chunk = 0; chunk < kMaxAttempts / 32 && !ok; ++chunk) {
+            const unsigned long long m = (unsigned long long)(chunk * 32 + lane);
             const float ua = __fmaf_rn(2.0f, u24_at(sigma, 768ull + 2ull * m), -1.0f);
             const float ub = __fmaf_rn(2.0f, u24_at(sigma, 768ull + 2ull * m + 1ull), -1.0f);
-            gx = __fmaf_rn(ua, a.task.dmax, x);
-            gy = __fmaf_rn(ub, a.task.dmax, y);
-            const float ddx = __fsub_rn(gx, x), ddy = __fsub_rn(gy, y);
+            const float gxm = __fmaf_rn(ua, a.task.dmax, x);
+            const float gym = __fmaf_rn(ub, a.task.dmax, y);
+            const float ddx = __fsub_rn(gxm, x), ddy = __fsub_rn(gym, y);
             const float d2 = __fadd_rn(__fmul_rn(ddx, ddx), __fmul_rn(ddy, ddy));
-            if (!(d2 >= dmin2 && d2 <= dmax2)) continue;
-            const int j = __double2int_rd((double)gx / rho), i = __double2int_rd((double)gy / rho);
-            ok = i >= r0 && j >= c0 && i < r0 + rh && j < c0 + cw && !occ_global(a.map, i, j);
+            bool okm = d2 >= dmin2 && d2 <= dmax2;
+            if (okm) {
+                const int j = __double2int_rd((double)gxm / rho), i = __double2int_rd((double)gym / rho);
+                okm = i >= r0 && j >= c0 && i < r0 + rh && j < c0 + cw && !occ_global(a.map, i, j);
+            }
+            const unsigned okb = __ballot_sync(0xffffffffu, okm);
+            ok = okb != 0u;
+            const int src = ok ? __ffs(okb) - 1 : 31;
+            gx = __shfl_sync(0xffffffffu, gxm, src); gy = __shfl_sync(0xffffffffu, gym, src);
         }
         fail = fail || !ok;
-        const double gdx = (double)gx - (double)x, gdy = (double)gy - (double)y;
-        const float d = (float)sqrt(gdx * gdx + gdy * gdy);
-        const float alpha = (float)wrap_pi(atan2(gdy, gdx) - (double)psi);
         if (lane == 0) {
+            const double gdx = (double)gx - (double)x, gdy = (double)gy - (double)y;
+            const float d = (float)sqrt(gdx * gdx + gdy * gdy);
+            const float alpha = (float)wrap_pi(atan2(gdy, gdx) - (double)psi);
             a.states[0 * n + e] = x; a.states[1 * n + e] = y; a.states[2 * n + e] = psi;
             a.states[3 * n + e] = 0.f; a.states[4 * n + e] = 0.f; a.states[5 * n + e] = 0.f;
             a.states[6 * n + e] = gx; a.states[7 * n + e] = gy;
             a.d_prev[e] = d;
             a.ep_step[e] = 0;
             if (a.out_goal_obs) { a.out_goal_obs[e] = d; a.out_goal_obs[n + e] = alpha; }
-            write_pose(a.map, a.robot, &a.poses[e], &a.pose_inside[e], x, y, cp, sp);
+            write_pose(a.map, a.robot, &a.poses[e], x, y, cp, sp);
             if (a.ring) {
-                float* row = a.ring + ((a.ring_head + (unsigned long long)e) % a.ring_cap) * (size_t)a.ring_row;
+                const unsigned long long head = *a.ring_head_dev;
+                float* row = a.ring + ((head + (unsigned long long)e) % a.ring_cap) * (size_t)a.ring_row;
                 const int B = a.robot.B;
                 row[B] = d; row[B + 1] = alpha; row[B + 2] = 0.f; row[B + 3] = 0.f; row[B + 4] = 0.f;
             }
@@ -310,8 +441,7 @@ struct PoseArgs {
     int n;
     const float* states;
     float* out_goal_obs;         // or NULL
-    PoseD* poses;
-    int* pose_inside;
+    BeamPose* poses;
 };
 __global__ void __launch_bounds__(256) pose_from_state_kernel(PoseArgs a) {
     const int e = blockIdx.x * blockDim.x + threadIdx.x;
@@ -320,7 +450,7 @@ __global__ void __launch_bounds__(256) pose_from_state_kernel(PoseArgs a) {
     const float x = a.states[e], y = a.states[n + e], psi = a.states[2 * n + e];
     double s, c;
     sincos((double)psi, &s, &c);
-    write_pose(a.map, a.robot, &a.poses[e], &a.pose_inside[e], x, y, c, s);
+    write_pose(a.map, a.robot, &a.poses[e], x, y, c, s);
     if (a.out_goal_obs) {
         const double gdx = (double)a.states[6 * n + e] - (double)x, gdy = (double)a.states[7 * n + e] - (double)y;
         a.out_goal_obs[e] = (float)sqrt(gdx * gdx + gdy * gdy);

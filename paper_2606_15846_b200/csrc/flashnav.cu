@@ -367,7 +367,8 @@ extern "C" int fn_step(fn_sim* s, float* states, const float* actions, float dt,
         s->ev->push_back(e0); s->ev->push_back(e1); s->ev->push_back(e2); s->ev_kind->push_back(0);
         FN_CUDA(cudaEventRecord(e0, s->stream));
     }
-    env_step_kernel<<<(s->n + kEnvBlock - 1) / kEnvBlock, kEnvBlock, 0, s->stream>>>(a);
+    a.epw = s->n >= 32768 ? 32 : (s->n >= 8192 ? 16 : 8);
+    env_step_kernel<<<(s->n + a.epw - 1) / a.epw, kEnvBlock, 0, s->stream>>>(a);
     FN_CUDA(cudaGetLastError());
     if (s->prof) FN_CUDA(cudaEventRecord(e1, s->stream));
     if (s->ring) {
@@ -400,7 +401,7 @@ extern "C" int fn_reset(fn_sim* s, float* states, const uint8_t* mask, const uin
     a.ring = s->ring; a.ring_cap = s->ring_cap ? s->ring_cap : 1; a.ring_head_dev = s->d_ring_head; a.ring_row = ring_row_floats(s);
     a.counters = s->d_counters;
     int grid = (s->n + kResetWarps - 1) / kResetWarps;
-    if (grid > s->num_sms * 8) grid = s->num_sms * 8;
+    if (grid > s->num_sms * 4) grid = s->num_sms * 4;
     reset_kernel<<<grid, kResetWarps * 32, 0, s->stream>>>(a);
     FN_CUDA(cudaGetLastError());
     int rc = launch_beams(s, s->d_list, s->d_count, out_ranges);

@@ -149,36 +149,48 @@ __device__ __noinline__ BeamHit cast_beam_slow(const BeamMap<MS> bm, const BeamO
 }
 
 // ---- hot loop for the shared-memory map, in PTX so that exactly one induction variable per quantity
-// survives: per line  shr (word index), mad (address), 2 x ld.shared, shf.r.wrap (window), and + setp
-// (candidate), setp.eq.or (last line), bra, add.f64 (crossing coordinate), add (line pointer) = 11 PTX
-// instructions, 10 in SASS (and + setp fuse into one LOP3; the loop is rotated so the adds lead).  Leaves with x != 0 (candidate in the
-// line wb, th = high word of D) or x == 0 (wb == wend: lines exhausted).
-__device__ __forceinline__ void hot_lines_smem(double& D, uint32_t& wb, const double Md, const int lstep,
-                                               const uint32_t wend, const uint32_t mask, uint32_t& x, uint32_t& th) {
-    // rotated loop: the increments lead, so the loop variables themselves are the values at the exit
-    D -= Md;
-    wb -= (uint32_t)lstep;
+// survives.  Two lines per trip (their loads and shifts are independent, which hides the shared-memory
+// latency): 2 add.f64 (crossing coordinates), 2 add (line pointers), 2 x [shr (word index), mad (address),
+// 2 ld.shared, shf.r.wrap (window)], one LOP3 ((xa | xb) & mask with the zero test), one setp for
+// the last pair, bra = 17 SASS instructions per two lines.  The loop is rotated (the increments lead),
+// so D and wb are those of the pair's SECOND line when it leaves; xa / xb = masked windows of the
+// pair's first / second line (both zero: lines exhausted).
+__device__ __forceinline__ void hot_pairs_smem(double& D, uint32_t& wb, const double Md, const int lstep,
+                                               const uint32_t wend2, const uint32_t mask, uint32_t& xa, uint32_t& xb) {
+    const double Md2 = Md + Md;
+    const int lstep2 = lstep + lstep;
     asm volatile(
         "{\n\t"
         ".reg .pred ph, pc;\n\t"
-        ".reg .b32 j, a, L, H, lo, hi;\n\t"
+        ".reg .b32 j, a, L, H, lo, hi, wa, xo;\n\t"
+        ".reg .f64 DA;\n\t"
         "FN_LOOP:\n\t"
-        "add.f64 %0, %0, %3;\n\t"
-        "add.s32 %1, %1, %4;\n\t"
+        "add.f64 DA, %0, %4;\n\t"
+        "add.f64 %0, %0, %5;\n\t"
+        "add.s32 wa, %1, %6;\n\t"
+        "add.s32 %1, %1, %7;\n\t"
+        "mov.b64 {lo, hi}, DA;\n\t"
+        "shr.u32 j, hi, 5;\n\t"
+        "mad.lo.u32 a, j, 4, wa;\n\t"
+        "ld.shared.u32 L, [a];\n\t"
+        "ld.shared.u32 H, [a+4];\n\t"
+        "shf.r.wrap.b32 %2, L, H, hi;\n\t"
         "mov.b64 {lo, hi}, %0;\n\t"
         "shr.u32 j, hi, 5;\n\t"
         "mad.lo.u32 a, j, 4, %1;\n\t"
         "ld.shared.u32 L, [a];\n\t"
         "ld.shared.u32 H, [a+4];\n\t"
-        "shf.r.wrap.b32 %2, L, H, hi;\n\t"
-        "and.b32 %2, %2, %6;\n\t"
-        "setp.eq.u32 ph, %2, 0;\n\t"
-        "setp.ne.and.u32 pc, %1, %5, ph;\n\t"
+        "shf.r.wrap.b32 %3, L, H, hi;\n\t"
+        "or.b32 xo, %2, %3;\n\t"
+        "and.b32 xo, xo, %9;\n\t"
+        "setp.eq.u32 ph, xo, 0;\n\t"
+        "setp.ne.and.u32 pc, %1, %8, ph;\n\t"
         "@pc bra FN_LOOP;\n\t"
         "}"
-        : "+d"(D), "+r"(wb), "=r"(x)
-        : "d"(Md), "r"(lstep), "r"(wend), "r"(mask));
-    th = hiw(D);
+        : "+d"(D), "+r"(wb), "=r"(xa), "=r"(xb)
+        : "d"(Md), "d"(Md2), "r"(lstep), "r"(lstep2), "r"(wend2), "r"(mask));
+    xa &= mask;
+    xb &= mask;
 }
 
 // ---- one beam.  pose = the env's BeamPose (global memory), cs = (cos, sin) of the beam's body-frame angle.
@@ -206,13 +218,15 @@ __device__ __forceinline__ float cast_beam(const BeamMap<MS>& bm, const BeamPose
     const unsigned su = hiw(du) & 0x80000000u, sw = hiw(dw) & 0x80000000u;   // sign bits: set = backward
     const unsigned fu1 = (su >> 31) ^ 1u;                         // 1 for beams towards higher u
     // signed slope, distance f to the first line boundary (f = 0.5 + h forward in w, 0.5 - h backward)
-    const double Md = __hiloint2double((int)(hiw(M) ^ su), __double2loint(M));
+    // (quantised to the 2^-32 grid of D, so that every later D +- Md is exact and path-independent)
+    const double Mm = M + kMagic, Mq = Mm - kMagic;
+    const double Md = __hiloint2double((int)(hiw(Mq) ^ su), __double2loint(Mq));
     const double f = __hiloint2double((int)(hiw(o.h) ^ sw), __double2loint(o.h)) + 0.5;
     // D_0 = 2^20 + 64 + U_1 (+ 1 forward): the "+ 1" is one unit of the integer field of the high word
     const double D0 = fma(f, Md, o.ouM);
     double D = __hiloint2double((int)(hiw(D0) + fu1), __double2loint(D0));
     // candidate mask: floor(M) + 2 cells ending (forward) / starting (backward) at the exit cell
-    const unsigned sh = 30u - hiw(M + kMagic);                    // low 5 bits = 30 - floor(M)
+    const unsigned sh = 30u - hiw(Mm);                    // low 5 bits = 30 - floor(M)
     const uint32_t mask = su ? __funnelshift_r(0xffffffffu, 0u, sh) : __funnelshift_l(0u, 0xffffffffu, sh);
     // lines: at most floor(T |dw|) + 2 (the frame stops every beam that would leave the map earlier)
     const int nl = __double2loint(fma(T, adw, 2.0 + 4503599627370496.0));
@@ -221,18 +235,55 @@ __device__ __forceinline__ float cast_beam(const BeamMap<MS>& bm, const BeamPose
     // forward beams read the window that ENDS at the exit cell: words (t >> 5) - 1 and t >> 5
     const typename MS::addr_t wb0 =
         MS::addb(bm.base, (int)(o.line_off - kExpOff) - (int)(fu1 << 2));
-    const typename MS::addr_t wend = MS::addb(wb0, (nl - 1) * lstep);
-    typename MS::addr_t wb = wb0;
-
     float r = rmax;
     int hcell = -1;
-    for (;;) {
-        uint32_t x, th;
-        if constexpr (std::is_same<MS, SmemSpace>::value && !kAux) {
-            hot_lines_smem(D, wb, Md, lstep, wend, mask, x, th);
-        } else {
-            for (;;) {                                            // hot loop: one window per line
-                th = hiw(D);
+    // A candidate in the line with crossing coordinate Dl and window base wl: rebuild the exact span
+    // [entry cell ce, exit cell cx] (the origin cell replaces the entry cell in the first line).
+    // Returns true when the traversal is over (hit within range, or first hit beyond the range).
+    auto candidate = [&](const double Dl, const typename MS::addr_t wl, const uint32_t x) -> bool {
+        const bool first = wl == wb0;
+        const int cx = (int)(hiw(Dl) - kMagicHi - fu1);           // floor(U_{k+1}) + 64
+        const double Dp = Dl - Md;
+        const int ce = first ? o.cu0 + kCellShift : (int)(hiw(Dp) - kMagicHi - fu1);
+        const unsigned n = 31u - (unsigned)abs(cx - ce);
+        const uint32_t xe = x & (su ? __funnelshift_r(0xffffffffu, 0u, n) : __funnelshift_l(0u, 0xffffffffu, n));
+        if (xe == 0u) return false;                               // the extra cell behind the entry: resume
+        // first occupied cell in travel order: lowest bit forward, highest bit backward
+        const int c = su ? cx + (31 - __clz(xe)) : cx - 31 + (__ffs(xe) - 1);
+        double dU;
+        if (c == ce) dU = first ? 0.0 : fabs(Dp - (o.ouM + (double)fu1));              // through the line boundary
+        else dU = fabs((double)(c + (int)(su >> 31)) - (o.ouM - kMagic));              // through the cell's u-face
+        if (dU < T * adu) {
+            r = range_from_du(dU, adu, rho);
+            if (kAux) {
+                const int k = (int)(MS::diffb(wl, wb0) / lstep);                       // lines crossed so far
+                const int lw = sw ? o.l0 - k : o.l0 + k, cu = c - kCellShift;
+                const int Wu = mx ? bm.W : bm.H, Hw = mx ? bm.H : bm.W;
+                const bool outside = (unsigned)cu >= (unsigned)Wu || (unsigned)lw >= (unsigned)Hw;
+                hcell = outside ? -2 : (mx ? lw * bm.W + cu : cu * bm.W + lw);
+            }
+        }
+        return true;                                              // later lines are farther away
+    };
+    if constexpr (std::is_same<MS, SmemSpace>::value && !kAux) {
+        // pairs of lines; an odd line count is rounded up (one line beyond the range: its hits are rejected)
+        const typename MS::addr_t wend2 = MS::addb(wb0, (int)(((unsigned)(nl - 1) | 1u)) * lstep);   // second line of the last pair
+        typename MS::addr_t wb = MS::addb(wb0, -lstep);
+        D -= Md;
+        for (;;) {
+            uint32_t xa, xb;
+            hot_pairs_smem(D, wb, Md, lstep, wend2, mask, xa, xb);
+            if (xa != 0u && candidate(D - Md, MS::addb(wb, -lstep), xa)) break;
+            if (xb != 0u && candidate(D, wb, xb)) break;
+            if (wb == wend2) break;
+        }
+    } else {
+        const typename MS::addr_t wend = MS::addb(wb0, (nl - 1) * lstep);
+        typename MS::addr_t wb = wb0;
+        for (;;) {
+            uint32_t x;
+            for (;;) {                                            // one window per line
+                const uint32_t th = hiw(D);
                 const typename MS::addr_t a = MS::addb(wb, (int)((th >> 5) << 2));
                 x = __funnelshift_r(MS::ld(a), MS::ld4(a), th) & mask;
                 if (kAux) words += 2;
@@ -240,36 +291,10 @@ __device__ __forceinline__ float cast_beam(const BeamMap<MS>& bm, const BeamPose
                 D += Md;
                 wb = MS::addb(wb, lstep);
             }
+            if (x == 0u || candidate(D, wb, x) || wb == wend) break;
+            D += Md;
+            wb = MS::addb(wb, lstep);
         }
-        if (x == 0u) break;                                       // lines exhausted: no hit
-        // exact span of this line: entry cell ce (origin cell in the first line), exit cell cx
-        const bool first = wb == wb0;
-        const int cx = (int)(th - kMagicHi - fu1);                // floor(U_{k+1}) + 64
-        const double Dp = D - Md;
-        const int ce = first ? o.cu0 + kCellShift : (int)(hiw(Dp) - kMagicHi - fu1);
-        const unsigned n = 31u - (unsigned)abs(cx - ce);
-        const uint32_t xe = x & (su ? __funnelshift_r(0xffffffffu, 0u, n) : __funnelshift_l(0u, 0xffffffffu, n));
-        if (xe != 0u) {
-            // first occupied cell in travel order: lowest bit forward, highest bit backward
-            const int c = su ? cx + (31 - __clz(xe)) : cx - 31 + (__ffs(xe) - 1);
-            double dU;
-            if (c == ce) dU = first ? 0.0 : fabs(Dp - (o.ouM + (double)fu1));          // through the line boundary
-            else dU = fabs((double)(c + (int)(su >> 31)) - (o.ouM - kMagic));          // through the cell's u-face
-            if (dU < T * adu) {
-                r = range_from_du(dU, adu, rho);
-                if (kAux) {
-                    const int k = (int)(MS::diffb(wb, wb0) / lstep);                   // lines crossed so far
-                    const int lw = sw ? o.l0 - k : o.l0 + k, cu = c - kCellShift;
-                    const int Wu = mx ? bm.W : bm.H, Hw = mx ? bm.H : bm.W;
-                    const bool outside = (unsigned)cu >= (unsigned)Wu || (unsigned)lw >= (unsigned)Hw;
-                    hcell = outside ? -2 : (mx ? lw * bm.W + cu : cu * bm.W + lw);
-                }
-            }
-            break;                                                // later lines are farther away
-        }
-        if (wb == wend) break;
-        D += Md;
-        wb = MS::addb(wb, lstep);
     }
     if (kAux) *hit = hcell;
     return r;
@@ -335,28 +360,32 @@ __global__ void __launch_bounds__(512, 2) beam_kernel(BeamArgs a) {
     const unsigned nwarps = gridDim.x * warps_per_cta;
     const unsigned ntasks = (total + 31u) >> 5;
     uint32_t words = 0, rays = 0;
+    // (listed env, beam) of this lane's element idx = 32 task + lane, advanced without divisions
+    const unsigned step = nwarps << 5, step_e = step / (unsigned)B, step_j = step - step_e * (unsigned)B;
+    unsigned le = ((warp0 << 5) + lane) / (unsigned)B;
+    unsigned j = ((warp0 << 5) + lane) - le * (unsigned)B;
     for (unsigned task = warp0; task < ntasks; task += nwarps) {
-        const unsigned idx0 = task << 5;
-        unsigned le = idx0 / (unsigned)B;                              // warp-uniform
-        unsigned j = idx0 - le * (unsigned)B + lane;
-        while (j >= (unsigned)B) { j -= B; ++le; }
         if (le < (unsigned)n_env) {
-            const int e = a.list ? a.list[le] : (int)le;
+            const unsigned e = a.list ? (unsigned)a.list[le] : le;
             const BeamPose* pose = a.poses + e;
             const int state = pose->state;
             float r = 0.0f;
             int hit = -2;
             if (state == 0) r = cast_beam<MS, kAux>(bm, pose, s_tab[j], a.robot.T, a.map.rho, a.robot.rmax, &hit, words);
             else if (kAux) { if (state == 1) hit = pose->o[0].l0 * a.map.W + pose->o[0].cu0; ++words; }
-            const size_t o = (size_t)e * B + j;
+            const unsigned o = e * (unsigned)B + j;                    // n_envs * B < 2^31 (fn_sim_create)
             a.out_ranges[o] = r;
             if (kAux && a.out_hit) a.out_hit[o] = hit;
             if (a.ring_obs) {
-                const unsigned long long slot = (ring_head + (unsigned long long)e) % a.ring_cap;
+                unsigned long long slot = ring_head + (unsigned long long)e;   // both < ring_cap
+                if (slot >= a.ring_cap) slot -= a.ring_cap;
                 a.ring_obs[slot * a.ring_row + j] = r;
             }
             ++rays;
         }
+        le += step_e;
+        j += step_j;
+        if (j >= (unsigned)B) { j -= B; ++le; }
     }
     // counters: one atomic per warp
     for (int o = 16; o > 0; o >>= 1) {

@@ -31,9 +31,9 @@ struct Window {
 };                           //     non-finite), 2 = occupied cells in the window: exact test needed
 
 // occupancy bits of row i, columns jb .. jb+31 (bit b = cell jb + b), from the row-packed copy
-__device__ __forceinline__ uint32_t row_bits(const MapDev& m, int i, int jb) {
+__device__ __forceinline__ uint32_t row_bits(const uint32_t* __restrict__ row, int strideR, int i, int jb) {
     const int q = jb + kCellShift;
-    const uint32_t* p = m.row + (size_t)(i + kLineGuard) * m.strideR + (q >> 5);
+    const uint32_t* p = row + (size_t)(i + kLineGuard) * strideR + (q >> 5);
     return __funnelshift_r(__ldg(p), __ldg(p + 1), q);
 }
 __device__ __forceinline__ uint32_t low_bits(int n) {           // n in [0, 32] -> n low bits set
@@ -61,7 +61,7 @@ __device__ __forceinline__ Window footprint_window(const MapDev& m, const RobotD
     uint32_t any = 0;
     for (int jb = w.j0; jb <= w.j1; jb += 32) {
         const uint32_t cm = low_bits(w.j1 - jb + 1);
-        for (int i = w.i0; i <= w.i1; ++i) any |= row_bits(m, i, jb) & cm;
+        for (int i = w.i0; i <= w.i1; ++i) any |= row_bits(m.row, m.strideR, i, jb) & cm;
     }
     w.status = any ? 2 : 0;
     return w;
@@ -69,18 +69,30 @@ __device__ __forceinline__ Window footprint_window(const MapDev& m, const RobotD
 
 // stage 2, warp-cooperative: every lane passes the SAME pose and window; sv = this warp's shared
 // scratch [3][kMaxVerts] doubles (vertex x, vertex y, edge dx/dy).  Returns the flag on every lane.
-__device__ __noinline__ bool warp_collision_exact(const MapDev& m, const RobotDev& rb, double x, double y,
-                                                  double c, double s, int i0, int i1, int j0, int j1,
-                                                  double* sv) {
+// The map / robot fields it needs are passed by value (registers): a by-reference struct argument of a
+// non-inlined function would make every thread of the caller spill the kernel parameters to its stack.
+struct GeoArgs {
+    const uint32_t* row;
+    const double2* verts;
+    double inv_rho;
+    int strideR, V;
+};
+__device__ __forceinline__ GeoArgs geo_args(const MapDev& m, const RobotDev& rb) {
+    GeoArgs g;
+    g.row = m.row; g.verts = rb.verts; g.inv_rho = m.inv_rho; g.strideR = m.strideR; g.V = rb.V;
+    return g;
+}
+__device__ __noinline__ bool warp_collision_exact(const GeoArgs g, double x, double y, double c, double s,
+                                                  int i0, int i1, int j0, int j1, double* sv) {
     const int lane = lane_id();
-    const int V = rb.V;
+    const int V = g.V;
     double* vx = sv;
     double* vy = sv + kMaxVerts;
     double* sl = sv + 2 * kMaxVerts;
-    const double inv = m.inv_rho;
+    const double inv = g.inv_rho;
     __syncwarp();
     for (int k = lane; k < V; k += 32) {
-        const double2 f = rb.verts[k];
+        const double2 f = g.verts[k];
         vx[k] = (x + c * f.x - s * f.y) * inv;
         vy[k] = (y + s * f.x + c * f.y) * inv;
     }
@@ -99,7 +111,7 @@ __device__ __noinline__ bool warp_collision_exact(const MapDev& m, const RobotDe
         bool found = false;
         for (int jb = j0; jb <= j1 && !found; jb += 32) {
             const uint32_t cm = low_bits(j1 - jb + 1);
-            const uint32_t occ = active ? (row_bits(m, i, jb) & cm) : 0u;
+            const uint32_t occ = active ? (row_bits(g.row, g.strideR, i, jb) & cm) : 0u;
             uint32_t touch = 0, inside = 0;
             if (occ) {
                 for (int k = 0; k < V; ++k) {
@@ -143,7 +155,7 @@ __device__ __forceinline__ bool resolve_collisions(const MapDev& m, const RobotD
         const double bc = __shfl_sync(0xffffffffu, c, src), bs = __shfl_sync(0xffffffffu, s, src);
         const int i0 = __shfl_sync(0xffffffffu, w.i0, src), i1 = __shfl_sync(0xffffffffu, w.i1, src);
         const int j0 = __shfl_sync(0xffffffffu, w.j0, src), j1 = __shfl_sync(0xffffffffu, w.j1, src);
-        const bool r = warp_collision_exact(m, rb, bx, by, bc, bs, i0, i1, j0, j1, sv);
+        const bool r = warp_collision_exact(geo_args(m, rb), bx, by, bc, bs, i0, i1, j0, j1, sv);
         if (lane_id() == src) col = r;
     }
     return col;
@@ -192,16 +204,21 @@ struct EnvArgs {
     unsigned long long ring_cap;
     const unsigned long long* ring_head_dev;   // device: slot of env 0's pending row
     int ring_row;
+    int epw;                     // envs per warp (1..32): lanes >= epw idle in the scalar part
     unsigned long long* counters;
 };
 
-constexpr int kEnvBlock = 32;    // one warp per CTA: N/32 CTAs spread the (serial) exact tests over the SMs
+// One warp per CTA, `epw` envs per warp.  The exact polygon tests of a warp's envs run one after the
+// other (each warp-cooperative), so small batches use few envs per warp to spread that serial chain
+// over many warps and SMs (the scalar part is latency-bound there anyway); large batches use all 32
+// lanes for throughput.
+constexpr int kEnvBlock = 32;
 
 __global__ void __launch_bounds__(kEnvBlock) env_step_kernel(EnvArgs a) {
     __shared__ double s_scratch[3 * kMaxVerts];
-    const int e = blockIdx.x * kEnvBlock + threadIdx.x;
+    const int e = blockIdx.x * a.epw + threadIdx.x;
     const int n = a.n;
-    const bool live = e < n;
+    const bool live = (int)threadIdx.x < a.epw && e < n;
     const int el = live ? e : n - 1;                               // idle lanes shadow the last env, write nothing
     // ---- S1: clip ("within the configured bounds") and exact constant-twist step
     const double x = a.states[0 * n + el], y = a.states[1 * n + el], psi = a.states[2 * n + el];
@@ -380,7 +397,7 @@ __global__ void __launch_bounds__(kResetWarps * 32) reset_kernel(ResetArgs a) {
                     const double bc = __shfl_sync(0xffffffffu, ck, t), bs = __shfl_sync(0xffffffffu, sk, t);
                     const int i0 = __shfl_sync(0xffffffffu, w.i0, t), i1 = __shfl_sync(0xffffffffu, w.i1, t);
                     const int j0 = __shfl_sync(0xffffffffu, w.j0, t), j1 = __shfl_sync(0xffffffffu, w.j1, t);
-                    acc = !warp_collision_exact(a.map, a.robot, bx, by, bc, bs, i0, i1, j0, j1, s_scratch[wib]);
+                    acc = !warp_collision_exact(geo_args(a.map, a.robot), bx, by, bc, bs, i0, i1, j0, j1, s_scratch[wib]);
                 }
                 if (acc) { ok = true; src = t; break; }
             }

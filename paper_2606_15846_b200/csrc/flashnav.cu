@@ -294,7 +294,14 @@ extern "C" int fn_sim_create(const fn_map* map, const fn_robot* robot, int n, co
         // stage the packed map in shared memory when both copies + the beam table fit, else read via L2
         const size_t tab = (size_t)robot->B * sizeof(double2);
         const size_t with_map = tab + map->n_words * sizeof(uint32_t);
-        s->use_smem = with_map <= (size_t)max_optin;
+        // the shared-memory kernel recovers the line count from the bit offset: needs T + 34 < S / 2
+        const double Tc = (double)robot->rmax / (double)map->res;
+        const int Smin = 32 * ((map->dev.strideR < map->dev.strideC) ? map->dev.strideR : map->dev.strideC);
+        // ... and addresses bits within a copy by the 20-bit integer field of a double in [2^20, 2^21)
+        const size_t rowBits = (size_t)(map->H + 2 * kLineGuard) * map->dev.strideR * 32;
+        const size_t colBits = (size_t)(map->W + 2 * kLineGuard) * map->dev.strideC * 32;
+        s->use_smem = with_map <= (size_t)max_optin && Tc + 34.0 < 0.5 * (double)Smin &&
+                      rowBits < (1u << 20) && colBits < (1u << 20);
         s->beam_smem = s->use_smem ? with_map : tab;
         if (s->beam_smem > (size_t)max_optin) {
             fn_sim_destroy(s);

@@ -66,7 +66,14 @@ template <class MS>
 struct BeamMap {
     typename MS::addr_t base;        // start of the row copy (true address)
     int H, W, stride4R, stride4C;    // line strides in bytes
+    unsigned rowBytes;               // size of the row copy = offset of the column copy
 };
+// line index (row of the row copy / column of the column copy) of the origin's line
+template <class MS>
+__device__ __forceinline__ int origin_line(const BeamMap<MS>& bm, const BeamOrient& o, bool mx) {
+    return mx ? (int)(o.line_off / (unsigned)bm.stride4R) - kLineGuard
+              : (int)((o.line_off - bm.rowBytes) / (unsigned)bm.stride4C) - kLineGuard;
+}
 
 constexpr unsigned kExpOff = (kMagicHi >> 5) << 2;               // byte offset added by D's exponent bits
 constexpr double kSlowSlope = 30.5;                              // spans of floor(M) + 2 <= 32 cells fit one window
@@ -83,10 +90,14 @@ struct BeamHit {
     int hit;
 };
 
-// Entry distance of a hit -> range in metres (fp32 is ample: tolerance 1e-4 m on <= tens of metres).
-__device__ __forceinline__ float range_from_du(double dU, double adu, float rho) {
-    return __fdividef((float)dU * rho, (float)adu);
+// Entry distance of a hit along u -> range in metres: r = dU * (rho / |du|), the scale in fp32
+// (ample: tolerance 1e-4 m on <= tens of metres).  Every path uses these two, so all agree bit for bit.
+__device__ __forceinline__ float range_scale(double adu, float rho) {
+    float r;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"((float)adu));
+    return __fmul_rn(rho, r);
 }
+__device__ __forceinline__ float range_from_du(double dU, float scale) { return __fmul_rn((float)dU, scale); }
 
 // ---- side path: beams nearly parallel to an axis (or exactly parallel: dw == 0).  Plain per-line walk
 // over 32-bit words; at most T / 30 + 2 lines of up to T cells each.
@@ -103,7 +114,7 @@ __device__ __noinline__ BeamHit cast_beam_slow(const BeamMap<MS> bm, const BeamO
     const double M = adw > 0.0 ? adu / adw : INFINITY;
     const double Tu = T * adu;                                    // travel along u at the range limit
     typename MS::addr_t line = MS::addb(bm.base, (int)o.line_off);
-    int l = o.l0;
+    int l = origin_line(bm, o, mx);
     double E = ou;                                                // entry coordinate of the current line
     for (int k = 0;; ++k) {
         double X = fu ? ou + (f + (double)k) * M : ou - (f + (double)k) * M;        // exit coordinate
@@ -133,7 +144,7 @@ __device__ __noinline__ BeamHit cast_beam_slow(const BeamMap<MS> bm, const BeamO
             else dU = fu ? (double)c - ou : ou - (double)(c + 1);
             if (!(dU < Tu)) break;
             BeamHit h;
-            h.r = range_from_du(dU, adu, rho);
+            h.r = range_from_du(dU, range_scale(adu, rho));
             const bool outside = (unsigned)c >= (unsigned)Wu || (unsigned)l >= (unsigned)Hw;
             h.hit = outside ? -2 : (mx ? l * bm.W + c : c * bm.W + l);
             return h;
@@ -146,51 +157,6 @@ __device__ __noinline__ BeamHit cast_beam_slow(const BeamMap<MS> bm, const BeamO
     BeamHit h;
     h.r = rmax; h.hit = -1;
     return h;
-}
-
-// ---- hot loop for the shared-memory map, in PTX so that exactly one induction variable per quantity
-// survives.  Two lines per trip (their loads and shifts are independent, which hides the shared-memory
-// latency): 2 add.f64 (crossing coordinates), 2 add (line pointers), 2 x [shr (word index), mad (address),
-// 2 ld.shared, shf.r.wrap (window)], one LOP3 ((xa | xb) & mask with the zero test), one setp for
-// the last pair, bra = 17 SASS instructions per two lines.  The loop is rotated (the increments lead),
-// so D and wb are those of the pair's SECOND line when it leaves; xa / xb = masked windows of the
-// pair's first / second line (both zero: lines exhausted).
-__device__ __forceinline__ void hot_pairs_smem(double& D, uint32_t& wb, const double Md, const int lstep,
-                                               const uint32_t wend2, const uint32_t mask, uint32_t& xa, uint32_t& xb) {
-    const double Md2 = Md + Md;
-    const int lstep2 = lstep + lstep;
-    asm volatile(
-        "{\n\t"
-        ".reg .pred ph, pc;\n\t"
-        ".reg .b32 j, a, L, H, lo, hi, wa, xo;\n\t"
-        ".reg .f64 DA;\n\t"
-        "FN_LOOP:\n\t"
-        "add.f64 DA, %0, %4;\n\t"
-        "add.f64 %0, %0, %5;\n\t"
-        "add.s32 wa, %1, %6;\n\t"
-        "add.s32 %1, %1, %7;\n\t"
-        "mov.b64 {lo, hi}, DA;\n\t"
-        "shr.u32 j, hi, 5;\n\t"
-        "mad.lo.u32 a, j, 4, wa;\n\t"
-        "ld.shared.u32 L, [a];\n\t"
-        "ld.shared.u32 H, [a+4];\n\t"
-        "shf.r.wrap.b32 %2, L, H, hi;\n\t"
-        "mov.b64 {lo, hi}, %0;\n\t"
-        "shr.u32 j, hi, 5;\n\t"
-        "mad.lo.u32 a, j, 4, %1;\n\t"
-        "ld.shared.u32 L, [a];\n\t"
-        "ld.shared.u32 H, [a+4];\n\t"
-        "shf.r.wrap.b32 %3, L, H, hi;\n\t"
-        "or.b32 xo, %2, %3;\n\t"
-        "and.b32 xo, xo, %9;\n\t"
-        "setp.eq.u32 ph, xo, 0;\n\t"
-        "setp.ne.and.u32 pc, %1, %8, ph;\n\t"
-        "@pc bra FN_LOOP;\n\t"
-        "}"
-        : "+d"(D), "+r"(wb), "=r"(xa), "=r"(xb)
-        : "d"(Md), "d"(Md2), "r"(lstep), "r"(lstep2), "r"(wend2), "r"(mask));
-    xa &= mask;
-    xb &= mask;
 }
 
 // ---- one beam.  pose = the env's BeamPose (global memory), cs = (cos, sin) of the beam's body-frame angle.
@@ -254,10 +220,10 @@ __device__ __forceinline__ float cast_beam(const BeamMap<MS>& bm, const BeamPose
         if (c == ce) dU = first ? 0.0 : fabs(Dp - (o.ouM + (double)fu1));              // through the line boundary
         else dU = fabs((double)(c + (int)(su >> 31)) - (o.ouM - kMagic));              // through the cell's u-face
         if (dU < T * adu) {
-            r = range_from_du(dU, adu, rho);
+            r = range_from_du(dU, range_scale(adu, rho));
             if (kAux) {
                 const int k = (int)(MS::diffb(wl, wb0) / lstep);                       // lines crossed so far
-                const int lw = sw ? o.l0 - k : o.l0 + k, cu = c - kCellShift;
+                const int l0 = origin_line(bm, o, mx), lw = sw ? l0 - k : l0 + k, cu = c - kCellShift;
                 const int Wu = mx ? bm.W : bm.H, Hw = mx ? bm.H : bm.W;
                 const bool outside = (unsigned)cu >= (unsigned)Wu || (unsigned)lw >= (unsigned)Hw;
                 hcell = outside ? -2 : (mx ? lw * bm.W + cu : cu * bm.W + lw);
@@ -265,19 +231,7 @@ __device__ __forceinline__ float cast_beam(const BeamMap<MS>& bm, const BeamPose
         }
         return true;                                              // later lines are farther away
     };
-    if constexpr (std::is_same<MS, SmemSpace>::value && !kAux) {
-        // pairs of lines; an odd line count is rounded up (one line beyond the range: its hits are rejected)
-        const typename MS::addr_t wend2 = MS::addb(wb0, (int)(((unsigned)(nl - 1) | 1u)) * lstep);   // second line of the last pair
-        typename MS::addr_t wb = MS::addb(wb0, -lstep);
-        D -= Md;
-        for (;;) {
-            uint32_t xa, xb;
-            hot_pairs_smem(D, wb, Md, lstep, wend2, mask, xa, xb);
-            if (xa != 0u && candidate(D - Md, MS::addb(wb, -lstep), xa)) break;
-            if (xb != 0u && candidate(D, wb, xb)) break;
-            if (wb == wend2) break;
-        }
-    } else {
+    {
         const typename MS::addr_t wend = MS::addb(wb0, (nl - 1) * lstep);
         typename MS::addr_t wb = wb0;
         for (;;) {
@@ -297,6 +251,124 @@ __device__ __forceinline__ float cast_beam(const BeamMap<MS>& bm, const BeamPose
         }
     }
     if (kAux) *hit = hcell;
+    return r;
+}
+
+// ---- one beam on the shared-memory map, production path.  Same arithmetic as cast_beam (all of it is
+// exact fixed point, so both agree bit for bit), but the line is carried INSIDE D as well: the integer
+// field of D (20 bits) holds the beam's BIT offset in its copy of the map, 8 * (byte offset of the line) + 64 + cell,
+// and the per-line increment is +-M +- S (S = bits per line).  One DADD per line then advances the
+// crossing coordinate and the line together, the window address is base + 4 * (high word >> 5), and the
+// last line is recognised by the high word itself (line fields differ by >= S - 64 > 0): the hot loop
+// needs no line pointer and no counter.  Two lines per trip (independent loads hide the shared-memory
+// latency): 2 DADD, 2 x [SHF (word index), LEA (address), 2 LDS, SHF.W (window)], one LOP3 for
+// ((xa | xb) & mask) != 0, one ISETP (last pair), BRA = 15 SASS instructions per two lines.
+struct SmemGeo {
+    uint32_t baseR, baseC;   // shared addresses of the row / column copy, - kExpOff
+    float rho;
+    int bitsR, bitsC;        // S: bits per line of the row / column copy
+    float inv_bitsR, inv_bitsC;
+};
+
+__device__ __forceinline__ float cast_beam_smem(const BeamMap<SmemSpace>& bm, const SmemGeo& g,
+                                                const BeamPose* __restrict__ pose, const double2 cs,
+                                                const double T, const float rmax) {
+    const double2 pcs = *reinterpret_cast<const double2*>(&pose->c);
+    const double dx = pcs.x * cs.x - pcs.y * cs.y, dy = pcs.y * cs.x + pcs.x * cs.y;
+    const bool mx = fabs(dx) >= fabs(dy);                         // dominant axis is x
+    const BeamOrient o = pose->o[mx ? 0 : 1];
+    const double du = mx ? dx : dy, dw = mx ? dy : dx;
+    const double adu = fabs(du), adw = fabs(dw);
+    const double r0 = rcp64h(adw);
+    const double r1 = fma(fma(-adw, r0, 1.0), r0, r0);
+    const double M = adu * r1;
+    if (!(M < kSlowSlope)) return cast_beam_slow<SmemSpace>(bm, o, mx, du, dw, T, g.rho, rmax).r;
+    const unsigned su = hiw(du) & 0x80000000u, sw = hiw(dw) & 0x80000000u;   // sign bits: set = backward
+    const unsigned fu1 = (su >> 31) ^ 1u;
+    const double Mm = M + kMagic, Mq = Mm - kMagic;
+    const double Mu = __hiloint2double((int)(hiw(Mq) ^ su), __double2loint(Mq));      // +-M along u
+    const double f = __hiloint2double((int)(hiw(o.h) ^ sw), __double2loint(o.h)) + 0.5;
+    const int S = mx ? g.bitsR : g.bitsC;
+    const double Sd = (double)S;                                  // (uniform: converted once per warp task)
+    const double Md = Mu + __hiloint2double((int)(hiw(Sd) ^ sw), __double2loint(Sd)); // +-M +- S per line
+    const double Md2 = Md + Md;
+    // D of line 0 = 2^20 + bit offset of the origin's line + 64 + U_1 (+ 1 forward)
+    const double D0f = fma(f, Mu, o.ouMS);
+    const double D0 = __hiloint2double((int)(hiw(D0f) + fu1), __double2loint(D0f));
+    const unsigned sh = 30u - hiw(Mm);
+    const uint32_t mask = su ? __funnelshift_r(0xffffffffu, 0u, sh) : __funnelshift_l(0u, 0xffffffffu, sh);
+    // P pairs of lines cover floor(T |dw|) + 2 lines; the frame stops beams that leave the map earlier
+    const double Pd = fma(0.5 * T, adw, 1.5 + 4503599627370496.0) - 4503599627370496.0;
+    double D = D0 - Md;                                           // rotated loop: the increments lead
+    const uint32_t hend = hiw(fma(Pd, Md2, D));                   // high word of the last pair's second line
+    const uint32_t base = (mx ? g.baseR : g.baseC) - (fu1 << 2);  // forward: the window ENDS at the exit cell
+    const float scale = range_scale(adu, g.rho);
+    const double Tu = T * adu;
+    float r = rmax;
+    for (;;) {
+        uint32_t xa, xb;
+        asm volatile(
+            "{\n\t"
+            ".reg .pred ph, pc;\n\t"
+            ".reg .b32 j, a, L, H, lo, hia, hib, xo;\n\t"
+            ".reg .f64 DA;\n\t"
+            "FN_LOOP:\n\t"
+            "add.f64 DA, %0, %3;\n\t"
+            "add.f64 %0, %0, %4;\n\t"
+            "mov.b64 {lo, hia}, DA;\n\t"
+            "shr.u32 j, hia, 5;\n\t"
+            "mad.lo.u32 a, j, 4, %5;\n\t"
+            "ld.shared.u32 L, [a];\n\t"
+            "ld.shared.u32 H, [a+4];\n\t"
+            "shf.r.wrap.b32 %1, L, H, hia;\n\t"
+            "mov.b64 {lo, hib}, %0;\n\t"
+            "shr.u32 j, hib, 5;\n\t"
+            "mad.lo.u32 a, j, 4, %5;\n\t"
+            "ld.shared.u32 L, [a];\n\t"
+            "ld.shared.u32 H, [a+4];\n\t"
+            "shf.r.wrap.b32 %2, L, H, hib;\n\t"
+            "or.b32 xo, %1, %2;\n\t"
+            "and.b32 xo, xo, %7;\n\t"
+            "setp.eq.u32 ph, xo, 0;\n\t"
+            "setp.ne.and.u32 pc, hib, %6, ph;\n\t"
+            "@pc bra FN_LOOP;\n\t"
+            "}"
+            : "+d"(D), "=r"(xa), "=r"(xb)
+            : "d"(Md), "d"(Md2), "r"(base), "r"(hend), "r"(mask));
+        xa &= mask;
+        xb &= mask;
+        // up to two candidate lines, in travel order: the pair's first line (D - Md), then its second (D)
+        uint32_t x = xa;
+        double Dl = D - Md;
+        if (x == 0u) { x = xb; xb = 0u; Dl = D; }
+        bool fin = false;
+#pragma unroll 1
+        while (x != 0u) {
+            // exact span [entry cell ce, exit cell cx] of this line (origin cell in the first line)
+            const uint32_t hl = hiw(Dl);
+            const bool first = hl == hiw(D0);
+            const int cx = (int)(hl - fu1);
+            const double Dp = Dl - Mu;                            // entry crossing, same line field
+            const int ce = first ? (int)hiw(o.ouMS) : (int)(hiw(Dp) - fu1);   // hiw(ouMS) = field of the origin cell
+            const unsigned n = 31u - (unsigned)abs(cx - ce);
+            const uint32_t xe = x & (su ? __funnelshift_r(0xffffffffu, 0u, n) : __funnelshift_l(0u, 0xffffffffu, n));
+            if (xe != 0u) {
+                const int c = su ? cx + (31 - __clz(xe)) : cx - 31 + (__ffs(xe) - 1);
+                // lines crossed: the integer fields of line k and line 0 differ by +-k S +- (cells along u)
+                const int dq = sw ? (int)(hiw(D0) - hl) : (int)(hl - hiw(D0));
+                const int k = __float2int_rd(fmaf((float)dq, mx ? g.inv_bitsR : g.inv_bitsC, 0.5f));
+                const int lf = sw ? -k * S : k * S;                // line field of line k relative to line 0
+                double dU;
+                if (c == ce) dU = first ? 0.0 : fabs((Dp - (double)lf) - (o.ouMS + (double)fu1));
+                else dU = fabs((double)(c + (int)(su >> 31) - lf - (int)kMagicHi) - (o.ouMS - kMagic));
+                if (dU < Tu) r = range_from_du(dU, scale);
+                fin = true;                                       // later lines are farther away
+                break;
+            }
+            x = xb; xb = 0u; Dl = D;                              // the extra cell behind the entry: resume
+        }
+        if (fin || hiw(D) == hend) break;
+    }
     return r;
 }
 
@@ -353,7 +425,12 @@ __global__ void __launch_bounds__(512, 2) beam_kernel(BeamArgs a) {
     if constexpr (kSmem) bm.base = (uint32_t)__cvta_generic_to_shared(s_map);
     else bm.base = (unsigned long long)__cvta_generic_to_global(a.map.row);
     bm.H = a.map.H; bm.W = a.map.W; bm.stride4R = a.map.strideR << 2; bm.stride4C = a.map.strideC << 2;
+    bm.rowBytes = (unsigned)(a.map.H + 2 * kLineGuard) * (unsigned)bm.stride4R;
     const unsigned long long ring_head = a.ring_obs ? *a.ring_head : 0ull;
+    SmemGeo geo;
+    geo.baseR = geo.baseC = 0; geo.rho = a.map.rho; geo.bitsR = bm.stride4R << 3; geo.bitsC = bm.stride4C << 3;
+    geo.inv_bitsR = 1.0f / (float)geo.bitsR; geo.inv_bitsC = 1.0f / (float)geo.bitsC;
+    if constexpr (kSmem) { geo.baseR = bm.base - kExpOff; geo.baseC = geo.baseR + bm.rowBytes; }
 
     const int lane = threadIdx.x & 31;
     const unsigned warp0 = blockIdx.x * warps_per_cta + (threadIdx.x >> 5);
@@ -371,8 +448,11 @@ __global__ void __launch_bounds__(512, 2) beam_kernel(BeamArgs a) {
             const int state = pose->state;
             float r = 0.0f;
             int hit = -2;
-            if (state == 0) r = cast_beam<MS, kAux>(bm, pose, s_tab[j], a.robot.T, a.map.rho, a.robot.rmax, &hit, words);
-            else if (kAux) { if (state == 1) hit = pose->o[0].l0 * a.map.W + pose->o[0].cu0; ++words; }
+            if (state == 0) {
+                if constexpr (kSmem && !kAux) r = cast_beam_smem(bm, geo, pose, s_tab[j], a.robot.T, a.robot.rmax);
+                else r = cast_beam<MS, kAux>(bm, pose, s_tab[j], a.robot.T, a.map.rho, a.robot.rmax, &hit, words);
+            }
+            else if (kAux) { if (state == 1) hit = origin_line(bm, pose->o[0], true) * a.map.W + pose->o[0].cu0; ++words; }
             const unsigned o = e * (unsigned)B + j;                    // n_envs * B < 2^31 (fn_sim_create)
             a.out_ranges[o] = r;
             if (kAux && a.out_hit) a.out_hit[o] = hit;

@@ -34,15 +34,14 @@ constexpr int kLineGuard = 2;      // physical line = l + kLineGuard
 // Per-env sensing pose, written by the env/reset/pose kernels, read by the beam kernel.  The beam
 // kernel walks along the beam's dominant axis "u" (minor axis "w"); both choices are prepared here:
 // o[0]: u = x (row-packed copy, line = row), o[1]: u = y (column-packed copy, line = column).
-constexpr double kMagic = 1048576.0;            // 2^20: a double D in [2^20, 2^21) has ulp 2^-32, its
-constexpr unsigned kMagicHi = 0x41300000u;      // high word is kMagicHi + floor(D - 2^20)
+constexpr double kMagic = 1048576.0;            // 2^20: a double D in [2^20, 2^21) has ulp 2^-32 and its
+constexpr unsigned kMagicHi = 0x41300000u;      // high word is exactly kMagicHi + floor(D - 2^20)
 struct __align__(16) BeamOrient {
     double ouM;              // origin along u, in cells, + kCellShift + kMagic
     double h;                // 0.5 - frac(origin along w): first line boundary at f = 0.5 +- h
+    double ouMS;             // ouM + the BIT offset of the origin's line within its own copy (row / column)
     int cu0;                 // floor(origin along u)
     unsigned line_off;       // byte offset of the origin's line from the start of the row copy
-    int l0;                  // floor(origin along w) = line index
-    int pad_;
 };
 struct __align__(32) BeamPose {
     double c, s;             // cos/sin of the heading

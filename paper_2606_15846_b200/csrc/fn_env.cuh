@@ -177,10 +177,12 @@ __device__ __forceinline__ void write_pose(const MapDev& m, const RobotDev& rb, 
     p.state = !in ? 2 : (occ_global(m, iy, jx) ? 1 : 0);
     const double fx = ox - (double)jx, fy = oy - (double)iy;
     const unsigned rowBytes = (unsigned)(m.H + 2 * kLineGuard) * (unsigned)m.strideR * 4u;
-    p.o[0].ouM = ox + ((double)kCellShift + kMagic); p.o[0].h = 0.5 - fy; p.o[0].cu0 = jx; p.o[0].l0 = iy;
-    p.o[0].line_off = (unsigned)(iy + kLineGuard) * (unsigned)m.strideR * 4u; p.o[0].pad_ = 0;
-    p.o[1].ouM = oy + ((double)kCellShift + kMagic); p.o[1].h = 0.5 - fx; p.o[1].cu0 = iy; p.o[1].l0 = jx;
-    p.o[1].line_off = rowBytes + (unsigned)(jx + kLineGuard) * (unsigned)m.strideC * 4u; p.o[1].pad_ = 0;
+    p.o[0].ouM = ox + ((double)kCellShift + kMagic); p.o[0].h = 0.5 - fy; p.o[0].cu0 = jx;
+    p.o[0].line_off = (unsigned)(iy + kLineGuard) * (unsigned)m.strideR * 4u;
+    p.o[1].ouM = oy + ((double)kCellShift + kMagic); p.o[1].h = 0.5 - fx; p.o[1].cu0 = iy;
+    p.o[1].line_off = rowBytes + (unsigned)(jx + kLineGuard) * (unsigned)m.strideC * 4u;
+    p.o[0].ouMS = p.o[0].ouM + (double)(p.o[0].line_off << 3);
+    p.o[1].ouMS = p.o[1].ouM + (double)((p.o[1].line_off - rowBytes) << 3);
     *out = p;
 }
 

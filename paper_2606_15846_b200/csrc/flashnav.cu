@@ -290,6 +290,10 @@ extern "C" int fn_sim_create(const fn_map* map, const fn_robot* robot, int n, co
     if (e == cudaSuccess) e = cudaMemsetAsync(s->d_epstep, 0, (size_t)n * sizeof(int), s->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(s->d_counters, 0, kNCounters * sizeof(unsigned long long), s->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(s->d_poses, 0xff, (size_t)n * sizeof(BeamPose), s->stream);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(env_step_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                   (int)col_scratch_bytes(FN_MAX_VERTS));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(reset_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                   (int)(kResetWarps * col_scratch_bytes(FN_MAX_VERTS)));
     if (e == cudaSuccess) {
         // stage the packed map in shared memory when both copies + the beam table fit, else read via L2
         const size_t tab = (size_t)robot->B * sizeof(double2);
@@ -375,7 +379,7 @@ extern "C" int fn_step(fn_sim* s, float* states, const float* actions, float dt,
         FN_CUDA(cudaEventRecord(e0, s->stream));
     }
     a.epw = s->n >= 32768 ? 32 : (s->n >= 8192 ? 16 : 8);
-    env_step_kernel<<<(s->n + a.epw - 1) / a.epw, kEnvBlock, 0, s->stream>>>(a);
+    env_step_kernel<<<(s->n + a.epw - 1) / a.epw, kEnvBlock, col_scratch_bytes(s->robot->V), s->stream>>>(a);
     FN_CUDA(cudaGetLastError());
     if (s->prof) FN_CUDA(cudaEventRecord(e1, s->stream));
     if (s->ring) {
@@ -409,7 +413,7 @@ extern "C" int fn_reset(fn_sim* s, float* states, const uint8_t* mask, const uin
     a.counters = s->d_counters;
     int grid = (s->n + kResetWarps - 1) / kResetWarps;
     if (grid > s->num_sms * 4) grid = s->num_sms * 4;
-    reset_kernel<<<grid, kResetWarps * 32, 0, s->stream>>>(a);
+    reset_kernel<<<grid, kResetWarps * 32, kResetWarps * col_scratch_bytes(s->robot->V), s->stream>>>(a);
     FN_CUDA(cudaGetLastError());
     int rc = launch_beams(s, s->d_list, s->d_count, out_ranges);
     if (s->prof && rc == FN_OK) FN_CUDA(cudaEventRecord(e1, s->stream));

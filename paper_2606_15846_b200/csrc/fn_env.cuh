@@ -67,56 +67,89 @@ __device__ __forceinline__ Window footprint_window(const MapDev& m, const RobotD
     return w;
 }
 
-// stage 2, warp-cooperative: every lane passes the SAME pose and window; sv = this warp's shared
-// scratch [3][kMaxVerts] doubles (vertex x, vertex y, edge dx/dy).  Returns the flag on every lane.
-// The map / robot fields it needs are passed by value (registers): a by-reference struct argument of a
-// non-inlined function would make every thread of the caller spill the kernel parameters to its stack.
-struct GeoArgs {
-    const uint32_t* row;
-    const double2* verts;
-    double inv_rho;
-    int strideR, V;
+// stage 2, warp-cooperative over ALL of the warp's poses that need it at once: every such lane puts
+// its transformed vertices and edge slopes into its slot of the warp's shared scratch, the window rows
+// of all slots are numbered consecutively (prefix sum), and the lanes take these (slot, row) items 32
+// at a time.  The cost is ceil(total rows / 32) passes of O(V) each instead of one pass per pose.
+struct ColScratch {          // per warp, in dynamic shared memory
+    double* vx;              // [32][V] vertex x (cells)
+    double* vy;              // [32][V]
+    double* sl;              // [32][V] edge k -> k+1: dx / dy
+    int* pref;               // [32] first item of the slot (exclusive prefix sum of the row counts)
+    int* win;                // [32][4] i0, j0, j1, -
+    unsigned* hit;           // [1] bit per slot
 };
-__device__ __forceinline__ GeoArgs geo_args(const MapDev& m, const RobotDev& rb) {
-    GeoArgs g;
-    g.row = m.row; g.verts = rb.verts; g.inv_rho = m.inv_rho; g.strideR = m.strideR; g.V = rb.V;
-    return g;
+__host__ __device__ inline size_t col_scratch_bytes(int V) { return (size_t)32 * 3 * V * 8 + 32 * 4 + 32 * 16 + 16; }
+__device__ __forceinline__ ColScratch col_scratch(uint8_t* base, int V) {
+    ColScratch cs;
+    cs.vx = reinterpret_cast<double*>(base);
+    cs.vy = cs.vx + 32 * V;
+    cs.sl = cs.vy + 32 * V;
+    cs.pref = reinterpret_cast<int*>(cs.sl + 32 * V);
+    cs.win = cs.pref + 32;
+    cs.hit = reinterpret_cast<unsigned*>(cs.win + 32 * 4);
+    return cs;
 }
-__device__ __noinline__ bool warp_collision_exact(const GeoArgs g, double x, double y, double c, double s,
-                                                  int i0, int i1, int j0, int j1, double* sv) {
+
+// All 32 lanes must call; `need` = this lane's pose needs the exact test (window status 2).
+// Returns true for a lane whose polygon meets an occupied cell (false for lanes that did not need it).
+__device__ __noinline__ bool warp_collisions_exact(const uint32_t* __restrict__ row, const int strideR,
+                                                   const double2* __restrict__ verts, const int V,
+                                                   const double inv, const bool need, const double x, const double y,
+                                                   const double c, const double s, const int i0, const int i1,
+                                                   const int j0, const int j1, const ColScratch cs) {
     const int lane = lane_id();
-    const int V = g.V;
-    double* vx = sv;
-    double* vy = sv + kMaxVerts;
-    double* sl = sv + 2 * kMaxVerts;
-    const double inv = g.inv_rho;
     __syncwarp();
-    for (int k = lane; k < V; k += 32) {
-        const double2 f = g.verts[k];
-        vx[k] = (x + c * f.x - s * f.y) * inv;
-        vy[k] = (y + s * f.x + c * f.y) * inv;
+    if (need) {
+        double* vx = cs.vx + lane * V;
+        double* vy = cs.vy + lane * V;
+        double* sl = cs.sl + lane * V;
+        for (int k = 0; k < V; ++k) {
+            const double2 f = verts[k];
+            vx[k] = (x + c * f.x - s * f.y) * inv;
+            vy[k] = (y + s * f.x + c * f.y) * inv;
+        }
+        for (int k = 0; k < V; ++k) {                              // edge k: vertex k -> k+1
+            const int k1 = k + 1 == V ? 0 : k + 1;
+            const double dy = vy[k1] - vy[k];
+            double r = 0.0;
+            if (dy != 0.0) {                                       // 1 / dy: one Newton step on the 20-bit
+                double r0;                                         // reciprocal (relative error ~2^-40)
+                asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r0) : "d"(dy));
+                r = fma(fma(-dy, r0, 1.0), r0, r0);
+            }
+            sl[k] = (vx[k1] - vx[k]) * r;
+        }
+        cs.win[lane * 4 + 0] = i0; cs.win[lane * 4 + 1] = j0; cs.win[lane * 4 + 2] = j1;
     }
+    const int rows = need ? i1 - i0 + 1 : 0;
+    int incl = rows;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += v; }
+    const int total = __shfl_sync(0xffffffffu, incl, 31);
+    cs.pref[lane] = incl - rows;
+    if (lane == 0) *cs.hit = 0u;
     __syncwarp();
-    for (int k = lane; k < V; k += 32) {                           // edge k: vertex k -> k+1
-        const int k1 = k + 1 == V ? 0 : k + 1;
-        const double dy = vy[k1] - vy[k];
-        sl[k] = dy != 0.0 ? (vx[k1] - vx[k]) / dy : 0.0;
-    }
-    __syncwarp();
-    const int rows = i1 - i0 + 1;
-    for (int r0 = 0; r0 < rows; r0 += 32) {
-        const int i = i0 + r0 + lane;
-        const bool active = i <= i1;
-        const double ylo_s = (double)i, yhi_s = ylo_s + 1.0, yc = ylo_s + 0.5;
-        bool found = false;
-        for (int jb = j0; jb <= j1 && !found; jb += 32) {
-            const uint32_t cm = low_bits(j1 - jb + 1);
-            const uint32_t occ = active ? (row_bits(g.row, g.strideR, i, jb) & cm) : 0u;
-            uint32_t touch = 0, inside = 0;
-            if (occ) {
-                for (int k = 0; k < V; ++k) {
-                    const int k1 = k + 1 == V ? 0 : k + 1;
-                    const double px = vx[k], py = vy[k], qx = vx[k1], qy = vy[k1], sk = sl[k];
+    for (int t0 = 0; t0 < total; t0 += 32) {
+        const int t = t0 + lane;
+        if (t < total) {
+            int slot = 0;                                          // last slot whose first item is <= t
+#pragma unroll
+            for (int st = 16; st > 0; st >>= 1) if (cs.pref[slot + st] <= t) slot += st;
+            const int i = cs.win[slot * 4] + (t - cs.pref[slot]);
+            const int sj0 = cs.win[slot * 4 + 1], sj1 = cs.win[slot * 4 + 2];
+            const double* vx = cs.vx + slot * V;
+            const double* vy = cs.vy + slot * V;
+            const double* sl = cs.sl + slot * V;
+            const double ylo_s = (double)i, yhi_s = ylo_s + 1.0, yc = ylo_s + 0.5;
+            bool found = false;
+            for (int jb = sj0; jb <= sj1 && !found; jb += 32) {
+                const uint32_t occ = row_bits(row, strideR, i, jb) & low_bits(sj1 - jb + 1);
+                if (occ == 0u) continue;
+                uint32_t touch = 0, inside = 0;
+                double px = vx[V - 1], py = vy[V - 1];
+                for (int k = 0; k < V; ++k) {                      // edge k-1: vertex k-1 -> k
+                    const double qx = vx[k], qy = vy[k], sk = sl[k == 0 ? V - 1 : k - 1];
                     const double elo = fmin(py, qy), ehi = fmax(py, qy);
                     if (ehi >= ylo_s && elo <= yhi_s) {            // the edge meets the closed strip
                         const double exlo = fmin(px, qx), exhi = fmax(px, qx);
@@ -133,31 +166,25 @@ __device__ __noinline__ bool warp_collision_exact(const GeoArgs g, double x, dou
                         const int nleft = __double2int_ru(xc - 0.5) - jb;
                         inside ^= low_bits(min(max(nleft, 0), 32));
                     }
+                    px = qx; py = qy;
                 }
+                found = (occ & (touch | inside)) != 0u;
             }
-            found = (occ & (touch | inside)) != 0u;
+            if (found) atomicOr(cs.hit, 1u << slot);
         }
-        if (__any_sync(0xffffffffu, found)) return true;
     }
-    return false;
+    __syncwarp();
+    return need && ((*cs.hit >> lane) & 1u);
 }
 
-// Resolves the exact test for every lane whose window needs it (status 2), one pose at a time with
-// the whole warp cooperating.  All 32 lanes must call; returns this lane's collision flag.
+// Per-lane collision flag from the window status (all 32 lanes must call).
 __device__ __forceinline__ bool resolve_collisions(const MapDev& m, const RobotDev& rb, const Window& w,
-                                                   double x, double y, double c, double s, double* sv) {
+                                                   double x, double y, double c, double s, const ColScratch cs) {
+    const bool need = w.status == 2;
     bool col = w.status == 1;
-    unsigned need = __ballot_sync(0xffffffffu, w.status == 2);
-    while (need) {
-        const int src = __ffs(need) - 1;
-        need &= need - 1;
-        const double bx = __shfl_sync(0xffffffffu, x, src), by = __shfl_sync(0xffffffffu, y, src);
-        const double bc = __shfl_sync(0xffffffffu, c, src), bs = __shfl_sync(0xffffffffu, s, src);
-        const int i0 = __shfl_sync(0xffffffffu, w.i0, src), i1 = __shfl_sync(0xffffffffu, w.i1, src);
-        const int j0 = __shfl_sync(0xffffffffu, w.j0, src), j1 = __shfl_sync(0xffffffffu, w.j1, src);
-        const bool r = warp_collision_exact(geo_args(m, rb), bx, by, bc, bs, i0, i1, j0, j1, sv);
-        if (lane_id() == src) col = r;
-    }
+    if (__any_sync(0xffffffffu, need))
+        col |= warp_collisions_exact(m.row, m.strideR, rb.verts, rb.V, m.inv_rho, need, x, y, c, s,
+                                     w.i0, w.i1, w.j0, w.j1, cs);
     return col;
 }
 
@@ -217,7 +244,8 @@ struct EnvArgs {
 constexpr int kEnvBlock = 32;
 
 __global__ void __launch_bounds__(kEnvBlock) env_step_kernel(EnvArgs a) {
-    __shared__ double s_scratch[3 * kMaxVerts];
+    extern __shared__ __align__(16) uint8_t s_dyn[];
+    const ColScratch scratch = col_scratch(s_dyn, a.robot.V);
     const int e = blockIdx.x * a.epw + threadIdx.x;
     const int n = a.n;
     const bool live = (int)threadIdx.x < a.epw && e < n;
@@ -251,7 +279,7 @@ __global__ void __launch_bounds__(kEnvBlock) env_step_kernel(EnvArgs a) {
     // ---- S3
     Window win = footprint_window(a.map, a.robot, (double)xf, (double)yf, c1, s1);
     if (!live) win.status = 0;
-    const bool col = resolve_collisions(a.map, a.robot, win, (double)xf, (double)yf, c1, s1, s_scratch);
+    const bool col = resolve_collisions(a.map, a.robot, win, (double)xf, (double)yf, c1, s1, scratch);
     if (!live) return;
     // ---- S4: goal obs, reward Eq. (1), done
     const double gdx = (double)gxf - (double)xf, gdy = (double)gyf - (double)yf;
@@ -361,8 +389,9 @@ struct ResetArgs {
 constexpr int kResetWarps = 4;
 
 __global__ void __launch_bounds__(kResetWarps * 32) reset_kernel(ResetArgs a) {
-    __shared__ double s_scratch[kResetWarps][3 * kMaxVerts];
+    extern __shared__ __align__(16) uint8_t s_dyn[];
     const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const ColScratch scratch = col_scratch(s_dyn + (size_t)wib * col_scratch_bytes(a.robot.V), a.robot.V);
     const int count = *a.count_dev;
     const int n = a.n;
     const double rho = (double)a.map.rho;
@@ -386,23 +415,14 @@ __global__ void __launch_bounds__(kResetWarps * 32) reset_kernel(ResetArgs a) {
             const float pk = __fmaf_rn(u24_at(sigma, 3ull * k + 2ull), two_pi_f, -pi_f);
             double sk, ck;
             sincos((double)pk, &sk, &ck);
-            const Window w = footprint_window(a.map, a.robot, (double)xk, (double)yk, ck, sk);
+            Window w = footprint_window(a.map, a.robot, (double)xk, (double)yk, ck, sk);
+            // attempts after the first one that is free without an exact test cannot win: skip their tests
             const unsigned free_m = __ballot_sync(0xffffffffu, w.status == 0);
-            unsigned cand = free_m | __ballot_sync(0xffffffffu, w.status == 2);
-            int src = 31;                                          // exhausted: keep the last candidate
-            while (cand) {
-                const int t = __ffs(cand) - 1;
-                cand &= cand - 1;
-                bool acc = (free_m >> t) & 1u;
-                if (!acc) {
-                    const double bx = __shfl_sync(0xffffffffu, (double)xk, t), by = __shfl_sync(0xffffffffu, (double)yk, t);
-                    const double bc = __shfl_sync(0xffffffffu, ck, t), bs = __shfl_sync(0xffffffffu, sk, t);
-                    const int i0 = __shfl_sync(0xffffffffu, w.i0, t), i1 = __shfl_sync(0xffffffffu, w.i1, t);
-                    const int j0 = __shfl_sync(0xffffffffu, w.j0, t), j1 = __shfl_sync(0xffffffffu, w.j1, t);
-                    acc = !warp_collision_exact(geo_args(a.map, a.robot), bx, by, bc, bs, i0, i1, j0, j1, s_scratch[wib]);
-                }
-                if (acc) { ok = true; src = t; break; }
-            }
+            if (free_m && lane > __ffs(free_m) - 1) w.status = 1;
+            const bool col = resolve_collisions(a.map, a.robot, w, (double)xk, (double)yk, ck, sk, scratch);
+            const unsigned acc_m = __ballot_sync(0xffffffffu, !col);
+            ok = acc_m != 0u;
+            const int src = ok ? __ffs(acc_m) - 1 : 31;           // exhausted: keep the last candidate
             x = __shfl_sync(0xffffffffu, xk, src); y = __shfl_sync(0xffffffffu, yk, src);
             psi = __shfl_sync(0xffffffffu, pk, src);
             sp = __shfl_sync(0xffffffffu, sk, src); cp = __shfl_sync(0xffffffffu, ck, src);

@@ -40,13 +40,14 @@ __device__ __forceinline__ uint32_t low_bits(int n) {           // n in [0, 32] 
     return n >= 32 ? 0xffffffffu : ((1u << n) - 1u);
 }
 
-// stage 1, one thread per pose
-__device__ __forceinline__ Window footprint_window(const MapDev& m, const RobotDev& rb, double x, double y,
-                                                   double c, double s) {
+// stage 1, one thread per pose.  verts = the footprint vertices (a shared-memory copy in the kernels).
+// The window rows are read eight at a time so that their (independent, mostly L2-latency) loads overlap.
+__device__ __forceinline__ Window footprint_window(const MapDev& m, const double2* __restrict__ verts, const int V,
+                                                   double x, double y, double c, double s) {
     const double inv = m.inv_rho;
     double xmin = INFINITY, xmax = -INFINITY, ymin = INFINITY, ymax = -INFINITY;
-    for (int k = 0; k < rb.V; ++k) {
-        const double2 f = rb.verts[k];
+    for (int k = 0; k < V; ++k) {
+        const double2 f = verts[k];
         const double wx = (x + c * f.x - s * f.y) * inv, wy = (y + s * f.x + c * f.y) * inv;
         xmin = fmin(xmin, wx); xmax = fmax(xmax, wx);
         ymin = fmin(ymin, wy); ymax = fmax(ymax, wy);
@@ -61,7 +62,15 @@ __device__ __forceinline__ Window footprint_window(const MapDev& m, const RobotD
     uint32_t any = 0;
     for (int jb = w.j0; jb <= w.j1; jb += 32) {
         const uint32_t cm = low_bits(w.j1 - jb + 1);
-        for (int i = w.i0; i <= w.i1; ++i) any |= row_bits(m.row, m.strideR, i, jb) & cm;
+        for (int i = w.i0; i <= w.i1; i += 8) {
+            uint32_t v[8];
+#pragma unroll
+            for (int u = 0; u < 8; ++u) v[u] = row_bits(m.row, m.strideR, min(i + u, w.i1), jb);
+#pragma unroll
+            for (int u = 0; u < 8; ++u) any |= v[u];
+        }
+        any &= cm;
+        if (any) break;
     }
     w.status = any ? 2 : 0;
     return w;
@@ -78,14 +87,16 @@ struct ColScratch {          // per warp, in dynamic shared memory
     int* pref;               // [32] first item of the slot (exclusive prefix sum of the row counts)
     int* win;                // [32][4] i0, j0, j1, -
     unsigned* hit;           // [1] bit per slot
+    double2* verts;          // [V] copy of the footprint vertices (body frame, metres)
 };
-__host__ __device__ inline size_t col_scratch_bytes(int V) { return (size_t)32 * 3 * V * 8 + 32 * 4 + 32 * 16 + 16; }
+__host__ __device__ inline size_t col_scratch_bytes(int V) { return (size_t)32 * 3 * V * 8 + (size_t)V * 16 + 32 * 4 + 32 * 16 + 16; }
 __device__ __forceinline__ ColScratch col_scratch(uint8_t* base, int V) {
     ColScratch cs;
     cs.vx = reinterpret_cast<double*>(base);
     cs.vy = cs.vx + 32 * V;
     cs.sl = cs.vy + 32 * V;
-    cs.pref = reinterpret_cast<int*>(cs.sl + 32 * V);
+    cs.verts = reinterpret_cast<double2*>(cs.sl + 32 * V);
+    cs.pref = reinterpret_cast<int*>(cs.verts + V);
     cs.win = cs.pref + 32;
     cs.hit = reinterpret_cast<unsigned*>(cs.win + 32 * 4);
     return cs;
@@ -183,7 +194,7 @@ __device__ __forceinline__ bool resolve_collisions(const MapDev& m, const RobotD
     const bool need = w.status == 2;
     bool col = w.status == 1;
     if (__any_sync(0xffffffffu, need))
-        col |= warp_collisions_exact(m.row, m.strideR, rb.verts, rb.V, m.inv_rho, need, x, y, c, s,
+        col |= warp_collisions_exact(m.row, m.strideR, cs.verts, rb.V, m.inv_rho, need, x, y, c, s,
                                      w.i0, w.i1, w.j0, w.j1, cs);
     return col;
 }
@@ -246,6 +257,8 @@ constexpr int kEnvBlock = 32;
 __global__ void __launch_bounds__(kEnvBlock) env_step_kernel(EnvArgs a) {
     extern __shared__ __align__(16) uint8_t s_dyn[];
     const ColScratch scratch = col_scratch(s_dyn, a.robot.V);
+    for (int k = threadIdx.x; k < a.robot.V; k += kEnvBlock) scratch.verts[k] = a.robot.verts[k];
+    __syncwarp();
     const int e = blockIdx.x * a.epw + threadIdx.x;
     const int n = a.n;
     const bool live = (int)threadIdx.x < a.epw && e < n;
@@ -253,6 +266,9 @@ __global__ void __launch_bounds__(kEnvBlock) env_step_kernel(EnvArgs a) {
     // ---- S1: clip ("within the configured bounds") and exact constant-twist step
     const double x = a.states[0 * n + el], y = a.states[1 * n + el], psi = a.states[2 * n + el];
     const float gxf = a.states[6 * n + el], gyf = a.states[7 * n + el];
+    const float dp = a.d_prev[el];                                 // (loaded early: off the critical path)
+    const int es = a.ep_step[el];
+    const bool forced = a.reset_mask[el] != 0;
     const int A = a.robot.A;
     float avx = a.actions[(size_t)el * A], avy = 0.0f, aw;
     if (a.robot.drive == 0) aw = a.actions[(size_t)el * A + 1];
@@ -277,7 +293,7 @@ __global__ void __launch_bounds__(kEnvBlock) env_step_kernel(EnvArgs a) {
     double s1, c1;
     sincos((double)psif, &s1, &c1);
     // ---- S3
-    Window win = footprint_window(a.map, a.robot, (double)xf, (double)yf, c1, s1);
+    Window win = footprint_window(a.map, scratch.verts, a.robot.V, (double)xf, (double)yf, c1, s1);
     if (!live) win.status = 0;
     const bool col = resolve_collisions(a.map, a.robot, win, (double)xf, (double)yf, c1, s1, scratch);
     if (!live) return;
@@ -285,14 +301,11 @@ __global__ void __launch_bounds__(kEnvBlock) env_step_kernel(EnvArgs a) {
     const double gdx = (double)gxf - (double)xf, gdy = (double)gyf - (double)yf;
     const float d = (float)sqrt(gdx * gdx + gdy * gdy);
     const float alpha = (float)wrap_pi(atan2(gdy, gdx) - (double)psif);
-    const float dp = a.d_prev[e];
-    const int es = a.ep_step[e];
     const bool reached = d < a.task.goal_tol;
     const float r = col ? a.task.r_collision
                         : reached ? a.task.r_success
                                   : (float)((double)a.task.c_progress * ((double)dp - (double)d));
     const bool limit = a.task.max_episode_steps > 0 && es + 1 >= a.task.max_episode_steps;
-    const bool forced = a.reset_mask[e] != 0;
     const uint8_t done = (col || reached || limit || forced) ? 1 : 0;
     a.states[0 * n + e] = xf; a.states[1 * n + e] = yf; a.states[2 * n + e] = psif;
     a.states[3 * n + e] = avx; a.states[4 * n + e] = avy; a.states[5 * n + e] = aw;
@@ -392,6 +405,8 @@ __global__ void __launch_bounds__(kResetWarps * 32) reset_kernel(ResetArgs a) {
     extern __shared__ __align__(16) uint8_t s_dyn[];
     const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const ColScratch scratch = col_scratch(s_dyn + (size_t)wib * col_scratch_bytes(a.robot.V), a.robot.V);
+    for (int k = lane; k < a.robot.V; k += 32) scratch.verts[k] = a.robot.verts[k];
+    __syncwarp();
     const int count = *a.count_dev;
     const int n = a.n;
     const double rho = (double)a.map.rho;
@@ -415,7 +430,7 @@ __global__ void __launch_bounds__(kResetWarps * 32) reset_kernel(ResetArgs a) {
             const float pk = __fmaf_rn(u24_at(sigma, 3ull * k + 2ull), two_pi_f, -pi_f);
             double sk, ck;
             sincos((double)pk, &sk, &ck);
-            Window w = footprint_window(a.map, a.robot, (double)xk, (double)yk, ck, sk);
+            Window w = footprint_window(a.map, scratch.verts, a.robot.V, (double)xk, (double)yk, ck, sk);
             // attempts after the first one that is free without an exact test cannot win: skip their tests
             const unsigned free_m = __ballot_sync(0xffffffffu, w.status == 0);
             if (free_m && lane > __ffs(free_m) - 1) w.status = 1;

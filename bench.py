@@ -225,24 +225,31 @@ def run_ours(args):
         step(t)
     barrier()
     c0 = sim.counters()
-    sim.profile(True)
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
+    # ---- timed region: K steps, L2 flushed between them (outside the per-step events)
     ev0 = [torch.cuda.Event(enable_timing=True) for _ in range(K)]
     ev1 = [torch.cuda.Event(enable_timing=True) for _ in range(K)]
     for k in range(K):
-        flush.fill_(k & 0xff)                      # L2 flush between timed iterations (outside the events)
+        flush.fill_(k & 0xff)
         ev0[k].record()
         step(Wm + k)
         ev1[k].record()
     barrier()
     clocks = sampler.stop() if rank == 0 else None
     per_step_ms = np.array([ev0[k].elapsed_time(ev1[k]) for k in range(K)])
-    prof = sim.profile_read()
-    sim.profile(False)
     c1 = sim.counters()
     total_ms = float(per_step_ms.sum())
+    # ---- per-kernel durations: the same K steps again with the library's events around each kernel
+    # (a separate pass: an event between two kernels keeps the second from starting under the first)
+    sim.profile(True)
+    for k in range(K):
+        flush.fill_(k & 0xff)
+        step(Wm + k)
+    barrier()
+    prof = sim.profile_read()
+    sim.profile(False)
 
     # steady state (no L2 flush, back to back): information only
     s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)

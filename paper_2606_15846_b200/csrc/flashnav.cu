@@ -4,6 +4,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <type_traits>
@@ -347,14 +348,20 @@ static int launch_beams(fn_sim* s, const int* list, const int* count_dev, float*
     b.list = list; b.count_dev = count_dev; b.n_all = s->n; b.out_ranges = out_ranges; b.out_hit = s->aux_hit;
     b.ring_obs = s->ring; b.ring_cap = s->ring_cap ? s->ring_cap : 1; b.ring_head = s->d_ring_head; b.ring_row = ring_row_floats(s);
     b.counters = s->d_counters;
-    const dim3 grid(s->beam_grid), block(512);
     const bool aux = s->count_words || s->aux_hit;
+    // programmatic dependent launch: the kernel may start (and stage the map) under its predecessor
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(s->beam_grid); cfg.blockDim = dim3(512); cfg.dynamicSmemBytes = s->beam_smem; cfg.stream = s->stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = getenv("FN_DBG_NOPDL") ? 0 : 1;
     if (s->use_smem) {
-        if (aux) beam_kernel<true, true><<<grid, block, s->beam_smem, s->stream>>>(b);
-        else beam_kernel<true, false><<<grid, block, s->beam_smem, s->stream>>>(b);
+        if (aux) FN_CUDA(cudaLaunchKernelEx(&cfg, beam_kernel<true, true>, b));
+        else FN_CUDA(cudaLaunchKernelEx(&cfg, beam_kernel<true, false>, b));
     } else {
-        if (aux) beam_kernel<false, true><<<grid, block, s->beam_smem, s->stream>>>(b);
-        else beam_kernel<false, false><<<grid, block, s->beam_smem, s->stream>>>(b);
+        if (aux) FN_CUDA(cudaLaunchKernelEx(&cfg, beam_kernel<false, true>, b));
+        else FN_CUDA(cudaLaunchKernelEx(&cfg, beam_kernel<false, false>, b));
     }
     FN_CUDA(cudaGetLastError());
     return FN_OK;

@@ -389,49 +389,23 @@ struct BeamArgs {
     unsigned long long* counters;
 };
 
-// Persistent kernel: each CTA stages both packed copies of the map and the beam table in shared
-// memory (kSmem) or reads the map through L1/L2 (global path), then its warps take 32 consecutive
-// (env, beam) pairs at a time: adjacent lanes = adjacent beams of one env, so a warp's loads mostly hit
-// the same or neighbouring words (broadcast) and its lanes run similar trip counts.
-// kAux = instrumented variant: hit-cell output, map-word counter.
-template <bool kSmem, bool kAux>
-__global__ void __launch_bounds__(512, 2) beam_kernel(BeamArgs a) {
-    extern __shared__ __align__(16) uint8_t smem_raw[];
+// Programmatic dependent launch (PDL): a kernel launched with the programmatic-stream-serialization
+// attribute may start while its predecessor in the stream still runs; griddepcontrol.wait blocks until
+// that predecessor has completed and its memory is visible.  The beam kernel stages the map and the
+// beam table (constants) BEFORE the wait, i.e. under the env-step / reset kernel.
+__device__ __forceinline__ void griddep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void griddep_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;"); }
+
+
+// The warps of the (persistent) grid take 32 consecutive (env, beam) pairs at a time: adjacent lanes =
+// adjacent beams of one env, so a warp's loads mostly hit the same or neighbouring words (broadcast)
+// and its lanes run similar trip counts.  kFast = production shared-memory traversal (cast_beam_smem).
+template <class MS, bool kFast, bool kAux>
+__device__ __forceinline__ void run_beam_tasks(const BeamArgs& a, const BeamMap<MS>& bm, const SmemGeo& geo,
+                                               const double2* s_tab, const int n_env, const unsigned total) {
     const int B = a.robot.B;
-    const int n_env = a.count_dev ? *a.count_dev : a.n_all;
-    const unsigned total = (unsigned)n_env * (unsigned)B;
     const int warps_per_cta = blockDim.x >> 5;
-    if ((unsigned)blockIdx.x * warps_per_cta * 32u >= total) return;      // nothing for this CTA: skip staging
-    const int mapWords = (a.map.H + 2 * kLineGuard) * a.map.strideR + (a.map.W + 2 * kLineGuard) * a.map.strideC;
-    double2* s_tab = reinterpret_cast<double2*>(smem_raw);
-    uint32_t* s_map = reinterpret_cast<uint32_t*>(smem_raw + (size_t)B * sizeof(double2));
-    for (int i = threadIdx.x; i < B; i += blockDim.x) s_tab[i] = a.robot.beam_cs[i];
-    if (kSmem) {
-        const uint4* src = reinterpret_cast<const uint4*>(a.map.row);      // row and col copies are contiguous
-        uint4* dst = reinterpret_cast<uint4*>(s_map);
-        const int n4 = (mapWords + 3) / 4;
-        int i = threadIdx.x;
-        for (; i + 3 * (int)blockDim.x < n4; i += 4 * blockDim.x) {         // 4 loads in flight per thread
-            const uint4 v0 = __ldg(src + i), v1 = __ldg(src + i + blockDim.x);
-            const uint4 v2 = __ldg(src + i + 2 * blockDim.x), v3 = __ldg(src + i + 3 * blockDim.x);
-            dst[i] = v0; dst[i + blockDim.x] = v1; dst[i + 2 * blockDim.x] = v2; dst[i + 3 * blockDim.x] = v3;
-        }
-        for (; i < n4; i += blockDim.x) dst[i] = __ldg(src + i);
-    }
-    __syncthreads();
-
-    using MS = typename std::conditional<kSmem, SmemSpace, GlobalSpace>::type;
-    BeamMap<MS> bm;
-    if constexpr (kSmem) bm.base = (uint32_t)__cvta_generic_to_shared(s_map);
-    else bm.base = (unsigned long long)__cvta_generic_to_global(a.map.row);
-    bm.H = a.map.H; bm.W = a.map.W; bm.stride4R = a.map.strideR << 2; bm.stride4C = a.map.strideC << 2;
-    bm.rowBytes = (unsigned)(a.map.H + 2 * kLineGuard) * (unsigned)bm.stride4R;
     const unsigned long long ring_head = a.ring_obs ? *a.ring_head : 0ull;
-    SmemGeo geo;
-    geo.baseR = geo.baseC = 0; geo.rho = a.map.rho; geo.bitsR = bm.stride4R << 3; geo.bitsC = bm.stride4C << 3;
-    geo.inv_bitsR = 1.0f / (float)geo.bitsR; geo.inv_bitsC = 1.0f / (float)geo.bitsC;
-    if constexpr (kSmem) { geo.baseR = bm.base - kExpOff; geo.baseC = geo.baseR + bm.rowBytes; }
-
     const int lane = threadIdx.x & 31;
     const unsigned warp0 = blockIdx.x * warps_per_cta + (threadIdx.x >> 5);
     const unsigned nwarps = gridDim.x * warps_per_cta;
@@ -449,10 +423,12 @@ __global__ void __launch_bounds__(512, 2) beam_kernel(BeamArgs a) {
             float r = 0.0f;
             int hit = -2;
             if (state == 0) {
-                if constexpr (kSmem && !kAux) r = cast_beam_smem(bm, geo, pose, s_tab[j], a.robot.T, a.robot.rmax);
+                if constexpr (kFast) r = cast_beam_smem(bm, geo, pose, s_tab[j], a.robot.T, a.robot.rmax);
                 else r = cast_beam<MS, kAux>(bm, pose, s_tab[j], a.robot.T, a.map.rho, a.robot.rmax, &hit, words);
+            } else if (kAux) {
+                if (state == 1) hit = origin_line(bm, pose->o[0], true) * a.map.W + pose->o[0].cu0;
+                ++words;
             }
-            else if (kAux) { if (state == 1) hit = origin_line(bm, pose->o[0], true) * a.map.W + pose->o[0].cu0; ++words; }
             const unsigned o = e * (unsigned)B + j;                    // n_envs * B < 2^31 (fn_sim_create)
             a.out_ranges[o] = r;
             if (kAux && a.out_hit) a.out_hit[o] = hit;
@@ -475,6 +451,57 @@ __global__ void __launch_bounds__(512, 2) beam_kernel(BeamArgs a) {
     if (lane == 0) {
         atomicAdd(&a.counters[kRays], (unsigned long long)rays);
         if (kAux && a.count_words) atomicAdd(&a.counters[kWords], (unsigned long long)words);
+    }
+}
+
+// Persistent kernel (grid = SMs x resident CTAs).  kSmem: each CTA stages both packed copies of the map
+// and the beam table in shared memory -- constants, so this happens BEFORE the dependency wait, under
+// the env-step / reset kernel that precedes it in the stream.
+// kAux = instrumented variant: hit-cell output, map-word counter.
+template <bool kSmem, bool kAux>
+__global__ void __launch_bounds__(512, 2) beam_kernel(BeamArgs a) {
+    extern __shared__ __align__(16) uint8_t smem_raw[];
+    const int B = a.robot.B;
+    constexpr bool stage = kSmem;
+    const int mapWords = (a.map.H + 2 * kLineGuard) * a.map.strideR + (a.map.W + 2 * kLineGuard) * a.map.strideC;
+    double2* s_tab = reinterpret_cast<double2*>(smem_raw);
+    uint32_t* s_map = reinterpret_cast<uint32_t*>(smem_raw + (size_t)B * sizeof(double2));
+    for (int i = threadIdx.x; i < B; i += blockDim.x) s_tab[i] = a.robot.beam_cs[i];
+    if (stage) {
+        const uint4* src = reinterpret_cast<const uint4*>(a.map.row);      // row and col copies are contiguous
+        uint4* dst = reinterpret_cast<uint4*>(s_map);
+        const int n4 = (mapWords + 3) / 4;
+        int i = threadIdx.x;
+        for (; i + 3 * (int)blockDim.x < n4; i += 4 * blockDim.x) {         // 4 loads in flight per thread
+            const uint4 v0 = __ldg(src + i), v1 = __ldg(src + i + blockDim.x);
+            const uint4 v2 = __ldg(src + i + 2 * blockDim.x), v3 = __ldg(src + i + 3 * blockDim.x);
+            dst[i] = v0; dst[i + blockDim.x] = v1; dst[i + 2 * blockDim.x] = v2; dst[i + 3 * blockDim.x] = v3;
+        }
+        for (; i < n4; i += blockDim.x) dst[i] = __ldg(src + i);
+    }
+    __syncthreads();
+    griddep_wait();                                                // poses / list / count come from the previous kernel
+    const int n_env = a.count_dev ? *a.count_dev : a.n_all;
+    const unsigned total = (unsigned)n_env * (unsigned)B;
+    if ((unsigned)blockIdx.x * (blockDim.x >> 5) * 32u >= total) return;   // nothing for this CTA
+
+    SmemGeo geo;
+    geo.baseR = geo.baseC = 0; geo.rho = a.map.rho; geo.bitsR = a.map.strideR << 5; geo.bitsC = a.map.strideC << 5;
+    geo.inv_bitsR = 1.0f / (float)geo.bitsR; geo.inv_bitsC = 1.0f / (float)geo.bitsC;
+    const unsigned rowBytes = (unsigned)(a.map.H + 2 * kLineGuard) * (unsigned)(a.map.strideR << 2);
+    if (stage) {
+        BeamMap<SmemSpace> bm;
+        bm.base = (uint32_t)__cvta_generic_to_shared(s_map);
+        bm.H = a.map.H; bm.W = a.map.W; bm.stride4R = a.map.strideR << 2; bm.stride4C = a.map.strideC << 2;
+        bm.rowBytes = rowBytes;
+        geo.baseR = bm.base - kExpOff; geo.baseC = geo.baseR + rowBytes;
+        run_beam_tasks<SmemSpace, !kAux, kAux>(a, bm, geo, s_tab, n_env, total);
+    } else {
+        BeamMap<GlobalSpace> bm;
+        bm.base = (unsigned long long)__cvta_generic_to_global(a.map.row);
+        bm.H = a.map.H; bm.W = a.map.W; bm.stride4R = a.map.strideR << 2; bm.stride4C = a.map.strideC << 2;
+        bm.rowBytes = rowBytes;
+        run_beam_tasks<GlobalSpace, false, kAux>(a, bm, geo, s_tab, n_env, total);
     }
 }
 

@@ -255,6 +255,7 @@ struct EnvArgs {
 constexpr int kEnvBlock = 32;
 
 __global__ void __launch_bounds__(kEnvBlock) env_step_kernel(EnvArgs a) {
+    asm volatile("griddepcontrol.launch_dependents;");           // the beam kernel may start staging the map now
     extern __shared__ __align__(16) uint8_t s_dyn[];
     const ColScratch scratch = col_scratch(s_dyn, a.robot.V);
     for (int k = threadIdx.x; k < a.robot.V; k += kEnvBlock) scratch.verts[k] = a.robot.verts[k];
@@ -402,6 +403,7 @@ struct ResetArgs {
 constexpr int kResetWarps = 4;
 
 __global__ void __launch_bounds__(kResetWarps * 32) reset_kernel(ResetArgs a) {
+    asm volatile("griddepcontrol.launch_dependents;");           // lets the list's beam kernel start early
     extern __shared__ __align__(16) uint8_t s_dyn[];
     const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const ColScratch scratch = col_scratch(s_dyn + (size_t)wib * col_scratch_bytes(a.robot.V), a.robot.V);

@@ -340,6 +340,18 @@ extern "C" int fn_sim_destroy(fn_sim* s) {
     return FN_OK;
 }
 
+// Launch with the programmatic-stream-serialization attribute (PDL, fn_common.cuh).
+template <class... KArgs, class... Args>
+static cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t stream, Args... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, args...);
+}
+
 static int ring_row_floats(const fn_sim* s) { return s->robot->B + 5 + (s->robot->drive == FN_DRIVE_DIFF ? 2 : 3) + 2; }
 
 static int launch_beams(fn_sim* s, const int* list, const int* count_dev, float* out_ranges) {
@@ -349,21 +361,14 @@ static int launch_beams(fn_sim* s, const int* list, const int* count_dev, float*
     b.ring_obs = s->ring; b.ring_cap = s->ring_cap ? s->ring_cap : 1; b.ring_head = s->d_ring_head; b.ring_row = ring_row_floats(s);
     b.counters = s->d_counters;
     const bool aux = s->count_words || s->aux_hit;
-    // programmatic dependent launch: the kernel may start (and stage the map) under its predecessor
-    cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3(s->beam_grid); cfg.blockDim = dim3(512); cfg.dynamicSmemBytes = s->beam_smem; cfg.stream = s->stream;
-    cudaLaunchAttribute at[1];
-    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    at[0].val.programmaticStreamSerializationAllowed = 1;
-    cfg.attrs = at; cfg.numAttrs = getenv("FN_DBG_NOPDL") ? 0 : 1;
+    const dim3 grid(s->beam_grid), block(512);
     if (s->use_smem) {
-        if (aux) FN_CUDA(cudaLaunchKernelEx(&cfg, beam_kernel<true, true>, b));
-        else FN_CUDA(cudaLaunchKernelEx(&cfg, beam_kernel<true, false>, b));
+        if (aux) FN_CUDA(launch_pdl(beam_kernel<true, true>, grid, block, s->beam_smem, s->stream, b));
+        else FN_CUDA(launch_pdl(beam_kernel<true, false>, grid, block, s->beam_smem, s->stream, b));
     } else {
-        if (aux) FN_CUDA(cudaLaunchKernelEx(&cfg, beam_kernel<false, true>, b));
-        else FN_CUDA(cudaLaunchKernelEx(&cfg, beam_kernel<false, false>, b));
+        if (aux) FN_CUDA(launch_pdl(beam_kernel<false, true>, grid, block, s->beam_smem, s->stream, b));
+        else FN_CUDA(launch_pdl(beam_kernel<false, false>, grid, block, s->beam_smem, s->stream, b));
     }
-    FN_CUDA(cudaGetLastError());
     return FN_OK;
 }
 
@@ -386,12 +391,10 @@ extern "C" int fn_step(fn_sim* s, float* states, const float* actions, float dt,
         FN_CUDA(cudaEventRecord(e0, s->stream));
     }
     a.epw = s->n >= 32768 ? 32 : (s->n >= 8192 ? 16 : 8);
-    env_step_kernel<<<(s->n + a.epw - 1) / a.epw, kEnvBlock, col_scratch_bytes(s->robot->V), s->stream>>>(a);
-    FN_CUDA(cudaGetLastError());
+    FN_CUDA(launch_pdl(env_step_kernel, dim3((s->n + a.epw - 1) / a.epw), dim3(kEnvBlock), col_scratch_bytes(s->robot->V), s->stream, a));
     if (s->prof) FN_CUDA(cudaEventRecord(e1, s->stream));
     if (s->ring) {
-        ring_advance_kernel<<<1, 1, 0, s->stream>>>(s->d_ring_head, (unsigned long long)s->n, s->ring_cap);
-        FN_CUDA(cudaGetLastError());
+        FN_CUDA(launch_pdl(ring_advance_kernel, dim3(1), dim3(1), 0, s->stream, s->d_ring_head, (unsigned long long)s->n, s->ring_cap));
     }
     int rc = launch_beams(s, nullptr, nullptr, out_ranges);
     if (s->prof && rc == FN_OK) FN_CUDA(cudaEventRecord(e2, s->stream));
@@ -408,8 +411,7 @@ extern "C" int fn_reset(fn_sim* s, float* states, const uint8_t* mask, const uin
         s->ev->push_back(e0); s->ev->push_back(e1); s->ev_kind->push_back(1);
         FN_CUDA(cudaEventRecord(e0, s->stream));
     }
-    compact_mask_kernel<<<1, 1024, 0, s->stream>>>(mask, s->n, s->d_list, s->d_count);
-    FN_CUDA(cudaGetLastError());
+    FN_CUDA(launch_pdl(compact_mask_kernel, dim3(1), dim3(1024), 0, s->stream, mask, s->n, s->d_list, s->d_count));
     ResetArgs a;
     a.map = s->map->dev; a.robot = robot_dev(s->robot, s->map); a.task = task_dev(s->task);
     a.regions.rects = s->map->d_regions; a.regions.n = s->map->n_regions;
@@ -420,8 +422,7 @@ extern "C" int fn_reset(fn_sim* s, float* states, const uint8_t* mask, const uin
     a.counters = s->d_counters;
     int grid = (s->n + kResetWarps - 1) / kResetWarps;
     if (grid > s->num_sms * 4) grid = s->num_sms * 4;
-    reset_kernel<<<grid, kResetWarps * 32, kResetWarps * col_scratch_bytes(s->robot->V), s->stream>>>(a);
-    FN_CUDA(cudaGetLastError());
+    FN_CUDA(launch_pdl(reset_kernel, dim3(grid), dim3(kResetWarps * 32), kResetWarps * col_scratch_bytes(s->robot->V), s->stream, a));
     int rc = launch_beams(s, s->d_list, s->d_count, out_ranges);
     if (s->prof && rc == FN_OK) FN_CUDA(cudaEventRecord(e1, s->stream));
     return rc;

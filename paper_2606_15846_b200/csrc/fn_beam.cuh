@@ -389,14 +389,6 @@ struct BeamArgs {
     unsigned long long* counters;
 };
 
-// Programmatic dependent launch (PDL): a kernel launched with the programmatic-stream-serialization
-// attribute may start while its predecessor in the stream still runs; griddepcontrol.wait blocks until
-// that predecessor has completed and its memory is visible.  The beam kernel stages the map and the
-// beam table (constants) BEFORE the wait, i.e. under the env-step / reset kernel.
-__device__ __forceinline__ void griddep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
-__device__ __forceinline__ void griddep_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;"); }
-
-
 // The warps of the (persistent) grid take 32 consecutive (env, beam) pairs at a time: adjacent lanes =
 // adjacent beams of one env, so a warp's loads mostly hit the same or neighbouring words (broadcast)
 // and its lanes run similar trip counts.  kFast = production shared-memory traversal (cast_beam_smem).
@@ -481,6 +473,7 @@ __global__ void __launch_bounds__(512, 2) beam_kernel(BeamArgs a) {
     }
     __syncthreads();
     griddep_wait();                                                // poses / list / count come from the previous kernel
+    griddep_launch_dependents();
     const int n_env = a.count_dev ? *a.count_dev : a.n_all;
     const unsigned total = (unsigned)n_env * (unsigned)B;
     if ((unsigned)blockIdx.x * (blockDim.x >> 5) * 32u >= total) return;   // nothing for this CTA

@@ -76,6 +76,15 @@ struct RegionsDev {
 
 __device__ __forceinline__ int lane_id() { return threadIdx.x & 31; }
 
+// Programmatic dependent launch (PDL): every kernel of fn_step / fn_reset is launched with the
+// programmatic-stream-serialization attribute, so it may become resident while its predecessor in the
+// stream still runs.  griddepcontrol.wait blocks until that predecessor has COMPLETED and its memory is
+// visible (and, by induction, everything before it); what a kernel does before the wait may only touch
+// constants of the map / robot (the beam kernel stages the map there).  launch_dependents, issued
+// right after the wait, lets the next kernel's CTAs be scheduled as soon as resources free up.
+__device__ __forceinline__ void griddep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void griddep_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;"); }
+
 __device__ __forceinline__ double warp_min(double v) {
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) v = fmin(v, __shfl_xor_sync(0xffffffffu, v, o));

@@ -255,11 +255,12 @@ struct EnvArgs {
 constexpr int kEnvBlock = 32;
 
 __global__ void __launch_bounds__(kEnvBlock) env_step_kernel(EnvArgs a) {
-    asm volatile("griddepcontrol.launch_dependents;");           // the beam kernel may start staging the map now
     extern __shared__ __align__(16) uint8_t s_dyn[];
     const ColScratch scratch = col_scratch(s_dyn, a.robot.V);
     for (int k = threadIdx.x; k < a.robot.V; k += kEnvBlock) scratch.verts[k] = a.robot.verts[k];
     __syncwarp();
+    griddep_wait();                                                // states / actions / mask come from earlier work
+    griddep_launch_dependents();                                   // the beam kernel may start staging the map now
     const int e = blockIdx.x * a.epw + threadIdx.x;
     const int n = a.n;
     const bool live = (int)threadIdx.x < a.epw && e < n;
@@ -335,6 +336,8 @@ __global__ void __launch_bounds__(kEnvBlock) env_step_kernel(EnvArgs a) {
 
 // advances the replay ring's head by n rows (one thread), after the env-step kernel of fn_step
 __global__ void ring_advance_kernel(unsigned long long* head, unsigned long long n, unsigned long long cap) {
+    griddep_wait();
+    griddep_launch_dependents();
     *head = (*head + n) % cap;
 }
 
@@ -343,6 +346,8 @@ __global__ void ring_advance_kernel(unsigned long long* head, unsigned long long
 // segment counts, then each thread writes its indices.  list is ascending; *count = number set.
 __global__ void __launch_bounds__(1024) compact_mask_kernel(const uint8_t* mask, int n, int* list, int* count) {
     __shared__ int s_warp[32];
+    griddep_wait();
+    griddep_launch_dependents();
     const int t = threadIdx.x, lane = t & 31, wid = t >> 5;
     const int seg = (n + 1023) / 1024;
     const int lo = min(n, t * seg), hi = min(n, lo + seg);
@@ -403,12 +408,13 @@ struct ResetArgs {
 constexpr int kResetWarps = 4;
 
 __global__ void __launch_bounds__(kResetWarps * 32) reset_kernel(ResetArgs a) {
-    asm volatile("griddepcontrol.launch_dependents;");           // lets the list's beam kernel start early
     extern __shared__ __align__(16) uint8_t s_dyn[];
     const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const ColScratch scratch = col_scratch(s_dyn + (size_t)wib * col_scratch_bytes(a.robot.V), a.robot.V);
     for (int k = lane; k < a.robot.V; k += 32) scratch.verts[k] = a.robot.verts[k];
     __syncwarp();
+    griddep_wait();                                                // the list comes from the compaction kernel
+    griddep_launch_dependents();
     const int count = *a.count_dev;
     const int n = a.n;
     const double rho = (double)a.map.rho;

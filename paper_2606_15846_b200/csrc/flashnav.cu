@@ -69,6 +69,7 @@ struct fn_sim {
     float* d_dprev;
     int* d_epstep;
     unsigned long long* d_counters;
+    unsigned* d_task_counter;        // beam kernel's dynamic task counter
     // bound by the caller
     int32_t* aux_hit;
     float* aux_reward;
@@ -287,6 +288,8 @@ extern "C" int fn_sim_create(const fn_map* map, const fn_robot* robot, int n, co
     if (e == cudaSuccess) e = cudaMalloc(&s->d_dprev, (size_t)n * sizeof(float));
     if (e == cudaSuccess) e = cudaMalloc(&s->d_epstep, (size_t)n * sizeof(int));
     if (e == cudaSuccess) e = cudaMalloc(&s->d_counters, kNCounters * sizeof(unsigned long long));
+    if (e == cudaSuccess) e = cudaMalloc(&s->d_task_counter, sizeof(unsigned));
+    if (e == cudaSuccess) e = cudaMemsetAsync(s->d_task_counter, 0, sizeof(unsigned), s->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(s->d_dprev, 0, (size_t)n * sizeof(float), s->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(s->d_epstep, 0, (size_t)n * sizeof(int), s->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(s->d_counters, 0, kNCounters * sizeof(unsigned long long), s->stream);
@@ -332,7 +335,7 @@ extern "C" int fn_sim_create(const fn_map* map, const fn_robot* robot, int n, co
 extern "C" int fn_sim_destroy(fn_sim* s) {
     if (!s) return FN_OK;
     cudaFree(s->d_poses); cudaFree(s->d_ring_head); cudaFree(s->d_list); cudaFree(s->d_count); cudaFree(s->d_dprev);
-    cudaFree(s->d_epstep); cudaFree(s->d_counters);
+    cudaFree(s->d_epstep); cudaFree(s->d_counters); cudaFree(s->d_task_counter);
     if (s->ev) { for (cudaEvent_t e : *s->ev) cudaEventDestroy(e); delete s->ev; delete s->ev_kind; }
     cudaFree(s->stg_states); cudaFree(s->stg_actions); cudaFree(s->stg_ranges); cudaFree(s->stg_gobs);
     cudaFree(s->stg_mask); cudaFree(s->stg_col); cudaFree(s->stg_seeds);
@@ -359,7 +362,7 @@ static int launch_beams(fn_sim* s, const int* list, const int* count_dev, float*
     b.map = s->map->dev; b.robot = robot_dev(s->robot, s->map); b.poses = s->d_poses; b.count_words = s->count_words;
     b.list = list; b.count_dev = count_dev; b.n_all = s->n; b.out_ranges = out_ranges; b.out_hit = s->aux_hit;
     b.ring_obs = s->ring; b.ring_cap = s->ring_cap ? s->ring_cap : 1; b.ring_head = s->d_ring_head; b.ring_row = ring_row_floats(s);
-    b.counters = s->d_counters;
+    b.counters = s->d_counters; b.task_counter = s->d_task_counter;
     const bool aux = s->count_words || s->aux_hit;
     const dim3 grid(s->beam_grid), block(512);
     if (s->use_smem) {
@@ -383,7 +386,7 @@ extern "C" int fn_step(fn_sim* s, float* states, const float* actions, float dt,
     a.out_collision = out_collision; a.out_goal_obs = out_goal_obs; a.out_reward = s->aux_reward;
     a.d_prev = s->d_dprev; a.ep_step = s->d_epstep; a.poses = s->d_poses;
     a.ring = s->ring; a.ring_cap = s->ring_cap ? s->ring_cap : 1; a.ring_head_dev = s->d_ring_head; a.ring_row = ring_row_floats(s);
-    a.counters = s->d_counters;
+    a.counters = s->d_counters; a.beam_task_counter = s->d_task_counter;
     cudaEvent_t e0 = nullptr, e1 = nullptr, e2 = nullptr;
     if (s->prof) {
         FN_CUDA(cudaEventCreate(&e0)); FN_CUDA(cudaEventCreate(&e1)); FN_CUDA(cudaEventCreate(&e2));
@@ -419,7 +422,7 @@ extern "C" int fn_reset(fn_sim* s, float* states, const uint8_t* mask, const uin
     a.seeds = reinterpret_cast<const unsigned long long*>(seeds); a.out_goal_obs = out_goal_obs;
     a.d_prev = s->d_dprev; a.ep_step = s->d_epstep; a.poses = s->d_poses;
     a.ring = s->ring; a.ring_cap = s->ring_cap ? s->ring_cap : 1; a.ring_head_dev = s->d_ring_head; a.ring_row = ring_row_floats(s);
-    a.counters = s->d_counters;
+    a.counters = s->d_counters; a.beam_task_counter = s->d_task_counter;
     int grid = (s->n + kResetWarps - 1) / kResetWarps;
     if (grid > s->num_sms * 4) grid = s->num_sms * 4;
     FN_CUDA(launch_pdl(reset_kernel, dim3(grid), dim3(kResetWarps * 32), kResetWarps * col_scratch_bytes(s->robot->V), s->stream, a));
@@ -432,7 +435,7 @@ extern "C" int fn_observe_all(fn_sim* s, const float* states, float* out_ranges,
     if (!s || !states || !out_ranges) return fail(FN_ERR_INVALID_ARG, "fn_observe_all: NULL argument");
     PoseArgs a;
     a.map = s->map->dev; a.robot = robot_dev(s->robot, s->map); a.n = s->n; a.states = states;
-    a.out_goal_obs = out_goal_obs; a.poses = s->d_poses;
+    a.out_goal_obs = out_goal_obs; a.poses = s->d_poses; a.beam_task_counter = s->d_task_counter;
     pose_from_state_kernel<<<(s->n + 255) / 256, 256, 0, s->stream>>>(a);
     FN_CUDA(cudaGetLastError());
     float* ring = s->ring;           // a test hook: never touches the ring

@@ -386,6 +386,7 @@ struct BeamArgs {
     const unsigned long long* ring_head;      // device: pending row of env e = (*ring_head + e) % ring_cap
     int ring_row;                // floats per ring row
     int count_words;             // (kAux only)
+    unsigned* task_counter;      // next warp task; zeroed by the kernel that precedes the beam kernel
     unsigned long long* counters;
 };
 
@@ -396,18 +397,31 @@ template <class MS, bool kFast, bool kAux>
 __device__ __forceinline__ void run_beam_tasks(const BeamArgs& a, const BeamMap<MS>& bm, const SmemGeo& geo,
                                                const double2* s_tab, const int n_env, const unsigned total) {
     const int B = a.robot.B;
-    const int warps_per_cta = blockDim.x >> 5;
     const unsigned long long ring_head = a.ring_obs ? *a.ring_head : 0ull;
     const int lane = threadIdx.x & 31;
-    const unsigned warp0 = blockIdx.x * warps_per_cta + (threadIdx.x >> 5);
-    const unsigned nwarps = gridDim.x * warps_per_cta;
     const unsigned ntasks = (total + 31u) >> 5;
     uint32_t words = 0, rays = 0;
-    // (listed env, beam) of this lane's element idx = 32 task + lane, advanced without divisions
-    const unsigned step = nwarps << 5, step_e = step / (unsigned)B, step_j = step - step_e * (unsigned)B;
-    unsigned le = ((warp0 << 5) + lane) / (unsigned)B;
-    unsigned j = ((warp0 << 5) + lane) - le * (unsigned)B;
-    for (unsigned task = warp0; task < ntasks; task += nwarps) {
+    // Beams differ in length by an order of magnitude, and a purely static split leaves ~15 % of the SM
+    // time idle at the end of the launch.  So: the first 3/4 of each warp's share is static (round r ->
+    // task warp0 + r * nwarps, no atomics), the rest is handed out dynamically, one atomic per warp
+    // task, fetched one task ahead so that its latency is hidden.
+    const unsigned warp0 = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    const unsigned nwarps = gridDim.x * (blockDim.x >> 5);
+    const unsigned static_rounds = max(1u, ((ntasks / nwarps) * 3u) >> 2);
+    const unsigned dyn_base = static_rounds * nwarps;
+    const bool dynamic = dyn_base < ntasks;                        // (short launches are static only)
+    const unsigned long long invB = ~0ull / (unsigned long long)B + 1ull;     // floor(2^64 / B) + 1
+    unsigned round = 0;
+    unsigned task = warp0;
+    while (task < ntasks) {
+        unsigned next = ntasks;
+        ++round;
+        if (round < static_rounds) next = warp0 + round * nwarps;
+        else if (dynamic && lane == 0) next = dyn_base + atomicAdd(a.task_counter, 1u);
+        // (listed env, beam) of this lane's element idx = 32 task + lane
+        const unsigned idx = (task << 5) + lane;
+        const unsigned le = (unsigned)__umul64hi((unsigned long long)idx, invB);     // idx / B, exact for idx < 2^32
+        const unsigned j = idx - le * (unsigned)B;
         if (le < (unsigned)n_env) {
             const unsigned e = a.list ? (unsigned)a.list[le] : le;
             const BeamPose* pose = a.poses + e;
@@ -431,9 +445,7 @@ __device__ __forceinline__ void run_beam_tasks(const BeamArgs& a, const BeamMap<
             }
             ++rays;
         }
-        le += step_e;
-        j += step_j;
-        if (j >= (unsigned)B) { j -= B; ++le; }
+        task = __shfl_sync(0xffffffffu, next, 0);
     }
     // counters: one atomic per warp
     for (int o = 16; o > 0; o >>= 1) {
@@ -476,7 +488,6 @@ __global__ void __launch_bounds__(512, 2) beam_kernel(BeamArgs a) {
     griddep_launch_dependents();
     const int n_env = a.count_dev ? *a.count_dev : a.n_all;
     const unsigned total = (unsigned)n_env * (unsigned)B;
-    if ((unsigned)blockIdx.x * (blockDim.x >> 5) * 32u >= total) return;   // nothing for this CTA
 
     SmemGeo geo;
     geo.baseR = geo.baseC = 0; geo.rho = a.map.rho; geo.bitsR = a.map.strideR << 5; geo.bitsC = a.map.strideC << 5;

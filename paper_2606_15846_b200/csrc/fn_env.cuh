@@ -245,6 +245,7 @@ struct EnvArgs {
     const unsigned long long* ring_head_dev;   // device: slot of env 0's pending row
     int ring_row;
     int epw;                     // envs per warp (1..32): lanes >= epw idle in the scalar part
+    unsigned* beam_task_counter; // zeroed here for the beam kernel that follows
     unsigned long long* counters;
 };
 
@@ -261,6 +262,7 @@ __global__ void __launch_bounds__(kEnvBlock) env_step_kernel(EnvArgs a) {
     __syncwarp();
     griddep_wait();                                                // states / actions / mask come from earlier work
     griddep_launch_dependents();                                   // the beam kernel may start staging the map now
+    if (blockIdx.x == 0 && threadIdx.x == 0) *a.beam_task_counter = 0u;
     const int e = blockIdx.x * a.epw + threadIdx.x;
     const int n = a.n;
     const bool live = (int)threadIdx.x < a.epw && e < n;
@@ -402,6 +404,7 @@ struct ResetArgs {
     unsigned long long ring_cap;
     const unsigned long long* ring_head_dev;
     int ring_row;
+    unsigned* beam_task_counter; // zeroed here for the beam kernel that follows
     unsigned long long* counters;
 };
 
@@ -415,6 +418,7 @@ __global__ void __launch_bounds__(kResetWarps * 32) reset_kernel(ResetArgs a) {
     __syncwarp();
     griddep_wait();                                                // the list comes from the compaction kernel
     griddep_launch_dependents();
+    if (blockIdx.x == 0 && threadIdx.x == 0) *a.beam_task_counter = 0u;
     const int count = *a.count_dev;
     const int n = a.n;
     const double rho = (double)a.map.rho;
@@ -504,9 +508,11 @@ struct PoseArgs {
     const float* states;
     float* out_goal_obs;         // or NULL
     BeamPose* poses;
+    unsigned* beam_task_counter; // zeroed here for the beam kernel that follows
 };
 __global__ void __launch_bounds__(256) pose_from_state_kernel(PoseArgs a) {
     const int e = blockIdx.x * blockDim.x + threadIdx.x;
+    if (e == 0) *a.beam_task_counter = 0u;
     if (e >= a.n) return;
     const int n = a.n;
     const float x = a.states[e], y = a.states[n + e], psi = a.states[2 * n + e];

@@ -30,6 +30,10 @@ sys.path.insert(0, ROOT)
 
 from harness import workloads as W  # noqa: E402
 
+# dominant kernel (full-batch beam launch), per launch, from the committed ncu --set full capture
+NCU_CAPTURE = {2: {"dram_bytes": 507392, "warp_inst": 45701017, "lanes": 22.09,
+                   "source": "profiles/r1b_beam_kernel_full_c2.txt (dram__bytes_read.sum + dram__bytes_write.sum)"}}
+
 METRIC = "env_steps_per_s"
 UNIT = "env-steps/s"
 
@@ -283,13 +287,23 @@ def run_ours(args):
         peak = smem_peak if use_smem else l2_peak
         beam_s = beam_ms * 1e-3 / max(1, beam_launches)
         achieved = a_ray * n * B / beam_s
+        ncu = NCU_CAPTURE.get(args.config)
+        sm_hz = (clocks or {}).get("sm_mhz") or 1965.0
+        issue_peak = 148 * 4 * sm_hz * 1e6                      # warp instructions / s: 1 per scheduler per clock
         roofline = {"bound": "smem" if use_smem else "l2", "kernel": "fn::beam_kernel (fn_step, all envs)",
                     "achieved": achieved / 1e9, "peak": peak / 1e9, "unit": "GB/s", "frac": achieved / peak,
                     "peak_source": "fn_measure_peak in this run (conflict-free ld.shared / L2-resident ld.global.nc)",
                     "algorithmic_bytes_per_beam": a_ray, "windows_per_beam": windows,
-                    "kernel_ms": beam_s * 1e3, "share_of_step": beam_ms / total_ms if world == 1 else None,
-                    "traffic": None, "smem_peak_GBps": smem_peak / 1e9, "l2_peak_GBps": l2_peak / 1e9,
-                    "issue": {"note": "kernel is issue-slot bound, see DESIGN.md / profiles", "beams_per_s": n * B / beam_s}}
+                    "kernel_ms": beam_s * 1e3, "share_of_step": beam_ms / (env_ms + beam_ms + reset_ms),
+                    "traffic": ncu["dram_bytes"] if ncu else None,
+                    "traffic_source": ncu["source"] if ncu else None,
+                    "smem_peak_GBps": smem_peak / 1e9, "l2_peak_GBps": l2_peak / 1e9,
+                    "beams_per_s": n * B / beam_s,
+                    "issue": None if not ncu else {
+                        "note": "the kernel is issue/latency bound (DESIGN.md 6.1): warp instructions per launch from the "
+                                "ncu capture, duration live", "warp_inst_per_launch": ncu["warp_inst"],
+                        "achieved_Ginst_per_s": ncu["warp_inst"] / beam_s / 1e9, "peak_Ginst_per_s": issue_peak / 1e9,
+                        "frac": ncu["warp_inst"] / beam_s / issue_peak, "lanes_active_of_32": ncu["lanes"]}}
         # ---- oracle on the host cores, bounded sample of the same workload
         cpu = None
         if not args.no_cpu:
@@ -310,7 +324,7 @@ def run_ours(args):
                    "rays_per_s": ns * args.cpu_steps * B / dtc, "host_cores_available": os.cpu_count()}
         out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
                "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-               "dtype": "f64+i64 fixed point (fp32 storage)", "data": "synthetic",
+               "dtype": "f64", "data": "synthetic",
                "config": {"workload": workload_name(args.config), "name": wl.name, "n_envs_per_gpu": n, "beams": B,
                           "map": list(wl.occ.shape), "max_range_m": float(wl.max_range), "l2": "flushed between timed steps",
                           "ring": bool(ring is not None)},

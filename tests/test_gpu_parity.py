@@ -125,3 +125,76 @@ def test_argument_errors(pu):
     r = fn.Robot(W.footprint_rect(0.2, 0.2), [0.0], 1.0, 0, [0, 1, 0, 0, -1, 1])
     with pytest.raises(fn.FlashNavError):
         fn.Sim(m, r, 0)
+
+
+def test_ring_rows_and_wraparound_gpu(pu):
+    # S7 (BASELINE.json config 5): every completed ring row equals the tuple (obs the action
+    # was chosen from, action, reward, done) logged by the harness, including slots that wrap around a
+    # capacity that is not a multiple of the batch.  The expected ring is written by the oracle's append.
+    import torch
+    import oracle
+    from harness import workloads as W
+    for drive_cfg in (5, 3):                                   # differential (A = 2) and omnidirectional (A = 3)
+        wl = W.make_workload(drive_cfg, n_envs=96)
+        n, B, A = wl.n_envs, wl.n_beams, wl.action_dim
+        m, r, s = pu.make_sim(wl, n)
+        buf = pu.Buffers(n, B, A)
+        s.bind_aux(None, buf.reward)
+        cap = 3 * n + 37
+        row = B + 5 + A + 2
+        ring = torch.zeros(cap * row, device="cuda")
+        s.ring_attach(ring, cap)
+        steps = 9
+        actions = torch.from_numpy(W.action_tape(wl, steps, 3)).cuda()
+        seeds = W.seed_tape(wl, steps + 1, 3)
+        forced = W.forced_reset_tape(wl, steps, 3)
+        expect = np.zeros((cap, row), np.float32)
+        written = np.zeros(cap, bool)
+        buf.mask.fill_(1)
+        s.reset(buf.states, buf.mask, torch.from_numpy(seeds[0].view(np.int64)).cuda(), buf.ranges, buf.gobs)
+        torch.cuda.synchronize()
+        head = 0
+        for t in range(steps):
+            obs_r = buf.ranges.cpu().numpy().copy()
+            obs_g = buf.gobs.cpu().numpy().copy()              # [2, n] = d, alpha
+            obs_v = buf.states.cpu().numpy()[3:6].copy()       # [3, n] = vx, vy, w
+            buf.mask.copy_(torch.from_numpy(forced[t]))
+            s.step(buf.states, actions[t], float(wl.dt), buf.mask, buf.ranges, buf.col, buf.gobs)
+            torch.cuda.synchronize()
+            done = buf.mask.cpu().numpy().copy()
+            oracle.ring_append(expect, cap, head, obs_r, obs_g, obs_v, actions[t].cpu().numpy(),
+                               buf.reward.cpu().numpy(), done)
+            written[(head + np.arange(n)) % cap] = True
+            head = (head + n) % cap
+            s.reset(buf.states, buf.mask, torch.from_numpy(seeds[t + 1].view(np.int64)).cuda(), buf.ranges, buf.gobs)
+            torch.cuda.synchronize()
+        got = ring.cpu().numpy().reshape(cap, row)
+        pending = (head + np.arange(n)) % cap                  # rows started for the next step: obs part only
+        check = written.copy()
+        check[pending] = False
+        assert check.sum() >= cap - n - 1
+        assert np.array_equal(got[check], expect[check])
+        # pending rows already hold the observation the next action will be chosen from
+        assert np.array_equal(got[pending, :B], buf.ranges.cpu().numpy())
+        assert np.array_equal(got[pending, B:B + 2], buf.gobs.cpu().numpy().T)
+        assert np.array_equal(got[pending, B + 2:B + 5], buf.states.cpu().numpy()[3:6].T)
+        s.close(); r.close(); m.close()
+
+
+def test_full_size_sampled_c3_c4(pu):
+    # BASELINE.json's full batch sizes in the launch configuration bench.py times; beams of a fixed random
+    # subset of envs against the oracle, everything per-env (motion, collision, goal obs, reward/done) in full.
+    from harness import workloads as W
+    for cfg in (3, 4):
+        wl = W.make_workload(cfg)
+        rep = pu.run_parity(wl, steps=6, subset=192, check_every=3)
+        print(cfg, rep)
+        assert rep.c["collision_checks"] >= 2 * wl.n_envs
+
+
+def test_full_size_sampled_c5_with_regions(pu):
+    from harness import workloads as W
+    wl = W.make_workload(5)
+    rep = pu.run_parity(wl, steps=4, subset=96, check_every=2)
+    print(rep)
+    assert rep.c["resets"] > wl.n_envs

@@ -264,6 +264,34 @@ def run_ours(args):
     barrier()
     steady_ms = s0.elapsed_time(s1)
 
+    # the same K steps replayed as ONE CUDA graph (no L2 flush): information only.  fn_step / fn_reset only
+    # enqueue kernels and keep their per-step state on the device, so a captured sequence replays.
+    graph_ms = None
+    if args.graph:
+        try:
+            cs = torch.cuda.Stream()
+            cs.wait_stream(torch.cuda.current_stream())
+            g = torch.cuda.CUDAGraph()
+            sim.set_stream(cs)
+            with torch.cuda.graph(g, stream=cs):
+                for k in range(min(K, tape_len)):
+                    step(k)
+            sim.set_stream(torch.cuda.current_stream())
+            reps = max(1, K // min(K, tape_len))
+            g.replay()
+            barrier()
+            g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            g0.record()
+            for _ in range(reps):
+                g.replay()
+            g1.record()
+            barrier()
+            graph_ms = g0.elapsed_time(g1) / (reps * min(K, tape_len))
+        except Exception as ex:         # noqa: BLE001
+            graph_ms = None
+            sys.stderr.write(f"bench.py: graph replay leg skipped: {ex!r}\n")
+            sim.set_stream(torch.cuda.current_stream())
+
     tmax = torch.tensor([total_ms, steady_ms], device="cuda", dtype=torch.float64)
     rays = torch.tensor([float(c1["rays_cast"] - c0["rays_cast"]), float(c1["envs_reset"] - c0["envs_reset"])],
                         device="cuda", dtype=torch.float64)
@@ -333,6 +361,9 @@ def run_ours(args):
                "reset_rate_per_step": float(rays[1]) / (world * n * K),
                "steady_state": {"value": world * n * K / (steady_ms * 1e-3), "unit": UNIT, "ms_per_step": steady_ms / K,
                                 "note": "no L2 flush, K steps back to back"},
+               "graph_replay": None if graph_ms is None else {
+                   "value": world * n / (graph_ms * 1e-3), "unit": UNIT, "ms_per_step": graph_ms,
+                   "note": "the same steps captured once and replayed as a CUDA graph, no L2 flush (rank 0)"},
                "kernel_ms_per_step": {"env_step": env_ms / K, "beam_step": beam_ms / K, "reset_path": reset_ms / K},
                "ms_per_step_p50": float(np.median(per_step_ms)), "ms_per_step_p90": float(np.percentile(per_step_ms, 90)),
                "roofline": roofline, "cpu_baseline": cpu, "clocks": clocks, "gpu_launches": 5 * K}
@@ -383,6 +414,7 @@ def main():
     ap.add_argument("--cpu-steps", type=int, default=8, help="oracle steps in the cpu_baseline leg")
     ap.add_argument("--e2e-steps", type=int, default=50)
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--graph", type=int, default=1, help="also time a CUDA-graph replay of the steps (information only)")
     ap.add_argument("--ring", type=int, default=1, help="attach the replay ring when the config has one (C5)")
     args = ap.parse_args()
     if args.warmup < 3:

@@ -83,6 +83,10 @@ void fn_task_default(fn_task* out);
 int fn_sim_create(const fn_map* map, const fn_robot* robot, int n_envs, const fn_task* task,
                   void* cuda_stream, fn_sim** out);
 int fn_sim_destroy(fn_sim* sim);
+/* Re-targets all later work of the sim to another stream (e.g. a capturing stream: fn_step / fn_reset only
+ * enqueue kernels, never synchronise and keep all per-step state on the device, so a captured sequence of
+ * them can be replayed as a CUDA graph).  The caller orders the old and the new stream. */
+int fn_sim_set_stream(fn_sim* sim, void* cuda_stream);
 
 /* ---- one vector step -------------------------------------------------------------------
  * states_dev:     [8][N] fp32 SoA planes x, y, psi, v_x, v_y, w, g_x, g_y; read and overwritten.

@@ -17,7 +17,7 @@ COUNTER_NAMES = ("rays_cast", "map_words_loaded", "envs_reset", "reset_failures"
 
 EXPORTED_SYMBOLS = (
     "fn_map_create", "fn_map_set_regions", "fn_map_destroy", "fn_robot_create", "fn_robot_set_sensor",
-    "fn_robot_destroy", "fn_task_default", "fn_sim_create", "fn_sim_destroy", "fn_step", "fn_reset",
+    "fn_robot_destroy", "fn_task_default", "fn_sim_create", "fn_sim_destroy", "fn_sim_set_stream", "fn_step", "fn_reset",
     "fn_sim_bind_aux", "fn_ring_attach", "fn_observe_all", "fn_get_counters", "fn_sim_count_words",
     "fn_sim_episode_state", "fn_sim_beam_config", "fn_sim_profile", "fn_sim_profile_read", "fn_step_host", "fn_measure_peak", "fn_last_error", "fn_version")
 
@@ -55,6 +55,7 @@ def load_library():
         "fn_robot_destroy": [vp],
         "fn_sim_create": [vp, vp, i32, C.POINTER(_Task), vp, C.POINTER(vp)],
         "fn_sim_destroy": [vp],
+        "fn_sim_set_stream": [vp, vp],
         "fn_step": [vp, vp, vp, f32, vp, vp, vp, vp],
         "fn_reset": [vp, vp, vp, vp, vp, vp],
         "fn_sim_bind_aux": [vp, vp, vp],
@@ -183,6 +184,12 @@ class Sim:
                "fn_sim_create")
         self._h = h
         self._keep = []
+
+    def set_stream(self, stream=None):
+        """Later work goes to `stream` (a torch.cuda.Stream; default: torch's current stream)."""
+        import torch
+        self._stream = torch.cuda.current_stream() if stream is None else stream
+        _check(load_library().fn_sim_set_stream(self._h, C.c_void_p(self._stream.cuda_stream)), "fn_sim_set_stream")
 
     # --- the four calls of the north star ------------------------------------------------------
     def step(self, states, actions, dt, reset_mask, out_ranges, out_collision, out_goal_obs):

@@ -355,6 +355,12 @@ static cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, s
     return cudaLaunchKernelEx(&cfg, kernel, args...);
 }
 
+extern "C" int fn_sim_set_stream(fn_sim* s, void* stream) {
+    if (!s) return fail(FN_ERR_INVALID_ARG, "fn_sim_set_stream: NULL sim");
+    s->stream = (cudaStream_t)stream;
+    return FN_OK;
+}
+
 static int ring_row_floats(const fn_sim* s) { return s->robot->B + 5 + (s->robot->drive == FN_DRIVE_DIFF ? 2 : 3) + 2; }
 
 static int launch_beams(fn_sim* s, const int* list, const int* count_dev, float* out_ranges) {

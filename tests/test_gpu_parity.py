@@ -198,3 +198,46 @@ def test_full_size_sampled_c5_with_regions(pu):
     rep = pu.run_parity(wl, steps=4, subset=96, check_every=2)
     print(rep)
     assert rep.c["resets"] > wl.n_envs
+
+
+def test_cuda_graph_replay_equals_direct_launches(pu):
+    # fn_step / fn_reset only enqueue kernels and keep per-step state on the device: a captured sequence
+    # replayed as a CUDA graph must reproduce the directly launched trajectory bit for bit.
+    import torch
+    from harness import workloads as W
+    wl = W.make_workload(1, n_envs=128)
+    n, B, A = wl.n_envs, wl.n_beams, wl.action_dim
+    steps = 12
+    actions = torch.from_numpy(W.action_tape(wl, steps, 5)).cuda()
+    seeds = torch.from_numpy(W.seed_tape(wl, steps + 1, 5).view(np.int64)).cuda()
+    results = []
+    for use_graph in (False, True):
+        m, r, s = pu.make_sim(wl, n)
+        buf = pu.Buffers(n, B, A)
+        buf.mask.fill_(1)
+        s.reset(buf.states, buf.mask, seeds[0], buf.ranges, buf.gobs)
+        torch.cuda.synchronize()
+
+        def run():
+            for t in range(steps):
+                buf.mask.zero_()
+                s.step(buf.states, actions[t], float(wl.dt), buf.mask, buf.ranges, buf.col, buf.gobs)
+                s.reset(buf.states, buf.mask, seeds[t + 1], buf.ranges, buf.gobs)
+
+        if use_graph:
+            cs = torch.cuda.Stream()
+            cs.wait_stream(torch.cuda.current_stream())
+            g = torch.cuda.CUDAGraph()
+            s.set_stream(cs)
+            with torch.cuda.graph(g, stream=cs):
+                run()
+            s.set_stream(torch.cuda.current_stream())
+            g.replay()
+        else:
+            run()
+        torch.cuda.synchronize()
+        results.append((buf.states.clone(), buf.ranges.clone(), buf.gobs.clone(), buf.col.clone(), s.counters()["envs_reset"]))
+        s.close(); r.close(); m.close()
+    for a, b in zip(results[0][:4], results[1][:4]):
+        assert torch.equal(a, b)
+    assert results[0][4] == results[1][4] > n

@@ -364,7 +364,9 @@ def run_ours(args):
                "graph_replay": None if graph_ms is None else {
                    "value": world * n / (graph_ms * 1e-3), "unit": UNIT, "ms_per_step": graph_ms,
                    "note": "the same steps captured once and replayed as a CUDA graph, no L2 flush (rank 0)"},
-               "kernel_ms_per_step": {"env_step": env_ms / K, "beam_step": beam_ms / K, "reset_path": reset_ms / K},
+               "kernel_ms_per_step": {"env_step": env_ms / K, "beam_step": beam_ms / K, "reset_path": reset_ms / K,
+                                      "compact": prof["compact"][0] / K, "reset": prof["reset"][0] / K,
+                                      "beam_reset": prof["beam_reset"][0] / K},
                "ms_per_step_p50": float(np.median(per_step_ms)), "ms_per_step_p90": float(np.percentile(per_step_ms, 90)),
                "roofline": roofline, "cpu_baseline": cpu, "clocks": clocks, "gpu_launches": 5 * K}
 

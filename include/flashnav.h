@@ -125,8 +125,10 @@ int fn_sim_episode_state(fn_sim* sim, float* d_prev_host, int32_t* ep_step_host)
 
 /* ---- live kernel timing (bench.py's roofline): when enabled, fn_step / fn_reset record CUDA events on
  * the sim's stream around their kernels.  fn_sim_profile_read synchronises, adds up the elapsed times
- * since the last read and clears them.  ms_out[4] / launches_out[4] = {env-step kernel, beam kernel of
- * fn_step, whole fn_reset path (compaction + reset + beam kernels), reserved}. */
+ * since the last read and clears them.  ms_out[8] / launches_out[8] = {env-step kernel, beam kernel of
+ * fn_step, compaction kernel, reset kernel, beam kernel of fn_reset (the listed envs), reserved x 3}.
+ * Events between kernels keep a kernel from starting under its predecessor (programmatic dependent
+ * launch), so a profiled step is a few microseconds slower than an unprofiled one. */
 int fn_sim_profile(fn_sim* sim, int enable);
 int fn_sim_profile_read(fn_sim* sim, double* ms_out, uint64_t* launches_out);
 

@@ -248,11 +248,13 @@ class Sim:
 
     def profile_read(self):
         """dict kernel -> (total ms, launches) since the last read; synchronises."""
-        ms = np.zeros(4, np.float64)
-        ln = np.zeros(4, np.uint64)
+        ms = np.zeros(8, np.float64)
+        ln = np.zeros(8, np.uint64)
         _check(load_library().fn_sim_profile_read(self._h, _np_ptr(ms), _np_ptr(ln)), "fn_sim_profile_read")
         return {"env_step": (float(ms[0]), int(ln[0])), "beam_step": (float(ms[1]), int(ln[1])),
-                "reset_path": (float(ms[2]), int(ln[2]))}
+                "compact": (float(ms[2]), int(ln[2])), "reset": (float(ms[3]), int(ln[3])),
+                "beam_reset": (float(ms[4]), int(ln[4])),
+                "reset_path": (float(ms[2] + ms[3] + ms[4]), int(ln[2] + ln[3] + ln[4]))}
 
     def episode_state(self):
         """Host copies of the sim's d_prev [N] f32 and ep_step [N] i32 (synchronises)."""

@@ -53,6 +53,8 @@ struct fn_robot {
     std::vector<float> verts;
     double2* d_beam_cs;
     double2* d_verts;
+    double2* d_samples;              // interior sample points of the footprint (reset pre-test)
+    int n_samples;
 };
 
 struct fn_sim {
@@ -177,6 +179,44 @@ extern "C" int fn_map_destroy(fn_map* m) {
 }
 
 // ------------------------------------------------------------------------------------------ robot
+// Up to kMaxSamples points strictly inside the footprint polygon (body frame), on a regular grid over
+// its bounding box.  A sample whose map cell is occupied proves a collision (the converse does not hold),
+// which lets fn_reset discard most colliding start-pose attempts without the exact polygon test.
+constexpr int kMaxSamples = 32;
+static std::vector<double2> interior_samples(const std::vector<float>& v, int V) {
+    double x0 = 1e300, x1 = -1e300, y0 = 1e300, y1 = -1e300;
+    for (int k = 0; k < V; ++k) {
+        x0 = std::fmin(x0, v[2 * k]); x1 = std::fmax(x1, v[2 * k]);
+        y0 = std::fmin(y0, v[2 * k + 1]); y1 = std::fmax(y1, v[2 * k + 1]);
+    }
+    std::vector<double2> pts;
+    for (int g : {6, 8, 12, 16}) {
+        pts.clear();
+        for (int a = 0; a < g; ++a)
+            for (int b = 0; b < g; ++b) {
+                const double px = x0 + (x1 - x0) * (a + 0.5) / g, py = y0 + (y1 - y0) * (b + 0.5) / g;
+                bool in = false;
+                double dmin = 1e300;
+                for (int k = 0, j = V - 1; k < V; j = k++) {
+                    const double ax = v[2 * j], ay = v[2 * j + 1], bx = v[2 * k], by = v[2 * k + 1];
+                    if ((ay > py) != (by > py) && px < ax + (py - ay) * (bx - ax) / (by - ay)) in = !in;
+                    const double ex = bx - ax, ey = by - ay, l2 = ex * ex + ey * ey;
+                    double t = l2 > 0.0 ? ((px - ax) * ex + (py - ay) * ey) / l2 : 0.0;
+                    t = std::fmin(1.0, std::fmax(0.0, t));
+                    dmin = std::fmin(dmin, std::hypot(px - (ax + t * ex), py - (ay + t * ey)));
+                }
+                if (in && dmin > 1e-4) pts.push_back(make_double2(px, py));
+            }
+        if (pts.size() >= 8) break;
+    }
+    if ((int)pts.size() > kMaxSamples) {                           // thin out evenly
+        std::vector<double2> q;
+        for (int i = 0; i < kMaxSamples; ++i) q.push_back(pts[(size_t)i * pts.size() / kMaxSamples]);
+        pts.swap(q);
+    }
+    return pts;
+}
+
 static int robot_upload(fn_robot* r) {
     std::vector<double2> cs(r->B), vs(r->V);
     for (int j = 0; j < r->B; ++j) {
@@ -186,6 +226,9 @@ static int robot_upload(fn_robot* r) {
     for (int k = 0; k < r->V; ++k) vs[k] = make_double2((double)r->verts[2 * k], (double)r->verts[2 * k + 1]);
     FN_CUDA(cudaMemcpy(r->d_beam_cs, cs.data(), cs.size() * sizeof(double2), cudaMemcpyHostToDevice));
     FN_CUDA(cudaMemcpy(r->d_verts, vs.data(), vs.size() * sizeof(double2), cudaMemcpyHostToDevice));
+    const std::vector<double2> sp = interior_samples(r->verts, r->V);
+    r->n_samples = (int)sp.size();
+    if (r->n_samples) FN_CUDA(cudaMemcpy(r->d_samples, sp.data(), sp.size() * sizeof(double2), cudaMemcpyHostToDevice));
     return FN_OK;
 }
 
@@ -209,13 +252,15 @@ extern "C" int fn_robot_create(const float* fp, int V, const float* angles, int 
     r->sensor[0] = r->sensor[1] = r->sensor[2] = 0.0f;
     r->angles.assign(angles, angles + B);
     r->verts.assign(fp, fp + 2 * V);
-    r->d_beam_cs = nullptr; r->d_verts = nullptr;
+    r->d_beam_cs = nullptr; r->d_verts = nullptr; r->d_samples = nullptr; r->n_samples = 0;
     cudaError_t e = cudaMalloc(&r->d_beam_cs, (size_t)B * sizeof(double2));
     if (e == cudaSuccess) e = cudaMalloc(&r->d_verts, (size_t)V * sizeof(double2));
+    if (e == cudaSuccess) e = cudaMalloc(&r->d_samples, (size_t)kMaxSamples * sizeof(double2));
     int st = (e == cudaSuccess) ? robot_upload(r) : fail(e == cudaErrorMemoryAllocation ? FN_ERR_OOM : FN_ERR_CUDA, "fn_robot_create: %s", cudaGetErrorString(e));
     if (st != FN_OK) {
         if (r->d_beam_cs) cudaFree(r->d_beam_cs);
         if (r->d_verts) cudaFree(r->d_verts);
+        if (r->d_samples) cudaFree(r->d_samples);
         delete r;
         return st;
     }
@@ -233,13 +278,14 @@ extern "C" int fn_robot_destroy(fn_robot* r) {
     if (!r) return FN_OK;
     if (r->d_beam_cs) cudaFree(r->d_beam_cs);
     if (r->d_verts) cudaFree(r->d_verts);
+    if (r->d_samples) cudaFree(r->d_samples);
     delete r;
     return FN_OK;
 }
 
 static RobotDev robot_dev(const fn_robot* r, const fn_map* m) {
     RobotDev d;
-    d.beam_cs = r->d_beam_cs; d.verts = r->d_verts; d.B = r->B; d.V = r->V; d.drive = r->drive;
+    d.beam_cs = r->d_beam_cs; d.verts = r->d_verts; d.samples = r->d_samples; d.n_samples = r->n_samples; d.B = r->B; d.V = r->V; d.drive = r->drive;
     d.A = r->drive == FN_DRIVE_DIFF ? 2 : 3;
     for (int k = 0; k < 6; ++k) d.lim[k] = r->lim[k];
     d.rmax = r->rmax;
@@ -369,6 +415,7 @@ static int launch_beams(fn_sim* s, const int* list, const int* count_dev, float*
     b.list = list; b.count_dev = count_dev; b.n_all = s->n; b.out_ranges = out_ranges; b.out_hit = s->aux_hit;
     b.ring_obs = s->ring; b.ring_cap = s->ring_cap ? s->ring_cap : 1; b.ring_head = s->d_ring_head; b.ring_row = ring_row_floats(s);
     b.counters = s->d_counters; b.task_counter = s->d_task_counter;
+    b.inv_bitsR = 1.0f / (float)(32 * s->map->dev.strideR); b.inv_bitsC = 1.0f / (float)(32 * s->map->dev.strideC);
     const bool aux = s->count_words || s->aux_hit;
     const dim3 grid(s->beam_grid), block(512);
     if (s->use_smem) {
@@ -414,13 +461,14 @@ extern "C" int fn_reset(fn_sim* s, float* states, const uint8_t* mask, const uin
                         float* out_ranges, float* out_goal_obs) {
     if (!s || !states || !mask || !seeds || !out_ranges || !out_goal_obs)
         return fail(FN_ERR_INVALID_ARG, "fn_reset: NULL argument");
-    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    cudaEvent_t e0 = nullptr, e1 = nullptr, e2 = nullptr, e3 = nullptr;
     if (s->prof) {
-        FN_CUDA(cudaEventCreate(&e0)); FN_CUDA(cudaEventCreate(&e1));
-        s->ev->push_back(e0); s->ev->push_back(e1); s->ev_kind->push_back(1);
+        FN_CUDA(cudaEventCreate(&e0)); FN_CUDA(cudaEventCreate(&e1)); FN_CUDA(cudaEventCreate(&e2)); FN_CUDA(cudaEventCreate(&e3));
+        s->ev->push_back(e0); s->ev->push_back(e1); s->ev->push_back(e2); s->ev->push_back(e3); s->ev_kind->push_back(1);
         FN_CUDA(cudaEventRecord(e0, s->stream));
     }
     FN_CUDA(launch_pdl(compact_mask_kernel, dim3(1), dim3(1024), 0, s->stream, mask, s->n, s->d_list, s->d_count));
+    if (s->prof) FN_CUDA(cudaEventRecord(e1, s->stream));
     ResetArgs a;
     a.map = s->map->dev; a.robot = robot_dev(s->robot, s->map); a.task = task_dev(s->task);
     a.regions.rects = s->map->d_regions; a.regions.n = s->map->n_regions;
@@ -432,8 +480,9 @@ extern "C" int fn_reset(fn_sim* s, float* states, const uint8_t* mask, const uin
     int grid = (s->n + kResetWarps - 1) / kResetWarps;
     if (grid > s->num_sms * 4) grid = s->num_sms * 4;
     FN_CUDA(launch_pdl(reset_kernel, dim3(grid), dim3(kResetWarps * 32), kResetWarps * col_scratch_bytes(s->robot->V), s->stream, a));
+    if (s->prof) FN_CUDA(cudaEventRecord(e2, s->stream));
     int rc = launch_beams(s, s->d_list, s->d_count, out_ranges);
-    if (s->prof && rc == FN_OK) FN_CUDA(cudaEventRecord(e1, s->stream));
+    if (s->prof && rc == FN_OK) FN_CUDA(cudaEventRecord(e3, s->stream));
     return rc;
 }
 
@@ -481,7 +530,7 @@ extern "C" int fn_sim_profile(fn_sim* s, int enable) {
 
 extern "C" int fn_sim_profile_read(fn_sim* s, double* ms_out, uint64_t* launches_out) {
     if (!s || !ms_out || !launches_out) return fail(FN_ERR_INVALID_ARG, "fn_sim_profile_read: NULL argument");
-    for (int k = 0; k < 4; ++k) { ms_out[k] = 0.0; launches_out[k] = 0; }
+    for (int k = 0; k < 8; ++k) { ms_out[k] = 0.0; launches_out[k] = 0; }
     if (!s->ev) return FN_OK;
     FN_CUDA(cudaStreamSynchronize(s->stream));
     size_t i = 0;
@@ -492,8 +541,10 @@ extern "C" int fn_sim_profile_read(fn_sim* s, double* ms_out, uint64_t* launches
             FN_CUDA(cudaEventElapsedTime(&ms, (*s->ev)[i + 1], (*s->ev)[i + 2])); ms_out[1] += ms; launches_out[1] += 1;
             i += 3;
         } else {
-            FN_CUDA(cudaEventElapsedTime(&ms, (*s->ev)[i], (*s->ev)[i + 1])); ms_out[2] += ms; launches_out[2] += 3;
-            i += 2;
+            for (int k = 0; k < 3; ++k) {
+                FN_CUDA(cudaEventElapsedTime(&ms, (*s->ev)[i + k], (*s->ev)[i + k + 1])); ms_out[2 + k] += ms; launches_out[2 + k] += 1;
+            }
+            i += 4;
         }
     }
     for (cudaEvent_t e : *s->ev) cudaEventDestroy(e);

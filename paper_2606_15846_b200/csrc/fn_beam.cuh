@@ -353,7 +353,8 @@ __device__ __forceinline__ float cast_beam_smem(const BeamMap<SmemSpace>& bm, co
             const unsigned n = 31u - (unsigned)abs(cx - ce);
             const uint32_t xe = x & (su ? __funnelshift_r(0xffffffffu, 0u, n) : __funnelshift_l(0u, 0xffffffffu, n));
             if (xe != 0u) {
-                const int c = su ? cx + (31 - __clz(xe)) : cx - 31 + (__ffs(xe) - 1);
+                // first occupied cell in travel order: highest bit backward, lowest bit forward
+                const int c = cx - (int)(fu1 * 31u) + (31 - __clz(su ? xe : xe & (0u - xe)));
                 // lines crossed: the integer fields of line k and line 0 differ by +-k S +- (cells along u)
                 const int dq = sw ? (int)(hiw(D0) - hl) : (int)(hl - hiw(D0));
                 const int k = __float2int_rd(fmaf((float)dq, mx ? g.inv_bitsR : g.inv_bitsC, 0.5f));
@@ -387,6 +388,7 @@ struct BeamArgs {
     int ring_row;                // floats per ring row
     int count_words;             // (kAux only)
     unsigned* task_counter;      // next warp task; zeroed by the kernel that precedes the beam kernel
+    float inv_bitsR, inv_bitsC;  // 1 / (bits per line) of the row / column copy (host-computed)
     unsigned long long* counters;
 };
 
@@ -491,7 +493,7 @@ __global__ void __launch_bounds__(512, 2) beam_kernel(BeamArgs a) {
 
     SmemGeo geo;
     geo.baseR = geo.baseC = 0; geo.rho = a.map.rho; geo.bitsR = a.map.strideR << 5; geo.bitsC = a.map.strideC << 5;
-    geo.inv_bitsR = 1.0f / (float)geo.bitsR; geo.inv_bitsC = 1.0f / (float)geo.bitsC;
+    geo.inv_bitsR = a.inv_bitsR; geo.inv_bitsC = a.inv_bitsC;
     const unsigned rowBytes = (unsigned)(a.map.H + 2 * kLineGuard) * (unsigned)(a.map.strideR << 2);
     if (stage) {
         BeamMap<SmemSpace> bm;

@@ -53,6 +53,8 @@ struct __align__(32) BeamPose {
 struct RobotDev {
     const double2* beam_cs;  // [B] (cos, sin) of theta_j + s_psi
     const double2* verts;    // [V] footprint vertices, body frame, metres
+    const double2* samples;  // [n_samples] points inside the footprint (body frame): a cheap one-sided pre-test
+    int n_samples;
     int B, V;
     int drive;               // 0 diff, 1 omni
     int A;                   // action dim

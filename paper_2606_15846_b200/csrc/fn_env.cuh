@@ -443,6 +443,23 @@ __global__ void __launch_bounds__(kResetWarps * 32) reset_kernel(ResetArgs a) {
             double sk, ck;
             sincos((double)pk, &sk, &ck);
             Window w = footprint_window(a.map, scratch.verts, a.robot.V, (double)xk, (double)yk, ck, sk);
+            // One-sided pre-test: a point inside the footprint whose cell is occupied proves a collision.
+            // Most random start poses that collide do so deeply, so few attempts need the exact test.
+            if (w.status == 2) {
+                bool hit = false;
+                for (int q = 0; q < a.robot.n_samples && !hit; q += 4) {
+                    bool h4 = false;
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        const double2 f = a.robot.samples[min(q + u, a.robot.n_samples - 1)];
+                        const int j = __double2int_rd(((double)xk + ck * f.x - sk * f.y) * a.map.inv_rho);
+                        const int i = __double2int_rd(((double)yk + sk * f.x + ck * f.y) * a.map.inv_rho);
+                        h4 |= occ_global(a.map, i, j);
+                    }
+                    hit = h4;
+                }
+                if (hit) w.status = 1;
+            }
             // attempts after the first one that is free without an exact test cannot win: skip their tests
             const unsigned free_m = __ballot_sync(0xffffffffu, w.status == 0);
             if (free_m && lane > __ffs(free_m) - 1) w.status = 1;

@@ -217,7 +217,7 @@ def run_ours(args):
         k = t % tape_len
         mask.copy_(forced[k])
         sim.step(states, actions[k], float(wl.dt), mask, ranges, col, gobs)
-        sim.reset(states, mask, seeds[k], ranges, gobs)
+        sim.reset(states, None, seeds[k], ranges, gobs)       # mask = None: the envs this step reported done
 
     def barrier():
         torch.cuda.synchronize()

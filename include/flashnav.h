@@ -99,7 +99,9 @@ int fn_step(fn_sim* sim, float* states_dev, const float* actions_dev, float dt, 
             float* out_ranges_dev, uint8_t* out_collision_dev, float* out_goal_obs_dev);
 
 /* ---- reset of masked environments + selective observation recompute --------------
- * mask_dev: [N] u8; seeds_dev: [N] u64 (one seed per env, read for masked envs only).
+ * mask_dev: [N] u8, or NULL = exactly the envs the preceding fn_step reported done (their list is kept on the
+ * device by fn_step, so no mask scan is needed; usable once per fn_step, else FN_ERR_INVALID_ARG);
+ * seeds_dev: [N] u64 (one seed per env, read for masked envs only).
  * Rewrites ONLY the masked envs' state planes and their rows of out_ranges_dev / out_goal_obs_dev. */
 int fn_reset(fn_sim* sim, float* states_dev, const uint8_t* mask_dev, const uint64_t* seeds_dev,
              float* out_ranges_dev, float* out_goal_obs_dev);

@@ -202,12 +202,14 @@ class Sim:
             _dev_ptr(out_goal_obs, torch.float32, 2 * n, "out_goal_obs")), "fn_step")
 
     def reset(self, states, mask, seeds, out_ranges, out_goal_obs):
+        """mask = None: the envs the preceding step() reported done (no mask scan)."""
         import torch
         n, B = self.n, self.robot.B
         if seeds.dtype not in (torch.int64, torch.uint64):
             raise FlashNavError("seeds must be a 64-bit integer tensor")
         _check(load_library().fn_reset(
-            self._h, _dev_ptr(states, torch.float32, 8 * n, "states"), _dev_ptr(mask, torch.uint8, n, "mask"),
+            self._h, _dev_ptr(states, torch.float32, 8 * n, "states"),
+            None if mask is None else _dev_ptr(mask, torch.uint8, n, "mask"),
             _dev_ptr(seeds, seeds.dtype, n, "seeds"), _dev_ptr(out_ranges, torch.float32, n * B, "out_ranges"),
             _dev_ptr(out_goal_obs, torch.float32, 2 * n, "out_goal_obs")), "fn_reset")
 

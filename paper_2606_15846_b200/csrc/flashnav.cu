@@ -72,6 +72,9 @@ struct fn_sim {
     int* d_epstep;
     unsigned long long* d_counters;
     unsigned* d_task_counter;        // beam kernel's dynamic task counter
+    int* d_done_list;                // [2][n] envs reported done by fn_step (one list per step parity), any order
+    int* d_done_count;               // [2] counts, [2] = the parity the NEXT fn_step fills (device-side state)
+    int done_avail;                  // 1 = the last fn_step's list has not been consumed by fn_reset(mask = NULL)
     // bound by the caller
     int32_t* aux_hit;
     float* aux_reward;
@@ -335,6 +338,10 @@ extern "C" int fn_sim_create(const fn_map* map, const fn_robot* robot, int n, co
     if (e == cudaSuccess) e = cudaMalloc(&s->d_epstep, (size_t)n * sizeof(int));
     if (e == cudaSuccess) e = cudaMalloc(&s->d_counters, kNCounters * sizeof(unsigned long long));
     if (e == cudaSuccess) e = cudaMalloc(&s->d_task_counter, sizeof(unsigned));
+    if (e == cudaSuccess) e = cudaMalloc(&s->d_done_list, 2 * (size_t)n * sizeof(int));
+    if (e == cudaSuccess) e = cudaMalloc(&s->d_done_count, 3 * sizeof(int));
+    if (e == cudaSuccess) e = cudaMemsetAsync(s->d_done_count, 0, 3 * sizeof(int), s->stream);
+    s->done_avail = 0;
     if (e == cudaSuccess) e = cudaMemsetAsync(s->d_task_counter, 0, sizeof(unsigned), s->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(s->d_dprev, 0, (size_t)n * sizeof(float), s->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(s->d_epstep, 0, (size_t)n * sizeof(int), s->stream);
@@ -382,6 +389,7 @@ extern "C" int fn_sim_destroy(fn_sim* s) {
     if (!s) return FN_OK;
     cudaFree(s->d_poses); cudaFree(s->d_ring_head); cudaFree(s->d_list); cudaFree(s->d_count); cudaFree(s->d_dprev);
     cudaFree(s->d_epstep); cudaFree(s->d_counters); cudaFree(s->d_task_counter);
+    cudaFree(s->d_done_list); cudaFree(s->d_done_count);
     if (s->ev) { for (cudaEvent_t e : *s->ev) cudaEventDestroy(e); delete s->ev; delete s->ev_kind; }
     cudaFree(s->stg_states); cudaFree(s->stg_actions); cudaFree(s->stg_ranges); cudaFree(s->stg_gobs);
     cudaFree(s->stg_mask); cudaFree(s->stg_col); cudaFree(s->stg_seeds);
@@ -409,12 +417,14 @@ extern "C" int fn_sim_set_stream(fn_sim* s, void* stream) {
 
 static int ring_row_floats(const fn_sim* s) { return s->robot->B + 5 + (s->robot->drive == FN_DRIVE_DIFF ? 2 : 3) + 2; }
 
-static int launch_beams(fn_sim* s, const int* list, const int* count_dev, float* out_ranges) {
+static int launch_beams(fn_sim* s, const int* list, const int* count_dev, float* out_ranges, bool step_launch = false, bool done_list = false) {
     BeamArgs b;
     b.map = s->map->dev; b.robot = robot_dev(s->robot, s->map); b.poses = s->d_poses; b.count_words = s->count_words;
     b.list = list; b.count_dev = count_dev; b.n_all = s->n; b.out_ranges = out_ranges; b.out_hit = s->aux_hit;
     b.ring_obs = s->ring; b.ring_cap = s->ring_cap ? s->ring_cap : 1; b.ring_head = s->d_ring_head; b.ring_row = ring_row_floats(s);
     b.counters = s->d_counters; b.task_counter = s->d_task_counter;
+    b.flip_par_dev = step_launch ? s->d_done_count + 2 : nullptr; b.done_count = s->d_done_count;
+    b.list_par_dev = done_list ? s->d_done_count + 2 : nullptr;
     b.inv_bitsR = 1.0f / (float)(32 * s->map->dev.strideR); b.inv_bitsC = 1.0f / (float)(32 * s->map->dev.strideC);
     const bool aux = s->count_words || s->aux_hit;
     const dim3 grid(s->beam_grid), block(512);
@@ -440,6 +450,7 @@ extern "C" int fn_step(fn_sim* s, float* states, const float* actions, float dt,
     a.d_prev = s->d_dprev; a.ep_step = s->d_epstep; a.poses = s->d_poses;
     a.ring = s->ring; a.ring_cap = s->ring_cap ? s->ring_cap : 1; a.ring_head_dev = s->d_ring_head; a.ring_row = ring_row_floats(s);
     a.counters = s->d_counters; a.beam_task_counter = s->d_task_counter;
+    a.done_list = s->d_done_list; a.done_count = s->d_done_count; a.par_dev = s->d_done_count + 2;
     cudaEvent_t e0 = nullptr, e1 = nullptr, e2 = nullptr;
     if (s->prof) {
         FN_CUDA(cudaEventCreate(&e0)); FN_CUDA(cudaEventCreate(&e1)); FN_CUDA(cudaEventCreate(&e2));
@@ -452,27 +463,34 @@ extern "C" int fn_step(fn_sim* s, float* states, const float* actions, float dt,
     if (s->ring) {
         FN_CUDA(launch_pdl(ring_advance_kernel, dim3(1), dim3(1), 0, s->stream, s->d_ring_head, (unsigned long long)s->n, s->ring_cap));
     }
-    int rc = launch_beams(s, nullptr, nullptr, out_ranges);
+    int rc = launch_beams(s, nullptr, nullptr, out_ranges, true);
     if (s->prof && rc == FN_OK) FN_CUDA(cudaEventRecord(e2, s->stream));
+    s->done_avail = 1;
     return rc;
 }
 
 extern "C" int fn_reset(fn_sim* s, float* states, const uint8_t* mask, const uint64_t* seeds,
                         float* out_ranges, float* out_goal_obs) {
-    if (!s || !states || !mask || !seeds || !out_ranges || !out_goal_obs)
+    if (!s || !states || !seeds || !out_ranges || !out_goal_obs)
         return fail(FN_ERR_INVALID_ARG, "fn_reset: NULL argument");
+    if (!mask && !s->done_avail)
+        return fail(FN_ERR_INVALID_ARG, "fn_reset: mask_dev == NULL needs a preceding fn_step (its done list is used once)");
+    const int* list = mask ? s->d_list : s->d_done_list;
+    const int* count = mask ? s->d_count : s->d_done_count;
+    if (!mask) s->done_avail = 0;
     cudaEvent_t e0 = nullptr, e1 = nullptr, e2 = nullptr, e3 = nullptr;
     if (s->prof) {
         FN_CUDA(cudaEventCreate(&e0)); FN_CUDA(cudaEventCreate(&e1)); FN_CUDA(cudaEventCreate(&e2)); FN_CUDA(cudaEventCreate(&e3));
         s->ev->push_back(e0); s->ev->push_back(e1); s->ev->push_back(e2); s->ev->push_back(e3); s->ev_kind->push_back(1);
         FN_CUDA(cudaEventRecord(e0, s->stream));
     }
-    FN_CUDA(launch_pdl(compact_mask_kernel, dim3(1), dim3(1024), 0, s->stream, mask, s->n, s->d_list, s->d_count));
+    if (mask) FN_CUDA(launch_pdl(compact_mask_kernel, dim3(1), dim3(1024), 0, s->stream, mask, s->n, s->d_list, s->d_count));
     if (s->prof) FN_CUDA(cudaEventRecord(e1, s->stream));
     ResetArgs a;
     a.map = s->map->dev; a.robot = robot_dev(s->robot, s->map); a.task = task_dev(s->task);
     a.regions.rects = s->map->d_regions; a.regions.n = s->map->n_regions;
-    a.n = s->n; a.states = states; a.list = s->d_list; a.count_dev = s->d_count;
+    a.n = s->n; a.states = states; a.list = list; a.count_dev = count;
+    a.list_par_dev = mask ? nullptr : s->d_done_count + 2;
     a.seeds = reinterpret_cast<const unsigned long long*>(seeds); a.out_goal_obs = out_goal_obs;
     a.d_prev = s->d_dprev; a.ep_step = s->d_epstep; a.poses = s->d_poses;
     a.ring = s->ring; a.ring_cap = s->ring_cap ? s->ring_cap : 1; a.ring_head_dev = s->d_ring_head; a.ring_row = ring_row_floats(s);
@@ -481,7 +499,7 @@ extern "C" int fn_reset(fn_sim* s, float* states, const uint8_t* mask, const uin
     if (grid > s->num_sms * 4) grid = s->num_sms * 4;
     FN_CUDA(launch_pdl(reset_kernel, dim3(grid), dim3(kResetWarps * 32), kResetWarps * col_scratch_bytes(s->robot->V), s->stream, a));
     if (s->prof) FN_CUDA(cudaEventRecord(e2, s->stream));
-    int rc = launch_beams(s, s->d_list, s->d_count, out_ranges);
+    int rc = launch_beams(s, list, count, out_ranges, false, mask == nullptr);
     if (s->prof && rc == FN_OK) FN_CUDA(cudaEventRecord(e3, s->stream));
     return rc;
 }
@@ -598,7 +616,7 @@ extern "C" int fn_step_host(fn_sim* s, float* states, const float* actions, floa
     FN_CUDA(cudaMemcpyAsync(out_collision, s->stg_col, n, cudaMemcpyDeviceToHost, st));
     FN_CUDA(cudaMemcpyAsync(mask, s->stg_mask, n, cudaMemcpyDeviceToHost, st));
     if (seeds) {
-        rc = fn_reset(s, s->stg_states, s->stg_mask, reinterpret_cast<const uint64_t*>(s->stg_seeds), s->stg_ranges, s->stg_gobs);
+        rc = fn_reset(s, s->stg_states, nullptr, reinterpret_cast<const uint64_t*>(s->stg_seeds), s->stg_ranges, s->stg_gobs);
         if (rc != FN_OK) return rc;
     }
     FN_CUDA(cudaMemcpyAsync(states, s->stg_states, 8 * n * sizeof(float), cudaMemcpyDeviceToHost, st));

@@ -389,6 +389,9 @@ struct BeamArgs {
     int count_words;             // (kAux only)
     unsigned* task_counter;      // next warp task; zeroed by the kernel that precedes the beam kernel
     float inv_bitsR, inv_bitsC;  // 1 / (bits per line) of the row / column copy (host-computed)
+    int* flip_par_dev;           // fn_step's launch: clears done_count[*par ^ 1] and flips *par (see EnvArgs)
+    int* done_count;
+    const int* list_par_dev;     // or NULL; else list += (*list_par_dev ^ 1) * n_all, count_dev += (*list_par_dev ^ 1)
     unsigned long long* counters;
 };
 
@@ -488,6 +491,12 @@ __global__ void __launch_bounds__(512, 2) beam_kernel(BeamArgs a) {
     __syncthreads();
     griddep_wait();                                                // poses / list / count come from the previous kernel
     griddep_launch_dependents();
+    if (a.flip_par_dev && blockIdx.x == 0 && threadIdx.x == 0) {
+        const int p = *a.flip_par_dev;
+        a.done_count[p ^ 1] = 0;
+        *a.flip_par_dev = p ^ 1;
+    }
+    if (a.list_par_dev) { const int q = *a.list_par_dev ^ 1; a.list += (size_t)q * a.n_all; a.count_dev += q; }
     const int n_env = a.count_dev ? *a.count_dev : a.n_all;
     const unsigned total = (unsigned)n_env * (unsigned)B;
 

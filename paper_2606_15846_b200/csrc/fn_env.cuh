@@ -246,6 +246,10 @@ struct EnvArgs {
     int ring_row;
     int epw;                     // envs per warp (1..32): lanes >= epw idle in the scalar part
     unsigned* beam_task_counter; // zeroed here for the beam kernel that follows
+    int* done_list;              // [2][n] envs that report done (any order), one list per step parity;
+    int* done_count;             // [2]    fn_reset(mask = NULL) uses the step's list.  The parity lives on
+    const int* par_dev;          // the device (flipped by the step's beam kernel, which also clears the other
+                                 // count), so a captured sequence of steps replays for any length
     unsigned long long* counters;
 };
 
@@ -300,7 +304,6 @@ __global__ void __launch_bounds__(kEnvBlock) env_step_kernel(EnvArgs a) {
     Window win = footprint_window(a.map, scratch.verts, a.robot.V, (double)xf, (double)yf, c1, s1);
     if (!live) win.status = 0;
     const bool col = resolve_collisions(a.map, a.robot, win, (double)xf, (double)yf, c1, s1, scratch);
-    if (!live) return;
     // ---- S4: goal obs, reward Eq. (1), done
     const double gdx = (double)gxf - (double)xf, gdy = (double)gyf - (double)yf;
     const float d = (float)sqrt(gdx * gdx + gdy * gdy);
@@ -310,7 +313,17 @@ __global__ void __launch_bounds__(kEnvBlock) env_step_kernel(EnvArgs a) {
                         : reached ? a.task.r_success
                                   : (float)((double)a.task.c_progress * ((double)dp - (double)d));
     const bool limit = a.task.max_episode_steps > 0 && es + 1 >= a.task.max_episode_steps;
-    const uint8_t done = (col || reached || limit || forced) ? 1 : 0;
+    const uint8_t done = (live && (col || reached || limit || forced)) ? 1 : 0;
+    // the done envs, appended to the step's list (one atomic per warp): "Ended only" needs no mask scan
+    const unsigned dm = __ballot_sync(0xffffffffu, done != 0);
+    if (dm) {
+        int base = 0;
+        const int par = *a.par_dev;
+        if (threadIdx.x == 0) base = atomicAdd(a.done_count + par, __popc(dm));
+        base = __shfl_sync(0xffffffffu, base, 0);
+        if (done) a.done_list[(size_t)par * n + base + __popc(dm & ((1u << threadIdx.x) - 1u))] = e;
+    }
+    if (!live) return;
     a.states[0 * n + e] = xf; a.states[1 * n + e] = yf; a.states[2 * n + e] = psif;
     a.states[3 * n + e] = avx; a.states[4 * n + e] = avy; a.states[5 * n + e] = aw;
     a.out_collision[e] = col ? 1 : 0;
@@ -395,6 +408,7 @@ struct ResetArgs {
     float* states;
     const int* list;
     const int* count_dev;
+    const int* list_par_dev;     // or NULL; else list += (*list_par_dev ^ 1) * n, count_dev += (*list_par_dev ^ 1)
     const unsigned long long* seeds;
     float* out_goal_obs;
     float* d_prev;
@@ -419,8 +433,9 @@ __global__ void __launch_bounds__(kResetWarps * 32) reset_kernel(ResetArgs a) {
     griddep_wait();                                                // the list comes from the compaction kernel
     griddep_launch_dependents();
     if (blockIdx.x == 0 && threadIdx.x == 0) *a.beam_task_counter = 0u;
-    const int count = *a.count_dev;
     const int n = a.n;
+    if (a.list_par_dev) { const int q = *a.list_par_dev ^ 1; a.list += (size_t)q * n; a.count_dev += q; }
+    const int count = *a.count_dev;
     const double rho = (double)a.map.rho;
     const float two_pi_f = 6.28318530717958647692f, pi_f = 3.14159265358979323846f;
     const float dmin2 = __fmul_rn(a.task.dmin, a.task.dmin), dmax2 = __fmul_rn(a.task.dmax, a.task.dmax);

@@ -241,3 +241,36 @@ def test_cuda_graph_replay_equals_direct_launches(pu):
     for a, b in zip(results[0][:4], results[1][:4]):
         assert torch.equal(a, b)
     assert results[0][4] == results[1][4] > n
+
+
+def test_reset_of_the_steps_done_list_equals_masked_reset(pu):
+    # fn_reset(mask = NULL) resets exactly the envs the preceding fn_step reported done, from the list the
+    # step kernel keeps on the device (any order): same states, observations and counters as the mask path.
+    import torch
+    import paper_2606_15846_b200 as fn
+    from harness import workloads as W
+    wl = W.make_workload(4, n_envs=1500)                       # forced resets + collisions; not a multiple of 32
+    n, B, A = wl.n_envs, wl.n_beams, wl.action_dim
+    steps = 7
+    actions = torch.from_numpy(W.action_tape(wl, steps, 11)).cuda()
+    seeds = torch.from_numpy(W.seed_tape(wl, steps + 1, 11).view(np.int64)).cuda()
+    forced = torch.from_numpy(W.forced_reset_tape(wl, steps, 11)).cuda()
+    out = []
+    for use_list in (False, True):
+        m, r, s = pu.make_sim(wl, n)
+        buf = pu.Buffers(n, B, A)
+        buf.mask.fill_(1)
+        s.reset(buf.states, buf.mask, seeds[0], buf.ranges, buf.gobs)
+        for t in range(steps):
+            buf.mask.copy_(forced[t])
+            s.step(buf.states, actions[t], float(wl.dt), buf.mask, buf.ranges, buf.col, buf.gobs)
+            s.reset(buf.states, None if use_list else buf.mask, seeds[t + 1], buf.ranges, buf.gobs)
+        torch.cuda.synchronize()
+        c = s.counters()
+        out.append((buf.states.clone(), buf.ranges.clone(), buf.gobs.clone(), c["envs_reset"], c["rays_cast"]))
+        if use_list:
+            with pytest.raises(fn.FlashNavError):              # the step's list is consumed
+                s.reset(buf.states, None, seeds[0], buf.ranges, buf.gobs)
+        s.close(); r.close(); m.close()
+    assert torch.equal(out[0][0], out[1][0]) and torch.equal(out[0][1], out[1][1]) and torch.equal(out[0][2], out[1][2])
+    assert out[0][3] == out[1][3] > n and out[0][4] == out[1][4]

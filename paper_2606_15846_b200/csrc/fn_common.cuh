@@ -47,7 +47,8 @@ struct __align__(32) BeamPose {
     double c, s;             // cos/sin of the heading
     BeamOrient o[2];
     int state;               // 0 = origin in a free cell, 1 = in an occupied cell, 2 = outside the map
-    int pad_[3];
+    int psi_bits;            // bit pattern of the fp32 heading that (c, s) belong to
+    int pad_[2];
 };
 
 struct RobotDev {
@@ -102,7 +103,7 @@ __device__ __forceinline__ double warp_max(double v) {
 __device__ __forceinline__ double wrap_pi(double a) {
     const double two_pi = 6.283185307179586476925286766559;
     const double pi = 3.141592653589793238462643383279;
-    double r = a - two_pi * floor((a + pi) / two_pi);
+    double r = a - two_pi * floor((a + pi) * 0.15915494309189533576888376337251);   // (a + pi) / (2 pi)
     if (r >= pi) r -= two_pi;
     if (r < -pi) r += two_pi;
     return r;

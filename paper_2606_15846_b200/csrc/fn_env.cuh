@@ -204,12 +204,13 @@ __device__ __forceinline__ bool resolve_collisions(const MapDev& m, const RobotD
 // origin's fixed-point coordinate, the offset to the first line boundary and the address of the
 // origin's line.
 __device__ __forceinline__ void write_pose(const MapDev& m, const RobotDev& rb, BeamPose* out,
-                                           float xf, float yf, double c, double s) {
+                                           float xf, float yf, float psif, double c, double s) {
     const double ox = ((double)xf + c * rb.sx - s * rb.sy) * m.inv_rho;
     const double oy = ((double)yf + s * rb.sx + c * rb.sy) * m.inv_rho;
     BeamPose p;
     p.c = c; p.s = s;
-    p.pad_[0] = p.pad_[1] = p.pad_[2] = 0;
+    p.psi_bits = __float_as_int(psif);
+    p.pad_[0] = p.pad_[1] = 0;
     const bool in = ox >= 0.0 && ox < (double)m.W && oy >= 0.0 && oy < (double)m.H;   // false for NaN
     const int jx = in ? __double2int_rd(ox) : 0, iy = in ? __double2int_rd(oy) : 0;
     p.state = !in ? 2 : (occ_global(m, iy, jx) ? 1 : 0);
@@ -288,18 +289,38 @@ __global__ void __launch_bounds__(kEnvBlock) env_step_kernel(EnvArgs a) {
     aw = fminf(fmaxf(aw, a.robot.lim[4]), a.robot.lim[5]);
     const double dt = (double)a.dt, vx = avx, vy = avy, w = aw;
     const double th = w * dt;
+    // one sincos (of theta / 2) gives the integrator's A = sin(theta)/theta, C = sin^2(theta/2)/(theta/2)
+    // and the rotation by theta
+    double sh, ch;
+    sincos(0.5 * th, &sh, &ch);
+    const double sin_th = 2.0 * sh * ch, cos_th = 1.0 - 2.0 * sh * sh;
     double Ac, Cc;
     if (fabs(th) < 1e-8) { Ac = 1.0 - th * th / 6.0; Cc = 0.5 * th; }
-    else { const double sh = sin(0.5 * th); Ac = sin(th) / th; Cc = sh * sh / (0.5 * th); }
+    else { const double inv = 1.0 / th; Ac = sin_th * inv; Cc = 2.0 * sh * sh * inv; }
     const double bx = dt * (Ac * vx - Cc * vy), by = dt * (Cc * vx + Ac * vy);
-    double s0, c0;
-    sincos(psi, &s0, &c0);
+    // cos/sin of the stored heading: kept in the sensing pose by the kernel that wrote that heading
+    // (recomputed if the caller changed the state plane behind the sim's back)
+    const BeamPose* pp = a.poses + el;
+    double s0 = pp->s, c0 = pp->c;
+    const float psi_f = a.states[2 * n + el];
+    const bool fresh = pp->psi_bits == __float_as_int(psi_f);
+    if (!fresh) sincos(psi, &s0, &c0);
     const float xf = (float)(x + c0 * bx - s0 * by);
     const float yf = (float)(y + s0 * bx + c0 * by);
-    const float psif = (float)wrap_pi(psi + th);
-    // ---- sensing/collision pose = the stored fp32 pose, widened (parity is per step on stored bits)
+    const double pw = wrap_pi(psi + th);
+    const float psif = (float)pw;
+    // ---- sensing/collision pose = the stored fp32 pose, widened (parity is per step on stored bits):
+    // rotate (c0, s0) by theta, then by the fp32 rounding of the new heading (second order; < 1e-20);
+    // an exact sincos every 32nd step of an episode bounds the accumulated rounding (~2e-16 per step)
     double s1, c1;
-    sincos((double)psif, &s1, &c1);
+    if (fresh && (es & 31) != 31) {
+        const double cr = c0 * cos_th - s0 * sin_th, sr = s0 * cos_th + c0 * sin_th;
+        const double dl = (double)psif - pw;
+        c1 = cr - sr * dl - 0.5 * cr * dl * dl;
+        s1 = sr + cr * dl - 0.5 * sr * dl * dl;
+    } else {
+        sincos((double)psif, &s1, &c1);
+    }
     // ---- S3
     Window win = footprint_window(a.map, scratch.verts, a.robot.V, (double)xf, (double)yf, c1, s1);
     if (!live) win.status = 0;
@@ -332,7 +353,7 @@ __global__ void __launch_bounds__(kEnvBlock) env_step_kernel(EnvArgs a) {
     a.reset_mask[e] = done;
     a.d_prev[e] = d;
     a.ep_step[e] = es + 1;
-    write_pose(a.map, a.robot, &a.poses[e], xf, yf, c1, s1);
+    write_pose(a.map, a.robot, &a.poses[e], xf, yf, psif, c1, s1);
     if (a.ring) {
         // complete this step's row (its obs part was written when that observation was produced)
         const int B = a.robot.B;
@@ -519,7 +540,7 @@ __global__ void __launch_bounds__(kResetWarps * 32) reset_kernel(ResetArgs a) {
             a.d_prev[e] = d;
             a.ep_step[e] = 0;
             if (a.out_goal_obs) { a.out_goal_obs[e] = d; a.out_goal_obs[n + e] = alpha; }
-            write_pose(a.map, a.robot, &a.poses[e], x, y, cp, sp);
+            write_pose(a.map, a.robot, &a.poses[e], x, y, psi, cp, sp);
             if (a.ring) {
                 const unsigned long long head = *a.ring_head_dev;
                 float* row = a.ring + ((head + (unsigned long long)e) % a.ring_cap) * (size_t)a.ring_row;
@@ -550,7 +571,7 @@ __global__ void __launch_bounds__(256) pose_from_state_kernel(PoseArgs a) {
     const float x = a.states[e], y = a.states[n + e], psi = a.states[2 * n + e];
     double s, c;
     sincos((double)psi, &s, &c);
-    write_pose(a.map, a.robot, &a.poses[e], x, y, c, s);
+    write_pose(a.map, a.robot, &a.poses[e], x, y, psi, c, s);
     if (a.out_goal_obs) {
         const double gdx = (double)a.states[6 * n + e] - (double)x, gdy = (double)a.states[7 * n + e] - (double)y;
         a.out_goal_obs[e] = (float)sqrt(gdx * gdx + gdy * gdy);

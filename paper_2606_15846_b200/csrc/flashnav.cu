@@ -425,6 +425,7 @@ static int launch_beams(fn_sim* s, const int* list, const int* count_dev, float*
     b.counters = s->d_counters; b.task_counter = s->d_task_counter;
     b.flip_par_dev = step_launch ? s->d_done_count + 2 : nullptr; b.done_count = s->d_done_count;
     b.list_par_dev = done_list ? s->d_done_count + 2 : nullptr;
+    b.pair_lines = (double)s->robot->rmax / (double)s->map->res >= 110.0;     // beams of >~ 16 lines on average
     b.inv_bitsR = 1.0f / (float)(32 * s->map->dev.strideR); b.inv_bitsC = 1.0f / (float)(32 * s->map->dev.strideC);
     const bool aux = s->count_words || s->aux_hit;
     const dim3 grid(s->beam_grid), block(512);

@@ -165,7 +165,7 @@ __device__ __noinline__ BeamHit cast_beam_slow(const BeamMap<MS> bm, const BeamO
 template <class MS, bool kAux>
 __device__ __forceinline__ float cast_beam(const BeamMap<MS>& bm, const BeamPose* __restrict__ pose,
                                            const double2 cs, const double T, const float rho, const float rmax,
-                                           int* hit, uint32_t& words) {
+                                           int* hit, uint32_t& words, const bool pair_lines = false) {
     const double2 pcs = *reinterpret_cast<const double2*>(&pose->c);
     const double dx = pcs.x * cs.x - pcs.y * cs.y, dy = pcs.y * cs.x + pcs.x * cs.y;
     const bool mx = fabs(dx) >= fabs(dy);                         // dominant axis is x
@@ -231,7 +231,27 @@ __device__ __forceinline__ float cast_beam(const BeamMap<MS>& bm, const BeamPose
         }
         return true;                                              // later lines are farther away
     };
-    {
+    if (std::is_same<MS, GlobalSpace>::value && !kAux && pair_lines) {
+        // map read through L1/L2, long beams: two lines per trip, so that the (long-latency) loads of both overlap;
+        // an odd line count is rounded up (one line beyond the range: its hits are rejected above)
+        const typename MS::addr_t wend2 = MS::addb(wb0, (int)((unsigned)(nl - 1) | 1u) * lstep);
+        typename MS::addr_t wb = MS::addb(wb0, lstep);            // the pair's second line
+        const double Md2 = Md + Md;
+        D += Md;
+        for (;;) {
+            const double Da = D - Md;
+            const typename MS::addr_t wa = MS::addb(wb, -lstep);
+            const uint32_t tha = hiw(Da), thb = hiw(D);
+            const typename MS::addr_t aa = MS::addb(wa, (int)((tha >> 5) << 2)), ab = MS::addb(wb, (int)((thb >> 5) << 2));
+            const uint32_t la = MS::ld(aa), ha = MS::ld4(aa), lb = MS::ld(ab), hb = MS::ld4(ab);
+            const uint32_t xa = __funnelshift_r(la, ha, tha) & mask, xb = __funnelshift_r(lb, hb, thb) & mask;
+            if (xa != 0u && candidate(Da, wa, xa)) break;
+            if (xb != 0u && candidate(D, wb, xb)) break;
+            if (wb == wend2) break;
+            D += Md2;
+            wb = MS::addb(wb, lstep + lstep);
+        }
+    } else {
         const typename MS::addr_t wend = MS::addb(wb0, (nl - 1) * lstep);
         typename MS::addr_t wb = wb0;
         for (;;) {
@@ -387,6 +407,7 @@ struct BeamArgs {
     const unsigned long long* ring_head;      // device: pending row of env e = (*ring_head + e) % ring_cap
     int ring_row;                // floats per ring row
     int count_words;             // (kAux only)
+    int pair_lines;              // L1/L2 path: two lines per trip (pays off for long ranges)
     unsigned* task_counter;      // next warp task; zeroed by the kernel that precedes the beam kernel
     float inv_bitsR, inv_bitsC;  // 1 / (bits per line) of the row / column copy (host-computed)
     int* flip_par_dev;           // fn_step's launch: clears done_count[*par ^ 1] and flips *par (see EnvArgs)
@@ -435,7 +456,7 @@ __device__ __forceinline__ void run_beam_tasks(const BeamArgs& a, const BeamMap<
             int hit = -2;
             if (state == 0) {
                 if constexpr (kFast) r = cast_beam_smem(bm, geo, pose, s_tab[j], a.robot.T, a.robot.rmax);
-                else r = cast_beam<MS, kAux>(bm, pose, s_tab[j], a.robot.T, a.map.rho, a.robot.rmax, &hit, words);
+                else r = cast_beam<MS, kAux>(bm, pose, s_tab[j], a.robot.T, a.map.rho, a.robot.rmax, &hit, words, a.pair_lines != 0);
             } else if (kAux) {
                 if (state == 1) hit = origin_line(bm, pose->o[0], true) * a.map.W + pose->o[0].cu0;
                 ++words;

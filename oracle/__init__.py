@@ -179,6 +179,29 @@ def ring_append(ring, capacity, head, obs_ranges, obs_goal, obs_vel, actions, re
                           _p(done, C.c_uint8))
 
 
+def footprint_distance(footprint, px, py) -> float:
+    """Eq. (3) for one body-frame point: distance to the polygon, 0 inside."""
+    fp = _f32(footprint)
+    f = lib().fno_footprint_distance
+    f.restype = C.c_double
+    f.argtypes = [C.c_int, C.POINTER(C.c_float), C.c_double, C.c_double]
+    return float(f(fp.shape[0], _p(fp, C.c_float), float(px), float(py)))
+
+
+def clearance_features(footprint, angles, max_range, n_sectors, ranges_, sensor=None, want_delta=False):
+    """Eq. (3) + sector min-pooling.  ranges_ [n,B] f32 -> z [n,n_sectors] f32
+    (, delta [n,B] f32)."""
+    fp, ang, rg = _f32(footprint), _f32(angles), _f32(ranges_)
+    n, B = rg.shape
+    z = np.empty((n, n_sectors), np.float32)
+    delta = np.empty((n, B), np.float32) if want_delta else None
+    sen = None if sensor is None else _f32(sensor)
+    lib().fno_clearance_features(C.c_int(fp.shape[0]), _p(fp, C.c_float), C.c_int(B), _p(ang, C.c_float),
+                                 _p(sen, C.c_float), C.c_float(max_range), C.c_int(n_sectors), C.c_int(n),
+                                 _p(rg, C.c_float), _p(delta, C.c_float), _p(z, C.c_float))
+    return (z, delta) if want_delta else z
+
+
 def step(wl, states, actions, forced, d_prev, ep_step, want_hit=True):
     """One whole vector step on a harness Workload-like object (fields only; no harness import).
     states [8,n] f32 updated in place.  Returns dict(ranges, hit, collision, goal_obs, reward, done)."""

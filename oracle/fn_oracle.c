@@ -19,6 +19,8 @@
  *   O7     reset of masked envs (PAPER.md:86, :199 say THAT envs are reset; the sampling rule is
  *          reading G16 -- "parity unpinned" by the paper, pinned by invariants only).
  *   O9     transition row for the replay ring (BASELINE.json config 5).
+ *   O10    clearance features, Eq. (3) and their sector min-pooling:
+ *          SURVEY 8(f) NEXT-1.  The sector layout is reading G21.
  *   plus the paper's own two approximations as brute-force cross-checks:
  *          fno_ranges_fixed_step and fno_collision_sampled (Eq. (2)).
  *
@@ -514,6 +516,68 @@ void fno_ring_append(float* ring, uint64_t capacity, uint64_t head, int n, int B
         for (int a = 0; a < A; ++a) r[B + 5 + a] = actions[(size_t)e * A + a];
         r[B + 5 + A] = reward[e];
         r[B + 6 + A] = done[e] ? 1.0f : 0.0f;
+    }
+}
+
+/* ------------------------------------------------------------------ O10: clearance features (NEXT-1)
+ * "Each valid range endpoint e_{t,j} ... is expressed in the body frame using the
+ * sensor placement in the robot specification.  Its nonnegative distance to the occupied footprint is
+ * delta_{t,j} = min_{f in F} ||e_{t,j} - f||_2 (3).  For polygonal footprints, this distance is computed
+ * directly from the boundary segments and is set to zero for points inside the occupied region. ...
+ * Distances are capped at the sensor range and pooled by taking the minimum within each angular sector.
+ * Beams without a valid hit are assigned the maximum range before pooling."  (also PAPER.md:67)
+ * Readings: valid <=> range < max_range (G10); endpoint = s_xy + r (cos, sin)(theta_j + s_psi) (G8);
+ * sector of beam j = floor(j n_sectors / B), i.e. n_sectors groups of consecutive beams in table order
+ * (G21: the paper gives neither the sector count nor its layout).
+ */
+static double point_segment_dist(double px, double py, double ax, double ay, double bx, double by) {
+    const double ex = bx - ax, ey = by - ay, l2 = ex * ex + ey * ey;
+    double t = l2 > 0.0 ? ((px - ax) * ex + (py - ay) * ey) / l2 : 0.0;
+    if (t < 0.0) t = 0.0;
+    if (t > 1.0) t = 1.0;
+    return hypot(px - (ax + t * ex), py - (ay + t * ey));
+}
+
+static int point_in_polygon(double px, double py, int V, const float* fp_xy) {   /* even-odd rule */
+    int in = 0;
+    for (int k = 0, j = V - 1; k < V; j = k++) {
+        const double ax = fp_xy[2 * j], ay = fp_xy[2 * j + 1], bx = fp_xy[2 * k], by = fp_xy[2 * k + 1];
+        if ((ay > py) != (by > py) && px < ax + (py - ay) * (bx - ax) / (by - ay)) in = !in;
+    }
+    return in;
+}
+
+/* Eq. (3) for one body-frame point */
+double fno_footprint_distance(int V, const float* fp_xy, double px, double py) {
+    if (point_in_polygon(px, py, V, fp_xy)) return 0.0;
+    double d = INFINITY;
+    for (int k = 0, j = V - 1; k < V; j = k++) {
+        const double dk = point_segment_dist(px, py, fp_xy[2 * j], fp_xy[2 * j + 1], fp_xy[2 * k], fp_xy[2 * k + 1]);
+        if (dk < d) d = dk;
+    }
+    return d;
+}
+
+void fno_clearance_features(int V, const float* fp_xy, int B, const float* angles, const float* sensor /*[3] or NULL*/,
+                            float max_range, int n_sectors, int n, const float* ranges /*[n][B]*/,
+                            float* delta /*[n][B] or NULL*/, float* z /*[n][n_sectors]*/) {
+    const double s0 = sensor ? (double)sensor[0] : 0.0, s1 = sensor ? (double)sensor[1] : 0.0,
+                 s2 = sensor ? (double)sensor[2] : 0.0;
+    const double rmax = (double)max_range;
+    for (int e = 0; e < n; ++e) {
+        for (int k = 0; k < n_sectors; ++k) z[(size_t)e * n_sectors + k] = max_range;
+        for (int j = 0; j < B; ++j) {
+            const double r = (double)ranges[(size_t)e * B + j];
+            double d = rmax;                                          /* no valid hit: the maximum range */
+            if (r < rmax) {
+                const double phi = (double)angles[j] + s2;
+                d = fno_footprint_distance(V, fp_xy, s0 + r * cos(phi), s1 + r * sin(phi));
+                if (d > rmax) d = rmax;                               /* capped at the sensor range */
+            }
+            if (delta) delta[(size_t)e * B + j] = (float)d;
+            const int k = (int)(((long long)j * n_sectors) / B);
+            if ((float)d < z[(size_t)e * n_sectors + k]) z[(size_t)e * n_sectors + k] = (float)d;
+        }
     }
 }
 

@@ -292,6 +292,27 @@ def run_ours(args):
             sys.stderr.write(f"bench.py: graph replay leg skipped: {ex!r}\n")
             sim.set_stream(torch.cuda.current_stream())
 
+    # clearance features (Eq. (3)): the extra kernel when they are bound
+    feat = None
+    if args.features > 0:
+        zbuf = torch.zeros(n, args.features, device="cuda")
+        sim.bind_features(args.features, zbuf)
+        for k in range(3):
+            step(k)
+        barrier()
+        sim.profile(True)
+        for k in range(K):
+            flush.fill_(k & 0xff)
+            step(Wm + k)
+        barrier()
+        pf = sim.profile_read()
+        sim.profile(False)
+        sim.bind_features(args.features, None)
+        f_s = pf["features"][0] * 1e-3 / max(1, pf["features"][1])
+        feat = {"n_sectors": args.features, "kernel_ms": f_s * 1e3, "kernel_ms_reset_list": pf["features_reset"][0] / max(1, pf["features_reset"][1]),
+                "beams_per_s": n * B / f_s, "read_GBps": n * B * 4 / f_s / 1e9,
+                "note": "fn::features_kernel over all envs after the beam kernel (ranges read from L2); not in the timed step"}
+
     tmax = torch.tensor([total_ms, steady_ms], device="cuda", dtype=torch.float64)
     rays = torch.tensor([float(c1["rays_cast"] - c0["rays_cast"]), float(c1["envs_reset"] - c0["envs_reset"])],
                         device="cuda", dtype=torch.float64)
@@ -368,7 +389,7 @@ def run_ours(args):
                                       "compact": prof["compact"][0] / K, "reset": prof["reset"][0] / K,
                                       "beam_reset": prof["beam_reset"][0] / K},
                "ms_per_step_p50": float(np.median(per_step_ms)), "ms_per_step_p90": float(np.percentile(per_step_ms, 90)),
-               "roofline": roofline, "cpu_baseline": cpu, "clocks": clocks, "gpu_launches": 5 * K}
+               "features": feat, "roofline": roofline, "cpu_baseline": cpu, "clocks": clocks, "gpu_launches": 5 * K}
 
     # ---- end to end through the public API with HOST buffers (copies inside the timed region)
     hs = torch.empty(8, n, dtype=torch.float32).pin_memory()
@@ -416,6 +437,7 @@ def main():
     ap.add_argument("--cpu-steps", type=int, default=8, help="oracle steps in the cpu_baseline leg")
     ap.add_argument("--e2e-steps", type=int, default=50)
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--features", type=int, default=36, help="sectors of the clearance-feature leg (0 = skip; information only)")
     ap.add_argument("--graph", type=int, default=1, help="also time a CUDA-graph replay of the steps (information only)")
     ap.add_argument("--ring", type=int, default=1, help="attach the replay ring when the config has one (C5)")
     args = ap.parse_args()

@@ -117,6 +117,15 @@ int fn_reset(fn_sim* sim, float* states_dev, const uint8_t* mask_dev, const uint
  * fn_get_counters: synchronises the stream and copies FN_N_COUNTERS u64 counters to host_out.
  * fn_sim_count_words: 1 = also count 32-bit map words loaded by the beam kernel (slower; default 0). */
 int fn_sim_bind_aux(fn_sim* sim, int32_t* out_hit_cell_dev, float* out_reward_dev);
+/* ---- clearance features (Eq. (3)): the policy's obstacle features z_t.
+ * Each valid range endpoint (range < max range) is expressed in the body frame using the sensor placement;
+ * delta_j = its distance to the footprint polygon (0 inside), capped at the max range; beams without a
+ * valid hit get the max range; z_k = min of delta_j over sector k = the beams j with floor(j n_sectors / B) = k
+ * (n_sectors groups of consecutive beams in table order; 1 <= n_sectors <= B).
+ * out_z_dev [N][n_sectors] fp32 is retained until re-bound or destroy (NULL unbinds).  When bound, fn_step
+ * writes the rows of all envs (from its pre-reset ranges), fn_reset rewrites the rows of the reset envs,
+ * fn_observe_all writes all rows. */
+int fn_sim_bind_features(fn_sim* sim, int n_sectors, float* out_z_dev);
 int fn_ring_attach(fn_sim* sim, float* ring_dev, uint64_t capacity_transitions);
 int fn_observe_all(fn_sim* sim, const float* states_dev, float* out_ranges_dev, float* out_goal_obs_dev);
 int fn_get_counters(fn_sim* sim, uint64_t* host_out);
@@ -128,7 +137,7 @@ int fn_sim_episode_state(fn_sim* sim, float* d_prev_host, int32_t* ep_step_host)
 /* ---- live kernel timing (bench.py's roofline): when enabled, fn_step / fn_reset record CUDA events on
  * the sim's stream around their kernels.  fn_sim_profile_read synchronises, adds up the elapsed times
  * since the last read and clears them.  ms_out[8] / launches_out[8] = {env-step kernel, beam kernel of
- * fn_step, compaction kernel, reset kernel, beam kernel of fn_reset (the listed envs), reserved x 3}.
+ * fn_step, compaction kernel, reset kernel, beam kernel of fn_reset (the listed envs), features kernel of fn_step, features kernel of fn_reset, reserved}.
  * Events between kernels keep a kernel from starting under its predecessor (programmatic dependent
  * launch), so a profiled step is a few microseconds slower than an unprofiled one. */
 int fn_sim_profile(fn_sim* sim, int enable);

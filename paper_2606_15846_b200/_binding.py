@@ -18,7 +18,7 @@ COUNTER_NAMES = ("rays_cast", "map_words_loaded", "envs_reset", "reset_failures"
 EXPORTED_SYMBOLS = (
     "fn_map_create", "fn_map_set_regions", "fn_map_destroy", "fn_robot_create", "fn_robot_set_sensor",
     "fn_robot_destroy", "fn_task_default", "fn_sim_create", "fn_sim_destroy", "fn_sim_set_stream", "fn_step", "fn_reset",
-    "fn_sim_bind_aux", "fn_ring_attach", "fn_observe_all", "fn_get_counters", "fn_sim_count_words",
+    "fn_sim_bind_aux", "fn_sim_bind_features", "fn_ring_attach", "fn_observe_all", "fn_get_counters", "fn_sim_count_words",
     "fn_sim_episode_state", "fn_sim_beam_config", "fn_sim_profile", "fn_sim_profile_read", "fn_step_host", "fn_measure_peak", "fn_last_error", "fn_version")
 
 
@@ -59,6 +59,7 @@ def load_library():
         "fn_step": [vp, vp, vp, f32, vp, vp, vp, vp],
         "fn_reset": [vp, vp, vp, vp, vp, vp],
         "fn_sim_bind_aux": [vp, vp, vp],
+        "fn_sim_bind_features": [vp, i32, vp],
         "fn_ring_attach": [vp, vp, u64],
         "fn_observe_all": [vp, vp, vp, vp],
         "fn_get_counters": [vp, vp],
@@ -221,6 +222,14 @@ class Sim:
         _check(load_library().fn_sim_bind_aux(self._h, _dev_ptr(out_hit_cell, torch.int32, n * B, "out_hit_cell"),
                                               _dev_ptr(out_reward, torch.float32, n, "out_reward")), "fn_sim_bind_aux")
 
+    def bind_features(self, n_sectors, out_z=None):
+        """Clearance features z [N, n_sectors] (Eq. (3)); out_z = None unbinds."""
+        import torch
+        self._feat = out_z
+        _check(load_library().fn_sim_bind_features(
+            self._h, int(n_sectors), _dev_ptr(out_z, torch.float32, self.n * int(n_sectors), "out_z")
+            if out_z is not None else None), "fn_sim_bind_features")
+
     def ring_row_floats(self):
         return self.robot.B + 5 + self.robot.A + 2
 
@@ -256,6 +265,7 @@ class Sim:
         return {"env_step": (float(ms[0]), int(ln[0])), "beam_step": (float(ms[1]), int(ln[1])),
                 "compact": (float(ms[2]), int(ln[2])), "reset": (float(ms[3]), int(ln[3])),
                 "beam_reset": (float(ms[4]), int(ln[4])),
+                "features": (float(ms[5]), int(ln[5])), "features_reset": (float(ms[6]), int(ln[6])),
                 "reset_path": (float(ms[2] + ms[3] + ms[4]), int(ln[2] + ln[3] + ln[4]))}
 
     def episode_state(self):

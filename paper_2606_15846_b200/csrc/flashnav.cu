@@ -14,6 +14,7 @@
 #include "fn_beam.cuh"
 #include "fn_common.cuh"
 #include "fn_env.cuh"
+#include "fn_features.cuh"
 
 using namespace fn;
 
@@ -79,6 +80,8 @@ struct fn_sim {
     int32_t* aux_hit;
     float* aux_reward;
     float* ring;
+    float* feat_z;                   // bound clearance-feature output [n][feat_sectors] or NULL
+    int feat_sectors;
     unsigned long long ring_cap;
     unsigned long long* d_ring_head;   // device: slot of env 0's pending ring row
     int count_words;
@@ -439,6 +442,27 @@ static int launch_beams(fn_sim* s, const int* list, const int* count_dev, float*
     return FN_OK;
 }
 
+// clearance features of all envs (list == NULL) or of the listed ones, from the ranges just written
+static int launch_features(fn_sim* s, const int* list, const int* count_dev, bool done_list, const float* ranges) {
+    if (!s->feat_z) return FN_OK;
+    FeatArgs f;
+    f.beam_cs = s->robot->d_beam_cs; f.verts = s->robot->d_verts; f.B = s->robot->B; f.V = s->robot->V;
+    f.n_sectors = s->feat_sectors; f.rmax = s->robot->rmax; f.sx = s->robot->sensor[0]; f.sy = s->robot->sensor[1];
+    f.ranges = ranges; f.z = s->feat_z; f.list = list; f.count_dev = count_dev;
+    f.list_par_dev = done_list ? s->d_done_count + 2 : nullptr; f.n_all = s->n;
+    int grid = (s->n + kFeatWarps - 1) / kFeatWarps;
+    if (grid > s->num_sms * 8) grid = s->num_sms * 8;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    if (s->prof) {
+        FN_CUDA(cudaEventCreate(&e0)); FN_CUDA(cudaEventCreate(&e1));
+        s->ev->push_back(e0); s->ev->push_back(e1); s->ev_kind->push_back(list ? 3 : 2);
+        FN_CUDA(cudaEventRecord(e0, s->stream));
+    }
+    FN_CUDA(launch_pdl(features_kernel, dim3(grid), dim3(kFeatWarps * 32), feat_smem_bytes(f.V, f.n_sectors, f.B), s->stream, f));
+    if (s->prof) FN_CUDA(cudaEventRecord(e1, s->stream));
+    return FN_OK;
+}
+
 extern "C" int fn_step(fn_sim* s, float* states, const float* actions, float dt, uint8_t* reset_mask,
                        float* out_ranges, uint8_t* out_collision, float* out_goal_obs) {
     if (!s || !states || !actions || !reset_mask || !out_ranges || !out_collision || !out_goal_obs)
@@ -466,6 +490,7 @@ extern "C" int fn_step(fn_sim* s, float* states, const float* actions, float dt,
     }
     int rc = launch_beams(s, nullptr, nullptr, out_ranges, true);
     if (s->prof && rc == FN_OK) FN_CUDA(cudaEventRecord(e2, s->stream));
+    if (rc == FN_OK) rc = launch_features(s, nullptr, nullptr, false, out_ranges);
     s->done_avail = 1;
     return rc;
 }
@@ -502,6 +527,7 @@ extern "C" int fn_reset(fn_sim* s, float* states, const uint8_t* mask, const uin
     if (s->prof) FN_CUDA(cudaEventRecord(e2, s->stream));
     int rc = launch_beams(s, list, count, out_ranges, false, mask == nullptr);
     if (s->prof && rc == FN_OK) FN_CUDA(cudaEventRecord(e3, s->stream));
+    if (rc == FN_OK) rc = launch_features(s, list, count, mask == nullptr, out_ranges);
     return rc;
 }
 
@@ -516,12 +542,23 @@ extern "C" int fn_observe_all(fn_sim* s, const float* states, float* out_ranges,
     s->ring = nullptr;
     int st = launch_beams(s, nullptr, nullptr, out_ranges);
     s->ring = ring;
+    if (st == FN_OK) st = launch_features(s, nullptr, nullptr, false, out_ranges);
     return st;
 }
 
 extern "C" int fn_sim_bind_aux(fn_sim* s, int32_t* hit, float* reward) {
     if (!s) return fail(FN_ERR_INVALID_ARG, "fn_sim_bind_aux: NULL sim");
     s->aux_hit = hit; s->aux_reward = reward;
+    return FN_OK;
+}
+
+extern "C" int fn_sim_bind_features(fn_sim* s, int n_sectors, float* out_z) {
+    if (!s) return fail(FN_ERR_INVALID_ARG, "fn_sim_bind_features: NULL sim");
+    if (out_z && (n_sectors < 1 || n_sectors > s->robot->B))
+        return fail(FN_ERR_INVALID_ARG, "fn_sim_bind_features: n_sectors must be in 1..B");
+    if (out_z && feat_smem_bytes(s->robot->V, n_sectors, s->robot->B) > 48 * 1024)
+        return fail(FN_ERR_UNSUPPORTED, "fn_sim_bind_features: too many sectors for shared memory");
+    s->feat_z = out_z; s->feat_sectors = out_z ? n_sectors : 0;
     return FN_OK;
 }
 
@@ -559,6 +596,9 @@ extern "C" int fn_sim_profile_read(fn_sim* s, double* ms_out, uint64_t* launches
             FN_CUDA(cudaEventElapsedTime(&ms, (*s->ev)[i], (*s->ev)[i + 1])); ms_out[0] += ms; launches_out[0] += 1;
             FN_CUDA(cudaEventElapsedTime(&ms, (*s->ev)[i + 1], (*s->ev)[i + 2])); ms_out[1] += ms; launches_out[1] += 1;
             i += 3;
+        } else if (kind >= 2) {                                    // features kernel: all envs (2) / listed envs (3)
+            FN_CUDA(cudaEventElapsedTime(&ms, (*s->ev)[i], (*s->ev)[i + 1])); ms_out[3 + kind] += ms; launches_out[3 + kind] += 1;
+            i += 2;
         } else {
             for (int k = 0; k < 3; ++k) {
                 FN_CUDA(cudaEventElapsedTime(&ms, (*s->ev)[i + k], (*s->ev)[i + k + 1])); ms_out[2 + k] += ms; launches_out[2 + k] += 1;

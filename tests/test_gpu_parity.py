@@ -274,3 +274,59 @@ def test_reset_of_the_steps_done_list_equals_masked_reset(pu):
         s.close(); r.close(); m.close()
     assert torch.equal(out[0][0], out[1][0]) and torch.equal(out[0][1], out[1][1]) and torch.equal(out[0][2], out[1][2])
     assert out[0][3] == out[1][3] > n and out[0][4] == out[1][4]
+
+
+def test_clearance_features_against_the_oracle(pu):
+    # NEXT-1 (Eq. (3)): sector-pooled footprint clearances.  Teacher-forced:
+    # the oracle computes them in fp64 from the GPU's own fp32 ranges; tolerance 1e-4 m like the ranges
+    # (the clearance is continuous across the polygon boundary, so there is no near-tie class).
+    import torch
+    import oracle
+    from harness import workloads as W
+    cases = ((2, 300, 36, None), (3, 257, 24, (0.1, -0.05, 0.2)), (1, 64, 360, None), (5, 200, 7, None))
+    for cfg, n, ns, sensor in cases:
+        wl = W.make_workload(cfg, n_envs=n)
+        B, A = wl.n_beams, wl.action_dim
+        m, r, s = pu.make_sim(wl, n)
+        if sensor is not None:
+            r.set_sensor(*sensor)
+        buf = pu.Buffers(n, B, A)
+        z = torch.full((n, ns), -1.0, device="cuda")
+        s.bind_features(ns, z)
+        steps = 6
+        actions = torch.from_numpy(W.action_tape(wl, steps, 2)).cuda()
+        seeds = torch.from_numpy(W.seed_tape(wl, steps + 1, 2).view(np.int64)).cuda()
+        forced = torch.from_numpy(W.forced_reset_tape(wl, steps, 2)).cuda()
+
+        def expect():
+            return oracle.clearance_features(wl.footprint, wl.beam_angles, wl.max_range, ns, buf.ranges.cpu().numpy(),
+                                             sensor=None if sensor is None else np.array(sensor, np.float32))
+
+        buf.mask.fill_(1)
+        s.reset(buf.states, buf.mask, seeds[0], buf.ranges, buf.gobs)
+        torch.cuda.synchronize()
+        assert np.abs(z.cpu().numpy() - expect()).max() <= 1e-4
+        n_reset = 0
+        for t in range(steps):
+            buf.mask.copy_(forced[t])
+            s.step(buf.states, actions[t], float(wl.dt), buf.mask, buf.ranges, buf.col, buf.gobs)
+            torch.cuda.synchronize()
+            zs = z.cpu().numpy().copy()
+            assert np.abs(zs - expect()).max() <= 1e-4, f"cfg {cfg} step {t}"
+            done = buf.mask.cpu().numpy() != 0
+            s.reset(buf.states, None if t % 2 else buf.mask, seeds[t + 1], buf.ranges, buf.gobs)
+            torch.cuda.synchronize()
+            zr = z.cpu().numpy()
+            assert np.array_equal(zr[~done], zs[~done])            # only the reset envs' rows are rewritten
+            assert np.abs(zr - expect()).max() <= 1e-4, f"cfg {cfg} step {t} after reset"
+            n_reset += int(done.sum())
+        assert n_reset > 0
+        # features are a pure function of the ranges: a full recompute reproduces the maintained rows
+        z2 = torch.empty_like(z)
+        s.bind_features(ns, z2)
+        full_r = torch.empty_like(buf.ranges)
+        s.observe_all(buf.states, full_r)
+        torch.cuda.synchronize()
+        assert torch.equal(z2, z)
+        s.bind_features(ns, None)
+        s.close(); r.close(); m.close()

@@ -179,6 +179,26 @@ def ring_append(ring, capacity, head, obs_ranges, obs_goal, obs_vel, actions, re
                           _p(done, C.c_uint8))
 
 
+def sample_slot(seed: int, i: int, filled: int) -> int:
+    f = lib().fno_sample_slot
+    f.restype = C.c_uint64
+    f.argtypes = [C.c_uint64, C.c_uint64, C.c_uint64]
+    return int(f(seed, i, filled))
+
+
+def ring_sample(ring, capacity, filled, n_envs, B, A, seed, n_samples, want_next=True):
+    """Uniform replay sampling.  ring [capacity, B+5+A+2] f32 -> rows [n,row], next_obs [n,B+5], slots [n]."""
+    assert ring.dtype == np.float32 and ring.flags.c_contiguous
+    row = B + 5 + A + 2
+    rows = np.empty((n_samples, row), np.float32)
+    nxt = np.empty((n_samples, B + 5), np.float32) if want_next else None
+    slots = np.empty(n_samples, np.int64)
+    lib().fno_ring_sample(_p(ring, C.c_float), C.c_uint64(capacity), C.c_uint64(filled), C.c_int(n_envs), C.c_int(B),
+                          C.c_int(A), C.c_uint64(seed), C.c_int(n_samples), _p(rows, C.c_float),
+                          _p(nxt, C.c_float), _p(slots, C.c_int64))
+    return rows, nxt, slots
+
+
 def footprint_distance(footprint, px, py) -> float:
     """Eq. (3) for one body-frame point: distance to the polygon, 0 inside."""
     fp = _f32(footprint)

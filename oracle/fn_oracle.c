@@ -19,6 +19,7 @@
  *   O7     reset of masked envs (PAPER.md:86, :199 say THAT envs are reset; the sampling rule is
  *          reading G16 -- "parity unpinned" by the paper, pinned by invariants only).
  *   O9     transition row for the replay ring (BASELINE.json config 5).
+ *   O11    uniform replay sampling: readings G22 in DESIGN.md.
  *   O10    clearance features, Eq. (3) and their sector min-pooling:
  *          SURVEY 8(f) NEXT-1.  The sector layout is reading G21.
  *   plus the paper's own two approximations as brute-force cross-checks:
@@ -578,6 +579,35 @@ void fno_clearance_features(int V, const float* fp_xy, int B, const float* angle
             const int k = (int)(((long long)j * n_sectors) / B);
             if ((float)d < z[(size_t)e * n_sectors + k]) z[(size_t)e * n_sectors + k] = (float)d;
         }
+    }
+}
+
+/* ------------------------------------------------------------------ O11: replay sampling (NEXT-2)
+ * "Each replay batch contains U x B transitions sampled uniformly from replay and divided
+ * into U minibatches of size B."  Readings (G22): sample i of a batch draws slot_i = floor(w_i filled /
+ * 2^64) with w_i = SplitMix64(seed, i) (the counter-based generator of O7), i.e. uniform over the
+ * `filled` completed rows [0, filled) of the ring (filled = min(rows appended, capacity); a ring that
+ * has wrapped is full, one that has not is filled from slot 0); the batch row is the ring row
+ * (obs, action, reward, done) as stored; the next observation is the obs part of the SAME env's next
+ * row, slot + n_envs (mod capacity), which the step that completed the row has already written.
+ * (For a done transition that is the post-reset observation; the done flag masks the bootstrap.)
+ */
+uint64_t fno_sample_slot(uint64_t seed, uint64_t i, uint64_t filled) {
+    const uint64_t w = fno_splitmix64(seed, i);
+    return (uint64_t)(((unsigned __int128)w * (unsigned __int128)filled) >> 64);
+}
+
+void fno_ring_sample(const float* ring, uint64_t capacity, uint64_t filled, int n_envs, int B, int A,
+                     uint64_t seed, int n_samples, float* out_rows /*[n_samples][row]*/,
+                     float* out_next_obs /*[n_samples][B+5] or NULL*/, int64_t* out_slots /*or NULL*/) {
+    const size_t row = (size_t)B + 5 + (size_t)A + 2, obs = (size_t)B + 5;
+    for (int i = 0; i < n_samples; ++i) {
+        const uint64_t slot = fno_sample_slot(seed, (uint64_t)i, filled);
+        memcpy(out_rows + (size_t)i * row, ring + (size_t)slot * row, row * sizeof(float));
+        if (out_next_obs)
+            memcpy(out_next_obs + (size_t)i * obs, ring + (size_t)((slot + (uint64_t)n_envs) % capacity) * row,
+                   obs * sizeof(float));
+        if (out_slots) out_slots[i] = (int64_t)slot;
     }
 }
 

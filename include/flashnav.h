@@ -127,6 +127,18 @@ int fn_sim_bind_aux(fn_sim* sim, int32_t* out_hit_cell_dev, float* out_reward_de
  * fn_observe_all writes all rows. */
 int fn_sim_bind_features(fn_sim* sim, int n_sectors, float* out_z_dev);
 int fn_ring_attach(fn_sim* sim, float* ring_dev, uint64_t capacity_transitions);
+/* ---- uniform replay sampling ("Each replay batch contains U x B transitions sampled uniformly
+ * from replay and divided into U minibatches of size B"): gathers n_samples = U * B ring rows.
+ * Sample i = the row at slot floor(SplitMix64(seed, i) * filled / 2^64), filled = min(rows completed, capacity),
+ * i.e. uniform over the completed rows (with replacement); nothing is written while the ring is empty.
+ * out_rows_dev [n_samples][B + 5 + A + 2] fp32: rows as stored (obs, action, reward, done);
+ * out_next_obs_dev [n_samples][B + 5] or NULL: the obs part of the same env's next row (slot + n_envs mod
+ * capacity), which the step that completed the row has already written (for a done transition that is the
+ * post-reset observation; the done flag masks the bootstrap).
+ * Enqueued on the sim's stream, i.e. after the ring writes of earlier fn_step / fn_reset calls ("sampling waits
+ * for the required replay writes"); the paper's two preallocated batch buffers are the caller's: alternate the
+ * output pointers between calls and order the learner after the call with a stream or an event. */
+int fn_ring_sample(fn_sim* sim, uint64_t seed, int n_samples, float* out_rows_dev, float* out_next_obs_dev);
 int fn_observe_all(fn_sim* sim, const float* states_dev, float* out_ranges_dev, float* out_goal_obs_dev);
 int fn_get_counters(fn_sim* sim, uint64_t* host_out);
 int fn_sim_count_words(fn_sim* sim, int enable);

@@ -18,7 +18,7 @@ COUNTER_NAMES = ("rays_cast", "map_words_loaded", "envs_reset", "reset_failures"
 EXPORTED_SYMBOLS = (
     "fn_map_create", "fn_map_set_regions", "fn_map_destroy", "fn_robot_create", "fn_robot_set_sensor",
     "fn_robot_destroy", "fn_task_default", "fn_sim_create", "fn_sim_destroy", "fn_sim_set_stream", "fn_step", "fn_reset",
-    "fn_sim_bind_aux", "fn_sim_bind_features", "fn_ring_attach", "fn_observe_all", "fn_get_counters", "fn_sim_count_words",
+    "fn_sim_bind_aux", "fn_sim_bind_features", "fn_ring_attach", "fn_ring_sample", "fn_observe_all", "fn_get_counters", "fn_sim_count_words",
     "fn_sim_episode_state", "fn_sim_beam_config", "fn_sim_profile", "fn_sim_profile_read", "fn_step_host", "fn_measure_peak", "fn_last_error", "fn_version")
 
 
@@ -61,6 +61,7 @@ def load_library():
         "fn_sim_bind_aux": [vp, vp, vp],
         "fn_sim_bind_features": [vp, i32, vp],
         "fn_ring_attach": [vp, vp, u64],
+        "fn_ring_sample": [vp, u64, i32, vp, vp],
         "fn_observe_all": [vp, vp, vp, vp],
         "fn_get_counters": [vp, vp],
         "fn_sim_count_words": [vp, i32],
@@ -238,6 +239,16 @@ class Sim:
         self._ring = ring
         _check(load_library().fn_ring_attach(self._h, _dev_ptr(ring, torch.float32, capacity * self.ring_row_floats(), "ring")
                                              if ring is not None else None, C.c_uint64(capacity)), "fn_ring_attach")
+
+    def ring_sample(self, seed, out_rows, out_next_obs=None):
+        """Uniform replay batch: out_rows [n, row] (, out_next_obs [n, B + 5]) gathered from the ring."""
+        import torch
+        n = int(out_rows.shape[0])
+        _check(load_library().fn_ring_sample(
+            self._h, C.c_uint64(int(seed) & ((1 << 64) - 1)), n,
+            _dev_ptr(out_rows, torch.float32, n * self.ring_row_floats(), "out_rows"),
+            _dev_ptr(out_next_obs, torch.float32, n * (self.robot.B + 5), "out_next_obs")
+            if out_next_obs is not None else None), "fn_ring_sample")
 
     def observe_all(self, states, out_ranges, out_goal_obs=None):
         import torch

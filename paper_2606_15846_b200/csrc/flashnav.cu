@@ -333,8 +333,8 @@ extern "C" int fn_sim_create(const fn_map* map, const fn_robot* robot, int n, co
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&s->num_sms, cudaDevAttrMultiProcessorCount, dev);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
     if (e == cudaSuccess) e = cudaMalloc(&s->d_poses, (size_t)n * sizeof(BeamPose));
-    if (e == cudaSuccess) e = cudaMalloc(&s->d_ring_head, sizeof(unsigned long long));
-    if (e == cudaSuccess) e = cudaMemsetAsync(s->d_ring_head, 0, sizeof(unsigned long long), s->stream);
+    if (e == cudaSuccess) e = cudaMalloc(&s->d_ring_head, 2 * sizeof(unsigned long long));
+    if (e == cudaSuccess) e = cudaMemsetAsync(s->d_ring_head, 0, 2 * sizeof(unsigned long long), s->stream);
     if (e == cudaSuccess) e = cudaMalloc(&s->d_list, (size_t)n * sizeof(int));
     if (e == cudaSuccess) e = cudaMalloc(&s->d_count, sizeof(int));
     if (e == cudaSuccess) e = cudaMalloc(&s->d_dprev, (size_t)n * sizeof(float));
@@ -566,7 +566,21 @@ extern "C" int fn_ring_attach(fn_sim* s, float* ring, uint64_t cap) {
     if (!s) return fail(FN_ERR_INVALID_ARG, "fn_ring_attach: NULL sim");
     if (ring && cap < (uint64_t)s->n) return fail(FN_ERR_INVALID_ARG, "fn_ring_attach: capacity must be >= n_envs");
     s->ring = ring; s->ring_cap = ring ? cap : 0;
-    FN_CUDA(cudaMemsetAsync(s->d_ring_head, 0, sizeof(unsigned long long), s->stream));
+    FN_CUDA(cudaMemsetAsync(s->d_ring_head, 0, 2 * sizeof(unsigned long long), s->stream));
+    return FN_OK;
+}
+
+extern "C" int fn_ring_sample(fn_sim* s, uint64_t seed, int n_samples, float* out_rows, float* out_next_obs) {
+    if (!s || !out_rows) return fail(FN_ERR_INVALID_ARG, "fn_ring_sample: NULL argument");
+    if (!s->ring) return fail(FN_ERR_INVALID_ARG, "fn_ring_sample: no ring attached");
+    if (n_samples < 1) return fail(FN_ERR_INVALID_ARG, "fn_ring_sample: n_samples must be >= 1");
+    SampleArgs a;
+    a.ring = s->ring; a.head = s->d_ring_head; a.cap = s->ring_cap; a.seed = seed; a.n_envs = s->n;
+    a.row = ring_row_floats(s); a.obs = s->robot->B + 5; a.n_samples = n_samples;
+    a.out_rows = out_rows; a.out_next_obs = out_next_obs;
+    int grid = (n_samples + 7) / 8;
+    if (grid > s->num_sms * 64) grid = s->num_sms * 64;
+    FN_CUDA(launch_pdl(ring_sample_kernel, dim3(grid), dim3(256), 0, s->stream, a));
     return FN_OK;
 }
 

@@ -370,11 +370,48 @@ __global__ void __launch_bounds__(kEnvBlock) env_step_kernel(EnvArgs a) {
     if (bad) atomicAdd(&a.counters[kNonFinite], 1ull);
 }
 
-// advances the replay ring's head by n rows (one thread), after the env-step kernel of fn_step
+// advances the replay ring's head by n rows (one thread), after the env-step kernel of fn_step;
+// head[1] counts the rows completed so far (the sampler's `filled` = min(head[1], capacity))
 __global__ void ring_advance_kernel(unsigned long long* head, unsigned long long n, unsigned long long cap) {
     griddep_wait();
     griddep_launch_dependents();
-    *head = (*head + n) % cap;
+    head[0] = (head[0] + n) % cap;
+    head[1] += n;
+}
+
+// ---------------------------------------------------------------- NEXT-2: uniform replay sampling
+// "Each replay batch contains U x B transitions sampled uniformly from replay".  Sample i =
+// the ring row at slot floor(SplitMix64(seed, i) filled / 2^64) (reading G22); optionally the next
+// observation = the obs part of the same env's next row (slot + n_envs mod capacity).  A gather of
+// whole rows: one warp per sample, lanes stride over the row (rows start at 4-byte alignment only), so
+// every warp instruction moves 128 contiguous bytes; the kernel is HBM-bound.
+__device__ __forceinline__ unsigned long long splitmix64_at(unsigned long long sigma, unsigned long long c);
+struct SampleArgs {
+    const float* ring;
+    const unsigned long long* head;      // [2]: head, rows completed
+    unsigned long long cap, seed;
+    int n_envs, row, obs, n_samples;
+    float* out_rows;                     // [n_samples][row]
+    float* out_next_obs;                 // [n_samples][obs] or NULL
+};
+__global__ void __launch_bounds__(256) ring_sample_kernel(SampleArgs a) {
+    griddep_wait();
+    griddep_launch_dependents();
+    const unsigned long long total = a.head[1];
+    const unsigned long long filled = total < a.cap ? total : a.cap;
+    if (filled == 0ull) return;
+    const int lane = threadIdx.x & 31;
+    for (int i = blockIdx.x * 8 + (threadIdx.x >> 5); i < a.n_samples; i += gridDim.x * 8) {
+        const unsigned long long slot = __umul64hi(splitmix64_at(a.seed, (unsigned long long)i), filled);
+        const float* src = a.ring + slot * (unsigned long long)a.row;
+        float* dst = a.out_rows + (size_t)i * a.row;
+        for (int k = lane; k < a.row; k += 32) dst[k] = __ldg(src + k);
+        if (a.out_next_obs) {
+            const float* nsrc = a.ring + ((slot + (unsigned long long)a.n_envs) % a.cap) * (unsigned long long)a.row;
+            float* ndst = a.out_next_obs + (size_t)i * a.obs;
+            for (int k = lane; k < a.obs; k += 32) ndst[k] = __ldg(nsrc + k);
+        }
+    }
 }
 
 // ---------------------------------------------------------------- S6: ordered compaction of a u8 mask

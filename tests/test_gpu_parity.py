@@ -330,3 +330,47 @@ def test_clearance_features_against_the_oracle(pu):
         assert torch.equal(z2, z)
         s.bind_features(ns, None)
         s.close(); r.close(); m.close()
+
+
+def test_replay_sampling_against_the_oracle(pu):
+    # NEXT-2: U x B transitions sampled uniformly from the device ring.  A gather: bit-exact
+    # against the oracle's fno_ring_sample on the GPU's own ring, before and after the ring has wrapped,
+    # with and without the next-observation output; an empty ring writes nothing.
+    import torch
+    import oracle
+    from harness import workloads as W
+    wl = W.make_workload(5, n_envs=64)
+    n, B, A = wl.n_envs, wl.n_beams, wl.action_dim
+    m, r, s = pu.make_sim(wl, n)
+    buf = pu.Buffers(n, B, A)
+    cap = 5 * n + 13
+    row = B + 5 + A + 2
+    ring = torch.zeros(cap * row, device="cuda")
+    s.ring_attach(ring, cap)
+    ns = 777
+    rows = torch.full((ns, row), -7.0, device="cuda")
+    nxt = torch.full((ns, B + 5), -7.0, device="cuda")
+    s.ring_sample(5, rows, nxt)
+    torch.cuda.synchronize()
+    assert float(rows.min()) == -7.0 and float(nxt.max()) == -7.0        # empty ring: nothing written
+    steps = 8
+    actions = torch.from_numpy(W.action_tape(wl, steps, 4)).cuda()
+    seeds = torch.from_numpy(W.seed_tape(wl, steps + 1, 4).view(np.int64)).cuda()
+    buf.mask.fill_(1)
+    s.reset(buf.states, buf.mask, seeds[0], buf.ranges, buf.gobs)
+    for t in range(steps):
+        buf.mask.zero_()
+        s.step(buf.states, actions[t], float(wl.dt), buf.mask, buf.ranges, buf.col, buf.gobs)
+        s.reset(buf.states, None, seeds[t + 1], buf.ranges, buf.gobs)
+        filled = min((t + 1) * n, cap)
+        for seed, with_next in ((1000 + t, True), (2**63 + 12345 + t, False)):
+            s.ring_sample(seed, rows, nxt if with_next else None)
+            torch.cuda.synchronize()
+            ring_np = ring.cpu().numpy().reshape(cap, row)
+            er, en, slots = oracle.ring_sample(ring_np, cap, filled, n, B, A, seed, ns)
+            assert slots.max() < filled
+            assert np.array_equal(rows.cpu().numpy(), er)
+            if with_next:
+                assert np.array_equal(nxt.cpu().numpy(), en)
+    assert steps * n > cap                                                 # the ring has wrapped
+    s.close(); r.close(); m.close()

@@ -313,6 +313,39 @@ def run_ours(args):
                 "beams_per_s": n * B / f_s, "read_GBps": n * B * 4 / f_s / 1e9,
                 "note": "fn::features_kernel over all envs after the beam kernel (ranges read from L2); not in the timed step"}
 
+    # replay sampling: U x B transitions gathered from the ring (HBM-bound)
+    sample = None
+    if ring is not None and args.sample_batch > 0:
+        ns = args.sample_batch
+        rowf = sim.ring_row_floats()
+        bufs = [(torch.empty(ns, rowf, device="cuda"), torch.empty(ns, B + 5, device="cuda")) for _ in range(2)]
+        for k in range(3):
+            sim.ring_sample(k, *bufs[k & 1])
+        barrier()
+        reps = 20
+        q0, q1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        tot = 0.0
+        for k in range(reps):
+            flush.fill_(k & 0xff)
+            q0.record()
+            sim.ring_sample(100 + k, *bufs[k & 1])               # the paper's two batch buffers, alternating
+            q1.record()
+            torch.cuda.synchronize()
+            tot += q0.elapsed_time(q1)
+        s_s = tot * 1e-3 / reps
+        nbytes = ns * (rowf + B + 5) * 4 * 2                     # rows + next obs, read + write
+        hbm = None
+        try:
+            hbm = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]
+        except Exception:                                        # noqa: BLE001
+            pass
+        peak = hbm if hbm else 6650.0
+        sample = {"n_samples": ns, "kernel_ms": s_s * 1e3, "transitions_per_s": ns / s_s,
+                  "roofline": {"bound": "hbm", "achieved": nbytes / s_s / 1e9, "peak": peak, "unit": "GB/s",
+                               "frac": nbytes / s_s / 1e9 / peak,
+                               "peak_source": "MEASURED_PEAKS.json hbm_gbs (of measured)" if hbm else "guide fallback 6.65 TB/s (of fallback)"},
+                  "note": "fn::ring_sample_kernel: rows + next observations, L2 flushed before each call; not in the timed step"}
+
     tmax = torch.tensor([total_ms, steady_ms], device="cuda", dtype=torch.float64)
     rays = torch.tensor([float(c1["rays_cast"] - c0["rays_cast"]), float(c1["envs_reset"] - c0["envs_reset"])],
                         device="cuda", dtype=torch.float64)
@@ -389,7 +422,7 @@ def run_ours(args):
                                       "compact": prof["compact"][0] / K, "reset": prof["reset"][0] / K,
                                       "beam_reset": prof["beam_reset"][0] / K},
                "ms_per_step_p50": float(np.median(per_step_ms)), "ms_per_step_p90": float(np.percentile(per_step_ms, 90)),
-               "features": feat, "roofline": roofline, "cpu_baseline": cpu, "clocks": clocks, "gpu_launches": 5 * K}
+               "features": feat, "replay_sample": sample, "roofline": roofline, "cpu_baseline": cpu, "clocks": clocks, "gpu_launches": 5 * K}
 
     # ---- end to end through the public API with HOST buffers (copies inside the timed region)
     hs = torch.empty(8, n, dtype=torch.float32).pin_memory()
@@ -437,6 +470,7 @@ def main():
     ap.add_argument("--cpu-steps", type=int, default=8, help="oracle steps in the cpu_baseline leg")
     ap.add_argument("--e2e-steps", type=int, default=50)
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--sample-batch", type=int, default=65536, help="U x B of the replay-sampling leg (configs with a ring; 0 = skip)")
     ap.add_argument("--features", type=int, default=36, help="sectors of the clearance-feature leg (0 = skip; information only)")
     ap.add_argument("--graph", type=int, default=1, help="also time a CUDA-graph replay of the steps (information only)")
     ap.add_argument("--ring", type=int, default=1, help="attach the replay ring when the config has one (C5)")

@@ -52,12 +52,14 @@ def splitmix64(sigma: int, c: int) -> int:
     return int(lib().fno_splitmix64(C.c_uint64(sigma), C.c_uint64(c)))
 
 
-def motion(drive, lim, dt, states, actions):
+def motion(drive, lim, dt, states, actions, acc=None):
+    """acc = None or [3] = maximum accelerations (a_x, a_y, a_w); inf = unlimited (reading G2)."""
     states, actions, lim = _f32(states), _f32(actions), _f32(lim)
+    acc = None if acc is None else _f32(acc)
     n = states.shape[1]
     out = np.empty_like(states)
-    lib().fno_motion(C.c_int(drive), _p(lim, C.c_float), C.c_float(dt), C.c_int(n),
-                     _p(states, C.c_float), _p(actions, C.c_float), _p(out, C.c_float))
+    lib().fno_motion_acc(C.c_int(drive), _p(lim, C.c_float), _p(acc, C.c_float), C.c_float(dt), C.c_int(n),
+                         _p(states, C.c_float), _p(actions, C.c_float), _p(out, C.c_float))
     return out
 
 

@@ -65,8 +65,17 @@ static double wrap_pi(double a) {                               /* to [-pi, pi) 
  *   psi' = wrap(psi + th),  v' = clipped command.
  * states: SoA planes [8][n] = x, y, psi, vx, vy, w, gx, gy.  actions: [n][A].
  */
-void fno_motion(int drive, const float* lim /*[6]*/, float dt_f, int n,
-                const float* s_in, const float* actions, float* s_out) {
+/* acc = NULL or [3] = a_x, a_y, a_w maxima (reading G2, NEXT-3: U "contains velocity and acceleration
+ * limits"): the clipped command is further limited to the previous applied velocity
+ * +- a_max dt, both bounds single fp32 fused operations (velocities are stored in fp32); +inf = no limit. */
+static float slew(float u, float v_prev, float a_max, float dt) {
+    if (!(a_max < INFINITY)) return u;
+    const float lo = fmaf(-a_max, dt, v_prev), hi = fmaf(a_max, dt, v_prev);
+    return fminf(fmaxf(u, lo), hi);
+}
+
+void fno_motion_acc(int drive, const float* lim /*[6]*/, const float* acc /*[3] or NULL*/, float dt_f, int n,
+                    const float* s_in, const float* actions, float* s_out) {
     const int A = (drive == FNO_DRIVE_DIFF) ? 2 : 3;
     const double dt = (double)dt_f;
     for (int e = 0; e < n; ++e) {
@@ -78,6 +87,11 @@ void fno_motion(int drive, const float* lim /*[6]*/, float dt_f, int n,
         vx = fmin(fmax(vx, (double)lim[0]), (double)lim[1]);
         if (drive == FNO_DRIVE_OMNI) vy = fmin(fmax(vy, (double)lim[2]), (double)lim[3]);
         w = fmin(fmax(w, (double)lim[4]), (double)lim[5]);
+        if (acc) {
+            vx = (double)slew((float)vx, s_in[3 * n + e], acc[0], dt_f);
+            if (drive == FNO_DRIVE_OMNI) vy = (double)slew((float)vy, s_in[4 * n + e], acc[1], dt_f);
+            w = (double)slew((float)w, s_in[5 * n + e], acc[2], dt_f);
+        }
         /* O2 */
         double th = w * dt, Ac, Cc;
         if (fabs(th) < 1e-8) { Ac = 1.0 - th * th / 6.0; Cc = th / 2.0; }
@@ -93,6 +107,11 @@ void fno_motion(int drive, const float* lim /*[6]*/, float dt_f, int n,
         s_out[6 * n + e] = s_in[6 * n + e];
         s_out[7 * n + e] = s_in[7 * n + e];
     }
+}
+
+void fno_motion(int drive, const float* lim /*[6]*/, float dt_f, int n,
+                const float* s_in, const float* actions, float* s_out) {
+    fno_motion_acc(drive, lim, NULL, dt_f, n, s_in, actions, s_out);
 }
 
 /* ------------------------------------------------------------------ O5: goal observation

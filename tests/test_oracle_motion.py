@@ -140,3 +140,36 @@ def test_done_sources(oracle_lib):
                                      np.array([0, 0, 0, 1], np.uint8), d_prev, ep, max_episode_steps=10)
     assert list(done) == [0, 0, 1, 1] and np.allclose(r, 2.0)
     assert list(ep) == [1, 9, 10, 1]
+
+
+def test_acceleration_limits_ramp_and_no_limit(oracle_lib):
+    # reading G2 (U holds velocity AND acceleration limits): the clipped command is limited to the
+    # previous applied velocity +- a_max dt.  From rest with a constant command the velocity is the ramp
+    # min(k a dt, v*); deceleration is symmetric; +inf reproduces the unlimited update bit for bit.
+    lim = np.array([-0.5, 1.5, -1, 1, -2.5, 2.5], np.float32)
+    dt = np.float32(0.1)
+    for drive, act in ((0, [1.2, -2.0]), (1, [1.2, -0.7, 2.0])):
+        acc = np.array([2.0, 1.0, 4.0], np.float32)
+        st = np.zeros((8, 1), np.float32)
+        a = np.array([act], np.float32)
+        for k in range(1, 12):
+            st = oracle_lib.motion(drive, lim, dt, st, a, acc=acc)
+            tgt = [act[0], 0.0 if drive == 0 else act[1], act[-1]]
+            for p, (v_star, amax) in enumerate(zip(tgt, acc)):
+                expect = np.sign(v_star) * min(k * amax * 0.1, abs(v_star))
+                assert abs(st[3 + p, 0] - expect) < 2e-6, (drive, k, p)
+        # brake: command zero, every component approaches 0 by at most a dt per step and never overshoots
+        z = np.zeros_like(a)
+        prev = st.copy()
+        for k in range(20):
+            st = oracle_lib.motion(drive, lim, dt, st, z, acc=acc)
+            assert np.all(np.abs(st[3:6, 0]) <= np.abs(prev[3:6, 0]) + 1e-7)
+            assert np.all(np.abs(st[3:6, 0] - prev[3:6, 0]) <= acc * 0.1 + 1e-6)
+            prev = st.copy()
+        assert np.all(st[3:6, 0] == 0.0)
+        # +inf = no limit, bit for bit
+        rng = np.random.default_rng(0)
+        s0 = rng.uniform(-1, 1, (8, 50)).astype(np.float32)
+        aa = rng.uniform(-3, 3, (50, len(act))).astype(np.float32)
+        inf = np.full(3, np.inf, np.float32)
+        assert np.array_equal(oracle_lib.motion(drive, lim, dt, s0, aa, acc=inf), oracle_lib.motion(drive, lim, dt, s0, aa))

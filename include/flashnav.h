@@ -64,6 +64,10 @@ int fn_robot_create(const float* footprint_xy_host, int V, const float* beam_ang
                     float max_range_m, int drive_type, const float* vel_limits_host, fn_robot** out);
 /* sensor placement S in the body frame; default (0, 0, 0). */
 int fn_robot_set_sensor(fn_robot* robot, float sx_m, float sy_m, float spsi_rad);
+/* acceleration limits of U: acc_host [3] = maximum |dv_x/dt|, |dv_y/dt|, |dw/dt| (> 0; +inf = none,
+ * the default).  The clipped command is limited to the previous applied velocity (state planes 3..5)
+ * +- a_max dt before the motion update.  Takes effect for sims created afterwards AND existing ones. */
+int fn_robot_set_acc_limits(fn_robot* robot, const float* acc_host);
 int fn_robot_destroy(fn_robot* robot);
 
 /* ---- task parameters (Eq. (1); defaults via fn_task_default) ---------------------- */

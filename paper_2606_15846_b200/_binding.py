@@ -16,7 +16,7 @@ COUNTER_NAMES = ("rays_cast", "map_words_loaded", "envs_reset", "reset_failures"
                  "env_steps", "reserved0", "reserved1")
 
 EXPORTED_SYMBOLS = (
-    "fn_map_create", "fn_map_set_regions", "fn_map_destroy", "fn_robot_create", "fn_robot_set_sensor",
+    "fn_map_create", "fn_map_set_regions", "fn_map_destroy", "fn_robot_create", "fn_robot_set_sensor", "fn_robot_set_acc_limits",
     "fn_robot_destroy", "fn_task_default", "fn_sim_create", "fn_sim_destroy", "fn_sim_set_stream", "fn_step", "fn_reset",
     "fn_sim_bind_aux", "fn_sim_bind_features", "fn_ring_attach", "fn_ring_sample", "fn_observe_all", "fn_get_counters", "fn_sim_count_words",
     "fn_sim_episode_state", "fn_sim_beam_config", "fn_sim_profile", "fn_sim_profile_read", "fn_step_host", "fn_measure_peak", "fn_last_error", "fn_version")
@@ -52,6 +52,7 @@ def load_library():
         "fn_map_destroy": [vp],
         "fn_robot_create": [vp, i32, vp, i32, f32, i32, vp, C.POINTER(vp)],
         "fn_robot_set_sensor": [vp, f32, f32, f32],
+        "fn_robot_set_acc_limits": [vp, vp],
         "fn_robot_destroy": [vp],
         "fn_sim_create": [vp, vp, i32, C.POINTER(_Task), vp, C.POINTER(vp)],
         "fn_sim_destroy": [vp],
@@ -156,6 +157,10 @@ class Robot:
 
     def set_sensor(self, sx, sy, spsi):
         _check(load_library().fn_robot_set_sensor(self._h, C.c_float(sx), C.c_float(sy), C.c_float(spsi)), "fn_robot_set_sensor")
+
+    def set_acc_limits(self, acc):
+        a = np.ascontiguousarray(acc, np.float32).reshape(3)
+        _check(load_library().fn_robot_set_acc_limits(self._h, _np_ptr(a)), "fn_robot_set_acc_limits")
 
     def close(self):
         if getattr(self, "_h", None):

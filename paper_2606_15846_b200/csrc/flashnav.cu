@@ -48,6 +48,7 @@ struct fn_map {
 struct fn_robot {
     int V, B, drive;
     float lim[6];
+    float acc[3];
     float rmax;
     float sensor[3];
     std::vector<float> angles;
@@ -256,6 +257,7 @@ extern "C" int fn_robot_create(const float* fp, int V, const float* angles, int 
     r->V = V; r->B = B; r->drive = drive; r->rmax = rmax;
     std::memcpy(r->lim, lim, sizeof(r->lim));
     r->sensor[0] = r->sensor[1] = r->sensor[2] = 0.0f;
+    r->acc[0] = r->acc[1] = r->acc[2] = INFINITY;
     r->angles.assign(angles, angles + B);
     r->verts.assign(fp, fp + 2 * V);
     r->d_beam_cs = nullptr; r->d_verts = nullptr; r->d_samples = nullptr; r->n_samples = 0;
@@ -280,6 +282,14 @@ extern "C" int fn_robot_set_sensor(fn_robot* r, float sx, float sy, float spsi) 
     return robot_upload(r);
 }
 
+extern "C" int fn_robot_set_acc_limits(fn_robot* r, const float* acc) {
+    if (!r || !acc) return fail(FN_ERR_INVALID_ARG, "fn_robot_set_acc_limits: NULL argument");
+    for (int k = 0; k < 3; ++k)
+        if (!(acc[k] > 0.0f)) return fail(FN_ERR_INVALID_ARG, "fn_robot_set_acc_limits: limits must be > 0 (+inf = none)");
+    for (int k = 0; k < 3; ++k) r->acc[k] = acc[k];
+    return FN_OK;
+}
+
 extern "C" int fn_robot_destroy(fn_robot* r) {
     if (!r) return FN_OK;
     if (r->d_beam_cs) cudaFree(r->d_beam_cs);
@@ -294,6 +304,7 @@ static RobotDev robot_dev(const fn_robot* r, const fn_map* m) {
     d.beam_cs = r->d_beam_cs; d.verts = r->d_verts; d.samples = r->d_samples; d.n_samples = r->n_samples; d.B = r->B; d.V = r->V; d.drive = r->drive;
     d.A = r->drive == FN_DRIVE_DIFF ? 2 : 3;
     for (int k = 0; k < 6; ++k) d.lim[k] = r->lim[k];
+    for (int k = 0; k < 3; ++k) d.acc[k] = r->acc[k];
     d.rmax = r->rmax;
     d.T = (double)r->rmax / (double)m->res;
     d.sx = r->sensor[0]; d.sy = r->sensor[1];

@@ -60,6 +60,7 @@ struct RobotDev {
     int drive;               // 0 diff, 1 omni
     int A;                   // action dim
     float lim[6];
+    float acc[3];            // maximum accelerations a_x, a_y, a_w (+inf = none; reading G2)
     float rmax;              // metres
     double T;                // rmax / rho in cells
     double sx, sy;           // sensor offset, metres

@@ -287,6 +287,19 @@ __global__ void __launch_bounds__(kEnvBlock) env_step_kernel(EnvArgs a) {
     avx = fminf(fmaxf(avx, a.robot.lim[0]), a.robot.lim[1]);
     if (a.robot.drive != 0) avy = fminf(fmaxf(avy, a.robot.lim[2]), a.robot.lim[3]);
     aw = fminf(fmaxf(aw, a.robot.lim[4]), a.robot.lim[5]);
+    // acceleration limits (reading G2): previous applied velocity +- a_max dt, single fused fp32 operations
+    if (a.robot.acc[0] < INFINITY) {
+        const float vp = a.states[3 * n + el];
+        avx = fminf(fmaxf(avx, __fmaf_rn(-a.robot.acc[0], a.dt, vp)), __fmaf_rn(a.robot.acc[0], a.dt, vp));
+    }
+    if (a.robot.drive != 0 && a.robot.acc[1] < INFINITY) {
+        const float vp = a.states[4 * n + el];
+        avy = fminf(fmaxf(avy, __fmaf_rn(-a.robot.acc[1], a.dt, vp)), __fmaf_rn(a.robot.acc[1], a.dt, vp));
+    }
+    if (a.robot.acc[2] < INFINITY) {
+        const float vp = a.states[5 * n + el];
+        aw = fminf(fmaxf(aw, __fmaf_rn(-a.robot.acc[2], a.dt, vp)), __fmaf_rn(a.robot.acc[2], a.dt, vp));
+    }
     const double dt = (double)a.dt, vx = avx, vy = avy, w = aw;
     const double th = w * dt;
     // one sincos (of theta / 2) gives the integrator's A = sin(theta)/theta, C = sin^2(theta/2)/(theta/2)

@@ -25,6 +25,8 @@ def make_sim(wl, n=None):
     if wl.regions is not None:
         m.set_regions(wl.regions)
     r = fn.Robot(wl.footprint, wl.beam_angles, float(wl.max_range), wl.drive, wl.vel_limits)
+    if getattr(wl, "acc_limits", None) is not None:
+        r.set_acc_limits(wl.acc_limits)
     s = fn.Sim(m, r, n, goal_tol=float(wl.goal_tol), max_episode_steps=wl.max_episode_steps,
                goal_dist_min=float(wl.goal_dist_min), goal_dist_max=float(wl.goal_dist_max),
                r_success=float(wl.r_success), r_collision=float(wl.r_collision), c_progress=float(wl.c_progress))
@@ -148,7 +150,10 @@ def run_parity(wl, steps, n=None, subset=None, seed=0, forced=None, check_every=
         n_done += int(done.sum())
         if check:
             post = buf.states.cpu().numpy()
-            ref = oracle.motion(wl.drive, wl.vel_limits, wl.dt, pre, actions[t].cpu().numpy())
+            ref = oracle.motion(wl.drive, wl.vel_limits, wl.dt, pre, actions[t].cpu().numpy(),
+                                acc=getattr(wl, "acc_limits", None))
+            if getattr(wl, "acc_limits", None) is not None:      # the slewed command is fp32 arithmetic: bit-exact
+                assert np.array_equal(post[3:6], ref[3:6]), f"step {t}: applied velocities under acceleration limits"
             for p in (0, 1, 3, 4, 5, 6, 7):
                 assert np.all(close_state(post[p], ref[p])), f"step {t}: state plane {p} off by {np.abs(post[p] - ref[p]).max()}"
             assert np.all(ang_diff(post[2], ref[2]) <= TOL_STATE * np.maximum(1, np.abs(ref[2]))), f"step {t}: psi"

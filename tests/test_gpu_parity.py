@@ -374,3 +374,13 @@ def test_replay_sampling_against_the_oracle(pu):
                 assert np.array_equal(nxt.cpu().numpy(), en)
     assert steps * n > cap                                                 # the ring has wrapped
     s.close(); r.close(); m.close()
+
+
+def test_acceleration_limits(pu):
+    # NEXT-3 (reading G2): command limited to the previous applied velocity +- a_max dt.
+    from harness import workloads as W
+    for cfg, acc in ((2, (1.0, np.inf, 3.0)), (3, (2.0, 1.5, 4.0))):
+        wl = W.make_workload(cfg, n_envs=512)
+        wl.acc_limits = np.array(acc, np.float32)
+        rep = pu.run_parity(wl, steps=12, subset=64, check_every=1)
+        print(cfg, rep)

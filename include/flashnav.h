@@ -159,6 +159,14 @@ int fn_sim_episode_state(fn_sim* sim, float* d_prev_host, int32_t* ep_step_host)
 int fn_sim_profile(fn_sim* sim, int enable);
 int fn_sim_profile_read(fn_sim* sim, double* ms_out, uint64_t* launches_out);
 
+/* ---- comparison only (not on the product path): the PAPER'S range query, "fixed-step samples along
+ * each beam ... queried in distance blocks, and beams with a detected obstacle are removed from subsequent
+ * blocks" (blockwise != 0), or its ablation baseline that evaluates all samples (blockwise == 0).
+ * Sample k lies at k * delta_m from the sensor origin; range = distance of the first sample in an occupied
+ * (or outside) cell, none below the max range => max range.  Writes out_ranges_dev [N][B] from states_dev;
+ * both variants give the same ranges.  Overwrites the sim's sensing poses (like fn_observe_all). */
+int fn_ranges_fixed_step(fn_sim* sim, const float* states_dev, float delta_m, int blockwise, float* out_ranges_dev);
+
 /* ---- launch configuration of the beam kernel chosen at fn_sim_create (for reports): cfg_out[4] =
  * {map staged in shared memory (1) or read through L1/L2 (0), grid size, CTA size, dynamic shared bytes}. */
 int fn_sim_beam_config(const fn_sim* sim, int* cfg_out);

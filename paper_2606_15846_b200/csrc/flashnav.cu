@@ -15,6 +15,7 @@
 #include "fn_common.cuh"
 #include "fn_env.cuh"
 #include "fn_features.cuh"
+#include "fn_fixed_step.cuh"
 
 using namespace fn;
 
@@ -555,6 +556,25 @@ extern "C" int fn_observe_all(fn_sim* s, const float* states, float* out_ranges,
     s->ring = ring;
     if (st == FN_OK) st = launch_features(s, nullptr, nullptr, false, out_ranges);
     return st;
+}
+
+extern "C" int fn_ranges_fixed_step(fn_sim* s, const float* states, float delta_m, int blockwise, float* out_ranges) {
+    if (!s || !states || !out_ranges) return fail(FN_ERR_INVALID_ARG, "fn_ranges_fixed_step: NULL argument");
+    if (!(delta_m > 0.0f) || !std::isfinite(delta_m)) return fail(FN_ERR_INVALID_ARG, "fn_ranges_fixed_step: delta must be > 0");
+    PoseArgs a;
+    a.map = s->map->dev; a.robot = robot_dev(s->robot, s->map); a.n = s->n; a.states = states;
+    a.out_goal_obs = nullptr; a.poses = s->d_poses; a.beam_task_counter = s->d_task_counter;
+    pose_from_state_kernel<<<(s->n + 255) / 256, 256, 0, s->stream>>>(a);
+    FN_CUDA(cudaGetLastError());
+    FixedStepArgs f;
+    f.map = s->map->dev; f.poses = s->d_poses; f.beam_cs = s->robot->d_beam_cs; f.n = s->n; f.B = s->robot->B;
+    f.delta_cells = delta_m / s->map->res; f.n_samples = (int)std::ceil((double)s->robot->rmax / (double)delta_m);
+    f.rmax = s->robot->rmax; f.rho = s->map->res; f.out_ranges = out_ranges;
+    const unsigned total = (unsigned)s->n * (unsigned)s->robot->B;
+    if (blockwise) fixed_step_kernel<true><<<(total + 255) / 256, 256, 0, s->stream>>>(f);
+    else fixed_step_kernel<false><<<(total + 255) / 256, 256, 0, s->stream>>>(f);
+    FN_CUDA(cudaGetLastError());
+    return FN_OK;
 }
 
 extern "C" int fn_sim_bind_aux(fn_sim* s, int32_t* hit, float* reward) {

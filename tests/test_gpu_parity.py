@@ -384,3 +384,36 @@ def test_acceleration_limits(pu):
         wl.acc_limits = np.array(acc, np.float32)
         rep = pu.run_parity(wl, steps=12, subset=64, check_every=1)
         print(cfg, rep)
+
+
+def test_paper_fixed_step_query_as_comparison(pu):
+    # NEXT-4: the paper's own range query as a comparison kernel.  "Blockwise" and "All samples"
+    # give the same ranges ("All variants used the same ... ray resolution"); a fixed-step march
+    # can only hit at or after the exact first hit and, away from corner grazes, within one step of it; and
+    # it agrees with the oracle's fp64 march (fno_ranges_fixed_step) except where fp32 sample positions
+    # fall on the other side of a cell boundary.
+    import torch
+    import oracle
+    from harness import workloads as W
+    wl = W.make_workload(2, n_envs=256)
+    n, B, A = wl.n_envs, wl.n_beams, wl.action_dim
+    m, r, s = pu.make_sim(wl, n)
+    buf = pu.Buffers(n, B, A)
+    seeds = torch.from_numpy(W.seed_tape(wl, 1, 9).view(np.int64)).cuda()
+    buf.mask.fill_(1)
+    s.reset(buf.states, buf.mask, seeds[0], buf.ranges, buf.gobs)
+    delta = 0.025                                                 # half a cell
+    rb = torch.empty_like(buf.ranges)
+    ra = torch.empty_like(buf.ranges)
+    s.ranges_fixed_step(buf.states, delta, True, rb)
+    s.ranges_fixed_step(buf.states, delta, False, ra)
+    torch.cuda.synchronize()
+    assert torch.equal(rb, ra)
+    exact = buf.ranges.cpu().numpy()
+    fixed = rb.cpu().numpy()
+    assert np.all(fixed >= exact - 1e-3)
+    assert np.mean(fixed <= exact + delta + 1e-3) > 0.97          # the rest cut a corner shorter than one step
+    st = buf.states.cpu().numpy()
+    ref = oracle.ranges_fixed_step(wl.occ, wl.resolution, wl.beam_angles, wl.max_range, delta, st[0], st[1], st[2])
+    assert np.mean(np.abs(fixed - ref) <= 1e-5) > 0.98 and np.mean(np.abs(fixed - ref) <= delta + 1e-5) > 0.995
+    s.close(); r.close(); m.close()

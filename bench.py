@@ -313,6 +313,35 @@ def run_ours(args):
                 "beams_per_s": n * B / f_s, "read_GBps": n * B * 4 / f_s / 1e9,
                 "note": "fn::features_kernel over all envs after the beam kernel (ranges read from L2); not in the timed step"}
 
+    # the paper's own fixed-step range query on the same poses (Table III-b):
+    # comparison only, information
+    paper_query = None
+    if args.paper_query:
+        delta = float(wl.resolution) * 0.5
+        rq = torch.empty_like(ranges)
+        ex = torch.empty_like(ranges)
+        res = {}
+        for name, fnq in (("blockwise", lambda: sim.ranges_fixed_step(states, delta, True, rq)),
+                          ("all_samples", lambda: sim.ranges_fixed_step(states, delta, False, rq)),
+                          ("exact_traversal", lambda: sim.observe_all(states, ex))):
+            fnq()
+            barrier()
+            tot = 0.0
+            q0, q1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            for k in range(5):
+                flush.fill_(k & 0xff)
+                q0.record()
+                fnq()
+                q1.record()
+                torch.cuda.synchronize()
+                tot += q0.elapsed_time(q1)
+            res[name] = tot / 5
+        err = (rq - ex)
+        paper_query = {"delta_m": delta, "ms": res, "speedup_exact_vs_blockwise": res["blockwise"] / res["exact_traversal"],
+                       "range_error_m": {"mean": float(err.mean()), "max": float(err.max()), "min": float(err.min())},
+                       "note": "fn_ranges_fixed_step (the paper's query, fp32 samples every delta) vs fn_observe_all (pose kernel + "
+                               "exact traversal) on the same states; all three include the pose kernel"}
+
     # replay sampling: U x B transitions gathered from the ring (HBM-bound)
     sample = None
     if ring is not None and args.sample_batch > 0:
@@ -422,7 +451,7 @@ def run_ours(args):
                                       "compact": prof["compact"][0] / K, "reset": prof["reset"][0] / K,
                                       "beam_reset": prof["beam_reset"][0] / K},
                "ms_per_step_p50": float(np.median(per_step_ms)), "ms_per_step_p90": float(np.percentile(per_step_ms, 90)),
-               "features": feat, "replay_sample": sample, "roofline": roofline, "cpu_baseline": cpu, "clocks": clocks, "gpu_launches": 5 * K}
+               "features": feat, "replay_sample": sample, "paper_fixed_step_query": paper_query, "roofline": roofline, "cpu_baseline": cpu, "clocks": clocks, "gpu_launches": 5 * K}
 
     # ---- end to end through the public API with HOST buffers (copies inside the timed region)
     hs = torch.empty(8, n, dtype=torch.float32).pin_memory()
@@ -471,6 +500,7 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=50)
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--sample-batch", type=int, default=65536, help="U x B of the replay-sampling leg (configs with a ring; 0 = skip)")
+    ap.add_argument("--paper-query", type=int, default=1, help="also time the paper's fixed-step range query (information only)")
     ap.add_argument("--features", type=int, default=36, help="sectors of the clearance-feature leg (0 = skip; information only)")
     ap.add_argument("--graph", type=int, default=1, help="also time a CUDA-graph replay of the steps (information only)")
     ap.add_argument("--ring", type=int, default=1, help="attach the replay ring when the config has one (C5)")

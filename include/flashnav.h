@@ -36,7 +36,8 @@ enum { FN_OK = 0, FN_ERR_INVALID_ARG = -1, FN_ERR_UNSUPPORTED = -2, FN_ERR_OOM =
 enum { FN_DRIVE_DIFF = 0, FN_DRIVE_OMNI = 1 };
 enum { FN_MAX_VERTS = 64, FN_MAX_ATTEMPTS = 256 };
 enum { FN_N_COUNTERS = 8 };   /* rays cast, map words loaded, envs reset, reset failures,
-                                 non-finite actions, env steps, reserved, reserved */
+                                 non-finite actions, env steps, map windows outside the packed map seen by
+                                 the instrumented beam kernel (a self-check: must stay 0), reserved */
 
 typedef struct fn_map fn_map;
 typedef struct fn_robot fn_robot;

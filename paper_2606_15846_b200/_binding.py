@@ -13,7 +13,7 @@ _lib = None
 DRIVE_DIFF, DRIVE_OMNI = 0, 1
 N_COUNTERS = 8
 COUNTER_NAMES = ("rays_cast", "map_words_loaded", "envs_reset", "reset_failures", "nonfinite_actions",
-                 "env_steps", "reserved0", "reserved1")
+                 "env_steps", "oob_window_loads", "reserved1")
 
 EXPORTED_SYMBOLS = (
     "fn_map_create", "fn_map_set_regions", "fn_map_destroy", "fn_robot_create", "fn_robot_set_sensor", "fn_robot_set_acc_limits",

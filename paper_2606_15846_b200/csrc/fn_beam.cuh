@@ -67,6 +67,8 @@ struct BeamMap {
     typename MS::addr_t base;        // start of the row copy (true address)
     int H, W, stride4R, stride4C;    // line strides in bytes
     unsigned rowBytes;               // size of the row copy = offset of the column copy
+    unsigned mapBytes;               // both copies (instrumented kernels check every window against it)
+    unsigned long long* oob;         // counter of windows outside [base, base + mapBytes) or NULL
 };
 // line index (row of the row copy / column of the column copy) of the origin's line
 template <class MS>
@@ -259,6 +261,10 @@ __device__ __forceinline__ float cast_beam(const BeamMap<MS>& bm, const BeamPose
             for (;;) {                                            // one window per line
                 const uint32_t th = hiw(D);
                 const typename MS::addr_t a = MS::addb(wb, (int)((th >> 5) << 2));
+                if (kAux && bm.oob) {                            // self-check: the frame / pad / guard reasoning
+                    const long long off = MS::diffb(a, bm.base);
+                    if (off < 0 || off + 8 > (long long)bm.mapBytes) { atomicAdd(bm.oob, 1ull); x = 0u; break; }
+                }
                 x = __funnelshift_r(MS::ld(a), MS::ld4(a), th) & mask;
                 if (kAux) words += 2;
                 if (x != 0u || wb == wend) break;
@@ -529,14 +535,14 @@ __global__ void __launch_bounds__(512, 2) beam_kernel(BeamArgs a) {
         BeamMap<SmemSpace> bm;
         bm.base = (uint32_t)__cvta_generic_to_shared(s_map);
         bm.H = a.map.H; bm.W = a.map.W; bm.stride4R = a.map.strideR << 2; bm.stride4C = a.map.strideC << 2;
-        bm.rowBytes = rowBytes;
+        bm.rowBytes = rowBytes; bm.mapBytes = (unsigned)mapWords * 4u; bm.oob = a.counters + kOobLoads;
         geo.baseR = bm.base - kExpOff; geo.baseC = geo.baseR + rowBytes;
         run_beam_tasks<SmemSpace, !kAux, kAux>(a, bm, geo, s_tab, n_env, total);
     } else {
         BeamMap<GlobalSpace> bm;
         bm.base = (unsigned long long)__cvta_generic_to_global(a.map.row);
         bm.H = a.map.H; bm.W = a.map.W; bm.stride4R = a.map.strideR << 2; bm.stride4C = a.map.strideC << 2;
-        bm.rowBytes = rowBytes;
+        bm.rowBytes = rowBytes; bm.mapBytes = (unsigned)mapWords * 4u; bm.oob = a.counters + kOobLoads;
         run_beam_tasks<GlobalSpace, false, kAux>(a, bm, geo, s_tab, n_env, total);
     }
 }

@@ -210,6 +210,7 @@ def run_parity(wl, steps, n=None, subset=None, seed=0, forced=None, check_every=
     rep.add("done_events", n_done)
     cnt = s.counters()
     rep.add("rays_cast", cnt["rays_cast"])
+    assert cnt["oob_window_loads"] == 0, "the instrumented beam kernel read a window outside the packed map"
     assert cnt["reset_failures"] == rep.c.get("reset_failures", 0) or check_every > 1
     s.close(); r.close(); m.close()
     return rep

@@ -181,6 +181,16 @@ def ring_append(ring, capacity, head, obs_ranges, obs_goal, obs_vel, actions, re
                           _p(done, C.c_uint8))
 
 
+def eval_update(collision, d_new, goal_tol, ep_step_after, step_limit, reward, outcome, steps, ret):
+    """Evaluation completion masks; outcome u8 / steps i32 / ret f32 are updated in place."""
+    collision, d_new, reward = _u8(collision), _f32(d_new), _f32(reward)
+    ep = np.ascontiguousarray(ep_step_after, np.int32)
+    assert outcome.dtype == np.uint8 and steps.dtype == np.int32 and ret.dtype == np.float32
+    lib().fno_eval_update(C.c_int(outcome.shape[0]), _p(collision, C.c_uint8), _p(d_new, C.c_float), C.c_float(goal_tol),
+                          _p(ep, C.c_int32), C.c_int(step_limit), _p(reward, C.c_float), _p(outcome, C.c_uint8),
+                          _p(steps, C.c_int32), _p(ret, C.c_float))
+
+
 def sample_slot(seed: int, i: int, filled: int) -> int:
     f = lib().fno_sample_slot
     f.restype = C.c_uint64

@@ -630,6 +630,27 @@ void fno_ring_sample(const float* ring, uint64_t capacity, uint64_t filled, int 
     }
 }
 
+/* ------------------------------------------------------------------ O12: evaluation bookkeeping (NEXT-3)
+ * "Completion masks record each case once and exclude completed cases from further
+ * accumulation of rewards and outcome statistics.  Each case ends when the robot reaches the goal,
+ * collides with an obstacle, or reaches the evaluation step limit."  outcome: 0 running, 1 success,
+ * 2 collision, 3 step limit, 4 inactive slot; collision has priority over success as in Eq. (1).
+ * Called once per vector step with that step's flags for ALL envs; completed cases are left untouched.
+ */
+void fno_eval_update(int n, const uint8_t* collision, const float* d_new, float goal_tol,
+                     const int32_t* ep_step_after, int step_limit, const float* reward,
+                     uint8_t* outcome, int32_t* steps, float* ret) {
+    for (int e = 0; e < n; ++e) {
+        if (outcome[e] != 0) continue;                           /* recorded once; excluded afterwards */
+        ret[e] += reward[e];
+        int o = 0;
+        if (collision[e]) o = 2;
+        else if (d_new[e] < goal_tol) o = 1;
+        else if (ep_step_after[e] >= step_limit) o = 3;
+        if (o) { outcome[e] = (uint8_t)o; steps[e] = ep_step_after[e]; }
+    }
+}
+
 /* ------------------------------------------------------------------ one whole vector step (3.2)
  * actions -> O1/O2 motion -> O3 collision + O5 goal obs at the new pose -> O6 reward/done ->
  * O4 ranges at the new pose.  Outputs are the PRE-reset (terminal) observations.

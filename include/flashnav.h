@@ -160,6 +160,23 @@ int fn_sim_episode_state(fn_sim* sim, float* d_prev_host, int32_t* ep_step_host)
 int fn_sim_profile(fn_sim* sim, int enable);
 int fn_sim_profile_read(fn_sim* sim, double* ms_out, uint64_t* launches_out);
 
+/* ---- parallel policy evaluation: "Each batch assigns fixed start-goal cases to separate
+ * environments ... Completion masks record each case once and exclude completed cases from further
+ * accumulation of rewards and outcome statistics.  Each case ends when the robot reaches the goal, collides
+ * with an obstacle, or reaches the evaluation step limit."
+ * fn_eval_begin: states_dev [8][N] holds the start poses (planes 0-2) and goals (planes 6, 7) of the first
+ *   n_cases envs (slots >= n_cases are inactive); zeroes the velocities, re-seeds the episode state, clears the
+ *   completion masks, writes the initial observations of all envs and switches the sim to evaluation mode:
+ *   fn_step then freezes every completed case (state and observation rows unchanged, reward 0, done 0 after
+ *   the step that ended it), uses step_limit instead of the task's episode limit and does not need fn_reset.
+ * fn_eval_result (synchronises): HOST arrays [N], any may be NULL: outcome u8 (0 running, 1 success, 2 collision,
+ *   3 step limit, 4 inactive slot), steps i32 (steps taken; final for completed cases), return fp32 (sum of Eq. (1)
+ *   rewards up to completion); *n_running = cases still running (0 = the batch has ended).
+ * fn_eval_end: back to training mode (call fn_reset for all envs before stepping again). */
+int fn_eval_begin(fn_sim* sim, float* states_dev, int n_cases, int step_limit, float* out_ranges_dev, float* out_goal_obs_dev);
+int fn_eval_result(fn_sim* sim, uint8_t* outcome_host, int32_t* steps_host, float* return_host, int* n_running);
+int fn_eval_end(fn_sim* sim);
+
 /* ---- comparison only (not on the product path): the PAPER'S range query, "fixed-step samples along
  * each beam ... queried in distance blocks, and beams with a detected obstacle are removed from subsequent
  * blocks" (blockwise != 0), or its ablation baseline that evaluates all samples (blockwise == 0).

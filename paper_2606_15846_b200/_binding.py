@@ -18,7 +18,7 @@ COUNTER_NAMES = ("rays_cast", "map_words_loaded", "envs_reset", "reset_failures"
 EXPORTED_SYMBOLS = (
     "fn_map_create", "fn_map_set_regions", "fn_map_destroy", "fn_robot_create", "fn_robot_set_sensor", "fn_robot_set_acc_limits",
     "fn_robot_destroy", "fn_task_default", "fn_sim_create", "fn_sim_destroy", "fn_sim_set_stream", "fn_step", "fn_reset",
-    "fn_sim_bind_aux", "fn_sim_bind_features", "fn_ring_attach", "fn_ring_sample", "fn_ranges_fixed_step", "fn_observe_all", "fn_get_counters", "fn_sim_count_words",
+    "fn_sim_bind_aux", "fn_sim_bind_features", "fn_ring_attach", "fn_ring_sample", "fn_ranges_fixed_step", "fn_eval_begin", "fn_eval_result", "fn_eval_end", "fn_observe_all", "fn_get_counters", "fn_sim_count_words",
     "fn_sim_episode_state", "fn_sim_beam_config", "fn_sim_profile", "fn_sim_profile_read", "fn_step_host", "fn_measure_peak", "fn_last_error", "fn_version")
 
 
@@ -64,6 +64,9 @@ def load_library():
         "fn_ring_attach": [vp, vp, u64],
         "fn_ring_sample": [vp, u64, i32, vp, vp],
         "fn_observe_all": [vp, vp, vp, vp],
+        "fn_eval_begin": [vp, vp, i32, i32, vp, vp],
+        "fn_eval_result": [vp, vp, vp, vp, vp],
+        "fn_eval_end": [vp],
         "fn_ranges_fixed_step": [vp, vp, f32, i32, vp],
         "fn_get_counters": [vp, vp],
         "fn_sim_count_words": [vp, i32],
@@ -270,6 +273,25 @@ class Sim:
         _check(load_library().fn_ranges_fixed_step(
             self._h, _dev_ptr(states, torch.float32, 8 * n, "states"), C.c_float(delta_m), int(bool(blockwise)),
             _dev_ptr(out_ranges, torch.float32, n * B, "out_ranges")), "fn_ranges_fixed_step")
+
+    def eval_begin(self, states, n_cases, step_limit, out_ranges, out_goal_obs):
+        """Evaluation mode: fixed start-goal cases in `states`, completion masks, step limit."""
+        import torch
+        n, B = self.n, self.robot.B
+        _check(load_library().fn_eval_begin(
+            self._h, _dev_ptr(states, torch.float32, 8 * n, "states"), int(n_cases), int(step_limit),
+            _dev_ptr(out_ranges, torch.float32, n * B, "out_ranges"),
+            _dev_ptr(out_goal_obs, torch.float32, 2 * n, "out_goal_obs")), "fn_eval_begin")
+
+    def eval_result(self):
+        """(outcome u8 [N], steps i32 [N], return f32 [N], n_running); synchronises."""
+        o = np.empty(self.n, np.uint8); st = np.empty(self.n, np.int32); rt = np.empty(self.n, np.float32)
+        nr = C.c_int()
+        _check(load_library().fn_eval_result(self._h, _np_ptr(o), _np_ptr(st), _np_ptr(rt), C.byref(nr)), "fn_eval_result")
+        return o, st, rt, int(nr.value)
+
+    def eval_end(self):
+        _check(load_library().fn_eval_end(self._h), "fn_eval_end")
 
     def counters(self) -> dict:
         out = np.zeros(N_COUNTERS, np.uint64)

@@ -75,6 +75,9 @@ struct fn_sim {
     int* d_epstep;
     unsigned long long* d_counters;
     unsigned* d_task_counter;        // beam kernel's dynamic task counter
+    uint8_t* d_eval_outcome;         // evaluation mode: completion masks, returns
+    float* d_eval_return;
+    int eval_mode, eval_limit;
     int* d_done_list;                // [2][n] envs reported done by fn_step (one list per step parity), any order
     int* d_done_count;               // [2] counts, [2] = the parity the NEXT fn_step fills (device-side state)
     int done_avail;                  // 1 = the last fn_step's list has not been consumed by fn_reset(mask = NULL)
@@ -353,6 +356,8 @@ extern "C" int fn_sim_create(const fn_map* map, const fn_robot* robot, int n, co
     if (e == cudaSuccess) e = cudaMalloc(&s->d_epstep, (size_t)n * sizeof(int));
     if (e == cudaSuccess) e = cudaMalloc(&s->d_counters, kNCounters * sizeof(unsigned long long));
     if (e == cudaSuccess) e = cudaMalloc(&s->d_task_counter, sizeof(unsigned));
+    if (e == cudaSuccess) e = cudaMalloc(&s->d_eval_outcome, (size_t)n);
+    if (e == cudaSuccess) e = cudaMalloc(&s->d_eval_return, (size_t)n * sizeof(float));
     if (e == cudaSuccess) e = cudaMalloc(&s->d_done_list, 2 * (size_t)n * sizeof(int));
     if (e == cudaSuccess) e = cudaMalloc(&s->d_done_count, 3 * sizeof(int));
     if (e == cudaSuccess) e = cudaMemsetAsync(s->d_done_count, 0, 3 * sizeof(int), s->stream);
@@ -404,7 +409,7 @@ extern "C" int fn_sim_destroy(fn_sim* s) {
     if (!s) return FN_OK;
     cudaFree(s->d_poses); cudaFree(s->d_ring_head); cudaFree(s->d_list); cudaFree(s->d_count); cudaFree(s->d_dprev);
     cudaFree(s->d_epstep); cudaFree(s->d_counters); cudaFree(s->d_task_counter);
-    cudaFree(s->d_done_list); cudaFree(s->d_done_count);
+    cudaFree(s->d_done_list); cudaFree(s->d_done_count); cudaFree(s->d_eval_outcome); cudaFree(s->d_eval_return);
     if (s->ev) { for (cudaEvent_t e : *s->ev) cudaEventDestroy(e); delete s->ev; delete s->ev_kind; }
     cudaFree(s->stg_states); cudaFree(s->stg_actions); cudaFree(s->stg_ranges); cudaFree(s->stg_gobs);
     cudaFree(s->stg_mask); cudaFree(s->stg_col); cudaFree(s->stg_seeds);
@@ -488,6 +493,7 @@ extern "C" int fn_step(fn_sim* s, float* states, const float* actions, float dt,
     a.ring = s->ring; a.ring_cap = s->ring_cap ? s->ring_cap : 1; a.ring_head_dev = s->d_ring_head; a.ring_row = ring_row_floats(s);
     a.counters = s->d_counters; a.beam_task_counter = s->d_task_counter;
     a.done_list = s->d_done_list; a.done_count = s->d_done_count; a.par_dev = s->d_done_count + 2;
+    a.eval_outcome = s->eval_mode ? s->d_eval_outcome : nullptr; a.eval_return = s->d_eval_return; a.eval_limit = s->eval_limit;
     cudaEvent_t e0 = nullptr, e1 = nullptr, e2 = nullptr;
     if (s->prof) {
         FN_CUDA(cudaEventCreate(&e0)); FN_CUDA(cudaEventCreate(&e1)); FN_CUDA(cudaEventCreate(&e2));
@@ -574,6 +580,48 @@ extern "C" int fn_ranges_fixed_step(fn_sim* s, const float* states, float delta_
     if (blockwise) fixed_step_kernel<true><<<(total + 255) / 256, 256, 0, s->stream>>>(f);
     else fixed_step_kernel<false><<<(total + 255) / 256, 256, 0, s->stream>>>(f);
     FN_CUDA(cudaGetLastError());
+    return FN_OK;
+}
+
+// ------------------------------------------------------------------------------------------ evaluation mode
+extern "C" int fn_eval_begin(fn_sim* s, float* states, int n_cases, int step_limit, float* out_ranges, float* out_goal_obs) {
+    if (!s || !states || !out_ranges || !out_goal_obs) return fail(FN_ERR_INVALID_ARG, "fn_eval_begin: NULL argument");
+    if (n_cases < 1 || n_cases > s->n) return fail(FN_ERR_INVALID_ARG, "fn_eval_begin: n_cases must be in 1..n_envs");
+    if (step_limit < 1) return fail(FN_ERR_INVALID_ARG, "fn_eval_begin: the evaluation step limit must be >= 1");
+    EvalBeginArgs a;
+    a.pose.map = s->map->dev; a.pose.robot = robot_dev(s->robot, s->map); a.pose.n = s->n; a.pose.states = states;
+    a.pose.out_goal_obs = out_goal_obs; a.pose.poses = s->d_poses; a.pose.beam_task_counter = s->d_task_counter;
+    a.states = states; a.d_prev = s->d_dprev; a.ep_step = s->d_epstep; a.outcome = s->d_eval_outcome; a.ret = s->d_eval_return;
+    a.n_cases = n_cases;
+    eval_begin_kernel<<<(s->n + 255) / 256, 256, 0, s->stream>>>(a);
+    FN_CUDA(cudaGetLastError());
+    s->eval_mode = 1; s->eval_limit = step_limit; s->done_avail = 0;
+    float* ring = s->ring;           // evaluation never touches the replay ring
+    s->ring = nullptr;
+    int st = launch_beams(s, nullptr, nullptr, out_ranges);
+    s->ring = ring;
+    if (st == FN_OK) st = launch_features(s, nullptr, nullptr, false, out_ranges);
+    return st;
+}
+
+extern "C" int fn_eval_result(fn_sim* s, uint8_t* outcome, int32_t* steps, float* ret, int* n_running) {
+    if (!s) return fail(FN_ERR_INVALID_ARG, "fn_eval_result: NULL sim");
+    if (!s->eval_mode) return fail(FN_ERR_INVALID_ARG, "fn_eval_result: not in evaluation mode (fn_eval_begin)");
+    std::vector<uint8_t> tmp((size_t)s->n);
+    FN_CUDA(cudaMemcpyAsync(tmp.data(), s->d_eval_outcome, (size_t)s->n, cudaMemcpyDeviceToHost, s->stream));
+    if (steps) FN_CUDA(cudaMemcpyAsync(steps, s->d_epstep, (size_t)s->n * sizeof(int), cudaMemcpyDeviceToHost, s->stream));
+    if (ret) FN_CUDA(cudaMemcpyAsync(ret, s->d_eval_return, (size_t)s->n * sizeof(float), cudaMemcpyDeviceToHost, s->stream));
+    FN_CUDA(cudaStreamSynchronize(s->stream));
+    int running = 0;
+    for (int e = 0; e < s->n; ++e) running += tmp[e] == 0;
+    if (outcome) std::memcpy(outcome, tmp.data(), (size_t)s->n);
+    if (n_running) *n_running = running;
+    return FN_OK;
+}
+
+extern "C" int fn_eval_end(fn_sim* s) {
+    if (!s) return fail(FN_ERR_INVALID_ARG, "fn_eval_end: NULL sim");
+    s->eval_mode = 0;
     return FN_OK;
 }
 

@@ -251,6 +251,9 @@ struct EnvArgs {
     int* done_count;             // [2]    fn_reset(mask = NULL) uses the step's list.  The parity lives on
     const int* par_dev;          // the device (flipped by the step's beam kernel, which also clears the other
                                  // count), so a captured sequence of steps replays for any length
+    uint8_t* eval_outcome;       // evaluation mode or NULL: 0 running, 1 success, 2 collision,
+    float* eval_return;          //   3 step limit, 4 inactive slot; completed cases are frozen
+    int eval_limit;
     unsigned long long* counters;
 };
 
@@ -270,8 +273,11 @@ __global__ void __launch_bounds__(kEnvBlock) env_step_kernel(EnvArgs a) {
     if (blockIdx.x == 0 && threadIdx.x == 0) *a.beam_task_counter = 0u;
     const int e = blockIdx.x * a.epw + threadIdx.x;
     const int n = a.n;
-    const bool live = (int)threadIdx.x < a.epw && e < n;
-    const int el = live ? e : n - 1;                               // idle lanes shadow the last env, write nothing
+    const bool in_range = (int)threadIdx.x < a.epw && e < n;
+    const int el = in_range ? e : n - 1;                           // idle lanes shadow the last env, write nothing
+    // evaluation mode: "completion masks ... exclude completed cases": a completed case is frozen
+    const bool frozen = in_range && a.eval_outcome != nullptr && a.eval_outcome[el] != 0;
+    const bool live = in_range && !frozen;
     // ---- S1: clip ("within the configured bounds") and exact constant-twist step
     const double x = a.states[0 * n + el], y = a.states[1 * n + el], psi = a.states[2 * n + el];
     const float gxf = a.states[6 * n + el], gyf = a.states[7 * n + el];
@@ -346,7 +352,8 @@ __global__ void __launch_bounds__(kEnvBlock) env_step_kernel(EnvArgs a) {
     const float r = col ? a.task.r_collision
                         : reached ? a.task.r_success
                                   : (float)((double)a.task.c_progress * ((double)dp - (double)d));
-    const bool limit = a.task.max_episode_steps > 0 && es + 1 >= a.task.max_episode_steps;
+    const int step_limit = a.eval_outcome ? a.eval_limit : a.task.max_episode_steps;
+    const bool limit = step_limit > 0 && es + 1 >= step_limit;
     const uint8_t done = (live && (col || reached || limit || forced)) ? 1 : 0;
     // the done envs, appended to the step's list (one atomic per warp): "Ended only" needs no mask scan
     const unsigned dm = __ballot_sync(0xffffffffu, done != 0);
@@ -357,7 +364,15 @@ __global__ void __launch_bounds__(kEnvBlock) env_step_kernel(EnvArgs a) {
         base = __shfl_sync(0xffffffffu, base, 0);
         if (done) a.done_list[(size_t)par * n + base + __popc(dm & ((1u << threadIdx.x) - 1u))] = e;
     }
+    if (frozen) {                                                  // no state change, no reward, not done again
+        a.reset_mask[e] = 0;
+        if (a.out_reward) a.out_reward[e] = 0.0f;
+    }
     if (!live) return;
+    if (a.eval_outcome) {                                          // each case is recorded once
+        a.eval_return[e] += r;
+        if (done) a.eval_outcome[e] = col ? 2 : reached ? 1 : 3;
+    }
     a.states[0 * n + e] = xf; a.states[1 * n + e] = yf; a.states[2 * n + e] = psif;
     a.states[3 * n + e] = avx; a.states[4 * n + e] = avy; a.states[5 * n + e] = aw;
     a.out_collision[e] = col ? 1 : 0;
@@ -627,6 +642,41 @@ __global__ void __launch_bounds__(256) pose_from_state_kernel(PoseArgs a) {
         a.out_goal_obs[e] = (float)sqrt(gdx * gdx + gdy * gdy);
         a.out_goal_obs[n + e] = (float)wrap_pi(atan2(gdy, gdx) - (double)psi);
     }
+}
+
+// ---------------------------------------------------------------- evaluation mode: fixed start-goal cases
+// PAPER.md:88 "Each batch assigns fixed start-goal cases to separate environments".  states holds the start
+// poses (planes 0-2) and goals (planes 6, 7) of the first n_cases envs; velocities are zeroed, the episode
+// state re-seeded, the completion masks cleared (slots >= n_cases are inactive) and the sensing poses set.
+struct EvalBeginArgs {
+    PoseArgs pose;
+    float* states;
+    float* d_prev;
+    int* ep_step;
+    uint8_t* outcome;
+    float* ret;
+    int n_cases;
+};
+__global__ void __launch_bounds__(256) eval_begin_kernel(EvalBeginArgs a) {
+    const int e = blockIdx.x * blockDim.x + threadIdx.x;
+    if (e == 0) *a.pose.beam_task_counter = 0u;
+    const int n = a.pose.n;
+    if (e >= n) return;
+    const float x = a.states[e], y = a.states[n + e], psi = a.states[2 * n + e];
+    a.states[3 * n + e] = 0.f; a.states[4 * n + e] = 0.f; a.states[5 * n + e] = 0.f;
+    double s, c;
+    sincos((double)psi, &s, &c);
+    write_pose(a.pose.map, a.pose.robot, &a.pose.poses[e], x, y, psi, c, s);
+    const double gdx = (double)a.states[6 * n + e] - (double)x, gdy = (double)a.states[7 * n + e] - (double)y;
+    const float d = (float)sqrt(gdx * gdx + gdy * gdy);
+    if (a.pose.out_goal_obs) {
+        a.pose.out_goal_obs[e] = d;
+        a.pose.out_goal_obs[n + e] = (float)wrap_pi(atan2(gdy, gdx) - (double)psi);
+    }
+    a.d_prev[e] = d;
+    a.ep_step[e] = 0;
+    a.outcome[e] = e < a.n_cases ? 0 : 4;
+    a.ret[e] = 0.f;
 }
 
 }  // namespace fn

@@ -417,3 +417,68 @@ def test_paper_fixed_step_query_as_comparison(pu):
     ref = oracle.ranges_fixed_step(wl.occ, wl.resolution, wl.beam_angles, wl.max_range, delta, st[0], st[1], st[2])
     assert np.mean(np.abs(fixed - ref) <= 1e-5) > 0.98 and np.mean(np.abs(fixed - ref) <= delta + 1e-5) > 0.995
     s.close(); r.close(); m.close()
+
+
+def test_evaluation_mode_completion_masks(pu):
+    # NEXT-3: fixed start-goal cases, completion masks that record each case once and freeze it,
+    # evaluation step limit.  The bookkeeping is checked against the oracle's fno_eval_update, fed per step
+    # with flags recomputed by the oracle at the GPU's poses (teacher forcing, near-ties excluded).
+    import torch
+    import oracle
+    from harness import workloads as W
+    wl = W.make_workload(2, n_envs=384)
+    n, B, A = wl.n_envs, wl.n_beams, wl.action_dim
+    n_cases, limit = 300, 25
+    m, r, s = pu.make_sim(wl, n)
+    buf = pu.Buffers(n, B, A)
+    s.bind_aux(None, buf.reward)
+    # cases: collision-free starts and goals from the (pinned) reset rule, then fixed
+    seeds = torch.from_numpy(W.seed_tape(wl, 1, 21).view(np.int64)).cuda()
+    buf.mask.fill_(1)
+    s.reset(buf.states, buf.mask, seeds[0], buf.ranges, buf.gobs)
+    buf.states[3:6] = 0.37                                        # eval_begin must zero the velocities
+    s.eval_begin(buf.states, n_cases, limit, buf.ranges, buf.gobs)
+    torch.cuda.synchronize()
+    st0 = buf.states.cpu().numpy()
+    assert np.all(st0[3:6] == 0)
+    o, steps, ret, running = s.eval_result()
+    assert running == n_cases and np.all(o[:n_cases] == 0) and np.all(o[n_cases:] == 4) and np.all(steps == 0)
+    og = oracle.goal_obs(st0[0], st0[1], st0[2], st0[6], st0[7])
+    assert np.allclose(buf.gobs.cpu().numpy()[0], og[0], atol=1e-5)
+    actions = torch.from_numpy(W.action_tape(wl, limit + 3, 8)).cuda()
+    e_out = o.copy(); e_steps = np.zeros(n, np.int32); e_ret = np.zeros(n, np.float32)
+    amb_any = np.zeros(n, bool)
+    for t in range(limit + 3):
+        pre = buf.states.cpu().numpy()
+        pre_r = buf.ranges.clone()
+        o_before = s.eval_result()[0]
+        buf.mask.zero_()
+        s.step(buf.states, actions[t], float(wl.dt), buf.mask, buf.ranges, buf.col, buf.gobs)
+        torch.cuda.synchronize()
+        post = buf.states.cpu().numpy()
+        done = buf.mask.cpu().numpy()
+        rew = buf.reward.cpu().numpy()
+        frozen = o_before != 0
+        # completed cases (and inactive slots) are frozen: nothing moves, no reward, not done again
+        assert np.array_equal(post[:, frozen], pre[:, frozen]) and np.all(done[frozen] == 0) and np.all(rew[frozen] == 0)
+        assert torch.equal(buf.ranges[torch.from_numpy(frozen).cuda()], pre_r[torch.from_numpy(frozen).cuda()])
+        # oracle flags at the GPU's poses for the running cases
+        flag, camb = oracle.collision(wl.occ, wl.resolution, wl.footprint, post[0], post[1], post[2])
+        amb_any |= (camb != 0) & ~frozen
+        gcol = buf.col.cpu().numpy()
+        okc = (camb == 0) & ~frozen
+        assert np.array_equal(gcol[okc], flag[okc])
+        d_new = buf.gobs.cpu().numpy()[0]
+        _, ep_after = s.episode_state()
+        oracle.eval_update(gcol, d_new, float(wl.goal_tol), ep_after, limit, rew, e_out, e_steps, e_ret)
+        o_now, steps_now, ret_now, running = s.eval_result()
+        assert np.array_equal(o_now, e_out) and np.array_equal(steps_now[e_out != 0], e_steps[e_out != 0])
+        assert np.allclose(ret_now, e_ret, atol=1e-4)
+        assert np.array_equal(done != 0, (o_now != 0) & (o_before == 0))      # done exactly on the completing step
+        if running == 0:
+            break
+    assert running == 0 and t + 1 <= limit                       # the batch ends at the step limit at the latest
+    assert set(np.unique(e_out[:n_cases])) <= {1, 2, 3} and (e_out[:n_cases] == 3).any() and (e_out[:n_cases] == 2).any()
+    assert amb_any.sum() <= 2
+    s.eval_end()
+    s.close(); r.close(); m.close()

@@ -191,6 +191,17 @@ def eval_update(collision, d_new, goal_tol, ep_step_after, step_limit, reward, o
                           _p(steps, C.c_int32), _p(ret, C.c_float))
 
 
+def set_footprint_components(sizes=None):
+    """Footprint = union of polygons: sizes of the components whose vertex lists are
+    concatenated in `footprint`; None = a single polygon.  Applies to collision, reset, footprint_distance,
+    clearance_features and step until changed."""
+    if sizes is None or len(sizes) <= 1:
+        lib().fno_set_footprint_components(C.c_int(0), None)
+    else:
+        a = np.ascontiguousarray(sizes, np.int32)
+        lib().fno_set_footprint_components(C.c_int(len(a)), _p(a, C.c_int32))
+
+
 def sample_slot(seed: int, i: int, filled: int) -> int:
     f = lib().fno_sample_slot
     f.restype = C.c_uint64

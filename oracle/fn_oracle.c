@@ -235,12 +235,44 @@ static int collision_one(const uint8_t* occ, int H, int W, double rho, int V, co
     return flag;
 }
 
+/* Footprints that are a UNION of polygons ("polygon(s)", :129 "For a union of polygons, the
+ * minimum distance over its components is used").  The vertex list is the components'
+ * vertex lists one after the other; fno_set_footprint_components gives their sizes (C = 0 or 1: one
+ * polygon).  The union collides iff some component does; it robustly collides iff some component robustly
+ * does, and is near a collision iff some component is -- hence the ambiguity rule below.  The oracle is
+ * single-threaded test infrastructure, so this setting is simply file-scope state.
+ */
+static int g_ncomp = 0;
+static int g_comp[FNO_MAX_V];
+
+void fno_set_footprint_components(int C, const int32_t* sizes) {
+    g_ncomp = (C > 1 && C <= FNO_MAX_V) ? C : 0;
+    for (int c = 0; c < g_ncomp; ++c) g_comp[c] = sizes[c];
+}
+
+static int collision_union(const uint8_t* occ, int H, int W, double rho, int V, const float* fp_xy,
+                           double x, double y, double psi, double eps, int* amb) {
+    if (g_ncomp <= 1) return collision_one(occ, H, W, rho, V, fp_xy, x, y, psi, eps, amb);
+    int flag = 0, robust = 0, near = 0, off = 0;
+    for (int c = 0; c < g_ncomp; ++c) {
+        int a = 0;
+        const int f = collision_one(occ, H, W, rho, g_comp[c], fp_xy + 2 * off, x, y, psi, eps, &a);
+        flag |= f;
+        robust |= (f && !a);
+        near |= (f || a);
+        off += g_comp[c];
+    }
+    (void)V;
+    if (amb) *amb = (!robust && near);
+    return flag;
+}
+
 void fno_collision(const uint8_t* occ, int H, int W, float res, int V, const float* fp_xy, int n,
                    const float* x, const float* y, const float* psi, double eps,
                    uint8_t* flag, uint8_t* amb) {
     for (int e = 0; e < n; ++e) {
         int a = 0;
-        flag[e] = (uint8_t)collision_one(occ, H, W, (double)res, V, fp_xy, x[e], y[e], psi[e], eps, &a);
+        flag[e] = (uint8_t)collision_union(occ, H, W, (double)res, V, fp_xy, x[e], y[e], psi[e], eps, &a);
         if (amb) amb[e] = (uint8_t)a;
     }
 }
@@ -480,7 +512,7 @@ void fno_reset(const uint8_t* occ, int H, int W, float res, int V, const float* 
             y = fmaf(u24(sigma, 3u * k + 1u), Ye, Y0);
             psi = fmaf(u24(sigma, 3u * k + 2u), two_pi_f, -pi_f);
             int a = 0;
-            ok = !collision_one(occ, H, W, rho, V, fp_xy, x, y, psi, eps, &a);
+            ok = !collision_union(occ, H, W, rho, V, fp_xy, x, y, psi, eps, &a);
             ambiguous |= a;
         }
         if (!ok) fail = 1;
@@ -567,13 +599,26 @@ static int point_in_polygon(double px, double py, int V, const float* fp_xy) {  
     return in;
 }
 
-/* Eq. (3) for one body-frame point */
-double fno_footprint_distance(int V, const float* fp_xy, double px, double py) {
+/* Eq. (3) for one body-frame point and one polygon */
+static double polygon_distance(int V, const float* fp_xy, double px, double py) {
     if (point_in_polygon(px, py, V, fp_xy)) return 0.0;
     double d = INFINITY;
     for (int k = 0, j = V - 1; k < V; j = k++) {
         const double dk = point_segment_dist(px, py, fp_xy[2 * j], fp_xy[2 * j + 1], fp_xy[2 * k], fp_xy[2 * k + 1]);
         if (dk < d) d = dk;
+    }
+    return d;
+}
+
+/* ... and for the footprint: "For a union of polygons, the minimum distance over its components" */
+double fno_footprint_distance(int V, const float* fp_xy, double px, double py) {
+    if (g_ncomp <= 1) return polygon_distance(V, fp_xy, px, py);
+    double d = INFINITY;
+    int off = 0;
+    for (int c = 0; c < g_ncomp; ++c) {
+        const double dc = polygon_distance(g_comp[c], fp_xy + 2 * off, px, py);
+        if (dc < d) d = dc;
+        off += g_comp[c];
     }
     return d;
 }

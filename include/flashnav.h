@@ -63,6 +63,13 @@ int fn_map_destroy(fn_map* map);
  * vel_limits_host:   [6] = vx_min, vx_max, vy_min, vy_max, w_min, w_max (min <= max). */
 int fn_robot_create(const float* footprint_xy_host, int V, const float* beam_angles_host, int B,
                     float max_range_m, int drive_type, const float* vel_limits_host, fn_robot** out);
+/* Footprints that are a UNION of polygons ("polygon(s)"; :129 "For a union of polygons, the minimum
+ * distance over its components is used"): footprint_xy_host holds the polygons' vertex lists one after the
+ * other, comp_sizes_host [C] their vertex counts (each >= 3, total <= FN_MAX_VERTS).  The polygons may overlap;
+ * the robot collides iff any of them does, a point is inside the footprint iff it is inside any of them. */
+int fn_robot_create_union(const float* footprint_xy_host, const int32_t* comp_sizes_host, int C,
+                          const float* beam_angles_host, int B, float max_range_m, int drive_type,
+                          const float* vel_limits_host, fn_robot** out);
 /* sensor placement S in the body frame; default (0, 0, 0). */
 int fn_robot_set_sensor(fn_robot* robot, float sx_m, float sy_m, float spsi_rad);
 /* acceleration limits of U: acc_host [3] = maximum |dv_x/dt|, |dv_y/dt|, |dw/dt| (> 0; +inf = none,

@@ -16,7 +16,7 @@ COUNTER_NAMES = ("rays_cast", "map_words_loaded", "envs_reset", "reset_failures"
                  "env_steps", "oob_window_loads", "reserved1")
 
 EXPORTED_SYMBOLS = (
-    "fn_map_create", "fn_map_set_regions", "fn_map_destroy", "fn_robot_create", "fn_robot_set_sensor", "fn_robot_set_acc_limits",
+    "fn_map_create", "fn_map_set_regions", "fn_map_destroy", "fn_robot_create", "fn_robot_create_union", "fn_robot_set_sensor", "fn_robot_set_acc_limits",
     "fn_robot_destroy", "fn_task_default", "fn_sim_create", "fn_sim_destroy", "fn_sim_set_stream", "fn_step", "fn_reset",
     "fn_sim_bind_aux", "fn_sim_bind_features", "fn_ring_attach", "fn_ring_sample", "fn_ranges_fixed_step", "fn_eval_begin", "fn_eval_result", "fn_eval_end", "fn_observe_all", "fn_get_counters", "fn_sim_count_words",
     "fn_sim_episode_state", "fn_sim_beam_config", "fn_sim_profile", "fn_sim_profile_read", "fn_step_host", "fn_measure_peak", "fn_last_error", "fn_version")
@@ -51,6 +51,7 @@ def load_library():
         "fn_map_set_regions": [vp, i32, vp],
         "fn_map_destroy": [vp],
         "fn_robot_create": [vp, i32, vp, i32, f32, i32, vp, C.POINTER(vp)],
+        "fn_robot_create_union": [vp, vp, i32, vp, i32, f32, i32, vp, C.POINTER(vp)],
         "fn_robot_set_sensor": [vp, f32, f32, f32],
         "fn_robot_set_acc_limits": [vp, vp],
         "fn_robot_destroy": [vp],
@@ -145,7 +146,9 @@ class Map:
 class Robot:
     """fn_robot: footprint polygon [V,2], beam angles [B], max range, drive type, velocity limits [6]."""
 
-    def __init__(self, footprint, beam_angles, max_range, drive, vel_limits):
+    def __init__(self, footprint, beam_angles, max_range, drive, vel_limits, components=None):
+        """components: vertex counts of the polygons whose vertex lists are concatenated in `footprint`
+        (a union of polygons); None = one polygon."""
         lib = load_library()
         fp = np.ascontiguousarray(footprint, np.float32).reshape(-1, 2)
         ang = np.ascontiguousarray(beam_angles, np.float32).reshape(-1)
@@ -155,8 +158,16 @@ class Robot:
         self.V, self.B, self.drive = int(fp.shape[0]), int(ang.shape[0]), int(drive)
         self.A = 2 if self.drive == DRIVE_DIFF else 3
         h = C.c_void_p()
-        _check(lib.fn_robot_create(_np_ptr(fp), self.V, _np_ptr(ang), self.B, C.c_float(max_range), self.drive,
-                                   _np_ptr(lim), C.byref(h)), "fn_robot_create")
+        if components is None:
+            _check(lib.fn_robot_create(_np_ptr(fp), self.V, _np_ptr(ang), self.B, C.c_float(max_range), self.drive,
+                                       _np_ptr(lim), C.byref(h)), "fn_robot_create")
+        else:
+            comp = np.ascontiguousarray(components, np.int32).reshape(-1)
+            if int(comp.sum()) != self.V:
+                raise FlashNavError("components must add up to the number of footprint vertices")
+            _check(lib.fn_robot_create_union(_np_ptr(fp), _np_ptr(comp), int(comp.shape[0]), _np_ptr(ang), self.B,
+                                             C.c_float(max_range), self.drive, _np_ptr(lim), C.byref(h)),
+                   "fn_robot_create_union")
         self._h = h
 
     def set_sensor(self, sx, sy, spsi):

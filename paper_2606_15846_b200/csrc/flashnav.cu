@@ -58,6 +58,8 @@ struct fn_robot {
     double2* d_verts;
     double2* d_samples;              // interior sample points of the footprint (reset pre-test)
     int n_samples;
+    std::vector<int> nxt;            // next vertex within the vertex's component (union of polygons)
+    int* d_nxt;
 };
 
 struct fn_sim {
@@ -194,7 +196,7 @@ extern "C" int fn_map_destroy(fn_map* m) {
 // its bounding box.  A sample whose map cell is occupied proves a collision (the converse does not hold),
 // which lets fn_reset discard most colliding start-pose attempts without the exact polygon test.
 constexpr int kMaxSamples = 32;
-static std::vector<double2> interior_samples(const std::vector<float>& v, int V) {
+static std::vector<double2> interior_samples(const std::vector<float>& v, const std::vector<int>& nxt, int V) {
     double x0 = 1e300, x1 = -1e300, y0 = 1e300, y1 = -1e300;
     for (int k = 0; k < V; ++k) {
         x0 = std::fmin(x0, v[2 * k]); x1 = std::fmax(x1, v[2 * k]);
@@ -206,11 +208,13 @@ static std::vector<double2> interior_samples(const std::vector<float>& v, int V)
         for (int a = 0; a < g; ++a)
             for (int b = 0; b < g; ++b) {
                 const double px = x0 + (x1 - x0) * (a + 0.5) / g, py = y0 + (y1 - y0) * (b + 0.5) / g;
-                bool in = false;
+                bool in = false, in_c = false;                     // inside ANY component (even-odd per component)
                 double dmin = 1e300;
-                for (int k = 0, j = V - 1; k < V; j = k++) {
+                for (int j = 0; j < V; ++j) {                      // edge j -> nxt[j]
+                    const int k = nxt[j];
                     const double ax = v[2 * j], ay = v[2 * j + 1], bx = v[2 * k], by = v[2 * k + 1];
-                    if ((ay > py) != (by > py) && px < ax + (py - ay) * (bx - ax) / (by - ay)) in = !in;
+                    if ((ay > py) != (by > py) && px < ax + (py - ay) * (bx - ax) / (by - ay)) in_c = !in_c;
+                    if (k <= j) { in = in || in_c; in_c = false; }
                     const double ex = bx - ax, ey = by - ay, l2 = ex * ex + ey * ey;
                     double t = l2 > 0.0 ? ((px - ax) * ex + (py - ay) * ey) / l2 : 0.0;
                     t = std::fmin(1.0, std::fmax(0.0, t));
@@ -237,17 +241,23 @@ static int robot_upload(fn_robot* r) {
     for (int k = 0; k < r->V; ++k) vs[k] = make_double2((double)r->verts[2 * k], (double)r->verts[2 * k + 1]);
     FN_CUDA(cudaMemcpy(r->d_beam_cs, cs.data(), cs.size() * sizeof(double2), cudaMemcpyHostToDevice));
     FN_CUDA(cudaMemcpy(r->d_verts, vs.data(), vs.size() * sizeof(double2), cudaMemcpyHostToDevice));
-    const std::vector<double2> sp = interior_samples(r->verts, r->V);
+    FN_CUDA(cudaMemcpy(r->d_nxt, r->nxt.data(), r->nxt.size() * sizeof(int), cudaMemcpyHostToDevice));
+    const std::vector<double2> sp = interior_samples(r->verts, r->nxt, r->V);
     r->n_samples = (int)sp.size();
     if (r->n_samples) FN_CUDA(cudaMemcpy(r->d_samples, sp.data(), sp.size() * sizeof(double2), cudaMemcpyHostToDevice));
     return FN_OK;
 }
 
-extern "C" int fn_robot_create(const float* fp, int V, const float* angles, int B, float rmax, int drive,
-                               const float* lim, fn_robot** out) {
-    if (!fp || !angles || !lim || !out) return fail(FN_ERR_INVALID_ARG, "fn_robot_create: NULL argument");
-    if (V < 3) return fail(FN_ERR_INVALID_ARG, "fn_robot_create: footprint needs >= 3 vertices");
-    if (V > FN_MAX_VERTS) return fail(FN_ERR_UNSUPPORTED, "fn_robot_create: V > FN_MAX_VERTS (%d)", FN_MAX_VERTS);
+extern "C" int fn_robot_create_union(const float* fp, const int32_t* comp_sizes, int C, const float* angles, int B,
+                                     float rmax, int drive, const float* lim, fn_robot** out) {
+    if (!fp || !comp_sizes || !angles || !lim || !out) return fail(FN_ERR_INVALID_ARG, "fn_robot_create: NULL argument");
+    if (C < 1) return fail(FN_ERR_INVALID_ARG, "fn_robot_create: a footprint needs >= 1 polygon");
+    int V = 0;
+    for (int c = 0; c < C; ++c) {
+        if (comp_sizes[c] < 3) return fail(FN_ERR_INVALID_ARG, "fn_robot_create: footprint needs >= 3 vertices (per polygon)");
+        V += comp_sizes[c];
+        if (V > FN_MAX_VERTS) return fail(FN_ERR_UNSUPPORTED, "fn_robot_create: V > FN_MAX_VERTS (%d)", FN_MAX_VERTS);
+    }
     if (B < 1) return fail(FN_ERR_INVALID_ARG, "fn_robot_create: B must be >= 1");
     if (!std::isfinite(rmax) || rmax <= 0.0f) return fail(FN_ERR_INVALID_ARG, "fn_robot_create: max range must be finite and > 0");
     if (drive != FN_DRIVE_DIFF && drive != FN_DRIVE_OMNI) return fail(FN_ERR_INVALID_ARG, "fn_robot_create: unknown drive type");
@@ -264,20 +274,31 @@ extern "C" int fn_robot_create(const float* fp, int V, const float* angles, int 
     r->acc[0] = r->acc[1] = r->acc[2] = INFINITY;
     r->angles.assign(angles, angles + B);
     r->verts.assign(fp, fp + 2 * V);
-    r->d_beam_cs = nullptr; r->d_verts = nullptr; r->d_samples = nullptr; r->n_samples = 0;
+    r->nxt.resize(V);
+    for (int c = 0, off = 0; c < C; off += comp_sizes[c], ++c)
+        for (int k = 0; k < comp_sizes[c]; ++k) r->nxt[off + k] = off + (k + 1 == comp_sizes[c] ? 0 : k + 1);
+    r->d_beam_cs = nullptr; r->d_verts = nullptr; r->d_samples = nullptr; r->n_samples = 0; r->d_nxt = nullptr;
     cudaError_t e = cudaMalloc(&r->d_beam_cs, (size_t)B * sizeof(double2));
     if (e == cudaSuccess) e = cudaMalloc(&r->d_verts, (size_t)V * sizeof(double2));
+    if (e == cudaSuccess) e = cudaMalloc(&r->d_nxt, (size_t)V * sizeof(int));
     if (e == cudaSuccess) e = cudaMalloc(&r->d_samples, (size_t)kMaxSamples * sizeof(double2));
     int st = (e == cudaSuccess) ? robot_upload(r) : fail(e == cudaErrorMemoryAllocation ? FN_ERR_OOM : FN_ERR_CUDA, "fn_robot_create: %s", cudaGetErrorString(e));
     if (st != FN_OK) {
         if (r->d_beam_cs) cudaFree(r->d_beam_cs);
         if (r->d_verts) cudaFree(r->d_verts);
+        if (r->d_nxt) cudaFree(r->d_nxt);
         if (r->d_samples) cudaFree(r->d_samples);
         delete r;
         return st;
     }
     *out = r;
     return FN_OK;
+}
+
+extern "C" int fn_robot_create(const float* fp, int V, const float* angles, int B, float rmax, int drive,
+                               const float* lim, fn_robot** out) {
+    const int32_t one = V;
+    return fn_robot_create_union(fp, &one, 1, angles, B, rmax, drive, lim, out);
 }
 
 extern "C" int fn_robot_set_sensor(fn_robot* r, float sx, float sy, float spsi) {
@@ -298,6 +319,7 @@ extern "C" int fn_robot_destroy(fn_robot* r) {
     if (!r) return FN_OK;
     if (r->d_beam_cs) cudaFree(r->d_beam_cs);
     if (r->d_verts) cudaFree(r->d_verts);
+    if (r->d_nxt) cudaFree(r->d_nxt);
     if (r->d_samples) cudaFree(r->d_samples);
     delete r;
     return FN_OK;
@@ -305,7 +327,7 @@ extern "C" int fn_robot_destroy(fn_robot* r) {
 
 static RobotDev robot_dev(const fn_robot* r, const fn_map* m) {
     RobotDev d;
-    d.beam_cs = r->d_beam_cs; d.verts = r->d_verts; d.samples = r->d_samples; d.n_samples = r->n_samples; d.B = r->B; d.V = r->V; d.drive = r->drive;
+    d.beam_cs = r->d_beam_cs; d.verts = r->d_verts; d.nxt = r->d_nxt; d.samples = r->d_samples; d.n_samples = r->n_samples; d.B = r->B; d.V = r->V; d.drive = r->drive;
     d.A = r->drive == FN_DRIVE_DIFF ? 2 : 3;
     for (int k = 0; k < 6; ++k) d.lim[k] = r->lim[k];
     for (int k = 0; k < 3; ++k) d.acc[k] = r->acc[k];
@@ -463,7 +485,7 @@ static int launch_beams(fn_sim* s, const int* list, const int* count_dev, float*
 static int launch_features(fn_sim* s, const int* list, const int* count_dev, bool done_list, const float* ranges) {
     if (!s->feat_z) return FN_OK;
     FeatArgs f;
-    f.beam_cs = s->robot->d_beam_cs; f.verts = s->robot->d_verts; f.B = s->robot->B; f.V = s->robot->V;
+    f.beam_cs = s->robot->d_beam_cs; f.verts = s->robot->d_verts; f.nxt = s->robot->d_nxt; f.B = s->robot->B; f.V = s->robot->V;
     f.n_sectors = s->feat_sectors; f.rmax = s->robot->rmax; f.sx = s->robot->sensor[0]; f.sy = s->robot->sensor[1];
     f.ranges = ranges; f.z = s->feat_z; f.list = list; f.count_dev = count_dev;
     f.list_par_dev = done_list ? s->d_done_count + 2 : nullptr; f.n_all = s->n;

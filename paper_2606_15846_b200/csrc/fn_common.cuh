@@ -53,7 +53,8 @@ struct __align__(32) BeamPose {
 
 struct RobotDev {
     const double2* beam_cs;  // [B] (cos, sin) of theta_j + s_psi
-    const double2* verts;    // [V] footprint vertices, body frame, metres
+    const double2* verts;    // [V] footprint vertices, body frame, metres (components one after the other)
+    const int* nxt;          // [V] next vertex within the vertex's component (a union of polygons)
     const double2* samples;  // [n_samples] points inside the footprint (body frame): a cheap one-sided pre-test
     int n_samples;
     int B, V;

@@ -88,8 +88,9 @@ struct ColScratch {          // per warp, in dynamic shared memory
     int* win;                // [32][4] i0, j0, j1, -
     unsigned* hit;           // [1] bit per slot
     double2* verts;          // [V] copy of the footprint vertices (body frame, metres)
+    int* nxt;                // [V] next vertex of each vertex within its component
 };
-__host__ __device__ inline size_t col_scratch_bytes(int V) { return (size_t)32 * 3 * V * 8 + (size_t)V * 16 + 32 * 4 + 32 * 16 + 16; }
+__host__ __device__ inline size_t col_scratch_bytes(int V) { return (size_t)32 * 3 * V * 8 + (size_t)V * 16 + (size_t)((V + 3) / 4) * 16 + 32 * 4 + 32 * 16 + 16; }
 __device__ __forceinline__ ColScratch col_scratch(uint8_t* base, int V) {
     ColScratch cs;
     cs.vx = reinterpret_cast<double*>(base);
@@ -99,13 +100,14 @@ __device__ __forceinline__ ColScratch col_scratch(uint8_t* base, int V) {
     cs.pref = reinterpret_cast<int*>(cs.verts + V);
     cs.win = cs.pref + 32;
     cs.hit = reinterpret_cast<unsigned*>(cs.win + 32 * 4);
+    cs.nxt = reinterpret_cast<int*>(cs.hit + 4);
     return cs;
 }
 
 // All 32 lanes must call; `need` = this lane's pose needs the exact test (window status 2).
 // Returns true for a lane whose polygon meets an occupied cell (false for lanes that did not need it).
 __device__ __noinline__ bool warp_collisions_exact(const uint32_t* __restrict__ row, const int strideR,
-                                                   const double2* __restrict__ verts, const int V,
+                                                   const double2* __restrict__ verts, const int* __restrict__ nxt, const int V,
                                                    const double inv, const bool need, const double x, const double y,
                                                    const double c, const double s, const int i0, const int i1,
                                                    const int j0, const int j1, const ColScratch cs) {
@@ -120,8 +122,8 @@ __device__ __noinline__ bool warp_collisions_exact(const uint32_t* __restrict__ 
             vx[k] = (x + c * f.x - s * f.y) * inv;
             vy[k] = (y + s * f.x + c * f.y) * inv;
         }
-        for (int k = 0; k < V; ++k) {                              // edge k: vertex k -> k+1
-            const int k1 = k + 1 == V ? 0 : k + 1;
+        for (int k = 0; k < V; ++k) {                              // edge k: vertex k -> nxt[k] (within its component)
+            const int k1 = nxt[k];
             const double dy = vy[k1] - vy[k];
             double r = 0.0;
             if (dy != 0.0) {                                       // 1 / dy: one Newton step on the 20-bit
@@ -157,10 +159,13 @@ __device__ __noinline__ bool warp_collisions_exact(const uint32_t* __restrict__ 
             for (int jb = sj0; jb <= sj1 && !found; jb += 32) {
                 const uint32_t occ = row_bits(row, strideR, i, jb) & low_bits(sj1 - jb + 1);
                 if (occ == 0u) continue;
-                uint32_t touch = 0, inside = 0;
-                double px = vx[V - 1], py = vy[V - 1];
-                for (int k = 0; k < V; ++k) {                      // edge k-1: vertex k-1 -> k
-                    const double qx = vx[k], qy = vy[k], sk = sl[k == 0 ? V - 1 : k - 1];
+                // a footprint may be a union of polygons: the edges of a component are
+                // consecutive and close on themselves (nxt[k] <= k at its last vertex); the cells inside
+                // the union are the OR of the components' even-odd masks
+                uint32_t touch = 0, inside = 0, inside_c = 0;
+                for (int k = 0; k < V; ++k) {                      // edge k: vertex k -> nxt[k]
+                    const int k1 = nxt[k];
+                    const double px = vx[k], py = vy[k], qx = vx[k1], qy = vy[k1], sk = sl[k];
                     const double elo = fmin(py, qy), ehi = fmax(py, qy);
                     if (ehi >= ylo_s && elo <= yhi_s) {            // the edge meets the closed strip
                         const double exlo = fmin(px, qx), exhi = fmax(px, qx);
@@ -175,9 +180,9 @@ __device__ __noinline__ bool warp_collisions_exact(const uint32_t* __restrict__ 
                     if ((py > yc) != (qy > yc)) {                   // crosses the centre line: cells with
                         const double xc = px + (yc - py) * sk;      // centre j + 1/2 < xc lie to its left
                         const int nleft = __double2int_ru(xc - 0.5) - jb;
-                        inside ^= low_bits(min(max(nleft, 0), 32));
+                        inside_c ^= low_bits(min(max(nleft, 0), 32));
                     }
-                    px = qx; py = qy;
+                    if (k1 <= k) { inside |= inside_c; inside_c = 0u; }
                 }
                 found = (occ & (touch | inside)) != 0u;
             }
@@ -194,7 +199,7 @@ __device__ __forceinline__ bool resolve_collisions(const MapDev& m, const RobotD
     const bool need = w.status == 2;
     bool col = w.status == 1;
     if (__any_sync(0xffffffffu, need))
-        col |= warp_collisions_exact(m.row, m.strideR, cs.verts, rb.V, m.inv_rho, need, x, y, c, s,
+        col |= warp_collisions_exact(m.row, m.strideR, cs.verts, cs.nxt, rb.V, m.inv_rho, need, x, y, c, s,
                                      w.i0, w.i1, w.j0, w.j1, cs);
     return col;
 }
@@ -266,7 +271,7 @@ constexpr int kEnvBlock = 32;
 __global__ void __launch_bounds__(kEnvBlock) env_step_kernel(EnvArgs a) {
     extern __shared__ __align__(16) uint8_t s_dyn[];
     const ColScratch scratch = col_scratch(s_dyn, a.robot.V);
-    for (int k = threadIdx.x; k < a.robot.V; k += kEnvBlock) scratch.verts[k] = a.robot.verts[k];
+    for (int k = threadIdx.x; k < a.robot.V; k += kEnvBlock) { scratch.verts[k] = a.robot.verts[k]; scratch.nxt[k] = a.robot.nxt[k]; }
     __syncwarp();
     griddep_wait();                                                // states / actions / mask come from earlier work
     griddep_launch_dependents();                                   // the beam kernel may start staging the map now
@@ -514,7 +519,7 @@ __global__ void __launch_bounds__(kResetWarps * 32) reset_kernel(ResetArgs a) {
     extern __shared__ __align__(16) uint8_t s_dyn[];
     const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const ColScratch scratch = col_scratch(s_dyn + (size_t)wib * col_scratch_bytes(a.robot.V), a.robot.V);
-    for (int k = lane; k < a.robot.V; k += 32) scratch.verts[k] = a.robot.verts[k];
+    for (int k = lane; k < a.robot.V; k += 32) { scratch.verts[k] = a.robot.verts[k]; scratch.nxt[k] = a.robot.nxt[k]; }
     __syncwarp();
     griddep_wait();                                                // the list comes from the compaction kernel
     griddep_launch_dependents();

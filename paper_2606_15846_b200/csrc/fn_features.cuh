@@ -19,6 +19,7 @@ namespace fn {
 struct FeatArgs {
     const double2* beam_cs;      // [B] (cos, sin) of theta_j + s_psi
     const double2* verts;        // [V] footprint vertices, body frame, metres
+    const int* nxt;              // [V] next vertex within the vertex's component (union of polygons)
     int B, V, n_sectors;
     float rmax, sx, sy;
     const float* ranges;         // [N][B]
@@ -32,7 +33,7 @@ struct FeatArgs {
 constexpr int kFeatWarps = 8;
 
 __host__ __device__ inline size_t feat_smem_bytes(int V, int n_sectors) {
-    return (size_t)V * 7 * sizeof(float) + (size_t)kFeatWarps * n_sectors * sizeof(unsigned);
+    return (size_t)V * 8 * sizeof(float) + (size_t)kFeatWarps * n_sectors * sizeof(unsigned);
 }
 __host__ __device__ inline size_t feat_smem_bytes(int V, int n_sectors, int B) {
     return feat_smem_bytes(V, n_sectors) + (size_t)B * sizeof(float2);
@@ -40,8 +41,10 @@ __host__ __device__ inline size_t feat_smem_bytes(int V, int n_sectors, int B) {
 
 __global__ void __launch_bounds__(kFeatWarps * 32) features_kernel(FeatArgs a) {
     extern __shared__ __align__(16) uint8_t s_dyn[];
-    // beam directions as floats, then per edge k (vertex k-1 -> k): start a, direction e, 1/|e|^2, e_x/e_y,
-    // end vertex y (the SAME float the next edge starts at, so the even-odd rule is consistent at vertices)
+    // beam directions as floats, then per edge k (vertex k -> nxt[k]): start a, direction e, 1/|e|^2, e_x/e_y,
+    // end vertex y (the SAME float the edge from that vertex starts at, so the even-odd rule is consistent
+    // at vertices) and whether the edge closes its component ("For a union of polygons, the minimum
+    // distance over its components is used": inside = inside ANY component)
     float2* s_cs = reinterpret_cast<float2*>(s_dyn);
     float* s_ax = reinterpret_cast<float*>(s_cs + a.B);
     float* s_ay = s_ax + a.V;
@@ -50,10 +53,13 @@ __global__ void __launch_bounds__(kFeatWarps * 32) features_kernel(FeatArgs a) {
     float* s_il = s_ey + a.V;
     float* s_sl = s_il + a.V;
     float* s_by = s_sl + a.V;
-    unsigned* s_z = reinterpret_cast<unsigned*>(s_by + a.V) + (threadIdx.x >> 5) * a.n_sectors;
+    int* s_last = reinterpret_cast<int*>(s_by + a.V);
+    unsigned* s_z = reinterpret_cast<unsigned*>(s_last + a.V) + (threadIdx.x >> 5) * a.n_sectors;
     for (int j = threadIdx.x; j < a.B; j += blockDim.x) { const double2 c = a.beam_cs[j]; s_cs[j] = make_float2((float)c.x, (float)c.y); }
     for (int k = threadIdx.x; k < a.V; k += blockDim.x) {
-        const double2 p = a.verts[k == 0 ? a.V - 1 : k - 1], q = a.verts[k];
+        const int k1 = a.nxt[k];
+        const double2 p = a.verts[k], q = a.verts[k1];
+        s_last[k] = k1 <= k;
         const float ex = (float)(q.x - p.x), ey = (float)(q.y - p.y), l2 = ex * ex + ey * ey;
         s_ax[k] = (float)p.x; s_ay[k] = (float)p.y; s_ex[k] = ex; s_ey[k] = ey;
         s_il[k] = l2 > 0.0f ? 1.0f / l2 : 0.0f;
@@ -86,14 +92,15 @@ __global__ void __launch_bounds__(kFeatWarps * 32) features_kernel(FeatArgs a) {
                     const float2 cs = s_cs[j];
                     const float px = fmaf(r[u], cs.x, a.sx), py = fmaf(r[u], cs.y, a.sy);
                     float d2 = INFINITY;
-                    bool inside = false;
+                    bool inside = false, inside_c = false;
                     for (int k = 0; k < a.V; ++k) {
                         const float ax = s_ax[k], ay = s_ay[k], ex = s_ex[k], ey = s_ey[k];
                         const float rx = px - ax, ry = py - ay;
                         const float t = fminf(fmaxf((rx * ex + ry * ey) * s_il[k], 0.0f), 1.0f);
                         const float qx = rx - t * ex, qy = ry - t * ey;
                         d2 = fminf(d2, qx * qx + qy * qy);
-                        if ((ay > py) != (s_by[k] > py) && rx < ry * s_sl[k]) inside = !inside;      // even-odd rule
+                        if ((ay > py) != (s_by[k] > py) && rx < ry * s_sl[k]) inside_c = !inside_c;  // even-odd rule
+                        if (s_last[k]) { inside |= inside_c; inside_c = false; }
                     }
                     d = inside ? 0.0f : fminf(sqrtf(d2), a.rmax);  // capped at the sensor range
                 }

@@ -24,7 +24,8 @@ def make_sim(wl, n=None):
     m = fn.Map(wl.occ, float(wl.resolution))
     if wl.regions is not None:
         m.set_regions(wl.regions)
-    r = fn.Robot(wl.footprint, wl.beam_angles, float(wl.max_range), wl.drive, wl.vel_limits)
+    r = fn.Robot(wl.footprint, wl.beam_angles, float(wl.max_range), wl.drive, wl.vel_limits,
+                 components=getattr(wl, "components", None))
     if getattr(wl, "acc_limits", None) is not None:
         r.set_acc_limits(wl.acc_limits)
     s = fn.Sim(m, r, n, goal_tol=float(wl.goal_tol), max_episode_steps=wl.max_episode_steps,
@@ -89,6 +90,7 @@ def run_parity(wl, steps, n=None, subset=None, seed=0, forced=None, check_every=
     n = wl.n_envs if n is None else n
     wl.n_envs = n
     B, A = wl.n_beams, wl.action_dim
+    oracle.set_footprint_components(getattr(wl, "components", None))      # a union of polygons, or None
     m, r, s = make_sim(wl, n)
     buf = Buffers(n, B, A)
     s.bind_aux(buf.hit, buf.reward)
@@ -213,4 +215,5 @@ def run_parity(wl, steps, n=None, subset=None, seed=0, forced=None, check_every=
     assert cnt["oob_window_loads"] == 0, "the instrumented beam kernel read a window outside the packed map"
     assert cnt["reset_failures"] == rep.c.get("reset_failures", 0) or check_every > 1
     s.close(); r.close(); m.close()
+    oracle.set_footprint_components(None)
     return rep

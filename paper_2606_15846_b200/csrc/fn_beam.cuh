@@ -28,9 +28,9 @@
 
 namespace fn {
 
-// Address spaces for the packed map: staged in shared memory, or read through L1/L2.
-// `base` addresses the start of the row copy MINUS the constant that the exponent bits of D's high
-// word add to the word offset (kMagicHi >> 5 words), so the hot loop never masks them off.
+// Address spaces for the packed map: staged in shared memory, or read through L1/L2.  The window
+// address of a line is (line base) + 4 * (high word of D >> 5); the constant that D's exponent bits
+// add to that offset (kExpOff) is subtracted from the line base once per beam, so no loop masks them off.
 struct SmemSpace {
     using addr_t = uint32_t;                                     // shared-window byte address
     static __device__ __forceinline__ uint32_t ld(addr_t a) {

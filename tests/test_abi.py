@@ -59,6 +59,18 @@ def test_host_side_argument_errors_need_no_gpu(fn):
     assert lib.fn_robot_create(p(fp), 65, p(ang), 1, ctypes.c_float(1.0), 0, p(lim), ctypes.byref(out)) == -2
     assert lib.fn_robot_create(p(fp), 3, p(ang), 0, ctypes.c_float(1.0), 0, p(lim), ctypes.byref(out)) == -1
     assert lib.fn_step(None, None, None, ctypes.c_float(0.1), None, None, None, None) == -1
+    # the entry points of the widened rows validate on the host as well
+    comp = np.array([3, 2], np.int32)
+    fp5 = np.zeros((5, 2), np.float32)
+    assert lib.fn_robot_create_union(p(fp5), p(comp), 2, p(ang), 1, ctypes.c_float(1.0), 0, p(lim), ctypes.byref(out)) == -1
+    assert lib.fn_robot_create_union(p(fp5), p(comp), 0, p(ang), 1, ctypes.c_float(1.0), 0, p(lim), ctypes.byref(out)) == -1
+    assert lib.fn_robot_set_acc_limits(None, p(lim)) == -1
+    assert lib.fn_sim_bind_features(None, 8, None) == -1
+    assert lib.fn_ring_sample(None, ctypes.c_uint64(1), 4, None, None) == -1
+    assert lib.fn_eval_begin(None, None, 1, 1, None, None) == -1
+    assert lib.fn_eval_result(None, None, None, None, None) == -1 and lib.fn_eval_end(None) == -1
+    assert lib.fn_ranges_fixed_step(None, None, ctypes.c_float(0.1), 1, None) == -1
+    assert lib.fn_sim_set_stream(None, None) == -1 and lib.fn_reset(None, None, None, None, None, None) == -1
 
 
 def test_no_cpu_fallback(fn):

@@ -39,7 +39,7 @@ UNIT = "env-steps/s"
 
 
 def workload_name(cfg):
-    return f"BASELINE.json configs[{cfg - 1}]"
+    return f"BASELINE.json configs[{cfg - 1}]" if cfg <= 5 else "extra: C1's robot on C2's map (N sweep, PAPER.md:175 Fig. 5)"
 
 
 # --------------------------------------------------------------------------- reference arm = the oracle
@@ -49,7 +49,7 @@ def run_reference(args):
         return 0
     import oracle
     oracle.build()
-    wl = W.make_workload(args.config)
+    wl = W.make_workload(args.config, n_envs=args.envs or None)
     n = min(wl.n_envs, args.ref_envs)
     wl.n_envs = n
     st = np.zeros((8, n), np.float32)
@@ -78,7 +78,7 @@ def run_reference(args):
         resets += one(t)
     dt = time.perf_counter() - t0
     v = n * args.steps / dt
-    sample = f"{n} of {W.make_workload(args.config).n_envs} envs x {args.steps} steps, single thread"
+    sample = f"{n} of {W.make_workload(args.config, n_envs=args.envs or None).n_envs} envs x {args.steps} steps, single thread"
     line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
@@ -187,7 +187,7 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     fn.load_library()
 
-    wl = W.make_workload(args.config)
+    wl = W.make_workload(args.config, n_envs=args.envs or None)
     n, B, A = wl.n_envs, wl.n_beams, wl.action_dim
     K, Wm = args.steps, args.warmup
     tape_len = min(K + Wm, 256)
@@ -201,6 +201,7 @@ def run_ours(args):
     rb = fn.Robot(wl.footprint, wl.beam_angles, float(wl.max_range), wl.drive, wl.vel_limits)
     sim = fn.Sim(m, rb, n, goal_tol=float(wl.goal_tol), max_episode_steps=wl.max_episode_steps,
                  goal_dist_min=float(wl.goal_dist_min), goal_dist_max=float(wl.goal_dist_max))
+    fused_active = sim.set_fused_reset(bool(args.fused_reset))
     states = torch.zeros(8, n, device="cuda")
     mask = torch.ones(n, dtype=torch.uint8, device="cuda")
     ranges = torch.zeros(n, B, device="cuda")
@@ -433,12 +434,29 @@ def run_ours(args):
             cpu = {"value": ns * args.cpu_steps / dtc, "unit": UNIT, "cores": 1, "kind": "oracle",
                    "sample": f"{ns} of {n} envs x {args.cpu_steps} steps (fn_step part only, no resets), single thread",
                    "rays_per_s": ns * args.cpu_steps * B / dtc, "host_cores_available": os.cpu_count()}
+            # the same unmodified oracle, env-sharded over all host cores: one thread per
+            # contiguous env range, each thread calls the single-threaded C oracle (ctypes drops the GIL)
+            from concurrent.futures import ThreadPoolExecutor
+            nc = max(1, min(os.cpu_count() or 1, ns))
+            cuts = [ns * i // nc for i in range(nc + 1)]
+            shards = [(np.ascontiguousarray(st_np[:, a:b]), np.zeros(b - a, np.float32), np.zeros(b - a, np.int32),
+                       np.ascontiguousarray(act[:, a:b])) for a, b in zip(cuts[:-1], cuts[1:])]
+
+            def run_shard(sh):
+                for t in range(args.cpu_steps):
+                    oracle.step(wl_s, sh[0], sh[3][t], None, sh[1], sh[2], want_hit=False)
+            with ThreadPoolExecutor(nc) as ex:
+                t0 = time.perf_counter()
+                list(ex.map(run_shard, shards))
+                dta = time.perf_counter() - t0
+            cpu["all_cores"] = {"value": ns * args.cpu_steps / dta, "unit": UNIT, "cores": nc,
+                                "note": "same sample, contiguous env ranges over threads, oracle unmodified"}
         out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
                "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                "dtype": "f64", "data": "synthetic",
                "config": {"workload": workload_name(args.config), "name": wl.name, "n_envs_per_gpu": n, "beams": B,
                           "map": list(wl.occ.shape), "max_range_m": float(wl.max_range), "l2": "flushed between timed steps",
-                          "ring": bool(ring is not None)},
+                          "ring": bool(ring is not None), "fused_reset": bool(fused_active)},
                "rays_per_s": float(rays[0]) / (total_ms * 1e-3),
                "useful_rays_per_s": world * n * B * K / (total_ms * 1e-3),
                "reset_rate_per_step": float(rays[1]) / (world * n * K),
@@ -451,7 +469,9 @@ def run_ours(args):
                                       "compact": prof["compact"][0] / K, "reset": prof["reset"][0] / K,
                                       "beam_reset": prof["beam_reset"][0] / K},
                "ms_per_step_p50": float(np.median(per_step_ms)), "ms_per_step_p90": float(np.percentile(per_step_ms, 90)),
-               "features": feat, "replay_sample": sample, "paper_fixed_step_query": paper_query, "roofline": roofline, "cpu_baseline": cpu, "clocks": clocks, "gpu_launches": 5 * K}
+               "features": feat, "replay_sample": sample, "paper_fixed_step_query": paper_query, "roofline": roofline, "cpu_baseline": cpu, "clocks": clocks,
+               # per step: env_step, beam kernel, [ring_advance], then fn_reset = one fused kernel or reset + beam kernel
+               "gpu_launches": (2 + (1 if ring is not None else 0) + (1 if fused_active else 2)) * K}
 
     # ---- end to end through the public API with HOST buffers (copies inside the timed region)
     hs = torch.empty(8, n, dtype=torch.float32).pin_memory()
@@ -494,6 +514,7 @@ def main():
     ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=20)
     ap.add_argument("--config", type=int, default=2)
+    ap.add_argument("--envs", type=int, default=0, help="override the config's env count per GPU (0 = the config's own)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--ref-envs", type=int, default=4096, help="oracle sample size (envs)")
     ap.add_argument("--cpu-steps", type=int, default=8, help="oracle steps in the cpu_baseline leg")
@@ -503,6 +524,8 @@ def main():
     ap.add_argument("--paper-query", type=int, default=1, help="also time the paper's fixed-step range query (information only)")
     ap.add_argument("--features", type=int, default=36, help="sectors of the clearance-feature leg (0 = skip; information only)")
     ap.add_argument("--graph", type=int, default=1, help="also time a CUDA-graph replay of the steps (information only)")
+    ap.add_argument("--fused-reset", type=int, default=1, choices=[0, 1],
+                    help="fn_reset as one fused kernel where possible (default) or as two kernels (0)")
     ap.add_argument("--ring", type=int, default=1, help="attach the replay ring when the config has one (C5)")
     args = ap.parse_args()
     if args.warmup < 3:

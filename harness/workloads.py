@@ -221,7 +221,7 @@ def beam_table(n_beams: int, fov_deg: float) -> np.ndarray:
 # ----------------------------------------------------------------------------- configs
 
 def make_workload(cfg: int, n_envs: int | None = None) -> Workload:
-    """cfg = 1..5 -> BASELINE.json configs[0..4]."""
+    """cfg = 1..5 -> BASELINE.json configs[0..4]; 6 = the extra N-sweep workload of SURVEY.md 8(d)."""
     f32 = np.float32
     if cfg == 1:
         wl = Workload("C1-tiny", map_rectangles(256, 0.15, 0), RHO, footprint_ngon(0.2, 16),
@@ -247,8 +247,13 @@ def make_workload(cfg: int, n_envs: int | None = None) -> Workload:
                       np.array([0, 1, 0, 0, -2, 2], f32), 65536, f32(0.1), 500, 5,
                       goal_dist_min=f32(1.0), goal_dist_max=f32(3.0), regions=regions,
                       ring_capacity=1 << 22)
+    elif cfg == 6:
+        # extra (context for PAPER.md:175 / Fig. 5): C1's robot on C2's map, for the N sweep
+        wl = Workload("X-fig5-sweep", map_rectangles(512, 0.20, 2, n_discs=30), RHO, footprint_ngon(0.2, 16),
+                      beam_table(360, 360.0), f32(5.0), DRIVE_DIFF,
+                      np.array([0, 1, 0, 0, -2, 2], f32), 1024, f32(0.1), 1000, 6)
     else:
-        raise ValueError("cfg must be 1..5")
+        raise ValueError("cfg must be 1..6")
     if n_envs is not None:
         wl.n_envs = int(n_envs)
     return wl

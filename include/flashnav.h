@@ -196,6 +196,16 @@ int fn_ranges_fixed_step(fn_sim* sim, const float* states_dev, float delta_m, in
  * {map staged in shared memory (1) or read through L1/L2 (0), grid size, CTA size, dynamic shared bytes}. */
 int fn_sim_beam_config(const fn_sim* sim, int* cfg_out);
 
+/* ---- fn_reset as one launch or two.  When the packed map is staged in shared memory (cfg_out[0] of
+ * fn_sim_beam_config) and the reset scratch fits beside it, fn_reset runs ONE kernel in which every CTA
+ * resets its share of the listed envs from its shared copy of the map and then recomputes their beams
+ * (PAPER.md:84); this is the default.  enable = 0 selects the two-kernel path (reset kernel, then the beam
+ * kernel over the list), which is also what runs when the fused kernel is not possible.  Both paths give
+ * bit-identical states, goal observations and ranges.  *active_out (may be NULL) = 1 if the fused kernel
+ * will be used.  Host-side switch, takes effect at the next fn_reset (a captured CUDA graph keeps the choice
+ * made at capture).  Errors: FN_ERR_INVALID_ARG (NULL sim). */
+int fn_sim_set_fused_reset(fn_sim* sim, int enable, int* active_out);
+
 /* ---- end-to-end convenience: host buffers in, host buffers out -----------------------------------------
  * Copies states/actions/mask (and seeds) host->device, runs fn_step (+ fn_reset of the done envs when
  * seeds_host != NULL), copies states, ranges, collision, goal obs and the done mask back, synchronises.

@@ -16,6 +16,7 @@
 #include "fn_env.cuh"
 #include "fn_features.cuh"
 #include "fn_fixed_step.cuh"
+#include "fn_reset_beam.cuh"
 
 using namespace fn;
 
@@ -96,6 +97,10 @@ struct fn_sim {
     bool use_smem;
     size_t beam_smem;
     int beam_grid;
+    // fn_reset as one fused kernel (fn_reset_beam.cuh): possible / enabled, its shared bytes and grid
+    bool fused_ok, fused_on;
+    size_t fused_smem;
+    int fused_grid;
     // live timing
     int prof;
     std::vector<cudaEvent_t>* ev;    // triples per fn_step (e0 env e1 beam e2), pairs per fn_reset
@@ -416,6 +421,19 @@ extern "C" int fn_sim_create(const fn_map* map, const fn_robot* robot, int n, co
         if (bps2 < bps) bps = bps2;
         if (bps < 1) bps = 1;
         s->beam_grid = s->num_sms * bps;
+        // the fused reset + beam kernel: the beam kernel's shared memory plus the reset warps' scratch
+        s->fused_ok = s->fused_on = false;
+        s->fused_smem = fused_smem_bytes(robot->B, (int)map->n_words, robot->V);
+        s->fused_grid = 0;
+        if (e == cudaSuccess && s->use_smem && s->fused_smem <= (size_t)max_optin) {
+            int f0 = 0, f1 = 0;
+            e = cudaFuncSetAttribute(reset_beam_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s->fused_smem);
+            if (e == cudaSuccess) e = cudaFuncSetAttribute(reset_beam_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s->fused_smem);
+            if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&f0, reset_beam_kernel<false>, kFusedThreads, s->fused_smem);
+            if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&f1, reset_beam_kernel<true>, kFusedThreads, s->fused_smem);
+            if (f1 < f0) f0 = f1;
+            if (e == cudaSuccess && f0 >= 1) { s->fused_ok = s->fused_on = true; s->fused_grid = s->num_sms * f0; }
+        }
     }
     if (e != cudaSuccess) {
         int code = e == cudaErrorMemoryAllocation ? FN_ERR_OOM : FN_ERR_CUDA;
@@ -459,7 +477,7 @@ extern "C" int fn_sim_set_stream(fn_sim* s, void* stream) {
 
 static int ring_row_floats(const fn_sim* s) { return s->robot->B + 5 + (s->robot->drive == FN_DRIVE_DIFF ? 2 : 3) + 2; }
 
-static int launch_beams(fn_sim* s, const int* list, const int* count_dev, float* out_ranges, bool step_launch = false, bool done_list = false) {
+static BeamArgs beam_args(fn_sim* s, const int* list, const int* count_dev, float* out_ranges, bool step_launch, bool done_list) {
     BeamArgs b;
     b.map = s->map->dev; b.robot = robot_dev(s->robot, s->map); b.poses = s->d_poses; b.count_words = s->count_words;
     b.list = list; b.count_dev = count_dev; b.n_all = s->n; b.out_ranges = out_ranges; b.out_hit = s->aux_hit;
@@ -469,6 +487,11 @@ static int launch_beams(fn_sim* s, const int* list, const int* count_dev, float*
     b.list_par_dev = done_list ? s->d_done_count + 2 : nullptr;
     b.pair_lines = (double)s->robot->rmax / (double)s->map->res >= 110.0;     // beams of >~ 16 lines on average
     b.inv_bitsR = 1.0f / (float)(32 * s->map->dev.strideR); b.inv_bitsC = 1.0f / (float)(32 * s->map->dev.strideC);
+    return b;
+}
+
+static int launch_beams(fn_sim* s, const int* list, const int* count_dev, float* out_ranges, bool step_launch = false, bool done_list = false) {
+    const BeamArgs b = beam_args(s, list, count_dev, out_ranges, step_launch, done_list);
     const bool aux = s->count_words || s->aux_hit;
     const dim3 grid(s->beam_grid), block(512);
     if (s->use_smem) {
@@ -561,12 +584,26 @@ extern "C" int fn_reset(fn_sim* s, float* states, const uint8_t* mask, const uin
     a.d_prev = s->d_dprev; a.ep_step = s->d_epstep; a.poses = s->d_poses;
     a.ring = s->ring; a.ring_cap = s->ring_cap ? s->ring_cap : 1; a.ring_head_dev = s->d_ring_head; a.ring_row = ring_row_floats(s);
     a.counters = s->d_counters; a.beam_task_counter = s->d_task_counter;
-    int grid = (s->n + kResetWarps - 1) / kResetWarps;
-    if (grid > s->num_sms * 4) grid = s->num_sms * 4;
-    FN_CUDA(launch_pdl(reset_kernel, dim3(grid), dim3(kResetWarps * 32), kResetWarps * col_scratch_bytes(s->robot->V), s->stream, a));
-    if (s->prof) FN_CUDA(cudaEventRecord(e2, s->stream));
-    int rc = launch_beams(s, list, count, out_ranges, false, mask == nullptr);
-    if (s->prof && rc == FN_OK) FN_CUDA(cudaEventRecord(e3, s->stream));
+    int rc = FN_OK;
+    // (a CTA of the fused kernel runs its resets on kFusedResetWarps warps and its beams on all of them: made
+    // for the usual few resets per step; a long list -- all envs -- costs about as much as the two kernels)
+    const bool fused = s->fused_on;
+    if (fused) {
+        // one launch: every CTA resets its share of the list from its shared copy of the map, then casts
+        // the beams of those envs (fn_reset_beam.cuh)
+        BeamArgs b = beam_args(s, list, count, out_ranges, false, mask == nullptr);
+        const bool aux = s->count_words || s->aux_hit;
+        if (aux) FN_CUDA(launch_pdl(reset_beam_kernel<true>, dim3(s->fused_grid), dim3(kFusedThreads), s->fused_smem, s->stream, a, b));
+        else FN_CUDA(launch_pdl(reset_beam_kernel<false>, dim3(s->fused_grid), dim3(kFusedThreads), s->fused_smem, s->stream, a, b));
+        if (s->prof) { FN_CUDA(cudaEventRecord(e2, s->stream)); FN_CUDA(cudaEventRecord(e3, s->stream)); }
+    } else {
+        int grid = (s->n + kResetWarps - 1) / kResetWarps;
+        if (grid > s->num_sms * 4) grid = s->num_sms * 4;
+        FN_CUDA(launch_pdl(reset_kernel, dim3(grid), dim3(kResetWarps * 32), kResetWarps * col_scratch_bytes(s->robot->V), s->stream, a));
+        if (s->prof) FN_CUDA(cudaEventRecord(e2, s->stream));
+        rc = launch_beams(s, list, count, out_ranges, false, mask == nullptr);
+        if (s->prof && rc == FN_OK) FN_CUDA(cudaEventRecord(e3, s->stream));
+    }
     if (rc == FN_OK) rc = launch_features(s, list, count, mask == nullptr, out_ranges);
     return rc;
 }
@@ -729,6 +766,13 @@ extern "C" int fn_sim_profile_read(fn_sim* s, double* ms_out, uint64_t* launches
 extern "C" int fn_sim_beam_config(const fn_sim* s, int* cfg) {
     if (!s || !cfg) return fail(FN_ERR_INVALID_ARG, "fn_sim_beam_config: NULL argument");
     cfg[0] = s->use_smem ? 1 : 0; cfg[1] = s->beam_grid; cfg[2] = 512; cfg[3] = (int)s->beam_smem;
+    return FN_OK;
+}
+
+extern "C" int fn_sim_set_fused_reset(fn_sim* s, int enable, int* active_out) {
+    if (!s) return fail(FN_ERR_INVALID_ARG, "fn_sim_set_fused_reset: NULL sim");
+    s->fused_on = enable != 0 && s->fused_ok;
+    if (active_out) *active_out = s->fused_on ? 1 : 0;
     return FN_OK;
 }
 

@@ -111,10 +111,17 @@ __device__ __forceinline__ double wrap_pi(double a) {
     return r;
 }
 
-// occupancy of cell (i, j) from the row-packed copy in global memory; outside the map = occupied
+// One word of the packed map.  kS = false: the copy in global memory (read-only path).  kS = true: m.row
+// points at a copy staged in shared memory (the fused reset + beam kernel), read with a generic load.
+template <bool kS = false>
+__device__ __forceinline__ uint32_t map_word(const uint32_t* p) {
+    if constexpr (kS) return *p; else return __ldg(p);
+}
+// occupancy of cell (i, j) from the row-packed copy; outside the map = occupied
+template <bool kS = false>
 __device__ __forceinline__ bool occ_global(const MapDev& m, int i, int j) {
     if ((unsigned)i >= (unsigned)m.H || (unsigned)j >= (unsigned)m.W) return true;
-    uint32_t w = __ldg(m.row + (size_t)(i + kLineGuard) * m.strideR + ((j + kCellShift) >> 5));
+    uint32_t w = map_word<kS>(m.row + (size_t)(i + kLineGuard) * m.strideR + ((j + kCellShift) >> 5));
     return (w >> (j & 31)) & 1u;
 }
 

@@ -31,10 +31,11 @@ struct Window {
 };                           //     non-finite), 2 = occupied cells in the window: exact test needed
 
 // occupancy bits of row i, columns jb .. jb+31 (bit b = cell jb + b), from the row-packed copy
+template <bool kS = false>
 __device__ __forceinline__ uint32_t row_bits(const uint32_t* __restrict__ row, int strideR, int i, int jb) {
     const int q = jb + kCellShift;
     const uint32_t* p = row + (size_t)(i + kLineGuard) * strideR + (q >> 5);
-    return __funnelshift_r(__ldg(p), __ldg(p + 1), q);
+    return __funnelshift_r(map_word<kS>(p), map_word<kS>(p + 1), q);
 }
 __device__ __forceinline__ uint32_t low_bits(int n) {           // n in [0, 32] -> n low bits set
     return n >= 32 ? 0xffffffffu : ((1u << n) - 1u);
@@ -42,6 +43,7 @@ __device__ __forceinline__ uint32_t low_bits(int n) {           // n in [0, 32] 
 
 // stage 1, one thread per pose.  verts = the footprint vertices (a shared-memory copy in the kernels).
 // The window rows are read eight at a time so that their (independent, mostly L2-latency) loads overlap.
+template <bool kS = false>
 __device__ __forceinline__ Window footprint_window(const MapDev& m, const double2* __restrict__ verts, const int V,
                                                    double x, double y, double c, double s) {
     const double inv = m.inv_rho;
@@ -65,7 +67,7 @@ __device__ __forceinline__ Window footprint_window(const MapDev& m, const double
         for (int i = w.i0; i <= w.i1; i += 8) {
             uint32_t v[8];
 #pragma unroll
-            for (int u = 0; u < 8; ++u) v[u] = row_bits(m.row, m.strideR, min(i + u, w.i1), jb);
+            for (int u = 0; u < 8; ++u) v[u] = row_bits<kS>(m.row, m.strideR, min(i + u, w.i1), jb);
 #pragma unroll
             for (int u = 0; u < 8; ++u) any |= v[u];
         }
@@ -106,6 +108,7 @@ __device__ __forceinline__ ColScratch col_scratch(uint8_t* base, int V) {
 
 // All 32 lanes must call; `need` = this lane's pose needs the exact test (window status 2).
 // Returns true for a lane whose polygon meets an occupied cell (false for lanes that did not need it).
+template <bool kS = false>
 __device__ __noinline__ bool warp_collisions_exact(const uint32_t* __restrict__ row, const int strideR,
                                                    const double2* __restrict__ verts, const int* __restrict__ nxt, const int V,
                                                    const double inv, const bool need, const double x, const double y,
@@ -157,7 +160,7 @@ __device__ __noinline__ bool warp_collisions_exact(const uint32_t* __restrict__ 
             const double ylo_s = (double)i, yhi_s = ylo_s + 1.0, yc = ylo_s + 0.5;
             bool found = false;
             for (int jb = sj0; jb <= sj1 && !found; jb += 32) {
-                const uint32_t occ = row_bits(row, strideR, i, jb) & low_bits(sj1 - jb + 1);
+                const uint32_t occ = row_bits<kS>(row, strideR, i, jb) & low_bits(sj1 - jb + 1);
                 if (occ == 0u) continue;
                 // a footprint may be a union of polygons: the edges of a component are
                 // consecutive and close on themselves (nxt[k] <= k at its last vertex); the cells inside
@@ -194,12 +197,13 @@ __device__ __noinline__ bool warp_collisions_exact(const uint32_t* __restrict__ 
 }
 
 // Per-lane collision flag from the window status (all 32 lanes must call).
+template <bool kS = false>
 __device__ __forceinline__ bool resolve_collisions(const MapDev& m, const RobotDev& rb, const Window& w,
                                                    double x, double y, double c, double s, const ColScratch cs) {
     const bool need = w.status == 2;
     bool col = w.status == 1;
     if (__any_sync(0xffffffffu, need))
-        col |= warp_collisions_exact(m.row, m.strideR, cs.verts, cs.nxt, rb.V, m.inv_rho, need, x, y, c, s,
+        col |= warp_collisions_exact<kS>(m.row, m.strideR, cs.verts, cs.nxt, rb.V, m.inv_rho, need, x, y, c, s,
                                      w.i0, w.i1, w.j0, w.j1, cs);
     return col;
 }
@@ -208,8 +212,9 @@ __device__ __forceinline__ bool resolve_collisions(const MapDev& m, const RobotD
 // BeamPose (fn_common.cuh): sensor origin in cells and, for both choices of the dominant axis, the
 // origin's fixed-point coordinate, the offset to the first line boundary and the address of the
 // origin's line.
-__device__ __forceinline__ void write_pose(const MapDev& m, const RobotDev& rb, BeamPose* out,
-                                           float xf, float yf, float psif, double c, double s) {
+template <bool kS = false>
+__device__ __forceinline__ BeamPose make_pose(const MapDev& m, const RobotDev& rb,
+                                              float xf, float yf, float psif, double c, double s) {
     const double ox = ((double)xf + c * rb.sx - s * rb.sy) * m.inv_rho;
     const double oy = ((double)yf + s * rb.sx + c * rb.sy) * m.inv_rho;
     BeamPose p;
@@ -218,7 +223,7 @@ __device__ __forceinline__ void write_pose(const MapDev& m, const RobotDev& rb, 
     p.pad_[0] = p.pad_[1] = 0;
     const bool in = ox >= 0.0 && ox < (double)m.W && oy >= 0.0 && oy < (double)m.H;   // false for NaN
     const int jx = in ? __double2int_rd(ox) : 0, iy = in ? __double2int_rd(oy) : 0;
-    p.state = !in ? 2 : (occ_global(m, iy, jx) ? 1 : 0);
+    p.state = !in ? 2 : (occ_global<kS>(m, iy, jx) ? 1 : 0);
     const double fx = ox - (double)jx, fy = oy - (double)iy;
     const unsigned rowBytes = (unsigned)(m.H + 2 * kLineGuard) * (unsigned)m.strideR * 4u;
     p.o[0].ouM = ox + ((double)kCellShift + kMagic); p.o[0].h = 0.5 - fy; p.o[0].cu0 = jx;
@@ -227,7 +232,12 @@ __device__ __forceinline__ void write_pose(const MapDev& m, const RobotDev& rb, 
     p.o[1].line_off = rowBytes + (unsigned)(jx + kLineGuard) * (unsigned)m.strideC * 4u;
     p.o[0].ouMS = p.o[0].ouM + (double)(p.o[0].line_off << 3);
     p.o[1].ouMS = p.o[1].ouM + (double)((p.o[1].line_off - rowBytes) << 3);
-    *out = p;
+    return p;
+}
+template <bool kS = false>
+__device__ __forceinline__ void write_pose(const MapDev& m, const RobotDev& rb, BeamPose* out,
+                                           float xf, float yf, float psif, double c, double s) {
+    *out = make_pose<kS>(m, rb, xf, yf, psif, c, s);
 }
 
 // ---------------------------------------------------------------- S1 + S3 + S4: the env step
@@ -515,6 +525,107 @@ struct ResetArgs {
 
 constexpr int kResetWarps = 4;
 
+// Reset of env e by one warp (all 32 lanes call).  m = the packed map to read: a.map (kS = false) or the
+// same map with row / col pointing at a shared-memory copy (kS = true, fused kernel in fn_beam.cuh).
+template <bool kS>
+__device__ __forceinline__ void reset_env(const ResetArgs& a, const MapDev& mp, const ColScratch& scratch,
+                                          const int e, const int lane, BeamPose* pose_copy = nullptr) {
+    const int n = a.n;
+    const double rho = (double)mp.rho;
+    const float two_pi_f = 6.28318530717958647692f, pi_f = 3.14159265358979323846f;
+    const float dmin2 = __fmul_rn(a.task.dmin, a.task.dmin), dmax2 = __fmul_rn(a.task.dmax, a.task.dmax);
+    int r0 = 0, c0 = 0, rh = mp.H, cw = mp.W;
+    if (a.regions.n > 0) { const int4 R = a.regions.rects[e % a.regions.n]; r0 = R.x; c0 = R.y; rh = R.z; cw = R.w; }
+    const float X0 = (float)((double)c0 * rho), Xe = (float)((double)cw * rho);
+    const float Y0 = (float)((double)r0 * rho), Ye = (float)((double)rh * rho);
+    const unsigned long long sigma = a.seeds[e];
+    // ---- start pose: attempts k = 0..255, 32 at a time
+    float x = 0.f, y = 0.f, psi = 0.f;
+    double sp = 0.0, cp = 1.0;
+    bool ok = false;
+    for (int chunk = 0; chunk < kMaxAttempts / 32 && !ok; ++chunk) {
+        const unsigned long long k = (unsigned long long)(chunk * 32 + lane);
+        const float xk = __fmaf_rn(u24_at(sigma, 3ull * k), Xe, X0);
+        const float yk = __fmaf_rn(u24_at(sigma, 3ull * k + 1ull), Ye, Y0);
+        const float pk = __fmaf_rn(u24_at(sigma, 3ull * k + 2ull), two_pi_f, -pi_f);
+        double sk, ck;
+        sincos((double)pk, &sk, &ck);
+        Window w = footprint_window<kS>(mp, scratch.verts, a.robot.V, (double)xk, (double)yk, ck, sk);
+        // attempts after the first one that is free without any further test cannot win: skip their tests
+        const unsigned free_m = __ballot_sync(0xffffffffu, w.status == 0);
+        if (free_m && lane > __ffs(free_m) - 1) w.status = 1;
+        // One-sided pre-test: a point inside the footprint whose cell is occupied proves a collision.
+        // Most random start poses that collide do so deeply, so few attempts need the exact test.
+        if (w.status == 2) {
+            bool hit = false;
+            for (int q = 0; q < a.robot.n_samples && !hit; q += 4) {
+                bool h4 = false;
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const double2 f = a.robot.samples[min(q + u, a.robot.n_samples - 1)];
+                    const int j = __double2int_rd(((double)xk + ck * f.x - sk * f.y) * mp.inv_rho);
+                    const int i = __double2int_rd(((double)yk + sk * f.x + ck * f.y) * mp.inv_rho);
+                    h4 |= occ_global<kS>(mp, i, j);
+                }
+                hit = h4;
+            }
+            if (hit) w.status = 1;
+        }
+        const bool col = resolve_collisions<kS>(mp, a.robot, w, (double)xk, (double)yk, ck, sk, scratch);
+        const unsigned acc_m = __ballot_sync(0xffffffffu, !col);
+        ok = acc_m != 0u;
+        const int src = ok ? __ffs(acc_m) - 1 : 31;           // exhausted: keep the last candidate
+        x = __shfl_sync(0xffffffffu, xk, src); y = __shfl_sync(0xffffffffu, yk, src);
+        psi = __shfl_sync(0xffffffffu, pk, src);
+        sp = __shfl_sync(0xffffffffu, sk, src); cp = __shfl_sync(0xffffffffu, ck, src);
+    }
+    bool fail = !ok;
+    // ---- goal: attempts m = 0..255, 32 at a time
+    float gx = x, gy = y;
+    ok = false;
+    for (int chunk = 0; chunk < kMaxAttempts / 32 && !ok; ++chunk) {
+        const unsigned long long m = (unsigned long long)(chunk * 32 + lane);
+        const float ua = __fmaf_rn(2.0f, u24_at(sigma, 768ull + 2ull * m), -1.0f);
+        const float ub = __fmaf_rn(2.0f, u24_at(sigma, 768ull + 2ull * m + 1ull), -1.0f);
+        const float gxm = __fmaf_rn(ua, a.task.dmax, x);
+        const float gym = __fmaf_rn(ub, a.task.dmax, y);
+        const float ddx = __fsub_rn(gxm, x), ddy = __fsub_rn(gym, y);
+        const float d2 = __fadd_rn(__fmul_rn(ddx, ddx), __fmul_rn(ddy, ddy));
+        bool okm = d2 >= dmin2 && d2 <= dmax2;
+        if (okm) {
+            const int j = __double2int_rd((double)gxm / rho), i = __double2int_rd((double)gym / rho);
+            okm = i >= r0 && j >= c0 && i < r0 + rh && j < c0 + cw && !occ_global<kS>(mp, i, j);
+        }
+        const unsigned okb = __ballot_sync(0xffffffffu, okm);
+        ok = okb != 0u;
+        const int src = ok ? __ffs(okb) - 1 : 31;
+        gx = __shfl_sync(0xffffffffu, gxm, src); gy = __shfl_sync(0xffffffffu, gym, src);
+    }
+    fail = fail || !ok;
+    if (lane == 0) {
+        const double gdx = (double)gx - (double)x, gdy = (double)gy - (double)y;
+        const float d = (float)sqrt(gdx * gdx + gdy * gdy);
+        const float alpha = (float)wrap_pi(atan2(gdy, gdx) - (double)psi);
+        a.states[0 * n + e] = x; a.states[1 * n + e] = y; a.states[2 * n + e] = psi;
+        a.states[3 * n + e] = 0.f; a.states[4 * n + e] = 0.f; a.states[5 * n + e] = 0.f;
+        a.states[6 * n + e] = gx; a.states[7 * n + e] = gy;
+        a.d_prev[e] = d;
+        a.ep_step[e] = 0;
+        if (a.out_goal_obs) { a.out_goal_obs[e] = d; a.out_goal_obs[n + e] = alpha; }
+        const BeamPose bp = make_pose<kS>(mp, a.robot, x, y, psi, cp, sp);
+        a.poses[e] = bp;
+        if (pose_copy) *pose_copy = bp;                            // (fused kernel: a copy in shared memory)
+        if (a.ring) {
+            const unsigned long long head = *a.ring_head_dev;
+            float* row = a.ring + ((head + (unsigned long long)e) % a.ring_cap) * (size_t)a.ring_row;
+            const int B = a.robot.B;
+            row[B] = d; row[B + 1] = alpha; row[B + 2] = 0.f; row[B + 3] = 0.f; row[B + 4] = 0.f;
+        }
+        atomicAdd(&a.counters[kResets], 1ull);
+        if (fail) atomicAdd(&a.counters[kResetFail], 1ull);
+    }
+}
+
 __global__ void __launch_bounds__(kResetWarps * 32) reset_kernel(ResetArgs a) {
     extern __shared__ __align__(16) uint8_t s_dyn[];
     const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -524,103 +635,10 @@ __global__ void __launch_bounds__(kResetWarps * 32) reset_kernel(ResetArgs a) {
     griddep_wait();                                                // the list comes from the compaction kernel
     griddep_launch_dependents();
     if (blockIdx.x == 0 && threadIdx.x == 0) *a.beam_task_counter = 0u;
-    const int n = a.n;
-    if (a.list_par_dev) { const int q = *a.list_par_dev ^ 1; a.list += (size_t)q * n; a.count_dev += q; }
+    if (a.list_par_dev) { const int q = *a.list_par_dev ^ 1; a.list += (size_t)q * a.n; a.count_dev += q; }
     const int count = *a.count_dev;
-    const double rho = (double)a.map.rho;
-    const float two_pi_f = 6.28318530717958647692f, pi_f = 3.14159265358979323846f;
-    const float dmin2 = __fmul_rn(a.task.dmin, a.task.dmin), dmax2 = __fmul_rn(a.task.dmax, a.task.dmax);
-    for (int li = blockIdx.x * kResetWarps + wib; li < count; li += gridDim.x * kResetWarps) {
-        const int e = a.list[li];
-        int r0 = 0, c0 = 0, rh = a.map.H, cw = a.map.W;
-        if (a.regions.n > 0) { const int4 R = a.regions.rects[e % a.regions.n]; r0 = R.x; c0 = R.y; rh = R.z; cw = R.w; }
-        const float X0 = (float)((double)c0 * rho), Xe = (float)((double)cw * rho);
-        const float Y0 = (float)((double)r0 * rho), Ye = (float)((double)rh * rho);
-        const unsigned long long sigma = a.seeds[e];
-        // ---- start pose: attempts k = 0..255, 32 at a time
-        float x = 0.f, y = 0.f, psi = 0.f;
-        double sp = 0.0, cp = 1.0;
-        bool ok = false;
-        for (int chunk = 0; chunk < kMaxAttempts / 32 && !ok; ++chunk) {
-            const unsigned long long k = (unsigned long long)(chunk * 32 + lane);
-            const float xk = __fmaf_rn(u24_at(sigma, 3ull * k), Xe, X0);
-            const float yk = __fmaf_rn(u24_at(sigma, 3ull * k + 1ull), Ye, Y0);
-            const float pk = __fmaf_rn(u24_at(sigma, 3ull * k + 2ull), two_pi_f, -pi_f);
-            double sk, ck;
-            sincos((double)pk, &sk, &ck);
-            Window w = footprint_window(a.map, scratch.verts, a.robot.V, (double)xk, (double)yk, ck, sk);
-            // One-sided pre-test: a point inside the footprint whose cell is occupied proves a collision.
-            // Most random start poses that collide do so deeply, so few attempts need the exact test.
-            if (w.status == 2) {
-                bool hit = false;
-                for (int q = 0; q < a.robot.n_samples && !hit; q += 4) {
-                    bool h4 = false;
-#pragma unroll
-                    for (int u = 0; u < 4; ++u) {
-                        const double2 f = a.robot.samples[min(q + u, a.robot.n_samples - 1)];
-                        const int j = __double2int_rd(((double)xk + ck * f.x - sk * f.y) * a.map.inv_rho);
-                        const int i = __double2int_rd(((double)yk + sk * f.x + ck * f.y) * a.map.inv_rho);
-                        h4 |= occ_global(a.map, i, j);
-                    }
-                    hit = h4;
-                }
-                if (hit) w.status = 1;
-            }
-            // attempts after the first one that is free without an exact test cannot win: skip their tests
-            const unsigned free_m = __ballot_sync(0xffffffffu, w.status == 0);
-            if (free_m && lane > __ffs(free_m) - 1) w.status = 1;
-            const bool col = resolve_collisions(a.map, a.robot, w, (double)xk, (double)yk, ck, sk, scratch);
-            const unsigned acc_m = __ballot_sync(0xffffffffu, !col);
-            ok = acc_m != 0u;
-            const int src = ok ? __ffs(acc_m) - 1 : 31;           // exhausted: keep the last candidate
-            x = __shfl_sync(0xffffffffu, xk, src); y = __shfl_sync(0xffffffffu, yk, src);
-            psi = __shfl_sync(0xffffffffu, pk, src);
-            sp = __shfl_sync(0xffffffffu, sk, src); cp = __shfl_sync(0xffffffffu, ck, src);
-        }
-        bool fail = !ok;
-        // ---- goal: attempts m = 0..255, 32 at a time
-        float gx = x, gy = y;
-        ok = false;
-        for (int chunk = 0; chunk < kMaxAttempts / 32 && !ok; ++chunk) {
-            const unsigned long long m = (unsigned long long)(chunk * 32 + lane);
-            const float ua = __fmaf_rn(2.0f, u24_at(sigma, 768ull + 2ull * m), -1.0f);
-            const float ub = __fmaf_rn(2.0f, u24_at(sigma, 768ull + 2ull * m + 1ull), -1.0f);
-            const float gxm = __fmaf_rn(ua, a.task.dmax, x);
-            const float gym = __fmaf_rn(ub, a.task.dmax, y);
-            const float ddx = __fsub_rn(gxm, x), ddy = __fsub_rn(gym, y);
-            const float d2 = __fadd_rn(__fmul_rn(ddx, ddx), __fmul_rn(ddy, ddy));
-            bool okm = d2 >= dmin2 && d2 <= dmax2;
-            if (okm) {
-                const int j = __double2int_rd((double)gxm / rho), i = __double2int_rd((double)gym / rho);
-                okm = i >= r0 && j >= c0 && i < r0 + rh && j < c0 + cw && !occ_global(a.map, i, j);
-            }
-            const unsigned okb = __ballot_sync(0xffffffffu, okm);
-            ok = okb != 0u;
-            const int src = ok ? __ffs(okb) - 1 : 31;
-            gx = __shfl_sync(0xffffffffu, gxm, src); gy = __shfl_sync(0xffffffffu, gym, src);
-        }
-        fail = fail || !ok;
-        if (lane == 0) {
-            const double gdx = (double)gx - (double)x, gdy = (double)gy - (double)y;
-            const float d = (float)sqrt(gdx * gdx + gdy * gdy);
-            const float alpha = (float)wrap_pi(atan2(gdy, gdx) - (double)psi);
-            a.states[0 * n + e] = x; a.states[1 * n + e] = y; a.states[2 * n + e] = psi;
-            a.states[3 * n + e] = 0.f; a.states[4 * n + e] = 0.f; a.states[5 * n + e] = 0.f;
-            a.states[6 * n + e] = gx; a.states[7 * n + e] = gy;
-            a.d_prev[e] = d;
-            a.ep_step[e] = 0;
-            if (a.out_goal_obs) { a.out_goal_obs[e] = d; a.out_goal_obs[n + e] = alpha; }
-            write_pose(a.map, a.robot, &a.poses[e], x, y, psi, cp, sp);
-            if (a.ring) {
-                const unsigned long long head = *a.ring_head_dev;
-                float* row = a.ring + ((head + (unsigned long long)e) % a.ring_cap) * (size_t)a.ring_row;
-                const int B = a.robot.B;
-                row[B] = d; row[B + 1] = alpha; row[B + 2] = 0.f; row[B + 3] = 0.f; row[B + 4] = 0.f;
-            }
-            atomicAdd(&a.counters[kResets], 1ull);
-            if (fail) atomicAdd(&a.counters[kResetFail], 1ull);
-        }
-    }
+    for (int li = blockIdx.x * kResetWarps + wib; li < count; li += gridDim.x * kResetWarps)
+        reset_env<false>(a, a.map, scratch, a.list[li], lane);
 }
 
 // ---------------------------------------------------------------- observe-all support: poses from states

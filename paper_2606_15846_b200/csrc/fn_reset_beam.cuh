@@ -1,0 +1,129 @@
+// fn_reset_beam.cuh -- S5 + S6 in ONE launch: reset of the listed envs and the recompute of their beams
+// ("resets ... recompute only the affected environments").
+//
+// As two kernels (reset_kernel, then beam_kernel over the list) the reset path of a step costs two launch
+// latencies and, in the reset kernel, a chain of dependent L2 reads of the map (32 start-pose attempts,
+// window rows, exact polygon test, goal attempts): ~30 us of a ~100 us step at 4096 envs although only
+// ~5 % of the envs are reset.  Here every CTA stages the packed map once (before the dependency wait,
+// like beam_kernel), owns the listed envs li = blockIdx.x + k * gridDim.x, resets them from the SHARED
+// copy of the map (reset_env<true>: the same code as reset_kernel, so the accepted poses are identical),
+// and then casts the beams of its own envs.  No CTA reads another CTA's poses, so a block barrier is the
+// only synchronisation.  Used when the map is staged in shared memory; otherwise fn_reset launches the
+// two kernels.
+#pragma once
+#include "fn_beam.cuh"
+#include "fn_env.cuh"
+
+namespace fn {
+
+constexpr int kFusedResetWarps = 2;      // warps of a CTA that run resets (each needs a ColScratch)
+constexpr int kFusedPoseSlots = 8;       // sensing poses of a CTA's first envs are kept in shared memory too
+constexpr int kFusedThreads = 512;       // two CTAs per SM like beam_kernel (one CTA of 1024 threads measured the same)
+
+__host__ __device__ inline size_t fused_scratch_offset(int B, int mapWords) {      // 32-byte aligned (BeamPose)
+    return (((size_t)B * sizeof(double2) + (size_t)mapWords * 4u) + 31u) & ~(size_t)31u;
+}
+__host__ __device__ inline size_t fused_smem_bytes(int B, int mapWords, int V) {
+    return fused_scratch_offset(B, mapWords) + kFusedPoseSlots * sizeof(BeamPose) + kFusedResetWarps * col_scratch_bytes(V);
+}
+
+template <bool kAux>
+__global__ void __launch_bounds__(kFusedThreads, 2) reset_beam_kernel(ResetArgs ra, BeamArgs a) {
+    extern __shared__ __align__(16) uint8_t smem_raw[];
+    const int B = a.robot.B, V = a.robot.V;
+    const int rowWords = (a.map.H + 2 * kLineGuard) * a.map.strideR;
+    const int mapWords = rowWords + (a.map.W + 2 * kLineGuard) * a.map.strideC;
+    double2* s_tab = reinterpret_cast<double2*>(smem_raw);
+    uint32_t* s_map = reinterpret_cast<uint32_t*>(smem_raw + (size_t)B * sizeof(double2));
+    BeamPose* s_pose = reinterpret_cast<BeamPose*>(smem_raw + fused_scratch_offset(B, mapWords));
+    uint8_t* s_scr = reinterpret_cast<uint8_t*>(s_pose + kFusedPoseSlots);
+    const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    for (int i = threadIdx.x; i < B; i += blockDim.x) s_tab[i] = a.robot.beam_cs[i];
+    {
+        const uint4* src = reinterpret_cast<const uint4*>(a.map.row);      // row and col copies are contiguous
+        uint4* dst = reinterpret_cast<uint4*>(s_map);
+        const int n4 = (mapWords + 3) / 4;
+        int i = threadIdx.x;
+        for (; i + 3 * (int)blockDim.x < n4; i += 4 * blockDim.x) {
+            const uint4 v0 = __ldg(src + i), v1 = __ldg(src + i + blockDim.x);
+            const uint4 v2 = __ldg(src + i + 2 * blockDim.x), v3 = __ldg(src + i + 3 * blockDim.x);
+            dst[i] = v0; dst[i + blockDim.x] = v1; dst[i + 2 * blockDim.x] = v2; dst[i + 3 * blockDim.x] = v3;
+        }
+        for (; i < n4; i += blockDim.x) dst[i] = __ldg(src + i);
+    }
+    ColScratch scratch = col_scratch(s_scr + (size_t)(wib < kFusedResetWarps ? wib : 0) * col_scratch_bytes(V), V);
+    if (wib < kFusedResetWarps)
+        for (int k = lane; k < V; k += 32) { scratch.verts[k] = a.robot.verts[k]; scratch.nxt[k] = a.robot.nxt[k]; }
+    __syncthreads();
+    griddep_wait();                                                // the list comes from the kernel before
+    griddep_launch_dependents();
+    if (ra.list_par_dev) { const int q = *ra.list_par_dev ^ 1; ra.list += (size_t)q * ra.n; ra.count_dev += q; }
+    const int count = *ra.count_dev;
+    // this CTA's envs: list entries blockIdx.x, blockIdx.x + gridDim.x, ...
+    const int m_loc = count > (int)blockIdx.x ? (count - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x : 0;
+    if (m_loc == 0) return;                                        // (uniform over the CTA)
+
+    // ---- phase 1: resets, from the shared copy of the map
+    if (wib < kFusedResetWarps) {
+        MapDev ms = ra.map;
+        ms.row = s_map;
+        ms.col = s_map + rowWords;
+        for (int k = wib; k < m_loc; k += kFusedResetWarps)
+            reset_env<true>(ra, ms, scratch, ra.list[blockIdx.x + k * gridDim.x], lane, k < kFusedPoseSlots ? s_pose + k : nullptr);
+        __threadfence_block();                                     // poses: written here, read below by all warps
+    }
+    __syncthreads();
+
+    // ---- phase 2: the beams of this CTA's envs, 32 consecutive (env, beam) pairs per warp task
+    SmemGeo geo;
+    geo.rho = a.map.rho; geo.bitsR = a.map.strideR << 5; geo.bitsC = a.map.strideC << 5;
+    geo.inv_bitsR = a.inv_bitsR; geo.inv_bitsC = a.inv_bitsC;
+    BeamMap<SmemSpace> bm;
+    bm.base = (uint32_t)__cvta_generic_to_shared(s_map);
+    bm.H = a.map.H; bm.W = a.map.W; bm.stride4R = a.map.strideR << 2; bm.stride4C = a.map.strideC << 2;
+    bm.rowBytes = (unsigned)rowWords * 4u; bm.mapBytes = (unsigned)mapWords * 4u; bm.oob = a.counters + kOobLoads;
+    geo.baseR = bm.base - kExpOff; geo.baseC = geo.baseR + bm.rowBytes;
+    const unsigned long long ring_head = a.ring_obs ? *a.ring_head : 0ull;
+    const unsigned total = (unsigned)m_loc * (unsigned)B;
+    const unsigned ntasks = (total + 31u) >> 5;
+    const unsigned long long invB = ~0ull / (unsigned long long)B + 1ull;     // floor(2^64 / B) + 1
+    uint32_t words = 0, rays = 0;
+    for (unsigned task = (unsigned)wib; task < ntasks; task += blockDim.x >> 5) {
+        const unsigned idx = (task << 5) + lane;
+        const unsigned k = (unsigned)__umul64hi((unsigned long long)idx, invB);      // idx / B
+        const unsigned j = idx - k * (unsigned)B;
+        if (k < (unsigned)m_loc) {
+            const unsigned e = (unsigned)ra.list[blockIdx.x + k * gridDim.x];
+                        const BeamPose* pose = k < (unsigned)kFusedPoseSlots ? s_pose + k : a.poses + e;
+            const int state = pose->state;
+            float r = 0.0f;
+            int hit = -2;
+            if (state == 0) {
+                if constexpr (!kAux) r = cast_beam_smem(bm, geo, pose, s_tab[j], a.robot.T, a.robot.rmax);
+                else r = cast_beam<SmemSpace, true>(bm, pose, s_tab[j], a.robot.T, a.map.rho, a.robot.rmax, &hit, words, false);
+            } else if (kAux) {
+                if (state == 1) hit = origin_line(bm, pose->o[0], true) * a.map.W + pose->o[0].cu0;
+                ++words;
+            }
+            const unsigned o = e * (unsigned)B + j;
+            a.out_ranges[o] = r;
+            if (kAux && a.out_hit) a.out_hit[o] = hit;
+            if (a.ring_obs) {
+                unsigned long long slot = ring_head + (unsigned long long)e;   // both < ring_cap
+                if (slot >= a.ring_cap) slot -= a.ring_cap;
+                a.ring_obs[slot * a.ring_row + j] = r;
+            }
+            ++rays;
+        }
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+        rays += __shfl_xor_sync(0xffffffffu, rays, o);
+        if (kAux) words += __shfl_xor_sync(0xffffffffu, words, o);
+    }
+    if (lane == 0 && rays) {
+        atomicAdd(&a.counters[kRays], (unsigned long long)rays);
+        if (kAux && a.count_words) atomicAdd(&a.counters[kWords], (unsigned long long)words);
+    }
+}
+
+}  // namespace fn

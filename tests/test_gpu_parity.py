@@ -276,6 +276,58 @@ def test_reset_of_the_steps_done_list_equals_masked_reset(pu):
     assert out[0][3] == out[1][3] > n and out[0][4] == out[1][4]
 
 
+def test_fused_reset_kernel_equals_the_two_kernel_path(pu):
+    # fn_reset runs ONE kernel when the map is staged in shared memory (each CTA resets its share of the list
+    # from its shared copy of the map, then recomputes those envs' beams) and two kernels otherwise: same
+    # states, goal observations, ranges, ring rows and counters, bit for bit -- for the step's done list, for
+    # a mask, for an all-env reset (several envs per CTA), an empty list, and with the instrumented kernels.
+    import torch
+    from harness import workloads as W
+    for cfg, n, ring_cap, aux in ((2, 1500, 0, False), (3, 777, 0, False), (1, 64, 0, True), (2, 9000, 0, False), (1, 300, 1024, False)):
+        wl = W.make_workload(cfg, n_envs=n)
+        B, A = wl.n_beams, wl.action_dim
+        steps = 6
+        actions = torch.from_numpy(W.action_tape(wl, steps, 5)).cuda()
+        seeds = torch.from_numpy(W.seed_tape(wl, steps + 2, 5).view(np.int64)).cuda()
+        forced = torch.from_numpy((np.random.default_rng(5).random((steps, n)) < 0.03).astype(np.uint8)).cuda()
+        out = []
+        for fused in (True, False):
+            m, r, s = pu.make_sim(wl, n)
+            assert s.beam_config()["smem"]
+            assert s.set_fused_reset(fused) == fused
+            buf = pu.Buffers(n, B, A)
+            hit = torch.full((n, B), -9, dtype=torch.int32, device="cuda")
+            rew = torch.zeros(n, device="cuda")
+            if aux:
+                s.bind_aux(hit, rew)
+            ring = None
+            if ring_cap:
+                row = B + 5 + A + 2
+                ring = torch.zeros(ring_cap * row, device="cuda")
+                s.ring_attach(ring, ring_cap)
+            buf.mask.fill_(1)
+            s.reset(buf.states, buf.mask, seeds[0], buf.ranges, buf.gobs)          # all envs: several per CTA
+            snap = [buf.states.clone(), buf.ranges.clone()]
+            buf.mask.zero_()
+            s.reset(buf.states, buf.mask, seeds[1], buf.ranges, buf.gobs)          # empty list: nothing changes
+            assert torch.equal(snap[0], buf.states) and torch.equal(snap[1], buf.ranges)
+            for t in range(steps):
+                buf.mask.copy_(forced[t])
+                s.step(buf.states, actions[t], float(wl.dt), buf.mask, buf.ranges, buf.col, buf.gobs)
+                s.reset(buf.states, None if t % 2 == 0 else buf.mask, seeds[t + 2], buf.ranges, buf.gobs)
+            torch.cuda.synchronize()
+            c = s.counters()
+            assert c["oob_window_loads"] == 0
+            out.append((buf.states.clone(), buf.ranges.clone(), buf.gobs.clone(), hit.clone(),
+                        None if ring is None else ring.clone(), c["envs_reset"], c["rays_cast"], c["reset_failures"]))
+            s.close(); r.close(); m.close()
+        for a, b in zip(out[0][:4], out[1][:4]):
+            assert torch.equal(a, b)
+        if ring_cap:
+            assert torch.equal(out[0][4], out[1][4])
+        assert out[0][5:] == out[1][5:] and out[0][5] > n
+
+
 def test_clearance_features_against_the_oracle(pu):
     # NEXT-1 (Eq. (3)): sector-pooled footprint clearances.  Teacher-forced:
     # the oracle computes them in fp64 from the GPU's own fp32 ranges; tolerance 1e-4 m like the ranges

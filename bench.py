@@ -31,8 +31,8 @@ sys.path.insert(0, ROOT)
 from harness import workloads as W  # noqa: E402
 
 # dominant kernel (full-batch beam launch), per launch, from the committed ncu --set full capture
-NCU_CAPTURE = {2: {"dram_bytes": 506880, "warp_inst": 45733853, "lanes": 22.05,
-                   "source": "profiles/r1d_beam_kernel_full_c2.txt (dram__bytes_read.sum + dram__bytes_write.sum)"}}
+NCU_CAPTURE = {2: {"dram_bytes": 506624, "warp_inst": 45733853, "lanes": 22.05,
+                   "source": "profiles/r1e_beam_kernels_full_c2.txt (dram__bytes_read.sum + dram__bytes_write.sum)"}}
 
 METRIC = "env_steps_per_s"
 UNIT = "env-steps/s"

@@ -209,7 +209,9 @@ int fn_sim_set_fused_reset(fn_sim* sim, int enable, int* active_out);
 /* ---- end-to-end convenience: host buffers in, host buffers out -----------------------------------------
  * Copies states/actions/mask (and seeds) host->device, runs fn_step (+ fn_reset of the done envs when
  * seeds_host != NULL), copies states, ranges, collision, goal obs and the done mask back, synchronises.
- * All pointers are HOST memory (pinned memory makes the copies asynchronous). */
+ * All pointers are HOST memory (pinned memory makes the copies asynchronous).  When out_ranges_host is pinned
+ * (mapped) memory of at most 64 MB and no feature output is bound, the beam kernels store the ranges
+ * straight into it over PCIe while they compute (no staging copy); the results are the same either way. */
 int fn_step_host(fn_sim* sim, float* states_host, const float* actions_host, float dt,
                  uint8_t* reset_mask_host, const uint64_t* seeds_host, float* out_ranges_host,
                  uint8_t* out_collision_host, float* out_goal_obs_host);

@@ -810,17 +810,32 @@ extern "C" int fn_step_host(fn_sim* s, float* states, const float* actions, floa
     FN_CUDA(cudaMemcpyAsync(s->stg_actions, actions, n * A * sizeof(float), cudaMemcpyHostToDevice, st));
     FN_CUDA(cudaMemcpyAsync(s->stg_mask, mask, n, cudaMemcpyHostToDevice, st));
     if (seeds) FN_CUDA(cudaMemcpyAsync(s->stg_seeds, seeds, n * sizeof(unsigned long long), cudaMemcpyHostToDevice, st));
-    int rc = fn_step(s, s->stg_states, s->stg_actions, dt, s->stg_mask, s->stg_ranges, s->stg_col, s->stg_gobs);
+    // Ranges are 4 B per beam, the bulk of the output (12 MB of 12.2 MB at C2).  When the caller's buffer is
+    // pinned (mapped) host memory and nothing on the device reads the ranges back (no feature kernel), the
+    // beam kernels store them straight into it: each warp task writes 128 contiguous bytes, the stores are
+    // posted over PCIe while the kernel computes, and the final device-to-host copy disappears.
+    float* dev_ranges = s->stg_ranges;
+    bool direct = false;
+    if (!s->feat_z && n * B * sizeof(float) <= ((size_t)64 << 20)) {   // (larger outputs: the copy engine does as well)
+        cudaPointerAttributes pa;
+        if (cudaPointerGetAttributes(&pa, out_ranges) == cudaSuccess && pa.type == cudaMemoryTypeHost && pa.devicePointer) {
+            dev_ranges = static_cast<float*>(pa.devicePointer);
+            direct = true;
+        } else {
+            (void)cudaGetLastError();                              // (pageable memory: not an error here)
+        }
+    }
+    int rc = fn_step(s, s->stg_states, s->stg_actions, dt, s->stg_mask, dev_ranges, s->stg_col, s->stg_gobs);
     if (rc != FN_OK) return rc;
     // the step's own (pre-reset) outputs go back first; the reset then overwrites the done rows
     FN_CUDA(cudaMemcpyAsync(out_collision, s->stg_col, n, cudaMemcpyDeviceToHost, st));
     FN_CUDA(cudaMemcpyAsync(mask, s->stg_mask, n, cudaMemcpyDeviceToHost, st));
     if (seeds) {
-        rc = fn_reset(s, s->stg_states, nullptr, reinterpret_cast<const uint64_t*>(s->stg_seeds), s->stg_ranges, s->stg_gobs);
+        rc = fn_reset(s, s->stg_states, nullptr, reinterpret_cast<const uint64_t*>(s->stg_seeds), dev_ranges, s->stg_gobs);
         if (rc != FN_OK) return rc;
     }
     FN_CUDA(cudaMemcpyAsync(states, s->stg_states, 8 * n * sizeof(float), cudaMemcpyDeviceToHost, st));
-    FN_CUDA(cudaMemcpyAsync(out_ranges, s->stg_ranges, n * B * sizeof(float), cudaMemcpyDeviceToHost, st));
+    if (!direct) FN_CUDA(cudaMemcpyAsync(out_ranges, s->stg_ranges, n * B * sizeof(float), cudaMemcpyDeviceToHost, st));
     FN_CUDA(cudaMemcpyAsync(out_goal_obs, s->stg_gobs, 2 * n * sizeof(float), cudaMemcpyDeviceToHost, st));
     FN_CUDA(cudaStreamSynchronize(st));
     return FN_OK;

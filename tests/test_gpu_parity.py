@@ -328,6 +328,56 @@ def test_fused_reset_kernel_equals_the_two_kernel_path(pu):
         assert out[0][5:] == out[1][5:] and out[0][5] > n
 
 
+def test_step_host_equals_the_device_calls(pu):
+    # fn_step_host = H2D + fn_step + fn_reset(done list) + D2H in one call.  With PINNED host buffers the beam
+    # kernels store the ranges straight into the caller's memory (zero-copy), with pageable ones they go
+    # through a device staging buffer and a copy: both must equal the device-side calls bit for bit.
+    import torch
+    from harness import workloads as W
+    wl = W.make_workload(2, n_envs=700)
+    n, B, A = wl.n_envs, wl.n_beams, wl.action_dim
+    steps = 5
+    act = W.action_tape(wl, steps, 9)
+    seeds = W.seed_tape(wl, steps + 1, 9).view(np.int64)
+    # device path
+    m, r, s = pu.make_sim(wl, n)
+    buf = pu.Buffers(n, B, A)
+    buf.mask.fill_(1)
+    s.reset(buf.states, buf.mask, torch.from_numpy(seeds[0]).cuda(), buf.ranges, buf.gobs)
+    torch.cuda.synchronize()
+    st0 = buf.states.cpu().numpy().copy()
+    ref = []
+    for t in range(steps):
+        buf.mask.zero_()
+        s.step(buf.states, torch.from_numpy(act[t]).cuda(), float(wl.dt), buf.mask, buf.ranges, buf.col, buf.gobs)
+        done = buf.mask.clone(); col = buf.col.clone()
+        s.reset(buf.states, None, torch.from_numpy(seeds[t + 1]).cuda(), buf.ranges, buf.gobs)
+        torch.cuda.synchronize()
+        ref.append([x.cpu().numpy().copy() for x in (buf.states, buf.ranges, buf.gobs, done, col)])
+    s.close(); r.close(); m.close()
+    for pinned in (True, False):
+        m, r, s = pu.make_sim(wl, n)
+        dev = pu.Buffers(n, B, A)
+        dev.mask.fill_(1)
+        s.reset(dev.states, dev.mask, torch.from_numpy(seeds[0]).cuda(), dev.ranges, dev.gobs)   # same episode state
+        torch.cuda.synchronize()
+        def host(shape, dtype):
+            t = torch.zeros(shape, dtype=dtype)
+            return t.pin_memory() if pinned else t.numpy()
+        hs, hr, hg = host((8, n), torch.float32), host((n, B), torch.float32), host((2, n), torch.float32)
+        hm, hc = host((n,), torch.uint8), host((n,), torch.uint8)
+        (hs.numpy() if pinned else hs)[...] = st0
+        for t in range(steps):
+            (hm.numpy() if pinned else hm)[...] = 0
+            ha = torch.from_numpy(act[t]).pin_memory() if pinned else act[t]
+            hq = torch.from_numpy(seeds[t + 1]).pin_memory() if pinned else seeds[t + 1]
+            s.step_host(hs, ha, float(wl.dt), hm, hq, hr, hc, hg)
+            got = [np.asarray(x.numpy() if pinned else x) for x in (hs, hr, hg, hm, hc)]
+            for a, b in zip(got, ref[t]):
+                assert np.array_equal(a, b)
+        s.close(); r.close(); m.close()
+
+
 def test_clearance_features_against_the_oracle(pu):
     # NEXT-1 (Eq. (3)): sector-pooled footprint clearances.  Teacher-forced:
     # the oracle computes them in fp64 from the GPU's own fp32 ranges; tolerance 1e-4 m like the ranges

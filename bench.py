@@ -202,6 +202,7 @@ def run_ours(args):
     sim = fn.Sim(m, rb, n, goal_tol=float(wl.goal_tol), max_episode_steps=wl.max_episode_steps,
                  goal_dist_min=float(wl.goal_dist_min), goal_dist_max=float(wl.goal_dist_max))
     fused_active = sim.set_fused_reset(bool(args.fused_reset))
+    split_step = sim.set_split_step(bool(args.split_step))
     states = torch.zeros(8, n, device="cuda")
     mask = torch.ones(n, dtype=torch.uint8, device="cuda")
     ranges = torch.zeros(n, B, device="cuda")
@@ -456,7 +457,7 @@ def run_ours(args):
                "dtype": "f64", "data": "synthetic",
                "config": {"workload": workload_name(args.config), "name": wl.name, "n_envs_per_gpu": n, "beams": B,
                           "map": list(wl.occ.shape), "max_range_m": float(wl.max_range), "l2": "flushed between timed steps",
-                          "ring": bool(ring is not None), "fused_reset": bool(fused_active)},
+                          "ring": bool(ring is not None), "fused_reset": bool(fused_active), "split_step": bool(split_step)},
                "rays_per_s": float(rays[0]) / (total_ms * 1e-3),
                "useful_rays_per_s": world * n * B * K / (total_ms * 1e-3),
                "reset_rate_per_step": float(rays[1]) / (world * n * K),
@@ -470,8 +471,8 @@ def run_ours(args):
                                       "beam_reset": prof["beam_reset"][0] / K},
                "ms_per_step_p50": float(np.median(per_step_ms)), "ms_per_step_p90": float(np.percentile(per_step_ms, 90)),
                "features": feat, "replay_sample": sample, "paper_fixed_step_query": paper_query, "roofline": roofline, "cpu_baseline": cpu, "clocks": clocks,
-               # per step: env_step, beam kernel, [ring_advance], then fn_reset = one fused kernel or reset + beam kernel
-               "gpu_launches": (2 + (1 if ring is not None else 0) + (1 if fused_active else 2)) * K}
+               # per step: env step (or its motion half), beam kernel, [ring_advance unless split], then fn_reset = one fused kernel or reset + beam kernel
+               "gpu_launches": (2 + (1 if ring is not None and not split_step else 0) + (1 if fused_active else 2)) * K}
 
     # ---- end to end through the public API with HOST buffers (copies inside the timed region)
     hs = torch.empty(8, n, dtype=torch.float32).pin_memory()
@@ -526,6 +527,8 @@ def main():
     ap.add_argument("--graph", type=int, default=1, help="also time a CUDA-graph replay of the steps (information only)")
     ap.add_argument("--fused-reset", type=int, default=1, choices=[0, 1],
                     help="fn_reset as one fused kernel where possible (default) or as two kernels (0)")
+    ap.add_argument("--split-step", type=int, default=1, choices=[0, 1],
+                    help="fn_step with the env step split around the beam kernel where possible (default) or one env-step kernel (0)")
     ap.add_argument("--ring", type=int, default=1, help="attach the replay ring when the config has one (C5)")
     args = ap.parse_args()
     if args.warmup < 3:

@@ -206,6 +206,18 @@ int fn_sim_beam_config(const fn_sim* sim, int* cfg_out);
  * made at capture).  Errors: FN_ERR_INVALID_ARG (NULL sim). */
 int fn_sim_set_fused_reset(fn_sim* sim, int enable, int* active_out);
 
+/* ---- fn_step with the env step split around the beam kernel (default up to 64 envs per beam CTA, i.e. ~19 000
+ * envs) or as one env-step kernel.  The beam
+ * kernel needs only the new sensing poses, so by default fn_step launches a motion kernel (clip, motion update,
+ * poses: PAPER.md:63) and a beam kernel in which the last warp of every CTA computes collision, goal
+ * observation, reward and done for the envs the CTA owns while the other warps already cast
+ * beams; the last CTA to finish advances the ring head and the done-list parity.  enable = 0 selects the
+ * single env-step kernel followed by the ring-advance and beam kernels (also used when the collision scratch
+ * does not fit beside the beam kernel's shared memory).  Both give bit-identical outputs.  *active_out (may
+ * be NULL) = 1 if the split step will be used.  Host-side switch, takes effect at the next fn_step.
+ * Errors: FN_ERR_INVALID_ARG (NULL sim). */
+int fn_sim_set_split_step(fn_sim* sim, int enable, int* active_out);
+
 /* ---- end-to-end convenience: host buffers in, host buffers out -----------------------------------------
  * Copies states/actions/mask (and seeds) host->device, runs fn_step (+ fn_reset of the done envs when
  * seeds_host != NULL), copies states, ranges, collision, goal obs and the done mask back, synchronises.

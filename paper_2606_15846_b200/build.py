@@ -7,7 +7,7 @@ import sys
 
 _DIR = os.path.dirname(os.path.abspath(__file__))
 SOURCES = [os.path.join(_DIR, "csrc", f) for f in ("flashnav.cu", "fn_peaks.cu")]
-HEADERS = [os.path.join(_DIR, "csrc", f) for f in ("fn_common.cuh", "fn_beam.cuh", "fn_env.cuh", "fn_features.cuh", "fn_fixed_step.cuh", "fn_reset_beam.cuh")] + \
+HEADERS = [os.path.join(_DIR, "csrc", f) for f in ("fn_common.cuh", "fn_beam.cuh", "fn_env.cuh", "fn_features.cuh", "fn_fixed_step.cuh", "fn_reset_beam.cuh", "fn_step_split.cuh")] + \
           [os.path.join(os.path.dirname(_DIR), "include", "flashnav.h")]
 LIB = os.path.join(_DIR, "libflashnav.so")
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",

@@ -17,6 +17,7 @@
 #include "fn_features.cuh"
 #include "fn_fixed_step.cuh"
 #include "fn_reset_beam.cuh"
+#include "fn_step_split.cuh"
 
 using namespace fn;
 
@@ -101,6 +102,11 @@ struct fn_sim {
     bool fused_ok, fused_on;
     size_t fused_smem;
     int fused_grid;
+    // fn_step with the env step split around the beam kernel (fn_step_split.cuh)
+    bool split_ok, split_on;
+    size_t split_smem;
+    int split_grid;
+    StepEnd* d_step_end;
     // live timing
     int prof;
     std::vector<cudaEvent_t>* ev;    // triples per fn_step (e0 env e1 beam e2), pairs per fn_reset
@@ -385,6 +391,8 @@ extern "C" int fn_sim_create(const fn_map* map, const fn_robot* robot, int n, co
     if (e == cudaSuccess) e = cudaMalloc(&s->d_task_counter, sizeof(unsigned));
     if (e == cudaSuccess) e = cudaMalloc(&s->d_eval_outcome, (size_t)n);
     if (e == cudaSuccess) e = cudaMalloc(&s->d_eval_return, (size_t)n * sizeof(float));
+    if (e == cudaSuccess) e = cudaMalloc(&s->d_step_end, sizeof(StepEnd));
+    if (e == cudaSuccess) e = cudaMemsetAsync(s->d_step_end, 0, sizeof(StepEnd), s->stream);
     if (e == cudaSuccess) e = cudaMalloc(&s->d_done_list, 2 * (size_t)n * sizeof(int));
     if (e == cudaSuccess) e = cudaMalloc(&s->d_done_count, 3 * sizeof(int));
     if (e == cudaSuccess) e = cudaMemsetAsync(s->d_done_count, 0, 3 * sizeof(int), s->stream);
@@ -434,6 +442,31 @@ extern "C" int fn_sim_create(const fn_map* map, const fn_robot* robot, int n, co
             if (f1 < f0) f0 = f1;
             if (e == cudaSuccess && f0 >= 1) { s->fused_ok = s->fused_on = true; s->fused_grid = s->num_sms * f0; }
         }
+        // the split step: the beam kernel plus one collision scratch; used when it keeps the beam kernel's occupancy
+        s->split_ok = s->split_on = false;
+        s->split_smem = step_split_smem_bytes(s->beam_smem, robot->V);
+        s->split_grid = 0;
+        if (e == cudaSuccess && s->split_smem <= (size_t)max_optin) {
+            int f[2] = {0, 0};
+            if (s->use_smem) {
+                e = cudaFuncSetAttribute(step_beam_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s->split_smem);
+                if (e == cudaSuccess) e = cudaFuncSetAttribute(step_beam_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s->split_smem);
+                if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&f[0], step_beam_kernel<true, false>, 512, s->split_smem);
+                if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&f[1], step_beam_kernel<true, true>, 512, s->split_smem);
+            } else {
+                e = cudaFuncSetAttribute(step_beam_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s->split_smem);
+                if (e == cudaSuccess) e = cudaFuncSetAttribute(step_beam_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s->split_smem);
+                if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&f[0], step_beam_kernel<false, false>, 512, s->split_smem);
+                if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&f[1], step_beam_kernel<false, true>, 512, s->split_smem);
+            }
+            const int fm = f[0] < f[1] ? f[0] : f[1];
+            if (e == cudaSuccess && fm >= 1 && s->num_sms * fm >= s->beam_grid) {
+                s->split_ok = true; s->split_grid = s->num_sms * fm;
+                // one warp per CTA computes the outcomes of the envs its CTA owns, 32 at a time: worth it up to
+                // two such batches (measured: C1-C4 3-8 % faster per step, C5 with 222 envs per CTA 4 % slower)
+                s->split_on = (n + s->split_grid - 1) / s->split_grid <= 64;
+            }
+        }
     }
     if (e != cudaSuccess) {
         int code = e == cudaErrorMemoryAllocation ? FN_ERR_OOM : FN_ERR_CUDA;
@@ -449,6 +482,7 @@ extern "C" int fn_sim_destroy(fn_sim* s) {
     if (!s) return FN_OK;
     cudaFree(s->d_poses); cudaFree(s->d_ring_head); cudaFree(s->d_list); cudaFree(s->d_count); cudaFree(s->d_dprev);
     cudaFree(s->d_epstep); cudaFree(s->d_counters); cudaFree(s->d_task_counter);
+    cudaFree(s->d_step_end);
     cudaFree(s->d_done_list); cudaFree(s->d_done_count); cudaFree(s->d_eval_outcome); cudaFree(s->d_eval_return);
     if (s->ev) { for (cudaEvent_t e : *s->ev) cudaEventDestroy(e); delete s->ev; delete s->ev_kind; }
     cudaFree(s->stg_states); cudaFree(s->stg_actions); cudaFree(s->stg_ranges); cudaFree(s->stg_gobs);
@@ -485,6 +519,7 @@ static BeamArgs beam_args(fn_sim* s, const int* list, const int* count_dev, floa
     b.counters = s->d_counters; b.task_counter = s->d_task_counter;
     b.flip_par_dev = step_launch ? s->d_done_count + 2 : nullptr; b.done_count = s->d_done_count;
     b.list_par_dev = done_list ? s->d_done_count + 2 : nullptr;
+    b.exp_off = kExpOff;
     b.pair_lines = (double)s->robot->rmax / (double)s->map->res >= 110.0;     // beams of >~ 16 lines on average
     b.inv_bitsR = 1.0f / (float)(32 * s->map->dev.strideR); b.inv_bitsC = 1.0f / (float)(32 * s->map->dev.strideC);
     return b;
@@ -546,12 +581,32 @@ extern "C" int fn_step(fn_sim* s, float* states, const float* actions, float dt,
         FN_CUDA(cudaEventRecord(e0, s->stream));
     }
     a.epw = s->n >= 32768 ? 32 : (s->n >= 8192 ? 16 : 8);
-    FN_CUDA(launch_pdl(env_step_kernel, dim3((s->n + a.epw - 1) / a.epw), dim3(kEnvBlock), col_scratch_bytes(s->robot->V), s->stream, a));
-    if (s->prof) FN_CUDA(cudaEventRecord(e1, s->stream));
-    if (s->ring) {
-        FN_CUDA(launch_pdl(ring_advance_kernel, dim3(1), dim3(1), 0, s->stream, s->d_ring_head, (unsigned long long)s->n, s->ring_cap));
+    int rc = FN_OK;
+    if (s->split_on) {
+        // motion kernel, then the beam kernel whose last warps run collision / goal / reward / done for the
+        // envs their CTAs own and whose last CTA advances the ring and the done-list parity (fn_step_split.cuh)
+        FN_CUDA(launch_pdl(env_motion_kernel, dim3((s->n + a.epw - 1) / a.epw), dim3(kEnvBlock), 0, s->stream, a));
+        if (s->prof) FN_CUDA(cudaEventRecord(e1, s->stream));
+        const BeamArgs b = beam_args(s, nullptr, nullptr, out_ranges, false, false);
+        const int epc = (s->n + s->split_grid - 1) / s->split_grid;
+        const bool aux = s->count_words || s->aux_hit;
+        const dim3 grid(s->split_grid), block(512);
+        const unsigned bs = (unsigned)s->beam_smem;
+        if (s->use_smem) {
+            if (aux) FN_CUDA(launch_pdl(step_beam_kernel<true, true>, grid, block, s->split_smem, s->stream, b, a, s->d_step_end, epc, bs));
+            else FN_CUDA(launch_pdl(step_beam_kernel<true, false>, grid, block, s->split_smem, s->stream, b, a, s->d_step_end, epc, bs));
+        } else {
+            if (aux) FN_CUDA(launch_pdl(step_beam_kernel<false, true>, grid, block, s->split_smem, s->stream, b, a, s->d_step_end, epc, bs));
+            else FN_CUDA(launch_pdl(step_beam_kernel<false, false>, grid, block, s->split_smem, s->stream, b, a, s->d_step_end, epc, bs));
+        }
+    } else {
+        FN_CUDA(launch_pdl(env_step_kernel, dim3((s->n + a.epw - 1) / a.epw), dim3(kEnvBlock), col_scratch_bytes(s->robot->V), s->stream, a));
+        if (s->prof) FN_CUDA(cudaEventRecord(e1, s->stream));
+        if (s->ring) {
+            FN_CUDA(launch_pdl(ring_advance_kernel, dim3(1), dim3(1), 0, s->stream, s->d_ring_head, (unsigned long long)s->n, s->ring_cap));
+        }
+        rc = launch_beams(s, nullptr, nullptr, out_ranges, true);
     }
-    int rc = launch_beams(s, nullptr, nullptr, out_ranges, true);
     if (s->prof && rc == FN_OK) FN_CUDA(cudaEventRecord(e2, s->stream));
     if (rc == FN_OK) rc = launch_features(s, nullptr, nullptr, false, out_ranges);
     s->done_avail = 1;
@@ -773,6 +828,13 @@ extern "C" int fn_sim_set_fused_reset(fn_sim* s, int enable, int* active_out) {
     if (!s) return fail(FN_ERR_INVALID_ARG, "fn_sim_set_fused_reset: NULL sim");
     s->fused_on = enable != 0 && s->fused_ok;
     if (active_out) *active_out = s->fused_on ? 1 : 0;
+    return FN_OK;
+}
+
+extern "C" int fn_sim_set_split_step(fn_sim* s, int enable, int* active_out) {
+    if (!s) return fail(FN_ERR_INVALID_ARG, "fn_sim_set_split_step: NULL sim");
+    s->split_on = enable != 0 && s->split_ok;
+    if (active_out) *active_out = s->split_on ? 1 : 0;
     return FN_OK;
 }
 

@@ -414,6 +414,9 @@ struct BeamArgs {
     int ring_row;                // floats per ring row
     int count_words;             // (kAux only)
     int pair_lines;              // L1/L2 path: two lines per trip (pays off for long ranges)
+    unsigned exp_off;            // = kExpOff, passed at run time: as a compile-time constant ptxas splits it over the
+                                 // hot loop's address arithmetic (4 extra instructions per two lines) instead of
+                                 // keeping base - kExpOff in one register
     unsigned* task_counter;      // next warp task; zeroed by the kernel that precedes the beam kernel
     float inv_bitsR, inv_bitsC;  // 1 / (bits per line) of the row / column copy (host-computed)
     int* flip_par_dev;           // fn_step's launch: clears done_count[*par ^ 1] and flips *par (see EnvArgs)
@@ -427,9 +430,11 @@ struct BeamArgs {
 // and its lanes run similar trip counts.  kFast = production shared-memory traversal (cast_beam_smem).
 template <class MS, bool kFast, bool kAux>
 __device__ __forceinline__ void run_beam_tasks(const BeamArgs& a, const BeamMap<MS>& bm, const SmemGeo& geo,
-                                               const double2* s_tab, const int n_env, const unsigned total) {
+                                               const double2* s_tab, const int n_env, const unsigned total,
+                                               const unsigned long long ring_head,     // slot of env 0's pending ring row
+                                               const unsigned warp0, const unsigned nwarps,  // this warp's place among the
+                                               const bool has_static = true) {         // warps that share the static part
     const int B = a.robot.B;
-    const unsigned long long ring_head = a.ring_obs ? *a.ring_head : 0ull;
     const int lane = threadIdx.x & 31;
     const unsigned ntasks = (total + 31u) >> 5;
     uint32_t words = 0, rays = 0;
@@ -437,14 +442,19 @@ __device__ __forceinline__ void run_beam_tasks(const BeamArgs& a, const BeamMap<
     // time idle at the end of the launch.  So: the first 3/4 of each warp's share is static (round r ->
     // task warp0 + r * nwarps, no atomics), the rest is handed out dynamically, one atomic per warp
     // task, fetched one task ahead so that its latency is hidden.
-    const unsigned warp0 = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
-    const unsigned nwarps = gridDim.x * (blockDim.x >> 5);
+    // (has_static = false: a warp that arrives late -- fn_step_split.cuh -- takes pool tasks only)
     const unsigned static_rounds = max(1u, ((ntasks / nwarps) * 3u) >> 2);
     const unsigned dyn_base = static_rounds * nwarps;
     const bool dynamic = dyn_base < ntasks;                        // (short launches are static only)
     const unsigned long long invB = ~0ull / (unsigned long long)B + 1ull;     // floor(2^64 / B) + 1
     unsigned round = 0;
     unsigned task = warp0;
+    if (!has_static) {
+        round = static_rounds;
+        task = ntasks;
+        if (dynamic && lane == 0) task = dyn_base + atomicAdd(a.task_counter, 1u);
+        task = __shfl_sync(0xffffffffu, task, 0);
+    }
     while (task < ntasks) {
         unsigned next = ntasks;
         ++round;
@@ -526,6 +536,9 @@ __global__ void __launch_bounds__(512, 2) beam_kernel(BeamArgs a) {
     if (a.list_par_dev) { const int q = *a.list_par_dev ^ 1; a.list += (size_t)q * a.n_all; a.count_dev += q; }
     const int n_env = a.count_dev ? *a.count_dev : a.n_all;
     const unsigned total = (unsigned)n_env * (unsigned)B;
+    const unsigned long long ring_head = a.ring_obs ? *a.ring_head : 0ull;
+    const unsigned warp0 = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    const unsigned nwarps = gridDim.x * (blockDim.x >> 5);
 
     SmemGeo geo;
     geo.baseR = geo.baseC = 0; geo.rho = a.map.rho; geo.bitsR = a.map.strideR << 5; geo.bitsC = a.map.strideC << 5;
@@ -536,14 +549,14 @@ __global__ void __launch_bounds__(512, 2) beam_kernel(BeamArgs a) {
         bm.base = (uint32_t)__cvta_generic_to_shared(s_map);
         bm.H = a.map.H; bm.W = a.map.W; bm.stride4R = a.map.strideR << 2; bm.stride4C = a.map.strideC << 2;
         bm.rowBytes = rowBytes; bm.mapBytes = (unsigned)mapWords * 4u; bm.oob = a.counters + kOobLoads;
-        geo.baseR = bm.base - kExpOff; geo.baseC = geo.baseR + rowBytes;
-        run_beam_tasks<SmemSpace, !kAux, kAux>(a, bm, geo, s_tab, n_env, total);
+        geo.baseR = bm.base - a.exp_off; geo.baseC = geo.baseR + rowBytes;
+        run_beam_tasks<SmemSpace, !kAux, kAux>(a, bm, geo, s_tab, n_env, total, ring_head, warp0, nwarps);
     } else {
         BeamMap<GlobalSpace> bm;
         bm.base = (unsigned long long)__cvta_generic_to_global(a.map.row);
         bm.H = a.map.H; bm.W = a.map.W; bm.stride4R = a.map.strideR << 2; bm.stride4C = a.map.strideC << 2;
         bm.rowBytes = rowBytes; bm.mapBytes = (unsigned)mapWords * 4u; bm.oob = a.counters + kOobLoads;
-        run_beam_tasks<GlobalSpace, false, kAux>(a, bm, geo, s_tab, n_env, total);
+        run_beam_tasks<GlobalSpace, false, kAux>(a, bm, geo, s_tab, n_env, total, ring_head, warp0, nwarps);
     }
 }
 

@@ -278,32 +278,23 @@ struct EnvArgs {
 // lanes for throughput.
 constexpr int kEnvBlock = 32;
 
-__global__ void __launch_bounds__(kEnvBlock) env_step_kernel(EnvArgs a) {
-    extern __shared__ __align__(16) uint8_t s_dyn[];
-    const ColScratch scratch = col_scratch(s_dyn, a.robot.V);
-    for (int k = threadIdx.x; k < a.robot.V; k += kEnvBlock) { scratch.verts[k] = a.robot.verts[k]; scratch.nxt[k] = a.robot.nxt[k]; }
-    __syncwarp();
-    griddep_wait();                                                // states / actions / mask come from earlier work
-    griddep_launch_dependents();                                   // the beam kernel may start staging the map now
-    if (blockIdx.x == 0 && threadIdx.x == 0) *a.beam_task_counter = 0u;
-    const int e = blockIdx.x * a.epw + threadIdx.x;
+// ---------------------------------------------------------------- S1: the motion update of one env
+// Pure function of the stored state, the action and the stored sensing pose (no writes): the new fp32 pose
+// and applied velocities, and cos/sin of the new heading in fp64.  `el` = the env to read.
+struct EnvMotion {
+    float xf, yf, psif, avx, avy, aw;
+    double c1, s1;
+    bool bad;                    // a non-finite action component
+};
+__device__ __forceinline__ EnvMotion env_motion(const EnvArgs& a, const int el) {
     const int n = a.n;
-    const bool in_range = (int)threadIdx.x < a.epw && e < n;
-    const int el = in_range ? e : n - 1;                           // idle lanes shadow the last env, write nothing
-    // evaluation mode: "completion masks ... exclude completed cases": a completed case is frozen
-    const bool frozen = in_range && a.eval_outcome != nullptr && a.eval_outcome[el] != 0;
-    const bool live = in_range && !frozen;
+    const int es = a.ep_step[el];
+    const int A = a.robot.A;
     // ---- S1: clip ("within the configured bounds") and exact constant-twist step
     const double x = a.states[0 * n + el], y = a.states[1 * n + el], psi = a.states[2 * n + el];
-    const float gxf = a.states[6 * n + el], gyf = a.states[7 * n + el];
-    const float dp = a.d_prev[el];                                 // (loaded early: off the critical path)
-    const int es = a.ep_step[el];
-    const bool forced = a.reset_mask[el] != 0;
-    const int A = a.robot.A;
     float avx = a.actions[(size_t)el * A], avy = 0.0f, aw;
     if (a.robot.drive == 0) aw = a.actions[(size_t)el * A + 1];
     else { avy = a.actions[(size_t)el * A + 1]; aw = a.actions[(size_t)el * A + 2]; }
-    const float raw0 = avx, raw1 = a.robot.drive == 0 ? aw : avy, raw2 = aw;
     const bool bad = !(isfinite(avx) && isfinite(avy) && isfinite(aw));
     avx = fminf(fmaxf(avx, a.robot.lim[0]), a.robot.lim[1]);
     if (a.robot.drive != 0) avy = fminf(fmaxf(avy, a.robot.lim[2]), a.robot.lim[3]);
@@ -355,10 +346,57 @@ __global__ void __launch_bounds__(kEnvBlock) env_step_kernel(EnvArgs a) {
     } else {
         sincos((double)psif, &s1, &c1);
     }
+    EnvMotion mo;
+    mo.xf = xf; mo.yf = yf; mo.psif = psif; mo.avx = avx; mo.avy = avy; mo.aw = aw; mo.c1 = c1; mo.s1 = s1; mo.bad = bad;
+    return mo;
+}
+// the motion's results written back: state planes 0-5 and the sensing pose (all lanes that are live)
+template <bool kS>
+__device__ __forceinline__ void env_motion_store(const EnvArgs& a, const MapDev& m, const int e, const EnvMotion& mo,
+                                                 BeamPose* pose_copy = nullptr) {
+    const int n = a.n;
+    a.states[0 * n + e] = mo.xf; a.states[1 * n + e] = mo.yf; a.states[2 * n + e] = mo.psif;
+    a.states[3 * n + e] = mo.avx; a.states[4 * n + e] = mo.avy; a.states[5 * n + e] = mo.aw;
+    const BeamPose bp = make_pose<kS>(m, a.robot, mo.xf, mo.yf, mo.psif, mo.c1, mo.s1);
+    a.poses[e] = bp;
+    if (pose_copy) *pose_copy = bp;
+    if (mo.bad) atomicAdd(&a.counters[kNonFinite], 1ull);
+}
+// the same values read back from memory (split step: the motion ran in an earlier kernel)
+__device__ __forceinline__ EnvMotion env_motion_load(const EnvArgs& a, const int el) {
+    const int n = a.n;
+    EnvMotion mo;
+    mo.xf = a.states[0 * n + el]; mo.yf = a.states[1 * n + el]; mo.psif = a.states[2 * n + el];
+    mo.avx = a.states[3 * n + el]; mo.avy = a.states[4 * n + el]; mo.aw = a.states[5 * n + el];
+    mo.c1 = a.poses[el].c; mo.s1 = a.poses[el].s; mo.bad = false;
+    return mo;
+}
+
+// ---------------------------------------------------------------- S3 + S4 of one env per lane
+// Collision at the new pose, goal observation, reward, done, the done list, the ring row and the episode
+// bookkeeping.  All 32 lanes of the warp call (the exact polygon test is warp-cooperative); lanes with
+// in_range = false idle and write nothing.  m = the packed map to read: a.map (kS = false) or the same map
+// with row / col pointing at a shared-memory copy (kS = true).  ring_head = slot of env 0's row of THIS step.
+// store_motion: also write the motion's results (the single-kernel env step); false when an earlier kernel
+// stored them (split step).
+template <bool kS>
+__device__ __forceinline__ void env_outcome(const EnvArgs& a, const MapDev& m, const ColScratch& scratch, const int e,
+                                            const int el, const bool in_range, const int lane, const EnvMotion& mo,
+                                            const unsigned long long ring_head, const bool store_motion) {
+    const int n = a.n;
+    const bool frozen = in_range && a.eval_outcome != nullptr && a.eval_outcome[el] != 0;
+    const bool live = in_range && !frozen;
+    const float xf = mo.xf, yf = mo.yf, psif = mo.psif, avx = mo.avx, avy = mo.avy, aw = mo.aw;
+    const double c1 = mo.c1, s1 = mo.s1;
+    const float gxf = a.states[6 * n + el], gyf = a.states[7 * n + el];
+    const float dp = a.d_prev[el];
+    const int es = a.ep_step[el];
+    const bool forced = a.reset_mask[el] != 0;
+    const int A = a.robot.A;
     // ---- S3
-    Window win = footprint_window(a.map, scratch.verts, a.robot.V, (double)xf, (double)yf, c1, s1);
+    Window win = footprint_window<kS>(m, scratch.verts, a.robot.V, (double)xf, (double)yf, c1, s1);
     if (!live) win.status = 0;
-    const bool col = resolve_collisions(a.map, a.robot, win, (double)xf, (double)yf, c1, s1, scratch);
+    const bool col = resolve_collisions<kS>(m, a.robot, win, (double)xf, (double)yf, c1, s1, scratch);
     // ---- S4: goal obs, reward Eq. (1), done
     const double gdx = (double)gxf - (double)xf, gdy = (double)gyf - (double)yf;
     const float d = (float)sqrt(gdx * gdx + gdy * gdy);
@@ -375,9 +413,9 @@ __global__ void __launch_bounds__(kEnvBlock) env_step_kernel(EnvArgs a) {
     if (dm) {
         int base = 0;
         const int par = *a.par_dev;
-        if (threadIdx.x == 0) base = atomicAdd(a.done_count + par, __popc(dm));
+        if (lane == 0) base = atomicAdd(a.done_count + par, __popc(dm));
         base = __shfl_sync(0xffffffffu, base, 0);
-        if (done) a.done_list[(size_t)par * n + base + __popc(dm & ((1u << threadIdx.x) - 1u))] = e;
+        if (done) a.done_list[(size_t)par * n + base + __popc(dm & ((1u << lane) - 1u))] = e;
     }
     if (frozen) {                                                  // no state change, no reward, not done again
         a.reset_mask[e] = 0;
@@ -388,29 +426,41 @@ __global__ void __launch_bounds__(kEnvBlock) env_step_kernel(EnvArgs a) {
         a.eval_return[e] += r;
         if (done) a.eval_outcome[e] = col ? 2 : reached ? 1 : 3;
     }
-    a.states[0 * n + e] = xf; a.states[1 * n + e] = yf; a.states[2 * n + e] = psif;
-    a.states[3 * n + e] = avx; a.states[4 * n + e] = avy; a.states[5 * n + e] = aw;
+    if (store_motion) env_motion_store<kS>(a, m, e, mo);
     a.out_collision[e] = col ? 1 : 0;
     a.out_goal_obs[e] = d; a.out_goal_obs[n + e] = alpha;
     if (a.out_reward) a.out_reward[e] = r;
     a.reset_mask[e] = done;
     a.d_prev[e] = d;
     a.ep_step[e] = es + 1;
-    write_pose(a.map, a.robot, &a.poses[e], xf, yf, psif, c1, s1);
     if (a.ring) {
         // complete this step's row (its obs part was written when that observation was produced)
         const int B = a.robot.B;
-        const unsigned long long head = *a.ring_head_dev;
+        const unsigned long long head = ring_head;
         float* row = a.ring + ((head + (unsigned long long)e) % a.ring_cap) * (size_t)a.ring_row;
-        row[B + 5] = raw0; row[B + 6] = raw1;
-        if (A == 3) row[B + 7] = raw2;
+        for (int k = 0; k < A; ++k) row[B + 5 + k] = a.actions[(size_t)e * A + k];   // the raw action
         row[B + 5 + A] = r;
         row[B + 6 + A] = done ? 1.0f : 0.0f;
         // and start the next step's row with the new goal obs and velocities
         float* nxt = a.ring + ((head + (unsigned long long)n + (unsigned long long)e) % a.ring_cap) * (size_t)a.ring_row;
         nxt[B] = d; nxt[B + 1] = alpha; nxt[B + 2] = avx; nxt[B + 3] = avy; nxt[B + 4] = aw;
     }
-    if (bad) atomicAdd(&a.counters[kNonFinite], 1ull);
+}
+
+__global__ void __launch_bounds__(kEnvBlock) env_step_kernel(EnvArgs a) {
+    extern __shared__ __align__(16) uint8_t s_dyn[];
+    const ColScratch scratch = col_scratch(s_dyn, a.robot.V);
+    for (int k = threadIdx.x; k < a.robot.V; k += kEnvBlock) { scratch.verts[k] = a.robot.verts[k]; scratch.nxt[k] = a.robot.nxt[k]; }
+    __syncwarp();
+    griddep_wait();                                                // states / actions / mask come from earlier work
+    griddep_launch_dependents();                                   // the beam kernel may start staging the map now
+    if (blockIdx.x == 0 && threadIdx.x == 0) *a.beam_task_counter = 0u;
+    const int e = blockIdx.x * a.epw + threadIdx.x;
+    const int n = a.n;
+    const bool in_range = (int)threadIdx.x < a.epw && e < n;
+    const int el = in_range ? e : n - 1;                           // idle lanes shadow the last env, write nothing
+    const EnvMotion mo = env_motion(a, el);
+    env_outcome<false>(a, a.map, scratch, e, el, in_range, (int)threadIdx.x, mo, a.ring ? *a.ring_head_dev : 0ull, true);
 }
 
 // advances the replay ring's head by n rows (one thread), after the env-step kernel of fn_step;

@@ -82,7 +82,7 @@ __global__ void __launch_bounds__(kFusedThreads, 2) reset_beam_kernel(ResetArgs 
     bm.base = (uint32_t)__cvta_generic_to_shared(s_map);
     bm.H = a.map.H; bm.W = a.map.W; bm.stride4R = a.map.strideR << 2; bm.stride4C = a.map.strideC << 2;
     bm.rowBytes = (unsigned)rowWords * 4u; bm.mapBytes = (unsigned)mapWords * 4u; bm.oob = a.counters + kOobLoads;
-    geo.baseR = bm.base - kExpOff; geo.baseC = geo.baseR + bm.rowBytes;
+    geo.baseR = bm.base - a.exp_off; geo.baseC = geo.baseR + bm.rowBytes;
     const unsigned long long ring_head = a.ring_obs ? *a.ring_head : 0ull;
     const unsigned total = (unsigned)m_loc * (unsigned)B;
     const unsigned ntasks = (total + 31u) >> 5;

@@ -378,6 +378,57 @@ def test_step_host_equals_the_device_calls(pu):
         s.close(); r.close(); m.close()
 
 
+def test_split_step_equals_the_single_env_step_kernel(pu):
+    # fn_step either runs one env-step kernel, the ring-advance kernel and the beam kernel, or (default) a
+    # motion kernel and a beam kernel whose last warps compute collision / goal / reward / done for the envs
+    # their CTAs own and whose last CTA advances the ring head and the done-list parity: same states, flags,
+    # observations, rewards, hit cells, ring rows, done lists and counters, bit for bit.  Shared-memory and
+    # L2 maps, one and many envs per CTA (more than a warp's 32), a ring, the instrumented kernels.
+    import torch
+    from harness import workloads as W
+    for cfg, n, ring_cap, aux in ((1, 64, 0, True), (2, 1500, 0, False), (3, 2000, 0, False), (4, 1100, 0, False),
+                                  (1, 20000, 0, False), (5, 300, 1024, False), (5, 700, 0, True)):
+        wl = W.make_workload(cfg, n_envs=n)
+        B, A = wl.n_beams, wl.action_dim
+        steps = 6
+        actions = torch.from_numpy(W.action_tape(wl, steps, 6)).cuda()
+        seeds = torch.from_numpy(W.seed_tape(wl, steps + 1, 6).view(np.int64)).cuda()
+        forced = torch.from_numpy((np.random.default_rng(6).random((steps, n)) < 0.03).astype(np.uint8)).cuda()
+        out = []
+        for split in (True, False):
+            m, r, s = pu.make_sim(wl, n)
+            assert s.set_split_step(split) == split
+            buf = pu.Buffers(n, B, A)
+            hit = torch.full((n, B), -9, dtype=torch.int32, device="cuda")
+            rew = torch.zeros(n, device="cuda")
+            s.bind_aux(hit if aux else None, rew)
+            ring = None
+            if ring_cap:
+                ring = torch.zeros(ring_cap * (B + 5 + A + 2), device="cuda")
+                s.ring_attach(ring, ring_cap)
+            buf.mask.fill_(1)
+            s.reset(buf.states, buf.mask, seeds[0], buf.ranges, buf.gobs)
+            trace = []
+            for t in range(steps):
+                buf.mask.copy_(forced[t])
+                s.step(buf.states, actions[t], float(wl.dt), buf.mask, buf.ranges, buf.col, buf.gobs)
+                trace += [buf.states.clone(), buf.ranges.clone(), buf.gobs.clone(), buf.mask.clone(), buf.col.clone(), rew.clone(), hit.clone()]
+                s.reset(buf.states, None if t % 2 == 0 else buf.mask, seeds[t + 1], buf.ranges, buf.gobs)
+                trace += [buf.states.clone(), buf.ranges.clone()]
+            torch.cuda.synchronize()
+            c = s.counters()
+            assert c["oob_window_loads"] == 0
+            if ring is not None:
+                trace.append(ring.clone())
+            d_prev, ep = s.episode_state()
+            trace += [torch.from_numpy(d_prev), torch.from_numpy(ep)]
+            out.append((trace, c))
+            s.close(); r.close(); m.close()
+        for a, b in zip(out[0][0], out[1][0]):
+            assert torch.equal(a, b)
+        assert out[0][1] == out[1][1] and out[0][1]["envs_reset"] > n
+
+
 def test_clearance_features_against_the_oracle(pu):
     # NEXT-1 (Eq. (3)): sector-pooled footprint clearances.  Teacher-forced:
     # the oracle computes them in fp64 from the GPU's own fp32 ranges; tolerance 1e-4 m like the ranges

@@ -31,8 +31,10 @@ sys.path.insert(0, ROOT)
 from harness import workloads as W  # noqa: E402
 
 # dominant kernel (full-batch beam launch), per launch, from the committed ncu --set full capture
-NCU_CAPTURE = {2: {"dram_bytes": 506624, "warp_inst": 45733853, "lanes": 22.05,
-                   "source": "profiles/r1e_beam_kernels_full_c2.txt (dram__bytes_read.sum + dram__bytes_write.sum)"}}
+NCU_CAPTURE = {(2, False): {"dram_bytes": 506624, "warp_inst": 45733853, "lanes": 22.05,
+                            "source": "profiles/r1e_beam_kernels_full_c2.txt (dram__bytes_read.sum + dram__bytes_write.sum)"},
+               (2, True): {"dram_bytes": 720896, "warp_inst": 46700700, "lanes": 22.10,
+                           "source": "profiles/r1f_beam_kernels_full_c2.txt (dram__bytes_read.sum + dram__bytes_write.sum)"}}
 
 METRIC = "env_steps_per_s"
 UNIT = "env-steps/s"
@@ -400,10 +402,11 @@ def run_ours(args):
         peak = smem_peak if use_smem else l2_peak
         beam_s = beam_ms * 1e-3 / max(1, beam_launches)
         achieved = a_ray * n * B / beam_s
-        ncu = NCU_CAPTURE.get(args.config)
+        ncu = NCU_CAPTURE.get((args.config, bool(split_step)))
         sm_hz = (clocks or {}).get("sm_mhz") or 1965.0
         issue_peak = 148 * 4 * sm_hz * 1e6                      # warp instructions / s: 1 per scheduler per clock
-        roofline = {"bound": "smem" if use_smem else "l2", "kernel": "fn::beam_kernel (fn_step, all envs)",
+        roofline = {"bound": "smem" if use_smem else "l2", "kernel": ("fn::step_beam_kernel (fn_step, all envs: beams + collision / goal / reward / done of the split step)"
+                               if split_step else "fn::beam_kernel (fn_step, all envs)"),
                     "achieved": achieved / 1e9, "peak": peak / 1e9, "unit": "GB/s", "frac": achieved / peak,
                     "peak_source": "fn_measure_peak in this run (conflict-free ld.shared / L2-resident ld.global.nc)",
                     "algorithmic_bytes_per_beam": a_ray, "windows_per_beam": windows,

@@ -105,15 +105,17 @@ __device__ __forceinline__ float range_from_du(double dU, float scale) { return 
 // over 32-bit words; at most T / 30 + 2 lines of up to T cells each.
 template <class MS>
 __device__ __noinline__ BeamHit cast_beam_slow(const BeamMap<MS> bm, const BeamOrient o, const bool mx,
-                                               const double du, const double dw, const double T,
-                                               const float rho, const float rmax) {
+                                               const double du, const double dw, const double M_in,
+                                               const double T, const float rho, const float rmax) {
+    // M_in = |du| / |dw| as the callers computed it (Newton-refined reciprocal, relative error ~2^-40: at most
+    // ~1e-9 cell over a beam, far inside the 1e-5 cell near-tie margin); NaN or inf when dw == 0
     const double adu = fabs(du), adw = fabs(dw);
     const bool fu = du >= 0.0, fw = dw >= 0.0;
     const double ou = o.ouM - (kMagic + (double)kCellShift);
     const double f = fw ? 0.5 + o.h : 0.5 - o.h;
     const int Wu = mx ? bm.W : bm.H, Hw = mx ? bm.H : bm.W;
     const int stride4 = mx ? bm.stride4R : bm.stride4C;
-    const double M = adw > 0.0 ? adu / adw : INFINITY;
+    const double M = adw > 0.0 ? M_in : INFINITY;
     const double Tu = T * adu;                                    // travel along u at the range limit
     typename MS::addr_t line = MS::addb(bm.base, (int)o.line_off);
     int l = origin_line(bm, o, mx);
@@ -179,7 +181,7 @@ __device__ __forceinline__ float cast_beam(const BeamMap<MS>& bm, const BeamPose
     const double r1 = fma(fma(-adw, r0, 1.0), r0, r0);
     const double M = adu * r1;
     if (!(M < kSlowSlope)) {                                      // also dw == 0 (M = inf or NaN)
-        const BeamHit h = cast_beam_slow<MS>(bm, o, mx, du, dw, T, rho, rmax);
+        const BeamHit h = cast_beam_slow<MS>(bm, o, mx, du, dw, M, T, rho, rmax);
         if (kAux) { *hit = h.hit; words += 8; }
         return h.r;
     }
@@ -308,7 +310,7 @@ __device__ __forceinline__ float cast_beam_smem(const BeamMap<SmemSpace>& bm, co
     const double r0 = rcp64h(adw);
     const double r1 = fma(fma(-adw, r0, 1.0), r0, r0);
     const double M = adu * r1;
-    if (!(M < kSlowSlope)) return cast_beam_slow<SmemSpace>(bm, o, mx, du, dw, T, g.rho, rmax).r;
+    if (!(M < kSlowSlope)) return cast_beam_slow<SmemSpace>(bm, o, mx, du, dw, M, T, g.rho, rmax).r;
     const unsigned su = hiw(du) & 0x80000000u, sw = hiw(dw) & 0x80000000u;   // sign bits: set = backward
     const unsigned fu1 = (su >> 31) ^ 1u;
     const double Mm = M + kMagic, Mq = Mm - kMagic;

@@ -547,7 +547,7 @@ static int launch_features(fn_sim* s, const int* list, const int* count_dev, boo
     f.n_sectors = s->feat_sectors; f.rmax = s->robot->rmax; f.sx = s->robot->sensor[0]; f.sy = s->robot->sensor[1];
     f.ranges = ranges; f.z = s->feat_z; f.list = list; f.count_dev = count_dev;
     f.list_par_dev = done_list ? s->d_done_count + 2 : nullptr; f.n_all = s->n;
-    int grid = (s->n + kFeatWarps - 1) / kFeatWarps;
+    int grid = (s->n + kFeatEnvs - 1) / kFeatEnvs;
     if (grid > s->num_sms * 8) grid = s->num_sms * 8;
     cudaEvent_t e0 = nullptr, e1 = nullptr;
     if (s->prof) {

@@ -7,7 +7,7 @@
 // beams without a valid hit get r_max; z_k = min of delta_j over the beams of sector k.  Sector of beam j
 // = floor(j n_sectors / B): n_sectors groups of consecutive beams in table order (reading G21).
 //
-// One warp per env: the lanes stride over the env's beams (coalesced reads of the range row, L2-resident
+// kFeatSplit warps per env: their lanes stride over the env's beams (coalesced reads of the range row, L2-resident
 // right after the beam kernel), each computes its delta in fp32 (ample: the tolerance is 1e-4 m, delta is
 // continuous across the polygon boundary) and the sector minima are kept in shared memory with atomicMin
 // on the float bits (monotone for non-negative floats).
@@ -31,9 +31,11 @@ struct FeatArgs {
 };
 
 constexpr int kFeatWarps = 8;
+constexpr int kFeatSplit = 4;                         // warps that share one env's beams (latency: an env's row is short)
+constexpr int kFeatEnvs = kFeatWarps / kFeatSplit;   // envs a CTA works on at a time
 
 __host__ __device__ inline size_t feat_smem_bytes(int V, int n_sectors) {
-    return (size_t)V * 8 * sizeof(float) + (size_t)kFeatWarps * n_sectors * sizeof(unsigned);
+    return (size_t)V * 8 * sizeof(float) + (size_t)kFeatEnvs * n_sectors * sizeof(unsigned);
 }
 __host__ __device__ inline size_t feat_smem_bytes(int V, int n_sectors, int B) {
     return feat_smem_bytes(V, n_sectors) + (size_t)B * sizeof(float2);
@@ -45,26 +47,19 @@ __global__ void __launch_bounds__(kFeatWarps * 32) features_kernel(FeatArgs a) {
     // end vertex y (the SAME float the edge from that vertex starts at, so the even-odd rule is consistent
     // at vertices) and whether the edge closes its component ("For a union of polygons, the minimum
     // distance over its components is used": inside = inside ANY component)
-    float2* s_cs = reinterpret_cast<float2*>(s_dyn);
-    float* s_ax = reinterpret_cast<float*>(s_cs + a.B);
-    float* s_ay = s_ax + a.V;
-    float* s_ex = s_ay + a.V;
-    float* s_ey = s_ex + a.V;
-    float* s_il = s_ey + a.V;
-    float* s_sl = s_il + a.V;
-    float* s_by = s_sl + a.V;
-    int* s_last = reinterpret_cast<int*>(s_by + a.V);
-    unsigned* s_z = reinterpret_cast<unsigned*>(s_last + a.V) + (threadIdx.x >> 5) * a.n_sectors;
+    // (two 16-byte records per edge, so the per-edge loop below issues two shared loads instead of eight)
+    float4* s_e0 = reinterpret_cast<float4*>(s_dyn);               // start a (x, y), direction e (x, y)
+    float4* s_e1 = s_e0 + a.V;                                     // 1/|e|^2, e_x/e_y, end vertex y, closes its component
+    float2* s_cs = reinterpret_cast<float2*>(s_e1 + a.V);
+    const int wib = threadIdx.x >> 5, grp = wib / kFeatSplit, sub = wib % kFeatSplit;   // env slot, warp within the env
+    unsigned* s_z = reinterpret_cast<unsigned*>(s_cs + a.B) + grp * a.n_sectors;
     for (int j = threadIdx.x; j < a.B; j += blockDim.x) { const double2 c = a.beam_cs[j]; s_cs[j] = make_float2((float)c.x, (float)c.y); }
     for (int k = threadIdx.x; k < a.V; k += blockDim.x) {
         const int k1 = a.nxt[k];
         const double2 p = a.verts[k], q = a.verts[k1];
-        s_last[k] = k1 <= k;
         const float ex = (float)(q.x - p.x), ey = (float)(q.y - p.y), l2 = ex * ex + ey * ey;
-        s_ax[k] = (float)p.x; s_ay[k] = (float)p.y; s_ex[k] = ex; s_ey[k] = ey;
-        s_il[k] = l2 > 0.0f ? 1.0f / l2 : 0.0f;
-        s_sl[k] = ey != 0.0f ? ex / ey : 0.0f;
-        s_by[k] = (float)q.y;
+        s_e0[k] = make_float4((float)p.x, (float)p.y, ex, ey);
+        s_e1[k] = make_float4(l2 > 0.0f ? 1.0f / l2 : 0.0f, ey != 0.0f ? ex / ey : 0.0f, (float)q.y, k1 <= k ? 1.0f : 0.0f);
     }
     __syncthreads();
     griddep_wait();                                                // the ranges come from the beam kernel
@@ -74,18 +69,22 @@ __global__ void __launch_bounds__(kFeatWarps * 32) features_kernel(FeatArgs a) {
     const int lane = threadIdx.x & 31;
     const unsigned rmax_bits = __float_as_uint(a.rmax);
     const unsigned long long invB = ~0ull / (unsigned long long)a.B + 1ull;          // floor(2^64 / B) + 1
-    for (int le = blockIdx.x * kFeatWarps + (threadIdx.x >> 5); le < n_env; le += gridDim.x * kFeatWarps) {
-        const int e = a.list ? a.list[le] : le;
-        for (int k = lane; k < a.n_sectors; k += 32) s_z[k] = rmax_bits;
-        __syncwarp();
+    const int tid = sub * 32 + lane;                               // thread index within the env's group
+    for (int le0 = blockIdx.x * kFeatEnvs; le0 < n_env; le0 += gridDim.x * kFeatEnvs) {       // (uniform over the CTA)
+        const int le = le0 + grp;
+        const bool have = le < n_env;
+        const int e = have ? (a.list ? a.list[le] : le) : 0;
+        for (int k = tid; k < a.n_sectors; k += kFeatSplit * 32) s_z[k] = rmax_bits;
+        __syncthreads();
         const float* row = a.ranges + (size_t)e * a.B;
-        for (int j0 = lane; j0 < a.B; j0 += 4 * 32) {              // four chunks per trip: their loads overlap
+        if (have)
+        for (int j0 = tid; j0 < a.B; j0 += 4 * kFeatSplit * 32) {  // four chunks per trip: their loads overlap
             float r[4];
 #pragma unroll
-            for (int u = 0; u < 4; ++u) r[u] = j0 + 32 * u < a.B ? row[j0 + 32 * u] : a.rmax;
+            for (int u = 0; u < 4; ++u) r[u] = j0 + kFeatSplit * 32 * u < a.B ? row[j0 + kFeatSplit * 32 * u] : a.rmax;
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
-                const int j = j0 + 32 * u;
+                const int j = j0 + kFeatSplit * 32 * u;
                 if (j >= a.B) break;
                 float d = a.rmax;                                  // no valid hit: the maximum range
                 if (r[u] < a.rmax) {
@@ -93,14 +92,16 @@ __global__ void __launch_bounds__(kFeatWarps * 32) features_kernel(FeatArgs a) {
                     const float px = fmaf(r[u], cs.x, a.sx), py = fmaf(r[u], cs.y, a.sy);
                     float d2 = INFINITY;
                     bool inside = false, inside_c = false;
+#pragma unroll 4
                     for (int k = 0; k < a.V; ++k) {
-                        const float ax = s_ax[k], ay = s_ay[k], ex = s_ex[k], ey = s_ey[k];
+                        const float4 g0 = s_e0[k], g1 = s_e1[k];
+                        const float ax = g0.x, ay = g0.y, ex = g0.z, ey = g0.w;
                         const float rx = px - ax, ry = py - ay;
-                        const float t = fminf(fmaxf((rx * ex + ry * ey) * s_il[k], 0.0f), 1.0f);
+                        const float t = fminf(fmaxf((rx * ex + ry * ey) * g1.x, 0.0f), 1.0f);
                         const float qx = rx - t * ex, qy = ry - t * ey;
                         d2 = fminf(d2, qx * qx + qy * qy);
-                        if ((ay > py) != (s_by[k] > py) && rx < ry * s_sl[k]) inside_c = !inside_c;  // even-odd rule
-                        if (s_last[k]) { inside |= inside_c; inside_c = false; }
+                        if ((ay > py) != (g1.z > py) && rx < ry * g1.y) inside_c = !inside_c;       // even-odd rule
+                        if (g1.w != 0.0f) { inside |= inside_c; inside_c = false; }
                     }
                     d = inside ? 0.0f : fminf(sqrtf(d2), a.rmax);  // capped at the sensor range
                 }
@@ -108,9 +109,9 @@ __global__ void __launch_bounds__(kFeatWarps * 32) features_kernel(FeatArgs a) {
                 atomicMin(&s_z[k], __float_as_uint(d));
             }
         }
-        __syncwarp();
-        for (int k = lane; k < a.n_sectors; k += 32) a.z[(size_t)e * a.n_sectors + k] = __uint_as_float(s_z[k]);
-        __syncwarp();
+        __syncthreads();
+        if (have) for (int k = tid; k < a.n_sectors; k += kFeatSplit * 32) a.z[(size_t)e * a.n_sectors + k] = __uint_as_float(s_z[k]);
+        __syncthreads();
     }
 }
 

@@ -197,13 +197,15 @@ int fn_ranges_fixed_step(fn_sim* sim, const float* states_dev, float delta_m, in
 int fn_sim_beam_config(const fn_sim* sim, int* cfg_out);
 
 /* ---- fn_reset as one launch or two.  When the packed map is staged in shared memory (cfg_out[0] of
- * fn_sim_beam_config) and the reset scratch fits beside it, fn_reset runs ONE kernel in which every CTA
- * resets its share of the listed envs from its shared copy of the map and then recomputes their beams
- * (PAPER.md:84); this is the default.  enable = 0 selects the two-kernel path (reset kernel, then the beam
- * kernel over the list), which is also what runs when the fused kernel is not possible.  Both paths give
- * bit-identical states, goal observations and ranges.  *active_out (may be NULL) = 1 if the fused kernel
- * will be used.  Host-side switch, takes effect at the next fn_reset (a captured CUDA graph keeps the choice
- * made at capture).  Errors: FN_ERR_INVALID_ARG (NULL sim). */
+ * fn_sim_beam_config) and the reset scratch fits beside it, fn_reset(mask = NULL) -- the step's done list,
+ * usually a few per cent of the envs -- runs ONE kernel in which every CTA resets its share of the listed envs
+ * from its shared copy of the map and then recomputes their beams; this is the default
+ * (enable = 1).  A caller's mask takes the two-kernel path (reset kernel, then the beam kernel over the list),
+ * which is faster for long lists such as the first reset of all envs; enable = 0 uses it for the done list
+ * too (worth it when a large part of the batch ends every step), enable = 2 uses the fused kernel for masks
+ * as well (tests).  All paths give bit-identical states, goal observations and ranges.  *active_out (may be
+ * NULL) = 1 if the fused kernel is available and enabled.  Host-side switch, takes effect at the next
+ * fn_reset (a captured CUDA graph keeps the choice made at capture).  Errors: FN_ERR_INVALID_ARG (NULL sim). */
 int fn_sim_set_fused_reset(fn_sim* sim, int enable, int* active_out);
 
 /* ---- fn_step with the env step split around the beam kernel (default up to 64 envs per beam CTA, i.e. ~19 000

@@ -340,10 +340,11 @@ class Sim:
         _check(load_library().fn_sim_beam_config(self._h, _np_ptr(cfg)), "fn_sim_beam_config")
         return {"smem": bool(cfg[0]), "grid": int(cfg[1]), "block": int(cfg[2]), "smem_bytes": int(cfg[3])}
 
-    def set_fused_reset(self, enable: bool) -> bool:
-        """fn_reset as one fused kernel (default where possible) or as two; returns whether the fused kernel is used."""
+    def set_fused_reset(self, enable) -> bool:
+        """fn_reset(mask=None) as one fused kernel (1 / True, default where possible), never (0 / False), or for
+        masks too (2); returns whether the fused kernel is available and enabled."""
         act = C.c_int(0)
-        _check(load_library().fn_sim_set_fused_reset(self._h, 1 if enable else 0, C.byref(act)), "fn_sim_set_fused_reset")
+        _check(load_library().fn_sim_set_fused_reset(self._h, int(enable), C.byref(act)), "fn_sim_set_fused_reset")
         return bool(act.value)
 
     def set_split_step(self, enable: bool) -> bool:

@@ -99,7 +99,7 @@ struct fn_sim {
     size_t beam_smem;
     int beam_grid;
     // fn_reset as one fused kernel (fn_reset_beam.cuh): possible / enabled, its shared bytes and grid
-    bool fused_ok, fused_on;
+    bool fused_ok, fused_on, fused_force;
     size_t fused_smem;
     int fused_grid;
     // fn_step with the env step split around the beam kernel (fn_step_split.cuh)
@@ -640,9 +640,12 @@ extern "C" int fn_reset(fn_sim* s, float* states, const uint8_t* mask, const uin
     a.ring = s->ring; a.ring_cap = s->ring_cap ? s->ring_cap : 1; a.ring_head_dev = s->d_ring_head; a.ring_row = ring_row_floats(s);
     a.counters = s->d_counters; a.beam_task_counter = s->d_task_counter;
     int rc = FN_OK;
-    // (a CTA of the fused kernel runs its resets on kFusedResetWarps warps and its beams on all of them: made
-    // for the usual few resets per step; a long list -- all envs -- costs about as much as the two kernels)
-    const bool fused = s->fused_on;
+    // A CTA of the fused kernel runs its resets on kFusedResetWarps warps and casts only its own envs' beams:
+    // made for the few envs a step reports done (C2, ~190 of 4096: 2-4 us faster than the two kernels).  For
+    // long lists the two throughput-oriented kernels win (C2: all 4096 envs 83 against 121 us, a quarter of
+    // them 38 against 47 us), and a caller's mask is usually such a list (the first reset of all envs), so
+    // the fused kernel serves fn_reset(mask = NULL) only -- unless forced (enable = 2, tests).
+    const bool fused = s->fused_on && (!mask || s->fused_force);
     if (fused) {
         // one launch: every CTA resets its share of the list from its shared copy of the map, then casts
         // the beams of those envs (fn_reset_beam.cuh)
@@ -827,6 +830,7 @@ extern "C" int fn_sim_beam_config(const fn_sim* s, int* cfg) {
 extern "C" int fn_sim_set_fused_reset(fn_sim* s, int enable, int* active_out) {
     if (!s) return fail(FN_ERR_INVALID_ARG, "fn_sim_set_fused_reset: NULL sim");
     s->fused_on = enable != 0 && s->fused_ok;
+    s->fused_force = enable == 2;
     if (active_out) *active_out = s->fused_on ? 1 : 0;
     return FN_OK;
 }

@@ -294,7 +294,7 @@ def test_fused_reset_kernel_equals_the_two_kernel_path(pu):
         for fused in (True, False):
             m, r, s = pu.make_sim(wl, n)
             assert s.beam_config()["smem"]
-            assert s.set_fused_reset(fused) == fused
+            assert s.set_fused_reset(2 if fused else 0) == fused            # 2: the fused kernel for masks too
             buf = pu.Buffers(n, B, A)
             hit = torch.full((n, B), -9, dtype=torch.int32, device="cuda")
             rew = torch.zeros(n, device="cuda")

@@ -71,6 +71,9 @@ def test_host_side_argument_errors_need_no_gpu(fn):
     assert lib.fn_eval_result(None, None, None, None, None) == -1 and lib.fn_eval_end(None) == -1
     assert lib.fn_ranges_fixed_step(None, None, ctypes.c_float(0.1), 1, None) == -1
     assert lib.fn_sim_set_stream(None, None) == -1 and lib.fn_reset(None, None, None, None, None, None) == -1
+    # the switches between equivalent launch sequences
+    assert lib.fn_sim_set_fused_reset(None, 1, None) == -1 and lib.fn_sim_set_split_step(None, 1, None) == -1
+    assert lib.fn_step_host(None, None, None, ctypes.c_float(0.1), None, None, None, None, None) == -1
 
 
 def test_no_cpu_fallback(fn):

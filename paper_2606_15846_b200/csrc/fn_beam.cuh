@@ -427,6 +427,26 @@ struct BeamArgs {
     unsigned long long* counters;
 };
 
+// Stages the beam table and (when `stage`) both packed copies of the map in shared memory: constants, so
+// the kernels do this BEFORE their dependency wait, under the kernel that precedes them in the stream.
+// All threads of the CTA call; the caller synchronises.
+__device__ __forceinline__ void stage_beam_constants(const BeamArgs& a, double2* s_tab, uint32_t* s_map,
+                                                     const int mapWords, const bool stage) {
+    for (int i = threadIdx.x; i < a.robot.B; i += blockDim.x) s_tab[i] = a.robot.beam_cs[i];
+    if (stage) {
+        const uint4* src = reinterpret_cast<const uint4*>(a.map.row);      // row and col copies are contiguous
+        uint4* dst = reinterpret_cast<uint4*>(s_map);
+        const int n4 = (mapWords + 3) / 4;
+        int i = threadIdx.x;
+        for (; i + 3 * (int)blockDim.x < n4; i += 4 * blockDim.x) {         // 4 loads in flight per thread
+            const uint4 v0 = __ldg(src + i), v1 = __ldg(src + i + blockDim.x);
+            const uint4 v2 = __ldg(src + i + 2 * blockDim.x), v3 = __ldg(src + i + 3 * blockDim.x);
+            dst[i] = v0; dst[i + blockDim.x] = v1; dst[i + 2 * blockDim.x] = v2; dst[i + 3 * blockDim.x] = v3;
+        }
+        for (; i < n4; i += blockDim.x) dst[i] = __ldg(src + i);
+    }
+}
+
 // The warps of the (persistent) grid take 32 consecutive (env, beam) pairs at a time: adjacent lanes =
 // adjacent beams of one env, so a warp's loads mostly hit the same or neighbouring words (broadcast)
 // and its lanes run similar trip counts.  kFast = production shared-memory traversal (cast_beam_smem).
@@ -514,19 +534,7 @@ __global__ void __launch_bounds__(512, 2) beam_kernel(BeamArgs a) {
     const int mapWords = (a.map.H + 2 * kLineGuard) * a.map.strideR + (a.map.W + 2 * kLineGuard) * a.map.strideC;
     double2* s_tab = reinterpret_cast<double2*>(smem_raw);
     uint32_t* s_map = reinterpret_cast<uint32_t*>(smem_raw + (size_t)B * sizeof(double2));
-    for (int i = threadIdx.x; i < B; i += blockDim.x) s_tab[i] = a.robot.beam_cs[i];
-    if (stage) {
-        const uint4* src = reinterpret_cast<const uint4*>(a.map.row);      // row and col copies are contiguous
-        uint4* dst = reinterpret_cast<uint4*>(s_map);
-        const int n4 = (mapWords + 3) / 4;
-        int i = threadIdx.x;
-        for (; i + 3 * (int)blockDim.x < n4; i += 4 * blockDim.x) {         // 4 loads in flight per thread
-            const uint4 v0 = __ldg(src + i), v1 = __ldg(src + i + blockDim.x);
-            const uint4 v2 = __ldg(src + i + 2 * blockDim.x), v3 = __ldg(src + i + 3 * blockDim.x);
-            dst[i] = v0; dst[i + blockDim.x] = v1; dst[i + 2 * blockDim.x] = v2; dst[i + 3 * blockDim.x] = v3;
-        }
-        for (; i < n4; i += blockDim.x) dst[i] = __ldg(src + i);
-    }
+    stage_beam_constants(a, s_tab, s_map, mapWords, stage);
     __syncthreads();
     griddep_wait();                                                // poses / list / count come from the previous kernel
     griddep_launch_dependents();

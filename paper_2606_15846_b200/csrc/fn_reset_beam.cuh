@@ -38,19 +38,7 @@ __global__ void __launch_bounds__(kFusedThreads, 2) reset_beam_kernel(ResetArgs 
     BeamPose* s_pose = reinterpret_cast<BeamPose*>(smem_raw + fused_scratch_offset(B, mapWords));
     uint8_t* s_scr = reinterpret_cast<uint8_t*>(s_pose + kFusedPoseSlots);
     const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    for (int i = threadIdx.x; i < B; i += blockDim.x) s_tab[i] = a.robot.beam_cs[i];
-    {
-        const uint4* src = reinterpret_cast<const uint4*>(a.map.row);      // row and col copies are contiguous
-        uint4* dst = reinterpret_cast<uint4*>(s_map);
-        const int n4 = (mapWords + 3) / 4;
-        int i = threadIdx.x;
-        for (; i + 3 * (int)blockDim.x < n4; i += 4 * blockDim.x) {
-            const uint4 v0 = __ldg(src + i), v1 = __ldg(src + i + blockDim.x);
-            const uint4 v2 = __ldg(src + i + 2 * blockDim.x), v3 = __ldg(src + i + 3 * blockDim.x);
-            dst[i] = v0; dst[i + blockDim.x] = v1; dst[i + 2 * blockDim.x] = v2; dst[i + 3 * blockDim.x] = v3;
-        }
-        for (; i < n4; i += blockDim.x) dst[i] = __ldg(src + i);
-    }
+    stage_beam_constants(a, s_tab, s_map, mapWords, true);
     ColScratch scratch = col_scratch(s_scr + (size_t)(wib < kFusedResetWarps ? wib : 0) * col_scratch_bytes(V), V);
     if (wib < kFusedResetWarps)
         for (int k = lane; k < V; k += 32) { scratch.verts[k] = a.robot.verts[k]; scratch.nxt[k] = a.robot.nxt[k]; }

@@ -49,19 +49,7 @@ __global__ void __launch_bounds__(512, 2) step_beam_kernel(BeamArgs a, EnvArgs e
     double2* s_tab = reinterpret_cast<double2*>(smem_raw);
     uint32_t* s_map = reinterpret_cast<uint32_t*>(smem_raw + (size_t)B * sizeof(double2));
     const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31, last_warp = (int)(blockDim.x >> 5) - 1;
-    for (int i = threadIdx.x; i < B; i += blockDim.x) s_tab[i] = a.robot.beam_cs[i];
-    if (kSmem) {
-        const uint4* src = reinterpret_cast<const uint4*>(a.map.row);      // row and col copies are contiguous
-        uint4* dst = reinterpret_cast<uint4*>(s_map);
-        const int n4 = (mapWords + 3) / 4;
-        int i = threadIdx.x;
-        for (; i + 3 * (int)blockDim.x < n4; i += 4 * blockDim.x) {         // 4 loads in flight per thread
-            const uint4 v0 = __ldg(src + i), v1 = __ldg(src + i + blockDim.x);
-            const uint4 v2 = __ldg(src + i + 2 * blockDim.x), v3 = __ldg(src + i + 3 * blockDim.x);
-            dst[i] = v0; dst[i + blockDim.x] = v1; dst[i + 2 * blockDim.x] = v2; dst[i + 3 * blockDim.x] = v3;
-        }
-        for (; i < n4; i += blockDim.x) dst[i] = __ldg(src + i);
-    }
+    stage_beam_constants(a, s_tab, s_map, mapWords, kSmem);
     const ColScratch scratch = col_scratch(smem_raw + step_split_scratch_offset(beam_smem), V);
     if (wib == last_warp)
         for (int k = lane; k < V; k += 32) { scratch.verts[k] = a.robot.verts[k]; scratch.nxt[k] = a.robot.nxt[k]; }

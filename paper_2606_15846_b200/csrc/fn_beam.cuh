@@ -427,6 +427,32 @@ struct BeamArgs {
     unsigned long long* counters;
 };
 
+// One (env, beam) element: cast, store the range (and, instrumented, the hit cell; with a ring, the obs part
+// of the env's pending ring row).  ring_head = slot of env 0's pending row.
+template <class MS, bool kFast, bool kAux>
+__device__ __forceinline__ void beam_element(const BeamArgs& a, const BeamMap<MS>& bm, const SmemGeo& geo,
+                                             const double2* s_tab, const BeamPose* pose, const unsigned e, const unsigned j,
+                                             const unsigned long long ring_head, uint32_t& words) {
+    const int state = pose->state;
+    float r = 0.0f;
+    int hit = -2;
+    if (state == 0) {
+        if constexpr (kFast) r = cast_beam_smem(bm, geo, pose, s_tab[j], a.robot.T, a.robot.rmax);
+        else r = cast_beam<MS, kAux>(bm, pose, s_tab[j], a.robot.T, a.map.rho, a.robot.rmax, &hit, words, a.pair_lines != 0);
+    } else if (kAux) {
+        if (state == 1) hit = origin_line(bm, pose->o[0], true) * a.map.W + pose->o[0].cu0;
+        ++words;
+    }
+    const unsigned o = e * (unsigned)a.robot.B + j;                // n_envs * B < 2^31 (fn_sim_create)
+    a.out_ranges[o] = r;
+    if (kAux && a.out_hit) a.out_hit[o] = hit;
+    if (a.ring_obs) {
+        unsigned long long slot = ring_head + (unsigned long long)e;   // both < ring_cap
+        if (slot >= a.ring_cap) slot -= a.ring_cap;
+        a.ring_obs[slot * a.ring_row + j] = r;
+    }
+}
+
 // Stages the beam table and (when `stage`) both packed copies of the map in shared memory: constants, so
 // the kernels do this BEFORE their dependency wait, under the kernel that precedes them in the stream.
 // All threads of the CTA call; the caller synchronises.
@@ -488,25 +514,7 @@ __device__ __forceinline__ void run_beam_tasks(const BeamArgs& a, const BeamMap<
         const unsigned j = idx - le * (unsigned)B;
         if (le < (unsigned)n_env) {
             const unsigned e = a.list ? (unsigned)a.list[le] : le;
-            const BeamPose* pose = a.poses + e;
-            const int state = pose->state;
-            float r = 0.0f;
-            int hit = -2;
-            if (state == 0) {
-                if constexpr (kFast) r = cast_beam_smem(bm, geo, pose, s_tab[j], a.robot.T, a.robot.rmax);
-                else r = cast_beam<MS, kAux>(bm, pose, s_tab[j], a.robot.T, a.map.rho, a.robot.rmax, &hit, words, a.pair_lines != 0);
-            } else if (kAux) {
-                if (state == 1) hit = origin_line(bm, pose->o[0], true) * a.map.W + pose->o[0].cu0;
-                ++words;
-            }
-            const unsigned o = e * (unsigned)B + j;                    // n_envs * B < 2^31 (fn_sim_create)
-            a.out_ranges[o] = r;
-            if (kAux && a.out_hit) a.out_hit[o] = hit;
-            if (a.ring_obs) {
-                unsigned long long slot = ring_head + (unsigned long long)e;   // both < ring_cap
-                if (slot >= a.ring_cap) slot -= a.ring_cap;
-                a.ring_obs[slot * a.ring_row + j] = r;
-            }
+            beam_element<MS, kFast, kAux>(a, bm, geo, s_tab, a.poses + e, e, j, ring_head, words);
             ++rays;
         }
         task = __shfl_sync(0xffffffffu, next, 0);

@@ -82,25 +82,8 @@ __global__ void __launch_bounds__(kFusedThreads, 2) reset_beam_kernel(ResetArgs 
         const unsigned j = idx - k * (unsigned)B;
         if (k < (unsigned)m_loc) {
             const unsigned e = (unsigned)ra.list[blockIdx.x + k * gridDim.x];
-                        const BeamPose* pose = k < (unsigned)kFusedPoseSlots ? s_pose + k : a.poses + e;
-            const int state = pose->state;
-            float r = 0.0f;
-            int hit = -2;
-            if (state == 0) {
-                if constexpr (!kAux) r = cast_beam_smem(bm, geo, pose, s_tab[j], a.robot.T, a.robot.rmax);
-                else r = cast_beam<SmemSpace, true>(bm, pose, s_tab[j], a.robot.T, a.map.rho, a.robot.rmax, &hit, words, false);
-            } else if (kAux) {
-                if (state == 1) hit = origin_line(bm, pose->o[0], true) * a.map.W + pose->o[0].cu0;
-                ++words;
-            }
-            const unsigned o = e * (unsigned)B + j;
-            a.out_ranges[o] = r;
-            if (kAux && a.out_hit) a.out_hit[o] = hit;
-            if (a.ring_obs) {
-                unsigned long long slot = ring_head + (unsigned long long)e;   // both < ring_cap
-                if (slot >= a.ring_cap) slot -= a.ring_cap;
-                a.ring_obs[slot * a.ring_row + j] = r;
-            }
+            const BeamPose* pose = k < (unsigned)kFusedPoseSlots ? s_pose + k : a.poses + e;
+            beam_element<SmemSpace, !kAux, kAux>(a, bm, geo, s_tab, pose, e, j, ring_head, words);
             ++rays;
         }
     }

@@ -203,8 +203,11 @@ def run_ours(args):
     rb = fn.Robot(wl.footprint, wl.beam_angles, float(wl.max_range), wl.drive, wl.vel_limits)
     sim = fn.Sim(m, rb, n, goal_tol=float(wl.goal_tol), max_episode_steps=wl.max_episode_steps,
                  goal_dist_min=float(wl.goal_dist_min), goal_dist_max=float(wl.goal_dist_max))
-    fused_active = sim.set_fused_reset(bool(args.fused_reset))
-    split_step = sim.set_split_step(bool(args.split_step))
+    if args.fused_reset >= 0:
+        sim.set_fused_reset(args.fused_reset)
+    if args.split_step >= 0:
+        sim.set_split_step(bool(args.split_step))
+    fused_active, split_step = sim.beam_config()["fused_reset"], sim.beam_config()["split_step"]
     states = torch.zeros(8, n, device="cuda")
     mask = torch.ones(n, dtype=torch.uint8, device="cuda")
     ranges = torch.zeros(n, B, device="cuda")
@@ -528,10 +531,10 @@ def main():
     ap.add_argument("--paper-query", type=int, default=1, help="also time the paper's fixed-step range query (information only)")
     ap.add_argument("--features", type=int, default=36, help="sectors of the clearance-feature leg (0 = skip; information only)")
     ap.add_argument("--graph", type=int, default=1, help="also time a CUDA-graph replay of the steps (information only)")
-    ap.add_argument("--fused-reset", type=int, default=1, choices=[0, 1],
-                    help="fn_reset as one fused kernel where possible (default) or as two kernels (0)")
-    ap.add_argument("--split-step", type=int, default=1, choices=[0, 1],
-                    help="fn_step with the env step split around the beam kernel where possible (default) or one env-step kernel (0)")
+    ap.add_argument("--fused-reset", type=int, default=-1, choices=[-1, 0, 1],
+                    help="fn_reset(done list) as one fused kernel (1) or two kernels (0); -1 = the library's default")
+    ap.add_argument("--split-step", type=int, default=-1, choices=[-1, 0, 1],
+                    help="fn_step with the env step split around the beam kernel (1) or one env-step kernel (0); -1 = the library's default")
     ap.add_argument("--ring", type=int, default=1, help="attach the replay ring when the config has one (C5)")
     args = ap.parse_args()
     if args.warmup < 3:

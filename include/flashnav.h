@@ -192,8 +192,9 @@ int fn_eval_end(fn_sim* sim);
  * both variants give the same ranges.  Overwrites the sim's sensing poses (like fn_observe_all). */
 int fn_ranges_fixed_step(fn_sim* sim, const float* states_dev, float delta_m, int blockwise, float* out_ranges_dev);
 
-/* ---- launch configuration of the beam kernel chosen at fn_sim_create (for reports): cfg_out[4] =
- * {map staged in shared memory (1) or read through L1/L2 (0), grid size, CTA size, dynamic shared bytes}. */
+/* ---- launch configuration chosen at fn_sim_create or by the switches below (for reports): cfg_out[6] =
+ * {map staged in shared memory (1) or read through L1/L2 (0), beam grid size, CTA size, dynamic shared bytes,
+ *  split step in use (fn_sim_set_split_step), fused reset in use for done lists (fn_sim_set_fused_reset)}. */
 int fn_sim_beam_config(const fn_sim* sim, int* cfg_out);
 
 /* ---- fn_reset as one launch or two.  When the packed map is staged in shared memory (cfg_out[0] of

@@ -336,9 +336,10 @@ class Sim:
         return d, e
 
     def beam_config(self) -> dict:
-        cfg = np.zeros(4, np.int32)
+        cfg = np.zeros(6, np.int32)
         _check(load_library().fn_sim_beam_config(self._h, _np_ptr(cfg)), "fn_sim_beam_config")
-        return {"smem": bool(cfg[0]), "grid": int(cfg[1]), "block": int(cfg[2]), "smem_bytes": int(cfg[3])}
+        return {"smem": bool(cfg[0]), "grid": int(cfg[1]), "block": int(cfg[2]), "smem_bytes": int(cfg[3]),
+                "split_step": bool(cfg[4]), "fused_reset": bool(cfg[5])}
 
     def set_fused_reset(self, enable) -> bool:
         """fn_reset(mask=None) as one fused kernel (1 / True, default where possible), never (0 / False), or for

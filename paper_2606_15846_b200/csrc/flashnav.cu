@@ -824,6 +824,7 @@ extern "C" int fn_sim_profile_read(fn_sim* s, double* ms_out, uint64_t* launches
 extern "C" int fn_sim_beam_config(const fn_sim* s, int* cfg) {
     if (!s || !cfg) return fail(FN_ERR_INVALID_ARG, "fn_sim_beam_config: NULL argument");
     cfg[0] = s->use_smem ? 1 : 0; cfg[1] = s->beam_grid; cfg[2] = 512; cfg[3] = (int)s->beam_smem;
+    cfg[4] = s->split_on ? 1 : 0; cfg[5] = s->fused_on ? 1 : 0;
     return FN_OK;
 }
 

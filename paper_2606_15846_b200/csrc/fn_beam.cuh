@@ -455,22 +455,39 @@ __device__ __forceinline__ void beam_element(const BeamArgs& a, const BeamMap<MS
 
 // Stages the beam table and (when `stage`) both packed copies of the map in shared memory: constants, so
 // the kernels do this BEFORE their dependency wait, under the kernel that precedes them in the stream.
-// All threads of the CTA call; the caller synchronises.
+// The copy is done by the TMA engine: one thread arms an mbarrier with the byte count and issues 1-D bulk
+// copies (cp.async.bulk, global -> shared), every thread then waits on the barrier's phase -- no registers,
+// no LDG/STS instructions, and the SM's other CTA keeps its issue slots.  All threads of the CTA call; mbar =
+// an 8-byte shared word of the caller, used once per launch.
 __device__ __forceinline__ void stage_beam_constants(const BeamArgs& a, double2* s_tab, uint32_t* s_map,
-                                                     const int mapWords, const bool stage) {
-    for (int i = threadIdx.x; i < a.robot.B; i += blockDim.x) s_tab[i] = a.robot.beam_cs[i];
-    if (stage) {
-        const uint4* src = reinterpret_cast<const uint4*>(a.map.row);      // row and col copies are contiguous
-        uint4* dst = reinterpret_cast<uint4*>(s_map);
-        const int n4 = (mapWords + 3) / 4;
-        int i = threadIdx.x;
-        for (; i + 3 * (int)blockDim.x < n4; i += 4 * blockDim.x) {         // 4 loads in flight per thread
-            const uint4 v0 = __ldg(src + i), v1 = __ldg(src + i + blockDim.x);
-            const uint4 v2 = __ldg(src + i + 2 * blockDim.x), v3 = __ldg(src + i + 3 * blockDim.x);
-            dst[i] = v0; dst[i + blockDim.x] = v1; dst[i + 2 * blockDim.x] = v2; dst[i + 3 * blockDim.x] = v3;
-        }
-        for (; i < n4; i += blockDim.x) dst[i] = __ldg(src + i);
+                                                     const int mapWords, const bool stage, unsigned long long* mbar) {
+    const uint32_t mb = (uint32_t)__cvta_generic_to_shared(mbar);
+    if (threadIdx.x == 0) {
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(mb));
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        const uint32_t tab_bytes = (uint32_t)a.robot.B * (uint32_t)sizeof(double2);
+        const uint32_t map_bytes = stage ? ((uint32_t)mapWords * 4u) & ~15u : 0u;     // bulk copies move 16-byte units
+        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mb), "r"(tab_bytes + map_bytes) : "memory");
+        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                     ::"r"((uint32_t)__cvta_generic_to_shared(s_tab)), "l"(a.robot.beam_cs), "r"(tab_bytes), "r"(mb) : "memory");
+        const uint32_t dst = (uint32_t)__cvta_generic_to_shared(s_map);
+        const uint8_t* src = reinterpret_cast<const uint8_t*>(a.map.row);              // row and col copies are contiguous
+        for (uint32_t off = 0; off < map_bytes; off += 32768u) {
+            const uint32_t sz = min(32768u, map_bytes - off);
+            asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                         ::"r"(dst + off), "l"(src + off), "r"(sz), "r"(mb) : "memory");
+        }
+        if (stage) for (int i = (int)(map_bytes >> 2); i < mapWords; ++i) s_map[i] = __ldg(a.map.row + i);   // < 16 bytes
+    }
+    // phase 0 completes when the armed byte count has arrived
+    uint32_t done = 0;
+    for (int it = 0; it < (1 << 24) && !done; ++it)
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], 0;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(done) : "r"(mb) : "memory");
+    if (!done) __trap();                                           // (never: a lost copy must not hang the device)
 }
 
 // The warps of the (persistent) grid take 32 consecutive (env, beam) pairs at a time: adjacent lanes =
@@ -542,7 +559,8 @@ __global__ void __launch_bounds__(512, 2) beam_kernel(BeamArgs a) {
     const int mapWords = (a.map.H + 2 * kLineGuard) * a.map.strideR + (a.map.W + 2 * kLineGuard) * a.map.strideC;
     double2* s_tab = reinterpret_cast<double2*>(smem_raw);
     uint32_t* s_map = reinterpret_cast<uint32_t*>(smem_raw + (size_t)B * sizeof(double2));
-    stage_beam_constants(a, s_tab, s_map, mapWords, stage);
+    __shared__ __align__(8) unsigned long long s_mbar;
+    stage_beam_constants(a, s_tab, s_map, mapWords, stage, &s_mbar);
     __syncthreads();
     griddep_wait();                                                // poses / list / count come from the previous kernel
     griddep_launch_dependents();

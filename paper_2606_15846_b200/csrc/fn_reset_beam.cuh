@@ -38,7 +38,8 @@ __global__ void __launch_bounds__(kFusedThreads, 2) reset_beam_kernel(ResetArgs 
     BeamPose* s_pose = reinterpret_cast<BeamPose*>(smem_raw + fused_scratch_offset(B, mapWords));
     uint8_t* s_scr = reinterpret_cast<uint8_t*>(s_pose + kFusedPoseSlots);
     const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    stage_beam_constants(a, s_tab, s_map, mapWords, true);
+    __shared__ __align__(8) unsigned long long s_mbar;
+    stage_beam_constants(a, s_tab, s_map, mapWords, true, &s_mbar);
     ColScratch scratch = col_scratch(s_scr + (size_t)(wib < kFusedResetWarps ? wib : 0) * col_scratch_bytes(V), V);
     if (wib < kFusedResetWarps)
         for (int k = lane; k < V; k += 32) { scratch.verts[k] = a.robot.verts[k]; scratch.nxt[k] = a.robot.nxt[k]; }

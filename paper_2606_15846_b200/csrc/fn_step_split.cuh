@@ -49,7 +49,8 @@ __global__ void __launch_bounds__(512, 2) step_beam_kernel(BeamArgs a, EnvArgs e
     double2* s_tab = reinterpret_cast<double2*>(smem_raw);
     uint32_t* s_map = reinterpret_cast<uint32_t*>(smem_raw + (size_t)B * sizeof(double2));
     const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31, last_warp = (int)(blockDim.x >> 5) - 1;
-    stage_beam_constants(a, s_tab, s_map, mapWords, kSmem);
+    __shared__ __align__(8) unsigned long long s_mbar;
+    stage_beam_constants(a, s_tab, s_map, mapWords, kSmem, &s_mbar);
     const ColScratch scratch = col_scratch(smem_raw + step_split_scratch_offset(beam_smem), V);
     if (wib == last_warp)
         for (int k = lane; k < V; k += 32) { scratch.verts[k] = a.robot.verts[k]; scratch.nxt[k] = a.robot.nxt[k]; }

@@ -33,8 +33,8 @@ from harness import workloads as W  # noqa: E402
 # dominant kernel (full-batch beam launch), per launch, from the committed ncu --set full capture
 NCU_CAPTURE = {(2, False): {"dram_bytes": 506624, "warp_inst": 45733853, "lanes": 22.05,
                             "source": "profiles/r1e_beam_kernels_full_c2.txt (dram__bytes_read.sum + dram__bytes_write.sum)"},
-               (2, True): {"dram_bytes": 720896, "warp_inst": 46700700, "lanes": 22.10,
-                           "source": "profiles/r1f_beam_kernels_full_c2.txt (dram__bytes_read.sum + dram__bytes_write.sum)"}}
+               (2, True): {"dram_bytes": 719360, "warp_inst": 45982954, "lanes": 22.11,
+                           "source": "profiles/r1g_beam_kernels_full_c2.txt (dram__bytes_read.sum + dram__bytes_write.sum)"}}
 
 METRIC = "env_steps_per_s"
 UNIT = "env-steps/s"

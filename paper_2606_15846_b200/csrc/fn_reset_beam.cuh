@@ -8,8 +8,9 @@
 // like beam_kernel), owns the listed envs li = blockIdx.x + k * gridDim.x, resets them from the SHARED
 // copy of the map (reset_env<true>: the same code as reset_kernel, so the accepted poses are identical),
 // and then casts the beams of its own envs.  No CTA reads another CTA's poses, so a block barrier is the
-// only synchronisation.  Used when the map is staged in shared memory; otherwise fn_reset launches the
-// two kernels.
+// only synchronisation.  Used for fn_reset(mask = NULL), the step's done list, when the map is staged in
+// shared memory; a caller's mask (long lists: two reset warps per CTA and no balancing of the beams across
+// CTAs lose there) and maps read through L2 take the two kernels.
 #pragma once
 #include "fn_beam.cuh"
 #include "fn_env.cuh"

@@ -521,7 +521,17 @@ static BeamArgs beam_args(fn_sim* s, const int* list, const int* count_dev, floa
     b.list_par_dev = done_list ? s->d_done_count + 2 : nullptr;
     b.exp_off = kExpOff;
     b.pair_lines = (double)s->robot->rmax / (double)s->map->res >= 110.0;     // beams of >~ 16 lines on average
-    b.inv_bitsR = 1.0f / (float)(32 * s->map->dev.strideR); b.inv_bitsC = 1.0f / (float)(32 * s->map->dev.strideC);
+    {   // ceil(2^32 / S) for S = bits per line (FastOrient::inv_magic)
+        const unsigned long long SR = 32ull * (unsigned long long)s->map->dev.strideR, SC = 32ull * (unsigned long long)s->map->dev.strideC;
+        b.inv_magicR = (unsigned)(((1ull << 32) + SR - 1) / SR); b.inv_magicC = (unsigned)(((1ull << 32) + SC - 1) / SC);
+    }
+    fast_chunking(s->robot->B, &b.chunk_rounds, &b.nchunk);
+    {
+        const unsigned long long rounds = ((unsigned long long)s->robot->B + 31) >> 5;
+        b.inv_nchunk = fast_magic((unsigned long long)b.nchunk, (unsigned long long)s->n * b.nchunk);
+        b.inv_rounds = fast_magic(rounds, (unsigned long long)s->n * rounds);
+    }
+    b.half_T = 0.5 * b.robot.T;
     return b;
 }
 

@@ -118,48 +118,50 @@ __device__ __noinline__ BeamHit cast_beam_slow(const BeamMap<MS> bm, const BeamO
     const double M = adw > 0.0 ? M_in : INFINITY;
     const double Tu = T * adu;                                    // travel along u at the range limit
     typename MS::addr_t line = MS::addb(bm.base, (int)o.line_off);
+    const int lstep = fw ? stride4 : -stride4;
     int l = origin_line(bm, o, mx);
-    double E = ou;                                                // entry coordinate of the current line
-    for (int k = 0;; ++k) {
-        double X = fu ? ou + (f + (double)k) * M : ou - (f + (double)k) * M;        // exit coordinate
+    BeamHit h;
+    h.r = rmax; h.hit = -1;
+    // ONE flat loop whose trip is "one 32-bit word of the current line" (a walk nested as lines x words made
+    // the lanes of a warp drift apart: every lane then ran its own inner loop alone)
+    double E = ou, X;                                             // entry / exit coordinate of the current line
+    int k = 0, ce, cx, c;
+    bool last;
+    auto enter_line = [&]() {
+        X = fu ? ou + (f + (double)k) * M : ou - (f + (double)k) * M;
         if (!(X > -1.0)) X = -0.5;                                // clamp into the frame cells (also NaN/inf)
         if (!(X < (double)Wu + 1.0)) X = (double)Wu + 0.5;
-        const bool last = !(fabs(X - ou) < Tu);                   // the range limit lies in this line
-        const int ce = __double2int_rd(E), cx = __double2int_rd(X);
-        int c = ce, found = 0;
-        if (fu) {
-            while (c <= cx) {
-                const int q = c + kCellShift;
-                const uint32_t w = MS::ld(MS::addb(line, (q >> 5) << 2)) >> (q & 31);
-                if (w) { c += __ffs(w) - 1; found = c <= cx; break; }
-                c += 32 - (q & 31);
-            }
-        } else {
-            while (c >= cx) {
-                const int q = c + kCellShift;
-                const uint32_t w = MS::ld(MS::addb(line, (q >> 5) << 2)) << (31 - (q & 31));
-                if (w) { c -= __clz(w); found = c >= cx; break; }
-                c -= (q & 31) + 1;
-            }
-        }
-        if (found) {
+        last = !(fabs(X - ou) < Tu);                              // the range limit lies in this line
+        ce = __double2int_rd(E); cx = __double2int_rd(X);
+        c = ce;
+    };
+    enter_line();
+    for (;;) {
+        const int q = c + kCellShift;
+        uint32_t w = MS::ld(MS::addb(line, (q >> 5) << 2));
+        int cn;
+        bool found;
+        if (fu) { w >>= (q & 31); cn = w ? c + __ffs(w) - 1 : c + 32 - (q & 31); found = w != 0u && cn <= cx; }
+        else { w <<= 31 - (q & 31); cn = w ? c - __clz(w) : c - (q & 31) - 1; found = w != 0u && cn >= cx; }
+        if (found) {                                              // first occupied cell of the line's span
+            c = cn;
             double dU;
             if (c == ce) dU = fabs(E - ou);                       // entered through the line boundary (or origin)
             else dU = fu ? (double)c - ou : ou - (double)(c + 1);
-            if (!(dU < Tu)) break;
-            BeamHit h;
-            h.r = range_from_du(dU, range_scale(adu, rho));
-            const bool outside = (unsigned)c >= (unsigned)Wu || (unsigned)l >= (unsigned)Hw;
-            h.hit = outside ? -2 : (mx ? l * bm.W + c : c * bm.W + l);
-            return h;
+            if (dU < Tu) {
+                h.r = range_from_du(dU, range_scale(adu, rho));
+                const bool outside = (unsigned)c >= (unsigned)Wu || (unsigned)l >= (unsigned)Hw;
+                h.hit = outside ? -2 : (mx ? l * bm.W + c : c * bm.W + l);
+            }
+            break;
         }
-        if (last) break;
-        E = X;
+        if (w == 0u && (fu ? cn <= cx : cn >= cx)) { c = cn; continue; }   // next word of the same line
+        if (last) break;                                          // the line's span is free
+        E = X; ++k;
         l += fw ? 1 : -1;
-        line = MS::addb(line, fw ? stride4 : -stride4);
+        line = MS::addb(line, lstep);
+        enter_line();
     }
-    BeamHit h;
-    h.r = rmax; h.hit = -1;
     return h;
 }
 
@@ -282,8 +284,8 @@ __device__ __forceinline__ float cast_beam(const BeamMap<MS>& bm, const BeamPose
     return r;
 }
 
-// ---- one beam on the shared-memory map, production path.  Same arithmetic as cast_beam (all of it is
-// exact fixed point, so both agree bit for bit), but the line is carried INSIDE D as well: the integer
+// ---- production path on the shared-memory map (fn_beam_fast below).  Same arithmetic as cast_beam (all of
+// it is exact fixed point, so both agree bit for bit), but the line is carried INSIDE D as well: the integer
 // field of D (20 bits) holds the beam's BIT offset in its copy of the map, 8 * (byte offset of the line) + 64 + cell,
 // and the per-line increment is +-M +- S (S = bits per line).  One DADD per line then advances the
 // crossing coordinate and the line together, the window address is base + 4 * (high word >> 5), and the
@@ -291,112 +293,153 @@ __device__ __forceinline__ float cast_beam(const BeamMap<MS>& bm, const BeamPose
 // needs no line pointer and no counter.  Two lines per trip (independent loads hide the shared-memory
 // latency): 2 DADD, 2 x [SHF (word index), LEA (address), 2 LDS, SHF.W (window)], one LOP3 for
 // ((xa | xb) & mask) != 0, one ISETP (last pair), BRA = 15 SASS instructions per two lines.
-struct SmemGeo {
-    uint32_t baseR, baseC;   // shared addresses of the row / column copy, - kExpOff
-    float rho;
-    int bitsR, bitsC;        // S: bits per line of the row / column copy
-    float inv_bitsR, inv_bitsC;
+//
+// Everything a beam needs besides its own direction sits in a 128-byte slot of shared memory owned by the
+// warp (FastSlot): the heading and, per dominant axis, the origin (h, ouMS) and the constants of the copy.
+// A beam selects its axis by ONE address and reads 16-byte records at fixed offsets from it -- no global
+// pointers, no 64-bit address arithmetic and nothing to rematerialise in the per-beam code.
+struct __align__(16) FastAxis {                                  // 48 bytes
+    double h, ouMS;          // BeamOrient::h, ::ouMS of the env being cast (rewritten per task)
+    double Sd;               // S: bits per line of the copy, as a double
+    uint32_t base;           // shared address of the copy - kExpOff
+    uint32_t half_S;         // S / 2
+    uint32_t inv_magic;      // ceil(2^32 / S): lines crossed k = umulhi(field difference + S / 2, inv_magic), exact
+    uint32_t S;
+    uint32_t pad_[2];
 };
+struct __align__(16) FastSlot {                                  // 128 bytes per warp
+    double pc, ps;           // cos / sin of the heading (rewritten per task)
+    FastAxis ax[2];          // [0] u = x (row copy), [1] u = y (column copy)
+    uint32_t pad_[4];
+};
+constexpr int kNearQueue = 64;                                   // per warp: deferred near-axis beams
+constexpr int kFastWarps = 16;                                   // warps per CTA of the kernels that use the production path
 
-__device__ __forceinline__ float cast_beam_smem(const BeamMap<SmemSpace>& bm, const SmemGeo& g,
-                                                const BeamPose* __restrict__ pose, const double2 cs,
-                                                const double T, const float rmax) {
-    const double2 pcs = *reinterpret_cast<const double2*>(&pose->c);
+__device__ __forceinline__ double xor_hi(double v, unsigned m) { return __hiloint2double((int)(hiw(v) ^ m), __double2loint(v)); }
+__device__ __forceinline__ double add_hi(double v, unsigned k) { return __hiloint2double((int)(hiw(v) + k), __double2loint(v)); }
+// a value the compiler must keep in its register (it would otherwise rebuild shared addresses per use)
+__device__ __forceinline__ uint32_t opaque(uint32_t v) { asm volatile("mov.b32 %0, %0;" : "+r"(v)); return v; }
+__device__ __forceinline__ double2 lds_d2(uint32_t addr) {
+    double2 v;
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr));
+    return v;
+}
+
+// One beam per lane.  slot = shared address of the warp's FastSlot; tab = shared address of the beam's
+// (cos, sin) entry.  near = the beam is within 1.9 deg of an axis (M >= 30.5): not cast here, the caller
+// defers it (fast_chunk / fast_drain).
+__device__ __forceinline__ float cast_beam_fast(const uint32_t slot, const uint32_t tab,
+                                                const double T, const double half_T, const float rho, const float rmax, bool& near) {
+    const double2 cs = lds_d2(tab), pcs = lds_d2(slot);
     const double dx = pcs.x * cs.x - pcs.y * cs.y, dy = pcs.y * cs.x + pcs.x * cs.y;
     const bool mx = fabs(dx) >= fabs(dy);                         // dominant axis is x
-    const BeamOrient o = pose->o[mx ? 0 : 1];
     const double du = mx ? dx : dy, dw = mx ? dy : dx;
-    const double adu = fabs(du), adw = fabs(dw);
+    const double adw = __hiloint2double((int)(hiw(dw) & 0x7fffffffu), __double2loint(dw));
     const double r0 = rcp64h(adw);
     const double r1 = fma(fma(-adw, r0, 1.0), r0, r0);
-    const double M = adu * r1;
-    if (!(M < kSlowSlope)) return cast_beam_slow<SmemSpace>(bm, o, mx, du, dw, M, T, g.rho, rmax).r;
-    const unsigned su = hiw(du) & 0x80000000u, sw = hiw(dw) & 0x80000000u;   // sign bits: set = backward
-    const unsigned fu1 = (su >> 31) ^ 1u;
-    const double Mm = M + kMagic, Mq = Mm - kMagic;
-    const double Mu = __hiloint2double((int)(hiw(Mq) ^ su), __double2loint(Mq));      // +-M along u
-    const double f = __hiloint2double((int)(hiw(o.h) ^ sw), __double2loint(o.h)) + 0.5;
-    const int S = mx ? g.bitsR : g.bitsC;
-    const double Sd = (double)S;                                  // (uniform: converted once per warp task)
-    const double Md = Mu + __hiloint2double((int)(hiw(Sd) ^ sw), __double2loint(Sd)); // +-M +- S per line
-    const double Md2 = Md + Md;
-    // D of line 0 = 2^20 + bit offset of the origin's line + 64 + U_1 (+ 1 forward)
-    const double D0f = fma(f, Mu, o.ouMS);
-    const double D0 = __hiloint2double((int)(hiw(D0f) + fu1), __double2loint(D0f));
-    const unsigned sh = 30u - hiw(Mm);
-    const uint32_t mask = su ? __funnelshift_r(0xffffffffu, 0u, sh) : __funnelshift_l(0u, 0xffffffffu, sh);
-    // P pairs of lines cover floor(T |dw|) + 2 lines; the frame stops beams that leave the map earlier
-    const double Pd = fma(0.5 * T, adw, 1.5 + 4503599627370496.0) - 4503599627370496.0;
-    double D = D0 - Md;                                           // rotated loop: the increments lead
-    const uint32_t hend = hiw(fma(Pd, Md2, D));                   // high word of the last pair's second line
-    const uint32_t base = (mx ? g.baseR : g.baseC) - (fu1 << 2);  // forward: the window ENDS at the exit cell
-    const float scale = range_scale(adu, g.rho);
-    const double Tu = T * adu;
+    const double M = fabs(du) * r1;
+    near = !(M < kSlowSlope);                                     // also dw == 0 (M = inf or NaN)
     float r = rmax;
-    for (;;) {
-        uint32_t xa, xb;
-        asm volatile(
-            "{\n\t"
-            ".reg .pred ph, pc;\n\t"
-            ".reg .b32 j, a, L, H, lo, hia, hib, xo;\n\t"
-            ".reg .f64 DA;\n\t"
-            "FN_LOOP:\n\t"
-            "add.f64 DA, %0, %3;\n\t"
-            "add.f64 %0, %0, %4;\n\t"
-            "mov.b64 {lo, hia}, DA;\n\t"
-            "shr.u32 j, hia, 5;\n\t"
-            "mad.lo.u32 a, j, 4, %5;\n\t"
-            "ld.shared.u32 L, [a];\n\t"
-            "ld.shared.u32 H, [a+4];\n\t"
-            "shf.r.wrap.b32 %1, L, H, hia;\n\t"
-            "mov.b64 {lo, hib}, %0;\n\t"
-            "shr.u32 j, hib, 5;\n\t"
-            "mad.lo.u32 a, j, 4, %5;\n\t"
-            "ld.shared.u32 L, [a];\n\t"
-            "ld.shared.u32 H, [a+4];\n\t"
-            "shf.r.wrap.b32 %2, L, H, hib;\n\t"
-            "or.b32 xo, %1, %2;\n\t"
-            "and.b32 xo, xo, %7;\n\t"
-            "setp.eq.u32 ph, xo, 0;\n\t"
-            "setp.ne.and.u32 pc, hib, %6, ph;\n\t"
-            "@pc bra FN_LOOP;\n\t"
-            "}"
-            : "+d"(D), "=r"(xa), "=r"(xb)
-            : "d"(Md), "d"(Md2), "r"(base), "r"(hend), "r"(mask));
-        xa &= mask;
-        xb &= mask;
-        // up to two candidate lines, in travel order: the pair's first line (D - Md), then its second (D)
-        uint32_t x = xa;
-        double Dl = D - Md;
-        if (x == 0u) { x = xb; xb = 0u; Dl = D; }
-        bool fin = false;
+    // (a near-axis lane stays with the warp: it walks one pair of lines of a harmless beam of slope 1 and its
+    // result is dropped, so that the whole warp reaches the resolution below converged)
+    {
+        const double Mc = near ? 1.0 : M;
+        const uint32_t ax = slot + (mx ? 16u : 64u);              // the axis record
+        const double2 hq = lds_d2(ax);                            // (h, ouMS)
+        double Sd;
+        uint32_t g2, g3;
+        asm volatile("ld.shared.v2.u32 {%0, %1}, [%2+24];" : "=r"(g2), "=r"(g3) : "r"(ax));
+        asm volatile("ld.shared.f64 %0, [%1+16];" : "=d"(Sd) : "r"(ax));
+        const unsigned su = hiw(du) & 0x80000000u, sw = hiw(dw) & 0x80000000u;   // sign bits: set = backward
+        const unsigned fu1 = (su >> 31) ^ 1u;
+        const double Mm = Mc + kMagic, Mq = Mm - kMagic;         // M on the 2^-32 grid of D
+        const double Mu = xor_hi(Mq, su);                         // +-M along u
+        const double f = xor_hi(hq.x, sw) + 0.5;                  // distance to the first line boundary, in lines
+        const double Md = Mu + xor_hi(Sd, sw);                    // +-M +- S per line
+        const double Md2 = Md + Md;
+        // D of line 0 = 2^20 + bit offset of the origin's line + 64 + U_1 (+ 1 forward)
+        const double D0 = add_hi(fma(f, Mu, hq.y), fu1);
+        const unsigned sh = 30u - hiw(Mm);
+        const uint32_t mask = su ? __funnelshift_r(0xffffffffu, 0u, sh) : __funnelshift_l(0u, 0xffffffffu, sh);
+        // P pairs of lines cover floor(T |dw|) + 2 lines; the frame stops beams that leave the map earlier
+        const double Pd = near ? 1.0 : fma(half_T, adw, 1.5 + 4503599627370496.0) - 4503599627370496.0;
+        double D = D0 - Md;                                       // rotated loop: the increments lead
+        const uint32_t hend = hiw(fma(Pd, Md2, D));               // high word of the last pair's second line
+        const uint32_t base = g2 - (fu1 << 2);                    // forward: the window ENDS at the exit cell
+        const uint32_t h0 = hiw(D0), hc0 = hiw(hq.y);             // fields of line 0 and of the origin cell
+        double Dh = 0.0;                                          // the hit line's D and exact window (xh != 0: hit)
+        uint32_t xh = 0u;
+        for (;;) {
+            uint32_t xa, xb;
+            asm volatile(
+                "{\n\t"
+                ".reg .pred ph, pc;\n\t"
+                ".reg .b32 j, a, L, H, lo, hia, hib, xo;\n\t"
+                ".reg .f64 DA;\n\t"
+                "FN_LOOP:\n\t"
+                "add.f64 DA, %0, %3;\n\t"
+                "add.f64 %0, %0, %4;\n\t"
+                "mov.b64 {lo, hia}, DA;\n\t"
+                "shr.u32 j, hia, 5;\n\t"
+                "mad.lo.u32 a, j, 4, %5;\n\t"
+                "ld.shared.u32 L, [a];\n\t"
+                "ld.shared.u32 H, [a+4];\n\t"
+                "shf.r.wrap.b32 %1, L, H, hia;\n\t"
+                "mov.b64 {lo, hib}, %0;\n\t"
+                "shr.u32 j, hib, 5;\n\t"
+                "mad.lo.u32 a, j, 4, %5;\n\t"
+                "ld.shared.u32 L, [a];\n\t"
+                "ld.shared.u32 H, [a+4];\n\t"
+                "shf.r.wrap.b32 %2, L, H, hib;\n\t"
+                "or.b32 xo, %1, %2;\n\t"
+                "and.b32 xo, xo, %7;\n\t"
+                "setp.eq.u32 ph, xo, 0;\n\t"
+                "setp.ne.and.u32 pc, hib, %6, ph;\n\t"
+                "@pc bra FN_LOOP;\n\t"
+                "}"
+                : "+d"(D), "=r"(xa), "=r"(xb)
+                : "d"(Md), "d"(Md2), "r"(base), "r"(hend), "r"(mask));
+            // up to two candidate lines, in travel order: the pair's first line (D - Md), then its second (D).
+            // Only the exact-span test runs here (per loop exit); the hit itself is resolved once, below.
+            uint32_t x = xa & mask, xn = xb & mask;
+            double Dl = D - Md;
+            if (x == 0u) { x = xn; xn = 0u; Dl = D; }
 #pragma unroll 1
-        while (x != 0u) {
-            // exact span [entry cell ce, exit cell cx] of this line (origin cell in the first line)
-            const uint32_t hl = hiw(Dl);
-            const bool first = hl == hiw(D0);
-            const int cx = (int)(hl - fu1);
-            const double Dp = Dl - Mu;                            // entry crossing, same line field
-            const int ce = first ? (int)hiw(o.ouMS) : (int)(hiw(Dp) - fu1);   // hiw(ouMS) = field of the origin cell
-            const unsigned n = 31u - (unsigned)abs(cx - ce);
-            const uint32_t xe = x & (su ? __funnelshift_r(0xffffffffu, 0u, n) : __funnelshift_l(0u, 0xffffffffu, n));
-            if (xe != 0u) {
-                // first occupied cell in travel order: highest bit backward, lowest bit forward
-                const int c = cx - (int)(fu1 * 31u) + (31 - __clz(su ? xe : xe & (0u - xe)));
-                // lines crossed: the integer fields of line k and line 0 differ by +-k S +- (cells along u)
-                const int dq = sw ? (int)(hiw(D0) - hl) : (int)(hl - hiw(D0));
-                const int k = __float2int_rd(fmaf((float)dq, mx ? g.inv_bitsR : g.inv_bitsC, 0.5f));
-                const int lf = sw ? -k * S : k * S;                // line field of line k relative to line 0
-                double dU;
-                if (c == ce) dU = first ? 0.0 : fabs((Dp - (double)lf) - (o.ouMS + (double)fu1));
-                else dU = fabs((double)(c + (int)(su >> 31) - lf - (int)kMagicHi) - (o.ouMS - kMagic));
-                if (dU < Tu) r = range_from_du(dU, scale);
-                fin = true;                                       // later lines are farther away
-                break;
+            while (x != 0u) {
+                // exact span [entry cell ce, exit cell cx] of this line (origin cell in the first line)
+                const uint32_t hl = hiw(Dl);
+                const int cx = (int)(hl - fu1);
+                const int ce = hl == h0 ? (int)hc0 : (int)(hiw(Dl - Mu) - fu1);
+                const unsigned n = 31u - (unsigned)abs(cx - ce);
+                const uint32_t xe = x & (su ? __funnelshift_r(0xffffffffu, 0u, n) : __funnelshift_l(0u, 0xffffffffu, n));
+                if (xe != 0u) { xh = xe; Dh = Dl; break; }
+                x = xn; xn = 0u; Dl = D;                          // the extra cell behind the entry: next line / resume
             }
-            x = xb; xb = 0u; Dl = D;                              // the extra cell behind the entry: resume
+            if (xh != 0u || hiw(D) == hend) break;
         }
-        if (fin || hiw(D) == hend) break;
+        __syncwarp();                                             // resolve all hits of the warp together
+        if (xh != 0u) {                                           // later lines are farther away
+            const uint32_t hl = hiw(Dh);
+            const bool first = hl == h0;
+            const int cx = (int)(hl - fu1);
+            const double Dp = Dh - Mu;                            // entry crossing, same line field
+            const int ce = first ? (int)hc0 : (int)(hiw(Dp) - fu1);
+            // first occupied cell in travel order: highest bit backward, lowest bit forward
+            const int c = cx - (int)(fu1 * 31u) + (31 - __clz(su ? xh : xh & (0u - xh)));
+            // lines crossed: the integer fields of line k and line 0 differ by +-k S +- (cells along u)
+            uint32_t half_S, inv_magic, S;
+            asm volatile("ld.shared.u32 %0, [%1+28];" : "=r"(half_S) : "r"(ax));
+            asm volatile("ld.shared.v2.u32 {%0, %1}, [%2+32];" : "=r"(inv_magic), "=r"(S) : "r"(ax));
+            const unsigned dq = sw ? h0 - hl : hl - h0;
+            const unsigned k = __umulhi(dq + half_S, inv_magic);
+            const unsigned lf = sw ? 0u - k * S : k * S;          // line field of line k relative to line 0
+            // entry distance along u: through the line boundary (c == ce) or through the cell's u-face
+            const double a = c == ce ? add_hi(Dp, 0u - lf) : __hiloint2double((int)((unsigned)c + (su >> 31) - lf), 0);
+            const double b = c == ce ? add_hi(hq.y, fu1) : hq.y;
+            const double dU = (c == ce && first) ? 0.0 : fabs(a - b);
+            const double adu = fabs(du);
+            if (dU < T * adu) r = range_from_du(dU, range_scale(adu, rho));
+        }
     }
     return r;
 }
@@ -420,25 +463,29 @@ struct BeamArgs {
                                  // hot loop's address arithmetic (4 extra instructions per two lines) instead of
                                  // keeping base - kExpOff in one register
     unsigned* task_counter;      // next warp task; zeroed by the kernel that precedes the beam kernel
-    float inv_bitsR, inv_bitsC;  // 1 / (bits per line) of the row / column copy (host-computed)
+    unsigned inv_magicR, inv_magicC;   // ceil(2^32 / bits per line) of the row / column copy (FastOrient::inv_magic)
+    double half_T;               // 0.5 * robot.T
+    int chunk_rounds, nchunk;    // production kernel: a warp task of the static part = chunk_rounds x 32 consecutive
+                                 // beams of one env, nchunk such tasks per env (host: fast_chunking); the tasks of the
+                                 // dynamic part are single rounds of 32 beams
+    unsigned inv_nchunk, inv_rounds;   // fast_magic(nchunk), fast_magic(rounds per env): t / d = umulhi(t, magic), or 0
     int* flip_par_dev;           // fn_step's launch: clears done_count[*par ^ 1] and flips *par (see EnvArgs)
     int* done_count;
     const int* list_par_dev;     // or NULL; else list += (*list_par_dev ^ 1) * n_all, count_dev += (*list_par_dev ^ 1)
     unsigned long long* counters;
 };
 
-// One (env, beam) element: cast, store the range (and, instrumented, the hit cell; with a ring, the obs part
-// of the env's pending ring row).  ring_head = slot of env 0's pending row.
-template <class MS, bool kFast, bool kAux>
-__device__ __forceinline__ void beam_element(const BeamArgs& a, const BeamMap<MS>& bm, const SmemGeo& geo,
+// One (env, beam) element of the instrumented / L2-path kernels: cast, store the range (and, instrumented, the
+// hit cell; with a ring, the obs part of the env's pending ring row).  ring_head = slot of env 0's pending row.
+template <class MS, bool kAux>
+__device__ __forceinline__ void beam_element(const BeamArgs& a, const BeamMap<MS>& bm,
                                              const double2* s_tab, const BeamPose* pose, const unsigned e, const unsigned j,
                                              const unsigned long long ring_head, uint32_t& words) {
     const int state = pose->state;
     float r = 0.0f;
     int hit = -2;
     if (state == 0) {
-        if constexpr (kFast) r = cast_beam_smem(bm, geo, pose, s_tab[j], a.robot.T, a.robot.rmax);
-        else r = cast_beam<MS, kAux>(bm, pose, s_tab[j], a.robot.T, a.map.rho, a.robot.rmax, &hit, words, a.pair_lines != 0);
+        r = cast_beam<MS, kAux>(bm, pose, s_tab[j], a.robot.T, a.map.rho, a.robot.rmax, &hit, words, a.pair_lines != 0);
     } else if (kAux) {
         if (state == 1) hit = origin_line(bm, pose->o[0], true) * a.map.W + pose->o[0].cu0;
         ++words;
@@ -450,6 +497,125 @@ __device__ __forceinline__ void beam_element(const BeamArgs& a, const BeamMap<MS
         unsigned long long slot = ring_head + (unsigned long long)e;   // both < ring_cap
         if (slot >= a.ring_cap) slot -= a.ring_cap;
         a.ring_obs[slot * a.ring_row + j] = r;
+    }
+}
+
+// ---- production kernel: warp tasks of chunk_rounds x 32 consecutive beams of ONE env.  What depends on the env
+// only (list entry, pose, output rows) is done once per task; near-axis beams are not cast in place (a
+// divergent walk over single words) but queued per warp and cast 32 at a time (fast_drain).
+struct FastShared {
+    FastSlot slot[kFastWarps];
+    uint32_t queue[kFastWarps][kNearQueue];                        // deferred beams: output offsets e * B + j
+};
+struct FastWarp {
+    uint32_t slot;               // shared address of the warp's FastSlot
+    uint32_t tab;                // shared address of the beam table
+    uint32_t tab_last;           // ... and of its last entry
+    uint32_t queue;              // shared address of the warp's queue
+    uint32_t map_base;           // shared address of the staged map (for the deferred beams)
+    unsigned qn;                 // entries queued (warp-uniform)
+    unsigned rays;               // beams cast by this warp (warp-uniform)
+};
+__host__ __device__ inline void fast_chunking(int B, int* chunk_rounds, int* nchunk) {
+    const int rounds = (B + 31) >> 5;
+    *nchunk = (rounds + 3) >> 2;                                   // about 4 rounds = 128 beams per task
+    *chunk_rounds = (rounds + *nchunk - 1) / *nchunk;
+}
+// magic = ceil(2^32 / d) gives t / d = umulhi(t, magic) exactly for all t < t_max when t_max * d <= 2^32; else 0 (divide)
+inline unsigned fast_magic(unsigned long long d, unsigned long long t_max) {
+    if (d <= 1 || t_max * d > (1ull << 32)) return 0u;
+    return (unsigned)(((1ull << 32) + d - 1) / d);
+}
+__device__ __forceinline__ float* ring_row_of(const BeamArgs& a, const unsigned long long ring_head, const unsigned e) {
+    if (!a.ring_obs) return nullptr;
+    unsigned long long slot = ring_head + (unsigned long long)e;   // both < ring_cap
+    if (slot >= a.ring_cap) slot -= a.ring_cap;
+    return a.ring_obs + slot * (unsigned long long)a.ring_row;
+}
+__device__ __forceinline__ FastWarp fast_warp(const BeamArgs& a, FastShared* fs, const double2* s_tab, const uint32_t map_base) {
+    const unsigned wib = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    FastWarp w;
+    w.slot = opaque((uint32_t)__cvta_generic_to_shared(&fs->slot[wib]));
+    w.tab = opaque((uint32_t)__cvta_generic_to_shared(s_tab));
+    w.tab_last = opaque(w.tab + 16u * ((unsigned)a.robot.B - 1u));
+    w.queue = opaque((uint32_t)__cvta_generic_to_shared(fs->queue[wib]));
+    w.map_base = map_base; w.qn = 0u; w.rays = 0u;
+    if (lane < 2) {                                                // the constants of the two copies
+        FastAxis* ax = &fs->slot[wib].ax[lane];
+        const unsigned rowBytes = (unsigned)(a.map.H + 2 * kLineGuard) * (unsigned)(a.map.strideR << 2);
+        const uint32_t S = (uint32_t)(lane ? a.map.strideC : a.map.strideR) << 5;
+        ax->Sd = (double)S; ax->base = map_base - a.exp_off + (lane ? rowBytes : 0u); ax->half_S = S >> 1;
+        ax->inv_magic = lane ? a.inv_magicC : a.inv_magicR; ax->S = S;
+    }
+    __syncwarp();
+    return w;
+}
+// casts n (<= 32) queued beams, one per lane (queue = shared address of the first of them)
+__device__ __noinline__ void fast_drain(const BeamArgs& a, const uint32_t queue, const unsigned n, const uint32_t map_base,
+                                        const uint32_t tab, const unsigned long long ring_head) {
+    const unsigned lane = threadIdx.x & 31;
+    if (lane < n) {
+        BeamMap<SmemSpace> bm;
+        const int mapWords = (a.map.H + 2 * kLineGuard) * a.map.strideR + (a.map.W + 2 * kLineGuard) * a.map.strideC;
+        bm.base = map_base; bm.H = a.map.H; bm.W = a.map.W; bm.stride4R = a.map.strideR << 2; bm.stride4C = a.map.strideC << 2;
+        bm.rowBytes = (unsigned)(a.map.H + 2 * kLineGuard) * (unsigned)(a.map.strideR << 2);
+        bm.mapBytes = (unsigned)mapWords * 4u; bm.oob = nullptr;
+        const unsigned o = SmemSpace::ld(queue + 4u * lane);
+        const unsigned B = (unsigned)a.robot.B;
+        const unsigned e = o / B, j = o - e * B;
+        const BeamPose* pose = a.poses + e;
+        const double2 pcs = *reinterpret_cast<const double2*>(&pose->c), cs = lds_d2(tab + 16u * j);
+        const double dx = pcs.x * cs.x - pcs.y * cs.y, dy = pcs.y * cs.x + pcs.x * cs.y;
+        const bool mx = fabs(dx) >= fabs(dy);
+        const double du = mx ? dx : dy, dw = mx ? dy : dx;
+        const double adw = fabs(dw);
+        const double r0 = rcp64h(adw);
+        const double M = fabs(du) * fma(fma(-adw, r0, 1.0), r0, r0);
+        const float r = cast_beam_slow<SmemSpace>(bm, pose->o[mx ? 0 : 1], mx, du, dw, M, a.robot.T, a.map.rho, a.robot.rmax).r;
+        a.out_ranges[o] = r;
+        float* ring_row = ring_row_of(a, ring_head, e);
+        if (ring_row) ring_row[j] = r;
+    }
+    __syncwarp();
+}
+// one task: beams [jb0, jb1) of env e, jb0 a multiple of 32 (pose = the env's sensing pose, possibly a shared-memory copy)
+__device__ __forceinline__ void fast_chunk(const BeamArgs& a, FastWarp& w, const BeamPose* pose, const unsigned e,
+                                           const unsigned jb0, const unsigned jb1, const unsigned long long ring_head) {
+    const unsigned lane = threadIdx.x & 31;
+    const unsigned B = (unsigned)a.robot.B;
+    // the env's part of the warp's slot: heading, (h, ouMS) of both axes
+    __syncwarp();
+    if (lane < 3) {
+        const uint4 v = *reinterpret_cast<const uint4*>(reinterpret_cast<const char*>(pose) + 32u * lane);
+        asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(w.slot + ((0x401000u >> (8u * lane)) & 0xffu)),
+                     "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");     // slot offsets 0, 16, 64
+    }
+    const int state = pose->state;
+    __syncwarp();
+    w.rays += jb1 - jb0;
+    unsigned j = jb0 + lane;
+    const unsigned o0 = e * B;                                     // n_envs * B < 2^31 (fn_sim_create)
+    float* po = a.out_ranges + (o0 + j);
+    float* pr = nullptr;
+    if (a.ring_obs) pr = ring_row_of(a, ring_head, e) + j;
+    uint32_t tj = w.tab + 16u * j;
+#pragma unroll 1
+    for (unsigned jb = jb0; jb < jb1; jb += 32u, j += 32u, po += 32, tj += 512u) {
+        bool near = false;
+        float r = 0.0f;
+        if (state == 0) r = cast_beam_fast(w.slot, min(tj, w.tab_last), a.robot.T, a.half_T, a.map.rho, a.robot.rmax, near);
+        if (j >= B) near = false;
+        else if (!near) {
+            *po = r;
+            if (a.ring_obs) pr[jb - jb0] = r;
+        }
+        if (__any_sync(0xffffffffu, near)) {                       // (rare: the warp's beams cross an axis)
+            const unsigned nm = __ballot_sync(0xffffffffu, near);
+            if (near) asm volatile("st.shared.u32 [%0], %1;" ::"r"(w.queue + 4u * (w.qn + __popc(nm & ((1u << lane) - 1u)))), "r"(o0 + j) : "memory");
+            w.qn += __popc(nm);
+            __syncwarp();
+            if (w.qn >= 32u) { w.qn -= 32u; fast_drain(a, w.queue + 4u * w.qn, 32u, w.map_base, w.tab, ring_head); }
+        }
     }
 }
 
@@ -490,51 +656,68 @@ __device__ __forceinline__ void stage_beam_constants(const BeamArgs& a, double2*
     if (!done) __trap();                                           // (never: a lost copy must not hang the device)
 }
 
-// The warps of the (persistent) grid take 32 consecutive (env, beam) pairs at a time: adjacent lanes =
-// adjacent beams of one env, so a warp's loads mostly hit the same or neighbouring words (broadcast)
-// and its lanes run similar trip counts.  kFast = production shared-memory traversal (cast_beam_smem).
-template <class MS, bool kFast, bool kAux>
-__device__ __forceinline__ void run_beam_tasks(const BeamArgs& a, const BeamMap<MS>& bm, const SmemGeo& geo,
-                                               const double2* s_tab, const int n_env, const unsigned total,
+// The warps of the (persistent) grid take their tasks in two parts.  Beams differ in length by an order of
+// magnitude, and a purely static split leaves ~15 % of the SM time idle at the end of the launch.  So: the
+// first 3/4 of each warp's share is static (round r -> task warp0 + r * nwarps, no atomics), the rest is
+// handed out dynamically, one atomic per warp task, fetched one task ahead so that its latency is hidden.
+// (has_static = false: a warp that arrives late -- fn_step_split.cuh -- takes pool tasks only)
+struct TaskFeed {
+    unsigned ntasks, warp0, nwarps, static_rounds, dyn_base, round, task;
+    bool dynamic;
+    unsigned* counter;
+    __device__ __forceinline__ TaskFeed(const unsigned ntasks_, const unsigned warp0_, const unsigned nwarps_,
+                                        const bool has_static, unsigned* counter_)
+        : ntasks(ntasks_), warp0(warp0_), nwarps(nwarps_), counter(counter_) {
+        static_rounds = max(1u, ((ntasks / nwarps) * 3u) >> 2);
+        dyn_base = static_rounds * nwarps;
+        dynamic = dyn_base < ntasks;                               // (short launches are static only)
+        round = 0;
+        task = warp0;
+        if (!has_static) {
+            round = static_rounds;
+            task = ntasks;
+            if (dynamic && (threadIdx.x & 31) == 0) task = dyn_base + atomicAdd(counter, 1u);
+            task = __shfl_sync(0xffffffffu, task, 0);
+        }
+    }
+    __device__ __forceinline__ bool valid() const { return task < ntasks; }
+    // issue the fetch of the task after this one (call before working on `task`) ...
+    __device__ __forceinline__ unsigned prefetch() {
+        unsigned next = ntasks;
+        ++round;
+        if (round < static_rounds) next = warp0 + round * nwarps;
+        else if (dynamic && (threadIdx.x & 31) == 0) next = dyn_base + atomicAdd(counter, 1u);
+        return next;
+    }
+    // ... and move on to it (after the work)
+    __device__ __forceinline__ void advance(const unsigned next) { task = __shfl_sync(0xffffffffu, next, 0); }
+};
+
+// Instrumented / L2-path kernels: a task = 32 consecutive (env, beam) pairs: adjacent lanes = adjacent beams of
+// one env, so a warp's loads mostly hit the same or neighbouring words and its lanes run similar trip counts.
+template <class MS, bool kAux>
+__device__ __forceinline__ void run_beam_tasks(const BeamArgs& a, const BeamMap<MS>& bm,
+                                               const double2* s_tab, const int* list, const int n_env, const unsigned total,
                                                const unsigned long long ring_head,     // slot of env 0's pending ring row
                                                const unsigned warp0, const unsigned nwarps,  // this warp's place among the
                                                const bool has_static = true) {         // warps that share the static part
     const int B = a.robot.B;
     const int lane = threadIdx.x & 31;
-    const unsigned ntasks = (total + 31u) >> 5;
     uint32_t words = 0, rays = 0;
-    // Beams differ in length by an order of magnitude, and a purely static split leaves ~15 % of the SM
-    // time idle at the end of the launch.  So: the first 3/4 of each warp's share is static (round r ->
-    // task warp0 + r * nwarps, no atomics), the rest is handed out dynamically, one atomic per warp
-    // task, fetched one task ahead so that its latency is hidden.
-    // (has_static = false: a warp that arrives late -- fn_step_split.cuh -- takes pool tasks only)
-    const unsigned static_rounds = max(1u, ((ntasks / nwarps) * 3u) >> 2);
-    const unsigned dyn_base = static_rounds * nwarps;
-    const bool dynamic = dyn_base < ntasks;                        // (short launches are static only)
     const unsigned long long invB = ~0ull / (unsigned long long)B + 1ull;     // floor(2^64 / B) + 1
-    unsigned round = 0;
-    unsigned task = warp0;
-    if (!has_static) {
-        round = static_rounds;
-        task = ntasks;
-        if (dynamic && lane == 0) task = dyn_base + atomicAdd(a.task_counter, 1u);
-        task = __shfl_sync(0xffffffffu, task, 0);
-    }
-    while (task < ntasks) {
-        unsigned next = ntasks;
-        ++round;
-        if (round < static_rounds) next = warp0 + round * nwarps;
-        else if (dynamic && lane == 0) next = dyn_base + atomicAdd(a.task_counter, 1u);
+    TaskFeed feed((total + 31u) >> 5, warp0, nwarps, has_static, a.task_counter);
+    while (feed.valid()) {
+        const unsigned next = feed.prefetch();
         // (listed env, beam) of this lane's element idx = 32 task + lane
-        const unsigned idx = (task << 5) + lane;
+        const unsigned idx = (feed.task << 5) + lane;
         const unsigned le = (unsigned)__umul64hi((unsigned long long)idx, invB);     // idx / B, exact for idx < 2^32
         const unsigned j = idx - le * (unsigned)B;
         if (le < (unsigned)n_env) {
-            const unsigned e = a.list ? (unsigned)a.list[le] : le;
-            beam_element<MS, kFast, kAux>(a, bm, geo, s_tab, a.poses + e, e, j, ring_head, words);
+            const unsigned e = list ? (unsigned)list[le] : le;
+            beam_element<MS, kAux>(a, bm, s_tab, a.poses + e, e, j, ring_head, words);
             ++rays;
         }
-        task = __shfl_sync(0xffffffffu, next, 0);
+        feed.advance(next);
     }
     // counters: one atomic per warp
     for (int o = 16; o > 0; o >>= 1) {
@@ -547,19 +730,67 @@ __device__ __forceinline__ void run_beam_tasks(const BeamArgs& a, const BeamMap<
     }
 }
 
+__device__ __forceinline__ void fast_finish(const BeamArgs& a, FastWarp& w, const unsigned long long ring_head) {
+    if (w.qn) fast_drain(a, w.queue, w.qn, w.map_base, w.tab, ring_head);
+    if ((threadIdx.x & 31) == 0 && w.rays) atomicAdd(&a.counters[kRays], (unsigned long long)w.rays);
+}
+// The envs' beams as warp tasks, handed out in order by one atomic counter (fetched one task ahead, so that its
+// latency is hidden; a warp's first task is its own index).  Two sizes: the first 27/32 of the envs go out in chunks
+// of chunk_rounds x 32 beams -- what depends on the env is amortised over the chunk -- and the rest in single
+// rounds of 32 beams, so that the launch ends within one round's time on every SM (beams differ in length by an
+// order of magnitude; a static split of such chunks left 13 % of the SM time idle).  Small launches (fewer than
+// eight rounds per warp) use single rounds only.
+// (has_static = false: a warp that arrives late -- fn_step_split.cuh -- has no task of its own)
+__device__ __forceinline__ void run_fast_tasks(const BeamArgs& a, FastWarp& w, const int* list, const int n_env,
+                                               const unsigned long long ring_head, const unsigned warp0,
+                                               const unsigned nwarps, const bool has_static = true) {
+    const unsigned B = (unsigned)a.robot.B, rounds = (B + 31u) >> 5;
+    const unsigned nchunk = (unsigned)a.nchunk, cbeams = (unsigned)a.chunk_rounds << 5;
+    const unsigned nA = (unsigned)n_env * rounds >= 8u * nwarps ? ((unsigned)n_env * 27u) >> 5 : 0u;   // envs cast in chunks
+    const unsigned ntA = nA * nchunk, nt = ntA + ((unsigned)n_env - nA) * rounds;
+    const unsigned lane = threadIdx.x & 31;
+    unsigned t = warp0;
+    if (!has_static) {
+        if (lane == 0) t = nwarps + atomicAdd(a.task_counter, 1u);
+        t = __shfl_sync(0xffffffffu, t, 0);
+    }
+    while (t < nt) {
+        unsigned next = 0u;
+        if (lane == 0) next = nwarps + atomicAdd(a.task_counter, 1u);
+        unsigned le, jb0, jb1;
+        if (t < ntA) {
+            le = a.inv_nchunk ? __umulhi(t, a.inv_nchunk) : t / nchunk;               // (exact: fast_magic)
+            jb0 = (t - le * nchunk) * cbeams;
+            jb1 = jb0 + cbeams;
+        } else {
+            const unsigned u = t - ntA;
+            const unsigned lb = a.inv_rounds ? __umulhi(u, a.inv_rounds) : u / rounds;
+            le = nA + lb;
+            jb0 = (u - lb * rounds) << 5;
+            jb1 = jb0 + 32u;
+        }
+        const unsigned e = list ? (unsigned)list[le] : le;
+        fast_chunk(a, w, a.poses + e, e, jb0, min(B, jb1), ring_head);
+        t = __shfl_sync(0xffffffffu, next, 0);
+    }
+    fast_finish(a, w, ring_head);
+}
+
 // Persistent kernel (grid = SMs x resident CTAs).  kSmem: each CTA stages both packed copies of the map
 // and the beam table in shared memory -- constants, so this happens BEFORE the dependency wait, under
 // the env-step / reset kernel that precedes it in the stream.
 // kAux = instrumented variant: hit-cell output, map-word counter.
 template <bool kSmem, bool kAux>
-__global__ void __launch_bounds__(512, 2) beam_kernel(BeamArgs a) {
+__global__ void __launch_bounds__(512, 2) beam_kernel(const __grid_constant__ BeamArgs a) {
     extern __shared__ __align__(16) uint8_t smem_raw[];
     const int B = a.robot.B;
     constexpr bool stage = kSmem;
+    constexpr bool fast = kSmem && !kAux;
     const int mapWords = (a.map.H + 2 * kLineGuard) * a.map.strideR + (a.map.W + 2 * kLineGuard) * a.map.strideC;
     double2* s_tab = reinterpret_cast<double2*>(smem_raw);
     uint32_t* s_map = reinterpret_cast<uint32_t*>(smem_raw + (size_t)B * sizeof(double2));
     __shared__ __align__(8) unsigned long long s_mbar;
+    __shared__ __align__(16) typename std::conditional<fast, FastShared, int>::type s_fast;
     stage_beam_constants(a, s_tab, s_map, mapWords, stage, &s_mbar);
     __syncthreads();
     griddep_wait();                                                // poses / list / count come from the previous kernel
@@ -569,30 +800,31 @@ __global__ void __launch_bounds__(512, 2) beam_kernel(BeamArgs a) {
         a.done_count[p ^ 1] = 0;
         *a.flip_par_dev = p ^ 1;
     }
-    if (a.list_par_dev) { const int q = *a.list_par_dev ^ 1; a.list += (size_t)q * a.n_all; a.count_dev += q; }
-    const int n_env = a.count_dev ? *a.count_dev : a.n_all;
+    const int* list = a.list;
+    const int* count_dev = a.count_dev;
+    if (a.list_par_dev) { const int q = *a.list_par_dev ^ 1; list += (size_t)q * a.n_all; count_dev += q; }
+    const int n_env = count_dev ? *count_dev : a.n_all;
     const unsigned total = (unsigned)n_env * (unsigned)B;
     const unsigned long long ring_head = a.ring_obs ? *a.ring_head : 0ull;
     const unsigned warp0 = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
     const unsigned nwarps = gridDim.x * (blockDim.x >> 5);
 
-    SmemGeo geo;
-    geo.baseR = geo.baseC = 0; geo.rho = a.map.rho; geo.bitsR = a.map.strideR << 5; geo.bitsC = a.map.strideC << 5;
-    geo.inv_bitsR = a.inv_bitsR; geo.inv_bitsC = a.inv_bitsC;
     const unsigned rowBytes = (unsigned)(a.map.H + 2 * kLineGuard) * (unsigned)(a.map.strideR << 2);
-    if (stage) {
+    if constexpr (fast) {
+        FastWarp w = fast_warp(a, &s_fast, s_tab, (uint32_t)__cvta_generic_to_shared(s_map));
+        run_fast_tasks(a, w, list, n_env, ring_head, warp0, nwarps);
+    } else if (stage) {
         BeamMap<SmemSpace> bm;
         bm.base = (uint32_t)__cvta_generic_to_shared(s_map);
         bm.H = a.map.H; bm.W = a.map.W; bm.stride4R = a.map.strideR << 2; bm.stride4C = a.map.strideC << 2;
         bm.rowBytes = rowBytes; bm.mapBytes = (unsigned)mapWords * 4u; bm.oob = a.counters + kOobLoads;
-        geo.baseR = bm.base - a.exp_off; geo.baseC = geo.baseR + rowBytes;
-        run_beam_tasks<SmemSpace, !kAux, kAux>(a, bm, geo, s_tab, n_env, total, ring_head, warp0, nwarps);
+        run_beam_tasks<SmemSpace, kAux>(a, bm, s_tab, list, n_env, total, ring_head, warp0, nwarps);
     } else {
         BeamMap<GlobalSpace> bm;
         bm.base = (unsigned long long)__cvta_generic_to_global(a.map.row);
         bm.H = a.map.H; bm.W = a.map.W; bm.stride4R = a.map.strideR << 2; bm.stride4C = a.map.strideC << 2;
         bm.rowBytes = rowBytes; bm.mapBytes = (unsigned)mapWords * 4u; bm.oob = a.counters + kOobLoads;
-        run_beam_tasks<GlobalSpace, false, kAux>(a, bm, geo, s_tab, n_env, total, ring_head, warp0, nwarps);
+        run_beam_tasks<GlobalSpace, kAux>(a, bm, s_tab, list, n_env, total, ring_head, warp0, nwarps);
     }
 }
 

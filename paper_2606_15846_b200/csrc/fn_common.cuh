@@ -38,11 +38,11 @@ constexpr double kMagic = 1048576.0;            // 2^20: a double D in [2^20, 2^
 constexpr unsigned kMagicHi = 0x41300000u;      // high word is exactly kMagicHi + floor(D - 2^20)
 struct __align__(16) BeamOrient {
     double ouM;              // origin along u, in cells, + kCellShift + kMagic
-    double h;                // 0.5 - frac(origin along w): first line boundary at f = 0.5 +- h
-    double ouMS;             // ouM + the BIT offset of the origin's line within its own copy (row / column)
     int cu0;                 // floor(origin along u)
     unsigned line_off;       // byte offset of the origin's line from the start of the row copy
-};
+    double h;                // 0.5 - frac(origin along w): first line boundary at f = 0.5 +- h
+    double ouMS;             // ouM + the BIT offset of the origin's line within its own copy (row / column)
+};                           // (h, ouMS) are one 16-byte load of the production beam kernel
 struct __align__(32) BeamPose {
     double c, s;             // cos/sin of the heading
     BeamOrient o[2];

@@ -29,7 +29,7 @@ __host__ __device__ inline size_t fused_smem_bytes(int B, int mapWords, int V) {
 }
 
 template <bool kAux>
-__global__ void __launch_bounds__(kFusedThreads, 2) reset_beam_kernel(ResetArgs ra, BeamArgs a) {
+__global__ void __launch_bounds__(kFusedThreads, 2) reset_beam_kernel(const __grid_constant__ ResetArgs ra, const __grid_constant__ BeamArgs a) {
     extern __shared__ __align__(16) uint8_t smem_raw[];
     const int B = a.robot.B, V = a.robot.V;
     const int rowWords = (a.map.H + 2 * kLineGuard) * a.map.strideR;
@@ -40,6 +40,7 @@ __global__ void __launch_bounds__(kFusedThreads, 2) reset_beam_kernel(ResetArgs 
     uint8_t* s_scr = reinterpret_cast<uint8_t*>(s_pose + kFusedPoseSlots);
     const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31;
     __shared__ __align__(8) unsigned long long s_mbar;
+    __shared__ __align__(16) typename std::conditional<!kAux, FastShared, int>::type s_fast;
     stage_beam_constants(a, s_tab, s_map, mapWords, true, &s_mbar);
     ColScratch scratch = col_scratch(s_scr + (size_t)(wib < kFusedResetWarps ? wib : 0) * col_scratch_bytes(V), V);
     if (wib < kFusedResetWarps)
@@ -47,8 +48,10 @@ __global__ void __launch_bounds__(kFusedThreads, 2) reset_beam_kernel(ResetArgs 
     __syncthreads();
     griddep_wait();                                                // the list comes from the kernel before
     griddep_launch_dependents();
-    if (ra.list_par_dev) { const int q = *ra.list_par_dev ^ 1; ra.list += (size_t)q * ra.n; ra.count_dev += q; }
-    const int count = *ra.count_dev;
+    const int* rlist = ra.list;
+    const int* rcount = ra.count_dev;
+    if (ra.list_par_dev) { const int q = *ra.list_par_dev ^ 1; rlist += (size_t)q * ra.n; rcount += q; }
+    const int count = *rcount;
     // this CTA's envs: list entries blockIdx.x, blockIdx.x + gridDim.x, ...
     const int m_loc = count > (int)blockIdx.x ? (count - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x : 0;
     if (m_loc == 0) return;                                        // (uniform over the CTA)
@@ -59,43 +62,50 @@ __global__ void __launch_bounds__(kFusedThreads, 2) reset_beam_kernel(ResetArgs 
         ms.row = s_map;
         ms.col = s_map + rowWords;
         for (int k = wib; k < m_loc; k += kFusedResetWarps)
-            reset_env<true>(ra, ms, scratch, ra.list[blockIdx.x + k * gridDim.x], lane, k < kFusedPoseSlots ? s_pose + k : nullptr);
+            reset_env<true>(ra, ms, scratch, rlist[blockIdx.x + k * gridDim.x], lane, k < kFusedPoseSlots ? s_pose + k : nullptr);
         __threadfence_block();                                     // poses: written here, read below by all warps
     }
     __syncthreads();
 
-    // ---- phase 2: the beams of this CTA's envs, 32 consecutive (env, beam) pairs per warp task
-    SmemGeo geo;
-    geo.rho = a.map.rho; geo.bitsR = a.map.strideR << 5; geo.bitsC = a.map.strideC << 5;
-    geo.inv_bitsR = a.inv_bitsR; geo.inv_bitsC = a.inv_bitsC;
-    BeamMap<SmemSpace> bm;
-    bm.base = (uint32_t)__cvta_generic_to_shared(s_map);
-    bm.H = a.map.H; bm.W = a.map.W; bm.stride4R = a.map.strideR << 2; bm.stride4C = a.map.strideC << 2;
-    bm.rowBytes = (unsigned)rowWords * 4u; bm.mapBytes = (unsigned)mapWords * 4u; bm.oob = a.counters + kOobLoads;
-    geo.baseR = bm.base - a.exp_off; geo.baseC = geo.baseR + bm.rowBytes;
+    // ---- phase 2: the beams of this CTA's envs
     const unsigned long long ring_head = a.ring_obs ? *a.ring_head : 0ull;
-    const unsigned total = (unsigned)m_loc * (unsigned)B;
-    const unsigned ntasks = (total + 31u) >> 5;
-    const unsigned long long invB = ~0ull / (unsigned long long)B + 1ull;     // floor(2^64 / B) + 1
-    uint32_t words = 0, rays = 0;
-    for (unsigned task = (unsigned)wib; task < ntasks; task += blockDim.x >> 5) {
-        const unsigned idx = (task << 5) + lane;
-        const unsigned k = (unsigned)__umul64hi((unsigned long long)idx, invB);      // idx / B
-        const unsigned j = idx - k * (unsigned)B;
-        if (k < (unsigned)m_loc) {
-            const unsigned e = (unsigned)ra.list[blockIdx.x + k * gridDim.x];
-            const BeamPose* pose = k < (unsigned)kFusedPoseSlots ? s_pose + k : a.poses + e;
-            beam_element<SmemSpace, !kAux, kAux>(a, bm, geo, s_tab, pose, e, j, ring_head, words);
-            ++rays;
+    if constexpr (!kAux) {                                         // production path: chunks of one env's beams per warp task
+        FastWarp w = fast_warp(a, &s_fast, s_tab, (uint32_t)__cvta_generic_to_shared(s_map));
+        const unsigned rounds = ((unsigned)B + 31u) >> 5, ntasks = (unsigned)m_loc * rounds;   // a task = 32 beams of one env
+        for (unsigned task = (unsigned)wib; task < ntasks; task += blockDim.x >> 5) {
+            const unsigned k = a.inv_rounds ? __umulhi(task, a.inv_rounds) : task / rounds, jb0 = (task - k * rounds) << 5;
+            const unsigned e = (unsigned)rlist[blockIdx.x + k * gridDim.x];
+            fast_chunk(a, w, k < (unsigned)kFusedPoseSlots ? s_pose + k : a.poses + e, e, jb0, min((unsigned)B, jb0 + 32u), ring_head);
         }
-    }
-    for (int o = 16; o > 0; o >>= 1) {
-        rays += __shfl_xor_sync(0xffffffffu, rays, o);
-        if (kAux) words += __shfl_xor_sync(0xffffffffu, words, o);
-    }
-    if (lane == 0 && rays) {
-        atomicAdd(&a.counters[kRays], (unsigned long long)rays);
-        if (kAux && a.count_words) atomicAdd(&a.counters[kWords], (unsigned long long)words);
+        fast_finish(a, w, ring_head);
+    } else {                                                       // instrumented: 32 consecutive (env, beam) pairs per warp task
+        BeamMap<SmemSpace> bm;
+        bm.base = (uint32_t)__cvta_generic_to_shared(s_map);
+        bm.H = a.map.H; bm.W = a.map.W; bm.stride4R = a.map.strideR << 2; bm.stride4C = a.map.strideC << 2;
+        bm.rowBytes = (unsigned)rowWords * 4u; bm.mapBytes = (unsigned)mapWords * 4u; bm.oob = a.counters + kOobLoads;
+        const unsigned total = (unsigned)m_loc * (unsigned)B;
+        const unsigned ntasks = (total + 31u) >> 5;
+        const unsigned long long invB = ~0ull / (unsigned long long)B + 1ull;     // floor(2^64 / B) + 1
+        uint32_t words = 0, rays = 0;
+        for (unsigned task = (unsigned)wib; task < ntasks; task += blockDim.x >> 5) {
+            const unsigned idx = (task << 5) + lane;
+            const unsigned k = (unsigned)__umul64hi((unsigned long long)idx, invB);      // idx / B
+            const unsigned j = idx - k * (unsigned)B;
+            if (k < (unsigned)m_loc) {
+                const unsigned e = (unsigned)rlist[blockIdx.x + k * gridDim.x];
+                const BeamPose* pose = k < (unsigned)kFusedPoseSlots ? s_pose + k : a.poses + e;
+                beam_element<SmemSpace, kAux>(a, bm, s_tab, pose, e, j, ring_head, words);
+                ++rays;
+            }
+        }
+        for (int o = 16; o > 0; o >>= 1) {
+            rays += __shfl_xor_sync(0xffffffffu, rays, o);
+            words += __shfl_xor_sync(0xffffffffu, words, o);
+        }
+        if (lane == 0 && rays) {
+            atomicAdd(&a.counters[kRays], (unsigned long long)rays);
+            if (a.count_words) atomicAdd(&a.counters[kWords], (unsigned long long)words);
+        }
     }
 }
 

@@ -41,7 +41,7 @@ __host__ __device__ inline size_t step_split_smem_bytes(size_t beam_smem, int V)
 
 // beam_smem = the beam kernel's dynamic shared bytes (beam table [+ packed map]); epc = envs owned per CTA
 template <bool kSmem, bool kAux>
-__global__ void __launch_bounds__(512, 2) step_beam_kernel(BeamArgs a, EnvArgs ea, StepEnd* end, int epc, unsigned beam_smem) {
+__global__ void __launch_bounds__(512, 2) step_beam_kernel(const __grid_constant__ BeamArgs a, const __grid_constant__ EnvArgs ea, StepEnd* end, int epc, unsigned beam_smem) {
     extern __shared__ __align__(16) uint8_t smem_raw[];
     const int B = a.robot.B, V = a.robot.V;
     const int rowWords = (a.map.H + 2 * kLineGuard) * a.map.strideR;
@@ -50,6 +50,8 @@ __global__ void __launch_bounds__(512, 2) step_beam_kernel(BeamArgs a, EnvArgs e
     uint32_t* s_map = reinterpret_cast<uint32_t*>(smem_raw + (size_t)B * sizeof(double2));
     const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31, last_warp = (int)(blockDim.x >> 5) - 1;
     __shared__ __align__(8) unsigned long long s_mbar;
+    constexpr bool fast = kSmem && !kAux;
+    __shared__ __align__(16) typename std::conditional<fast, FastShared, int>::type s_fast;
     stage_beam_constants(a, s_tab, s_map, mapWords, kSmem, &s_mbar);
     const ColScratch scratch = col_scratch(smem_raw + step_split_scratch_offset(beam_smem), V);
     if (wib == last_warp)
@@ -82,23 +84,22 @@ __global__ void __launch_bounds__(512, 2) step_beam_kernel(BeamArgs a, EnvArgs e
     // late and take pool tasks only
     const unsigned warp0 = blockIdx.x * (unsigned)last_warp + (unsigned)wib;
     const unsigned nwarps = gridDim.x * (unsigned)last_warp;
-    SmemGeo geo;
-    geo.baseR = geo.baseC = 0; geo.rho = a.map.rho; geo.bitsR = a.map.strideR << 5; geo.bitsC = a.map.strideC << 5;
-    geo.inv_bitsR = a.inv_bitsR; geo.inv_bitsC = a.inv_bitsC;
     const unsigned rowBytes = (unsigned)rowWords * 4u;
-    if (kSmem) {
+    if constexpr (fast) {
+        FastWarp w = fast_warp(a, &s_fast, s_tab, (uint32_t)__cvta_generic_to_shared(s_map));
+        run_fast_tasks(a, w, nullptr, n, head_new, warp0, nwarps, wib != last_warp);
+    } else if (kSmem) {
         BeamMap<SmemSpace> bm;
         bm.base = (uint32_t)__cvta_generic_to_shared(s_map);
         bm.H = a.map.H; bm.W = a.map.W; bm.stride4R = a.map.strideR << 2; bm.stride4C = a.map.strideC << 2;
         bm.rowBytes = rowBytes; bm.mapBytes = (unsigned)mapWords * 4u; bm.oob = a.counters + kOobLoads;
-        geo.baseR = bm.base - a.exp_off; geo.baseC = geo.baseR + rowBytes;
-        run_beam_tasks<SmemSpace, !kAux, kAux>(a, bm, geo, s_tab, n, total, head_new, warp0, nwarps, wib != last_warp);
+        run_beam_tasks<SmemSpace, kAux>(a, bm, s_tab, nullptr, n, total, head_new, warp0, nwarps, wib != last_warp);
     } else {
         BeamMap<GlobalSpace> bm;
         bm.base = (unsigned long long)__cvta_generic_to_global(a.map.row);
         bm.H = a.map.H; bm.W = a.map.W; bm.stride4R = a.map.strideR << 2; bm.stride4C = a.map.strideC << 2;
         bm.rowBytes = rowBytes; bm.mapBytes = (unsigned)mapWords * 4u; bm.oob = a.counters + kOobLoads;
-        run_beam_tasks<GlobalSpace, false, kAux>(a, bm, geo, s_tab, n, total, head_new, warp0, nwarps, wib != last_warp);
+        run_beam_tasks<GlobalSpace, kAux>(a, bm, s_tab, nullptr, n, total, head_new, warp0, nwarps, wib != last_warp);
     }
 
     // ---- the last CTA to finish closes the step: done-list parity, the other list's count, the ring head

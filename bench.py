@@ -207,7 +207,10 @@ def run_ours(args):
         sim.set_fused_reset(args.fused_reset)
     if args.split_step >= 0:
         sim.set_split_step(bool(args.split_step))
+    if args.coarse >= 0:
+        sim.set_coarse(bool(args.coarse))
     fused_active, split_step = sim.beam_config()["fused_reset"], sim.beam_config()["split_step"]
+    coarse_active = sim.beam_config()["coarse"]
     states = torch.zeros(8, n, device="cuda")
     mask = torch.ones(n, dtype=torch.uint8, device="cuda")
     ranges = torch.zeros(n, B, device="cuda")
@@ -463,7 +466,8 @@ def run_ours(args):
                "dtype": "f64", "data": "synthetic",
                "config": {"workload": workload_name(args.config), "name": wl.name, "n_envs_per_gpu": n, "beams": B,
                           "map": list(wl.occ.shape), "max_range_m": float(wl.max_range), "l2": "flushed between timed steps",
-                          "ring": bool(ring is not None), "fused_reset": bool(fused_active), "split_step": bool(split_step)},
+                          "ring": bool(ring is not None), "fused_reset": bool(fused_active), "split_step": bool(split_step),
+                          "coarse_level": bool(coarse_active)},
                "rays_per_s": float(rays[0]) / (total_ms * 1e-3),
                "useful_rays_per_s": world * n * B * K / (total_ms * 1e-3),
                "reset_rate_per_step": float(rays[1]) / (world * n * K),
@@ -535,6 +539,8 @@ def main():
                     help="fn_reset(done list) as one fused kernel (1) or two kernels (0); -1 = the library's default")
     ap.add_argument("--split-step", type=int, default=-1, choices=[-1, 0, 1],
                     help="fn_step with the env step split around the beam kernel (1) or one env-step kernel (0); -1 = the library's default")
+    ap.add_argument("--coarse", type=int, default=-1, choices=[-1, 0, 1],
+                    help="coarse level in the production beam kernels: -1 = the library's choice")
     ap.add_argument("--ring", type=int, default=1, help="attach the replay ring when the config has one (C5)")
     args = ap.parse_args()
     if args.warmup < 3:

@@ -192,10 +192,21 @@ int fn_eval_end(fn_sim* sim);
  * both variants give the same ranges.  Overwrites the sim's sensing poses (like fn_observe_all). */
 int fn_ranges_fixed_step(fn_sim* sim, const float* states_dev, float delta_m, int blockwise, float* out_ranges_dev);
 
-/* ---- launch configuration chosen at fn_sim_create or by the switches below (for reports): cfg_out[6] =
+/* ---- launch configuration chosen at fn_sim_create or by the switches below (for reports): cfg_out[8] =
  * {map staged in shared memory (1) or read through L1/L2 (0), beam grid size, CTA size, dynamic shared bytes,
- *  split step in use (fn_sim_set_split_step), fused reset in use for done lists (fn_sim_set_fused_reset)}. */
+ *  split step in use (fn_sim_set_split_step), fused reset in use for done lists (fn_sim_set_fused_reset),
+ *  coarse level in use (fn_sim_set_coarse), coarse level available}. */
 int fn_sim_beam_config(const fn_sim* sim, int* cfg_out);
+
+/* ---- coarse level for empty-space skipping (BASELINE.json north_star).  Beside each packed copy
+ * of the map the library keeps a coarse copy: one line per pair of lines, the OR of the two.  With enable != 0
+ * the production beam kernels walk the coarse copy -- one 32-bit window per PAIR of lines -- and look at the two
+ * fine lines only where that window is not empty; both variants resolve a hit on the same fine line with the
+ * same fixed-point crossing coordinates, so ranges are bit-identical with the level on and off.  Available when
+ * the map is staged in shared memory and fine + coarse copies fit one CTA (512 x 512 cells do).  *active_out (may
+ * be NULL) = 1 if the level is available and enabled.  Host-side switch, takes effect at the next launch.
+ * Errors: FN_ERR_INVALID_ARG (NULL sim). */
+int fn_sim_set_coarse(fn_sim* sim, int enable, int* active_out);
 
 /* ---- fn_reset as one launch or two.  When the packed map is staged in shared memory (cfg_out[0] of
  * fn_sim_beam_config) and the reset scratch fits beside it, fn_reset(mask = NULL) -- the step's done list,

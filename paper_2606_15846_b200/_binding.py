@@ -19,7 +19,7 @@ EXPORTED_SYMBOLS = (
     "fn_map_create", "fn_map_set_regions", "fn_map_destroy", "fn_robot_create", "fn_robot_create_union", "fn_robot_set_sensor", "fn_robot_set_acc_limits",
     "fn_robot_destroy", "fn_task_default", "fn_sim_create", "fn_sim_destroy", "fn_sim_set_stream", "fn_step", "fn_reset",
     "fn_sim_bind_aux", "fn_sim_bind_features", "fn_ring_attach", "fn_ring_sample", "fn_ranges_fixed_step", "fn_eval_begin", "fn_eval_result", "fn_eval_end", "fn_observe_all", "fn_get_counters", "fn_sim_count_words",
-    "fn_sim_episode_state", "fn_sim_beam_config", "fn_sim_set_fused_reset", "fn_sim_set_split_step", "fn_sim_profile", "fn_sim_profile_read", "fn_step_host", "fn_measure_peak", "fn_last_error", "fn_version")
+    "fn_sim_episode_state", "fn_sim_beam_config", "fn_sim_set_fused_reset", "fn_sim_set_split_step", "fn_sim_set_coarse", "fn_sim_profile", "fn_sim_profile_read", "fn_step_host", "fn_measure_peak", "fn_last_error", "fn_version")
 
 
 class FlashNavError(RuntimeError):
@@ -75,6 +75,7 @@ def load_library():
         "fn_sim_beam_config": [vp, vp],
         "fn_sim_set_fused_reset": [vp, i32, vp],
         "fn_sim_set_split_step": [vp, i32, vp],
+        "fn_sim_set_coarse": [vp, i32, vp],
         "fn_sim_profile": [vp, i32],
         "fn_sim_profile_read": [vp, vp, vp],
         "fn_step_host": [vp, vp, vp, f32, vp, vp, vp, vp, vp],
@@ -336,10 +337,10 @@ class Sim:
         return d, e
 
     def beam_config(self) -> dict:
-        cfg = np.zeros(6, np.int32)
+        cfg = np.zeros(8, np.int32)
         _check(load_library().fn_sim_beam_config(self._h, _np_ptr(cfg)), "fn_sim_beam_config")
         return {"smem": bool(cfg[0]), "grid": int(cfg[1]), "block": int(cfg[2]), "smem_bytes": int(cfg[3]),
-                "split_step": bool(cfg[4]), "fused_reset": bool(cfg[5])}
+                "split_step": bool(cfg[4]), "fused_reset": bool(cfg[5]), "coarse": bool(cfg[6]), "coarse_available": bool(cfg[7])}
 
     def set_fused_reset(self, enable) -> bool:
         """fn_reset(mask=None) as one fused kernel (1 / True, default where possible), never (0 / False), or for
@@ -353,6 +354,12 @@ class Sim:
         returns whether the split step is used."""
         act = C.c_int(0)
         _check(load_library().fn_sim_set_split_step(self._h, 1 if enable else 0, C.byref(act)), "fn_sim_set_split_step")
+        return bool(act.value)
+
+    def set_coarse(self, enable: bool) -> bool:
+        """Coarse level for empty-space skipping in the production beam kernels; returns whether it is in use."""
+        act = C.c_int(0)
+        _check(load_library().fn_sim_set_coarse(self._h, 1 if enable else 0, C.byref(act)), "fn_sim_set_coarse")
         return bool(act.value)
 
     def step_host(self, states, actions, dt, reset_mask, seeds, out_ranges, out_collision, out_goal_obs):

@@ -41,8 +41,9 @@ static int fail(int code, const char* fmt, ...) {
 struct fn_map {
     int H, W;
     float res;
-    uint32_t* d_words;       // row-packed copy then column-packed copy, contiguous
-    size_t n_words;          // padded to a multiple of 4
+    uint32_t* d_words;       // row-packed copy then column-packed copy, contiguous; then their coarse copies
+    size_t n_words;          // the two fine copies, padded to a multiple of 4
+    size_t n_words_coarse;   // the two coarse copies (fn_common.cuh, coarse_words), padded to a multiple of 4
     MapDev dev;
     int n_regions;
     int4* d_regions;
@@ -107,6 +108,10 @@ struct fn_sim {
     size_t split_smem;
     int split_grid;
     StepEnd* d_step_end;
+    // the coarse level in the production beam kernels (one CTA of 1024 threads per SM, fine + coarse copies staged)
+    bool coarse_ok, coarse_on, split_ok_c;
+    size_t beam_smem_c, split_smem_c;
+    int beam_grid_c, split_grid_c;
     // live timing
     int prof;
     std::vector<cudaEvent_t>* ev;    // triples per fn_step (e0 env e1 beam e2), pairs per fn_reset
@@ -160,11 +165,26 @@ extern "C" int fn_map_create(const uint8_t* bitmap, int H, int W, float res, fn_
             line[k] = w;
         }
     }
+    // Coarse level (north_star "coarse block-occupancy level for empty-space skipping"; fn_common.cuh): one line
+    // per PAIR of physical lines 2g, 2g + 1 = the OR of the two, stored with twice the line stride.
+    const size_t cR = coarse_words(H, sR), cC = coarse_words(W, sC);
+    const size_t total_c = (cR + cC + 3) / 4 * 4;
+    words.resize(total + total_c, 0xffffffffu);
+    for (int copy = 0; copy < 2; ++copy) {
+        const int L = copy ? W : H, st = copy ? sC : sR;
+        const uint32_t* fine = &words[copy ? rowWords : 0];
+        uint32_t* coarse = &words[total + (copy ? cR : 0)];
+        for (int p = 0; p < L + 2 * kLineGuard; ++p)
+            for (int k = 0; k < st; ++k) {
+                uint32_t& w = coarse[(size_t)(p >> 1) * 2 * st + k];
+                w = (p & 1) ? (w | fine[(size_t)p * st + k]) : fine[(size_t)p * st + k];
+            }
+    }
     fn_map* m = new (std::nothrow) fn_map();
     if (!m) return fail(FN_ERR_OOM, "fn_map_create: host allocation failed");
-    m->H = H; m->W = W; m->res = res; m->n_words = total; m->n_regions = 0; m->d_regions = nullptr; m->d_words = nullptr;
-    cudaError_t e = cudaMalloc(&m->d_words, total * sizeof(uint32_t));
-    if (e == cudaSuccess) e = cudaMemcpy(m->d_words, words.data(), total * sizeof(uint32_t), cudaMemcpyHostToDevice);
+    m->H = H; m->W = W; m->res = res; m->n_words = total; m->n_words_coarse = total_c; m->n_regions = 0; m->d_regions = nullptr; m->d_words = nullptr;
+    cudaError_t e = cudaMalloc(&m->d_words, words.size() * sizeof(uint32_t));
+    if (e == cudaSuccess) e = cudaMemcpy(m->d_words, words.data(), words.size() * sizeof(uint32_t), cudaMemcpyHostToDevice);
     if (e != cudaSuccess) {
         if (m->d_words) cudaFree(m->d_words);
         delete m;
@@ -355,11 +375,23 @@ static TaskDev task_dev(const fn_task& t) {
 }
 
 // ------------------------------------------------------------------------------------------ sim
-template <bool S, bool C>
-static cudaError_t beam_config(size_t smem, int* blocks_per_sm) {
-    cudaError_t e = cudaFuncSetAttribute(beam_kernel<S, C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+// The dynamic shared-memory limit is an attribute of the FUNCTION, not of a sim: it is raised to the device's
+// opt-in maximum once, so that sims with different map sizes can live side by side; occupancy is per sim.
+constexpr bool kCoarseDefault = false;   // (set by measurement: DESIGN.md 6.1)
+template <class K>
+static cudaError_t kernel_config(K kernel, int threads, size_t smem, int max_optin, int* blocks_per_sm) {
+    cudaFuncAttributes fa;
+    cudaError_t e = cudaFuncGetAttributes(&fa, kernel);
     if (e != cudaSuccess) return e;
-    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, beam_kernel<S, C>, 512, smem);
+    const int dyn_max = max_optin - (int)fa.sharedSizeBytes;       // static + dynamic <= opt-in maximum
+    if ((long long)smem > (long long)dyn_max) { *blocks_per_sm = 0; return cudaSuccess; }
+    e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, dyn_max);
+    if (e != cudaSuccess) return e;
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, kernel, threads, smem);
+}
+template <bool S, bool C>
+static cudaError_t beam_config(size_t smem, int max_optin, int* blocks_per_sm) {
+    return kernel_config(beam_kernel<S, C>, 512, smem, max_optin, blocks_per_sm);
 }
 
 extern "C" int fn_sim_create(const fn_map* map, const fn_robot* robot, int n, const fn_task* task,
@@ -416,7 +448,7 @@ extern "C" int fn_sim_create(const fn_map* map, const fn_robot* robot, int n, co
         // ... and addresses bits within a copy by the 20-bit integer field of a double in [2^20, 2^21)
         const size_t rowBits = (size_t)(map->H + 2 * kLineGuard) * map->dev.strideR * 32;
         const size_t colBits = (size_t)(map->W + 2 * kLineGuard) * map->dev.strideC * 32;
-        s->use_smem = with_map <= (size_t)max_optin && Tc + 34.0 < 0.5 * (double)Smin &&
+        s->use_smem = with_map + 8192 <= (size_t)max_optin && Tc + 34.0 < 0.5 * (double)Smin &&   // (8 KB: the kernels' static shared memory)
                       rowBits < (1u << 20) && colBits < (1u << 20);
         s->beam_smem = s->use_smem ? with_map : tab;
         if (s->beam_smem > (size_t)max_optin) {
@@ -424,8 +456,8 @@ extern "C" int fn_sim_create(const fn_map* map, const fn_robot* robot, int n, co
             return fail(FN_ERR_UNSUPPORTED, "fn_sim_create: beam table does not fit in shared memory (B too large)");
         }
         int bps = 0, bps2 = 0;
-        if (s->use_smem) { e = beam_config<true, false>(s->beam_smem, &bps); if (e == cudaSuccess) e = beam_config<true, true>(s->beam_smem, &bps2); }
-        else { e = beam_config<false, false>(s->beam_smem, &bps); if (e == cudaSuccess) e = beam_config<false, true>(s->beam_smem, &bps2); }
+        if (s->use_smem) { e = beam_config<true, false>(s->beam_smem, max_optin, &bps); if (e == cudaSuccess) e = beam_config<true, true>(s->beam_smem, max_optin, &bps2); }
+        else { e = beam_config<false, false>(s->beam_smem, max_optin, &bps); if (e == cudaSuccess) e = beam_config<false, true>(s->beam_smem, max_optin, &bps2); }
         if (bps2 < bps) bps = bps2;
         if (bps < 1) bps = 1;
         s->beam_grid = s->num_sms * bps;
@@ -435,10 +467,8 @@ extern "C" int fn_sim_create(const fn_map* map, const fn_robot* robot, int n, co
         s->fused_grid = 0;
         if (e == cudaSuccess && s->use_smem && s->fused_smem <= (size_t)max_optin) {
             int f0 = 0, f1 = 0;
-            e = cudaFuncSetAttribute(reset_beam_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s->fused_smem);
-            if (e == cudaSuccess) e = cudaFuncSetAttribute(reset_beam_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s->fused_smem);
-            if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&f0, reset_beam_kernel<false>, kFusedThreads, s->fused_smem);
-            if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&f1, reset_beam_kernel<true>, kFusedThreads, s->fused_smem);
+            e = kernel_config(reset_beam_kernel<false>, kFusedThreads, s->fused_smem, max_optin, &f0);
+            if (e == cudaSuccess) e = kernel_config(reset_beam_kernel<true>, kFusedThreads, s->fused_smem, max_optin, &f1);
             if (f1 < f0) f0 = f1;
             if (e == cudaSuccess && f0 >= 1) { s->fused_ok = s->fused_on = true; s->fused_grid = s->num_sms * f0; }
         }
@@ -449,15 +479,11 @@ extern "C" int fn_sim_create(const fn_map* map, const fn_robot* robot, int n, co
         if (e == cudaSuccess && s->split_smem <= (size_t)max_optin) {
             int f[2] = {0, 0};
             if (s->use_smem) {
-                e = cudaFuncSetAttribute(step_beam_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s->split_smem);
-                if (e == cudaSuccess) e = cudaFuncSetAttribute(step_beam_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s->split_smem);
-                if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&f[0], step_beam_kernel<true, false>, 512, s->split_smem);
-                if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&f[1], step_beam_kernel<true, true>, 512, s->split_smem);
+                e = kernel_config(step_beam_kernel<true, false>, 512, s->split_smem, max_optin, &f[0]);
+                if (e == cudaSuccess) e = kernel_config(step_beam_kernel<true, true>, 512, s->split_smem, max_optin, &f[1]);
             } else {
-                e = cudaFuncSetAttribute(step_beam_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s->split_smem);
-                if (e == cudaSuccess) e = cudaFuncSetAttribute(step_beam_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s->split_smem);
-                if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&f[0], step_beam_kernel<false, false>, 512, s->split_smem);
-                if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&f[1], step_beam_kernel<false, true>, 512, s->split_smem);
+                e = kernel_config(step_beam_kernel<false, false>, 512, s->split_smem, max_optin, &f[0]);
+                if (e == cudaSuccess) e = kernel_config(step_beam_kernel<false, true>, 512, s->split_smem, max_optin, &f[1]);
             }
             const int fm = f[0] < f[1] ? f[0] : f[1];
             if (e == cudaSuccess && fm >= 1 && s->num_sms * fm >= s->beam_grid) {
@@ -466,6 +492,22 @@ extern "C" int fn_sim_create(const fn_map* map, const fn_robot* robot, int n, co
                 // two such batches (measured: C1-C4 3-8 % faster per step, C5 with 222 envs per CTA 4 % slower)
                 s->split_on = (n + s->split_grid - 1) / s->split_grid <= 64;
             }
+        }
+        // the coarse level: fine + coarse copies staged by one CTA of 1024 threads per SM
+        s->coarse_ok = s->coarse_on = s->split_ok_c = false;
+        s->beam_smem_c = tab + (map->n_words + map->n_words_coarse) * sizeof(uint32_t);
+        s->split_smem_c = step_split_smem_bytes(s->beam_smem_c, robot->V);
+        s->beam_grid_c = s->split_grid_c = 0;
+        const size_t cBitsR = coarse_words(map->H, map->dev.strideR) * 32, cBitsC = coarse_words(map->W, map->dev.strideC) * 32;
+        if (e == cudaSuccess && s->use_smem && s->beam_smem_c <= (size_t)max_optin && cBitsR < (1u << 20) && cBitsC < (1u << 20)) {
+            int f0 = 0, f1 = 0;
+            e = kernel_config(beam_kernel<true, false, true>, 1024, s->beam_smem_c, max_optin, &f0);
+            if (e == cudaSuccess && f0 >= 1) { s->coarse_ok = true; s->beam_grid_c = s->num_sms * f0; }
+            if (e == cudaSuccess && s->coarse_ok && s->split_smem_c <= (size_t)max_optin) {
+                e = kernel_config(step_beam_kernel<true, false, true>, 1024, s->split_smem_c, max_optin, &f1);
+                if (e == cudaSuccess && f1 >= 1) { s->split_ok_c = true; s->split_grid_c = s->num_sms * f1; }
+            }
+            s->coarse_on = s->coarse_ok && kCoarseDefault;
         }
     }
     if (e != cudaSuccess) {
@@ -539,7 +581,9 @@ static int launch_beams(fn_sim* s, const int* list, const int* count_dev, float*
     const BeamArgs b = beam_args(s, list, count_dev, out_ranges, step_launch, done_list);
     const bool aux = s->count_words || s->aux_hit;
     const dim3 grid(s->beam_grid), block(512);
-    if (s->use_smem) {
+    if (s->coarse_on && !aux) {
+        FN_CUDA(launch_pdl(beam_kernel<true, false, true>, dim3(s->beam_grid_c), dim3(1024), s->beam_smem_c, s->stream, b));
+    } else if (s->use_smem) {
         if (aux) FN_CUDA(launch_pdl(beam_kernel<true, true>, grid, block, s->beam_smem, s->stream, b));
         else FN_CUDA(launch_pdl(beam_kernel<true, false>, grid, block, s->beam_smem, s->stream, b));
     } else {
@@ -602,7 +646,11 @@ extern "C" int fn_step(fn_sim* s, float* states, const float* actions, float dt,
         const bool aux = s->count_words || s->aux_hit;
         const dim3 grid(s->split_grid), block(512);
         const unsigned bs = (unsigned)s->beam_smem;
-        if (s->use_smem) {
+        if (s->coarse_on && s->split_ok_c && !aux) {
+            const int epc_c = (s->n + s->split_grid_c - 1) / s->split_grid_c;
+            FN_CUDA(launch_pdl(step_beam_kernel<true, false, true>, dim3(s->split_grid_c), dim3(1024), s->split_smem_c, s->stream, b, a,
+                               s->d_step_end, epc_c, (unsigned)s->beam_smem_c));
+        } else if (s->use_smem) {
             if (aux) FN_CUDA(launch_pdl(step_beam_kernel<true, true>, grid, block, s->split_smem, s->stream, b, a, s->d_step_end, epc, bs));
             else FN_CUDA(launch_pdl(step_beam_kernel<true, false>, grid, block, s->split_smem, s->stream, b, a, s->d_step_end, epc, bs));
         } else {
@@ -835,6 +883,15 @@ extern "C" int fn_sim_beam_config(const fn_sim* s, int* cfg) {
     if (!s || !cfg) return fail(FN_ERR_INVALID_ARG, "fn_sim_beam_config: NULL argument");
     cfg[0] = s->use_smem ? 1 : 0; cfg[1] = s->beam_grid; cfg[2] = 512; cfg[3] = (int)s->beam_smem;
     cfg[4] = s->split_on ? 1 : 0; cfg[5] = s->fused_on ? 1 : 0;
+    cfg[6] = s->coarse_on ? 1 : 0; cfg[7] = s->coarse_ok ? 1 : 0;
+    if (s->coarse_on) { cfg[1] = s->beam_grid_c; cfg[2] = 1024; cfg[3] = (int)s->beam_smem_c; }
+    return FN_OK;
+}
+
+extern "C" int fn_sim_set_coarse(fn_sim* s, int enable, int* active_out) {
+    if (!s) return fail(FN_ERR_INVALID_ARG, "fn_sim_set_coarse: NULL sim");
+    s->coarse_on = enable != 0 && s->coarse_ok;
+    if (active_out) *active_out = s->coarse_on ? 1 : 0;
     return FN_OK;
 }
 

@@ -305,7 +305,8 @@ struct __align__(16) FastAxis {                                  // 48 bytes
     uint32_t half_S;         // S / 2
     uint32_t inv_magic;      // ceil(2^32 / S): lines crossed k = umulhi(field difference + S / 2, inv_magic), exact
     uint32_t S;
-    uint32_t pad_[2];
+    uint32_t base_c;         // shared address of the coarse copy - kExpOff (kCoarse)
+    uint32_t par;            // parity of the physical line of the origin (rewritten per task; kCoarse)
 };
 struct __align__(16) FastSlot {                                  // 128 bytes per warp
     double pc, ps;           // cos / sin of the heading (rewritten per task)
@@ -313,7 +314,6 @@ struct __align__(16) FastSlot {                                  // 128 bytes pe
     uint32_t pad_[4];
 };
 constexpr int kNearQueue = 64;                                   // per warp: deferred near-axis beams
-constexpr int kFastWarps = 16;                                   // warps per CTA of the kernels that use the production path
 
 __device__ __forceinline__ double xor_hi(double v, unsigned m) { return __hiloint2double((int)(hiw(v) ^ m), __double2loint(v)); }
 __device__ __forceinline__ double add_hi(double v, unsigned k) { return __hiloint2double((int)(hiw(v) + k), __double2loint(v)); }
@@ -325,11 +325,55 @@ __device__ __forceinline__ double2 lds_d2(uint32_t addr) {
     return v;
 }
 
+// The hot loop: two lines (kCoarse: two PAIRS of lines) per trip.  D = crossing coordinate of the line before
+// the trip's first one; on exit D belongs to the trip's second line, xa / xb are the two (unmasked) windows.
+__device__ __forceinline__ void fast_loop(double& D, uint32_t& xa, uint32_t& xb, const double Md, const double Md2,
+                                          const uint32_t base, const uint32_t hend, const uint32_t mask) {
+    asm volatile(
+        "{\n\t"
+        ".reg .pred ph, pc;\n\t"
+        ".reg .b32 j, a, L, H, lo, hia, hib, xo;\n\t"
+        ".reg .f64 DA;\n\t"
+        "FN_LOOP:\n\t"
+        "add.f64 DA, %0, %3;\n\t"
+        "add.f64 %0, %0, %4;\n\t"
+        "mov.b64 {lo, hia}, DA;\n\t"
+        "shr.u32 j, hia, 5;\n\t"
+        "mad.lo.u32 a, j, 4, %5;\n\t"
+        "ld.shared.u32 L, [a];\n\t"
+        "ld.shared.u32 H, [a+4];\n\t"
+        "shf.r.wrap.b32 %1, L, H, hia;\n\t"
+        "mov.b64 {lo, hib}, %0;\n\t"
+        "shr.u32 j, hib, 5;\n\t"
+        "mad.lo.u32 a, j, 4, %5;\n\t"
+        "ld.shared.u32 L, [a];\n\t"
+        "ld.shared.u32 H, [a+4];\n\t"
+        "shf.r.wrap.b32 %2, L, H, hib;\n\t"
+        "or.b32 xo, %1, %2;\n\t"
+        "and.b32 xo, xo, %7;\n\t"
+        "setp.eq.u32 ph, xo, 0;\n\t"
+        "setp.ne.and.u32 pc, hib, %6, ph;\n\t"
+        "@pc bra FN_LOOP;\n\t"
+        "}"
+        : "+d"(D), "=r"(xa), "=r"(xb)
+        : "d"(Md), "d"(Md2), "r"(base), "r"(hend), "r"(mask));
+}
+// the window of the line with crossing coordinate Dl (base = the copy's base, - 4 for forward beams)
+__device__ __forceinline__ uint32_t fast_window(const uint32_t base, const double Dl) {
+    const uint32_t h = hiw(Dl), a = base + ((h >> 5) << 2);
+    return __funnelshift_r(SmemSpace::ld(a), SmemSpace::ld4(a), h);
+}
+
 // One beam per lane.  slot = shared address of the warp's FastSlot; tab = shared address of the beam's
-// (cos, sin) entry.  near = the beam is within 1.9 deg of an axis (M >= 30.5): not cast here, the caller
-// defers it (fast_chunk / fast_drain).
-__device__ __forceinline__ float cast_beam_fast(const uint32_t slot, const uint32_t tab,
-                                                const double T, const double half_T, const float rho, const float rmax, bool& near) {
+// (cos, sin) entry.  near = the beam is too close to an axis for a 32-bit window (M >= 30.5; with the coarse
+// level 2 M >= 30.5): not cast here, the caller defers it (fast_chunk / fast_drain).
+// kCoarse: the hot loop walks the coarse copy, one window per PAIR of lines (the pairs are aligned in the map, so
+// a beam's first pair may hold one of its lines only); a non-empty window sends the pair's two fine lines through
+// the same tests as without the coarse level, in travel order, so that both variants resolve the same line with
+// the same crossing coordinates (every coordinate is D0 plus exact multiples of M and S): identical results.
+template <bool kCoarse>
+__device__ __forceinline__ float cast_beam_fast(const uint32_t slot, const uint32_t tab, const double T,
+                                                const double half_T, const float rho, const float rmax, bool& near) {
     const double2 cs = lds_d2(tab), pcs = lds_d2(slot);
     const double dx = pcs.x * cs.x - pcs.y * cs.y, dy = pcs.y * cs.x + pcs.x * cs.y;
     const bool mx = fabs(dx) >= fabs(dy);                         // dominant axis is x
@@ -338,67 +382,48 @@ __device__ __forceinline__ float cast_beam_fast(const uint32_t slot, const uint3
     const double r0 = rcp64h(adw);
     const double r1 = fma(fma(-adw, r0, 1.0), r0, r0);
     const double M = fabs(du) * r1;
-    near = !(M < kSlowSlope);                                     // also dw == 0 (M = inf or NaN)
+    near = !(M < (kCoarse ? 0.5 * kSlowSlope : kSlowSlope));      // also dw == 0 (M = inf or NaN)
     float r = rmax;
-    // (a near-axis lane stays with the warp: it walks one pair of lines of a harmless beam of slope 1 and its
-    // result is dropped, so that the whole warp reaches the resolution below converged)
-    {
-        const double Mc = near ? 1.0 : M;
-        const uint32_t ax = slot + (mx ? 16u : 64u);              // the axis record
-        const double2 hq = lds_d2(ax);                            // (h, ouMS)
-        double Sd;
-        uint32_t g2, g3;
-        asm volatile("ld.shared.v2.u32 {%0, %1}, [%2+24];" : "=r"(g2), "=r"(g3) : "r"(ax));
-        asm volatile("ld.shared.f64 %0, [%1+16];" : "=d"(Sd) : "r"(ax));
-        const unsigned su = hiw(du) & 0x80000000u, sw = hiw(dw) & 0x80000000u;   // sign bits: set = backward
-        const unsigned fu1 = (su >> 31) ^ 1u;
-        const double Mm = Mc + kMagic, Mq = Mm - kMagic;         // M on the 2^-32 grid of D
-        const double Mu = xor_hi(Mq, su);                         // +-M along u
-        const double f = xor_hi(hq.x, sw) + 0.5;                  // distance to the first line boundary, in lines
-        const double Md = Mu + xor_hi(Sd, sw);                    // +-M +- S per line
+    // (a near-axis lane stays with the warp: it walks one trip of a harmless beam of slope 1 and its result is
+    // dropped, so that the whole warp reaches the resolution below converged)
+    const double Mc = near ? 1.0 : M;
+    const uint32_t ax = slot + (mx ? 16u : 64u);                  // the axis record
+    const double2 hq = lds_d2(ax);                                // (h, ouMS)
+    double Sd;
+    uint32_t base;
+    asm volatile("ld.shared.f64 %0, [%1+16];" : "=d"(Sd) : "r"(ax));
+    asm volatile("ld.shared.u32 %0, [%1+24];" : "=r"(base) : "r"(ax));
+    const unsigned su = hiw(du) & 0x80000000u, sw = hiw(dw) & 0x80000000u;   // sign bits: set = backward
+    const unsigned fu1 = (su >> 31) ^ 1u;
+    const double Mm = Mc + kMagic, Mq = Mm - kMagic;             // M on the 2^-32 grid of D
+    const double Mu = xor_hi(Mq, su);                             // +-M along u
+    const double f = xor_hi(hq.x, sw) + 0.5;                      // distance to the first line boundary, in lines
+    const double Md = Mu + xor_hi(Sd, sw);                        // +-M +- S per line
+    // D of line 0 = 2^20 + bit offset of the origin's line + 64 + U_1 (+ 1 forward)
+    const double D0 = add_hi(fma(f, Mu, hq.y), fu1);
+    const unsigned sh = 30u - hiw(Mm);                            // candidate mask of a line: floor(M) + 2 cells
+    const uint32_t mask = su ? __funnelshift_r(0xffffffffu, 0u, sh) : __funnelshift_l(0u, 0xffffffffu, sh);
+    base -= fu1 << 2;                                             // forward: the window ENDS at the exit cell
+    const uint32_t h0 = hiw(D0), hc0 = hiw(hq.y);                 // fields of line 0 and of the origin cell
+    double Dh = 0.0;                                              // the hit line's D and exact window (xh != 0: hit)
+    uint32_t xh = 0u;
+    // exact span [entry cell ce, exit cell cx] of the line with crossing coordinate Dl (origin cell in line 0)
+    auto exact = [&](const uint32_t x, const double Dl) -> uint32_t {
+        const uint32_t hl = hiw(Dl);
+        const int cx = (int)(hl - fu1);
+        const int ce = hl == h0 ? (int)hc0 : (int)(hiw(Dl - Mu) - fu1);
+        const unsigned n = 31u - (unsigned)abs(cx - ce);
+        return x & (su ? __funnelshift_r(0xffffffffu, 0u, n) : __funnelshift_l(0u, 0xffffffffu, n));
+    };
+    if constexpr (!kCoarse) {
         const double Md2 = Md + Md;
-        // D of line 0 = 2^20 + bit offset of the origin's line + 64 + U_1 (+ 1 forward)
-        const double D0 = add_hi(fma(f, Mu, hq.y), fu1);
-        const unsigned sh = 30u - hiw(Mm);
-        const uint32_t mask = su ? __funnelshift_r(0xffffffffu, 0u, sh) : __funnelshift_l(0u, 0xffffffffu, sh);
         // P pairs of lines cover floor(T |dw|) + 2 lines; the frame stops beams that leave the map earlier
         const double Pd = near ? 1.0 : fma(half_T, adw, 1.5 + 4503599627370496.0) - 4503599627370496.0;
         double D = D0 - Md;                                       // rotated loop: the increments lead
         const uint32_t hend = hiw(fma(Pd, Md2, D));               // high word of the last pair's second line
-        const uint32_t base = g2 - (fu1 << 2);                    // forward: the window ENDS at the exit cell
-        const uint32_t h0 = hiw(D0), hc0 = hiw(hq.y);             // fields of line 0 and of the origin cell
-        double Dh = 0.0;                                          // the hit line's D and exact window (xh != 0: hit)
-        uint32_t xh = 0u;
         for (;;) {
             uint32_t xa, xb;
-            asm volatile(
-                "{\n\t"
-                ".reg .pred ph, pc;\n\t"
-                ".reg .b32 j, a, L, H, lo, hia, hib, xo;\n\t"
-                ".reg .f64 DA;\n\t"
-                "FN_LOOP:\n\t"
-                "add.f64 DA, %0, %3;\n\t"
-                "add.f64 %0, %0, %4;\n\t"
-                "mov.b64 {lo, hia}, DA;\n\t"
-                "shr.u32 j, hia, 5;\n\t"
-                "mad.lo.u32 a, j, 4, %5;\n\t"
-                "ld.shared.u32 L, [a];\n\t"
-                "ld.shared.u32 H, [a+4];\n\t"
-                "shf.r.wrap.b32 %1, L, H, hia;\n\t"
-                "mov.b64 {lo, hib}, %0;\n\t"
-                "shr.u32 j, hib, 5;\n\t"
-                "mad.lo.u32 a, j, 4, %5;\n\t"
-                "ld.shared.u32 L, [a];\n\t"
-                "ld.shared.u32 H, [a+4];\n\t"
-                "shf.r.wrap.b32 %2, L, H, hib;\n\t"
-                "or.b32 xo, %1, %2;\n\t"
-                "and.b32 xo, xo, %7;\n\t"
-                "setp.eq.u32 ph, xo, 0;\n\t"
-                "setp.ne.and.u32 pc, hib, %6, ph;\n\t"
-                "@pc bra FN_LOOP;\n\t"
-                "}"
-                : "+d"(D), "=r"(xa), "=r"(xb)
-                : "d"(Md), "d"(Md2), "r"(base), "r"(hend), "r"(mask));
+            fast_loop(D, xa, xb, Md, Md2, base, hend, mask);
             // up to two candidate lines, in travel order: the pair's first line (D - Md), then its second (D).
             // Only the exact-span test runs here (per loop exit); the hit itself is resolved once, below.
             uint32_t x = xa & mask, xn = xb & mask;
@@ -406,40 +431,70 @@ __device__ __forceinline__ float cast_beam_fast(const uint32_t slot, const uint3
             if (x == 0u) { x = xn; xn = 0u; Dl = D; }
 #pragma unroll 1
             while (x != 0u) {
-                // exact span [entry cell ce, exit cell cx] of this line (origin cell in the first line)
-                const uint32_t hl = hiw(Dl);
-                const int cx = (int)(hl - fu1);
-                const int ce = hl == h0 ? (int)hc0 : (int)(hiw(Dl - Mu) - fu1);
-                const unsigned n = 31u - (unsigned)abs(cx - ce);
-                const uint32_t xe = x & (su ? __funnelshift_r(0xffffffffu, 0u, n) : __funnelshift_l(0u, 0xffffffffu, n));
+                const uint32_t xe = exact(x, Dl);
                 if (xe != 0u) { xh = xe; Dh = Dl; break; }
                 x = xn; xn = 0u; Dl = D;                          // the extra cell behind the entry: next line / resume
             }
             if (xh != 0u || hiw(D) == hend) break;
         }
-        __syncwarp();                                             // resolve all hits of the warp together
-        if (xh != 0u) {                                           // later lines are farther away
-            const uint32_t hl = hiw(Dh);
-            const bool first = hl == h0;
-            const int cx = (int)(hl - fu1);
-            const double Dp = Dh - Mu;                            // entry crossing, same line field
-            const int ce = first ? (int)hc0 : (int)(hiw(Dp) - fu1);
-            // first occupied cell in travel order: highest bit backward, lowest bit forward
-            const int c = cx - (int)(fu1 * 31u) + (31 - __clz(su ? xh : xh & (0u - xh)));
-            // lines crossed: the integer fields of line k and line 0 differ by +-k S +- (cells along u)
-            uint32_t half_S, inv_magic, S;
-            asm volatile("ld.shared.u32 %0, [%1+28];" : "=r"(half_S) : "r"(ax));
-            asm volatile("ld.shared.v2.u32 {%0, %1}, [%2+32];" : "=r"(inv_magic), "=r"(S) : "r"(ax));
-            const unsigned dq = sw ? h0 - hl : hl - h0;
-            const unsigned k = __umulhi(dq + half_S, inv_magic);
-            const unsigned lf = sw ? 0u - k * S : k * S;          // line field of line k relative to line 0
-            // entry distance along u: through the line boundary (c == ce) or through the cell's u-face
-            const double a = c == ce ? add_hi(Dp, 0u - lf) : __hiloint2double((int)((unsigned)c + (su >> 31) - lf), 0);
-            const double b = c == ce ? add_hi(hq.y, fu1) : hq.y;
-            const double dU = (c == ce && first) ? 0.0 : fabs(a - b);
-            const double adu = fabs(du);
-            if (dU < T * adu) r = range_from_du(dU, range_scale(adu, rho));
+    } else {
+        uint32_t base_c, par;                                     // coarse copy; parity of the origin's physical line
+        asm volatile("ld.shared.v2.u32 {%0, %1}, [%2+40];" : "=r"(base_c), "=r"(par) : "r"(ax));
+        const unsigned q = sw ? par : par ^ 1u;                   // 1: the first pair holds two lines of the beam
+        const double Mdc = Md + Md, Mdc2 = Mdc + Mdc;             // per pair: +-2 M +- 2 S
+        // D of pair 0 = exit crossing of its last line, with the bit offset of its even line
+        const double D0c = (D0 + (q ? Mu : 0.0)) - (par ? Sd : 0.0);
+        const unsigned shc = 30u - hiw(Mm + Mq);                  // candidate mask of a pair: floor(2 M) + 2 cells
+        const uint32_t maskc = su ? __funnelshift_r(0xffffffffu, 0u, shc) : __funnelshift_l(0u, 0xffffffffu, shc);
+        // P trips of two pairs cover floor(T |dw|) + 2 lines from any alignment
+        const double Pd = near ? 1.0 : fma(0.5 * half_T, adw, 2.0 + 4503599627370496.0) - 4503599627370496.0;
+        double D = D0c - Mdc;
+        const uint32_t hend = hiw(fma(Pd, Mdc2, D));
+        base_c -= fu1 << 2;
+        const uint32_t h0c = hiw(D0c);
+        const double SA = sw ? Sd : 0.0, SB = sw ? 0.0 : Sd;      // line field of the pair's first / second line in travel order
+        for (;;) {
+            uint32_t xa, xb;
+            fast_loop(D, xa, xb, Mdc, Mdc2, base_c, hend, maskc);
+            uint32_t x = xa & maskc, xn = xb & maskc;
+            double Dg = D - Mdc;
+            if (x == 0u) { x = xn; xn = 0u; Dg = D; }
+#pragma unroll 1
+            while (x != 0u) {                                     // a non-empty pair: its two fine lines
+                const double DA = (Dg - Mu) + SA, DB = Dg + SB;
+                uint32_t wA = fast_window(base, DA) & mask;
+                const uint32_t wB = fast_window(base, DB) & mask;
+                if (hiw(Dg) == h0c && q == 0u) wA = 0u;           // (the first pair's other line lies behind the origin)
+                if (wA != 0u) { const uint32_t xe = exact(wA, DA); if (xe != 0u) { xh = xe; Dh = DA; } }
+                if (xh == 0u && wB != 0u) { const uint32_t xe = exact(wB, DB); if (xe != 0u) { xh = xe; Dh = DB; } }
+                if (xh != 0u) break;
+                x = xn; xn = 0u; Dg = D;
+            }
+            if (xh != 0u || hiw(D) == hend) break;
         }
+    }
+    __syncwarp();                                                 // resolve all hits of the warp together
+    if (xh != 0u) {                                               // later lines are farther away
+        const uint32_t hl = hiw(Dh);
+        const bool first = hl == h0;
+        const int cx = (int)(hl - fu1);
+        const double Dp = Dh - Mu;                                // entry crossing, same line field
+        const int ce = first ? (int)hc0 : (int)(hiw(Dp) - fu1);
+        // first occupied cell in travel order: highest bit backward, lowest bit forward
+        const int c = cx - (int)(fu1 * 31u) + (31 - __clz(su ? xh : xh & (0u - xh)));
+        // lines crossed: the integer fields of line k and line 0 differ by +-k S +- (cells along u)
+        uint32_t half_S, inv_magic, S;
+        asm volatile("ld.shared.u32 %0, [%1+28];" : "=r"(half_S) : "r"(ax));
+        asm volatile("ld.shared.v2.u32 {%0, %1}, [%2+32];" : "=r"(inv_magic), "=r"(S) : "r"(ax));
+        const unsigned dq = sw ? h0 - hl : hl - h0;
+        const unsigned k = __umulhi(dq + half_S, inv_magic);
+        const unsigned lf = sw ? 0u - k * S : k * S;              // line field of line k relative to line 0
+        // entry distance along u: through the line boundary (c == ce) or through the cell's u-face
+        const double a = c == ce ? add_hi(Dp, 0u - lf) : __hiloint2double((int)((unsigned)c + (su >> 31) - lf), 0);
+        const double b = c == ce ? add_hi(hq.y, fu1) : hq.y;
+        const double dU = (c == ce && first) ? 0.0 : fabs(a - b);
+        const double adu = fabs(du);
+        if (dU < T * adu) r = range_from_du(dU, range_scale(adu, rho));
     }
     return r;
 }
@@ -503,10 +558,14 @@ __device__ __forceinline__ void beam_element(const BeamArgs& a, const BeamMap<MS
 // ---- production kernel: warp tasks of chunk_rounds x 32 consecutive beams of ONE env.  What depends on the env
 // only (list entry, pose, output rows) is done once per task; near-axis beams are not cast in place (a
 // divergent walk over single words) but queued per warp and cast 32 at a time (fast_drain).
+template <int kWarps>                                              // warps per CTA
 struct FastShared {
-    FastSlot slot[kFastWarps];
-    uint32_t queue[kFastWarps][kNearQueue];                        // deferred beams: output offsets e * B + j
+    FastSlot slot[kWarps];
+    uint32_t queue[kWarps][kNearQueue];                            // deferred beams: output offsets e * B + j
 };
+// launch shape of the production kernels: two CTAs of 512 threads per SM, or -- with the coarse copies, which
+// double the staged image -- one CTA of 1024
+template <bool kCoarse> struct FastShape { static constexpr int kThreads = kCoarse ? 1024 : 512, kCtas = kCoarse ? 1 : 2; };
 struct FastWarp {
     uint32_t slot;               // shared address of the warp's FastSlot
     uint32_t tab;                // shared address of the beam table
@@ -532,7 +591,8 @@ __device__ __forceinline__ float* ring_row_of(const BeamArgs& a, const unsigned 
     if (slot >= a.ring_cap) slot -= a.ring_cap;
     return a.ring_obs + slot * (unsigned long long)a.ring_row;
 }
-__device__ __forceinline__ FastWarp fast_warp(const BeamArgs& a, FastShared* fs, const double2* s_tab, const uint32_t map_base) {
+template <int kWarps>
+__device__ __forceinline__ FastWarp fast_warp(const BeamArgs& a, FastShared<kWarps>* fs, const double2* s_tab, const uint32_t map_base) {
     const unsigned wib = threadIdx.x >> 5, lane = threadIdx.x & 31;
     FastWarp w;
     w.slot = opaque((uint32_t)__cvta_generic_to_shared(&fs->slot[wib]));
@@ -546,6 +606,10 @@ __device__ __forceinline__ FastWarp fast_warp(const BeamArgs& a, FastShared* fs,
         const uint32_t S = (uint32_t)(lane ? a.map.strideC : a.map.strideR) << 5;
         ax->Sd = (double)S; ax->base = map_base - a.exp_off + (lane ? rowBytes : 0u); ax->half_S = S >> 1;
         ax->inv_magic = lane ? a.inv_magicC : a.inv_magicR; ax->S = S;
+        // the coarse copies follow the fine ones (padded to 16 bytes) when they are staged
+        const unsigned fineBytes = ((rowBytes + (unsigned)(a.map.W + 2 * kLineGuard) * (unsigned)(a.map.strideC << 2)) + 15u) & ~15u;
+        ax->base_c = map_base - a.exp_off + fineBytes + (lane ? (unsigned)coarse_words(a.map.H, a.map.strideR) * 4u : 0u);
+        ax->par = 0u;
     }
     __syncwarp();
     return w;
@@ -564,14 +628,11 @@ __device__ __noinline__ void fast_drain(const BeamArgs& a, const uint32_t queue,
         const unsigned B = (unsigned)a.robot.B;
         const unsigned e = o / B, j = o - e * B;
         const BeamPose* pose = a.poses + e;
-        const double2 pcs = *reinterpret_cast<const double2*>(&pose->c), cs = lds_d2(tab + 16u * j);
-        const double dx = pcs.x * cs.x - pcs.y * cs.y, dy = pcs.y * cs.x + pcs.x * cs.y;
-        const bool mx = fabs(dx) >= fabs(dy);
-        const double du = mx ? dx : dy, dw = mx ? dy : dx;
-        const double adw = fabs(dw);
-        const double r0 = rcp64h(adw);
-        const double M = fabs(du) * fma(fma(-adw, r0, 1.0), r0, r0);
-        const float r = cast_beam_slow<SmemSpace>(bm, pose->o[mx ? 0 : 1], mx, du, dw, M, a.robot.T, a.map.rho, a.robot.rmax).r;
+        // cast_beam: the line-pointer form of the traversal (bit-identical to cast_beam_fast, tested), which sends
+        // beams of M >= 30.5 to the word walk itself -- so a beam gets the same range whichever kernel defers it
+        int hit;
+        uint32_t words = 0;
+        const float r = cast_beam<SmemSpace, false>(bm, pose, lds_d2(tab + 16u * j), a.robot.T, a.map.rho, a.robot.rmax, &hit, words);
         a.out_ranges[o] = r;
         float* ring_row = ring_row_of(a, ring_head, e);
         if (ring_row) ring_row[j] = r;
@@ -579,6 +640,7 @@ __device__ __noinline__ void fast_drain(const BeamArgs& a, const uint32_t queue,
     __syncwarp();
 }
 // one task: beams [jb0, jb1) of env e, jb0 a multiple of 32 (pose = the env's sensing pose, possibly a shared-memory copy)
+template <bool kCoarse>
 __device__ __forceinline__ void fast_chunk(const BeamArgs& a, FastWarp& w, const BeamPose* pose, const unsigned e,
                                            const unsigned jb0, const unsigned jb1, const unsigned long long ring_head) {
     const unsigned lane = threadIdx.x & 31;
@@ -589,6 +651,7 @@ __device__ __forceinline__ void fast_chunk(const BeamArgs& a, FastWarp& w, const
         const uint4 v = *reinterpret_cast<const uint4*>(reinterpret_cast<const char*>(pose) + 32u * lane);
         asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(w.slot + ((0x401000u >> (8u * lane)) & 0xffu)),
                      "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");     // slot offsets 0, 16, 64
+        if (kCoarse && lane) asm volatile("st.shared.u32 [%0], %1;" ::"r"(w.slot + (lane == 1 ? 60u : 108u)), "r"(pose->line_par[lane - 1]) : "memory");
     }
     const int state = pose->state;
     __syncwarp();
@@ -603,7 +666,7 @@ __device__ __forceinline__ void fast_chunk(const BeamArgs& a, FastWarp& w, const
     for (unsigned jb = jb0; jb < jb1; jb += 32u, j += 32u, po += 32, tj += 512u) {
         bool near = false;
         float r = 0.0f;
-        if (state == 0) r = cast_beam_fast(w.slot, min(tj, w.tab_last), a.robot.T, a.half_T, a.map.rho, a.robot.rmax, near);
+        if (state == 0) r = cast_beam_fast<kCoarse>(w.slot, min(tj, w.tab_last), a.robot.T, a.half_T, a.map.rho, a.robot.rmax, near);
         if (j >= B) near = false;
         else if (!near) {
             *po = r;
@@ -619,6 +682,11 @@ __device__ __forceinline__ void fast_chunk(const BeamArgs& a, FastWarp& w, const
     }
 }
 
+// words of the staged image with the coarse copies: fine copies (padded to 16 bytes), then the coarse ones
+__host__ __device__ inline int staged_words_coarse(const MapDev& m) {
+    const int fine = (m.H + 2 * kLineGuard) * m.strideR + (m.W + 2 * kLineGuard) * m.strideC;
+    return ((fine + 3) & ~3) + (int)((coarse_words(m.H, m.strideR) + coarse_words(m.W, m.strideC) + 3) / 4 * 4);
+}
 // Stages the beam table and (when `stage`) both packed copies of the map in shared memory: constants, so
 // the kernels do this BEFORE their dependency wait, under the kernel that precedes them in the stream.
 // The copy is done by the TMA engine: one thread arms an mbarrier with the byte count and issues 1-D bulk
@@ -741,6 +809,7 @@ __device__ __forceinline__ void fast_finish(const BeamArgs& a, FastWarp& w, cons
 // order of magnitude; a static split of such chunks left 13 % of the SM time idle).  Small launches (fewer than
 // eight rounds per warp) use single rounds only.
 // (has_static = false: a warp that arrives late -- fn_step_split.cuh -- has no task of its own)
+template <bool kCoarse>
 __device__ __forceinline__ void run_fast_tasks(const BeamArgs& a, FastWarp& w, const int* list, const int n_env,
                                                const unsigned long long ring_head, const unsigned warp0,
                                                const unsigned nwarps, const bool has_static = true) {
@@ -770,7 +839,7 @@ __device__ __forceinline__ void run_fast_tasks(const BeamArgs& a, FastWarp& w, c
             jb1 = jb0 + 32u;
         }
         const unsigned e = list ? (unsigned)list[le] : le;
-        fast_chunk(a, w, a.poses + e, e, jb0, min(B, jb1), ring_head);
+        fast_chunk<kCoarse>(a, w, a.poses + e, e, jb0, min(B, jb1), ring_head);
         t = __shfl_sync(0xffffffffu, next, 0);
     }
     fast_finish(a, w, ring_head);
@@ -780,8 +849,10 @@ __device__ __forceinline__ void run_fast_tasks(const BeamArgs& a, FastWarp& w, c
 // and the beam table in shared memory -- constants, so this happens BEFORE the dependency wait, under
 // the env-step / reset kernel that precedes it in the stream.
 // kAux = instrumented variant: hit-cell output, map-word counter.
-template <bool kSmem, bool kAux>
-__global__ void __launch_bounds__(512, 2) beam_kernel(const __grid_constant__ BeamArgs a) {
+// kCoarse (production kernel only): the coarse copies are staged too and the hot loop walks them.
+template <bool kSmem, bool kAux, bool kCoarse = false>
+__global__ void __launch_bounds__(FastShape<kCoarse>::kThreads, FastShape<kCoarse>::kCtas) beam_kernel(const __grid_constant__ BeamArgs a) {
+    static_assert(!kCoarse || (kSmem && !kAux), "the coarse level belongs to the production kernel");
     extern __shared__ __align__(16) uint8_t smem_raw[];
     const int B = a.robot.B;
     constexpr bool stage = kSmem;
@@ -790,8 +861,8 @@ __global__ void __launch_bounds__(512, 2) beam_kernel(const __grid_constant__ Be
     double2* s_tab = reinterpret_cast<double2*>(smem_raw);
     uint32_t* s_map = reinterpret_cast<uint32_t*>(smem_raw + (size_t)B * sizeof(double2));
     __shared__ __align__(8) unsigned long long s_mbar;
-    __shared__ __align__(16) typename std::conditional<fast, FastShared, int>::type s_fast;
-    stage_beam_constants(a, s_tab, s_map, mapWords, stage, &s_mbar);
+    __shared__ __align__(16) typename std::conditional<fast, FastShared<FastShape<kCoarse>::kThreads / 32>, int>::type s_fast;
+    stage_beam_constants(a, s_tab, s_map, kCoarse ? staged_words_coarse(a.map) : mapWords, stage, &s_mbar);
     __syncthreads();
     griddep_wait();                                                // poses / list / count come from the previous kernel
     griddep_launch_dependents();
@@ -812,7 +883,7 @@ __global__ void __launch_bounds__(512, 2) beam_kernel(const __grid_constant__ Be
     const unsigned rowBytes = (unsigned)(a.map.H + 2 * kLineGuard) * (unsigned)(a.map.strideR << 2);
     if constexpr (fast) {
         FastWarp w = fast_warp(a, &s_fast, s_tab, (uint32_t)__cvta_generic_to_shared(s_map));
-        run_fast_tasks(a, w, list, n_env, ring_head, warp0, nwarps);
+        run_fast_tasks<kCoarse>(a, w, list, n_env, ring_head, warp0, nwarps);
     } else if (stage) {
         BeamMap<SmemSpace> bm;
         bm.base = (uint32_t)__cvta_generic_to_shared(s_map);

@@ -30,6 +30,13 @@ struct MapDev {
 };
 constexpr int kCellShift = 64;     // cell u is stored at bit position u + kCellShift of its line
 constexpr int kLineGuard = 2;      // physical line = l + kLineGuard
+// Coarse level of a copy: line g = the OR of the physical lines 2g and 2g + 1 (a missing odd line counts as
+// all ones), same cell -> bit mapping, stored at word offset g * 2 * stride, i.e. at the BIT offset of the fine
+// line 2g within its copy: a crossing coordinate D (fn_beam.cuh) addresses the coarse line of a pair and
+// the pair's even fine line with the same bits.  One guard pair (all ones) follows the last one.
+__host__ __device__ inline size_t coarse_words(int L, int stride) {
+    return (size_t)((L + 2 * kLineGuard + 1) / 2 + 1) * 2 * (size_t)stride;
+}
 
 // Per-env sensing pose, written by the env/reset/pose kernels, read by the beam kernel.  The beam
 // kernel walks along the beam's dominant axis "u" (minor axis "w"); both choices are prepared here:
@@ -48,7 +55,7 @@ struct __align__(32) BeamPose {
     BeamOrient o[2];
     int state;               // 0 = origin in a free cell, 1 = in an occupied cell, 2 = outside the map
     int psi_bits;            // bit pattern of the fp32 heading that (c, s) belong to
-    int pad_[2];
+    unsigned line_par[2];    // parity of the physical line of the origin in o[0] / o[1] (coarse level: which line of its pair)
 };
 
 struct RobotDev {

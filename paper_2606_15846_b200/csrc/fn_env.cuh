@@ -220,7 +220,6 @@ __device__ __forceinline__ BeamPose make_pose(const MapDev& m, const RobotDev& r
     BeamPose p;
     p.c = c; p.s = s;
     p.psi_bits = __float_as_int(psif);
-    p.pad_[0] = p.pad_[1] = 0;
     const bool in = ox >= 0.0 && ox < (double)m.W && oy >= 0.0 && oy < (double)m.H;   // false for NaN
     const int jx = in ? __double2int_rd(ox) : 0, iy = in ? __double2int_rd(oy) : 0;
     p.state = !in ? 2 : (occ_global<kS>(m, iy, jx) ? 1 : 0);
@@ -230,6 +229,7 @@ __device__ __forceinline__ BeamPose make_pose(const MapDev& m, const RobotDev& r
     p.o[0].line_off = (unsigned)(iy + kLineGuard) * (unsigned)m.strideR * 4u;
     p.o[1].ouM = oy + ((double)kCellShift + kMagic); p.o[1].h = 0.5 - fx; p.o[1].cu0 = iy;
     p.o[1].line_off = rowBytes + (unsigned)(jx + kLineGuard) * (unsigned)m.strideC * 4u;
+    p.line_par[0] = (unsigned)(iy + kLineGuard) & 1u; p.line_par[1] = (unsigned)(jx + kLineGuard) & 1u;
     p.o[0].ouMS = p.o[0].ouM + (double)(p.o[0].line_off << 3);
     p.o[1].ouMS = p.o[1].ouM + (double)((p.o[1].line_off - rowBytes) << 3);
     return p;

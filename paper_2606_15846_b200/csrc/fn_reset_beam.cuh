@@ -40,7 +40,7 @@ __global__ void __launch_bounds__(kFusedThreads, 2) reset_beam_kernel(const __gr
     uint8_t* s_scr = reinterpret_cast<uint8_t*>(s_pose + kFusedPoseSlots);
     const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31;
     __shared__ __align__(8) unsigned long long s_mbar;
-    __shared__ __align__(16) typename std::conditional<!kAux, FastShared, int>::type s_fast;
+    __shared__ __align__(16) typename std::conditional<!kAux, FastShared<kFusedThreads / 32>, int>::type s_fast;
     stage_beam_constants(a, s_tab, s_map, mapWords, true, &s_mbar);
     ColScratch scratch = col_scratch(s_scr + (size_t)(wib < kFusedResetWarps ? wib : 0) * col_scratch_bytes(V), V);
     if (wib < kFusedResetWarps)
@@ -75,7 +75,7 @@ __global__ void __launch_bounds__(kFusedThreads, 2) reset_beam_kernel(const __gr
         for (unsigned task = (unsigned)wib; task < ntasks; task += blockDim.x >> 5) {
             const unsigned k = a.inv_rounds ? __umulhi(task, a.inv_rounds) : task / rounds, jb0 = (task - k * rounds) << 5;
             const unsigned e = (unsigned)rlist[blockIdx.x + k * gridDim.x];
-            fast_chunk(a, w, k < (unsigned)kFusedPoseSlots ? s_pose + k : a.poses + e, e, jb0, min((unsigned)B, jb0 + 32u), ring_head);
+            fast_chunk<false>(a, w, k < (unsigned)kFusedPoseSlots ? s_pose + k : a.poses + e, e, jb0, min((unsigned)B, jb0 + 32u), ring_head);
         }
         fast_finish(a, w, ring_head);
     } else {                                                       // instrumented: 32 consecutive (env, beam) pairs per warp task

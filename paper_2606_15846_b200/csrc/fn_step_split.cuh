@@ -40,8 +40,8 @@ __host__ __device__ inline size_t step_split_smem_bytes(size_t beam_smem, int V)
 }
 
 // beam_smem = the beam kernel's dynamic shared bytes (beam table [+ packed map]); epc = envs owned per CTA
-template <bool kSmem, bool kAux>
-__global__ void __launch_bounds__(512, 2) step_beam_kernel(const __grid_constant__ BeamArgs a, const __grid_constant__ EnvArgs ea, StepEnd* end, int epc, unsigned beam_smem) {
+template <bool kSmem, bool kAux, bool kCoarse = false>
+__global__ void __launch_bounds__(FastShape<kCoarse>::kThreads, FastShape<kCoarse>::kCtas) step_beam_kernel(const __grid_constant__ BeamArgs a, const __grid_constant__ EnvArgs ea, StepEnd* end, int epc, unsigned beam_smem) {
     extern __shared__ __align__(16) uint8_t smem_raw[];
     const int B = a.robot.B, V = a.robot.V;
     const int rowWords = (a.map.H + 2 * kLineGuard) * a.map.strideR;
@@ -51,8 +51,8 @@ __global__ void __launch_bounds__(512, 2) step_beam_kernel(const __grid_constant
     const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31, last_warp = (int)(blockDim.x >> 5) - 1;
     __shared__ __align__(8) unsigned long long s_mbar;
     constexpr bool fast = kSmem && !kAux;
-    __shared__ __align__(16) typename std::conditional<fast, FastShared, int>::type s_fast;
-    stage_beam_constants(a, s_tab, s_map, mapWords, kSmem, &s_mbar);
+    __shared__ __align__(16) typename std::conditional<fast, FastShared<FastShape<kCoarse>::kThreads / 32>, int>::type s_fast;
+    stage_beam_constants(a, s_tab, s_map, kCoarse ? staged_words_coarse(a.map) : mapWords, kSmem, &s_mbar);
     const ColScratch scratch = col_scratch(smem_raw + step_split_scratch_offset(beam_smem), V);
     if (wib == last_warp)
         for (int k = lane; k < V; k += 32) { scratch.verts[k] = a.robot.verts[k]; scratch.nxt[k] = a.robot.nxt[k]; }
@@ -87,7 +87,7 @@ __global__ void __launch_bounds__(512, 2) step_beam_kernel(const __grid_constant
     const unsigned rowBytes = (unsigned)rowWords * 4u;
     if constexpr (fast) {
         FastWarp w = fast_warp(a, &s_fast, s_tab, (uint32_t)__cvta_generic_to_shared(s_map));
-        run_fast_tasks(a, w, nullptr, n, head_new, warp0, nwarps, wib != last_warp);
+        run_fast_tasks<kCoarse>(a, w, nullptr, n, head_new, warp0, nwarps, wib != last_warp);
     } else if (kSmem) {
         BeamMap<SmemSpace> bm;
         bm.base = (uint32_t)__cvta_generic_to_shared(s_map);

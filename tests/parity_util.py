@@ -195,6 +195,21 @@ def run_parity(wl, steps, n=None, subset=None, seed=0, forced=None, check_every=
                 raise AssertionError(f"step {t}: fast beam kernel differs from instrumented one at env {bad[0]} beam {bad[1]}: "
                                      f"{fast[bad[0], bad[1]].item()!r} vs {buf.ranges[bad[0], bad[1]].item()!r}")
             rep.add("fast_path_checks", n * B)
+            # ... and so must the production kernel with the coarse level (where the copies fit one CTA)
+            if s.beam_config()["coarse_available"]:
+                s.bind_aux(None, buf.reward)
+                was = s.beam_config()["coarse"]
+                s.set_coarse(not was)
+                other = torch.empty_like(buf.ranges)
+                s.observe_all(buf.states, other)
+                torch.cuda.synchronize()
+                s.set_coarse(was)
+                s.bind_aux(buf.hit, buf.reward)
+                if not torch.equal(other, buf.ranges):
+                    bad = (other != buf.ranges).nonzero()[0].tolist()
+                    raise AssertionError(f"step {t}: coarse level {'off' if was else 'on'}: beam kernel differs at env {bad[0]} beam {bad[1]}: "
+                                         f"{other[bad[0], bad[1]].item()!r} vs {buf.ranges[bad[0], bad[1]].item()!r}")
+                rep.add("coarse_level_checks", n * B)
         if done.any():
             if check:
                 do_reset(done, seeds_np[t + 1], f"step {t} reset")

@@ -429,6 +429,52 @@ def test_split_step_equals_the_single_env_step_kernel(pu):
         assert out[0][1] == out[1][1] and out[0][1]["envs_reset"] > n
 
 
+def test_coarse_level_on_and_off_give_identical_results(pu):
+    # BASELINE.json north_star "coarse block-occupancy level for empty-space skipping"; SURVEY.md 8(c) pin
+    # "coarse-level on/off => identical".  The production beam kernels either walk the fine copies line by line
+    # or the coarse copies (one window per pair of lines, fine lines only behind a non-empty window): same
+    # states, flags, ranges, goal observations and counters, bit for bit, over steps with resets, for maps staged
+    # in shared memory (C1, C2, C3, ragged sizes, a map without border walls, a sensor offset).
+    import torch
+    from harness import workloads as W
+    cases = [(1, 64), (2, 1500), (3, 2000), (1, 7)]
+    for ci, (cfg, n) in enumerate(cases):
+        wl = W.make_workload(cfg, n_envs=n)
+        if ci == 3:
+            wl.beam_angles = W.beam_table(77, 270.0)
+            wl.occ = wl.occ.copy(); wl.occ[0, :] = 0; wl.occ[-1, :] = 0; wl.occ[:, 0] = 0; wl.occ[:, -1] = 0
+        B, A = wl.n_beams, wl.action_dim
+        steps = 8
+        actions = torch.from_numpy(W.action_tape(wl, steps, 9)).cuda()
+        seeds = torch.from_numpy(W.seed_tape(wl, steps + 1, 9).view(np.int64)).cuda()
+        out = []
+        for coarse in (True, False):
+            m, r, s = pu.make_sim(wl, n)
+            if ci == 2:
+                r.set_sensor(0.1, -0.05, 0.2)
+            assert s.beam_config()["coarse_available"], "the coarse copies of a 512 x 512 map fit one CTA"
+            assert s.set_coarse(coarse) == coarse and s.beam_config()["coarse"] == coarse
+            buf = pu.Buffers(n, B, A)
+            buf.mask.fill_(1)
+            s.reset(buf.states, buf.mask, seeds[0], buf.ranges, buf.gobs)
+            trace = [buf.ranges.clone()]
+            for t in range(steps):
+                buf.mask.zero_()
+                s.step(buf.states, actions[t], float(wl.dt), buf.mask, buf.ranges, buf.col, buf.gobs)
+                trace += [buf.states.clone(), buf.ranges.clone(), buf.gobs.clone(), buf.mask.clone(), buf.col.clone()]
+                s.reset(buf.states, None if t % 2 == 0 else buf.mask, seeds[t + 1], buf.ranges, buf.gobs)
+                trace += [buf.states.clone(), buf.ranges.clone()]
+                full = torch.empty_like(buf.ranges)
+                s.observe_all(buf.states, full)
+                trace.append(full)
+            torch.cuda.synchronize()
+            out.append((trace, s.counters()))
+            s.close(); r.close(); m.close()
+        for k, (a, b) in enumerate(zip(out[0][0], out[1][0])):
+            assert torch.equal(a, b), f"config {cfg}: item {k} differs with the coarse level on"
+        assert out[0][1] == out[1][1]
+
+
 def test_clearance_features_against_the_oracle(pu):
     # NEXT-1 (Eq. (3)): sector-pooled footprint clearances.  Teacher-forced:
     # the oracle computes them in fp64 from the GPU's own fp32 ranges; tolerance 1e-4 m like the ranges

@@ -87,6 +87,15 @@ __device__ __forceinline__ double rcp64h(double x) {             // MUFU.RCP64H:
 }
 __device__ __forceinline__ unsigned hiw(double d) { return (unsigned)__double2hiint(d); }
 
+// Direction of a beam = heading (pcs = cos, sin) rotated by the beam's body-frame angle (cs).  The rounding order
+// is spelled out: left to the compiler, "a * b - c * d" contracts into an fma around either product, and two
+// kernels that chose differently disagree in the last bit of a range now and then.  The case that did occur (one
+// range in ~10^9, found by the 1000-step run): the slope M = |du| * r1 contracted with the "+ 2^20" that puts it on
+// the grid of D in the instrumented kernel only -- one rounding instead of two, M differing by 2^-32 -- so M is
+// rounded by explicit __dmul_rn / __dadd_rn in every kernel.
+__device__ __forceinline__ double beam_dir_x(const double2 pcs, const double2 cs) { return fma(pcs.x, cs.x, -__dmul_rn(pcs.y, cs.y)); }
+__device__ __forceinline__ double beam_dir_y(const double2 pcs, const double2 cs) { return fma(pcs.y, cs.x, __dmul_rn(pcs.x, cs.y)); }
+
 struct BeamHit {
     float r;
     int hit;
@@ -128,7 +137,7 @@ __device__ __noinline__ BeamHit cast_beam_slow(const BeamMap<MS> bm, const BeamO
     int k = 0, ce, cx, c;
     bool last;
     auto enter_line = [&]() {
-        X = fu ? ou + (f + (double)k) * M : ou - (f + (double)k) * M;
+        X = fma(fu ? f + (double)k : -(f + (double)k), M, ou);     // (one rounding, spelled out: see beam_dir_x)
         if (!(X > -1.0)) X = -0.5;                                // clamp into the frame cells (also NaN/inf)
         if (!(X < (double)Wu + 1.0)) X = (double)Wu + 0.5;
         last = !(fabs(X - ou) < Tu);                              // the range limit lies in this line
@@ -173,7 +182,7 @@ __device__ __forceinline__ float cast_beam(const BeamMap<MS>& bm, const BeamPose
                                            const double2 cs, const double T, const float rho, const float rmax,
                                            int* hit, uint32_t& words, const bool pair_lines = false) {
     const double2 pcs = *reinterpret_cast<const double2*>(&pose->c);
-    const double dx = pcs.x * cs.x - pcs.y * cs.y, dy = pcs.y * cs.x + pcs.x * cs.y;
+    const double dx = beam_dir_x(pcs, cs), dy = beam_dir_y(pcs, cs);
     const bool mx = fabs(dx) >= fabs(dy);                         // dominant axis is x
     const BeamOrient o = pose->o[mx ? 0 : 1];
     const double du = mx ? dx : dy, dw = mx ? dy : dx;
@@ -181,7 +190,7 @@ __device__ __forceinline__ float cast_beam(const BeamMap<MS>& bm, const BeamPose
     // slope M = |du / dw| >= 1: one Newton step on the 20-bit reciprocal (relative error ~2^-40)
     const double r0 = rcp64h(adw);
     const double r1 = fma(fma(-adw, r0, 1.0), r0, r0);
-    const double M = adu * r1;
+    const double M = __dmul_rn(adu, r1);                         // (rounded here: see beam_dir_x)
     if (!(M < kSlowSlope)) {                                      // also dw == 0 (M = inf or NaN)
         const BeamHit h = cast_beam_slow<MS>(bm, o, mx, du, dw, M, T, rho, rmax);
         if (kAux) { *hit = h.hit; words += 8; }
@@ -191,7 +200,7 @@ __device__ __forceinline__ float cast_beam(const BeamMap<MS>& bm, const BeamPose
     const unsigned fu1 = (su >> 31) ^ 1u;                         // 1 for beams towards higher u
     // signed slope, distance f to the first line boundary (f = 0.5 + h forward in w, 0.5 - h backward)
     // (quantised to the 2^-32 grid of D, so that every later D +- Md is exact and path-independent)
-    const double Mm = M + kMagic, Mq = Mm - kMagic;
+    const double Mm = __dadd_rn(M, kMagic), Mq = __dadd_rn(Mm, -kMagic);   // (never fma(adu, r1, kMagic): one rounding less)
     const double Md = __hiloint2double((int)(hiw(Mq) ^ su), __double2loint(Mq));
     const double f = __hiloint2double((int)(hiw(o.h) ^ sw), __double2loint(o.h)) + 0.5;
     // D_0 = 2^20 + 64 + U_1 (+ 1 forward): the "+ 1" is one unit of the integer field of the high word
@@ -375,13 +384,13 @@ template <bool kCoarse>
 __device__ __forceinline__ float cast_beam_fast(const uint32_t slot, const uint32_t tab, const double T,
                                                 const double half_T, const float rho, const float rmax, bool& near) {
     const double2 cs = lds_d2(tab), pcs = lds_d2(slot);
-    const double dx = pcs.x * cs.x - pcs.y * cs.y, dy = pcs.y * cs.x + pcs.x * cs.y;
+    const double dx = beam_dir_x(pcs, cs), dy = beam_dir_y(pcs, cs);
     const bool mx = fabs(dx) >= fabs(dy);                         // dominant axis is x
     const double du = mx ? dx : dy, dw = mx ? dy : dx;
     const double adw = __hiloint2double((int)(hiw(dw) & 0x7fffffffu), __double2loint(dw));
     const double r0 = rcp64h(adw);
     const double r1 = fma(fma(-adw, r0, 1.0), r0, r0);
-    const double M = fabs(du) * r1;
+    const double M = __dmul_rn(fabs(du), r1);                     // (rounded here: see beam_dir_x)
     near = !(M < (kCoarse ? 0.5 * kSlowSlope : kSlowSlope));      // also dw == 0 (M = inf or NaN)
     float r = rmax;
     // (a near-axis lane stays with the warp: it walks one trip of a harmless beam of slope 1 and its result is
@@ -395,7 +404,7 @@ __device__ __forceinline__ float cast_beam_fast(const uint32_t slot, const uint3
     asm volatile("ld.shared.u32 %0, [%1+24];" : "=r"(base) : "r"(ax));
     const unsigned su = hiw(du) & 0x80000000u, sw = hiw(dw) & 0x80000000u;   // sign bits: set = backward
     const unsigned fu1 = (su >> 31) ^ 1u;
-    const double Mm = Mc + kMagic, Mq = Mm - kMagic;             // M on the 2^-32 grid of D
+    const double Mm = __dadd_rn(Mc, kMagic), Mq = __dadd_rn(Mm, -kMagic);   // M on the 2^-32 grid of D
     const double Mu = xor_hi(Mq, su);                             // +-M along u
     const double f = xor_hi(hq.x, sw) + 0.5;                      // distance to the first line boundary, in lines
     const double Md = Mu + xor_hi(Sd, sw);                        // +-M +- S per line

@@ -28,6 +28,8 @@ def make_sim(wl, n=None):
                  components=getattr(wl, "components", None))
     if getattr(wl, "acc_limits", None) is not None:
         r.set_acc_limits(wl.acc_limits)
+    if getattr(wl, "sensor", None) is not None:                     # sensor placement S (reading G8)
+        r.set_sensor(*[float(v) for v in wl.sensor])
     s = fn.Sim(m, r, n, goal_tol=float(wl.goal_tol), max_episode_steps=wl.max_episode_steps,
                goal_dist_min=float(wl.goal_dist_min), goal_dist_max=float(wl.goal_dist_max),
                r_success=float(wl.r_success), r_collision=float(wl.r_collision), c_progress=float(wl.c_progress))
@@ -67,7 +69,8 @@ class Report:
 
 def check_observation(wl, rep, x, y, psi, g_ranges, g_hit, env_idx=None, tag="obs"):
     """ranges / hit cells of the listed envs at fp32 poses (x, y, psi) vs the oracle."""
-    r, hit, amb = oracle.ranges(wl.occ, wl.resolution, wl.beam_angles, wl.max_range, x, y, psi)
+    r, hit, amb = oracle.ranges(wl.occ, wl.resolution, wl.beam_angles, wl.max_range, x, y, psi,
+                                sensor=getattr(wl, "sensor", None))
     ok = amb == 0
     rep.add("beams", ok.size)
     rep.add("beams_ambiguous", (~ok).sum())
@@ -84,9 +87,10 @@ def check_observation(wl, rep, x, y, psi, g_ranges, g_hit, env_idx=None, tag="ob
     assert np.all(np.isfinite(g_ranges)) and g_ranges.min() >= 0 and g_ranges.max() <= float(wl.max_range) + 1e-6
 
 
-def run_parity(wl, steps, n=None, subset=None, seed=0, forced=None, check_every=1):
+def run_parity(wl, steps, n=None, subset=None, seed=0, forced=None, check_every=1, full_every=None):
     """Free-running GPU trajectory, teacher-forced oracle check each `check_every` steps.
-    subset: number of envs (a fixed random sample) whose beams are checked; None = all."""
+    subset: number of envs (a fixed random sample) whose beams are checked; None = all.
+    full_every: the beams of ALL envs are checked on steps 0, 1, 2 and every full_every-th one."""
     n = wl.n_envs if n is None else n
     wl.n_envs = n
     B, A = wl.n_beams, wl.action_dim
@@ -174,42 +178,62 @@ def run_parity(wl, steps, n=None, subset=None, seed=0, forced=None, check_every=
             assert np.all(close_state(g[0], og[0])), f"step {t}: goal distance"
             far = og[0] > 1e-3
             assert np.all(ang_diff(g[1], og[1])[far] <= 1e-5), f"step {t}: goal direction"
-            # reward / done from the GPU's own d (so that the fp32 threshold decision is taken on the same bits)
+            # reward / done from the ORACLE's own d and collision flag.  Near-tie class of the goal threshold: the
+            # decision d < goal_tol is taken on an fp32 d that may differ from the oracle's by 1e-5 (tolerance above),
+            # so envs with |d - goal_tol| < 1e-5 (and ambiguous collision flags) are excluded and counted.
             d_prev, ep = d_prev0.copy(), ep0.copy()
-            rew, odone = oracle.reward_done(g[0], gcol, forced_np[t], d_prev, ep, float(wl.goal_tol), wl.max_episode_steps,
+            tie = (np.abs(og[0].astype(np.float64) - float(wl.goal_tol)) < 1e-5) | ~okc
+            rep.add("done_checks", n)
+            rep.add("done_ambiguous", tie.sum())
+            rew, odone = oracle.reward_done(og[0], flag, forced_np[t], d_prev, ep, float(wl.goal_tol), wl.max_episode_steps,
                                             float(wl.r_success), float(wl.r_collision), float(wl.c_progress))
-            assert np.array_equal(done, odone), f"step {t}: done flags"
-            assert np.allclose(buf.reward.cpu().numpy(), rew, atol=1e-4), f"step {t}: reward"
+            assert np.array_equal(done[~tie], odone[~tie]), f"step {t}: done flags"
+            assert np.allclose(buf.reward.cpu().numpy()[~tie], rew[~tie], atol=1e-4), f"step {t}: reward"
             gd, ge = s.episode_state()
-            assert np.array_equal(ge, ep) and np.array_equal(gd, d_prev)
-            check_observation(wl, rep, x[sel], y[sel], psi[sel], buf.ranges.cpu().numpy()[sel], buf.hit.cpu().numpy()[sel],
-                              sel, f"step {t}")
-            # the production (non-instrumented) beam kernel must give bit-identical ranges
+            assert np.array_equal(ge[~tie], ep[~tie]) and np.allclose(gd[~tie], d_prev[~tie], atol=1e-5)
+            # (and, on the GPU's own bits, everything is exact: same d, same flags => same decisions)
+            d_prev2, ep2 = d_prev0.copy(), ep0.copy()
+            rew2, odone2 = oracle.reward_done(g[0], gcol, forced_np[t], d_prev2, ep2, float(wl.goal_tol), wl.max_episode_steps,
+                                              float(wl.r_success), float(wl.r_collision), float(wl.c_progress))
+            assert np.array_equal(done, odone2) and np.array_equal(ge, ep2) and np.array_equal(gd, d_prev2), f"step {t}: done / episode state"
+            selt = np.arange(n) if full_every is not None and (t < 3 or t % full_every == 0) else sel
+            check_observation(wl, rep, x[selt], y[selt], psi[selt], buf.ranges.cpu().numpy()[selt], buf.hit.cpu().numpy()[selt],
+                              selt, f"step {t}")
+            # The production (non-instrumented) beam kernel must give bit-identical ranges -- on the same sensing
+            # poses.  fn_observe_all builds the poses from the state planes (a fresh sincos of the fp32 heading),
+            # fn_step keeps cos / sin of the heading across steps (rotation by the step's angle, exact sincos every
+            # 32nd episode step: ~2e-16 per step), so the two pose sets differ in the last bits and, about once in
+            # 10^9 beams, so does the last bit of a range (found by the 1000-step run).  Hence: instrumented and
+            # production kernel both through fn_observe_all = bit-equal; maintained rows against them = equal up to
+            # one fp32 ulp on at most 1e-5 of the beams (counted).
+            hit2 = torch.empty_like(buf.hit)
+            s.bind_aux(hit2, buf.reward)
+            inst = torch.empty_like(buf.ranges)
+            s.observe_all(buf.states, inst)
             s.bind_aux(None, buf.reward)
             fast = torch.empty_like(buf.ranges)
             s.observe_all(buf.states, fast)
             torch.cuda.synchronize()
-            s.bind_aux(buf.hit, buf.reward)
-            if not torch.equal(fast, buf.ranges):
-                bad = (fast != buf.ranges).nonzero()[0].tolist()
+            if not torch.equal(fast, inst):
+                bad = (fast != inst).nonzero()[0].tolist()
                 raise AssertionError(f"step {t}: fast beam kernel differs from instrumented one at env {bad[0]} beam {bad[1]}: "
-                                     f"{fast[bad[0], bad[1]].item()!r} vs {buf.ranges[bad[0], bad[1]].item()!r}")
+                                     f"{fast[bad[0], bad[1]].item()!r} vs {inst[bad[0], bad[1]].item()!r}")
             rep.add("fast_path_checks", n * B)
+            assert_rows_equal_up_to_pose_rounding(rep, inst, buf.ranges, f"step {t}: maintained rows vs fn_observe_all")
             # ... and so must the production kernel with the coarse level (where the copies fit one CTA)
             if s.beam_config()["coarse_available"]:
-                s.bind_aux(None, buf.reward)
                 was = s.beam_config()["coarse"]
                 s.set_coarse(not was)
                 other = torch.empty_like(buf.ranges)
                 s.observe_all(buf.states, other)
                 torch.cuda.synchronize()
                 s.set_coarse(was)
-                s.bind_aux(buf.hit, buf.reward)
-                if not torch.equal(other, buf.ranges):
-                    bad = (other != buf.ranges).nonzero()[0].tolist()
+                if not torch.equal(other, fast):
+                    bad = (other != fast).nonzero()[0].tolist()
                     raise AssertionError(f"step {t}: coarse level {'off' if was else 'on'}: beam kernel differs at env {bad[0]} beam {bad[1]}: "
-                                         f"{other[bad[0], bad[1]].item()!r} vs {buf.ranges[bad[0], bad[1]].item()!r}")
+                                         f"{other[bad[0], bad[1]].item()!r} vs {fast[bad[0], bad[1]].item()!r}")
                 rep.add("coarse_level_checks", n * B)
+            s.bind_aux(buf.hit, buf.reward)
         if done.any():
             if check:
                 do_reset(done, seeds_np[t + 1], f"step {t} reset")
@@ -221,7 +245,7 @@ def run_parity(wl, steps, n=None, subset=None, seed=0, forced=None, check_every=
     full_g = torch.empty_like(buf.gobs)
     s.observe_all(buf.states, full_r, full_g)
     torch.cuda.synchronize()
-    assert torch.equal(full_r, buf.ranges), "observe_all differs from incrementally maintained ranges"
+    assert_rows_equal_up_to_pose_rounding(rep, full_r, buf.ranges, "observe_all vs incrementally maintained ranges")
     assert torch.equal(full_g, buf.gobs), "observe_all differs from incrementally maintained goal obs"
     rep.add("steps", steps)
     rep.add("done_events", n_done)
@@ -231,4 +255,27 @@ def run_parity(wl, steps, n=None, subset=None, seed=0, forced=None, check_every=
     assert cnt["reset_failures"] == rep.c.get("reset_failures", 0) or check_every > 1
     s.close(); r.close(); m.close()
     oracle.set_footprint_components(None)
+    assert_ambiguity_bounds(rep)
     return rep
+
+
+def assert_rows_equal_up_to_pose_rounding(rep, a, b, tag):
+    """Ranges cast from two pose sets that differ by the rounding of cos / sin of the heading (see run_parity):
+    equal, except for one fp32 ulp on at most 1e-5 of the beams."""
+    diff = a != b
+    k = int(diff.sum().item())
+    rep.add("pose_rounding_checks", a.numel())
+    rep.add("pose_rounding_ulp_diffs", k)
+    if k:
+        worst = (a[diff].double() - b[diff].double()).abs().max().item()
+        assert k <= max(1, 1e-5 * a.numel()) and worst <= 1e-6 * max(1.0, float(a.max().item())), \
+            f"{tag}: {k} ranges differ, worst by {worst!r}"
+
+
+def assert_ambiguity_bounds(rep):
+    """The excluded near-tie classes must stay small: an exclusion class that grows would hide mismatches."""
+    c = rep.c
+    assert c.get("beams_ambiguous", 0) <= max(2, 1e-3 * c.get("beams", 0)), f"too many ambiguous beams: {rep}"
+    assert c.get("collision_ambiguous", 0) <= max(2, 1e-3 * c.get("collision_checks", 0)), f"too many ambiguous collision flags: {rep}"
+    assert c.get("resets_ambiguous", 0) <= max(2, 1e-2 * c.get("resets", 0)), f"too many ambiguous resets: {rep}"
+    assert c.get("done_ambiguous", 0) <= max(2, 1e-3 * c.get("done_checks", 0)), f"too many ambiguous done flags: {rep}"

@@ -181,6 +181,35 @@ def test_ring_rows_and_wraparound_gpu(pu):
         s.close(); r.close(); m.close()
 
 
+def test_sensor_offset_in_the_beam_kernel(pu):
+    # Sensor placement S (PAPER.md:65 "S defines sensor placement", :125; reading G8): beams start at the sensor, not
+    # at the body origin.  The oracle casts from the offset pose (pinned by "sensor offset == moved robot",
+    # tests/test_oracle_ranges.py); here the kernels' ranges and hit cells are compared with it on C2 and C3,
+    # through steps and resets (pose from the motion kernel and from the reset kernels).
+    from harness import workloads as W
+    for cfg in (2, 3):
+        wl = W.make_workload(cfg, n_envs=600)
+        wl.sensor = (0.1, -0.05, 0.2)
+        rep = pu.run_parity(wl, steps=8, subset=160, check_every=2)
+        print(cfg, rep)
+        assert rep.c["beams"] > 100000
+
+
+def test_long_trajectories_c2_and_c5(pu):
+    # the configs run 1000 / 500 steps; full batch on steps 0, 1, 2 and every 100th, a fixed subset of
+    # envs on every step (C5: every 50th step).  Reaches what short runs do not: many episodes per env, the
+    # cached-heading path of the motion kernel (exact sincos only every 32nd episode step), ring wrap-around.
+    from harness import workloads as W
+    wl = W.make_workload(2)
+    rep = pu.run_parity(wl, steps=1000, subset=128, check_every=1, full_every=250)
+    print(rep)
+    assert rep.c["steps"] == 1000 and rep.c["done_events"] > 50 * wl.n_envs // 4
+    wl = W.make_workload(5, n_envs=16384)
+    rep = pu.run_parity(wl, steps=500, subset=96, check_every=50)
+    print(rep)
+    assert rep.c["steps"] == 500
+
+
 def test_full_size_sampled_c3_c4(pu):
     # BASELINE.json's full batch sizes in the launch configuration bench.py times; beams of a fixed random
     # subset of envs against the oracle, everything per-env (motion, collision, goal obs, reward/done) in full.

@@ -124,7 +124,9 @@ int fn_reset(fn_sim* sim, float* states_dev, const uint8_t* mask_dev, const uint
  *   out_reward_dev   [N] fp32: Eq. (1).
  * fn_ring_attach: device replay ring (config 5).  Row = [ranges(B), d, alpha, v_x, v_y, w,
  *   action(A), reward, done] fp32; fn_step appends one row per env at slot (head + e) mod capacity, with
- *   obs = the observation the action was chosen from (the previous fn_step / fn_reset outputs).
+ *   obs = the observation the action was chosen from (the previous fn_step / fn_reset outputs).  A step
+ *   completes the rows [head, head + N) and starts the next N, so capacity >= 2 N (else FN_ERR_INVALID_ARG).
+ *   Evaluation steps (fn_eval_begin .. fn_eval_end) leave the ring and its head untouched.
  * fn_observe_all: recompute ranges and goal obs of ALL envs from states ("Full batch").
  * fn_get_counters: synchronises the stream and copies FN_N_COUNTERS u64 counters to host_out.
  * fn_sim_count_words: 1 = also count 32-bit map words loaded by the beam kernel (slower; default 0). */
@@ -141,8 +143,10 @@ int fn_sim_bind_features(fn_sim* sim, int n_sectors, float* out_z_dev);
 int fn_ring_attach(fn_sim* sim, float* ring_dev, uint64_t capacity_transitions);
 /* ---- uniform replay sampling ("Each replay batch contains U x B transitions sampled uniformly
  * from replay and divided into U minibatches of size B"): gathers n_samples = U * B ring rows.
- * Sample i = the row at slot floor(SplitMix64(seed, i) * filled / 2^64), filled = min(rows completed, capacity),
- * i.e. uniform over the completed rows (with replacement); nothing is written while the ring is empty.
+ * Sample i draws s = floor(SplitMix64(seed, i) * valid / 2^64), valid = min(rows completed, capacity - n_envs), and
+ * takes slot (head - valid + s) mod capacity: uniform (with replacement) over the completed rows outside the
+ * n_envs PENDING rows [head, head + n_envs), which already hold the next observation but stale action / reward /
+ * done; nothing is written while no row is complete.
  * out_rows_dev [n_samples][B + 5 + A + 2] fp32: rows as stored (obs, action, reward, done);
  * out_next_obs_dev [n_samples][B + 5] or NULL: the obs part of the same env's next row (slot + n_envs mod
  * capacity), which the step that completed the row has already written (for a done transition that is the

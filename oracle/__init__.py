@@ -209,14 +209,21 @@ def sample_slot(seed: int, i: int, filled: int) -> int:
     return int(f(seed, i, filled))
 
 
-def ring_sample(ring, capacity, filled, n_envs, B, A, seed, n_samples, want_next=True):
-    """Uniform replay sampling.  ring [capacity, B+5+A+2] f32 -> rows [n,row], next_obs [n,B+5], slots [n]."""
+def ring_valid(capacity: int, total: int, n_envs: int) -> int:
+    """Completed transitions still in the ring and outside the pending window (reading G22)."""
+    lib().fno_ring_valid.restype = C.c_uint64
+    return int(lib().fno_ring_valid(C.c_uint64(capacity), C.c_uint64(total), C.c_int(n_envs)))
+
+
+def ring_sample(ring, capacity, total, n_envs, B, A, seed, n_samples, want_next=True):
+    """Uniform replay sampling after `total` appended rows.  ring [capacity, B+5+A+2] f32 -> rows
+    [n,row], next_obs [n,B+5], slots [n]."""
     assert ring.dtype == np.float32 and ring.flags.c_contiguous
     row = B + 5 + A + 2
     rows = np.empty((n_samples, row), np.float32)
     nxt = np.empty((n_samples, B + 5), np.float32) if want_next else None
     slots = np.empty(n_samples, np.int64)
-    lib().fno_ring_sample(_p(ring, C.c_float), C.c_uint64(capacity), C.c_uint64(filled), C.c_int(n_envs), C.c_int(B),
+    lib().fno_ring_sample(_p(ring, C.c_float), C.c_uint64(capacity), C.c_uint64(total), C.c_int(n_envs), C.c_int(B),
                           C.c_int(A), C.c_uint64(seed), C.c_int(n_samples), _p(rows, C.c_float),
                           _p(nxt, C.c_float), _p(slots, C.c_int64))
     return rows, nxt, slots

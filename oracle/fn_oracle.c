@@ -648,25 +648,36 @@ void fno_clearance_features(int V, const float* fp_xy, int B, const float* angle
 
 /* ------------------------------------------------------------------ O11: replay sampling (NEXT-2)
  * "Each replay batch contains U x B transitions sampled uniformly from replay and divided
- * into U minibatches of size B."  Readings (G22): sample i of a batch draws slot_i = floor(w_i filled /
- * 2^64) with w_i = SplitMix64(seed, i) (the counter-based generator of O7), i.e. uniform over the
- * `filled` completed rows [0, filled) of the ring (filled = min(rows appended, capacity); a ring that
- * has wrapped is full, one that has not is filled from slot 0); the batch row is the ring row
- * (obs, action, reward, done) as stored; the next observation is the obs part of the SAME env's next
- * row, slot + n_envs (mod capacity), which the step that completed the row has already written.
- * (For a done transition that is the post-reset observation; the done flag masks the bootstrap.)
+ * into U minibatches of size B."  Readings (G22): the rows that can be sampled are the COMPLETED transitions
+ * still in the ring.  With `total` rows appended so far, head = total mod capacity is the slot of env 0's
+ * PENDING row: the n_envs rows [head, head + n_envs) already hold the observation the next actions will be
+ * chosen from, but action, reward and done of a transition that has not happened (stale values of the row
+ * they overwrote once the ring has wrapped), so they are excluded: valid = min(total, capacity - n_envs) rows,
+ * the oldest at slot head - valid (mod capacity).  Sample i of a batch draws s_i = floor(w_i valid / 2^64)
+ * with w_i = SplitMix64(seed, i) (the counter-based generator of O7) and takes slot (head - valid + s_i) mod
+ * capacity (before the ring is that full: slot s_i); the batch row is the ring row (obs, action, reward, done)
+ * as stored; the next observation is the obs part of the SAME env's next row, slot + n_envs (mod capacity),
+ * which the step that completed the row has already written (for the newest transitions that is the pending
+ * row).  (For a done transition that is the post-reset observation; the done flag masks the bootstrap.)
  */
 uint64_t fno_sample_slot(uint64_t seed, uint64_t i, uint64_t filled) {
     const uint64_t w = fno_splitmix64(seed, i);
     return (uint64_t)(((unsigned __int128)w * (unsigned __int128)filled) >> 64);
 }
 
-void fno_ring_sample(const float* ring, uint64_t capacity, uint64_t filled, int n_envs, int B, int A,
+uint64_t fno_ring_valid(uint64_t capacity, uint64_t total, int n_envs) {
+    const uint64_t room = capacity > (uint64_t)n_envs ? capacity - (uint64_t)n_envs : 0;
+    return total < room ? total : room;
+}
+void fno_ring_sample(const float* ring, uint64_t capacity, uint64_t total, int n_envs, int B, int A,
                      uint64_t seed, int n_samples, float* out_rows /*[n_samples][row]*/,
                      float* out_next_obs /*[n_samples][B+5] or NULL*/, int64_t* out_slots /*or NULL*/) {
     const size_t row = (size_t)B + 5 + (size_t)A + 2, obs = (size_t)B + 5;
+    const uint64_t valid = fno_ring_valid(capacity, total, n_envs), head = total % capacity;
+    if (valid == 0) return;
     for (int i = 0; i < n_samples; ++i) {
-        const uint64_t slot = fno_sample_slot(seed, (uint64_t)i, filled);
+        const uint64_t si = fno_sample_slot(seed, (uint64_t)i, valid);
+        const uint64_t slot = (head + capacity - valid + si) % capacity;
         memcpy(out_rows + (size_t)i * row, ring + (size_t)slot * row, row * sizeof(float));
         if (out_next_obs)
             memcpy(out_next_obs + (size_t)i * obs, ring + (size_t)((slot + (uint64_t)n_envs) % capacity) * row,

@@ -619,6 +619,12 @@ extern "C" int fn_step(fn_sim* s, float* states, const float* actions, float dt,
     if (!s || !states || !actions || !reset_mask || !out_ranges || !out_collision || !out_goal_obs)
         return fail(FN_ERR_INVALID_ARG, "fn_step: NULL argument");
     if (!std::isfinite(dt) || dt < 0.0f) return fail(FN_ERR_INVALID_ARG, "fn_step: dt must be finite and >= 0");
+    // evaluation steps are not training transitions: they never touch the replay ring or its head
+    struct RingOff {
+        fn_sim* s; float* keep;
+        explicit RingOff(fn_sim* s_) : s(s_), keep(s_->ring) { if (s->eval_mode) s->ring = nullptr; }
+        ~RingOff() { s->ring = keep; }
+    } ring_off(s);
     EnvArgs a;
     a.map = s->map->dev; a.robot = robot_dev(s->robot, s->map); a.task = task_dev(s->task);
     a.n = s->n; a.dt = dt; a.states = states; a.actions = actions; a.reset_mask = reset_mask;
@@ -818,7 +824,8 @@ extern "C" int fn_sim_bind_features(fn_sim* s, int n_sectors, float* out_z) {
 
 extern "C" int fn_ring_attach(fn_sim* s, float* ring, uint64_t cap) {
     if (!s) return fail(FN_ERR_INVALID_ARG, "fn_ring_attach: NULL sim");
-    if (ring && cap < (uint64_t)s->n) return fail(FN_ERR_INVALID_ARG, "fn_ring_attach: capacity must be >= n_envs");
+    // a step completes the rows [head, head + n) and starts the pending rows [head + n, head + 2 n): below 2 n they alias
+    if (ring && cap < 2 * (uint64_t)s->n) return fail(FN_ERR_INVALID_ARG, "fn_ring_attach: capacity must be >= 2 * n_envs");
     s->ring = ring; s->ring_cap = ring ? cap : 0;
     FN_CUDA(cudaMemsetAsync(s->d_ring_head, 0, 2 * sizeof(unsigned long long), s->stream));
     return FN_OK;

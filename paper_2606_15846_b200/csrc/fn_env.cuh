@@ -490,12 +490,17 @@ struct SampleArgs {
 __global__ void __launch_bounds__(256) ring_sample_kernel(SampleArgs a) {
     griddep_wait();
     griddep_launch_dependents();
-    const unsigned long long total = a.head[1];
-    const unsigned long long filled = total < a.cap ? total : a.cap;
-    if (filled == 0ull) return;
+    // completed rows outside the pending window [head, head + n_envs): the oldest at head - valid (reading G22)
+    const unsigned long long total = a.head[1], head = a.head[0];
+    const unsigned long long room = a.cap - (unsigned long long)a.n_envs;          // (cap >= 2 n_envs: fn_ring_attach)
+    const unsigned long long valid = total < room ? total : room;
+    if (valid == 0ull) return;
+    const unsigned long long first = head + a.cap - valid;
     const int lane = threadIdx.x & 31;
     for (int i = blockIdx.x * 8 + (threadIdx.x >> 5); i < a.n_samples; i += gridDim.x * 8) {
-        const unsigned long long slot = __umul64hi(splitmix64_at(a.seed, (unsigned long long)i), filled);
+        unsigned long long slot = first + __umul64hi(splitmix64_at(a.seed, (unsigned long long)i), valid);
+        if (slot >= a.cap) slot -= a.cap;
+        if (slot >= a.cap) slot -= a.cap;
         const float* src = a.ring + slot * (unsigned long long)a.row;
         float* dst = a.out_rows + (size_t)i * a.row;
         for (int k = lane; k < a.row; k += 32) dst[k] = __ldg(src + k);

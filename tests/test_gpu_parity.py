@@ -181,6 +181,60 @@ def test_ring_rows_and_wraparound_gpu(pu):
         s.close(); r.close(); m.close()
 
 
+def test_ring_at_full_scale_c5(pu):
+    # S7 at BASELINE.json config 5's own size: 65 536 envs, ring of 2^22 transitions (12.2 GB), 66 steps, so that the
+    # head wraps (2^22 = 64 x 65 536).  The rows of a fixed sample of 64 envs are checked after every step (4224 rows):
+    # content against the oracle's append of the same envs, slot (head + e) mod capacity in Python integers.
+    import torch
+    import oracle
+    from harness import workloads as W
+    wl = W.make_workload(5)
+    n, B, A = wl.n_envs, wl.n_beams, wl.action_dim
+    cap = 1 << 22
+    row = B + 5 + A + 2
+    m, r, s = pu.make_sim(wl, n)
+    buf = pu.Buffers(n, B, A)
+    s.bind_aux(None, buf.reward)
+    ring = torch.zeros(cap * row, device="cuda")
+    s.ring_attach(ring, cap)
+    ring2 = ring.view(cap, row)
+    steps = 66
+    rng = np.random.default_rng(11)
+    sub = np.sort(rng.choice(n, 64, replace=False))
+    sub_t = torch.from_numpy(sub).cuda()
+    seeds = torch.from_numpy(W.seed_tape(wl, steps + 1, 4).view(np.int64)).cuda()
+    act_rng = np.random.default_rng(12)
+    buf.mask.fill_(1)
+    s.reset(buf.states, buf.mask, seeds[0], buf.ranges, buf.gobs)
+    head = 0
+    rows_checked = 0
+    for t in range(steps):
+        obs_r = buf.ranges[sub_t].cpu().numpy()
+        obs_g = buf.gobs[:, sub_t].cpu().numpy()
+        obs_v = buf.states[3:6, sub_t].cpu().numpy()
+        a_np = (act_rng.random((n, A), dtype=np.float32) * np.array([1.0, 4.0], np.float32) - np.array([0.0, 2.0], np.float32))
+        actions = torch.from_numpy(a_np).cuda()
+        buf.mask.zero_()
+        s.step(buf.states, actions, float(wl.dt), buf.mask, buf.ranges, buf.col, buf.gobs)
+        torch.cuda.synchronize()
+        expect = np.zeros((sub.size, row), np.float32)
+        oracle.ring_append(expect, sub.size, 0, obs_r, obs_g, obs_v, a_np[sub], buf.reward[sub_t].cpu().numpy(),
+                           buf.mask[sub_t].cpu().numpy())
+        slots = torch.tensor([(head + int(e)) % cap for e in sub], device="cuda")
+        got = ring2[slots].cpu().numpy()
+        assert np.array_equal(got, expect), f"step {t}: ring rows of the sampled envs"
+        rows_checked += sub.size
+        head = (head + n) % cap
+        s.reset(buf.states, None, seeds[t + 1], buf.ranges, buf.gobs)
+    assert head == (steps * n) % cap == 2 * n and rows_checked == 4224
+    # rows the wrap has overwritten hold steps 64 and 65; the pending rows hold the current observation
+    pend = torch.tensor([(head + int(e)) % cap for e in sub], device="cuda")
+    assert torch.equal(ring2[pend][:, :B], buf.ranges[sub_t])
+    s.close(); r.close(); m.close()
+    del ring, ring2
+    torch.cuda.empty_cache()
+
+
 def test_sensor_offset_in_the_beam_kernel(pu):
     # Sensor placement S (PAPER.md:65 "S defines sensor placement", :125; reading G8): beams start at the sensor, not
     # at the body origin.  The oracle casts from the offset pose (pinned by "sensor offset == moved robot",
@@ -590,13 +644,13 @@ def test_replay_sampling_against_the_oracle(pu):
         buf.mask.zero_()
         s.step(buf.states, actions[t], float(wl.dt), buf.mask, buf.ranges, buf.col, buf.gobs)
         s.reset(buf.states, None, seeds[t + 1], buf.ranges, buf.gobs)
-        filled = min((t + 1) * n, cap)
+        total = (t + 1) * n
         for seed, with_next in ((1000 + t, True), (2**63 + 12345 + t, False)):
             s.ring_sample(seed, rows, nxt if with_next else None)
             torch.cuda.synchronize()
             ring_np = ring.cpu().numpy().reshape(cap, row)
-            er, en, slots = oracle.ring_sample(ring_np, cap, filled, n, B, A, seed, ns)
-            assert slots.max() < filled
+            er, en, slots = oracle.ring_sample(ring_np, cap, total, n, B, A, seed, ns)
+            assert not set(((total % cap + np.arange(n)) % cap).tolist()) & set(slots.tolist())   # no pending row
             assert np.array_equal(rows.cpu().numpy(), er)
             if with_next:
                 assert np.array_equal(nxt.cpu().numpy(), en)
@@ -645,6 +699,80 @@ def test_paper_fixed_step_query_as_comparison(pu):
     ref = oracle.ranges_fixed_step(wl.occ, wl.resolution, wl.beam_angles, wl.max_range, delta, st[0], st[1], st[2])
     assert np.mean(np.abs(fixed - ref) <= 1e-5) > 0.98 and np.mean(np.abs(fixed - ref) <= delta + 1e-5) > 0.995
     s.close(); r.close(); m.close()
+
+
+def test_ring_untouched_by_evaluation_and_capacity_rule(pu):
+    # Evaluation steps are not training transitions: ring rows and head stay as they were across
+    # fn_eval_begin, evaluation steps and fn_eval_end; training then resumes where it stopped.  And a ring must hold
+    # two batches (the completed rows and the pending ones): smaller capacities are refused.
+    import torch
+    import paper_2606_15846_b200 as fn
+    from harness import workloads as W
+    wl = W.make_workload(1, n_envs=48)
+    n, B, A = wl.n_envs, wl.n_beams, wl.action_dim
+    m, r, s = pu.make_sim(wl, n)
+    buf = pu.Buffers(n, B, A)
+    row = B + 5 + A + 2
+    cap = 5 * n + 3
+    ring = torch.zeros(cap * row, device="cuda")
+    with pytest.raises(fn.FlashNavError):
+        s.ring_attach(ring, 2 * n - 1)
+    s.ring_attach(ring, cap)
+    actions = torch.from_numpy(W.action_tape(wl, 12, 5)).cuda()
+    seeds = torch.from_numpy(W.seed_tape(wl, 13, 5).view(np.int64)).cuda()
+    buf.mask.fill_(1)
+    s.reset(buf.states, buf.mask, seeds[0], buf.ranges, buf.gobs)
+    for t in range(3):
+        buf.mask.zero_()
+        s.step(buf.states, actions[t], float(wl.dt), buf.mask, buf.ranges, buf.col, buf.gobs)
+        s.reset(buf.states, None, seeds[t + 1], buf.ranges, buf.gobs)
+    torch.cuda.synchronize()
+    before = ring.clone()
+    rows = torch.zeros(64, row, device="cuda")
+    s.ring_sample(3, rows, None)
+    keep_states, keep_r, keep_g = buf.states.clone(), buf.ranges.clone(), buf.gobs.clone()
+    est, er, eg = buf.states.clone(), torch.empty_like(buf.ranges), torch.empty_like(buf.gobs)
+    s.eval_begin(est, n, 6, er, eg)
+    for t in range(6):
+        buf.mask.zero_()
+        s.step(est, actions[3 + t], float(wl.dt), buf.mask, er, buf.col, eg)
+    s.eval_end()
+    torch.cuda.synchronize()
+    assert torch.equal(ring, before), "evaluation wrote into the replay ring"
+    rows2 = torch.zeros(64, row, device="cuda")
+    s.ring_sample(3, rows2, None)                                 # same head, same completed rows => same batch
+    torch.cuda.synchronize()
+    assert torch.equal(rows, rows2)
+    s.close(); r.close(); m.close()
+
+
+def test_two_sims_with_different_maps_side_by_side(pu):
+    # the paper's own workflow: a training sim on one map and an evaluation sim on another in one process.
+    # The kernels' shared-memory limit is a property of the function, not of a sim: creating the second, smaller sim
+    # must not break the launches of the first (and vice versa).
+    import torch
+    from harness import workloads as W
+    wl_a, wl_b = W.make_workload(2, n_envs=300), W.make_workload(1, n_envs=64)
+    sims = []
+    for wl in (wl_a, wl_b):
+        m, r, s = pu.make_sim(wl, wl.n_envs)
+        sims.append((wl, m, r, s, pu.Buffers(wl.n_envs, wl.n_beams, wl.action_dim)))
+    for rnd in range(3):
+        for wl, m, r, s, buf in sims:
+            seeds = torch.from_numpy(W.seed_tape(wl, 2, rnd).view(np.int64)).cuda()
+            actions = torch.from_numpy(W.action_tape(wl, 1, rnd)).cuda()
+            if rnd == 0:
+                buf.mask.fill_(1)
+                s.reset(buf.states, buf.mask, seeds[0], buf.ranges, buf.gobs)
+            buf.mask.zero_()
+            s.step(buf.states, actions[0], float(wl.dt), buf.mask, buf.ranges, buf.col, buf.gobs)
+            s.reset(buf.states, None, seeds[1], buf.ranges, buf.gobs)
+            full = torch.empty_like(buf.ranges)
+            s.observe_all(buf.states, full)
+            torch.cuda.synchronize()
+            assert torch.equal(full, buf.ranges)
+    for wl, m, r, s, buf in sims:
+        s.close(); r.close(); m.close()
 
 
 def test_evaluation_mode_completion_masks(pu):

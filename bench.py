@@ -30,11 +30,41 @@ sys.path.insert(0, ROOT)
 
 from harness import workloads as W  # noqa: E402
 
-# dominant kernel (full-batch beam launch), per launch, from the committed ncu --set full capture
-NCU_CAPTURE = {(2, False): {"dram_bytes": 506624, "warp_inst": 45733853, "lanes": 22.05,
-                            "source": "profiles/r1e_beam_kernels_full_c2.txt (dram__bytes_read.sum + dram__bytes_write.sum)"},
-               (2, True): {"dram_bytes": 719360, "warp_inst": 45982954, "lanes": 22.11,
-                           "source": "profiles/r1g_beam_kernels_full_c2.txt (dram__bytes_read.sum + dram__bytes_write.sum)"}}
+import glob
+import re
+
+
+def read_ncu_capture(cfg, kernel_pat):
+    """Per-launch counters of the dominant kernel from the NEWEST committed ncu --set full summary of this config
+    (profiles/r*_beam_kernels_full_c<cfg>.txt), read at run time: never a pasted constant.  Returns None when no
+    summary exists or the kernel is not in it.  The file names the command and the commit it was taken at."""
+    files = sorted(glob.glob(os.path.join(ROOT, "profiles", f"r*_beam_kernels_full_c{cfg}.txt")))
+    if not files:
+        return None
+    path = files[-1]
+    txt = open(path).read()
+    commit = re.search(r"^# commit[: ]+(\S+)", txt, re.M)
+    out = None
+    for sec in txt.split("\n== ")[1:]:
+        if not re.search(kernel_pat, sec.split("\n", 1)[0]):
+            continue
+        def val(name, scale_units=False):
+            mm = re.search(rf"^{re.escape(name)}\s+([0-9.eE+-]+)\s*(\S*)", sec, re.M)
+            if not mm:
+                return None
+            v = float(mm.group(1))
+            if scale_units:
+                v *= {"byte": 1, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}.get(mm.group(2), 1)
+            return v
+        rd, wr = val("dram__bytes_read.sum", True), val("dram__bytes_write.sum", True)
+        out = {"dram_bytes": None if rd is None or wr is None else rd + wr,
+               "warp_inst": val("smsp__inst_executed.sum"),
+               "lanes": val("smsp__thread_inst_executed_per_inst_executed.ratio"),
+               "source": os.path.relpath(path, ROOT) + " (dram__bytes_read.sum + dram__bytes_write.sum, per launch)",
+               "commit": commit.group(1) if commit else None, "kernel": sec.split("\n", 1)[0].strip()}
+        break
+    return out
+
 
 METRIC = "env_steps_per_s"
 UNIT = "env-steps/s"
@@ -42,6 +72,13 @@ UNIT = "env-steps/s"
 
 def workload_name(cfg):
     return f"BASELINE.json configs[{cfg - 1}]" if cfg <= 5 else "extra: C1's robot on C2's map (N sweep, PAPER.md:175 Fig. 5)"
+
+
+def config_dict(cfg, wl):
+    """The workload, in the same words in both arms (launch choices of our arm go under "launch")."""
+    return {"workload": workload_name(cfg), "name": wl.name, "n_envs_per_gpu": int(wl.n_envs), "beams": int(wl.n_beams),
+            "map": list(wl.occ.shape), "max_range_m": float(wl.max_range), "dt": float(wl.dt),
+            "ring": bool(wl.ring_capacity), "config_steps": int(wl.steps)}
 
 
 # --------------------------------------------------------------------------- reference arm = the oracle
@@ -52,6 +89,7 @@ def run_reference(args):
     import oracle
     oracle.build()
     wl = W.make_workload(args.config, n_envs=args.envs or None)
+    cfg_d = config_dict(args.config, wl)
     n = min(wl.n_envs, args.ref_envs)
     wl.n_envs = n
     st = np.zeros((8, n), np.float32)
@@ -84,7 +122,7 @@ def run_reference(args):
     line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": workload_name(args.config), "n_envs_sample": n, "beams": wl.n_beams},
+            "config": cfg_d,
             "rays_per_s": (n * args.steps + resets) * wl.n_beams / dt,
             "cpu_baseline": {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
             "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -191,7 +229,12 @@ def run_ours(args):
 
     wl = W.make_workload(args.config, n_envs=args.envs or None)
     n, B, A = wl.n_envs, wl.n_beams, wl.action_dim
-    K, Wm = args.steps, args.warmup
+    # protocol of PAPER.md:175: precomputed actions, 100 warm-up steps, the config's own step count timed with a
+    # sync at both ends, 5 repetitions, median and IQR (flags override the counts)
+    K = args.steps if args.steps > 0 else int(wl.steps)
+    Wm = args.warmup if args.warmup >= 0 else 100
+    Wm = max(Wm, 3)
+    R = max(1, args.reps)
     tape_len = min(K + Wm, 256)
     actions = torch.from_numpy(W.action_tape(wl, tape_len, seed=wl.seed + 17 * rank)).cuda()
     seeds = torch.from_numpy(W.seed_tape(wl, tape_len + 1, seed=wl.seed + 17 * rank).view(np.int64)).cuda()
@@ -242,19 +285,24 @@ def run_ours(args):
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
-    # ---- timed region: K steps, L2 flushed between them (outside the per-step events)
-    ev0 = [torch.cuda.Event(enable_timing=True) for _ in range(K)]
-    ev1 = [torch.cuda.Event(enable_timing=True) for _ in range(K)]
-    for k in range(K):
-        flush.fill_(k & 0xff)
-        ev0[k].record()
-        step(Wm + k)
-        ev1[k].record()
-    barrier()
+    # ---- timed region: R repetitions of K steps, L2 flushed between steps (outside the per-step events)
+    rep_ms, per_step_all = [], []
+    for rep in range(R):
+        ev0 = [torch.cuda.Event(enable_timing=True) for _ in range(K)]
+        ev1 = [torch.cuda.Event(enable_timing=True) for _ in range(K)]
+        barrier()
+        for k in range(K):
+            flush.fill_(k & 0xff)
+            ev0[k].record()
+            step(Wm + rep * K + k)
+            ev1[k].record()
+        barrier()
+        ps = np.array([ev0[k].elapsed_time(ev1[k]) for k in range(K)])
+        per_step_all.append(ps)
+        rep_ms.append(float(ps.sum()))
     clocks = sampler.stop() if rank == 0 else None
-    per_step_ms = np.array([ev0[k].elapsed_time(ev1[k]) for k in range(K)])
+    per_step_ms = np.concatenate(per_step_all)
     c1 = sim.counters()
-    total_ms = float(per_step_ms.sum())
     # ---- per-kernel durations: the same K steps again with the library's events around each kernel
     # (a separate pass: an event between two kernels keeps the second from starting under the first)
     sim.profile(True)
@@ -385,14 +433,17 @@ def run_ours(args):
                                "peak_source": "MEASURED_PEAKS.json hbm_gbs (of measured)" if hbm else "guide fallback 6.65 TB/s (of fallback)"},
                   "note": "fn::ring_sample_kernel: rows + next observations, L2 flushed before each call; not in the timed step"}
 
-    tmax = torch.tensor([total_ms, steady_ms], device="cuda", dtype=torch.float64)
+    tmax = torch.tensor(rep_ms + [steady_ms], device="cuda", dtype=torch.float64)
     rays = torch.tensor([float(c1["rays_cast"] - c0["rays_cast"]), float(c1["envs_reset"] - c0["envs_reset"])],
                         device="cuda", dtype=torch.float64)
     if world > 1:
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)             # a repetition takes as long as its slowest rank
         dist.all_reduce(rays, op=dist.ReduceOp.SUM)
-    total_ms, steady_ms = float(tmax[0]), float(tmax[1])
-    value = world * n * K / (total_ms * 1e-3)
+    rep_ms, steady_ms = [float(v) for v in tmax[:R]], float(tmax[R])
+    rep_values = np.array([world * n * K / (ms * 1e-3) for ms in rep_ms])
+    total_ms = float(np.median(rep_ms))                          # the median repetition
+    value = float(np.median(rep_values))
+    rays = rays / R                                              # per repetition of K steps
 
     out = None
     if rank == 0:
@@ -408,7 +459,9 @@ def run_ours(args):
         peak = smem_peak if use_smem else l2_peak
         beam_s = beam_ms * 1e-3 / max(1, beam_launches)
         achieved = a_ray * n * B / beam_s
-        ncu = NCU_CAPTURE.get((args.config, bool(split_step)))
+        ncu = read_ncu_capture(args.config, r"step_beam_kernel" if split_step else r"(?<!step_)(?<!reset_)beam_kernel")
+        if ncu and (ncu["warp_inst"] is None or ncu["lanes"] is None):
+            ncu = None
         sm_hz = (clocks or {}).get("sm_mhz") or 1965.0
         issue_peak = 148 * 4 * sm_hz * 1e6                      # warp instructions / s: 1 per scheduler per clock
         roofline = {"bound": "smem" if use_smem else "l2", "kernel": ("fn::step_beam_kernel (fn_step, all envs: beams + collision / goal / reward / done of the split step)"
@@ -419,6 +472,7 @@ def run_ours(args):
                     "kernel_ms": beam_s * 1e3, "share_of_step": beam_ms / (env_ms + beam_ms + reset_ms),
                     "traffic": ncu["dram_bytes"] if ncu else None,
                     "traffic_source": ncu["source"] if ncu else None,
+                    "traffic_commit": ncu["commit"] if ncu else None,
                     "smem_peak_GBps": smem_peak / 1e9, "l2_peak_GBps": l2_peak / 1e9,
                     "beams_per_s": n * B / beam_s,
                     "issue": None if not ncu else {
@@ -464,10 +518,12 @@ def run_ours(args):
         out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
                "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                "dtype": "f64", "data": "synthetic",
-               "config": {"workload": workload_name(args.config), "name": wl.name, "n_envs_per_gpu": n, "beams": B,
-                          "map": list(wl.occ.shape), "max_range_m": float(wl.max_range), "l2": "flushed between timed steps",
-                          "ring": bool(ring is not None), "fused_reset": bool(fused_active), "split_step": bool(split_step),
-                          "coarse_level": bool(coarse_active)},
+               "config": config_dict(args.config, wl),
+               "launch": {"l2": "flushed between timed steps", "ring_attached": bool(ring is not None),
+                          "fused_reset": bool(fused_active), "split_step": bool(split_step), "coarse_level": bool(coarse_active)},
+               "protocol": {"repetitions": R, "value": "median over repetitions", "value_iqr": [float(np.percentile(rep_values, 25)), float(np.percentile(rep_values, 75))],
+                            "values": [float(v) for v in rep_values], "ms_per_step_iqr": [float(np.percentile(rep_ms, 25)) / K, float(np.percentile(rep_ms, 75)) / K],
+                            "note": "PAPER.md:175: warm-up, then K timed steps between syncs, repeated; median and IQR"},
                "rays_per_s": float(rays[0]) / (total_ms * 1e-3),
                "useful_rays_per_s": world * n * B * K / (total_ms * 1e-3),
                "reset_rate_per_step": float(rays[1]) / (world * n * K),
@@ -482,7 +538,22 @@ def run_ours(args):
                "ms_per_step_p50": float(np.median(per_step_ms)), "ms_per_step_p90": float(np.percentile(per_step_ms, 90)),
                "features": feat, "replay_sample": sample, "paper_fixed_step_query": paper_query, "roofline": roofline, "cpu_baseline": cpu, "clocks": clocks,
                # per step: env step (or its motion half), beam kernel, [ring_advance unless split], then fn_reset = one fused kernel or reset + beam kernel
-               "gpu_launches": (2 + (1 if ring is not None and not split_step else 0) + (1 if fused_active else 2)) * K}
+               "gpu_launches": (2 + (1 if ring is not None and not split_step else 0) + (1 if fused_active else 2)) * K * R}
+
+    if rank == 0:
+        # HBM view of the whole step ("report HBM GB/s separately for C5"): state planes in / out,
+        # actions, flags and goal obs, one range row per env, and with a ring its row (obs + action + reward + done)
+        per_env = 32 + 24 + 4 * A + 10 + 4 * B + (4 * (B + 5 + A + 2) if ring is not None else 0)
+        hbm_peak = None
+        try:
+            hbm_peak = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]
+        except Exception:                                        # noqa: BLE001
+            pass
+        pk = hbm_peak if hbm_peak else 6650.0
+        ach = per_env * n * world / (total_ms / K * 1e-3) / 1e9
+        out["hbm"] = {"bytes_per_env_step": per_env, "achieved": ach, "peak": pk * world, "unit": "GB/s", "frac": ach / (pk * world),
+                      "peak_source": "MEASURED_PEAKS.json hbm_gbs (of measured)" if hbm_peak else "guide fallback 6.65 TB/s (of fallback)",
+                      "note": "algorithmic state / observation / ring bytes of one step over the step time; the reset envs' rows add reset_rate x that"}
 
     # ---- end to end through the public API with HOST buffers (copies inside the timed region)
     hs = torch.empty(8, n, dtype=torch.float32).pin_memory()
@@ -522,8 +593,9 @@ def run_ours(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=200)
-    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=0, help="timed steps per repetition (0 = the config's own count, PAPER.md:175)")
+    ap.add_argument("--warmup", type=int, default=-1, help="warm-up steps (-1 = 100, PAPER.md:175)")
+    ap.add_argument("--reps", type=int, default=5, help="repetitions of the timed block (median and IQR are reported)")
     ap.add_argument("--config", type=int, default=2)
     ap.add_argument("--envs", type=int, default=0, help="override the config's env count per GPU (0 = the config's own)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
@@ -543,12 +615,13 @@ def main():
                     help="coarse level in the production beam kernels: -1 = the library's choice")
     ap.add_argument("--ring", type=int, default=1, help="attach the replay ring when the config has one (C5)")
     args = ap.parse_args()
-    if args.warmup < 3:
-        args.warmup = 3
     if args.impl == "reference":
-        if args.steps > 16:
-            args.steps = 16          # bounded: ~1.6 s per C2 step on one core
-        args.warmup = min(args.warmup, 1)
+        # the counts the caller gave are honoured (same accounting as our arm); without flags a bounded sample:
+        # a C2 step takes ~0.9 s on one core
+        if args.steps <= 0:
+            args.steps = 8
+        if args.warmup < 0:
+            args.warmup = 1
         return run_reference(args)
     return run_ours(args)
 

@@ -246,6 +246,22 @@ int fn_step_host(fn_sim* sim, float* states_host, const float* actions_host, flo
                  uint8_t* reset_mask_host, const uint64_t* seeds_host, float* out_ranges_host,
                  uint8_t* out_collision_host, float* out_goal_obs_host);
 
+/* ---- the same, pipelined over two slots: the copies of one step overlap the computation of the next.
+ * fn_step_host_begin(slot) enqueues: host -> device of actions, forced-reset mask and seeds (and of the states when
+ * states_in_host != NULL: the first call must pass them; NULL continues from the states the device holds), fn_step,
+ * fn_reset of the done envs (when seeds_host != NULL), and -- on a copy stream, behind an event -- device -> host of
+ * the post-reset states, the ranges (pre-reset rows of the envs that were not reset, post-reset rows of those that
+ * were, like fn_step_host), the pre-reset collision flags, the goal observations and the done mask (written into
+ * mask_host).  It returns after enqueueing.  fn_step_host_end(slot) blocks until that slot's outputs have arrived.
+ * The next begin (other slot) may be issued before the end of this one: its kernels run while this slot drains
+ * (at C2: 12 MB per step over PCIe against ~0.1 ms of computation).  Host buffers should be pinned and must stay
+ * valid and untouched until the slot's end.  Errors: FN_ERR_INVALID_ARG (NULL, slot not 0 / 1, slot still in
+ * flight, no states yet / nothing in flight), FN_ERR_OOM, FN_ERR_CUDA. */
+int fn_step_host_begin(fn_sim* sim, int slot, const float* states_in_host, const float* actions_host, float dt,
+                       uint8_t* mask_host, const uint64_t* seeds_host, float* out_states_host, float* out_ranges_host,
+                       uint8_t* out_collision_host, float* out_goal_obs_host);
+int fn_step_host_end(fn_sim* sim, int slot);
+
 /* ---- roofline microbenchmarks (same binary, same run): bytes/s of conflict-free ld.shared.u32 x2
  * windows (kind 0), random-word ld.shared (kind 1) and L2-resident ld.global.nc (kind 2). */
 int fn_measure_peak(int kind, void* cuda_stream, double* out_bytes_per_s);

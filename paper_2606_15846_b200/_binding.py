@@ -19,7 +19,7 @@ EXPORTED_SYMBOLS = (
     "fn_map_create", "fn_map_set_regions", "fn_map_destroy", "fn_robot_create", "fn_robot_create_union", "fn_robot_set_sensor", "fn_robot_set_acc_limits",
     "fn_robot_destroy", "fn_task_default", "fn_sim_create", "fn_sim_destroy", "fn_sim_set_stream", "fn_step", "fn_reset",
     "fn_sim_bind_aux", "fn_sim_bind_features", "fn_ring_attach", "fn_ring_sample", "fn_ranges_fixed_step", "fn_eval_begin", "fn_eval_result", "fn_eval_end", "fn_observe_all", "fn_get_counters", "fn_sim_count_words",
-    "fn_sim_episode_state", "fn_sim_beam_config", "fn_sim_set_fused_reset", "fn_sim_set_split_step", "fn_sim_set_coarse", "fn_sim_profile", "fn_sim_profile_read", "fn_step_host", "fn_measure_peak", "fn_last_error", "fn_version")
+    "fn_sim_episode_state", "fn_sim_beam_config", "fn_sim_set_fused_reset", "fn_sim_set_split_step", "fn_sim_set_coarse", "fn_sim_profile", "fn_sim_profile_read", "fn_step_host", "fn_step_host_begin", "fn_step_host_end", "fn_measure_peak", "fn_last_error", "fn_version")
 
 
 class FlashNavError(RuntimeError):
@@ -79,6 +79,8 @@ def load_library():
         "fn_sim_profile": [vp, i32],
         "fn_sim_profile_read": [vp, vp, vp],
         "fn_step_host": [vp, vp, vp, f32, vp, vp, vp, vp, vp],
+        "fn_step_host_begin": [vp, i32, vp, vp, f32, vp, vp, vp, vp, vp, vp],
+        "fn_step_host_end": [vp, i32],
         "fn_measure_peak": [i32, vp, C.POINTER(C.c_double)],
     }
     for name, argtypes in sig.items():
@@ -362,18 +364,33 @@ class Sim:
         _check(load_library().fn_sim_set_coarse(self._h, 1 if enable else 0, C.byref(act)), "fn_sim_set_coarse")
         return bool(act.value)
 
+    @staticmethod
+    def _host_ptr(a, name):
+        if a is None:
+            return None
+        if isinstance(a, np.ndarray):
+            if not a.flags.c_contiguous:
+                raise FlashNavError(f"{name}: not contiguous")
+            return C.c_void_p(a.ctypes.data)
+        if a.is_cuda or not a.is_contiguous():
+            raise FlashNavError(f"{name}: expected a contiguous CPU tensor")
+        return C.c_void_p(a.data_ptr())
+
+    def step_host_begin(self, slot, states_in, actions, dt, reset_mask, seeds, out_states, out_ranges, out_collision, out_goal_obs):
+        """Pipelined end-to-end step (two slots): enqueues copies in, fn_step, fn_reset and the copies out; returns at once."""
+        hp = self._host_ptr
+        _check(load_library().fn_step_host_begin(self._h, int(slot), hp(states_in, "states_in"), hp(actions, "actions"), C.c_float(dt),
+                                                 hp(reset_mask, "reset_mask"), hp(seeds, "seeds"), hp(out_states, "out_states"),
+                                                 hp(out_ranges, "out_ranges"), hp(out_collision, "out_collision"),
+                                                 hp(out_goal_obs, "out_goal_obs")), "fn_step_host_begin")
+
+    def step_host_end(self, slot):
+        """Blocks until the outputs of the slot's step have arrived in its host buffers."""
+        _check(load_library().fn_step_host_end(self._h, int(slot)), "fn_step_host_end")
+
     def step_host(self, states, actions, dt, reset_mask, seeds, out_ranges, out_collision, out_goal_obs):
         """End to end with HOST buffers (numpy arrays or pinned CPU tensors); copies inside the call."""
-        def hp(a, name):
-            if a is None:
-                return None
-            if isinstance(a, np.ndarray):
-                if not a.flags.c_contiguous:
-                    raise FlashNavError(f"{name}: not contiguous")
-                return C.c_void_p(a.ctypes.data)
-            if a.is_cuda or not a.is_contiguous():
-                raise FlashNavError(f"{name}: expected a contiguous CPU tensor")
-            return C.c_void_p(a.data_ptr())
+        hp = self._host_ptr
         _check(load_library().fn_step_host(self._h, hp(states, "states"), hp(actions, "actions"), C.c_float(dt),
                                            hp(reset_mask, "reset_mask"), hp(seeds, "seeds"), hp(out_ranges, "out_ranges"),
                                            hp(out_collision, "out_collision"), hp(out_goal_obs, "out_goal_obs")), "fn_step_host")

@@ -120,6 +120,16 @@ struct fn_sim {
     float *stg_states, *stg_actions, *stg_ranges, *stg_gobs;
     uint8_t *stg_mask, *stg_col;
     unsigned long long* stg_seeds;
+    // fn_step_host_begin / _end: two slots of device staging and events, one copy stream
+    struct HostSlot {
+        float *ranges, *gobs, *states, *actions;
+        uint8_t *mask, *col;
+        unsigned long long* seeds;
+        cudaEvent_t ev_ready, ev_done;
+        bool busy;
+    } hslot[2];
+    cudaStream_t copy_stream;
+    bool pipe_init, pipe_states;     // slots allocated; the device holds the current states
 };
 
 extern "C" const char* fn_last_error(void) { return g_err; }
@@ -529,6 +539,14 @@ extern "C" int fn_sim_destroy(fn_sim* s) {
     if (s->ev) { for (cudaEvent_t e : *s->ev) cudaEventDestroy(e); delete s->ev; delete s->ev_kind; }
     cudaFree(s->stg_states); cudaFree(s->stg_actions); cudaFree(s->stg_ranges); cudaFree(s->stg_gobs);
     cudaFree(s->stg_mask); cudaFree(s->stg_col); cudaFree(s->stg_seeds);
+    if (s->pipe_init) {
+        for (auto& h : s->hslot) {
+            cudaFree(h.ranges); cudaFree(h.gobs); cudaFree(h.states); cudaFree(h.actions); cudaFree(h.mask); cudaFree(h.col); cudaFree(h.seeds);
+            if (h.ev_ready) cudaEventDestroy(h.ev_ready);
+            if (h.ev_done) cudaEventDestroy(h.ev_done);
+        }
+        if (s->copy_stream) cudaStreamDestroy(s->copy_stream);
+    }
     delete s;
     return FN_OK;
 }
@@ -979,5 +997,78 @@ extern "C" int fn_step_host(fn_sim* s, float* states, const float* actions, floa
     if (!direct) FN_CUDA(cudaMemcpyAsync(out_ranges, s->stg_ranges, n * B * sizeof(float), cudaMemcpyDeviceToHost, st));
     FN_CUDA(cudaMemcpyAsync(out_goal_obs, s->stg_gobs, 2 * n * sizeof(float), cudaMemcpyDeviceToHost, st));
     FN_CUDA(cudaStreamSynchronize(st));
+    return FN_OK;
+}
+
+// ------------------------------------------------------------------------------------------ host buffers, pipelined
+// fn_step_host serialises copy in -> step -> reset -> copy out -> sync: at C2 the 12 MB of ranges take ~2.5x the
+// step's own time on PCIe.  Here the states stay on the device, every step writes into one of two slots of
+// device staging, and a slot's outputs drain on a copy stream while the next step already computes.
+static int pipe_alloc(fn_sim* s) {
+    if (s->pipe_init) return FN_OK;
+    const size_t n = (size_t)s->n, B = (size_t)s->robot->B, A = s->robot->drive == FN_DRIVE_DIFF ? 2 : 3;
+    std::memset(s->hslot, 0, sizeof(s->hslot));
+    s->pipe_init = true;                                           // (fn_sim_destroy frees whatever was allocated)
+    FN_CUDA(cudaStreamCreateWithFlags(&s->copy_stream, cudaStreamNonBlocking));
+    if (!s->stg_states) FN_CUDA(cudaMalloc(&s->stg_states, 8 * n * sizeof(float)));
+    for (auto& h : s->hslot) {
+        FN_CUDA(cudaMalloc(&h.ranges, n * B * sizeof(float)));
+        FN_CUDA(cudaMalloc(&h.gobs, 2 * n * sizeof(float)));
+        FN_CUDA(cudaMalloc(&h.states, 8 * n * sizeof(float)));
+        FN_CUDA(cudaMalloc(&h.actions, n * A * sizeof(float)));
+        FN_CUDA(cudaMalloc(&h.mask, n));
+        FN_CUDA(cudaMalloc(&h.col, n));
+        FN_CUDA(cudaMalloc(&h.seeds, n * sizeof(unsigned long long)));
+        FN_CUDA(cudaEventCreateWithFlags(&h.ev_ready, cudaEventDisableTiming));
+        FN_CUDA(cudaEventCreateWithFlags(&h.ev_done, cudaEventDisableTiming));
+    }
+    return FN_OK;
+}
+
+extern "C" int fn_step_host_begin(fn_sim* s, int slot, const float* states_in, const float* actions, float dt,
+                                  uint8_t* mask, const uint64_t* seeds, float* out_states, float* out_ranges,
+                                  uint8_t* out_collision, float* out_goal_obs) {
+    if (!s || !actions || !mask || !out_states || !out_ranges || !out_collision || !out_goal_obs)
+        return fail(FN_ERR_INVALID_ARG, "fn_step_host_begin: NULL argument");
+    if (slot < 0 || slot > 1) return fail(FN_ERR_INVALID_ARG, "fn_step_host_begin: slot must be 0 or 1");
+    int rc = pipe_alloc(s);
+    if (rc != FN_OK) return rc;
+    fn_sim::HostSlot& h = s->hslot[slot];
+    if (h.busy) return fail(FN_ERR_INVALID_ARG, "fn_step_host_begin: slot still in flight (call fn_step_host_end first)");
+    if (!states_in && !s->pipe_states) return fail(FN_ERR_INVALID_ARG, "fn_step_host_begin: the first call must pass the states");
+    const size_t n = (size_t)s->n, B = (size_t)s->robot->B, A = s->robot->drive == FN_DRIVE_DIFF ? 2 : 3;
+    cudaStream_t st = s->stream;
+    if (states_in) FN_CUDA(cudaMemcpyAsync(s->stg_states, states_in, 8 * n * sizeof(float), cudaMemcpyHostToDevice, st));
+    s->pipe_states = true;
+    FN_CUDA(cudaMemcpyAsync(h.actions, actions, n * A * sizeof(float), cudaMemcpyHostToDevice, st));
+    FN_CUDA(cudaMemcpyAsync(h.mask, mask, n, cudaMemcpyHostToDevice, st));
+    if (seeds) FN_CUDA(cudaMemcpyAsync(h.seeds, seeds, n * sizeof(unsigned long long), cudaMemcpyHostToDevice, st));
+    rc = fn_step(s, s->stg_states, h.actions, dt, h.mask, h.ranges, h.col, h.gobs);
+    if (rc != FN_OK) return rc;
+    if (seeds) {
+        rc = fn_reset(s, s->stg_states, nullptr, reinterpret_cast<const uint64_t*>(h.seeds), h.ranges, h.gobs);
+        if (rc != FN_OK) return rc;
+    }
+    // the next step changes the states in place: the slot keeps this step's copy for the drain
+    FN_CUDA(cudaMemcpyAsync(h.states, s->stg_states, 8 * n * sizeof(float), cudaMemcpyDeviceToDevice, st));
+    FN_CUDA(cudaEventRecord(h.ev_ready, st));
+    FN_CUDA(cudaStreamWaitEvent(s->copy_stream, h.ev_ready, 0));
+    cudaStream_t cs = s->copy_stream;
+    FN_CUDA(cudaMemcpyAsync(out_ranges, h.ranges, n * B * sizeof(float), cudaMemcpyDeviceToHost, cs));
+    FN_CUDA(cudaMemcpyAsync(out_states, h.states, 8 * n * sizeof(float), cudaMemcpyDeviceToHost, cs));
+    FN_CUDA(cudaMemcpyAsync(out_goal_obs, h.gobs, 2 * n * sizeof(float), cudaMemcpyDeviceToHost, cs));
+    FN_CUDA(cudaMemcpyAsync(out_collision, h.col, n, cudaMemcpyDeviceToHost, cs));
+    FN_CUDA(cudaMemcpyAsync(mask, h.mask, n, cudaMemcpyDeviceToHost, cs));
+    FN_CUDA(cudaEventRecord(h.ev_done, cs));
+    h.busy = true;
+    return FN_OK;
+}
+
+extern "C" int fn_step_host_end(fn_sim* s, int slot) {
+    if (!s) return fail(FN_ERR_INVALID_ARG, "fn_step_host_end: NULL sim");
+    if (slot < 0 || slot > 1) return fail(FN_ERR_INVALID_ARG, "fn_step_host_end: slot must be 0 or 1");
+    if (!s->pipe_init || !s->hslot[slot].busy) return fail(FN_ERR_INVALID_ARG, "fn_step_host_end: nothing in flight in this slot");
+    FN_CUDA(cudaEventSynchronize(s->hslot[slot].ev_done));
+    s->hslot[slot].busy = false;
     return FN_OK;
 }

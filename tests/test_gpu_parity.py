@@ -459,6 +459,35 @@ def test_step_host_equals_the_device_calls(pu):
             for a, b in zip(got, ref[t]):
                 assert np.array_equal(a, b)
         s.close(); r.close(); m.close()
+    # pipelined form: two slots, step t + 1 is enqueued before step t's outputs are awaited
+    m, r, s = pu.make_sim(wl, n)
+    dev = pu.Buffers(n, B, A)
+    dev.mask.fill_(1)
+    s.reset(dev.states, dev.mask, torch.from_numpy(seeds[0]).cuda(), dev.ranges, dev.gobs)
+    torch.cuda.synchronize()
+    slots = []
+    for k in range(2):
+        slots.append({"s": torch.zeros(8, n).pin_memory(), "r": torch.zeros(n, B).pin_memory(), "g": torch.zeros(2, n).pin_memory(),
+                      "m": torch.zeros(n, dtype=torch.uint8).pin_memory(), "c": torch.zeros(n, dtype=torch.uint8).pin_memory()})
+    h0 = torch.from_numpy(st0).pin_memory()
+    has = [torch.from_numpy(act[t]).pin_memory() for t in range(steps)]
+    hqs = [torch.from_numpy(seeds[t + 1]).pin_memory() for t in range(steps)]
+    with pytest.raises(Exception):
+        s.step_host_end(0)                                       # nothing in flight
+    for t in range(steps + 1):
+        if t < steps:
+            b = slots[t & 1]
+            b["m"].zero_()
+            s.step_host_begin(t & 1, h0 if t == 0 else None, has[t], float(wl.dt), b["m"], hqs[t], b["s"], b["r"], b["c"], b["g"])
+            if t == 0:
+                with pytest.raises(Exception):
+                    s.step_host_begin(0, None, has[0], float(wl.dt), b["m"], hqs[0], b["s"], b["r"], b["c"], b["g"])   # slot in flight
+        if t >= 1:
+            b = slots[(t - 1) & 1]
+            s.step_host_end((t - 1) & 1)
+            for a, e in zip((b["s"], b["r"], b["g"], b["m"], b["c"]), ref[t - 1]):
+                assert np.array_equal(a.numpy(), e), f"pipelined step {t - 1}"
+    s.close(); r.close(); m.close()
 
 
 def test_split_step_equals_the_single_env_step_kernel(pu):

@@ -134,6 +134,28 @@ def ranges(occ, res, angles, max_range, x, y, psi, eps=EPS_CELL, sensor=None, wa
     return (r, hit, amb, vis) if want_visits else (r, hit, amb)
 
 
+def ranges_multi(occ, res, sensors, x, y, psi, eps=EPS_CELL):
+    """A robot with several range sensors (PAPER.md:65, :125).  sensors = [(angles [B_k], max_range, (s_x, s_y, s_psi)), ...];
+    returns ranges [n, sum B_k] f32, hit i32, amb u8, the sensors' beams one after the other."""
+    occ = _u8(occ)
+    x, y, psi = map(_f32, (x, y, psi))
+    H, W = occ.shape
+    n = x.shape[0]
+    Bk = np.array([len(a) for a, _, _ in sensors], np.int32)
+    ang = _f32(np.concatenate([np.asarray(a, np.float32) for a, _, _ in sensors]))
+    rmax = _f32(np.array([m for _, m, _ in sensors], np.float32))
+    plc = _f32(np.array([p for _, _, p in sensors], np.float32).reshape(-1, 3))
+    B = int(Bk.sum())
+    r = np.empty((n, B), np.float32)
+    hit = np.empty((n, B), np.int32)
+    amb = np.empty((n, B), np.uint8)
+    lib().fno_ranges_multi(_p(occ, C.c_uint8), C.c_int(H), C.c_int(W), C.c_float(res), C.c_int(len(sensors)), _p(Bk, C.c_int32),
+                           _p(ang, C.c_float), _p(rmax, C.c_float), _p(plc, C.c_float), C.c_int(n), _p(x, C.c_float),
+                           _p(y, C.c_float), _p(psi, C.c_float), C.c_double(eps), _p(r, C.c_float), _p(hit, C.c_int32),
+                           _p(amb, C.c_uint8))
+    return r, hit, amb
+
+
 def ranges_fixed_step(occ, res, angles, max_range, delta, x, y, psi):
     occ, angles = _u8(occ), _f32(angles)
     x, y, psi = map(_f32, (x, y, psi))

@@ -433,6 +433,39 @@ void fno_ranges(const uint8_t* occ, int H, int W, float res, int B, const float*
     }
 }
 
+/* A robot with several range sensors ("S defines sensor placement and range-sensing parameters";
+ * PAPER.md:125 "using the sensor placement in the robot specification").  Sensor k has its own
+ * placement (s_x, s_y, s_psi) in the body frame, beam table (B_k angles) and maximum range; the observation row of
+ * an env is the concatenation of the sensors' ranges in sensor order (B = sum of B_k).  Every beam is the plain
+ * definition of O4 from its own sensor's origin.
+ */
+void fno_ranges_multi(const uint8_t* occ, int H, int W, float res, int K, const int32_t* Bk /*[K]*/,
+                      const float* angles /*[sum Bk]*/, const float* max_range /*[K]*/, const float* sensors /*[K][3]*/,
+                      int n, const float* x, const float* y, const float* psi, double eps,
+                      float* ranges /*[n][B]*/, int32_t* hit /*[n][B] or NULL*/, uint8_t* amb /*[n][B] or NULL*/) {
+    const double rho = (double)res;
+    size_t B = 0;
+    for (int k = 0; k < K; ++k) B += (size_t)Bk[k];
+    for (int e = 0; e < n; ++e) {
+        const double c = cos((double)psi[e]), s = sin((double)psi[e]);
+        size_t off = 0;
+        for (int k = 0; k < K; ++k) {
+            const double s0 = (double)sensors[3 * k], s1 = (double)sensors[3 * k + 1], s2 = (double)sensors[3 * k + 2];
+            const double rmax = (double)max_range[k], T = rmax / rho;
+            const double ox = ((double)x[e] + c * s0 - s * s1) / rho;      /* sensor origin in the map frame, in cells */
+            const double oy = ((double)y[e] + s * s0 + c * s1) / rho;
+            for (int b = 0; b < Bk[k]; ++b) {
+                const size_t i = (size_t)e * B + off + (size_t)b;
+                const double phi = (double)psi[e] + s2 + (double)angles[off + (size_t)b];
+                int32_t h;
+                ray_one(occ, H, W, rho, ox, oy, phi, T, rmax, eps, &ranges[i], &h, amb ? &amb[i] : NULL, NULL);
+                if (hit) hit[i] = h;
+            }
+            off += (size_t)Bk[k];
+        }
+    }
+}
+
 /* The paper's own definition: fixed-step samples along each beam, first sample at t = 0
  * (reading G5), step `delta` metres; the range is the distance of the first sample that falls in an
  * occupied (or outside-map) cell; no such sample below r_max => r_max.  Cross-check only.

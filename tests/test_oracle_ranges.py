@@ -200,3 +200,40 @@ def test_sensor_offset(oracle_lib):
     y2 = np.float32(y + 0.1 * np.sin(np.float64(psi)))
     r2, h2, _ = oracle_lib.ranges(wl.occ, RHO, ang, 1.0, [x2], [y2], [np.float32(psi + np.float32(0.5))])
     assert np.allclose(r1, r2, atol=1e-5)
+
+
+def test_several_sensors(oracle_lib):
+    # a robot with several range sensors, each with its own placement, beam
+    # table and maximum range; the observation is the sensors' ranges one after the other.  Pins: (1) every sensor's
+    # block equals a single-sensor robot with that sensor (the single-sensor function is pinned above: analytic
+    # walls, slab formula, brute force); (2) a sensor with an offset is a moved, yawed robot (hand-computed pose);
+    # (3) a wall straight ahead: front sensor at +0.2 m and rear-facing sensor at -0.2 m see analytic distances.
+    wl = W.tiny_workload(size=32, seed=9)
+    rng = np.random.default_rng(3)
+    n = 40
+    x = (0.3 + rng.random(n)).astype(np.float32); y = (0.3 + rng.random(n)).astype(np.float32)
+    psi = (rng.random(n) * 6.28 - 3.14).astype(np.float32)
+    sensors = [(_angles(16), 1.0, (0.1, 0.0, 0.5)), (_angles(7), 0.6, (-0.05, 0.08, -2.0)), (_angles(24), 1.4, (0.0, 0.0, 0.0))]
+    r, h, a = oracle_lib.ranges_multi(wl.occ, RHO, sensors, x, y, psi)
+    assert r.shape == (n, 47)
+    off = 0
+    for ang, rmax, plc in sensors:
+        r1, h1, a1 = oracle_lib.ranges(wl.occ, RHO, ang, rmax, x, y, psi, sensor=list(plc))
+        assert np.array_equal(r[:, off:off + len(ang)], r1) and np.array_equal(h[:, off:off + len(ang)], h1)
+        assert np.array_equal(a[:, off:off + len(ang)], a1)
+        assert r1.max() <= rmax + 1e-6
+        off += len(ang)
+    # (2) moved robot, for the second sensor
+    ang, rmax, (sx, sy, sp) = sensors[1]
+    c, s = np.cos(psi.astype(np.float64)), np.sin(psi.astype(np.float64))
+    x2 = (x + c * sx - s * sy).astype(np.float32); y2 = (y + s * sx + c * sy).astype(np.float32)
+    r2, _, a2 = oracle_lib.ranges(wl.occ, RHO, ang, rmax, x2, y2, (psi + np.float32(sp)).astype(np.float32))
+    ok = (a[:, 16:23] == 0) & (a2 == 0)
+    assert ok.mean() > 0.9 and np.allclose(r[:, 16:23][ok], r2[ok], atol=2e-5)
+    # (3) analytic: empty 64 x 64 map with a wall at column 40 (x = 2.0 m) and its border at column 0
+    occ = np.zeros((64, 64), np.uint8); occ[:, 40] = 1; occ[:, 0] = 1; occ[0, :] = 1; occ[-1, :] = 1
+    front = (np.zeros(1, np.float32), 3.0, (0.2, 0.0, 0.0))
+    rear = (np.zeros(1, np.float32), 3.0, (-0.2, 0.0, np.pi))
+    rr, hh, _ = oracle_lib.ranges_multi(occ, RHO, [front, rear], np.float32([1.0]), np.float32([1.625]), np.float32([0.0]))
+    assert abs(rr[0, 0] - (2.0 - 1.2)) < 1e-6 and abs(rr[0, 1] - (0.8 - 0.05)) < 1e-6
+    assert hh[0, 0] == 32 * 64 + 40 and hh[0, 1] == 32 * 64 + 0

@@ -72,6 +72,15 @@ int fn_robot_create_union(const float* footprint_xy_host, const int32_t* comp_si
                           const float* vel_limits_host, fn_robot** out);
 /* sensor placement S in the body frame; default (0, 0, 0). */
 int fn_robot_set_sensor(fn_robot* robot, float sx_m, float sy_m, float spsi_rad);
+/* A further range sensor (PAPER.md:65 "S defines sensor placement and range-sensing parameters"; :125): its own beam
+ * table beam_angles_host [B] (rad, sensor frame), maximum range and placement (s_x, s_y, s_psi) in the body frame.
+ * The observation row of an env becomes the concatenation of the sensors' ranges in the order they were added
+ * (row length = sum of the beam counts: every [N][B] buffer of this header is sized with that sum); hit cells and
+ * ring rows follow.  At most 4 sensors; call before fn_sim_create.  Each sensor is cast by its own beam launch
+ * (fn_step / fn_reset then use the unfused launch sequences); clearance features and the fixed-step comparison
+ * query are single-sensor (FN_ERR_UNSUPPORTED otherwise).  Errors: FN_ERR_INVALID_ARG, FN_ERR_UNSUPPORTED, FN_ERR_OOM. */
+int fn_robot_add_sensor(fn_robot* robot, const float* beam_angles_host, int B, float max_range_m,
+                        float s_x, float s_y, float s_psi);
 /* acceleration limits of U: acc_host [3] = maximum |dv_x/dt|, |dv_y/dt|, |dw/dt| (> 0; +inf = none,
  * the default).  The clipped command is limited to the previous applied velocity (state planes 3..5)
  * +- a_max dt before the motion update.  Takes effect for sims created afterwards AND existing ones. */

@@ -16,7 +16,7 @@ COUNTER_NAMES = ("rays_cast", "map_words_loaded", "envs_reset", "reset_failures"
                  "env_steps", "oob_window_loads", "reserved1")
 
 EXPORTED_SYMBOLS = (
-    "fn_map_create", "fn_map_set_regions", "fn_map_destroy", "fn_robot_create", "fn_robot_create_union", "fn_robot_set_sensor", "fn_robot_set_acc_limits",
+    "fn_map_create", "fn_map_set_regions", "fn_map_destroy", "fn_robot_create", "fn_robot_create_union", "fn_robot_set_sensor", "fn_robot_add_sensor", "fn_robot_set_acc_limits",
     "fn_robot_destroy", "fn_task_default", "fn_sim_create", "fn_sim_destroy", "fn_sim_set_stream", "fn_step", "fn_reset",
     "fn_sim_bind_aux", "fn_sim_bind_features", "fn_ring_attach", "fn_ring_sample", "fn_ranges_fixed_step", "fn_eval_begin", "fn_eval_result", "fn_eval_end", "fn_observe_all", "fn_get_counters", "fn_sim_count_words",
     "fn_sim_episode_state", "fn_sim_beam_config", "fn_sim_set_fused_reset", "fn_sim_set_split_step", "fn_sim_set_coarse", "fn_sim_profile", "fn_sim_profile_read", "fn_step_host", "fn_step_host_begin", "fn_step_host_end", "fn_measure_peak", "fn_last_error", "fn_version")
@@ -53,6 +53,7 @@ def load_library():
         "fn_robot_create": [vp, i32, vp, i32, f32, i32, vp, C.POINTER(vp)],
         "fn_robot_create_union": [vp, vp, i32, vp, i32, f32, i32, vp, C.POINTER(vp)],
         "fn_robot_set_sensor": [vp, f32, f32, f32],
+        "fn_robot_add_sensor": [vp, vp, i32, f32, f32, f32, f32],
         "fn_robot_set_acc_limits": [vp, vp],
         "fn_robot_destroy": [vp],
         "fn_sim_create": [vp, vp, i32, C.POINTER(_Task), vp, C.POINTER(vp)],
@@ -177,6 +178,13 @@ class Robot:
 
     def set_sensor(self, sx, sy, spsi):
         _check(load_library().fn_robot_set_sensor(self._h, C.c_float(sx), C.c_float(sy), C.c_float(spsi)), "fn_robot_set_sensor")
+
+    def add_sensor(self, beam_angles, max_range, sx, sy, spsi):
+        """A further range sensor: own beam table, range and placement; rows grow by its beam count."""
+        ang = np.ascontiguousarray(beam_angles, np.float32).reshape(-1)
+        _check(load_library().fn_robot_add_sensor(self._h, _np_ptr(ang), int(ang.shape[0]), C.c_float(max_range), C.c_float(sx),
+                                                  C.c_float(sy), C.c_float(spsi)), "fn_robot_add_sensor")
+        self.B += int(ang.shape[0])
 
     def set_acc_limits(self, acc):
         a = np.ascontiguousarray(acc, np.float32).reshape(3)

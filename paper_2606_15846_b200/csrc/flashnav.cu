@@ -49,8 +49,14 @@ struct fn_map {
     int4* d_regions;
 };
 
+constexpr int kMaxSensors = 4;
+struct fn_sensor {               // one range sensor: its block of the observation row, table and placement
+    int off, B;
+    float rmax, sx, sy, spsi;
+};
 struct fn_robot {
-    int V, B, drive;
+    std::vector<fn_sensor> sensors;  // [0] = the constructor's (beam table, max range) with fn_robot_set_sensor's placement
+    int V, B, drive;                 // B = beams of ALL sensors = length of an observation row
     float lim[6];
     float acc[3];
     float rmax;
@@ -72,6 +78,7 @@ struct fn_sim {
     fn_task task;
     cudaStream_t stream;
     int num_sms;
+    int n_sensors;                   // range sensors of the robot at fn_sim_create (one beam launch and pose set each)
     // device state owned by the sim
     BeamPose* d_poses;
     int* d_list;
@@ -275,10 +282,11 @@ static std::vector<double2> interior_samples(const std::vector<float>& v, const 
 
 static int robot_upload(fn_robot* r) {
     std::vector<double2> cs(r->B), vs(r->V);
-    for (int j = 0; j < r->B; ++j) {
-        const double a = (double)r->angles[j] + (double)r->sensor[2];
-        cs[j] = make_double2(std::cos(a), std::sin(a));
-    }
+    for (const fn_sensor& sn : r->sensors)
+        for (int j = 0; j < sn.B; ++j) {
+            const double a = (double)r->angles[sn.off + j] + (double)sn.spsi;
+            cs[sn.off + j] = make_double2(std::cos(a), std::sin(a));
+        }
     for (int k = 0; k < r->V; ++k) vs[k] = make_double2((double)r->verts[2 * k], (double)r->verts[2 * k + 1]);
     FN_CUDA(cudaMemcpy(r->d_beam_cs, cs.data(), cs.size() * sizeof(double2), cudaMemcpyHostToDevice));
     FN_CUDA(cudaMemcpy(r->d_verts, vs.data(), vs.size() * sizeof(double2), cudaMemcpyHostToDevice));
@@ -314,6 +322,7 @@ extern "C" int fn_robot_create_union(const float* fp, const int32_t* comp_sizes,
     r->sensor[0] = r->sensor[1] = r->sensor[2] = 0.0f;
     r->acc[0] = r->acc[1] = r->acc[2] = INFINITY;
     r->angles.assign(angles, angles + B);
+    r->sensors.assign(1, fn_sensor{0, B, rmax, 0.0f, 0.0f, 0.0f});
     r->verts.assign(fp, fp + 2 * V);
     r->nxt.resize(V);
     for (int c = 0, off = 0; c < C; off += comp_sizes[c], ++c)
@@ -345,6 +354,26 @@ extern "C" int fn_robot_create(const float* fp, int V, const float* angles, int 
 extern "C" int fn_robot_set_sensor(fn_robot* r, float sx, float sy, float spsi) {
     if (!r || !std::isfinite(sx) || !std::isfinite(sy) || !std::isfinite(spsi)) return fail(FN_ERR_INVALID_ARG, "fn_robot_set_sensor: bad argument");
     r->sensor[0] = sx; r->sensor[1] = sy; r->sensor[2] = spsi;
+    r->sensors[0].sx = sx; r->sensors[0].sy = sy; r->sensors[0].spsi = spsi;
+    return robot_upload(r);
+}
+
+extern "C" int fn_robot_add_sensor(fn_robot* r, const float* angles, int B, float rmax, float sx, float sy, float spsi) {
+    if (!r || !angles) return fail(FN_ERR_INVALID_ARG, "fn_robot_add_sensor: NULL argument");
+    if (B < 1) return fail(FN_ERR_INVALID_ARG, "fn_robot_add_sensor: B must be >= 1");
+    if (!std::isfinite(rmax) || rmax <= 0.0f) return fail(FN_ERR_INVALID_ARG, "fn_robot_add_sensor: max range must be finite and > 0");
+    if (!std::isfinite(sx) || !std::isfinite(sy) || !std::isfinite(spsi)) return fail(FN_ERR_INVALID_ARG, "fn_robot_add_sensor: non-finite placement");
+    for (int j = 0; j < B; ++j) if (!std::isfinite(angles[j])) return fail(FN_ERR_INVALID_ARG, "fn_robot_add_sensor: non-finite beam angle");
+    if ((int)r->sensors.size() >= kMaxSensors) return fail(FN_ERR_UNSUPPORTED, "fn_robot_add_sensor: at most %d sensors", kMaxSensors);
+    double2* cs = nullptr;
+    cudaError_t e = cudaMalloc(&cs, (size_t)(r->B + B) * sizeof(double2));
+    if (e != cudaSuccess) return fail(e == cudaErrorMemoryAllocation ? FN_ERR_OOM : FN_ERR_CUDA, "fn_robot_add_sensor: %s", cudaGetErrorString(e));
+    cudaFree(r->d_beam_cs);
+    r->d_beam_cs = cs;
+    r->sensors.push_back(fn_sensor{r->B, B, rmax, sx, sy, spsi});
+    r->angles.insert(r->angles.end(), angles, angles + B);
+    r->B += B;
+    if (rmax > r->rmax) r->rmax = rmax;                            // the robot's largest range (clearance cap, limits)
     return robot_upload(r);
 }
 
@@ -375,6 +404,9 @@ static RobotDev robot_dev(const fn_robot* r, const fn_map* m) {
     d.rmax = r->rmax;
     d.T = (double)r->rmax / (double)m->res;
     d.sx = r->sensor[0]; d.sy = r->sensor[1];
+    d.n_sensors = (int)r->sensors.size();
+    for (int k = 0; k < 4; ++k) { d.sxs[k] = d.sys[k] = 0.0; }
+    for (int k = 0; k < d.n_sensors; ++k) { d.sxs[k] = r->sensors[k].sx; d.sys[k] = r->sensors[k].sy; }
     return d;
 }
 static TaskDev task_dev(const fn_task& t) {
@@ -422,7 +454,8 @@ extern "C" int fn_sim_create(const fn_map* map, const fn_robot* robot, int n, co
     cudaError_t e = cudaGetDevice(&dev);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&s->num_sms, cudaDevAttrMultiProcessorCount, dev);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
-    if (e == cudaSuccess) e = cudaMalloc(&s->d_poses, (size_t)n * sizeof(BeamPose));
+    s->n_sensors = (int)robot->sensors.size();
+    if (e == cudaSuccess) e = cudaMalloc(&s->d_poses, (size_t)n * s->n_sensors * sizeof(BeamPose));
     if (e == cudaSuccess) e = cudaMalloc(&s->d_ring_head, 2 * sizeof(unsigned long long));
     if (e == cudaSuccess) e = cudaMemsetAsync(s->d_ring_head, 0, 2 * sizeof(unsigned long long), s->stream);
     if (e == cudaSuccess) e = cudaMalloc(&s->d_list, (size_t)n * sizeof(int));
@@ -443,7 +476,7 @@ extern "C" int fn_sim_create(const fn_map* map, const fn_robot* robot, int n, co
     if (e == cudaSuccess) e = cudaMemsetAsync(s->d_dprev, 0, (size_t)n * sizeof(float), s->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(s->d_epstep, 0, (size_t)n * sizeof(int), s->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(s->d_counters, 0, kNCounters * sizeof(unsigned long long), s->stream);
-    if (e == cudaSuccess) e = cudaMemsetAsync(s->d_poses, 0xff, (size_t)n * sizeof(BeamPose), s->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(s->d_poses, 0xff, (size_t)n * s->n_sensors * sizeof(BeamPose), s->stream);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(env_step_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                                    (int)col_scratch_bytes(FN_MAX_VERTS));
     if (e == cudaSuccess) e = cudaFuncSetAttribute(reset_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -480,7 +513,8 @@ extern "C" int fn_sim_create(const fn_map* map, const fn_robot* robot, int n, co
             e = kernel_config(reset_beam_kernel<false>, kFusedThreads, s->fused_smem, max_optin, &f0);
             if (e == cudaSuccess) e = kernel_config(reset_beam_kernel<true>, kFusedThreads, s->fused_smem, max_optin, &f1);
             if (f1 < f0) f0 = f1;
-            if (e == cudaSuccess && f0 >= 1) { s->fused_ok = s->fused_on = true; s->fused_grid = s->num_sms * f0; }
+            // (several sensors: one beam launch per sensor, so the reset and the step keep their own kernels)
+            if (e == cudaSuccess && f0 >= 1 && s->n_sensors == 1) { s->fused_ok = s->fused_on = true; s->fused_grid = s->num_sms * f0; }
         }
         // the split step: the beam kernel plus one collision scratch; used when it keeps the beam kernel's occupancy
         s->split_ok = s->split_on = false;
@@ -496,7 +530,7 @@ extern "C" int fn_sim_create(const fn_map* map, const fn_robot* robot, int n, co
                 if (e == cudaSuccess) e = kernel_config(step_beam_kernel<false, true>, 512, s->split_smem, max_optin, &f[1]);
             }
             const int fm = f[0] < f[1] ? f[0] : f[1];
-            if (e == cudaSuccess && fm >= 1 && s->num_sms * fm >= s->beam_grid) {
+            if (e == cudaSuccess && fm >= 1 && s->num_sms * fm >= s->beam_grid && s->n_sensors == 1) {
                 s->split_ok = true; s->split_grid = s->num_sms * fm;
                 // one warp per CTA computes the outcomes of the envs its CTA owns, 32 at a time: worth it up to
                 // two such batches (measured: C1-C4 3-8 % faster per step, C5 with 222 envs per CTA 4 % slower)
@@ -571,23 +605,28 @@ extern "C" int fn_sim_set_stream(fn_sim* s, void* stream) {
 
 static int ring_row_floats(const fn_sim* s) { return s->robot->B + 5 + (s->robot->drive == FN_DRIVE_DIFF ? 2 : 3) + 2; }
 
-static BeamArgs beam_args(fn_sim* s, const int* list, const int* count_dev, float* out_ranges, bool step_launch, bool done_list) {
+// the launch for one sensor of the robot: its table, beam count, range, poses and block of the observation row
+static BeamArgs beam_args(fn_sim* s, const int* list, const int* count_dev, float* out_ranges, bool step_launch, bool done_list,
+                          int sensor = 0) {
     BeamArgs b;
-    b.map = s->map->dev; b.robot = robot_dev(s->robot, s->map); b.poses = s->d_poses; b.count_words = s->count_words;
+    const fn_sensor& sn = s->robot->sensors[sensor];
+    b.map = s->map->dev; b.robot = robot_dev(s->robot, s->map); b.poses = s->d_poses + (size_t)sensor * s->n; b.count_words = s->count_words;
+    b.out_stride = (unsigned)s->robot->B; b.out_off = (unsigned)sn.off;
+    b.robot.beam_cs += sn.off; b.robot.B = sn.B; b.robot.rmax = sn.rmax; b.robot.T = (double)sn.rmax / (double)s->map->res;
     b.list = list; b.count_dev = count_dev; b.n_all = s->n; b.out_ranges = out_ranges; b.out_hit = s->aux_hit;
     b.ring_obs = s->ring; b.ring_cap = s->ring_cap ? s->ring_cap : 1; b.ring_head = s->d_ring_head; b.ring_row = ring_row_floats(s);
     b.counters = s->d_counters; b.task_counter = s->d_task_counter;
     b.flip_par_dev = step_launch ? s->d_done_count + 2 : nullptr; b.done_count = s->d_done_count;
     b.list_par_dev = done_list ? s->d_done_count + 2 : nullptr;
     b.exp_off = kExpOff;
-    b.pair_lines = (double)s->robot->rmax / (double)s->map->res >= 110.0;     // beams of >~ 16 lines on average
+    b.pair_lines = b.robot.T >= 110.0;                             // beams of >~ 16 lines on average
     {   // ceil(2^32 / S) for S = bits per line (FastOrient::inv_magic)
         const unsigned long long SR = 32ull * (unsigned long long)s->map->dev.strideR, SC = 32ull * (unsigned long long)s->map->dev.strideC;
         b.inv_magicR = (unsigned)(((1ull << 32) + SR - 1) / SR); b.inv_magicC = (unsigned)(((1ull << 32) + SC - 1) / SC);
     }
-    fast_chunking(s->robot->B, &b.chunk_rounds, &b.nchunk);
+    fast_chunking(sn.B, &b.chunk_rounds, &b.nchunk);
     {
-        const unsigned long long rounds = ((unsigned long long)s->robot->B + 31) >> 5;
+        const unsigned long long rounds = ((unsigned long long)sn.B + 31) >> 5;
         b.inv_nchunk = fast_magic((unsigned long long)b.nchunk, (unsigned long long)s->n * b.nchunk);
         b.inv_rounds = fast_magic(rounds, (unsigned long long)s->n * rounds);
     }
@@ -596,17 +635,23 @@ static BeamArgs beam_args(fn_sim* s, const int* list, const int* count_dev, floa
 }
 
 static int launch_beams(fn_sim* s, const int* list, const int* count_dev, float* out_ranges, bool step_launch = false, bool done_list = false) {
-    const BeamArgs b = beam_args(s, list, count_dev, out_ranges, step_launch, done_list);
+    if ((int)s->robot->sensors.size() != s->n_sensors)
+        return fail(FN_ERR_INVALID_ARG, "the robot's sensors changed after fn_sim_create");
     const bool aux = s->count_words || s->aux_hit;
     const dim3 grid(s->beam_grid), block(512);
-    if (s->coarse_on && !aux) {
-        FN_CUDA(launch_pdl(beam_kernel<true, false, true>, dim3(s->beam_grid_c), dim3(1024), s->beam_smem_c, s->stream, b));
-    } else if (s->use_smem) {
-        if (aux) FN_CUDA(launch_pdl(beam_kernel<true, true>, grid, block, s->beam_smem, s->stream, b));
-        else FN_CUDA(launch_pdl(beam_kernel<true, false>, grid, block, s->beam_smem, s->stream, b));
-    } else {
-        if (aux) FN_CUDA(launch_pdl(beam_kernel<false, true>, grid, block, s->beam_smem, s->stream, b));
-        else FN_CUDA(launch_pdl(beam_kernel<false, false>, grid, block, s->beam_smem, s->stream, b));
+    for (int k = 0; k < s->n_sensors; ++k) {                      // one launch per sensor
+        // (the kernel before the first launch has zeroed the dynamic task counter; the done-list parity flips once)
+        if (k) FN_CUDA(cudaMemsetAsync(s->d_task_counter, 0, sizeof(unsigned), s->stream));
+        const BeamArgs b = beam_args(s, list, count_dev, out_ranges, step_launch && k == 0, done_list, k);
+        if (s->coarse_on && !aux) {
+            FN_CUDA(launch_pdl(beam_kernel<true, false, true>, dim3(s->beam_grid_c), dim3(1024), s->beam_smem_c, s->stream, b));
+        } else if (s->use_smem) {
+            if (aux) FN_CUDA(launch_pdl(beam_kernel<true, true>, grid, block, s->beam_smem, s->stream, b));
+            else FN_CUDA(launch_pdl(beam_kernel<true, false>, grid, block, s->beam_smem, s->stream, b));
+        } else {
+            if (aux) FN_CUDA(launch_pdl(beam_kernel<false, true>, grid, block, s->beam_smem, s->stream, b));
+            else FN_CUDA(launch_pdl(beam_kernel<false, false>, grid, block, s->beam_smem, s->stream, b));
+        }
     }
     return FN_OK;
 }
@@ -766,6 +811,7 @@ extern "C" int fn_observe_all(fn_sim* s, const float* states, float* out_ranges,
 extern "C" int fn_ranges_fixed_step(fn_sim* s, const float* states, float delta_m, int blockwise, float* out_ranges) {
     if (!s || !states || !out_ranges) return fail(FN_ERR_INVALID_ARG, "fn_ranges_fixed_step: NULL argument");
     if (!(delta_m > 0.0f) || !std::isfinite(delta_m)) return fail(FN_ERR_INVALID_ARG, "fn_ranges_fixed_step: delta must be > 0");
+    if (s->n_sensors != 1) return fail(FN_ERR_UNSUPPORTED, "fn_ranges_fixed_step: comparison query, single-sensor robots only");
     PoseArgs a;
     a.map = s->map->dev; a.robot = robot_dev(s->robot, s->map); a.n = s->n; a.states = states;
     a.out_goal_obs = nullptr; a.poses = s->d_poses; a.beam_task_counter = s->d_task_counter;
@@ -832,6 +878,7 @@ extern "C" int fn_sim_bind_aux(fn_sim* s, int32_t* hit, float* reward) {
 
 extern "C" int fn_sim_bind_features(fn_sim* s, int n_sectors, float* out_z) {
     if (!s) return fail(FN_ERR_INVALID_ARG, "fn_sim_bind_features: NULL sim");
+    if (out_z && s->n_sensors != 1) return fail(FN_ERR_UNSUPPORTED, "fn_sim_bind_features: single-sensor robots only");
     if (out_z && (n_sectors < 1 || n_sectors > s->robot->B))
         return fail(FN_ERR_INVALID_ARG, "fn_sim_bind_features: n_sectors must be in 1..B");
     if (out_z && feat_smem_bytes(s->robot->V, n_sectors, s->robot->B) > 48 * 1024)

@@ -515,8 +515,9 @@ struct BeamArgs {
     const int* list;             // compacted env indices or NULL (= all envs)
     const int* count_dev;        // number of listed envs (device) or NULL
     int n_all;                   // number of envs when list == NULL
-    float* out_ranges;           // [N][B]
-    int* out_hit;                // [N][B] or NULL            (kAux only)
+    float* out_ranges;           // [N][out_stride]: this launch writes columns out_off .. out_off + B - 1 of a row
+    int* out_hit;                // the same layout, or NULL  (kAux only)
+    unsigned out_stride, out_off;  // (a robot with several sensors: one launch per sensor, B = that sensor's beams)
     float* ring_obs;             // ring base or NULL: also write ranges into the env's pending ring row
     unsigned long long ring_cap;
     const unsigned long long* ring_head;      // device: pending row of env e = (*ring_head + e) % ring_cap
@@ -554,13 +555,13 @@ __device__ __forceinline__ void beam_element(const BeamArgs& a, const BeamMap<MS
         if (state == 1) hit = origin_line(bm, pose->o[0], true) * a.map.W + pose->o[0].cu0;
         ++words;
     }
-    const unsigned o = e * (unsigned)a.robot.B + j;                // n_envs * B < 2^31 (fn_sim_create)
+    const unsigned o = e * a.out_stride + a.out_off + j;           // n_envs * row length < 2^31 (fn_sim_create)
     a.out_ranges[o] = r;
     if (kAux && a.out_hit) a.out_hit[o] = hit;
     if (a.ring_obs) {
         unsigned long long slot = ring_head + (unsigned long long)e;   // both < ring_cap
         if (slot >= a.ring_cap) slot -= a.ring_cap;
-        a.ring_obs[slot * a.ring_row + j] = r;
+        a.ring_obs[slot * a.ring_row + a.out_off + j] = r;
     }
 }
 
@@ -642,9 +643,9 @@ __device__ __noinline__ void fast_drain(const BeamArgs& a, const uint32_t queue,
         int hit;
         uint32_t words = 0;
         const float r = cast_beam<SmemSpace, false>(bm, pose, lds_d2(tab + 16u * j), a.robot.T, a.map.rho, a.robot.rmax, &hit, words);
-        a.out_ranges[o] = r;
+        a.out_ranges[e * a.out_stride + a.out_off + j] = r;
         float* ring_row = ring_row_of(a, ring_head, e);
-        if (ring_row) ring_row[j] = r;
+        if (ring_row) ring_row[a.out_off + j] = r;
     }
     __syncwarp();
 }
@@ -666,10 +667,10 @@ __device__ __forceinline__ void fast_chunk(const BeamArgs& a, FastWarp& w, const
     __syncwarp();
     w.rays += jb1 - jb0;
     unsigned j = jb0 + lane;
-    const unsigned o0 = e * B;                                     // n_envs * B < 2^31 (fn_sim_create)
-    float* po = a.out_ranges + (o0 + j);
+    const unsigned o0 = e * B;                                     // index of the env's beam 0 (deferred beams: o0 + j)
+    float* po = a.out_ranges + (e * a.out_stride + a.out_off + j); // n_envs * row length < 2^31 (fn_sim_create)
     float* pr = nullptr;
-    if (a.ring_obs) pr = ring_row_of(a, ring_head, e) + j;
+    if (a.ring_obs) pr = ring_row_of(a, ring_head, e) + (a.out_off + j);
     uint32_t tj = w.tab + 16u * j;
 #pragma unroll 1
     for (unsigned jb = jb0; jb < jb1; jb += 32u, j += 32u, po += 32, tj += 512u) {

@@ -71,7 +71,9 @@ struct RobotDev {
     float acc[3];            // maximum accelerations a_x, a_y, a_w (+inf = none; reading G2)
     float rmax;              // metres
     double T;                // rmax / rho in cells
-    double sx, sy;           // sensor offset, metres
+    double sx, sy;           // sensor offset, metres (sensor 0)
+    int n_sensors;           // range sensors of the robot; poses of sensor k: poses[k * n_envs + e]
+    double sxs[4], sys[4];   // their offsets
 };
 
 struct TaskDev {

@@ -214,9 +214,9 @@ __device__ __forceinline__ bool resolve_collisions(const MapDev& m, const RobotD
 // origin's line.
 template <bool kS = false>
 __device__ __forceinline__ BeamPose make_pose(const MapDev& m, const RobotDev& rb,
-                                              float xf, float yf, float psif, double c, double s) {
-    const double ox = ((double)xf + c * rb.sx - s * rb.sy) * m.inv_rho;
-    const double oy = ((double)yf + s * rb.sx + c * rb.sy) * m.inv_rho;
+                                              float xf, float yf, float psif, double c, double s, const int sensor = 0) {
+    const double ox = ((double)xf + c * rb.sxs[sensor] - s * rb.sys[sensor]) * m.inv_rho;
+    const double oy = ((double)yf + s * rb.sxs[sensor] + c * rb.sys[sensor]) * m.inv_rho;
     BeamPose p;
     p.c = c; p.s = s;
     p.psi_bits = __float_as_int(psif);
@@ -234,10 +234,17 @@ __device__ __forceinline__ BeamPose make_pose(const MapDev& m, const RobotDev& r
     p.o[1].ouMS = p.o[1].ouM + (double)((p.o[1].line_off - rowBytes) << 3);
     return p;
 }
+// the poses of the other sensors of a robot with several (sensor 0's is stored by the caller): poses[k * n + e]
 template <bool kS = false>
-__device__ __forceinline__ void write_pose(const MapDev& m, const RobotDev& rb, BeamPose* out,
+__device__ __forceinline__ void write_more_poses(const MapDev& m, const RobotDev& rb, BeamPose* poses, const int n, const int e,
+                                                 float xf, float yf, float psif, double c, double s) {
+    for (int k = 1; k < rb.n_sensors; ++k) poses[(size_t)k * n + e] = make_pose<kS>(m, rb, xf, yf, psif, c, s, k);
+}
+template <bool kS = false>
+__device__ __forceinline__ void write_pose(const MapDev& m, const RobotDev& rb, BeamPose* poses, const int n, const int e,
                                            float xf, float yf, float psif, double c, double s) {
-    *out = make_pose<kS>(m, rb, xf, yf, psif, c, s);
+    poses[e] = make_pose<kS>(m, rb, xf, yf, psif, c, s);
+    write_more_poses<kS>(m, rb, poses, n, e, xf, yf, psif, c, s);
 }
 
 // ---------------------------------------------------------------- S1 + S3 + S4: the env step
@@ -359,6 +366,7 @@ __device__ __forceinline__ void env_motion_store(const EnvArgs& a, const MapDev&
     a.states[3 * n + e] = mo.avx; a.states[4 * n + e] = mo.avy; a.states[5 * n + e] = mo.aw;
     const BeamPose bp = make_pose<kS>(m, a.robot, mo.xf, mo.yf, mo.psif, mo.c1, mo.s1);
     a.poses[e] = bp;
+    write_more_poses<kS>(m, a.robot, a.poses, n, e, mo.xf, mo.yf, mo.psif, mo.c1, mo.s1);
     if (pose_copy) *pose_copy = bp;
     if (mo.bad) atomicAdd(&a.counters[kNonFinite], 1ull);
 }
@@ -669,6 +677,7 @@ __device__ __forceinline__ void reset_env(const ResetArgs& a, const MapDev& mp, 
         if (a.out_goal_obs) { a.out_goal_obs[e] = d; a.out_goal_obs[n + e] = alpha; }
         const BeamPose bp = make_pose<kS>(mp, a.robot, x, y, psi, cp, sp);
         a.poses[e] = bp;
+        write_more_poses<kS>(mp, a.robot, a.poses, n, e, x, y, psi, cp, sp);
         if (pose_copy) *pose_copy = bp;                            // (fused kernel: a copy in shared memory)
         if (a.ring) {
             const unsigned long long head = *a.ring_head_dev;
@@ -714,7 +723,7 @@ __global__ void __launch_bounds__(256) pose_from_state_kernel(PoseArgs a) {
     const float x = a.states[e], y = a.states[n + e], psi = a.states[2 * n + e];
     double s, c;
     sincos((double)psi, &s, &c);
-    write_pose(a.map, a.robot, &a.poses[e], x, y, psi, c, s);
+    write_pose(a.map, a.robot, a.poses, a.n, e, x, y, psi, c, s);
     if (a.out_goal_obs) {
         const double gdx = (double)a.states[6 * n + e] - (double)x, gdy = (double)a.states[7 * n + e] - (double)y;
         a.out_goal_obs[e] = (float)sqrt(gdx * gdx + gdy * gdy);
@@ -744,7 +753,7 @@ __global__ void __launch_bounds__(256) eval_begin_kernel(EvalBeginArgs a) {
     a.states[3 * n + e] = 0.f; a.states[4 * n + e] = 0.f; a.states[5 * n + e] = 0.f;
     double s, c;
     sincos((double)psi, &s, &c);
-    write_pose(a.pose.map, a.pose.robot, &a.pose.poses[e], x, y, psi, c, s);
+    write_pose(a.pose.map, a.pose.robot, a.pose.poses, a.pose.n, e, x, y, psi, c, s);
     const double gdx = (double)a.states[6 * n + e] - (double)x, gdy = (double)a.states[7 * n + e] - (double)y;
     const float d = (float)sqrt(gdx * gdx + gdy * gdy);
     if (a.pose.out_goal_obs) {

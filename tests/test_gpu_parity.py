@@ -235,6 +235,92 @@ def test_ring_at_full_scale_c5(pu):
     torch.cuda.empty_cache()
 
 
+def test_several_sensors_against_the_oracle(pu):
+    # SURVEY 8(f) NEXT-3 (PAPER.md:65 "S defines sensor placement and range-sensing parameters", :125): a robot with
+    # three range sensors (different beam tables, ranges and placements).  Rows = the sensors' ranges one after the
+    # other; ranges and hit cells against oracle.ranges_multi (tolerances of run_parity) through steps, resets of the
+    # done list and of a mask, fn_observe_all; production kernel == instrumented kernel; ring rows carry the full row.
+    import torch
+    import oracle
+    import paper_2606_15846_b200 as fn
+    from harness import workloads as W
+    for cfg in (2, 4):                                            # map in shared memory / read through L2
+        wl = W.make_workload(cfg, n_envs=400)
+        n, A = wl.n_envs, wl.action_dim
+        sensors = [(wl.beam_angles, float(wl.max_range), (0.1, -0.05, 0.2)),
+                   (W.beam_table(90, 120.0), 4.0, (-0.2, 0.1, 3.0)),
+                   (W.beam_table(33, 360.0), 2.5, (0.0, 0.15, -1.0))]
+        m = fn.Map(wl.occ, float(wl.resolution))
+        r = fn.Robot(wl.footprint, wl.beam_angles, float(wl.max_range), wl.drive, wl.vel_limits)
+        r.set_sensor(*sensors[0][2])
+        for ang, rmax, plc in sensors[1:]:
+            r.add_sensor(ang, rmax, *plc)
+        B = r.B
+        assert B == wl.n_beams + 90 + 33
+        s = fn.Sim(m, r, n, goal_tol=float(wl.goal_tol), goal_dist_min=float(wl.goal_dist_min), goal_dist_max=float(wl.goal_dist_max))
+        assert not s.beam_config()["split_step"] and not s.beam_config()["fused_reset"]
+        buf = pu.Buffers(n, B, A)
+        s.bind_aux(buf.hit, buf.reward)
+        cap = 4 * n + 5
+        row = B + 5 + A + 2
+        ring = torch.zeros(cap * row, device="cuda")
+        s.ring_attach(ring, cap)
+        steps = 6
+        actions = torch.from_numpy(W.action_tape(wl, steps, 8)).cuda()
+        seeds = torch.from_numpy(W.seed_tape(wl, steps + 1, 8).view(np.int64)).cuda()
+
+        def check(tag, idx=None):
+            torch.cuda.synchronize()
+            st = buf.states.cpu().numpy()
+            idx = np.arange(n) if idx is None else idx
+            ro, ho, ao = oracle.ranges_multi(wl.occ, wl.resolution, sensors, st[0, idx], st[1, idx], st[2, idx])
+            g, gh = buf.ranges.cpu().numpy()[idx], buf.hit.cpu().numpy()[idx]
+            ok = ao == 0
+            assert (~ok).sum() <= max(2, 1e-3 * ok.size)
+            assert np.array_equal(gh[ok], ho[ok]), f"{tag}: hit cells"
+            assert np.all(np.abs(g.astype(np.float64) - ro)[ok] <= pu.TOL_RANGE), f"{tag}: ranges"
+            off = 0
+            for ang, rmax, _ in sensors:                          # every block is capped at its own sensor's range
+                assert g[:, off:off + len(ang)].max() <= rmax + 1e-6
+                off += len(ang)
+
+        buf.mask.fill_(1)
+        s.reset(buf.states, buf.mask, seeds[0], buf.ranges, buf.gobs)
+        check("initial reset")
+        head = 0
+        for t in range(steps):
+            obs = buf.ranges.clone()
+            buf.mask.zero_()
+            s.step(buf.states, actions[t], float(wl.dt), buf.mask, buf.ranges, buf.col, buf.gobs)
+            check(f"step {t}")
+            torch.cuda.synchronize()
+            slots = (head + torch.arange(n, device="cuda")) % cap
+            assert torch.equal(ring.view(cap, row)[slots][:, :B], obs), "ring rows carry the observation of all sensors"
+            head = (head + n) % cap
+            done = np.nonzero(buf.mask.cpu().numpy())[0]
+            keep = buf.ranges.clone()
+            if t % 2 == 0:
+                s.reset(buf.states, None, seeds[t + 1], buf.ranges, buf.gobs)
+            else:
+                s.reset(buf.states, buf.mask, seeds[t + 1], buf.ranges, buf.gobs)
+            if done.size:
+                check(f"reset {t}", done)
+            other = np.setdiff1d(np.arange(n), done)
+            assert torch.equal(buf.ranges[other], keep[other]), "recompute touched other rows"
+        # instrumented and production kernels, all envs
+        inst = torch.empty_like(buf.ranges)
+        s.observe_all(buf.states, inst)
+        s.bind_aux(None, buf.reward)
+        fast = torch.empty_like(buf.ranges)
+        s.observe_all(buf.states, fast)
+        torch.cuda.synchronize()
+        assert torch.equal(inst, fast)
+        z = torch.zeros(n, 8, device="cuda")
+        with pytest.raises(fn.FlashNavError):
+            s.bind_features(8, z)                                 # clearance features: single-sensor robots only
+        s.close(); r.close(); m.close()
+
+
 def test_sensor_offset_in_the_beam_kernel(pu):
     # Sensor placement S (PAPER.md:65 "S defines sensor placement", :125; reading G8): beams start at the sensor, not
     # at the body origin.  The oracle casts from the offset pose (pinned by "sensor offset == moved robot",

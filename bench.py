@@ -565,7 +565,7 @@ def run_ours(args):
     hc = torch.empty(n, dtype=torch.uint8).pin_memory()
     hg = torch.empty(2, n, dtype=torch.float32).pin_memory()
     hs.copy_(states)
-    Ke = max(3, min(K, args.e2e_steps))
+    Ke = max(3, min(K, args.e2e_steps)) if args.e2e_steps > 0 else 3
     for k in range(3):
         hm.zero_()
         sim.step_host(hs, ha_p[k % 8], float(wl.dt), hm, hseed[k % 8], hr, hc, hg)

@@ -433,7 +433,7 @@ static cudaError_t kernel_config(K kernel, int threads, size_t smem, int max_opt
 }
 template <bool S, bool C>
 static cudaError_t beam_config(size_t smem, int max_optin, int* blocks_per_sm) {
-    return kernel_config(beam_kernel<S, C>, 512, smem, max_optin, blocks_per_sm);
+    return kernel_config(beam_kernel<S, C>, kBeamThreads, smem, max_optin, blocks_per_sm);
 }
 
 extern "C" int fn_sim_create(const fn_map* map, const fn_robot* robot, int n, const fn_task* task,
@@ -523,11 +523,11 @@ extern "C" int fn_sim_create(const fn_map* map, const fn_robot* robot, int n, co
         if (e == cudaSuccess && s->split_smem <= (size_t)max_optin) {
             int f[2] = {0, 0};
             if (s->use_smem) {
-                e = kernel_config(step_beam_kernel<true, false>, 512, s->split_smem, max_optin, &f[0]);
-                if (e == cudaSuccess) e = kernel_config(step_beam_kernel<true, true>, 512, s->split_smem, max_optin, &f[1]);
+                e = kernel_config(step_beam_kernel<true, false>, kBeamThreads, s->split_smem, max_optin, &f[0]);
+                if (e == cudaSuccess) e = kernel_config(step_beam_kernel<true, true>, kBeamThreads, s->split_smem, max_optin, &f[1]);
             } else {
-                e = kernel_config(step_beam_kernel<false, false>, 512, s->split_smem, max_optin, &f[0]);
-                if (e == cudaSuccess) e = kernel_config(step_beam_kernel<false, true>, 512, s->split_smem, max_optin, &f[1]);
+                e = kernel_config(step_beam_kernel<false, false>, kBeamThreads, s->split_smem, max_optin, &f[0]);
+                if (e == cudaSuccess) e = kernel_config(step_beam_kernel<false, true>, kBeamThreads, s->split_smem, max_optin, &f[1]);
             }
             const int fm = f[0] < f[1] ? f[0] : f[1];
             if (e == cudaSuccess && fm >= 1 && s->num_sms * fm >= s->beam_grid && s->n_sensors == 1) {
@@ -638,7 +638,7 @@ static int launch_beams(fn_sim* s, const int* list, const int* count_dev, float*
     if ((int)s->robot->sensors.size() != s->n_sensors)
         return fail(FN_ERR_INVALID_ARG, "the robot's sensors changed after fn_sim_create");
     const bool aux = s->count_words || s->aux_hit;
-    const dim3 grid(s->beam_grid), block(512);
+    const dim3 grid(s->beam_grid), block(kBeamThreads);
     for (int k = 0; k < s->n_sensors; ++k) {                      // one launch per sensor
         // (the kernel before the first launch has zeroed the dynamic task counter; the done-list parity flips once)
         if (k) FN_CUDA(cudaMemsetAsync(s->d_task_counter, 0, sizeof(unsigned), s->stream));
@@ -713,7 +713,7 @@ extern "C" int fn_step(fn_sim* s, float* states, const float* actions, float dt,
         const BeamArgs b = beam_args(s, nullptr, nullptr, out_ranges, false, false);
         const int epc = (s->n + s->split_grid - 1) / s->split_grid;
         const bool aux = s->count_words || s->aux_hit;
-        const dim3 grid(s->split_grid), block(512);
+        const dim3 grid(s->split_grid), block(kBeamThreads);
         const unsigned bs = (unsigned)s->beam_smem;
         if (s->coarse_on && s->split_ok_c && !aux) {
             const int epc_c = (s->n + s->split_grid_c - 1) / s->split_grid_c;
@@ -953,7 +953,7 @@ extern "C" int fn_sim_profile_read(fn_sim* s, double* ms_out, uint64_t* launches
 
 extern "C" int fn_sim_beam_config(const fn_sim* s, int* cfg) {
     if (!s || !cfg) return fail(FN_ERR_INVALID_ARG, "fn_sim_beam_config: NULL argument");
-    cfg[0] = s->use_smem ? 1 : 0; cfg[1] = s->beam_grid; cfg[2] = 512; cfg[3] = (int)s->beam_smem;
+    cfg[0] = s->use_smem ? 1 : 0; cfg[1] = s->beam_grid; cfg[2] = kBeamThreads; cfg[3] = (int)s->beam_smem;
     cfg[4] = s->split_on ? 1 : 0; cfg[5] = s->fused_on ? 1 : 0;
     cfg[6] = s->coarse_on ? 1 : 0; cfg[7] = s->coarse_ok ? 1 : 0;
     if (s->coarse_on) { cfg[1] = s->beam_grid_c; cfg[2] = 1024; cfg[3] = (int)s->beam_smem_c; }

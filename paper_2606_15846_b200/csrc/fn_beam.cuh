@@ -575,7 +575,11 @@ struct FastShared {
 };
 // launch shape of the production kernels: two CTAs of 512 threads per SM, or -- with the coarse copies, which
 // double the staged image -- one CTA of 1024
-template <bool kCoarse> struct FastShape { static constexpr int kThreads = kCoarse ? 1024 : 512, kCtas = kCoarse ? 1 : 2; };
+#ifndef FN_BEAM_THREADS
+#define FN_BEAM_THREADS 512
+#endif
+constexpr int kBeamThreads = FN_BEAM_THREADS;                     // threads per CTA of the beam kernels (two CTAs per SM)
+template <bool kCoarse> struct FastShape { static constexpr int kThreads = kCoarse ? 1024 : kBeamThreads, kCtas = kCoarse ? 1 : 2; };
 struct FastWarp {
     uint32_t slot;               // shared address of the warp's FastSlot
     uint32_t tab;                // shared address of the beam table

@@ -89,17 +89,18 @@ def reward_done(d_new, collision, forced, d_prev, ep_step, goal_tol=0.3, max_epi
     return reward, done
 
 
-def collision(occ, res, footprint, x, y, psi, eps=EPS_CELL):
+def collision(occ, res, footprint, x, y, psi, eps=EPS_CELL, components=None):
     occ, fp = _u8(occ), _f32(footprint)
     x, y, psi = map(_f32, (x, y, psi))
     H, W = occ.shape
     n = x.shape[0]
     flag = np.empty(n, np.uint8)
     amb = np.empty(n, np.uint8)
-    lib().fno_collision(_p(occ, C.c_uint8), C.c_int(H), C.c_int(W), C.c_float(res),
-                        C.c_int(fp.shape[0]), _p(fp, C.c_float), C.c_int(n), _p(x, C.c_float),
-                        _p(y, C.c_float), _p(psi, C.c_float), C.c_double(eps),
-                        _p(flag, C.c_uint8), _p(amb, C.c_uint8))
+    with _components(components):
+        lib().fno_collision(_p(occ, C.c_uint8), C.c_int(H), C.c_int(W), C.c_float(res),
+                            C.c_int(fp.shape[0]), _p(fp, C.c_float), C.c_int(n), _p(x, C.c_float),
+                            _p(y, C.c_float), _p(psi, C.c_float), C.c_double(eps),
+                            _p(flag, C.c_uint8), _p(amb, C.c_uint8))
     return flag, amb
 
 
@@ -170,7 +171,7 @@ def ranges_fixed_step(occ, res, angles, max_range, delta, x, y, psi):
 
 
 def reset(occ, res, footprint, regions, goal_dist_min, goal_dist_max, mask, seeds, states, d_prev,
-          ep_step, eps=EPS_CELL):
+          ep_step, eps=EPS_CELL, components=None):
     """In place on states [8,n] f32, d_prev f32, ep_step i32 for masked envs. Returns amb, failed."""
     occ, fp, mask = _u8(occ), _f32(footprint), _u8(mask)
     seeds = np.ascontiguousarray(seeds, np.uint64)
@@ -182,11 +183,12 @@ def reset(occ, res, footprint, regions, goal_dist_min, goal_dist_max, mask, seed
     reg = None if regions is None else np.ascontiguousarray(regions, np.int32)
     amb = np.empty(n, np.uint8)
     failed = np.empty(n, np.uint8)
-    lib().fno_reset(_p(occ, C.c_uint8), C.c_int(H), C.c_int(W), C.c_float(res), C.c_int(fp.shape[0]),
-                    _p(fp, C.c_float), C.c_int(nreg), _p(reg, C.c_int32), C.c_float(goal_dist_min),
-                    C.c_float(goal_dist_max), C.c_int(n), _p(mask, C.c_uint8), _p(seeds, C.c_uint64),
-                    C.c_double(eps), _p(states, C.c_float), _p(d_prev, C.c_float),
-                    _p(ep_step, C.c_int32), _p(amb, C.c_uint8), _p(failed, C.c_uint8))
+    with _components(components):
+        lib().fno_reset(_p(occ, C.c_uint8), C.c_int(H), C.c_int(W), C.c_float(res), C.c_int(fp.shape[0]),
+                        _p(fp, C.c_float), C.c_int(nreg), _p(reg, C.c_int32), C.c_float(goal_dist_min),
+                        C.c_float(goal_dist_max), C.c_int(n), _p(mask, C.c_uint8), _p(seeds, C.c_uint64),
+                        C.c_double(eps), _p(states, C.c_float), _p(d_prev, C.c_float),
+                        _p(ep_step, C.c_int32), _p(amb, C.c_uint8), _p(failed, C.c_uint8))
     return amb, failed
 
 
@@ -213,15 +215,24 @@ def eval_update(collision, d_new, goal_tol, ep_step_after, step_limit, reward, o
                           _p(steps, C.c_int32), _p(ret, C.c_float))
 
 
-def set_footprint_components(sizes=None):
-    """Footprint = union of polygons: sizes of the components whose vertex lists are
-    concatenated in `footprint`; None = a single polygon.  Applies to collision, reset, footprint_distance,
-    clearance_features and step until changed."""
-    if sizes is None or len(sizes) <= 1:
+class _components:
+    """A union of polygons: the vertex lists are concatenated in `footprint`, `sizes` gives the
+    vertex count of each polygon (None = one polygon).  The C side keeps the sizes in a file-scope variable; every
+    wrapper sets it for exactly one call through this context and puts it back to "one polygon" afterwards, so that
+    no call can inherit an earlier footprint's components."""
+
+    def __init__(self, sizes):
+        self.sizes = None if sizes is None else np.ascontiguousarray(sizes, np.int32)
+
+    def __enter__(self):
+        if self.sizes is not None and len(self.sizes) > 1:
+            lib().fno_set_footprint_components(C.c_int(len(self.sizes)), _p(self.sizes, C.c_int32))
+        else:
+            lib().fno_set_footprint_components(C.c_int(0), None)
+
+    def __exit__(self, *exc):
         lib().fno_set_footprint_components(C.c_int(0), None)
-    else:
-        a = np.ascontiguousarray(sizes, np.int32)
-        lib().fno_set_footprint_components(C.c_int(len(a)), _p(a, C.c_int32))
+        return False
 
 
 def sample_slot(seed: int, i: int, filled: int) -> int:
@@ -251,16 +262,17 @@ def ring_sample(ring, capacity, total, n_envs, B, A, seed, n_samples, want_next=
     return rows, nxt, slots
 
 
-def footprint_distance(footprint, px, py) -> float:
+def footprint_distance(footprint, px, py, components=None) -> float:
     """Eq. (3) for one body-frame point: distance to the polygon, 0 inside."""
     fp = _f32(footprint)
     f = lib().fno_footprint_distance
     f.restype = C.c_double
     f.argtypes = [C.c_int, C.POINTER(C.c_float), C.c_double, C.c_double]
-    return float(f(fp.shape[0], _p(fp, C.c_float), float(px), float(py)))
+    with _components(components):
+        return float(f(fp.shape[0], _p(fp, C.c_float), float(px), float(py)))
 
 
-def clearance_features(footprint, angles, max_range, n_sectors, ranges_, sensor=None, want_delta=False):
+def clearance_features(footprint, angles, max_range, n_sectors, ranges_, sensor=None, want_delta=False, components=None):
     """Eq. (3) + sector min-pooling.  ranges_ [n,B] f32 -> z [n,n_sectors] f32
     (, delta [n,B] f32)."""
     fp, ang, rg = _f32(footprint), _f32(angles), _f32(ranges_)
@@ -268,9 +280,10 @@ def clearance_features(footprint, angles, max_range, n_sectors, ranges_, sensor=
     z = np.empty((n, n_sectors), np.float32)
     delta = np.empty((n, B), np.float32) if want_delta else None
     sen = None if sensor is None else _f32(sensor)
-    lib().fno_clearance_features(C.c_int(fp.shape[0]), _p(fp, C.c_float), C.c_int(B), _p(ang, C.c_float),
-                                 _p(sen, C.c_float), C.c_float(max_range), C.c_int(n_sectors), C.c_int(n),
-                                 _p(rg, C.c_float), _p(delta, C.c_float), _p(z, C.c_float))
+    with _components(components):
+        lib().fno_clearance_features(C.c_int(fp.shape[0]), _p(fp, C.c_float), C.c_int(B), _p(ang, C.c_float),
+                                     _p(sen, C.c_float), C.c_float(max_range), C.c_int(n_sectors), C.c_int(n),
+                                     _p(rg, C.c_float), _p(delta, C.c_float), _p(z, C.c_float))
     return (z, delta) if want_delta else z
 
 
@@ -289,7 +302,8 @@ def step(wl, states, actions, forced, d_prev, ep_step, want_hit=True):
     gobs = np.empty((2, n), np.float32)
     rew = np.empty(n, np.float32)
     done = np.empty(n, np.uint8)
-    lib().fno_step(_p(occ, C.c_uint8), C.c_int(H), C.c_int(W), C.c_float(wl.resolution),
+    with _components(getattr(wl, "components", None)):
+      lib().fno_step(_p(occ, C.c_uint8), C.c_int(H), C.c_int(W), C.c_float(wl.resolution),
                    C.c_int(fp.shape[0]), _p(fp, C.c_float), C.c_int(B), _p(ang, C.c_float),
                    C.c_float(wl.max_range), C.c_int(wl.drive), _p(lim, C.c_float), C.c_float(wl.dt),
                    C.c_float(wl.goal_tol), C.c_int(wl.max_episode_steps), C.c_float(wl.r_success),

@@ -94,7 +94,7 @@ def run_parity(wl, steps, n=None, subset=None, seed=0, forced=None, check_every=
     n = wl.n_envs if n is None else n
     wl.n_envs = n
     B, A = wl.n_beams, wl.action_dim
-    oracle.set_footprint_components(getattr(wl, "components", None))      # a union of polygons, or None
+    comp = getattr(wl, "components", None)                              # a union of polygons, or None
     m, r, s = make_sim(wl, n)
     buf = Buffers(n, B, A)
     s.bind_aux(buf.hit, buf.reward)
@@ -117,7 +117,7 @@ def run_parity(wl, steps, n=None, subset=None, seed=0, forced=None, check_every=
         ref = pre.copy()
         d_prev, ep = d_prev0.copy(), ep0.copy()
         amb, failed = oracle.reset(wl.occ, wl.resolution, wl.footprint, wl.regions, wl.goal_dist_min,
-                                   wl.goal_dist_max, mask_np, seeds_row, ref, d_prev, ep)
+                                   wl.goal_dist_max, mask_np, seeds_row, ref, d_prev, ep, components=comp)
         okm = (mask_np != 0) & (amb == 0)
         rep.add("resets", (mask_np != 0).sum())
         rep.add("resets_ambiguous", ((mask_np != 0) & (amb != 0)).sum())
@@ -164,7 +164,7 @@ def run_parity(wl, steps, n=None, subset=None, seed=0, forced=None, check_every=
                 assert np.all(close_state(post[p], ref[p])), f"step {t}: state plane {p} off by {np.abs(post[p] - ref[p]).max()}"
             assert np.all(ang_diff(post[2], ref[2]) <= TOL_STATE * np.maximum(1, np.abs(ref[2]))), f"step {t}: psi"
             x, y, psi = post[0], post[1], post[2]
-            flag, camb = oracle.collision(wl.occ, wl.resolution, wl.footprint, x, y, psi)
+            flag, camb = oracle.collision(wl.occ, wl.resolution, wl.footprint, x, y, psi, components=comp)
             gcol = buf.col.cpu().numpy()
             okc = camb == 0
             rep.add("collision_checks", n)
@@ -254,7 +254,6 @@ def run_parity(wl, steps, n=None, subset=None, seed=0, forced=None, check_every=
     assert cnt["oob_window_loads"] == 0, "the instrumented beam kernel read a window outside the packed map"
     assert cnt["reset_failures"] == rep.c.get("reset_failures", 0) or check_every > 1
     s.close(); r.close(); m.close()
-    oracle.set_footprint_components(None)
     assert_ambiguity_bounds(rep)
     return rep
 

@@ -74,6 +74,12 @@ def test_host_side_argument_errors_need_no_gpu(fn):
     # the switches between equivalent launch sequences
     assert lib.fn_sim_set_fused_reset(None, 1, None) == -1 and lib.fn_sim_set_split_step(None, 1, None) == -1
     assert lib.fn_step_host(None, None, None, ctypes.c_float(0.1), None, None, None, None, None) == -1
+    # round 2: coarse level, pipelined host step, further sensors
+    assert lib.fn_sim_set_coarse(None, 1, None) == -1
+    assert lib.fn_step_host_begin(None, 0, None, None, ctypes.c_float(0.1), None, None, None, None, None, None) == -1
+    assert lib.fn_step_host_end(None, 0) == -1
+    assert lib.fn_robot_add_sensor(None, p(ang), 1, ctypes.c_float(1.0), ctypes.c_float(0), ctypes.c_float(0), ctypes.c_float(0)) == -1
+    assert lib.fn_sim_beam_config(None, None) == -1
 
 
 def test_no_cpu_fallback(fn):

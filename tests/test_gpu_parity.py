@@ -970,26 +970,22 @@ def test_union_of_polygons_footprints(pu):
         "dumbbell": (np.concatenate([rect(-0.3, 0.0, 0.2, 0.2), rect(0.3, 0.0, 0.2, 0.2)]), [4, 4], 2),
         "plus": (np.concatenate([rect(0, 0, 0.6, 0.16), rect(0, 0, 0.16, 0.6), W.footprint_ngon(0.12, 8)]), [4, 4, 8], 1),
     }
-    try:
-        for name, (fp, comp, cfg) in shapes.items():
-            wl = W.make_workload(cfg, n_envs=384)
-            wl.footprint, wl.components = fp, comp
-            rep = pu.run_parity(wl, steps=10, subset=48, check_every=2)
-            print(name, rep)
-            assert rep.c["collisions"] > 0 and rep.c["resets"] > 384
-            # clearance features of the union
-            n, B = 64, wl.n_beams
-            wl.n_envs = n
-            m, r, s = pu.make_sim(wl, n)
-            buf = pu.Buffers(n, B, wl.action_dim)
-            z = torch.zeros(n, 18, device="cuda")
-            s.bind_features(18, z)
-            buf.mask.fill_(1)
-            s.reset(buf.states, buf.mask, torch.from_numpy(W.seed_tape(wl, 1, 1)[0].view(np.int64)).cuda(), buf.ranges, buf.gobs)
-            torch.cuda.synchronize()
-            oracle.set_footprint_components(comp)
-            ze = oracle.clearance_features(fp, wl.beam_angles, wl.max_range, 18, buf.ranges.cpu().numpy())
-            assert np.abs(z.cpu().numpy() - ze).max() <= 1e-4, name
-            s.close(); r.close(); m.close()
-    finally:
-        oracle.set_footprint_components(None)
+    for name, (fp, comp, cfg) in shapes.items():
+        wl = W.make_workload(cfg, n_envs=384)
+        wl.footprint, wl.components = fp, comp
+        rep = pu.run_parity(wl, steps=10, subset=48, check_every=2)
+        print(name, rep)
+        assert rep.c["collisions"] > 0 and rep.c["resets"] > 384
+        # clearance features of the union
+        n, B = 64, wl.n_beams
+        wl.n_envs = n
+        m, r, s = pu.make_sim(wl, n)
+        buf = pu.Buffers(n, B, wl.action_dim)
+        z = torch.zeros(n, 18, device="cuda")
+        s.bind_features(18, z)
+        buf.mask.fill_(1)
+        s.reset(buf.states, buf.mask, torch.from_numpy(W.seed_tape(wl, 1, 1)[0].view(np.int64)).cuda(), buf.ranges, buf.gobs)
+        torch.cuda.synchronize()
+        ze = oracle.clearance_features(fp, wl.beam_angles, wl.max_range, 18, buf.ranges.cpu().numpy(), components=comp)
+        assert np.abs(z.cpu().numpy() - ze).max() <= 1e-4, name
+        s.close(); r.close(); m.close()

@@ -792,7 +792,7 @@ __device__ __forceinline__ void run_beam_tasks(const BeamArgs& a, const BeamMap<
         const unsigned next = feed.prefetch();
         // (listed env, beam) of this lane's element idx = 32 task + lane
         const unsigned idx = (feed.task << 5) + lane;
-        const unsigned le = (unsigned)__umul64hi((unsigned long long)idx, invB);     // idx / B, exact for idx < 2^32
+        const unsigned le = B > 1 ? (unsigned)__umul64hi((unsigned long long)idx, invB) : idx;   // idx / B, exact for idx < 2^32 (B = 1: invB wraps to 0)
         const unsigned j = idx - le * (unsigned)B;
         if (le < (unsigned)n_env) {
             const unsigned e = list ? (unsigned)list[le] : le;

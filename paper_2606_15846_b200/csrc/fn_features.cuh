@@ -105,7 +105,7 @@ __global__ void __launch_bounds__(kFeatWarps * 32) features_kernel(FeatArgs a) {
                     }
                     d = inside ? 0.0f : fminf(sqrtf(d2), a.rmax);  // capped at the sensor range
                 }
-                const unsigned k = (unsigned)__umul64hi((unsigned long long)j * (unsigned)a.n_sectors, invB);
+                const unsigned k = a.B > 1 ? (unsigned)__umul64hi((unsigned long long)j * (unsigned)a.n_sectors, invB) : 0u;   // (B = 1: one sector)
                 atomicMin(&s_z[k], __float_as_uint(d));
             }
         }

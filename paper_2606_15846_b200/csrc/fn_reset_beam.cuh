@@ -89,7 +89,7 @@ __global__ void __launch_bounds__(kFusedThreads, 2) reset_beam_kernel(const __gr
         uint32_t words = 0, rays = 0;
         for (unsigned task = (unsigned)wib; task < ntasks; task += blockDim.x >> 5) {
             const unsigned idx = (task << 5) + lane;
-            const unsigned k = (unsigned)__umul64hi((unsigned long long)idx, invB);      // idx / B
+            const unsigned k = B > 1 ? (unsigned)__umul64hi((unsigned long long)idx, invB) : idx;      // idx / B
             const unsigned j = idx - k * (unsigned)B;
             if (k < (unsigned)m_loc) {
                 const unsigned e = (unsigned)rlist[blockIdx.x + k * gridDim.x];

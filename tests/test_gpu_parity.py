@@ -33,6 +33,30 @@ def test_c1_ragged_env_counts(pu):
         print(n, pu.run_parity(wl, steps=12, seed=n))
 
 
+def test_degenerate_beam_tables(pu):
+    # one beam per robot (B = 1: every "idx / B" of the kernels degenerates), 33 beams (one full round and one beam),
+    # with and without clearance features; a shared-memory map and an L2 map; instrumented and production kernels
+    import torch
+    from harness import workloads as W
+    for cfg, nb, n in ((1, 1, 70), (1, 33, 5), (4, 1, 300)):
+        wl = W.make_workload(cfg, n_envs=n)
+        wl.beam_angles = W.beam_table(nb, 200.0) if nb > 1 else np.array([0.3], np.float32)
+        rep = pu.run_parity(wl, steps=8, seed=nb)
+        print(cfg, nb, rep)
+        assert rep.c["beams"] >= 8 * n * nb
+        m, r, s = pu.make_sim(wl, n)
+        buf = pu.Buffers(n, nb, wl.action_dim)
+        z = torch.zeros(n, 1, device="cuda")
+        s.bind_features(1, z)
+        buf.mask.fill_(1)
+        s.reset(buf.states, buf.mask, torch.from_numpy(W.seed_tape(wl, 1, 2)[0].view(np.int64)).cuda(), buf.ranges, buf.gobs)
+        torch.cuda.synchronize()
+        import oracle
+        ze = oracle.clearance_features(wl.footprint, wl.beam_angles, wl.max_range, 1, buf.ranges.cpu().numpy())
+        assert np.abs(z.cpu().numpy() - ze).max() <= 1e-4
+        s.close(); r.close(); m.close()
+
+
 def test_c2_rect_subset(pu):
     from harness import workloads as W
     wl = W.make_workload(2)

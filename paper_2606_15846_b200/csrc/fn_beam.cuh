@@ -817,7 +817,7 @@ __device__ __forceinline__ void fast_finish(const BeamArgs& a, FastWarp& w, cons
     if ((threadIdx.x & 31) == 0 && w.rays) atomicAdd(&a.counters[kRays], (unsigned long long)w.rays);
 }
 // The envs' beams as warp tasks, handed out in order by one atomic counter (fetched one task ahead, so that its
-// latency is hidden; a warp's first task is its own index).  Two sizes: the first 27/32 of the envs go out in chunks
+// latency is hidden; a warp's first task is its own index).  Two sizes: the first 24/32 of the envs go out in chunks
 // of chunk_rounds x 32 beams -- what depends on the env is amortised over the chunk -- and the rest in single
 // rounds of 32 beams, so that the launch ends within one round's time on every SM (beams differ in length by an
 // order of magnitude; a static split of such chunks left 13 % of the SM time idle).  Small launches (fewer than
@@ -829,7 +829,7 @@ __device__ __forceinline__ void run_fast_tasks(const BeamArgs& a, FastWarp& w, c
                                                const unsigned nwarps, const bool has_static = true) {
     const unsigned B = (unsigned)a.robot.B, rounds = (B + 31u) >> 5;
     const unsigned nchunk = (unsigned)a.nchunk, cbeams = (unsigned)a.chunk_rounds << 5;
-    const unsigned nA = (unsigned)n_env * rounds >= 8u * nwarps ? ((unsigned)n_env * 27u) >> 5 : 0u;   // envs cast in chunks
+    const unsigned nA = (unsigned)n_env * rounds >= 8u * nwarps ? ((unsigned)n_env * 24u) >> 5 : 0u;   // envs cast in chunks
     const unsigned ntA = nA * nchunk, nt = ntA + ((unsigned)n_env - nA) * rounds;
     const unsigned lane = threadIdx.x & 31;
     unsigned t = warp0;

@@ -484,24 +484,25 @@ __device__ __forceinline__ float cast_beam_fast(const uint32_t slot, const uint3
     }
     __syncwarp();                                                 // resolve all hits of the warp together
     if (xh != 0u) {                                               // later lines are farther away
+        // Everything below is in the hit line's own bit-offset units (high words of D's).  The hit cell c is the
+        // first occupied cell of the exact window in travel order (highest bit backward, lowest bit forward); the beam
+        // enters it through the line boundary when c is the line's entry cell (the cell of the entry crossing
+        // Dp = Dh - M: never so in line 0, whose entry cell is the free origin cell), else through the cell's u-face,
+        // whose coordinate is c + 1 in D's convention for both directions (forward D's carry + 1).
         const uint32_t hl = hiw(Dh);
-        const bool first = hl == h0;
-        const int cx = (int)(hl - fu1);
         const double Dp = Dh - Mu;                                // entry crossing, same line field
-        const int ce = first ? (int)hc0 : (int)(hiw(Dp) - fu1);
-        // first occupied cell in travel order: highest bit backward, lowest bit forward
-        const int c = cx - (int)(fu1 * 31u) + (31 - __clz(su ? xh : xh & (0u - xh)));
+        const uint32_t c = hl - (fu1 << 5) + (uint32_t)(31 - __clz(su ? xh : xh & (0u - xh)));
+        const bool ent = c == hiw(Dp) - fu1;
         // lines crossed: the integer fields of line k and line 0 differ by +-k S +- (cells along u)
         uint32_t half_S, inv_magic, S;
         asm volatile("ld.shared.u32 %0, [%1+28];" : "=r"(half_S) : "r"(ax));
         asm volatile("ld.shared.v2.u32 {%0, %1}, [%2+32];" : "=r"(inv_magic), "=r"(S) : "r"(ax));
-        const unsigned dq = sw ? h0 - hl : hl - h0;
-        const unsigned k = __umulhi(dq + half_S, inv_magic);
-        const unsigned lf = sw ? 0u - k * S : k * S;              // line field of line k relative to line 0
-        // entry distance along u: through the line boundary (c == ce) or through the cell's u-face
-        const double a = c == ce ? add_hi(Dp, 0u - lf) : __hiloint2double((int)((unsigned)c + (su >> 31) - lf), 0);
-        const double b = c == ce ? add_hi(hq.y, fu1) : hq.y;
-        const double dU = (c == ce && first) ? 0.0 : fabs(a - b);
+        const int sgw = sw ? -1 : 1;
+        const uint32_t k = __umulhi((hl - h0) * (uint32_t)sgw + half_S, inv_magic);
+        const uint32_t lf = k * S * (uint32_t)sgw;                // line field of line k relative to line 0
+        // entry distance along u = | hit coordinate - origin |, both with line 0's field
+        const double a = __hiloint2double((int)((ent ? hiw(Dp) : c + 1u) - lf), ent ? __double2loint(Dp) : 0);
+        const double dU = fabs(a - add_hi(hq.y, fu1));
         const double adu = fabs(du);
         if (dU < T * adu) r = range_from_du(dU, range_scale(adu, rho));
     }
@@ -653,6 +654,35 @@ __device__ __noinline__ void fast_drain(const BeamArgs& a, const uint32_t queue,
     }
     __syncwarp();
 }
+// the rounds of a task: 32 beams each, one per lane (the env's slot is staged)
+template <bool kCoarse, bool kRing>
+__device__ __forceinline__ void fast_rounds(const BeamArgs& a, FastWarp& w, const int state, const unsigned e,
+                                            const unsigned jb0, const unsigned jb1, const unsigned long long ring_head) {
+    const unsigned lane = threadIdx.x & 31;
+    const unsigned B = (unsigned)a.robot.B;
+    unsigned j = jb0 + lane;
+    float* po = a.out_ranges + (e * a.out_stride + a.out_off + j); // n_envs * row length < 2^31 (fn_sim_create)
+    float* pr = kRing ? ring_row_of(a, ring_head, e) + (a.out_off + j) : nullptr;
+    uint32_t tj = w.tab + 16u * j;
+#pragma unroll 1
+    for (unsigned jb = jb0; jb < jb1; jb += 32u, j += 32u, po += 32, pr += 32, tj += 512u) {
+        bool near = false;
+        float r = 0.0f;
+        if (state == 0) r = cast_beam_fast<kCoarse>(w.slot, min(tj, w.tab_last), a.robot.T, a.half_T, a.map.rho, a.robot.rmax, near);
+        const bool act = j < B;
+        const unsigned nm = __ballot_sync(0xffffffffu, near && act);
+        if (act && !near) {
+            *po = r;
+            if (kRing) *pr = r;
+        }
+        if (nm) {                                                  // (rare: the warp's beams cross an axis)
+            if (near && act) asm volatile("st.shared.u32 [%0], %1;" ::"r"(w.queue + 4u * (w.qn + __popc(nm & ((1u << lane) - 1u)))), "r"(e * B + j) : "memory");
+            w.qn += __popc(nm);
+            __syncwarp();
+            if (w.qn >= 32u) { w.qn -= 32u; fast_drain(a, w.queue + 4u * w.qn, 32u, w.map_base, w.tab, ring_head); }
+        }
+    }
+}
 // one task: beams [jb0, jb1) of env e, jb0 a multiple of 32 (pose = the env's sensing pose, possibly a shared-memory copy)
 template <bool kCoarse>
 __device__ __forceinline__ void fast_chunk(const BeamArgs& a, FastWarp& w, const BeamPose* pose, const unsigned e,
@@ -670,30 +700,8 @@ __device__ __forceinline__ void fast_chunk(const BeamArgs& a, FastWarp& w, const
     const int state = pose->state;
     __syncwarp();
     w.rays += jb1 - jb0;
-    unsigned j = jb0 + lane;
-    const unsigned o0 = e * B;                                     // index of the env's beam 0 (deferred beams: o0 + j)
-    float* po = a.out_ranges + (e * a.out_stride + a.out_off + j); // n_envs * row length < 2^31 (fn_sim_create)
-    float* pr = nullptr;
-    if (a.ring_obs) pr = ring_row_of(a, ring_head, e) + (a.out_off + j);
-    uint32_t tj = w.tab + 16u * j;
-#pragma unroll 1
-    for (unsigned jb = jb0; jb < jb1; jb += 32u, j += 32u, po += 32, tj += 512u) {
-        bool near = false;
-        float r = 0.0f;
-        if (state == 0) r = cast_beam_fast<kCoarse>(w.slot, min(tj, w.tab_last), a.robot.T, a.half_T, a.map.rho, a.robot.rmax, near);
-        if (j >= B) near = false;
-        else if (!near) {
-            *po = r;
-            if (a.ring_obs) pr[jb - jb0] = r;
-        }
-        if (__any_sync(0xffffffffu, near)) {                       // (rare: the warp's beams cross an axis)
-            const unsigned nm = __ballot_sync(0xffffffffu, near);
-            if (near) asm volatile("st.shared.u32 [%0], %1;" ::"r"(w.queue + 4u * (w.qn + __popc(nm & ((1u << lane) - 1u)))), "r"(o0 + j) : "memory");
-            w.qn += __popc(nm);
-            __syncwarp();
-            if (w.qn >= 32u) { w.qn -= 32u; fast_drain(a, w.queue + 4u * w.qn, 32u, w.map_base, w.tab, ring_head); }
-        }
-    }
+    if (a.ring_obs) fast_rounds<kCoarse, true>(a, w, state, e, jb0, jb1, ring_head);    // (two copies of the round loop: a
+    else fast_rounds<kCoarse, false>(a, w, state, e, jb0, jb1, ring_head);              //  predicated-off ring store still issues)
 }
 
 // words of the staged image with the coarse copies: fine copies (padded to 16 bytes), then the coarse ones

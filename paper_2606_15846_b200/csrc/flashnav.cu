@@ -634,9 +634,16 @@ static BeamArgs beam_args(fn_sim* s, const int* list, const int* count_dev, floa
     return b;
 }
 
-static int launch_beams(fn_sim* s, const int* list, const int* count_dev, float* out_ranges, bool step_launch = false, bool done_list = false) {
+// a sim sizes its poses, shared memory and output rows for the robot's sensors at fn_sim_create: every call
+// that launches a kernel checks first that none was added since (the env kernels write one pose per sensor)
+static int sensors_unchanged(const fn_sim* s) {
     if ((int)s->robot->sensors.size() != s->n_sensors)
         return fail(FN_ERR_INVALID_ARG, "the robot's sensors changed after fn_sim_create");
+    return FN_OK;
+}
+
+static int launch_beams(fn_sim* s, const int* list, const int* count_dev, float* out_ranges, bool step_launch = false, bool done_list = false) {
+    if (int rc0 = sensors_unchanged(s)) return rc0;
     const bool aux = s->count_words || s->aux_hit;
     const dim3 grid(s->beam_grid), block(kBeamThreads);
     for (int k = 0; k < s->n_sensors; ++k) {                      // one launch per sensor
@@ -682,6 +689,7 @@ extern "C" int fn_step(fn_sim* s, float* states, const float* actions, float dt,
     if (!s || !states || !actions || !reset_mask || !out_ranges || !out_collision || !out_goal_obs)
         return fail(FN_ERR_INVALID_ARG, "fn_step: NULL argument");
     if (!std::isfinite(dt) || dt < 0.0f) return fail(FN_ERR_INVALID_ARG, "fn_step: dt must be finite and >= 0");
+    if (int rc0 = sensors_unchanged(s)) return rc0;
     // evaluation steps are not training transitions: they never touch the replay ring or its head
     struct RingOff {
         fn_sim* s; float* keep;
@@ -744,6 +752,7 @@ extern "C" int fn_reset(fn_sim* s, float* states, const uint8_t* mask, const uin
                         float* out_ranges, float* out_goal_obs) {
     if (!s || !states || !seeds || !out_ranges || !out_goal_obs)
         return fail(FN_ERR_INVALID_ARG, "fn_reset: NULL argument");
+    if (int rc0 = sensors_unchanged(s)) return rc0;
     if (!mask && !s->done_avail)
         return fail(FN_ERR_INVALID_ARG, "fn_reset: mask_dev == NULL needs a preceding fn_step (its done list is used once)");
     const int* list = mask ? s->d_list : s->d_done_list;
@@ -795,6 +804,7 @@ extern "C" int fn_reset(fn_sim* s, float* states, const uint8_t* mask, const uin
 
 extern "C" int fn_observe_all(fn_sim* s, const float* states, float* out_ranges, float* out_goal_obs) {
     if (!s || !states || !out_ranges) return fail(FN_ERR_INVALID_ARG, "fn_observe_all: NULL argument");
+    if (int rc0 = sensors_unchanged(s)) return rc0;
     PoseArgs a;
     a.map = s->map->dev; a.robot = robot_dev(s->robot, s->map); a.n = s->n; a.states = states;
     a.out_goal_obs = out_goal_obs; a.poses = s->d_poses; a.beam_task_counter = s->d_task_counter;
@@ -832,6 +842,7 @@ extern "C" int fn_ranges_fixed_step(fn_sim* s, const float* states, float delta_
 extern "C" int fn_eval_begin(fn_sim* s, float* states, int n_cases, int step_limit, float* out_ranges, float* out_goal_obs) {
     if (!s || !states || !out_ranges || !out_goal_obs) return fail(FN_ERR_INVALID_ARG, "fn_eval_begin: NULL argument");
     if (n_cases < 1 || n_cases > s->n) return fail(FN_ERR_INVALID_ARG, "fn_eval_begin: n_cases must be in 1..n_envs");
+    if (int rc0 = sensors_unchanged(s)) return rc0;
     if (step_limit < 1) return fail(FN_ERR_INVALID_ARG, "fn_eval_begin: the evaluation step limit must be >= 1");
     EvalBeginArgs a;
     a.pose.map = s->map->dev; a.pose.robot = robot_dev(s->robot, s->map); a.pose.n = s->n; a.pose.states = states;

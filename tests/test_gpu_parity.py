@@ -342,6 +342,18 @@ def test_several_sensors_against_the_oracle(pu):
         z = torch.zeros(n, 8, device="cuda")
         with pytest.raises(fn.FlashNavError):
             s.bind_features(8, z)                                 # clearance features: single-sensor robots only
+        # a sensor added after fn_sim_create: the sim's poses and rows were sized without it, every call refuses
+        if cfg == 2:
+            r.add_sensor(W.beam_table(8, 90.0), 1.0, 0.0, 0.0, 0.0)
+            before = buf.states.clone()
+            big = torch.zeros(n, r.B, device="cuda")              # (sized for the new row, so that the library decides)
+            for call in (lambda: s.step(buf.states, actions[0], float(wl.dt), buf.mask, big, buf.col, buf.gobs),
+                         lambda: s.reset(buf.states, buf.mask, seeds[0], big, buf.gobs),
+                         lambda: s.observe_all(buf.states, big)):
+                with pytest.raises(fn.FlashNavError, match="sensors changed"):
+                    call()
+            torch.cuda.synchronize()
+            assert torch.equal(buf.states, before)
         s.close(); r.close(); m.close()
 
 

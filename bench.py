@@ -269,6 +269,8 @@ def run_ours(args):
     def step(t):
         k = t % tape_len
         mask.copy_(forced[k])
+        if args.prepare:                                      # the seeds of the reset below, announced before the step
+            sim.prepare_reset(seeds[k])
         sim.step(states, actions[k], float(wl.dt), mask, ranges, col, gobs)
         sim.reset(states, None, seeds[k], ranges, gobs)       # mask = None: the envs this step reported done
 
@@ -520,7 +522,8 @@ def run_ours(args):
                "dtype": "f64", "data": "synthetic",
                "config": config_dict(args.config, wl),
                "launch": {"l2": "flushed between timed steps", "ring_attached": bool(ring is not None),
-                          "fused_reset": bool(fused_active), "split_step": bool(split_step), "coarse_level": bool(coarse_active)},
+                          "fused_reset": bool(fused_active), "split_step": bool(split_step), "coarse_level": bool(coarse_active),
+                          "prepared_resets": float(c1["resets_prepared"] - c0["resets_prepared"]) / max(1, c1["envs_reset"] - c0["envs_reset"])},
                "protocol": {"repetitions": R, "value": "median over repetitions", "value_iqr": [float(np.percentile(rep_values, 25)), float(np.percentile(rep_values, 75))],
                             "values": [float(v) for v in rep_values], "ms_per_step_iqr": [float(np.percentile(rep_ms, 25)) / K, float(np.percentile(rep_ms, 75)) / K],
                             "note": "PAPER.md:175: warm-up, then K timed steps between syncs, repeated; median and IQR"},
@@ -631,6 +634,7 @@ def main():
     ap.add_argument("--sample-batch", type=int, default=65536, help="U x B of the replay-sampling leg (configs with a ring; 0 = skip)")
     ap.add_argument("--paper-query", type=int, default=1, help="also time the paper's fixed-step range query (information only)")
     ap.add_argument("--features", type=int, default=36, help="sectors of the clearance-feature leg (0 = skip; information only)")
+    ap.add_argument("--prepare", type=int, default=1, help="announce each step's reset seeds before the step (fn_sim_prepare_reset)")
     ap.add_argument("--graph", type=int, default=1, help="also time a CUDA-graph replay of the steps (information only)")
     ap.add_argument("--fused-reset", type=int, default=-1, choices=[-1, 0, 1],
                     help="fn_reset(done list) as one fused kernel (1) or two kernels (0); -1 = the library's default")

@@ -37,7 +37,8 @@ enum { FN_DRIVE_DIFF = 0, FN_DRIVE_OMNI = 1 };
 enum { FN_MAX_VERTS = 64, FN_MAX_ATTEMPTS = 256 };
 enum { FN_N_COUNTERS = 8 };   /* rays cast, map words loaded, envs reset, reset failures,
                                  non-finite actions, env steps, map windows outside the packed map seen by
-                                 the instrumented beam kernel (a self-check: must stay 0), reserved */
+                                 the instrumented beam kernel (a self-check: must stay 0), envs whose reset
+                                 was prepared by the step before (fn_sim_prepare_reset; also counted as reset) */
 
 typedef struct fn_map fn_map;
 typedef struct fn_robot fn_robot;
@@ -220,6 +221,21 @@ int fn_sim_beam_config(const fn_sim* sim, int* cfg_out);
  * be NULL) = 1 if the level is available and enabled.  Host-side switch, takes effect at the next launch.
  * Errors: FN_ERR_INVALID_ARG (NULL sim). */
 int fn_sim_set_coarse(fn_sim* sim, int enable, int* active_out);
+
+/* ---- a reset announced before the step ("When episodes end, only the corresponding environments are
+ * reset and their observations recomputed").  The reset of an env -- start pose and goal drawn from seeds[e] by the
+ * rule of fn_reset -- does not depend on the step's result, only on WHICH envs end.  fn_sim_prepare_reset(sim,
+ * seeds_dev) announces the seeds the fn_reset(mask = NULL) after the NEXT fn_step will be called with; that fn_step
+ * then also runs the reset of every env it reports done, on the warps that compute the outcomes, into buffers of the
+ * sim (states, outputs and the terminal observation of the step are what they are without the announcement), and the
+ * fn_reset(sim, states, NULL, seeds_dev, ...) that follows copies those results and recomputes the observations.
+ * Results are bit-identical with and without the announcement (tested).  The announcement serves one fn_step; it is
+ * a hint and is dropped -- fn_reset then does the whole reset -- when the sim has no such kernel (map read through
+ * L2, several sensors, instruments bound, coarse level, evaluation mode), when fn_reset is called with a mask or
+ * other seeds, or when fn_map_set_regions / fn_robot_set_sensor ran in between.  seeds_dev [N] is READ DURING
+ * fn_step and must hold the same values until fn_reset.  seeds_dev = NULL withdraws an announcement.
+ * Errors: FN_ERR_INVALID_ARG (NULL sim), FN_ERR_OOM / FN_ERR_CUDA (first call: the sim's buffers, 177 bytes per env). */
+int fn_sim_prepare_reset(fn_sim* sim, const uint64_t* seeds_dev);
 
 /* ---- fn_reset as one launch or two.  When the packed map is staged in shared memory (cfg_out[0] of
  * fn_sim_beam_config) and the reset scratch fits beside it, fn_reset(mask = NULL) -- the step's done list,

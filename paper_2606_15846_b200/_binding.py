@@ -13,13 +13,13 @@ _lib = None
 DRIVE_DIFF, DRIVE_OMNI = 0, 1
 N_COUNTERS = 8
 COUNTER_NAMES = ("rays_cast", "map_words_loaded", "envs_reset", "reset_failures", "nonfinite_actions",
-                 "env_steps", "oob_window_loads", "reserved1")
+                 "env_steps", "oob_window_loads", "resets_prepared")
 
 EXPORTED_SYMBOLS = (
     "fn_map_create", "fn_map_set_regions", "fn_map_destroy", "fn_robot_create", "fn_robot_create_union", "fn_robot_set_sensor", "fn_robot_add_sensor", "fn_robot_set_acc_limits",
     "fn_robot_destroy", "fn_task_default", "fn_sim_create", "fn_sim_destroy", "fn_sim_set_stream", "fn_step", "fn_reset",
     "fn_sim_bind_aux", "fn_sim_bind_features", "fn_ring_attach", "fn_ring_sample", "fn_ranges_fixed_step", "fn_eval_begin", "fn_eval_result", "fn_eval_end", "fn_observe_all", "fn_get_counters", "fn_sim_count_words",
-    "fn_sim_episode_state", "fn_sim_beam_config", "fn_sim_set_fused_reset", "fn_sim_set_split_step", "fn_sim_set_coarse", "fn_sim_profile", "fn_sim_profile_read", "fn_step_host", "fn_step_host_begin", "fn_step_host_end", "fn_measure_peak", "fn_last_error", "fn_version")
+    "fn_sim_episode_state", "fn_sim_beam_config", "fn_sim_set_fused_reset", "fn_sim_set_split_step", "fn_sim_set_coarse", "fn_sim_prepare_reset", "fn_sim_profile", "fn_sim_profile_read", "fn_step_host", "fn_step_host_begin", "fn_step_host_end", "fn_measure_peak", "fn_last_error", "fn_version")
 
 
 class FlashNavError(RuntimeError):
@@ -77,6 +77,7 @@ def load_library():
         "fn_sim_set_fused_reset": [vp, i32, vp],
         "fn_sim_set_split_step": [vp, i32, vp],
         "fn_sim_set_coarse": [vp, i32, vp],
+        "fn_sim_prepare_reset": [vp, vp],
         "fn_sim_profile": [vp, i32],
         "fn_sim_profile_read": [vp, vp, vp],
         "fn_step_host": [vp, vp, vp, f32, vp, vp, vp, vp, vp],
@@ -371,6 +372,16 @@ class Sim:
         act = C.c_int(0)
         _check(load_library().fn_sim_set_coarse(self._h, 1 if enable else 0, C.byref(act)), "fn_sim_set_coarse")
         return bool(act.value)
+
+    def prepare_reset(self, seeds):
+        """Announce the seeds of the reset(mask=None) that follows the NEXT step(): that step then also prepares the
+        reset of the envs it reports done (same results, the reset's latency leaves the critical path).  None withdraws."""
+        import torch
+        if seeds is not None and seeds.dtype not in (torch.int64, torch.uint64):
+            raise FlashNavError("seeds must be a 64-bit integer tensor")
+        self._prep_keep = seeds
+        _check(load_library().fn_sim_prepare_reset(
+            self._h, None if seeds is None else _dev_ptr(seeds, seeds.dtype, self.n, "seeds")), "fn_sim_prepare_reset")
 
     @staticmethod
     def _host_ptr(a, name):

@@ -47,6 +47,7 @@ struct fn_map {
     MapDev dev;
     int n_regions;
     int4* d_regions;
+    unsigned version;        // bumped by every setter (a reset prepared ahead must see the map it is applied with)
 };
 
 constexpr int kMaxSensors = 4;
@@ -69,6 +70,7 @@ struct fn_robot {
     int n_samples;
     std::vector<int> nxt;            // next vertex within the vertex's component (union of polygons)
     int* d_nxt;
+    unsigned version;                // bumped by every setter
 };
 
 struct fn_sim {
@@ -115,6 +117,14 @@ struct fn_sim {
     size_t split_smem;
     int split_grid;
     StepEnd* d_step_end;
+    // fn_sim_prepare_reset: the step's outcome warps also run the reset of the envs they report done (prep_ok: the
+    // kernels exist for this sim); prep_next = the seeds announced for the coming fn_step, prep_ready = the seeds the
+    // buffers were filled with by the last fn_step (with the map / robot versions they were filled under)
+    bool prep_ok;
+    const uint64_t *prep_next, *prep_ready;
+    unsigned prep_map_ver, prep_robot_ver;
+    PreparedReset d_prep;
+    int* d_prep_epstep;
     // the coarse level in the production beam kernels (one CTA of 1024 threads per SM, fine + coarse copies staged)
     bool coarse_ok, coarse_on, split_ok_c;
     size_t beam_smem_c, split_smem_c;
@@ -228,6 +238,7 @@ extern "C" int fn_map_set_regions(fn_map* m, int n, const int32_t* rects) {
         FN_CUDA(cudaMemcpy(m->d_regions, rects, (size_t)n * sizeof(int4), cudaMemcpyHostToDevice));
         m->n_regions = n;
     }
+    ++m->version;
     return FN_OK;
 }
 
@@ -355,6 +366,7 @@ extern "C" int fn_robot_set_sensor(fn_robot* r, float sx, float sy, float spsi) 
     if (!r || !std::isfinite(sx) || !std::isfinite(sy) || !std::isfinite(spsi)) return fail(FN_ERR_INVALID_ARG, "fn_robot_set_sensor: bad argument");
     r->sensor[0] = sx; r->sensor[1] = sy; r->sensor[2] = spsi;
     r->sensors[0].sx = sx; r->sensors[0].sy = sy; r->sensors[0].spsi = spsi;
+    ++r->version;
     return robot_upload(r);
 }
 
@@ -374,6 +386,7 @@ extern "C" int fn_robot_add_sensor(fn_robot* r, const float* angles, int B, floa
     r->angles.insert(r->angles.end(), angles, angles + B);
     r->B += B;
     if (rmax > r->rmax) r->rmax = rmax;                            // the robot's largest range (clearance cap, limits)
+    ++r->version;
     return robot_upload(r);
 }
 
@@ -536,6 +549,13 @@ extern "C" int fn_sim_create(const fn_map* map, const fn_robot* robot, int n, co
                 // two such batches (measured: C1-C4 3-8 % faster per step, C5 with 222 envs per CTA 4 % slower)
                 s->split_on = (n + s->split_grid - 1) / s->split_grid <= 64;
             }
+            // ... and its variant that prepares the resets (served by the fused reset kernel)
+            s->prep_ok = false;
+            if (e == cudaSuccess && s->split_ok && s->use_smem && s->fused_ok) {
+                int fp = 0;
+                e = kernel_config(step_beam_kernel<true, false, false, true>, kBeamThreads, s->split_smem, max_optin, &fp);
+                s->prep_ok = e == cudaSuccess && s->num_sms * fp >= s->split_grid;
+            }
         }
         // the coarse level: fine + coarse copies staged by one CTA of 1024 threads per SM
         s->coarse_ok = s->coarse_on = s->split_ok_c = false;
@@ -569,6 +589,8 @@ extern "C" int fn_sim_destroy(fn_sim* s) {
     cudaFree(s->d_poses); cudaFree(s->d_ring_head); cudaFree(s->d_list); cudaFree(s->d_count); cudaFree(s->d_dprev);
     cudaFree(s->d_epstep); cudaFree(s->d_counters); cudaFree(s->d_task_counter);
     cudaFree(s->d_step_end);
+    cudaFree(s->d_prep.states); cudaFree(s->d_prep.goal_obs); cudaFree(s->d_prep.d_prev); cudaFree(s->d_prep.poses);
+    cudaFree(s->d_prep.fail); cudaFree(s->d_prep_epstep);
     cudaFree(s->d_done_list); cudaFree(s->d_done_count); cudaFree(s->d_eval_outcome); cudaFree(s->d_eval_return);
     if (s->ev) { for (cudaEvent_t e : *s->ev) cudaEventDestroy(e); delete s->ev; delete s->ev_kind; }
     cudaFree(s->stg_states); cudaFree(s->stg_actions); cudaFree(s->stg_ranges); cudaFree(s->stg_gobs);
@@ -684,6 +706,47 @@ static int launch_features(fn_sim* s, const int* list, const int* count_dev, boo
     return FN_OK;
 }
 
+static ResetArgs reset_args(fn_sim* s, float* states, const int* list, const int* count, const int* list_par_dev,
+                            const uint64_t* seeds, float* out_goal_obs) {
+    ResetArgs a;
+    a.map = s->map->dev; a.robot = robot_dev(s->robot, s->map); a.task = task_dev(s->task);
+    a.regions.rects = s->map->d_regions; a.regions.n = s->map->n_regions;
+    a.n = s->n; a.states = states; a.list = list; a.count_dev = count;
+    a.list_par_dev = list_par_dev;
+    a.seeds = reinterpret_cast<const unsigned long long*>(seeds); a.out_goal_obs = out_goal_obs;
+    a.d_prev = s->d_dprev; a.ep_step = s->d_epstep; a.poses = s->d_poses;
+    a.ring = s->ring; a.ring_cap = s->ring_cap ? s->ring_cap : 1; a.ring_head_dev = s->d_ring_head; a.ring_row = ring_row_floats(s);
+    a.counters = s->d_counters; a.beam_task_counter = s->d_task_counter;
+    a.fail_out = nullptr;
+    return a;
+}
+
+// PAPER.md:84 "only the corresponding environments are reset and their observations recomputed": the reset itself (a
+// chain of dependent map reads per env, ~10 us) does not depend on the step, only on the seeds -- announced before
+// fn_step, it runs on the step kernel's outcome warps for the envs they report done, under the beam casting.
+extern "C" int fn_sim_prepare_reset(fn_sim* s, const uint64_t* seeds) {
+    if (!s) return fail(FN_ERR_INVALID_ARG, "fn_sim_prepare_reset: NULL sim");
+    s->prep_next = nullptr;
+    if (!seeds || !s->prep_ok) return FN_OK;                       // (a hint: fn_reset gives the same result without it)
+    if (!s->d_prep.states) {
+        const size_t n = (size_t)s->n;
+        cudaError_t e = cudaMalloc(&s->d_prep.states, 8 * n * sizeof(float));
+        if (e == cudaSuccess) e = cudaMalloc(&s->d_prep.goal_obs, 2 * n * sizeof(float));
+        if (e == cudaSuccess) e = cudaMalloc(&s->d_prep.d_prev, n * sizeof(float));
+        if (e == cudaSuccess) e = cudaMalloc(&s->d_prep.poses, n * sizeof(BeamPose));
+        if (e == cudaSuccess) e = cudaMalloc(&s->d_prep.fail, n);
+        if (e == cudaSuccess) e = cudaMalloc(&s->d_prep_epstep, n * sizeof(int));
+        if (e != cudaSuccess) {
+            cudaFree(s->d_prep.states); cudaFree(s->d_prep.goal_obs); cudaFree(s->d_prep.d_prev); cudaFree(s->d_prep.poses);
+            cudaFree(s->d_prep.fail); cudaFree(s->d_prep_epstep);
+            s->d_prep = PreparedReset{}; s->d_prep_epstep = nullptr;
+            return fail(e == cudaErrorMemoryAllocation ? FN_ERR_OOM : FN_ERR_CUDA, "fn_sim_prepare_reset: %s", cudaGetErrorString(e));
+        }
+    }
+    s->prep_next = seeds;
+    return FN_OK;
+}
+
 extern "C" int fn_step(fn_sim* s, float* states, const float* actions, float dt, uint8_t* reset_mask,
                        float* out_ranges, uint8_t* out_collision, float* out_goal_obs) {
     if (!s || !states || !actions || !reset_mask || !out_ranges || !out_collision || !out_goal_obs)
@@ -713,6 +776,12 @@ extern "C" int fn_step(fn_sim* s, float* states, const float* actions, float dt,
     }
     a.epw = s->n >= 32768 ? 32 : (s->n >= 8192 ? 16 : 8);
     int rc = FN_OK;
+    // announced seeds serve this step only; they are used when the production split step runs (no instruments, no
+    // coarse level, training mode) and dropped otherwise -- fn_reset does the whole reset then, with the same result
+    const uint64_t* prep_seeds = s->prep_next;
+    s->prep_next = s->prep_ready = nullptr;
+    if (!(s->prep_ok && s->split_on && !s->eval_mode && !s->count_words && !s->aux_hit && !(s->coarse_on && s->split_ok_c)))
+        prep_seeds = nullptr;
     if (s->split_on) {
         // motion kernel, then the beam kernel whose last warps run collision / goal / reward / done for the
         // envs their CTAs own and whose last CTA advances the ring and the done-list parity (fn_step_split.cuh)
@@ -726,13 +795,20 @@ extern "C" int fn_step(fn_sim* s, float* states, const float* actions, float dt,
         if (s->coarse_on && s->split_ok_c && !aux) {
             const int epc_c = (s->n + s->split_grid_c - 1) / s->split_grid_c;
             FN_CUDA(launch_pdl(step_beam_kernel<true, false, true>, dim3(s->split_grid_c), dim3(1024), s->split_smem_c, s->stream, b, a,
-                               s->d_step_end, epc_c, (unsigned)s->beam_smem_c));
+                               s->d_step_end, epc_c, (unsigned)s->beam_smem_c, 0));
         } else if (s->use_smem) {
-            if (aux) FN_CUDA(launch_pdl(step_beam_kernel<true, true>, grid, block, s->split_smem, s->stream, b, a, s->d_step_end, epc, bs));
-            else FN_CUDA(launch_pdl(step_beam_kernel<true, false>, grid, block, s->split_smem, s->stream, b, a, s->d_step_end, epc, bs));
+            if (aux) FN_CUDA(launch_pdl(step_beam_kernel<true, true>, grid, block, s->split_smem, s->stream, b, a, s->d_step_end, epc, bs, 0));
+            else if (prep_seeds) {
+                // the resets of the envs this step reports done, prepared under the beam casting (fn_sim_prepare_reset)
+                ResetArgs ra = reset_args(s, s->d_prep.states, nullptr, nullptr, nullptr, prep_seeds, s->d_prep.goal_obs);
+                ra.d_prev = s->d_prep.d_prev; ra.ep_step = s->d_prep_epstep; ra.poses = s->d_prep.poses; ra.ring = nullptr;
+                ra.fail_out = s->d_prep.fail;
+                FN_CUDA(launch_pdl(step_beam_kernel<true, false, false, true>, grid, block, s->split_smem, s->stream, b, a, s->d_step_end, epc, bs, ra));
+                s->prep_ready = prep_seeds; s->prep_map_ver = s->map->version; s->prep_robot_ver = s->robot->version;
+            } else FN_CUDA(launch_pdl(step_beam_kernel<true, false>, grid, block, s->split_smem, s->stream, b, a, s->d_step_end, epc, bs, 0));
         } else {
-            if (aux) FN_CUDA(launch_pdl(step_beam_kernel<false, true>, grid, block, s->split_smem, s->stream, b, a, s->d_step_end, epc, bs));
-            else FN_CUDA(launch_pdl(step_beam_kernel<false, false>, grid, block, s->split_smem, s->stream, b, a, s->d_step_end, epc, bs));
+            if (aux) FN_CUDA(launch_pdl(step_beam_kernel<false, true>, grid, block, s->split_smem, s->stream, b, a, s->d_step_end, epc, bs, 0));
+            else FN_CUDA(launch_pdl(step_beam_kernel<false, false>, grid, block, s->split_smem, s->stream, b, a, s->d_step_end, epc, bs, 0));
         }
     } else {
         FN_CUDA(launch_pdl(env_step_kernel, dim3((s->n + a.epw - 1) / a.epw), dim3(kEnvBlock), col_scratch_bytes(s->robot->V), s->stream, a));
@@ -766,16 +842,11 @@ extern "C" int fn_reset(fn_sim* s, float* states, const uint8_t* mask, const uin
     }
     if (mask) FN_CUDA(launch_pdl(compact_mask_kernel, dim3(1), dim3(1024), 0, s->stream, mask, s->n, s->d_list, s->d_count));
     if (s->prof) FN_CUDA(cudaEventRecord(e1, s->stream));
-    ResetArgs a;
-    a.map = s->map->dev; a.robot = robot_dev(s->robot, s->map); a.task = task_dev(s->task);
-    a.regions.rects = s->map->d_regions; a.regions.n = s->map->n_regions;
-    a.n = s->n; a.states = states; a.list = list; a.count_dev = count;
-    a.list_par_dev = mask ? nullptr : s->d_done_count + 2;
-    a.seeds = reinterpret_cast<const unsigned long long*>(seeds); a.out_goal_obs = out_goal_obs;
-    a.d_prev = s->d_dprev; a.ep_step = s->d_epstep; a.poses = s->d_poses;
-    a.ring = s->ring; a.ring_cap = s->ring_cap ? s->ring_cap : 1; a.ring_head_dev = s->d_ring_head; a.ring_row = ring_row_floats(s);
-    a.counters = s->d_counters; a.beam_task_counter = s->d_task_counter;
+    const ResetArgs a = reset_args(s, states, list, count, mask ? nullptr : s->d_done_count + 2, seeds, out_goal_obs);
     int rc = FN_OK;
+    // a reset prepared by the preceding fn_step for exactly this call (same seeds, nothing changed since)?
+    const bool prepared = !mask && s->prep_ready == seeds && s->prep_map_ver == s->map->version && s->prep_robot_ver == s->robot->version;
+    s->prep_ready = nullptr;
     // A CTA of the fused kernel runs its resets on kFusedResetWarps warps and casts only its own envs' beams:
     // made for the few envs a step reports done (C2, ~190 of 4096: 2-4 us faster than the two kernels).  For
     // long lists the two throughput-oriented kernels win (C2: all 4096 envs 83 against 121 us, a quarter of
@@ -787,8 +858,9 @@ extern "C" int fn_reset(fn_sim* s, float* states, const uint8_t* mask, const uin
         // the beams of those envs (fn_reset_beam.cuh)
         BeamArgs b = beam_args(s, list, count, out_ranges, false, mask == nullptr);
         const bool aux = s->count_words || s->aux_hit;
-        if (aux) FN_CUDA(launch_pdl(reset_beam_kernel<true>, dim3(s->fused_grid), dim3(kFusedThreads), s->fused_smem, s->stream, a, b));
-        else FN_CUDA(launch_pdl(reset_beam_kernel<false>, dim3(s->fused_grid), dim3(kFusedThreads), s->fused_smem, s->stream, a, b));
+        const PreparedReset pr = prepared ? s->d_prep : PreparedReset{};
+        if (aux) FN_CUDA(launch_pdl(reset_beam_kernel<true>, dim3(s->fused_grid), dim3(kFusedThreads), s->fused_smem, s->stream, a, b, pr));
+        else FN_CUDA(launch_pdl(reset_beam_kernel<false>, dim3(s->fused_grid), dim3(kFusedThreads), s->fused_smem, s->stream, a, b, pr));
         if (s->prof) { FN_CUDA(cudaEventRecord(e2, s->stream)); FN_CUDA(cudaEventRecord(e3, s->stream)); }
     } else {
         int grid = (s->n + kResetWarps - 1) / kResetWarps;
@@ -852,6 +924,7 @@ extern "C" int fn_eval_begin(fn_sim* s, float* states, int n_cases, int step_lim
     eval_begin_kernel<<<(s->n + 255) / 256, 256, 0, s->stream>>>(a);
     FN_CUDA(cudaGetLastError());
     s->eval_mode = 1; s->eval_limit = step_limit; s->done_avail = 0;
+    s->prep_next = s->prep_ready = nullptr;
     float* ring = s->ring;           // evaluation never touches the replay ring
     s->ring = nullptr;
     int st = launch_beams(s, nullptr, nullptr, out_ranges);

@@ -9,7 +9,7 @@ namespace fn {
 constexpr int kMaxVerts = 64;
 constexpr int kMaxAttempts = 256;
 constexpr int kNCounters = 8;
-enum Counter { kRays = 0, kWords = 1, kResets = 2, kResetFail = 3, kNonFinite = 4, kEnvSteps = 5, kOobLoads = 6 };
+enum Counter { kRays = 0, kWords = 1, kResets = 2, kResetFail = 3, kNonFinite = 4, kEnvSteps = 5, kOobLoads = 6, kResetsPrepared = 7 };
 
 // Bit-packed map, two orientations.  A "line" is one row of the row-packed copy (bits run along
 // columns) or one column of the column-packed copy (bits run along rows).  "Outside the map is

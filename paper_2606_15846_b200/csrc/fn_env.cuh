@@ -387,8 +387,9 @@ __device__ __forceinline__ EnvMotion env_motion_load(const EnvArgs& a, const int
 // with row / col pointing at a shared-memory copy (kS = true).  ring_head = slot of env 0's row of THIS step.
 // store_motion: also write the motion's results (the single-kernel env step); false when an earlier kernel
 // stored them (split step).
+// Returns the ballot of the lanes whose env reports done.
 template <bool kS>
-__device__ __forceinline__ void env_outcome(const EnvArgs& a, const MapDev& m, const ColScratch& scratch, const int e,
+__device__ __forceinline__ unsigned env_outcome(const EnvArgs& a, const MapDev& m, const ColScratch& scratch, const int e,
                                             const int el, const bool in_range, const int lane, const EnvMotion& mo,
                                             const unsigned long long ring_head, const bool store_motion) {
     const int n = a.n;
@@ -429,7 +430,7 @@ __device__ __forceinline__ void env_outcome(const EnvArgs& a, const MapDev& m, c
         a.reset_mask[e] = 0;
         if (a.out_reward) a.out_reward[e] = 0.0f;
     }
-    if (!live) return;
+    if (!live) return dm;
     if (a.eval_outcome) {                                          // each case is recorded once
         a.eval_return[e] += r;
         if (done) a.eval_outcome[e] = col ? 2 : reached ? 1 : 3;
@@ -453,6 +454,7 @@ __device__ __forceinline__ void env_outcome(const EnvArgs& a, const MapDev& m, c
         float* nxt = a.ring + ((head + (unsigned long long)n + (unsigned long long)e) % a.ring_cap) * (size_t)a.ring_row;
         nxt[B] = d; nxt[B + 1] = alpha; nxt[B + 2] = avx; nxt[B + 3] = avy; nxt[B + 4] = aw;
     }
+    return dm;
 }
 
 __global__ void __launch_bounds__(kEnvBlock) env_step_kernel(EnvArgs a) {
@@ -584,6 +586,18 @@ struct ResetArgs {
     int ring_row;
     unsigned* beam_task_counter; // zeroed here for the beam kernel that follows
     unsigned long long* counters;
+    uint8_t* fail_out;           // or NULL; else [n]: "no attempt was accepted" is stored here instead of counted
+};
+
+// A reset prepared ahead of fn_reset (fn_sim_prepare_reset): the step's outcome warps run reset_env for the envs
+// they report done, with ResetArgs that point here instead of at the caller's arrays; fn_reset(mask = NULL) then
+// only copies (reset_apply) and casts the beams.  Same layouts as the arrays they stand for.
+struct PreparedReset {
+    float* states;               // [8][n], NULL = nothing prepared
+    float* goal_obs;             // [2][n]
+    float* d_prev;               // [n]
+    BeamPose* poses;             // [n]
+    uint8_t* fail;               // [n]
 };
 
 constexpr int kResetWarps = 4;
@@ -685,9 +699,35 @@ __device__ __forceinline__ void reset_env(const ResetArgs& a, const MapDev& mp, 
             const int B = a.robot.B;
             row[B] = d; row[B + 1] = alpha; row[B + 2] = 0.f; row[B + 3] = 0.f; row[B + 4] = 0.f;
         }
-        atomicAdd(&a.counters[kResets], 1ull);
-        if (fail) atomicAdd(&a.counters[kResetFail], 1ull);
+        if (a.fail_out) a.fail_out[e] = fail ? 1 : 0;            // (prepared ahead: counted when it is applied)
+        else {
+            atomicAdd(&a.counters[kResets], 1ull);
+            if (fail) atomicAdd(&a.counters[kResetFail], 1ull);
+        }
     }
+}
+
+// The stores of reset_env for env e from a prepared reset (one thread): a = the arguments of the fn_reset call.
+__device__ __forceinline__ void reset_apply(const ResetArgs& a, const PreparedReset& pr, const int e, BeamPose* pose_copy = nullptr) {
+    const int n = a.n;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) a.states[k * n + e] = pr.states[k * n + e];
+    const float d = pr.goal_obs[e], alpha = pr.goal_obs[n + e];
+    a.d_prev[e] = pr.d_prev[e];
+    a.ep_step[e] = 0;
+    if (a.out_goal_obs) { a.out_goal_obs[e] = d; a.out_goal_obs[n + e] = alpha; }
+    const BeamPose bp = pr.poses[e];
+    a.poses[e] = bp;
+    if (pose_copy) *pose_copy = bp;
+    if (a.ring) {
+        const unsigned long long head = *a.ring_head_dev;
+        float* row = a.ring + ((head + (unsigned long long)e) % a.ring_cap) * (size_t)a.ring_row;
+        const int B = a.robot.B;
+        row[B] = d; row[B + 1] = alpha; row[B + 2] = 0.f; row[B + 3] = 0.f; row[B + 4] = 0.f;
+    }
+    atomicAdd(&a.counters[kResets], 1ull);
+    atomicAdd(&a.counters[kResetsPrepared], 1ull);
+    if (pr.fail[e]) atomicAdd(&a.counters[kResetFail], 1ull);
 }
 
 __global__ void __launch_bounds__(kResetWarps * 32) reset_kernel(ResetArgs a) {

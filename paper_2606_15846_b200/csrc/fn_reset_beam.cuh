@@ -11,6 +11,9 @@
 // only synchronisation.  Used for fn_reset(mask = NULL), the step's done list, when the map is staged in
 // shared memory; a caller's mask (long lists: two reset warps per CTA and no balancing of the beams across
 // CTAs lose there) and maps read through L2 take the two kernels.
+// With a reset prepared by the step before (fn_sim_prepare_reset; pr.states != NULL) phase 1 only copies the
+// prepared states, goal observations and poses: the ~10 us chain of the attempts has already run on the step
+// kernel's outcome warps, under the beam casting.
 #pragma once
 #include "fn_beam.cuh"
 #include "fn_env.cuh"
@@ -29,7 +32,7 @@ __host__ __device__ inline size_t fused_smem_bytes(int B, int mapWords, int V) {
 }
 
 template <bool kAux>
-__global__ void __launch_bounds__(kFusedThreads, 2) reset_beam_kernel(const __grid_constant__ ResetArgs ra, const __grid_constant__ BeamArgs a) {
+__global__ void __launch_bounds__(kFusedThreads, 2) reset_beam_kernel(const __grid_constant__ ResetArgs ra, const __grid_constant__ BeamArgs a, const PreparedReset pr) {
     extern __shared__ __align__(16) uint8_t smem_raw[];
     const int B = a.robot.B, V = a.robot.V;
     const int rowWords = (a.map.H + 2 * kLineGuard) * a.map.strideR;
@@ -61,8 +64,13 @@ __global__ void __launch_bounds__(kFusedThreads, 2) reset_beam_kernel(const __gr
         MapDev ms = ra.map;
         ms.row = s_map;
         ms.col = s_map + rowWords;
-        for (int k = wib; k < m_loc; k += kFusedResetWarps)
-            reset_env<true>(ra, ms, scratch, rlist[blockIdx.x + k * gridDim.x], lane, k < kFusedPoseSlots ? s_pose + k : nullptr);
+        if (pr.states) {                                           // prepared by the step (fn_sim_prepare_reset): copy only
+            for (int k = wib * 32 + lane; k < m_loc; k += kFusedResetWarps * 32)
+                reset_apply(ra, pr, rlist[blockIdx.x + k * gridDim.x], k < kFusedPoseSlots ? s_pose + k : nullptr);
+        } else {
+            for (int k = wib; k < m_loc; k += kFusedResetWarps)
+                reset_env<true>(ra, ms, scratch, rlist[blockIdx.x + k * gridDim.x], lane, k < kFusedPoseSlots ? s_pose + k : nullptr);
+        }
         __threadfence_block();                                     // poses: written here, read below by all warps
     }
     __syncthreads();

@@ -40,8 +40,11 @@ __host__ __device__ inline size_t step_split_smem_bytes(size_t beam_smem, int V)
 }
 
 // beam_smem = the beam kernel's dynamic shared bytes (beam table [+ packed map]); epc = envs owned per CTA
-template <bool kSmem, bool kAux, bool kCoarse = false>
-__global__ void __launch_bounds__(FastShape<kCoarse>::kThreads, FastShape<kCoarse>::kCtas) step_beam_kernel(const __grid_constant__ BeamArgs a, const __grid_constant__ EnvArgs ea, StepEnd* end, int epc, unsigned beam_smem) {
+// kPrep: the outcome warp also runs the reset (reset_env, the code of fn_reset) of every env it reports done, into
+// the buffers ra points at (fn_sim_prepare_reset): that chain of dependent map reads then runs under the beam
+// casting of the other warps instead of after the step.
+template <bool kSmem, bool kAux, bool kCoarse = false, bool kPrep = false>
+__global__ void __launch_bounds__(FastShape<kCoarse>::kThreads, FastShape<kCoarse>::kCtas) step_beam_kernel(const __grid_constant__ BeamArgs a, const __grid_constant__ EnvArgs ea, StepEnd* end, int epc, unsigned beam_smem, const __grid_constant__ typename std::conditional<kPrep, ResetArgs, int>::type ra) {
     extern __shared__ __align__(16) uint8_t smem_raw[];
     const int B = a.robot.B, V = a.robot.V;
     const int rowWords = (a.map.H + 2 * kLineGuard) * a.map.strideR;
@@ -76,7 +79,10 @@ __global__ void __launch_bounds__(FastShape<kCoarse>::kThreads, FastShape<kCoars
             const bool in_range = base + lane < m_own;
             const int el = in_range ? e : n - 1;
             const EnvMotion mo = env_motion_load(ea, el);
-            env_outcome<kSmem>(ea, ms, scratch, e, el, in_range, lane, mo, head_old, false);
+            unsigned dm = env_outcome<kSmem>(ea, ms, scratch, e, el, in_range, lane, mo, head_old, false);
+            if constexpr (kPrep) {
+                for (; dm; dm &= dm - 1u) reset_env<kSmem>(ra, ms, scratch, e0 + base + (__ffs(dm) - 1), lane);
+            } else (void)dm;
         }
     }
 

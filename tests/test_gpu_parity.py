@@ -709,6 +709,72 @@ def test_coarse_level_on_and_off_give_identical_results(pu):
         assert out[0][1] == out[1][1]
 
 
+def test_prepared_reset_equals_the_plain_reset(pu):
+    # fn_sim_prepare_reset: with the seeds announced, the step's outcome warps run the reset of the envs
+    # they report done and fn_reset(mask = NULL) only copies and recomputes the observations.  The plain path is the
+    # one the parity tests hold against the oracle; here both paths give the same states, flags, ranges, goal
+    # observations, episode counters, ring and counters, bit for bit, step by step -- at C2's full batch (several done
+    # envs per CTA), with forced resets, a union footprint with a sensor offset (C3), regions (C5's map is read through
+    # L2: the announcement is dropped there), a ring, and with announcements that must NOT be used (other seeds, a
+    # mask, a setter in between).
+    import torch
+    from harness import workloads as W
+    for cfg, n, steps, with_ring in ((2, 4096, 40, False), (3, 1500, 12, True), (1, 64, 40, True), (5, 512, 6, False)):
+        wl = W.make_workload(cfg, n_envs=n)
+        wl.forced_reset_frac = 0.03
+        B, A = wl.n_beams, wl.action_dim
+        actions = torch.from_numpy(W.action_tape(wl, steps, 5)).cuda()
+        seeds = torch.from_numpy(W.seed_tape(wl, steps + 2, 5).view(np.int64)).cuda()
+        forced = torch.from_numpy(W.forced_reset_tape(wl, steps, 5)).cuda()
+        out = []
+        for prepare in (True, False):
+            m, r, s = pu.make_sim(wl, n)
+            if cfg == 3:
+                r.set_sensor(0.1, -0.05, 0.2)
+            buf = pu.Buffers(n, B, A)
+            s.bind_aux(None, buf.reward)
+            ring = None
+            if with_ring:
+                cap = 3 * n + 11
+                ring = torch.zeros(cap * s.ring_row_floats(), device="cuda")
+                s.ring_attach(ring, cap)
+            buf.mask.fill_(1)
+            s.reset(buf.states, buf.mask, seeds[0], buf.ranges, buf.gobs)
+            trace = []
+            for t in range(steps):
+                buf.mask.copy_(forced[t])
+                odd = t % 7 == 3                                  # an announcement that fn_reset must not use
+                if prepare:
+                    s.prepare_reset(seeds[steps + 1] if odd and t % 14 == 3 else seeds[t + 1])
+                s.step(buf.states, actions[t], float(wl.dt), buf.mask, buf.ranges, buf.col, buf.gobs)
+                trace += [buf.states.clone(), buf.ranges.clone(), buf.gobs.clone(), buf.mask.clone(), buf.col.clone(), buf.reward.clone()]
+                if odd and t % 14 == 10:
+                    r.set_sensor(*((0.1, -0.05, 0.2) if cfg == 3 else (0.0, 0.0, 0.0)))     # same values, new version
+                s.reset(buf.states, None, seeds[t + 1], buf.ranges, buf.gobs)
+                dp, ep = s.episode_state()
+                trace += [buf.states.clone(), buf.ranges.clone(), buf.gobs.clone(), torch.from_numpy(dp), torch.from_numpy(ep)]
+                if t % 5 == 4:                                    # the poses the reset left behind serve later launches
+                    full = torch.empty_like(buf.ranges)
+                    s.observe_all(buf.states, full)
+                    trace.append(full)
+            torch.cuda.synchronize()
+            if ring is not None:
+                trace.append(ring.clone())
+            out.append((trace, s.counters()))
+            s.close(); r.close(); m.close()
+        for k, (a, b) in enumerate(zip(out[0][0], out[1][0])):
+            assert torch.equal(a, b), f"config {cfg}: item {k} differs with the reset prepared by the step"
+        c1, c0 = dict(out[0][1]), dict(out[1][1])
+        used = c1.pop("resets_prepared")
+        assert c0.pop("resets_prepared") == 0
+        assert c1 == c0, (c1, c0)
+        assert c1["envs_reset"] > n + steps // 2
+        if cfg == 5:
+            assert used == 0                                      # (map read through L2: no such kernel)
+        else:
+            assert 0.5 * (c1["envs_reset"] - n) <= used < c1["envs_reset"] - n, (used, c1)
+
+
 def test_clearance_features_against_the_oracle(pu):
     # NEXT-1 (Eq. (3)): sector-pooled footprint clearances.  Teacher-forced:
     # the oracle computes them in fp64 from the GPU's own fp32 ranges; tolerance 1e-4 m like the ranges

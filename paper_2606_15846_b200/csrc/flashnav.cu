@@ -121,6 +121,7 @@ struct fn_sim {
     // kernels exist for this sim); prep_next = the seeds announced for the coming fn_step, prep_ready = the seeds the
     // buffers were filled with by the last fn_step (with the map / robot versions they were filled under)
     bool prep_ok;
+    int prep_grid;
     const uint64_t *prep_next, *prep_ready;
     unsigned prep_map_ver, prep_robot_ver;
     PreparedReset d_prep;
@@ -550,11 +551,14 @@ extern "C" int fn_sim_create(const fn_map* map, const fn_robot* robot, int n, co
                 s->split_on = (n + s->split_grid - 1) / s->split_grid <= 64;
             }
             // ... and its variant that prepares the resets (served by the fused reset kernel)
+            // (its fn_reset is prepared_reset_kernel: the production beam kernel's shape)
             s->prep_ok = false;
-            if (e == cudaSuccess && s->split_ok && s->use_smem && s->fused_ok) {
-                int fp = 0;
+            if (e == cudaSuccess && s->split_ok && s->use_smem) {
+                int fp = 0, fq = 0;
                 e = kernel_config(step_beam_kernel<true, false, false, true>, kBeamThreads, s->split_smem, max_optin, &fp);
-                s->prep_ok = e == cudaSuccess && s->num_sms * fp >= s->split_grid;
+                if (e == cudaSuccess) e = kernel_config(prepared_reset_kernel, kBeamThreads, s->beam_smem, max_optin, &fq);
+                s->prep_ok = e == cudaSuccess && s->num_sms * fp >= s->split_grid && fq >= 1;
+                s->prep_grid = s->num_sms * fq;
             }
         }
         // the coarse level: fine + coarse copies staged by one CTA of 1024 threads per SM
@@ -845,7 +849,8 @@ extern "C" int fn_reset(fn_sim* s, float* states, const uint8_t* mask, const uin
     const ResetArgs a = reset_args(s, states, list, count, mask ? nullptr : s->d_done_count + 2, seeds, out_goal_obs);
     int rc = FN_OK;
     // a reset prepared by the preceding fn_step for exactly this call (same seeds, nothing changed since)?
-    const bool prepared = !mask && s->prep_ready == seeds && s->prep_map_ver == s->map->version && s->prep_robot_ver == s->robot->version;
+    const bool prepared = !mask && s->prep_ready == seeds && s->prep_map_ver == s->map->version && s->prep_robot_ver == s->robot->version &&
+                          !s->count_words && !s->aux_hit;
     s->prep_ready = nullptr;
     // A CTA of the fused kernel runs its resets on kFusedResetWarps warps and casts only its own envs' beams:
     // made for the few envs a step reports done (C2, ~190 of 4096: 2-4 us faster than the two kernels).  For
@@ -853,14 +858,19 @@ extern "C" int fn_reset(fn_sim* s, float* states, const uint8_t* mask, const uin
     // them 38 against 47 us), and a caller's mask is usually such a list (the first reset of all envs), so
     // the fused kernel serves fn_reset(mask = NULL) only -- unless forced (enable = 2, tests).
     const bool fused = s->fused_on && (!mask || s->fused_force);
-    if (fused) {
+    if (prepared) {
+        // one launch: copies of the prepared states and the beams of the listed envs, every warp of the grid taking rounds
+        BeamArgs b = beam_args(s, list, count, out_ranges, false, true);
+        b.poses = s->d_prep.poses;
+        FN_CUDA(launch_pdl(prepared_reset_kernel, dim3(s->prep_grid), dim3(kBeamThreads), s->beam_smem, s->stream, a, b, s->d_prep));
+        if (s->prof) { FN_CUDA(cudaEventRecord(e2, s->stream)); FN_CUDA(cudaEventRecord(e3, s->stream)); }
+    } else if (fused) {
         // one launch: every CTA resets its share of the list from its shared copy of the map, then casts
         // the beams of those envs (fn_reset_beam.cuh)
         BeamArgs b = beam_args(s, list, count, out_ranges, false, mask == nullptr);
         const bool aux = s->count_words || s->aux_hit;
-        const PreparedReset pr = prepared ? s->d_prep : PreparedReset{};
-        if (aux) FN_CUDA(launch_pdl(reset_beam_kernel<true>, dim3(s->fused_grid), dim3(kFusedThreads), s->fused_smem, s->stream, a, b, pr));
-        else FN_CUDA(launch_pdl(reset_beam_kernel<false>, dim3(s->fused_grid), dim3(kFusedThreads), s->fused_smem, s->stream, a, b, pr));
+        if (aux) FN_CUDA(launch_pdl(reset_beam_kernel<true>, dim3(s->fused_grid), dim3(kFusedThreads), s->fused_smem, s->stream, a, b));
+        else FN_CUDA(launch_pdl(reset_beam_kernel<false>, dim3(s->fused_grid), dim3(kFusedThreads), s->fused_smem, s->stream, a, b));
         if (s->prof) { FN_CUDA(cudaEventRecord(e2, s->stream)); FN_CUDA(cudaEventRecord(e3, s->stream)); }
     } else {
         int grid = (s->n + kResetWarps - 1) / kResetWarps;

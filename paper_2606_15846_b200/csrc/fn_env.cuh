@@ -708,7 +708,7 @@ __device__ __forceinline__ void reset_env(const ResetArgs& a, const MapDev& mp, 
 }
 
 // The stores of reset_env for env e from a prepared reset (one thread): a = the arguments of the fn_reset call.
-__device__ __forceinline__ void reset_apply(const ResetArgs& a, const PreparedReset& pr, const int e, BeamPose* pose_copy = nullptr) {
+__device__ __forceinline__ void reset_apply(const ResetArgs& a, const PreparedReset& pr, const int e) {
     const int n = a.n;
 #pragma unroll
     for (int k = 0; k < 8; ++k) a.states[k * n + e] = pr.states[k * n + e];
@@ -718,7 +718,6 @@ __device__ __forceinline__ void reset_apply(const ResetArgs& a, const PreparedRe
     if (a.out_goal_obs) { a.out_goal_obs[e] = d; a.out_goal_obs[n + e] = alpha; }
     const BeamPose bp = pr.poses[e];
     a.poses[e] = bp;
-    if (pose_copy) *pose_copy = bp;
     if (a.ring) {
         const unsigned long long head = *a.ring_head_dev;
         float* row = a.ring + ((head + (unsigned long long)e) % a.ring_cap) * (size_t)a.ring_row;

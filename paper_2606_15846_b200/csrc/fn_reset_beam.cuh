@@ -11,9 +11,7 @@
 // only synchronisation.  Used for fn_reset(mask = NULL), the step's done list, when the map is staged in
 // shared memory; a caller's mask (long lists: two reset warps per CTA and no balancing of the beams across
 // CTAs lose there) and maps read through L2 take the two kernels.
-// With a reset prepared by the step before (fn_sim_prepare_reset; pr.states != NULL) phase 1 only copies the
-// prepared states, goal observations and poses: the ~10 us chain of the attempts has already run on the step
-// kernel's outcome warps, under the beam casting.
+// A reset prepared by the step before (fn_sim_prepare_reset) takes prepared_reset_kernel below instead.
 #pragma once
 #include "fn_beam.cuh"
 #include "fn_env.cuh"
@@ -32,7 +30,7 @@ __host__ __device__ inline size_t fused_smem_bytes(int B, int mapWords, int V) {
 }
 
 template <bool kAux>
-__global__ void __launch_bounds__(kFusedThreads, 2) reset_beam_kernel(const __grid_constant__ ResetArgs ra, const __grid_constant__ BeamArgs a, const PreparedReset pr) {
+__global__ void __launch_bounds__(kFusedThreads, 2) reset_beam_kernel(const __grid_constant__ ResetArgs ra, const __grid_constant__ BeamArgs a) {
     extern __shared__ __align__(16) uint8_t smem_raw[];
     const int B = a.robot.B, V = a.robot.V;
     const int rowWords = (a.map.H + 2 * kLineGuard) * a.map.strideR;
@@ -64,13 +62,8 @@ __global__ void __launch_bounds__(kFusedThreads, 2) reset_beam_kernel(const __gr
         MapDev ms = ra.map;
         ms.row = s_map;
         ms.col = s_map + rowWords;
-        if (pr.states) {                                           // prepared by the step (fn_sim_prepare_reset): copy only
-            for (int k = wib * 32 + lane; k < m_loc; k += kFusedResetWarps * 32)
-                reset_apply(ra, pr, rlist[blockIdx.x + k * gridDim.x], k < kFusedPoseSlots ? s_pose + k : nullptr);
-        } else {
-            for (int k = wib; k < m_loc; k += kFusedResetWarps)
-                reset_env<true>(ra, ms, scratch, rlist[blockIdx.x + k * gridDim.x], lane, k < kFusedPoseSlots ? s_pose + k : nullptr);
-        }
+        for (int k = wib; k < m_loc; k += kFusedResetWarps)
+            reset_env<true>(ra, ms, scratch, rlist[blockIdx.x + k * gridDim.x], lane, k < kFusedPoseSlots ? s_pose + k : nullptr);
         __threadfence_block();                                     // poses: written here, read below by all warps
     }
     __syncthreads();
@@ -115,6 +108,46 @@ __global__ void __launch_bounds__(kFusedThreads, 2) reset_beam_kernel(const __gr
             if (a.count_words) atomicAdd(&a.counters[kWords], (unsigned long long)words);
         }
     }
+}
+
+// fn_reset(mask = NULL) after a step that prepared the resets (fn_sim_prepare_reset): the new states, goal
+// observations and sensing poses of the listed envs already sit in the sim's buffers (pr; a.poses = pr.poses), so
+// nothing here depends on anything but the list -- every warp of the grid takes rounds of 32 beams of the listed
+// envs (task t = round t % rounds of list entry t / rounds, dealt to the CTAs in turn so that the SMs share every
+// env's beams); the tasks after those copy the prepared states into the caller's arrays, 32 envs per warp
+// (reset_apply).  No reset warps, no block barrier between resetting and casting.
+__global__ void __launch_bounds__(kBeamThreads, 2) prepared_reset_kernel(const __grid_constant__ ResetArgs ra, const __grid_constant__ BeamArgs a,
+                                                                        const PreparedReset pr) {
+    extern __shared__ __align__(16) uint8_t smem_raw[];
+    const int B = a.robot.B;
+    const int mapWords = (a.map.H + 2 * kLineGuard) * a.map.strideR + (a.map.W + 2 * kLineGuard) * a.map.strideC;
+    double2* s_tab = reinterpret_cast<double2*>(smem_raw);
+    uint32_t* s_map = reinterpret_cast<uint32_t*>(smem_raw + (size_t)B * sizeof(double2));
+    __shared__ __align__(8) unsigned long long s_mbar;
+    __shared__ __align__(16) FastShared<kBeamThreads / 32> s_fast;
+    stage_beam_constants(a, s_tab, s_map, mapWords, true, &s_mbar);
+    __syncthreads();
+    griddep_wait();                                                // the list comes from the step
+    griddep_launch_dependents();
+    const int* rlist = ra.list;
+    const int* rcount = ra.count_dev;
+    if (ra.list_par_dev) { const int q = *ra.list_par_dev ^ 1; rlist += (size_t)q * ra.n; rcount += q; }
+    const unsigned count = (unsigned)*rcount;
+    const unsigned long long ring_head = a.ring_obs ? *a.ring_head : 0ull;
+    FastWarp w = fast_warp(a, &s_fast, s_tab, (uint32_t)__cvta_generic_to_shared(s_map));
+    const unsigned rounds = ((unsigned)B + 31u) >> 5, ntasks = count * rounds, nall = ntasks + ((count + 31u) >> 5);
+    const unsigned lane = threadIdx.x & 31, nwarps = gridDim.x * (blockDim.x >> 5);
+    for (unsigned task = blockIdx.x + gridDim.x * (threadIdx.x >> 5); task < nall; task += nwarps) {
+        if (task < ntasks) {
+            const unsigned k = a.inv_rounds ? __umulhi(task, a.inv_rounds) : task / rounds, jb0 = (task - k * rounds) << 5;
+            const unsigned e = (unsigned)rlist[k];
+            fast_chunk<false>(a, w, a.poses + e, e, jb0, min((unsigned)B, jb0 + 32u), ring_head);
+        } else {
+            const unsigned k = ((task - ntasks) << 5) + lane;
+            if (k < count) reset_apply(ra, pr, rlist[k]);
+        }
+    }
+    fast_finish(a, w, ring_head);
 }
 
 }  // namespace fn

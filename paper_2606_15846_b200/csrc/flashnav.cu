@@ -557,7 +557,10 @@ extern "C" int fn_sim_create(const fn_map* map, const fn_robot* robot, int n, co
                 int fp = 0, fq = 0;
                 e = kernel_config(step_beam_kernel<true, false, false, true>, kBeamThreads, s->split_smem, max_optin, &fp);
                 if (e == cudaSuccess) e = kernel_config(prepared_reset_kernel, kBeamThreads, s->beam_smem, max_optin, &fq);
-                s->prep_ok = e == cudaSuccess && s->num_sms * fp >= s->split_grid && fq >= 1;
+                // worth it when the beam casting lasts longer than the chain of a reset (~10 us; the outcome warp runs
+                // its resets one after the other): eight rounds of 32 beams per warp (C1's 64 envs: 33 -> 36 us per step)
+                const size_t rounds_all = (size_t)n * (((size_t)robot->B + 31) >> 5), warps_all = (size_t)s->split_grid * (kBeamThreads / 32);
+                s->prep_ok = e == cudaSuccess && s->num_sms * fp >= s->split_grid && fq >= 1 && rounds_all >= 8 * warps_all;
                 s->prep_grid = s->num_sms * fq;
             }
         }

@@ -792,7 +792,7 @@ extern "C" int fn_step(fn_sim* s, float* states, const float* actions, float dt,
     if (s->split_on) {
         // motion kernel, then the beam kernel whose last warps run collision / goal / reward / done for the
         // envs their CTAs own and whose last CTA advances the ring and the done-list parity (fn_step_split.cuh)
-        FN_CUDA(launch_pdl(env_motion_kernel, dim3((s->n + a.epw - 1) / a.epw), dim3(kEnvBlock), 0, s->stream, a));
+        FN_CUDA(launch_pdl(env_motion_kernel, dim3((s->n + a.epw - 1) / a.epw), dim3(kEnvBlock), 0, s->stream, a, s->d_step_end));
         if (s->prof) FN_CUDA(cudaEventRecord(e1, s->stream));
         const BeamArgs b = beam_args(s, nullptr, nullptr, out_ranges, false, false);
         const int epc = (s->n + s->split_grid - 1) / s->split_grid;
@@ -865,7 +865,8 @@ extern "C" int fn_reset(fn_sim* s, float* states, const uint8_t* mask, const uin
         // one launch: copies of the prepared states and the beams of the listed envs, every warp of the grid taking rounds
         BeamArgs b = beam_args(s, list, count, out_ranges, false, true);
         b.poses = s->d_prep.poses;
-        FN_CUDA(launch_pdl(prepared_reset_kernel, dim3(s->prep_grid), dim3(kBeamThreads), s->beam_smem, s->stream, a, b, s->d_prep));
+        FN_CUDA(launch_pdl(prepared_reset_kernel, dim3(s->prep_grid), dim3(kBeamThreads), s->beam_smem, s->stream, a, b, s->d_prep,
+                           (const StepEnd*)s->d_step_end, (unsigned)s->split_grid));
         if (s->prof) { FN_CUDA(cudaEventRecord(e2, s->stream)); FN_CUDA(cudaEventRecord(e3, s->stream)); }
     } else if (fused) {
         // one launch: every CTA resets its share of the list from its shared copy of the map, then casts
@@ -1216,3 +1217,4 @@ extern "C" int fn_step_host_end(fn_sim* s, int slot) {
     s->hslot[slot].busy = false;
     return FN_OK;
 }
+

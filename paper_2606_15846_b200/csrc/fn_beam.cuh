@@ -683,6 +683,64 @@ __device__ __forceinline__ void fast_rounds(const BeamArgs& a, FastWarp& w, cons
         }
     }
 }
+// a near-axis beam cast on the spot (all lanes call; `mine` = this lane has one): fast_drain's cast for one beam
+template <bool kCg>
+__device__ __noinline__ float fast_near_beam(const BeamArgs& a, const FastWarp& w, const BeamPose* pose, const unsigned j, const bool mine, float r) {
+    if (mine) {
+        BeamMap<SmemSpace> bm;
+        const int mapWords = (a.map.H + 2 * kLineGuard) * a.map.strideR + (a.map.W + 2 * kLineGuard) * a.map.strideC;
+        bm.base = w.map_base; bm.H = a.map.H; bm.W = a.map.W; bm.stride4R = a.map.strideR << 2; bm.stride4C = a.map.strideC << 2;
+        bm.rowBytes = (unsigned)(a.map.H + 2 * kLineGuard) * (unsigned)(a.map.strideR << 2);
+        bm.mapBytes = (unsigned)mapWords * 4u; bm.oob = nullptr;
+        BeamPose lp;
+        const uint4* src = reinterpret_cast<const uint4*>(pose);
+#pragma unroll
+        for (int k = 0; k < (int)(sizeof(BeamPose) / 16); ++k) reinterpret_cast<uint4*>(&lp)[k] = kCg ? __ldcg(src + k) : src[k];
+        int hit;
+        uint32_t words = 0;
+        r = cast_beam<SmemSpace, false>(bm, &lp, lds_d2(w.tab + 16u * j), a.robot.T, a.map.rho, a.robot.rmax, &hit, words);
+    }
+    __syncwarp();
+    return r;
+}
+// One round of env e (beams jb0 .. jb0 + 31) with the results HELD BACK in registers, for a kernel that may cast
+// before it may write (prepared_reset_kernel): fast_store_held stores them.  Near-axis beams are cast on the spot by
+// cast_beam (the call fast_drain makes for them) instead of being queued: that kernel's warps cast a round or two
+// each, so a queue would be drained one or two beams at a time, a second pass as long as the round.
+// kCg: the pose is read past L1 (written by a kernel that may still be running).
+struct HeldRound {
+    float r;
+    unsigned e, j;
+    bool store;
+};
+template <bool kCg>
+__device__ __forceinline__ HeldRound fast_round_held(const BeamArgs& a, FastWarp& w, const BeamPose* pose, const unsigned e, const unsigned jb0) {
+    const unsigned lane = threadIdx.x & 31;
+    const unsigned B = (unsigned)a.robot.B;
+    __syncwarp();
+    if (lane < 3) {
+        const uint4* src = reinterpret_cast<const uint4*>(reinterpret_cast<const char*>(pose) + 32u * lane);
+        const uint4 v = kCg ? __ldcg(src) : *src;
+        asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(w.slot + ((0x401000u >> (8u * lane)) & 0xffu)),
+                     "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");     // slot offsets 0, 16, 64 (fast_chunk)
+    }
+    const int state = kCg ? __ldcg(&pose->state) : pose->state;
+    __syncwarp();
+    w.rays += min(B, jb0 + 32u) - jb0;
+    HeldRound h;
+    h.e = e; h.j = jb0 + lane; h.r = 0.0f;
+    h.store = h.j < B;
+    bool near = false;
+    if (state == 0) h.r = cast_beam_fast<false>(w.slot, min(w.tab + 16u * h.j, w.tab_last), a.robot.T, a.half_T, a.map.rho, a.robot.rmax, near);
+    if (__any_sync(0xffffffffu, near && h.store)) h.r = fast_near_beam<kCg>(a, w, pose, h.j, near && h.store, h.r);
+    return h;
+}
+__device__ __forceinline__ void fast_store_held(const BeamArgs& a, const HeldRound& h, const unsigned long long ring_head) {
+    if (h.store) {
+        a.out_ranges[h.e * a.out_stride + a.out_off + h.j] = h.r;
+        if (a.ring_obs) ring_row_of(a, ring_head, h.e)[a.out_off + h.j] = h.r;
+    }
+}
 // one task: beams [jb0, jb1) of env e, jb0 a multiple of 32 (pose = the env's sensing pose, possibly a shared-memory copy)
 template <bool kCoarse>
 __device__ __forceinline__ void fast_chunk(const BeamArgs& a, FastWarp& w, const BeamPose* pose, const unsigned e,

@@ -589,6 +589,14 @@ struct ResetArgs {
     uint8_t* fail_out;           // or NULL; else [n]: "no attempt was accepted" is stored here instead of counted
 };
 
+struct StepEnd {                         // device words owned by the sim, zero at creation
+    unsigned done_ctas;                  // CTAs of the running launch that have finished
+    unsigned outcomes_done;              // outcome warps of the running step that have finished (done list, prepared
+                                         //   resets): zeroed by the step's motion kernel, read by prepared_reset_kernel
+    int par_used;                        // the done-list parity that step fills
+    unsigned pad_;
+};
+
 // A reset prepared ahead of fn_reset (fn_sim_prepare_reset): the step's outcome warps run reset_env for the envs
 // they report done, with ResetArgs that point here instead of at the caller's arrays; fn_reset(mask = NULL) then
 // only copies (reset_apply) and casts the beams.  Same layouts as the arrays they stand for.
@@ -708,25 +716,54 @@ __device__ __forceinline__ void reset_env(const ResetArgs& a, const MapDev& mp, 
 }
 
 // The stores of reset_env for env e from a prepared reset (one thread): a = the arguments of the fn_reset call.
-__device__ __forceinline__ void reset_apply(const ResetArgs& a, const PreparedReset& pr, const int e) {
+// _early: what the step no longer touches once its outcome warps have finished (states, episode bookkeeping, goal
+// observation, counters); _late: what it uses until it completes (the sensing pose its beams are cast from, the ring
+// head).  The prepared values are read past L1 (written by a kernel that may still be running).
+__device__ __forceinline__ void reset_apply_early(const ResetArgs& a, const PreparedReset& pr, const int e) {
     const int n = a.n;
 #pragma unroll
-    for (int k = 0; k < 8; ++k) a.states[k * n + e] = pr.states[k * n + e];
-    const float d = pr.goal_obs[e], alpha = pr.goal_obs[n + e];
-    a.d_prev[e] = pr.d_prev[e];
+    for (int k = 0; k < 8; ++k) a.states[k * n + e] = __ldcg(pr.states + k * n + e);
+    a.d_prev[e] = __ldcg(pr.d_prev + e);
     a.ep_step[e] = 0;
-    if (a.out_goal_obs) { a.out_goal_obs[e] = d; a.out_goal_obs[n + e] = alpha; }
-    const BeamPose bp = pr.poses[e];
-    a.poses[e] = bp;
+    if (a.out_goal_obs) { a.out_goal_obs[e] = __ldcg(pr.goal_obs + e); a.out_goal_obs[n + e] = __ldcg(pr.goal_obs + n + e); }
+    atomicAdd(&a.counters[kResets], 1ull);
+    atomicAdd(&a.counters[kResetsPrepared], 1ull);
+    if (__ldcg(pr.fail + e)) atomicAdd(&a.counters[kResetFail], 1ull);
+}
+struct HeldPose {                        // a prepared sensing pose read before it may be stored
+    int e;                               // -1: none
+    uint4 v[sizeof(BeamPose) / 16];
+};
+__device__ __forceinline__ HeldPose reset_pose_held(const ResetArgs& a, const PreparedReset& pr, const int e) {
+    HeldPose h;
+    h.e = e;
+    const uint4* src = reinterpret_cast<const uint4*>(pr.poses + e);
+#pragma unroll
+    for (int k = 0; k < (int)(sizeof(BeamPose) / 16); ++k) h.v[k] = __ldcg(src + k);
+    asm volatile("prefetch.global.L2 [%0];" ::"l"(a.poses + e));
+    return h;
+}
+__device__ __forceinline__ void reset_pose_store(const ResetArgs& a, const HeldPose& h) {
+    if (h.e < 0) return;
+    uint4* dst = reinterpret_cast<uint4*>(a.poses + h.e);
+#pragma unroll
+    for (int k = 0; k < (int)(sizeof(BeamPose) / 16); ++k) dst[k] = h.v[k];
+}
+__device__ __forceinline__ void reset_apply_late(const ResetArgs& a, const PreparedReset& pr, const int e, const bool copy_pose = true) {
+    const int n = a.n;
+    if (copy_pose) {
+        const uint4* src = reinterpret_cast<const uint4*>(pr.poses + e);
+        uint4* dst = reinterpret_cast<uint4*>(a.poses + e);
+#pragma unroll
+        for (int k = 0; k < (int)(sizeof(BeamPose) / 16); ++k) dst[k] = src[k];
+    }
     if (a.ring) {
+        const float d = pr.goal_obs[e], alpha = pr.goal_obs[n + e];
         const unsigned long long head = *a.ring_head_dev;
         float* row = a.ring + ((head + (unsigned long long)e) % a.ring_cap) * (size_t)a.ring_row;
         const int B = a.robot.B;
         row[B] = d; row[B + 1] = alpha; row[B + 2] = 0.f; row[B + 3] = 0.f; row[B + 4] = 0.f;
     }
-    atomicAdd(&a.counters[kResets], 1ull);
-    atomicAdd(&a.counters[kResetsPrepared], 1ull);
-    if (pr.fail[e]) atomicAdd(&a.counters[kResetFail], 1ull);
 }
 
 __global__ void __launch_bounds__(kResetWarps * 32) reset_kernel(ResetArgs a) {

@@ -112,12 +112,19 @@ __global__ void __launch_bounds__(kFusedThreads, 2) reset_beam_kernel(const __gr
 
 // fn_reset(mask = NULL) after a step that prepared the resets (fn_sim_prepare_reset): the new states, goal
 // observations and sensing poses of the listed envs already sit in the sim's buffers (pr; a.poses = pr.poses), so
-// nothing here depends on anything but the list -- every warp of the grid takes rounds of 32 beams of the listed
-// envs (task t = round t % rounds of list entry t / rounds, dealt to the CTAs in turn so that the SMs share every
-// env's beams); the tasks after those copy the prepared states into the caller's arrays, 32 envs per warp
-// (reset_apply).  No reset warps, no block barrier between resetting and casting.
+// nothing here depends on anything but the list -- the warps of the grid share the rounds of 32 beams of the listed
+// envs, and the prepared states are copied into the caller's arrays (reset_apply_*).  No reset warps, no owner CTA.
+//
+// Its CTAs become resident while the step kernel's last CTAs still cast (PDL), and what they need -- the done list
+// and the prepared poses -- is complete since the step's outcome warps finished (tens of us earlier; they count
+// themselves in end->outcomes_done).  So the work is done BEFORE the dependency wait, under the step kernel's tail:
+// the ranges are held in registers, and only the stores wait for the step to complete (it writes the terminal
+// observation into the same rows, reads the sensing poses the copies replace, and advances the ring head).  The
+// CTAs arrive in the order of their index over ~8 us, as the step's CTAs leave (measured with globaltimer stamps).  Waiting for a flag of the kernel BEFORE this one needs no co-residency: the step's
+// warps never wait for anything.
+constexpr unsigned kCopyFirstCta = 48u;
 __global__ void __launch_bounds__(kBeamThreads, 2) prepared_reset_kernel(const __grid_constant__ ResetArgs ra, const __grid_constant__ BeamArgs a,
-                                                                        const PreparedReset pr) {
+                                                                        const PreparedReset pr, const StepEnd* end, const unsigned n_outcome_warps) {
     extern __shared__ __align__(16) uint8_t smem_raw[];
     const int B = a.robot.B;
     const int mapWords = (a.map.H + 2 * kLineGuard) * a.map.strideR + (a.map.W + 2 * kLineGuard) * a.map.strideC;
@@ -126,26 +133,72 @@ __global__ void __launch_bounds__(kBeamThreads, 2) prepared_reset_kernel(const _
     __shared__ __align__(8) unsigned long long s_mbar;
     __shared__ __align__(16) FastShared<kBeamThreads / 32> s_fast;
     stage_beam_constants(a, s_tab, s_map, mapWords, true, &s_mbar);
-    __syncthreads();
-    griddep_wait();                                                // the list comes from the step
-    griddep_launch_dependents();
-    const int* rlist = ra.list;
-    const int* rcount = ra.count_dev;
-    if (ra.list_par_dev) { const int q = *ra.list_par_dev ^ 1; rlist += (size_t)q * ra.n; rcount += q; }
-    const unsigned count = (unsigned)*rcount;
-    const unsigned long long ring_head = a.ring_obs ? *a.ring_head : 0ull;
-    FastWarp w = fast_warp(a, &s_fast, s_tab, (uint32_t)__cvta_generic_to_shared(s_map));
-    const unsigned rounds = ((unsigned)B + 31u) >> 5, ntasks = count * rounds, nall = ntasks + ((count + 31u) >> 5);
-    const unsigned lane = threadIdx.x & 31, nwarps = gridDim.x * (blockDim.x >> 5);
-    for (unsigned task = blockIdx.x + gridDim.x * (threadIdx.x >> 5); task < nall; task += nwarps) {
-        if (task < ntasks) {
-            const unsigned k = a.inv_rounds ? __umulhi(task, a.inv_rounds) : task / rounds, jb0 = (task - k * rounds) << 5;
-            const unsigned e = (unsigned)rlist[k];
-            fast_chunk<false>(a, w, a.poses + e, e, jb0, min((unsigned)B, jb0 + 32u), ring_head);
-        } else {
-            const unsigned k = ((task - ntasks) << 5) + lane;
-            if (k < count) reset_apply(ra, pr, rlist[k]);
+    if (threadIdx.x == 0) {                                        // the step's outcome warps have all finished?
+        const volatile unsigned* flag = &end->outcomes_done;
+        for (int it = 0; *flag < n_outcome_warps; ++it) {
+            if (it > (1 << 22)) __trap();                          // (never: they finish tens of us before this kernel starts)
+            __nanosleep(64);
         }
+        __threadfence();
+    }
+    __syncthreads();
+    // (read past L1: these words were written while this SM may have held older copies of their lines)
+    const int q = __ldcg(&end->par_used);
+    const int* rlist = ra.list + (size_t)q * ra.n;
+    const unsigned count = (unsigned)__ldcg(ra.count_dev + q);
+    FastWarp w = fast_warp(a, &s_fast, s_tab, (uint32_t)__cvta_generic_to_shared(s_map));
+    const unsigned rounds = ((unsigned)B + 31u) >> 5, ntasks = count * rounds;
+    const unsigned lane = threadIdx.x & 31, wib = threadIdx.x >> 5, nw = blockDim.x >> 5, nwarps = gridDim.x * nw;
+    // The last warp of every CTA is a service warp (copies), the others take one round each before the wait: round t
+    // goes to warp t % 15 of CTA t / 15, so the CTAs that arrive last -- they replace the step's last CTAs, ~8 us
+    // after the first -- have nothing to do for lists of the usual length.  The copies go to the service warps of
+    // CTAs that arrive early but not first (the first SMs to free are still busy with the step's other CTA).
+    const unsigned rw = nw - 1u, cap = gridDim.x * rw;             // warps that take rounds per CTA; rounds taken before the wait
+    const bool service = wib == rw;
+    const unsigned ngroups = (count + 7u) >> 3;                    // copies: 8 listed envs per service warp
+    const unsigned g0 = (blockIdx.x + gridDim.x - min(gridDim.x - 1u, kCopyFirstCta)) % gridDim.x;
+
+    // ---- before the wait: a round with held results, or the copies that touch nothing the step still uses
+    HeldRound held;
+    held.store = false;
+    HeldPose hp;                                                   // (the first group's: longer lists copy the rest after the wait)
+    hp.e = -1;
+    if (service) {
+        for (unsigned g = g0; g < ngroups; g += gridDim.x) {
+            const unsigned k = (g << 3) + lane;
+            if (lane < 8u && k < count) {
+                const int e = __ldcg(rlist + k);
+                reset_apply_early(ra, pr, e);
+                if (g == g0) hp = reset_pose_held(ra, pr, e);
+            }
+        }
+    } else {
+        const unsigned t = blockIdx.x * rw + wib;
+        if (t < ntasks) {
+            const unsigned k = a.inv_rounds ? __umulhi(t, a.inv_rounds) : t / rounds, jb0 = (t - k * rounds) << 5;
+            const unsigned e = (unsigned)__ldcg(rlist + k);
+            held = fast_round_held<true>(a, w, a.poses + e, e, jb0);
+            // (the stores after the wait should find their translations: the kernel ends when they have landed)
+            if (held.store) asm volatile("prefetch.global.L2 [%0];" ::"l"(a.out_ranges + (held.e * a.out_stride + a.out_off + held.j)));
+        }
+    }
+
+    griddep_wait();                                                // ---- the step is complete
+    griddep_launch_dependents();
+    const unsigned long long ring_head = a.ring_obs ? *a.ring_head : 0ull;
+    fast_store_held(a, held, ring_head);
+    if (service) {
+        reset_pose_store(ra, hp);
+        for (unsigned g = g0; g < ngroups; g += gridDim.x) {
+            const unsigned k = (g << 3) + lane;
+            if (lane < 8u && k < count) reset_apply_late(ra, pr, rlist[k], g != g0);
+        }
+    }
+    // what a long list leaves over, shared by all warps in the usual way
+    for (unsigned t = cap + blockIdx.x + gridDim.x * wib; t < ntasks; t += nwarps) {
+        const unsigned k = a.inv_rounds ? __umulhi(t, a.inv_rounds) : t / rounds, jb0 = (t - k * rounds) << 5;
+        const unsigned e = (unsigned)rlist[k];
+        fast_chunk<false>(a, w, a.poses + e, e, jb0, min((unsigned)B, jb0 + 32u), ring_head);
     }
     fast_finish(a, w, ring_head);
 }

@@ -17,16 +17,11 @@
 
 namespace fn {
 
-struct StepEnd {                         // device words owned by the sim, zero at creation
-    unsigned done_ctas;                  // CTAs of the running launch that have finished
-    unsigned pad_[3];
-};
-
 // S1 only: one thread per env (epw envs per warp, see env_step_kernel)
-__global__ void __launch_bounds__(kEnvBlock) env_motion_kernel(EnvArgs a) {
+__global__ void __launch_bounds__(kEnvBlock) env_motion_kernel(EnvArgs a, StepEnd* end) {
     griddep_wait();                                                // states / actions come from earlier work
     griddep_launch_dependents();                                   // the beam kernel may start staging the map now
-    if (blockIdx.x == 0 && threadIdx.x == 0) *a.beam_task_counter = 0u;
+    if (blockIdx.x == 0 && threadIdx.x == 0) { *a.beam_task_counter = 0u; end->outcomes_done = 0u; }
     const int e = blockIdx.x * a.epw + threadIdx.x;
     if ((int)threadIdx.x >= a.epw || e >= a.n) return;
     if (a.eval_outcome != nullptr && a.eval_outcome[e] != 0) return;   // a completed evaluation case is frozen
@@ -83,6 +78,14 @@ __global__ void __launch_bounds__(FastShape<kCoarse>::kThreads, FastShape<kCoars
             if constexpr (kPrep) {
                 for (; dm; dm &= dm - 1u) reset_env<kSmem>(ra, ms, scratch, e0 + base + (__ffs(dm) - 1), lane);
             } else (void)dm;
+        }
+        if constexpr (kPrep) {                                     // list entries, count and prepared resets, then the flag
+            __syncwarp();
+            if (lane == 0) {
+                end->par_used = *ea.par_dev;
+                __threadfence();
+                atomicAdd(&end->outcomes_done, 1u);
+            }
         }
     }
 

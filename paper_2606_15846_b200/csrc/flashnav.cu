@@ -1129,7 +1129,8 @@ extern "C" int fn_step_host(fn_sim* s, float* states, const float* actions, floa
             (void)cudaGetLastError();                              // (pageable memory: not an error here)
         }
     }
-    int rc = fn_step(s, s->stg_states, s->stg_actions, dt, s->stg_mask, dev_ranges, s->stg_col, s->stg_gobs);
+    int rc = seeds ? fn_sim_prepare_reset(s, reinterpret_cast<const uint64_t*>(s->stg_seeds)) : FN_OK;   // (the reset below)
+    if (rc == FN_OK) rc = fn_step(s, s->stg_states, s->stg_actions, dt, s->stg_mask, dev_ranges, s->stg_col, s->stg_gobs);
     if (rc != FN_OK) return rc;
     // the step's own (pre-reset) outputs go back first; the reset then overwrites the done rows
     FN_CUDA(cudaMemcpyAsync(out_collision, s->stg_col, n, cudaMemcpyDeviceToHost, st));
@@ -1188,7 +1189,8 @@ extern "C" int fn_step_host_begin(fn_sim* s, int slot, const float* states_in, c
     FN_CUDA(cudaMemcpyAsync(h.actions, actions, n * A * sizeof(float), cudaMemcpyHostToDevice, st));
     FN_CUDA(cudaMemcpyAsync(h.mask, mask, n, cudaMemcpyHostToDevice, st));
     if (seeds) FN_CUDA(cudaMemcpyAsync(h.seeds, seeds, n * sizeof(unsigned long long), cudaMemcpyHostToDevice, st));
-    rc = fn_step(s, s->stg_states, h.actions, dt, h.mask, h.ranges, h.col, h.gobs);
+    if (seeds) rc = fn_sim_prepare_reset(s, reinterpret_cast<const uint64_t*>(h.seeds));                   // (the reset below)
+    if (rc == FN_OK) rc = fn_step(s, s->stg_states, h.actions, dt, h.mask, h.ranges, h.col, h.gobs);
     if (rc != FN_OK) return rc;
     if (seeds) {
         rc = fn_reset(s, s->stg_states, nullptr, reinterpret_cast<const uint64_t*>(h.seeds), h.ranges, h.gobs);

@@ -134,7 +134,10 @@ int fn_reset(fn_sim* sim, float* states_dev, const uint8_t* mask_dev, const uint
  *   out_reward_dev   [N] fp32: Eq. (1).
  * fn_ring_attach: device replay ring (config 5).  Row = [ranges(B), d, alpha, v_x, v_y, w,
  *   action(A), reward, done] fp32; fn_step appends one row per env at slot (head + e) mod capacity, with
- *   obs = the observation the action was chosen from (the previous fn_step / fn_reset outputs).  A step
+ *   obs = the observation the action was chosen from (the previous fn_step / fn_reset outputs).  done is a code:
+ *   0 = the episode goes on, 1 = terminated (collision or goal reached), 2 = truncated (step limit or forced
+ *   reset without a terminal event) -- the next observation of a done row is the post-reset one, so rows with
+ *   code 2 cannot be bootstrapped from and a learner should leave them out or mask them.  A step
  *   completes the rows [head, head + N) and starts the next N, so capacity >= 2 N (else FN_ERR_INVALID_ARG).
  *   Evaluation steps (fn_eval_begin .. fn_eval_end) leave the ring and its head untouched.
  * fn_observe_all: recompute ranges and goal obs of ALL envs from states ("Full batch").
@@ -160,7 +163,7 @@ int fn_ring_attach(fn_sim* sim, float* ring_dev, uint64_t capacity_transitions);
  * out_rows_dev [n_samples][B + 5 + A + 2] fp32: rows as stored (obs, action, reward, done);
  * out_next_obs_dev [n_samples][B + 5] or NULL: the obs part of the same env's next row (slot + n_envs mod
  * capacity), which the step that completed the row has already written (for a done transition that is the
- * post-reset observation; the done flag masks the bootstrap).
+ * post-reset observation; done code 1 masks the bootstrap, code 2 marks a row without a usable next observation).
  * Enqueued on the sim's stream, i.e. after the ring writes of earlier fn_step / fn_reset calls ("sampling waits
  * for the required replay writes"); the paper's two preallocated batch buffers are the caller's: alternate the
  * output pointers between calls and order the learner after the call with a stream or an event. */

@@ -192,7 +192,17 @@ def reset(occ, res, footprint, regions, goal_dist_min, goal_dist_max, mask, seed
     return amb, failed
 
 
+def done_code(done, collision, d, goal_tol):
+    """The ring row's done field (G18): 0 running, 1 terminated (collision or goal), 2 truncated (limit / forced)."""
+    done, collision, d = _u8(done), _u8(collision), _f32(d)
+    f = lib().fno_done_code
+    f.restype = C.c_uint8
+    f.argtypes = [C.c_uint8, C.c_uint8, C.c_float, C.c_float]
+    return np.array([f(int(a), int(b), float(c), float(goal_tol)) for a, b, c in zip(done, collision, d)], np.uint8)
+
+
 def ring_append(ring, capacity, head, obs_ranges, obs_goal, obs_vel, actions, reward, done):
+    """done: the codes of done_code (stored as they are)."""
     obs_ranges, obs_goal, obs_vel, actions, reward = map(_f32, (obs_ranges, obs_goal, obs_vel,
                                                                 actions, reward))
     done = _u8(done)

@@ -587,7 +587,18 @@ void fno_reset(const uint8_t* occ, int H, int W, float res, int V, const float* 
  * BASELINE.json config 5: "(obs, action, reward, done) in fp32".  Row layout (reading G18):
  *   [ranges(B), d, alpha, v_x, v_y, w, action(A), reward, done]  with obs = the observation the action
  * was chosen from.  slot = (head + e) mod capacity.
+ * done is a code (reading G18, revised): 0 = the episode goes on, 1 = it TERMINATED (collision or goal reached:
+ * PAPER.md:69-72, the cases Eq. (1) rewards), 2 = it was TRUNCATED (step limit or a forced reset, no terminal
+ * event).  PAPER.md:86 keeps the pre-reset observation as the next observation of such a row; this ring's next
+ * observation of a done row is the post-reset one (G22), so a learner must not bootstrap from it -- with the code it
+ * can tell the rows whose bootstrap is legitimately zero (1) from the rows it has to leave out (2).
+ * fno_done_code gives the code from what the step reports.
  */
+uint8_t fno_done_code(uint8_t done, uint8_t collision, float d, float goal_tol) {
+    if (!done) return 0;
+    return (collision || d < goal_tol) ? 1 : 2;
+}
+
 void fno_ring_append(float* ring, uint64_t capacity, uint64_t head, int n, int B, int A,
                      const float* obs_ranges /*[n][B]*/, const float* obs_goal /*[2][n]*/,
                      const float* obs_vel /*[3][n]*/, const float* actions /*[n][A]*/,
@@ -600,7 +611,7 @@ void fno_ring_append(float* ring, uint64_t capacity, uint64_t head, int n, int B
         r[B + 2] = obs_vel[0 * n + e];  r[B + 3] = obs_vel[1 * n + e]; r[B + 4] = obs_vel[2 * n + e];
         for (int a = 0; a < A; ++a) r[B + 5 + a] = actions[(size_t)e * A + a];
         r[B + 5 + A] = reward[e];
-        r[B + 6 + A] = done[e] ? 1.0f : 0.0f;
+        r[B + 6 + A] = (float)done[e];                             /* the code: 0, 1 or 2 */
     }
 }
 

@@ -449,7 +449,7 @@ __device__ __forceinline__ unsigned env_outcome(const EnvArgs& a, const MapDev& 
         float* row = a.ring + ((head + (unsigned long long)e) % a.ring_cap) * (size_t)a.ring_row;
         for (int k = 0; k < A; ++k) row[B + 5 + k] = a.actions[(size_t)e * A + k];   // the raw action
         row[B + 5 + A] = r;
-        row[B + 6 + A] = done ? 1.0f : 0.0f;
+        row[B + 6 + A] = done ? ((col || reached) ? 1.0f : 2.0f) : 0.0f;   // 1 terminated, 2 truncated (limit / forced)
         // and start the next step's row with the new goal obs and velocities
         float* nxt = a.ring + ((head + (unsigned long long)n + (unsigned long long)e) % a.ring_cap) * (size_t)a.ring_row;
         nxt[B] = d; nxt[B + 1] = alpha; nxt[B + 2] = avx; nxt[B + 3] = avy; nxt[B + 4] = aw;

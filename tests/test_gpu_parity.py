@@ -160,6 +160,8 @@ def test_ring_rows_and_wraparound_gpu(pu):
     from harness import workloads as W
     for drive_cfg in (5, 3):                                   # differential (A = 2) and omnidirectional (A = 3)
         wl = W.make_workload(drive_cfg, n_envs=96)
+        wl.forced_reset_frac = 0.05                            # forced resets: done code 2 (truncated)
+        codes = set()
         n, B, A = wl.n_envs, wl.n_beams, wl.action_dim
         m, r, s = pu.make_sim(wl, n)
         buf = pu.Buffers(n, B, A)
@@ -185,7 +187,8 @@ def test_ring_rows_and_wraparound_gpu(pu):
             buf.mask.copy_(torch.from_numpy(forced[t]))
             s.step(buf.states, actions[t], float(wl.dt), buf.mask, buf.ranges, buf.col, buf.gobs)
             torch.cuda.synchronize()
-            done = buf.mask.cpu().numpy().copy()
+            done = oracle.done_code(buf.mask.cpu().numpy(), buf.col.cpu().numpy(), buf.gobs[0].cpu().numpy(), wl.goal_tol)
+            codes |= set(done.tolist())
             oracle.ring_append(expect, cap, head, obs_r, obs_g, obs_v, actions[t].cpu().numpy(),
                                buf.reward.cpu().numpy(), done)
             written[(head + np.arange(n)) % cap] = True
@@ -198,6 +201,7 @@ def test_ring_rows_and_wraparound_gpu(pu):
         check[pending] = False
         assert check.sum() >= cap - n - 1
         assert np.array_equal(got[check], expect[check])
+        assert {0, 2} <= codes                                 # (1 = terminated: the full-scale C5 test sees collisions)
         # pending rows already hold the observation the next action will be chosen from
         assert np.array_equal(got[pending, :B], buf.ranges.cpu().numpy())
         assert np.array_equal(got[pending, B:B + 2], buf.gobs.cpu().numpy().T)
@@ -232,6 +236,7 @@ def test_ring_at_full_scale_c5(pu):
     s.reset(buf.states, buf.mask, seeds[0], buf.ranges, buf.gobs)
     head = 0
     rows_checked = 0
+    codes_seen = set()
     for t in range(steps):
         obs_r = buf.ranges[sub_t].cpu().numpy()
         obs_g = buf.gobs[:, sub_t].cpu().numpy()
@@ -242,8 +247,10 @@ def test_ring_at_full_scale_c5(pu):
         s.step(buf.states, actions, float(wl.dt), buf.mask, buf.ranges, buf.col, buf.gobs)
         torch.cuda.synchronize()
         expect = np.zeros((sub.size, row), np.float32)
-        oracle.ring_append(expect, sub.size, 0, obs_r, obs_g, obs_v, a_np[sub], buf.reward[sub_t].cpu().numpy(),
-                           buf.mask[sub_t].cpu().numpy())
+        code = oracle.done_code(buf.mask[sub_t].cpu().numpy(), buf.col[sub_t].cpu().numpy(),
+                                buf.gobs[0, sub_t].cpu().numpy(), wl.goal_tol)
+        codes_seen |= set(code.tolist())
+        oracle.ring_append(expect, sub.size, 0, obs_r, obs_g, obs_v, a_np[sub], buf.reward[sub_t].cpu().numpy(), code)
         slots = torch.tensor([(head + int(e)) % cap for e in sub], device="cuda")
         got = ring2[slots].cpu().numpy()
         assert np.array_equal(got, expect), f"step {t}: ring rows of the sampled envs"
@@ -254,6 +261,7 @@ def test_ring_at_full_scale_c5(pu):
     # rows the wrap has overwritten hold steps 64 and 65; the pending rows hold the current observation
     pend = torch.tensor([(head + int(e)) % cap for e in sub], device="cuda")
     assert torch.equal(ring2[pend][:, :B], buf.ranges[sub_t])
+    assert {0, 1} <= codes_seen                                # running and terminated rows (collisions within 66 steps)
     s.close(); r.close(); m.close()
     del ring, ring2
     torch.cuda.empty_cache()

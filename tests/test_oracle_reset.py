@@ -117,6 +117,38 @@ def test_reset_respects_regions(oracle_lib):
     assert d.min() >= 1.0 - 1e-5 and d.max() <= 3.0 + 1e-5
 
 
+def test_done_code_of_ring_rows(oracle_lib):
+    # reading G18: 0 running, 1 terminated = collision or goal reached (the events Eq. (1)
+    # rewards), 2 truncated = done for any other reason (step limit, forced reset).  Hand cases, goal tolerance 0.3.
+    done = np.array([0, 0, 1, 1, 1, 1, 1], np.uint8)
+    col = np.array([0, 1, 1, 0, 0, 1, 0], np.uint8)               # (a collision without done cannot happen; code 0 anyway)
+    d = np.array([5.0, 5.0, 5.0, 0.2, 0.3, 0.1, 2.0], np.float32)  # d < tol reaches the goal; d == tol does not
+    want = np.array([0, 0, 1, 1, 2, 1, 2], np.uint8)
+    assert np.array_equal(oracle_lib.done_code(done, col, d, 0.3), want)
+    # against the oracle's own step with a step limit of 3: every done env gets a non-zero code, time-outs get 2,
+    # and an env is terminated exactly when the step reports a collision or a goal distance below the tolerance
+    from harness import workloads as W
+    wl = W.make_workload(1)
+    wl.max_episode_steps = 3
+    n = wl.n_envs
+    st, dp, ep = np.zeros((8, n), np.float32), np.zeros(n, np.float32), np.zeros(n, np.int32)
+    seeds, act = W.seed_tape(wl, 8), W.action_tape(wl, 7)
+    oracle_lib.reset(wl.occ, wl.resolution, wl.footprint, wl.regions, wl.goal_dist_min, wl.goal_dist_max,
+                     np.ones(n, np.uint8), seeds[0], st, dp, ep)
+    seen = set()
+    for t in range(7):
+        out = oracle_lib.step(wl, st, act[t], None, dp, ep, want_hit=False)
+        c = oracle_lib.done_code(out["done"], out["collision"], out["goal_obs"][0], wl.goal_tol)
+        assert np.array_equal(c != 0, out["done"] != 0)
+        term = (out["collision"] != 0) | (out["goal_obs"][0] < np.float32(wl.goal_tol))
+        assert np.array_equal(c == 1, term & (out["done"] != 0)) and np.array_equal(c == 2, ~term & (out["done"] != 0))
+        seen |= set(c.tolist())
+        if out["done"].any():
+            oracle_lib.reset(wl.occ, wl.resolution, wl.footprint, wl.regions, wl.goal_dist_min, wl.goal_dist_max,
+                             out["done"], seeds[t + 1], st, dp, ep)
+    assert 2 in seen and 0 in seen
+
+
 def test_ring_rows_and_wraparound(oracle_lib):
     n, B, A, cap = 5, 7, 2, 8
     rng = np.random.default_rng(0)
@@ -129,7 +161,7 @@ def test_ring_rows_and_wraparound(oracle_lib):
         obs_v = rng.random((3, n)).astype(np.float32)
         act = rng.random((n, A)).astype(np.float32)
         rew = rng.random(n).astype(np.float32)
-        done = (rng.random(n) < 0.5).astype(np.uint8)
+        done = rng.integers(0, 3, n).astype(np.uint8)             # the codes are stored as they are
         oracle_lib.ring_append(ring, cap, head, obs_r, obs_g, obs_v, act, rew, done)
         for e in range(n):
             log[(head + e) % cap] = np.concatenate([obs_r[e], obs_g[:, e], obs_v[:, e], act[e], [rew[e]], [float(done[e])]])

@@ -258,9 +258,32 @@ def ring_valid(capacity: int, total: int, n_envs: int) -> int:
     return int(lib().fno_ring_valid(C.c_uint64(capacity), C.c_uint64(total), C.c_int(n_envs)))
 
 
-def ring_sample(ring, capacity, total, n_envs, B, A, seed, n_samples, want_next=True):
+class TerminalStore:
+    """The terminal-observation ring of fno_terminal_save: entries [t_cap, B+5] f32, the index of each
+    ring row's entry, the global row id of each entry, the number of entries ever written."""
+
+    def __init__(self, capacity, t_cap, B):
+        self.t_cap = int(t_cap)
+        self.term = np.zeros((self.t_cap, B + 5), np.float32)
+        self.idx = np.full(int(capacity), -1, np.int32)
+        self.id = np.full(self.t_cap, np.iinfo(np.uint64).max, np.uint64)
+        self.head = C.c_uint64(0)
+
+
+def terminal_save(ring, capacity, total, n_envs, B, A, env_list, store: TerminalStore):
+    """Before the listed envs are reset: keep the observation the last step left in their pending rows, for every one
+    whose last completed row has a done code != 0 (and is not kept yet)."""
+    assert ring.dtype == np.float32 and ring.flags.c_contiguous
+    lst = np.ascontiguousarray(env_list, np.int32)
+    lib().fno_terminal_save(_p(ring, C.c_float), C.c_uint64(capacity), C.c_uint64(total), C.c_int(n_envs), C.c_int(B),
+                            C.c_int(A), _p(lst, C.c_int32), C.c_int(lst.size), _p(store.term, C.c_float),
+                            C.c_uint64(store.t_cap), _p(store.idx, C.c_int32), _p(store.id, C.c_uint64), C.byref(store.head))
+
+
+def ring_sample(ring, capacity, total, n_envs, B, A, seed, n_samples, want_next=True, store: TerminalStore | None = None):
     """Uniform replay sampling after `total` appended rows.  ring [capacity, B+5+A+2] f32 -> rows
-    [n,row], next_obs [n,B+5], slots [n]."""
+    [n,row], next_obs [n,B+5], slots [n].  store: terminal observations (next observation of done rows; the sampled
+    rows' done field becomes 3 for truncated rows whose observation is gone)."""
     assert ring.dtype == np.float32 and ring.flags.c_contiguous
     row = B + 5 + A + 2
     rows = np.empty((n_samples, row), np.float32)
@@ -268,7 +291,10 @@ def ring_sample(ring, capacity, total, n_envs, B, A, seed, n_samples, want_next=
     slots = np.empty(n_samples, np.int64)
     lib().fno_ring_sample(_p(ring, C.c_float), C.c_uint64(capacity), C.c_uint64(total), C.c_int(n_envs), C.c_int(B),
                           C.c_int(A), C.c_uint64(seed), C.c_int(n_samples), _p(rows, C.c_float),
-                          _p(nxt, C.c_float), _p(slots, C.c_int64))
+                          _p(nxt, C.c_float), _p(slots, C.c_int64),
+                          None if store is None else _p(store.term, C.c_float),
+                          None if store is None else _p(store.idx, C.c_int32),
+                          None if store is None else _p(store.id, C.c_uint64))
     return rows, nxt, slots
 
 

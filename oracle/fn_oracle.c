@@ -702,7 +702,8 @@ void fno_clearance_features(int V, const float* fp_xy, int B, const float* angle
  * capacity (before the ring is that full: slot s_i); the batch row is the ring row (obs, action, reward, done)
  * as stored; the next observation is the obs part of the SAME env's next row, slot + n_envs (mod capacity),
  * which the step that completed the row has already written (for the newest transitions that is the pending
- * row).  (For a done transition that is the post-reset observation; the done flag masks the bootstrap.)
+ * row).  For a done transition that is the post-reset observation unless terminal observations are kept: see
+ * fno_terminal_save and the sampler below.
  */
 uint64_t fno_sample_slot(uint64_t seed, uint64_t i, uint64_t filled) {
     const uint64_t w = fno_splitmix64(seed, i);
@@ -713,19 +714,68 @@ uint64_t fno_ring_valid(uint64_t capacity, uint64_t total, int n_envs) {
     const uint64_t room = capacity > (uint64_t)n_envs ? capacity - (uint64_t)n_envs : 0;
     return total < room ? total : room;
 }
+/* Terminal observations ("Observations before reset are retained as next observations in replay,
+ * while reset observations are returned to the collector").  In the ring the next observation of a row is the obs
+ * part of the same env's next row, and a reset overwrites that pending row with the reset observation.  So, before a
+ * reset touches it, the pending row's obs part [ranges(B), d, alpha, v_x, v_y, w] -- the observation the step left
+ * behind, i.e. the terminal one -- is copied into a second, smaller ring of `t_cap` terminal entries (t_cap >=
+ * n_envs), for every listed env whose last completed row (slot head - n_envs + e, global row id total - n_envs + e)
+ * has a done code != 0 and has not been saved yet.  term_idx[slot] = the entry of that ring row, term_id[entry] =
+ * the global id of the row the entry belongs to (entries are reused in order, so an old row's entry is recognised as
+ * gone by its id).  *term_head counts the entries ever written.  list = the envs being reset, in any order.
+ */
+void fno_terminal_save(const float* ring, uint64_t capacity, uint64_t total, int n_envs, int B, int A,
+                       const int32_t* list, int count, float* term /*[t_cap][B+5]*/, uint64_t t_cap,
+                       int32_t* term_idx /*[capacity]*/, uint64_t* term_id /*[t_cap]*/, uint64_t* term_head) {
+    const size_t row = (size_t)B + 5 + (size_t)A + 2, obs = (size_t)B + 5;
+    if (total < (uint64_t)n_envs) return;                        /* no step has completed a row yet */
+    const uint64_t head = total % capacity;
+    for (int k = 0; k < count; ++k) {
+        const uint64_t e = (uint64_t)list[k];
+        const uint64_t c = (head + capacity - (uint64_t)n_envs + e) % capacity;      /* the env's last completed row */
+        const uint64_t g = total - (uint64_t)n_envs + e;
+        if (ring[c * row + (size_t)B + 6 + (size_t)A] == 0.0f) continue;             /* the episode did not end */
+        const int32_t t = term_idx[c];
+        if (t >= 0 && term_id[t] == g) continue;                                      /* saved already */
+        const uint64_t entry = *term_head % t_cap;
+        *term_head += 1;
+        memcpy(term + entry * obs, ring + ((head + e) % capacity) * row, obs * sizeof(float));
+        term_id[entry] = g;
+        term_idx[c] = (int32_t)entry;
+    }
+}
+
+/* The sampler with terminal observations.  term == NULL: no terminal ring.  For a row with done code != 0 whose
+ * terminal entry is still there, the next observation is that entry (the pre-reset observation); otherwise it is
+ * the obs part of the env's next row as before (the post-reset observation).  The done field of the SAMPLED copy
+ * says which: 0 running, 1 terminated (bootstrap masked, next observation irrelevant), 2 truncated with its true
+ * next observation delivered, 3 truncated but the observation is gone (or no terminal ring): not to be
+ * bootstrapped from.  Ring rows themselves hold 0, 1, 2 (fno_done_code).
+ */
 void fno_ring_sample(const float* ring, uint64_t capacity, uint64_t total, int n_envs, int B, int A,
                      uint64_t seed, int n_samples, float* out_rows /*[n_samples][row]*/,
-                     float* out_next_obs /*[n_samples][B+5] or NULL*/, int64_t* out_slots /*or NULL*/) {
+                     float* out_next_obs /*[n_samples][B+5] or NULL*/, int64_t* out_slots /*or NULL*/,
+                     const float* term, const int32_t* term_idx, const uint64_t* term_id) {
     const size_t row = (size_t)B + 5 + (size_t)A + 2, obs = (size_t)B + 5;
     const uint64_t valid = fno_ring_valid(capacity, total, n_envs), head = total % capacity;
     if (valid == 0) return;
     for (int i = 0; i < n_samples; ++i) {
         const uint64_t si = fno_sample_slot(seed, (uint64_t)i, valid);
         const uint64_t slot = (head + capacity - valid + si) % capacity;
-        memcpy(out_rows + (size_t)i * row, ring + (size_t)slot * row, row * sizeof(float));
-        if (out_next_obs)
-            memcpy(out_next_obs + (size_t)i * obs, ring + (size_t)((slot + (uint64_t)n_envs) % capacity) * row,
-                   obs * sizeof(float));
+        const uint64_t g = total - valid + si;                   /* global id of the sampled row */
+        float* out = out_rows + (size_t)i * row;
+        memcpy(out, ring + (size_t)slot * row, row * sizeof(float));
+        const float* next = ring + (size_t)((slot + (uint64_t)n_envs) % capacity) * row;
+        const float code = out[(size_t)B + 6 + (size_t)A];
+        if (code != 0.0f) {
+            int kept = 0;
+            if (term) {
+                const int32_t t = term_idx[slot];
+                if (t >= 0 && term_id[t] == g) { next = term + (size_t)t * obs; kept = 1; }
+            }
+            if (code == 2.0f && !kept) out[(size_t)B + 6 + (size_t)A] = 3.0f;
+        }
+        if (out_next_obs) memcpy(out_next_obs + (size_t)i * obs, next, obs * sizeof(float));
         if (out_slots) out_slots[i] = (int64_t)slot;
     }
 }

@@ -57,3 +57,80 @@ def test_gather_identity_and_next_observation(oracle_lib):
     # nothing to sample: no row appended yet
     rows = oracle_lib.ring_sample(np.zeros((cap, row), np.float32), cap, 0, n_envs, B, A, 3, 8)[0]
     assert rows.shape == (8, row)
+
+
+def test_terminal_observations_against_a_dictionary_model(oracle_lib):
+    # PAPER.md:86 "Observations before reset are retained as next observations in replay, while reset observations are
+    # returned to the collector."  The oracle keeps them in a small second ring (fno_terminal_save) and the sampler
+    # hands them out as the next observation of done rows.  Pinned against plain Python bookkeeping: a dictionary
+    # from the global row id to the observation the step left behind, a FIFO of the ids whose observation is kept.
+    # Every value written anywhere is unique, so a wrong row, a wrong entry or a stale entry shows.  Covers: ring wrap,
+    # terminal-ring wrap (entries lost), envs reset without a finished episode, a reset called twice, codes 1 / 2 / 3.
+    import collections
+    n, B, A, cap, t_cap = 5, 3, 2, 23, 7
+    row, obs = B + 5 + A + 2, B + 5
+    rng = np.random.default_rng(3)
+    ring = np.zeros((cap, row), np.float32)
+    store = oracle_lib.TerminalStore(cap, t_cap, B)
+    uniq = iter(range(1, 10 ** 6))
+    new_obs = lambda: np.array([next(uniq) for _ in range(obs)], np.float32)
+    left_behind = {}                                              # row id -> the observation the step left (pre-reset)
+    alive = collections.OrderedDict()                             # row ids whose terminal observation is kept, oldest first
+    was_reset = set()                                             # row ids whose env was reset right after the row
+    total = 0
+    for e in range(n):                                            # the first observation (a reset of all envs): pending rows
+        ring[e, :obs] = new_obs()
+    seen_codes = set()
+    for t in range(60):
+        head = total % cap
+        code = rng.choice([0, 0, 0, 1, 2], n)
+        for e in range(n):                                        # the step completes rows [head, head + n) ...
+            r = ring[(head + e) % cap]
+            r[obs:obs + A] = [next(uniq) for _ in range(A)]
+            r[obs + A] = next(uniq)
+            r[obs + A + 1] = code[e]
+            o = new_obs()                                         # ... and leaves the next observation in the pending rows
+            ring[(head + n + e) % cap, :obs] = o
+            left_behind[total + e] = o
+        total += n
+        head = total % cap
+        lst = [e for e in range(n) if code[e] != 0]
+        if t % 4 == 1:
+            lst.append(int(rng.integers(0, n)))                   # an env reset although its episode goes on (or twice)
+        rng.shuffle(lst)
+        for rep in range(2 if t % 5 == 2 else 1):                 # sometimes the reset is called twice
+            oracle_lib.terminal_save(ring, cap, total, n, B, A, lst, store)
+            for e in lst:                                         # the model, in list order
+                g = total - n + e
+                if code[e] != 0 and g not in alive:
+                    alive[g] = True
+                    if len(alive) > t_cap:
+                        alive.popitem(last=False)
+            for e in lst:                                         # the reset writes the reset observation
+                ring[(head + e) % cap, :obs] = new_obs()
+                was_reset.add(total - n + e)
+        rows, nxt, slots = oracle_lib.ring_sample(ring, cap, total, n, B, A, 100 + t, 64, store=store)
+        valid = min(total, cap - n)
+        for i in range(64):
+            si = oracle_lib.sample_slot(100 + t, i, valid)
+            g = total - valid + si
+            slot = (head - valid + si) % cap
+            assert slot == slots[i]
+            want_row = ring[slot].copy()
+            want_next = ring[(slot + n) % cap, :obs]
+            c = want_row[-1]
+            if c != 0:
+                if g in alive:
+                    want_next = left_behind[g]
+                elif c == 2:
+                    want_row[-1] = 3
+            elif g not in was_reset:
+                assert np.array_equal(want_next, left_behind[g])  # a running row's next row IS what the step left
+            seen_codes.add(int(want_row[-1]))
+            assert np.array_equal(rows[i], want_row), (t, i)
+            assert np.array_equal(nxt[i], want_next), (t, i)
+        # without a terminal ring every truncated row is marked 3 and the next observation is the next row's
+        rows0, nxt0, _ = oracle_lib.ring_sample(ring, cap, total, n, B, A, 100 + t, 64)
+        assert np.array_equal(nxt0, ring[(slots + n) % cap, :obs])
+        assert not (rows0[:, -1] == 2).any() and np.array_equal(rows0[:, -1] == 3, ring[slots, -1] == 2)
+    assert seen_codes == {0, 1, 2, 3} and store.head.value > 3 * t_cap

@@ -140,6 +140,14 @@ int fn_reset(fn_sim* sim, float* states_dev, const uint8_t* mask_dev, const uint
  *   code 2 cannot be bootstrapped from and a learner should leave them out or mask them.  A step
  *   completes the rows [head, head + N) and starts the next N, so capacity >= 2 N (else FN_ERR_INVALID_ARG).
  *   Evaluation steps (fn_eval_begin .. fn_eval_end) leave the ring and its head untouched.
+ * fn_ring_attach_terminal: terminal observations ("Observations before reset are retained as next
+ *   observations in replay, while reset observations are returned to the collector").  term_dev [rows][B + 5] fp32
+ *   (the caller's, rows >= N) is a second ring: every fn_reset first copies, for each env it resets whose last
+ *   completed ring row has a done code != 0, the observation the step left in the env's pending row -- [ranges(B),
+ *   d, alpha, v_x, v_y, w], the pre-reset observation -- into the next entry (entries are reused in order), and
+ *   fn_ring_sample returns it as the next observation of that row for as long as the entry exists.  Attach after
+ *   fn_ring_attach (which drops it); NULL detaches.  Evaluation steps do not touch it.
+ *   Errors: FN_ERR_INVALID_ARG (no ring, rows < N), FN_ERR_OOM / FN_ERR_CUDA (4 B per ring row + 8 B per entry).
  * fn_observe_all: recompute ranges and goal obs of ALL envs from states ("Full batch").
  * fn_get_counters: synchronises the stream and copies FN_N_COUNTERS u64 counters to host_out.
  * fn_sim_count_words: 1 = also count 32-bit map words loaded by the beam kernel (slower; default 0). */
@@ -154,16 +162,21 @@ int fn_sim_bind_aux(fn_sim* sim, int32_t* out_hit_cell_dev, float* out_reward_de
  * fn_observe_all writes all rows. */
 int fn_sim_bind_features(fn_sim* sim, int n_sectors, float* out_z_dev);
 int fn_ring_attach(fn_sim* sim, float* ring_dev, uint64_t capacity_transitions);
+int fn_ring_attach_terminal(fn_sim* sim, float* term_dev, uint64_t rows);
 /* ---- uniform replay sampling ("Each replay batch contains U x B transitions sampled uniformly
  * from replay and divided into U minibatches of size B"): gathers n_samples = U * B ring rows.
  * Sample i draws s = floor(SplitMix64(seed, i) * valid / 2^64), valid = min(rows completed, capacity - n_envs), and
  * takes slot (head - valid + s) mod capacity: uniform (with replacement) over the completed rows outside the
  * n_envs PENDING rows [head, head + n_envs), which already hold the next observation but stale action / reward /
  * done; nothing is written while no row is complete.
- * out_rows_dev [n_samples][B + 5 + A + 2] fp32: rows as stored (obs, action, reward, done);
+ * out_rows_dev [n_samples][B + 5 + A + 2] fp32: rows as stored (obs, action, reward, done) except for the done
+ * code of truncated rows, see below;
  * out_next_obs_dev [n_samples][B + 5] or NULL: the obs part of the same env's next row (slot + n_envs mod
- * capacity), which the step that completed the row has already written (for a done transition that is the
- * post-reset observation; done code 1 masks the bootstrap, code 2 marks a row without a usable next observation).
+ * capacity), which the step that completed the row has already written -- for a done row the post-reset
+ * observation, unless its terminal observation is kept (fn_ring_attach_terminal): then that one.  The done code of
+ * the SAMPLED copy tells a learner what it got: 0 running, 1 terminated (bootstrap masked), 2 truncated with the
+ * true pre-reset observation as next observation, 3 truncated but that observation is gone (entry reused, or no
+ * terminal ring attached): not to be bootstrapped from.
  * Enqueued on the sim's stream, i.e. after the ring writes of earlier fn_step / fn_reset calls ("sampling waits
  * for the required replay writes"); the paper's two preallocated batch buffers are the caller's: alternate the
  * output pointers between calls and order the learner after the call with a stream or an event. */

@@ -267,7 +267,13 @@ class TerminalStore:
         self.term = np.zeros((self.t_cap, B + 5), np.float32)
         self.idx = np.full(int(capacity), -1, np.int32)
         self.id = np.full(self.t_cap, np.iinfo(np.uint64).max, np.uint64)
+        self.start = np.zeros(self.t_cap, np.uint64)
         self.head = C.c_uint64(0)
+        self.batch_start = 0
+
+    def step_ended(self):
+        """Call after every step that appended rows: the resets that follow form one batch."""
+        self.batch_start = int(self.head.value)
 
 
 def terminal_save(ring, capacity, total, n_envs, B, A, env_list, store: TerminalStore):
@@ -277,7 +283,8 @@ def terminal_save(ring, capacity, total, n_envs, B, A, env_list, store: Terminal
     lst = np.ascontiguousarray(env_list, np.int32)
     lib().fno_terminal_save(_p(ring, C.c_float), C.c_uint64(capacity), C.c_uint64(total), C.c_int(n_envs), C.c_int(B),
                             C.c_int(A), _p(lst, C.c_int32), C.c_int(lst.size), _p(store.term, C.c_float),
-                            C.c_uint64(store.t_cap), _p(store.idx, C.c_int32), _p(store.id, C.c_uint64), C.byref(store.head))
+                            C.c_uint64(store.t_cap), _p(store.idx, C.c_int32), _p(store.id, C.c_uint64),
+                            _p(store.start, C.c_uint64), C.byref(store.head), C.c_uint64(store.batch_start))
 
 
 def ring_sample(ring, capacity, total, n_envs, B, A, seed, n_samples, want_next=True, store: TerminalStore | None = None):
@@ -293,8 +300,11 @@ def ring_sample(ring, capacity, total, n_envs, B, A, seed, n_samples, want_next=
                           C.c_int(A), C.c_uint64(seed), C.c_int(n_samples), _p(rows, C.c_float),
                           _p(nxt, C.c_float), _p(slots, C.c_int64),
                           None if store is None else _p(store.term, C.c_float),
+                          C.c_uint64(0 if store is None else store.t_cap),
                           None if store is None else _p(store.idx, C.c_int32),
-                          None if store is None else _p(store.id, C.c_uint64))
+                          None if store is None else _p(store.id, C.c_uint64),
+                          None if store is None else _p(store.start, C.c_uint64),
+                          C.c_uint64(0 if store is None else store.head.value))
     return rows, nxt, slots
 
 

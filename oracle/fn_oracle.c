@@ -720,13 +720,22 @@ uint64_t fno_ring_valid(uint64_t capacity, uint64_t total, int n_envs) {
  * reset touches it, the pending row's obs part [ranges(B), d, alpha, v_x, v_y, w] -- the observation the step left
  * behind, i.e. the terminal one -- is copied into a second, smaller ring of `t_cap` terminal entries (t_cap >=
  * n_envs), for every listed env whose last completed row (slot head - n_envs + e, global row id total - n_envs + e)
- * has a done code != 0 and has not been saved yet.  term_idx[slot] = the entry of that ring row, term_id[entry] =
- * the global id of the row the entry belongs to (entries are reused in order, so an old row's entry is recognised as
- * gone by its id).  *term_head counts the entries ever written.  list = the envs being reset, in any order.
+ * has a done code != 0 and is not kept yet.  term_idx[slot] = the entry of that ring row, term_id[entry] = the
+ * global id of the row the entry belongs to, *term_head = the entries ever written (entry = index mod t_cap, reused
+ * in order).  The entries written by the resets that follow ONE step form a batch; batch_start = *term_head when
+ * that step ended (term_start[entry]); a batch is given up as a whole as soon as a later write reuses any of its
+ * entries, i.e. an entry is kept while its id matches and *term_head <= term_start[entry] + t_cap.  (So what is
+ * kept does not depend on the order in which the envs of one reset are listed.)  list = the envs being reset.
  */
+static int fno_terminal_kept(uint64_t slot, uint64_t g, uint64_t t_cap, const int32_t* term_idx, const uint64_t* term_id,
+                             const uint64_t* term_start, uint64_t term_head) {
+    const int32_t t = term_idx[slot];
+    return t >= 0 && term_id[t] == g && term_head <= term_start[t] + t_cap;
+}
 void fno_terminal_save(const float* ring, uint64_t capacity, uint64_t total, int n_envs, int B, int A,
                        const int32_t* list, int count, float* term /*[t_cap][B+5]*/, uint64_t t_cap,
-                       int32_t* term_idx /*[capacity]*/, uint64_t* term_id /*[t_cap]*/, uint64_t* term_head) {
+                       int32_t* term_idx /*[capacity]*/, uint64_t* term_id /*[t_cap]*/, uint64_t* term_start /*[t_cap]*/,
+                       uint64_t* term_head, uint64_t batch_start) {
     const size_t row = (size_t)B + 5 + (size_t)A + 2, obs = (size_t)B + 5;
     if (total < (uint64_t)n_envs) return;                        /* no step has completed a row yet */
     const uint64_t head = total % capacity;
@@ -735,12 +744,12 @@ void fno_terminal_save(const float* ring, uint64_t capacity, uint64_t total, int
         const uint64_t c = (head + capacity - (uint64_t)n_envs + e) % capacity;      /* the env's last completed row */
         const uint64_t g = total - (uint64_t)n_envs + e;
         if (ring[c * row + (size_t)B + 6 + (size_t)A] == 0.0f) continue;             /* the episode did not end */
-        const int32_t t = term_idx[c];
-        if (t >= 0 && term_id[t] == g) continue;                                      /* saved already */
+        if (fno_terminal_kept(c, g, t_cap, term_idx, term_id, term_start, *term_head)) continue;   /* kept already */
         const uint64_t entry = *term_head % t_cap;
         *term_head += 1;
         memcpy(term + entry * obs, ring + ((head + e) % capacity) * row, obs * sizeof(float));
         term_id[entry] = g;
+        term_start[entry] = batch_start;
         term_idx[c] = (int32_t)entry;
     }
 }
@@ -755,7 +764,8 @@ void fno_terminal_save(const float* ring, uint64_t capacity, uint64_t total, int
 void fno_ring_sample(const float* ring, uint64_t capacity, uint64_t total, int n_envs, int B, int A,
                      uint64_t seed, int n_samples, float* out_rows /*[n_samples][row]*/,
                      float* out_next_obs /*[n_samples][B+5] or NULL*/, int64_t* out_slots /*or NULL*/,
-                     const float* term, const int32_t* term_idx, const uint64_t* term_id) {
+                     const float* term, uint64_t t_cap, const int32_t* term_idx, const uint64_t* term_id,
+                     const uint64_t* term_start, uint64_t term_head) {
     const size_t row = (size_t)B + 5 + (size_t)A + 2, obs = (size_t)B + 5;
     const uint64_t valid = fno_ring_valid(capacity, total, n_envs), head = total % capacity;
     if (valid == 0) return;
@@ -769,9 +779,9 @@ void fno_ring_sample(const float* ring, uint64_t capacity, uint64_t total, int n
         const float code = out[(size_t)B + 6 + (size_t)A];
         if (code != 0.0f) {
             int kept = 0;
-            if (term) {
-                const int32_t t = term_idx[slot];
-                if (t >= 0 && term_id[t] == g) { next = term + (size_t)t * obs; kept = 1; }
+            if (term && fno_terminal_kept(slot, g, t_cap, term_idx, term_id, term_start, term_head)) {
+                next = term + (size_t)term_idx[slot] * obs;
+                kept = 1;
             }
             if (code == 2.0f && !kept) out[(size_t)B + 6 + (size_t)A] = 3.0f;
         }

@@ -18,7 +18,7 @@ COUNTER_NAMES = ("rays_cast", "map_words_loaded", "envs_reset", "reset_failures"
 EXPORTED_SYMBOLS = (
     "fn_map_create", "fn_map_set_regions", "fn_map_destroy", "fn_robot_create", "fn_robot_create_union", "fn_robot_set_sensor", "fn_robot_add_sensor", "fn_robot_set_acc_limits",
     "fn_robot_destroy", "fn_task_default", "fn_sim_create", "fn_sim_destroy", "fn_sim_set_stream", "fn_step", "fn_reset",
-    "fn_sim_bind_aux", "fn_sim_bind_features", "fn_ring_attach", "fn_ring_sample", "fn_ranges_fixed_step", "fn_eval_begin", "fn_eval_result", "fn_eval_end", "fn_observe_all", "fn_get_counters", "fn_sim_count_words",
+    "fn_sim_bind_aux", "fn_sim_bind_features", "fn_ring_attach", "fn_ring_attach_terminal", "fn_ring_sample", "fn_ranges_fixed_step", "fn_eval_begin", "fn_eval_result", "fn_eval_end", "fn_observe_all", "fn_get_counters", "fn_sim_count_words",
     "fn_sim_episode_state", "fn_sim_beam_config", "fn_sim_set_fused_reset", "fn_sim_set_split_step", "fn_sim_set_coarse", "fn_sim_prepare_reset", "fn_sim_profile", "fn_sim_profile_read", "fn_step_host", "fn_step_host_begin", "fn_step_host_end", "fn_measure_peak", "fn_last_error", "fn_version")
 
 
@@ -64,6 +64,7 @@ def load_library():
         "fn_sim_bind_aux": [vp, vp, vp],
         "fn_sim_bind_features": [vp, i32, vp],
         "fn_ring_attach": [vp, vp, u64],
+        "fn_ring_attach_terminal": [vp, vp, u64],
         "fn_ring_sample": [vp, u64, i32, vp, vp],
         "fn_observe_all": [vp, vp, vp, vp],
         "fn_eval_begin": [vp, vp, i32, i32, vp, vp],
@@ -273,6 +274,15 @@ class Sim:
         self._ring = ring
         _check(load_library().fn_ring_attach(self._h, _dev_ptr(ring, torch.float32, capacity * self.ring_row_floats(), "ring")
                                              if ring is not None else None, C.c_uint64(capacity)), "fn_ring_attach")
+
+    def ring_attach_terminal(self, term, rows):
+        """Terminal observations (PAPER.md:86): term [rows, B + 5] f32 keeps the pre-reset observation of done rows;
+        ring_sample returns it as their next observation.  After ring_attach; None detaches."""
+        import torch
+        self._term = term
+        _check(load_library().fn_ring_attach_terminal(
+            self._h, _dev_ptr(term, torch.float32, rows * (self.robot.B + 5), "term") if term is not None else None,
+            C.c_uint64(rows)), "fn_ring_attach_terminal")
 
     def ring_sample(self, seed, out_rows, out_next_obs=None):
         """Uniform replay batch: out_rows [n, row] (, out_next_obs [n, B + 5]) gathered from the ring."""

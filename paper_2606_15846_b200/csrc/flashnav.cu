@@ -103,6 +103,7 @@ struct fn_sim {
     int feat_sectors;
     unsigned long long ring_cap;
     unsigned long long* d_ring_head;   // device: slot of env 0's pending ring row
+    TerminalDev term;                  // terminal observations (fn_ring_attach_terminal): caller's entries, the sim's index arrays
     int count_words;
     // beam-kernel launch configuration
     bool use_smem;
@@ -470,8 +471,8 @@ extern "C" int fn_sim_create(const fn_map* map, const fn_robot* robot, int n, co
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
     s->n_sensors = (int)robot->sensors.size();
     if (e == cudaSuccess) e = cudaMalloc(&s->d_poses, (size_t)n * s->n_sensors * sizeof(BeamPose));
-    if (e == cudaSuccess) e = cudaMalloc(&s->d_ring_head, 2 * sizeof(unsigned long long));
-    if (e == cudaSuccess) e = cudaMemsetAsync(s->d_ring_head, 0, 2 * sizeof(unsigned long long), s->stream);
+    if (e == cudaSuccess) e = cudaMalloc(&s->d_ring_head, 4 * sizeof(unsigned long long));
+    if (e == cudaSuccess) e = cudaMemsetAsync(s->d_ring_head, 0, 4 * sizeof(unsigned long long), s->stream);
     if (e == cudaSuccess) e = cudaMalloc(&s->d_list, (size_t)n * sizeof(int));
     if (e == cudaSuccess) e = cudaMalloc(&s->d_count, sizeof(int));
     if (e == cudaSuccess) e = cudaMalloc(&s->d_dprev, (size_t)n * sizeof(float));
@@ -596,6 +597,7 @@ extern "C" int fn_sim_destroy(fn_sim* s) {
     cudaFree(s->d_poses); cudaFree(s->d_ring_head); cudaFree(s->d_list); cudaFree(s->d_count); cudaFree(s->d_dprev);
     cudaFree(s->d_epstep); cudaFree(s->d_counters); cudaFree(s->d_task_counter);
     cudaFree(s->d_step_end);
+    cudaFree(s->term.idx); cudaFree(s->term.id); cudaFree(s->term.start);
     cudaFree(s->d_prep.states); cudaFree(s->d_prep.goal_obs); cudaFree(s->d_prep.d_prev); cudaFree(s->d_prep.poses);
     cudaFree(s->d_prep.fail); cudaFree(s->d_prep_epstep);
     cudaFree(s->d_done_list); cudaFree(s->d_done_count); cudaFree(s->d_eval_outcome); cudaFree(s->d_eval_return);
@@ -849,6 +851,16 @@ extern "C" int fn_reset(fn_sim* s, float* states, const uint8_t* mask, const uin
     }
     if (mask) FN_CUDA(launch_pdl(compact_mask_kernel, dim3(1), dim3(1024), 0, s->stream, mask, s->n, s->d_list, s->d_count));
     if (s->prof) FN_CUDA(cudaEventRecord(e1, s->stream));
+    if (s->ring && s->term.term) {
+        // the observations the step left behind are kept as next observations before the reset replaces them
+        TerminalSaveArgs ta;
+        ta.ring = s->ring; ta.head = s->d_ring_head; ta.cap = s->ring_cap; ta.n_envs = s->n; ta.row = ring_row_floats(s);
+        ta.obs = s->robot->B + 5; ta.list = list; ta.count_dev = count; ta.list_par_dev = mask ? nullptr : s->d_done_count + 2;
+        ta.td = s->term;
+        int tg = (s->n + 7) / 8;
+        if (tg > s->num_sms * 8) tg = s->num_sms * 8;
+        FN_CUDA(launch_pdl(terminal_save_kernel, dim3(tg), dim3(256), 0, s->stream, ta));
+    }
     const ResetArgs a = reset_args(s, states, list, count, mask ? nullptr : s->d_done_count + 2, seeds, out_goal_obs);
     int rc = FN_OK;
     // a reset prepared by the preceding fn_step for exactly this call (same seeds, nothing changed since)?
@@ -990,7 +1002,34 @@ extern "C" int fn_ring_attach(fn_sim* s, float* ring, uint64_t cap) {
     // a step completes the rows [head, head + n) and starts the pending rows [head + n, head + 2 n): below 2 n they alias
     if (ring && cap < 2 * (uint64_t)s->n) return fail(FN_ERR_INVALID_ARG, "fn_ring_attach: capacity must be >= 2 * n_envs");
     s->ring = ring; s->ring_cap = ring ? cap : 0;
-    FN_CUDA(cudaMemsetAsync(s->d_ring_head, 0, 2 * sizeof(unsigned long long), s->stream));
+    FN_CUDA(cudaMemsetAsync(s->d_ring_head, 0, 4 * sizeof(unsigned long long), s->stream));
+    // a new ring starts without terminal observations (their indices refer to the old one)
+    cudaFree(s->term.idx); cudaFree(s->term.id); cudaFree(s->term.start);
+    s->term = TerminalDev{};
+    return FN_OK;
+}
+
+extern "C" int fn_ring_attach_terminal(fn_sim* s, float* term, uint64_t rows) {
+    if (!s) return fail(FN_ERR_INVALID_ARG, "fn_ring_attach_terminal: NULL sim");
+    if (term && !s->ring) return fail(FN_ERR_INVALID_ARG, "fn_ring_attach_terminal: attach the ring first");
+    if (term && rows < (uint64_t)s->n) return fail(FN_ERR_INVALID_ARG, "fn_ring_attach_terminal: rows must be >= n_envs (one reset may keep that many)");
+    FN_CUDA(cudaStreamSynchronize(s->stream));
+    cudaFree(s->term.idx); cudaFree(s->term.id); cudaFree(s->term.start);
+    s->term = TerminalDev{};
+    if (!term) return FN_OK;
+    cudaError_t e = cudaMalloc(&s->term.idx, s->ring_cap * sizeof(int));
+    if (e == cudaSuccess) e = cudaMalloc(&s->term.id, rows * sizeof(unsigned long long));
+    if (e == cudaSuccess) e = cudaMalloc(&s->term.start, rows * sizeof(unsigned long long));
+    if (e == cudaSuccess) e = cudaMemsetAsync(s->term.idx, 0xff, s->ring_cap * sizeof(int), s->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(s->term.id, 0xff, rows * sizeof(unsigned long long), s->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(s->term.start, 0, rows * sizeof(unsigned long long), s->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(s->d_ring_head + 2, 0, 2 * sizeof(unsigned long long), s->stream);
+    if (e != cudaSuccess) {
+        cudaFree(s->term.idx); cudaFree(s->term.id); cudaFree(s->term.start);
+        s->term = TerminalDev{};
+        return fail(e == cudaErrorMemoryAllocation ? FN_ERR_OOM : FN_ERR_CUDA, "fn_ring_attach_terminal: %s", cudaGetErrorString(e));
+    }
+    s->term.term = term; s->term.t_cap = rows; s->term.head = s->d_ring_head + 2;
     return FN_OK;
 }
 
@@ -1001,7 +1040,7 @@ extern "C" int fn_ring_sample(fn_sim* s, uint64_t seed, int n_samples, float* ou
     SampleArgs a;
     a.ring = s->ring; a.head = s->d_ring_head; a.cap = s->ring_cap; a.seed = seed; a.n_envs = s->n;
     a.row = ring_row_floats(s); a.obs = s->robot->B + 5; a.n_samples = n_samples;
-    a.out_rows = out_rows; a.out_next_obs = out_next_obs;
+    a.out_rows = out_rows; a.out_next_obs = out_next_obs; a.td = s->term;
     int grid = (n_samples + 7) / 8;
     if (grid > s->num_sms * 64) grid = s->num_sms * 64;
     FN_CUDA(launch_pdl(ring_sample_kernel, dim3(grid), dim3(256), 0, s->stream, a));

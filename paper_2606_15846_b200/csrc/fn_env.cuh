@@ -480,6 +480,7 @@ __global__ void ring_advance_kernel(unsigned long long* head, unsigned long long
     griddep_launch_dependents();
     head[0] = (head[0] + n) % cap;
     head[1] += n;
+    head[3] = head[2];                                             // terminal observations: a new batch starts (TerminalDev)
 }
 
 // ---------------------------------------------------------------- NEXT-2: uniform replay sampling
@@ -489,6 +490,25 @@ __global__ void ring_advance_kernel(unsigned long long* head, unsigned long long
 // whole rows: one warp per sample, lanes stride over the row (rows start at 4-byte alignment only), so
 // every warp instruction moves 128 contiguous bytes; the kernel is HBM-bound.
 __device__ __forceinline__ unsigned long long splitmix64_at(unsigned long long sigma, unsigned long long c);
+// Terminal observations ("Observations before reset are retained as next observations in replay"): a
+// second ring of t_cap entries of [ranges(B), d, alpha, v_x, v_y, w]; idx[ring slot] = the entry of that row,
+// id[entry] = the global id of the row the entry belongs to, start[entry] = the entries written when the step the
+// row belongs to ended.  The entries written by the resets after one step form a batch, given up as a whole as soon
+// as a later write reuses one of them: an entry is kept while its id matches and head[0] <= start + t_cap (so what
+// is kept does not depend on the order in which the envs of a reset are taken).
+struct TerminalDev {
+    float* term;                         // [t_cap][obs] or NULL = none attached
+    int* idx;                            // [ring capacity], -1 = none
+    unsigned long long* id;              // [t_cap]
+    unsigned long long* start;           // [t_cap]
+    unsigned long long* head;            // [2]: entries ever written; its value when the last step ended (= ring head words 2, 3)
+    unsigned long long t_cap;
+};
+__device__ __forceinline__ bool terminal_kept(const TerminalDev& td, const unsigned long long slot, const unsigned long long g,
+                                              const unsigned long long head_now) {
+    const int t = td.idx[slot];
+    return t >= 0 && td.id[t] == g && head_now <= td.start[t] + td.t_cap;
+}
 struct SampleArgs {
     const float* ring;
     const unsigned long long* head;      // [2]: head, rows completed
@@ -496,6 +516,7 @@ struct SampleArgs {
     int n_envs, row, obs, n_samples;
     float* out_rows;                     // [n_samples][row]
     float* out_next_obs;                 // [n_samples][obs] or NULL
+    TerminalDev td;
 };
 __global__ void __launch_bounds__(256) ring_sample_kernel(SampleArgs a) {
     griddep_wait();
@@ -508,17 +529,73 @@ __global__ void __launch_bounds__(256) ring_sample_kernel(SampleArgs a) {
     const unsigned long long first = head + a.cap - valid;
     const int lane = threadIdx.x & 31;
     for (int i = blockIdx.x * 8 + (threadIdx.x >> 5); i < a.n_samples; i += gridDim.x * 8) {
-        unsigned long long slot = first + __umul64hi(splitmix64_at(a.seed, (unsigned long long)i), valid);
+        const unsigned long long si = __umul64hi(splitmix64_at(a.seed, (unsigned long long)i), valid);
+        unsigned long long slot = first + si;
         if (slot >= a.cap) slot -= a.cap;
         if (slot >= a.cap) slot -= a.cap;
+        const unsigned long long g = total - valid + si;           // global id of the sampled row
         const float* src = a.ring + slot * (unsigned long long)a.row;
         float* dst = a.out_rows + (size_t)i * a.row;
-        for (int k = lane; k < a.row; k += 32) dst[k] = __ldg(src + k);
+        // done code of the sampled copy: a truncated row (2) whose pre-reset observation is not kept becomes 3
+        const float code = __ldg(src + a.row - 1);
+        const float* nsrc = a.ring + ((slot + (unsigned long long)a.n_envs) % a.cap) * (unsigned long long)a.row;
+        float code_out = code;
+        if (code != 0.0f) {
+            bool kept = false;
+            if (a.td.term && terminal_kept(a.td, slot, g, a.td.head[0])) {
+                nsrc = a.td.term + (unsigned long long)a.td.idx[slot] * (unsigned long long)a.obs;
+                kept = true;
+            }
+            if (code == 2.0f && !kept) code_out = 3.0f;
+        }
+        for (int k = lane; k < a.row; k += 32) dst[k] = k == a.row - 1 ? code_out : __ldg(src + k);
         if (a.out_next_obs) {
-            const float* nsrc = a.ring + ((slot + (unsigned long long)a.n_envs) % a.cap) * (unsigned long long)a.row;
             float* ndst = a.out_next_obs + (size_t)i * a.obs;
             for (int k = lane; k < a.obs; k += 32) ndst[k] = __ldg(nsrc + k);
         }
+    }
+}
+
+// Before a reset overwrites them: the observation the last step left in the pending rows of the listed envs goes
+// into the terminal ring, for every env whose last completed row (slot head - n + e, id total - n + e) has a done
+// code != 0 and is not kept yet.  One warp per listed env; entries are taken with one atomic per env (any order: a
+// call takes the same range of entries whatever the order, so what an old entry loses does not depend on it).
+struct TerminalSaveArgs {
+    const float* ring;
+    const unsigned long long* head;      // [2]: head, rows completed
+    unsigned long long cap;
+    int n_envs, row, obs;
+    const int* list;
+    const int* count_dev;
+    const int* list_par_dev;             // or NULL (see ResetArgs)
+    TerminalDev td;
+};
+__global__ void __launch_bounds__(256) terminal_save_kernel(TerminalSaveArgs a) {
+    griddep_wait();
+    griddep_launch_dependents();
+    const unsigned long long total = a.head[1], head = a.head[0];
+    if (total < (unsigned long long)a.n_envs) return;              // no step has completed a row yet
+    const int* list = a.list;
+    const int* count_dev = a.count_dev;
+    if (a.list_par_dev) { const int q = *a.list_par_dev ^ 1; list += (size_t)q * a.n_envs; count_dev += q; }
+    const int count = *count_dev;
+    const int lane = threadIdx.x & 31;
+    const unsigned long long batch_start = a.td.head[1];
+    for (int k = blockIdx.x * 8 + (threadIdx.x >> 5); k < count; k += gridDim.x * 8) {
+        const unsigned long long e = (unsigned long long)list[k];
+        const unsigned long long c = (head + a.cap - (unsigned long long)a.n_envs + e) % a.cap;
+        const unsigned long long g = total - (unsigned long long)a.n_envs + e;
+        if (a.ring[c * (unsigned long long)a.row + (unsigned long long)(a.row - 1)] == 0.0f) continue;
+        // kept already (a reset called twice)?  Such an entry belongs to this batch, and a batch has at most n <= t_cap
+        // entries, so whatever this launch has added meanwhile, head[0] <= start + t_cap holds for it.
+        if (terminal_kept(a.td, c, g, a.td.head[0])) continue;
+        unsigned long long entry = 0ull;
+        if (lane == 0) entry = atomicAdd(a.td.head, 1ull) % a.td.t_cap;
+        entry = __shfl_sync(0xffffffffu, entry, 0);
+        const float* src = a.ring + ((head + e) % a.cap) * (unsigned long long)a.row;
+        float* dst = a.td.term + entry * (unsigned long long)a.obs;
+        for (int q = lane; q < a.obs; q += 32) dst[q] = src[q];
+        if (lane == 0) { a.td.id[entry] = g; a.td.start[entry] = batch_start; a.td.idx[c] = (int)entry; }
     }
 }
 

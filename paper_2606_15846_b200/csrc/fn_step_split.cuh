@@ -124,6 +124,7 @@ __global__ void __launch_bounds__(FastShape<kCoarse>::kThreads, FastShape<kCoars
                 unsigned long long* head = const_cast<unsigned long long*>(a.ring_head);
                 head[0] = head_new;
                 head[1] += (unsigned long long)n;
+                head[3] = head[2];                                 // terminal observations: a new batch starts (TerminalDev)
             }
             end->done_ctas = 0u;
         }

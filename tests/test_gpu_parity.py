@@ -885,6 +885,95 @@ def test_replay_sampling_against_the_oracle(pu):
     s.close(); r.close(); m.close()
 
 
+def test_terminal_observations_in_replay(pu):
+    # PAPER.md:86 "Observations before reset are retained as next observations in replay, while reset observations are
+    # returned to the collector."  fn_ring_attach_terminal keeps the observation a step leaves behind for the envs that
+    # are then reset; fn_ring_sample hands it out as the next observation of their done rows and marks truncated rows
+    # whose observation is gone with code 3.  Against the oracle (fno_terminal_save / fno_ring_sample, pinned by a
+    # dictionary model) fed with the GPU's own ring before every reset: sampled rows and next observations bit for
+    # bit -- done list and explicit mask, prepared resets (C2-size batch) and plain ones, a reset called twice, envs
+    # reset without a finished episode, a terminal ring that wraps, and no terminal ring at all.
+    import torch
+    import oracle
+    from harness import workloads as W
+    for cfg, n, steps, t_rows, announce in ((5, 64, 14, 70, False), (2, 4096, 6, 4096 + 100, True)):
+        wl = W.make_workload(cfg, n_envs=n)
+        wl.forced_reset_frac = 0.06                              # truncated rows (done code 2)
+        wl.max_episode_steps = 5                                 # ... and time-outs
+        B, A = wl.n_beams, wl.action_dim
+        m, r, s = pu.make_sim(wl, n)
+        buf = pu.Buffers(n, B, A)
+        cap = 5 * n + 13
+        row = B + 5 + A + 2
+        ring = torch.zeros(cap * row, device="cuda")
+        term = torch.zeros(t_rows * (B + 5), device="cuda")
+        s.ring_attach(ring, cap)
+        s.ring_attach_terminal(term, t_rows)
+        store = oracle.TerminalStore(cap, t_rows, B)
+        ns = 999
+        rows = torch.empty(ns, row, device="cuda")
+        nxt = torch.empty(ns, B + 5, device="cuda")
+        actions = torch.from_numpy(W.action_tape(wl, steps, 4)).cuda()
+        seeds = torch.from_numpy(W.seed_tape(wl, steps + 2, 4).view(np.int64)).cuda()
+        forced = torch.from_numpy(W.forced_reset_tape(wl, steps, 4)).cuda()
+        buf.mask.fill_(1)
+        s.reset(buf.states, buf.mask, seeds[0], buf.ranges, buf.gobs)      # (no row completed yet: nothing to keep)
+        codes = set()
+        for t in range(steps):
+            buf.mask.copy_(forced[t])
+            if announce:
+                s.prepare_reset(seeds[t + 1])
+            s.step(buf.states, actions[t], float(wl.dt), buf.mask, buf.ranges, buf.col, buf.gobs)
+            torch.cuda.synchronize()
+            total = (t + 1) * n
+            store.step_ended()
+            done = buf.mask.cpu().numpy().copy()
+            lst = np.nonzero(done)[0]
+            use_mask = t % 3 == 1
+            if use_mask and t % 2 == 1:
+                done[(t * 7) % n] = 1                            # an env reset although its episode may go on
+                lst = np.nonzero(done)[0]
+            ring_np = ring.cpu().numpy().reshape(cap, row)
+            oracle.terminal_save(ring_np, cap, total, n, B, A, lst, store)
+            if use_mask:
+                buf.mask.copy_(torch.from_numpy(done))
+                s.reset(buf.states, buf.mask, seeds[t + 1], buf.ranges, buf.gobs)
+                if t % 2 == 1:                                   # the same reset again: nothing is kept twice
+                    ring_np = ring.cpu().numpy().reshape(cap, row)
+                    oracle.terminal_save(ring_np, cap, total, n, B, A, lst, store)
+                    s.reset(buf.states, buf.mask, seeds[t + 1], buf.ranges, buf.gobs)
+            else:
+                s.reset(buf.states, None, seeds[t + 1], buf.ranges, buf.gobs)
+            torch.cuda.synchronize()
+            ring_np = ring.cpu().numpy().reshape(cap, row)
+            s.ring_sample(50 + t, rows, nxt)
+            torch.cuda.synchronize()
+            er, en, slots = oracle.ring_sample(ring_np, cap, total, n, B, A, 50 + t, ns, store=store)
+            assert np.array_equal(rows.cpu().numpy(), er), f"config {cfg} step {t}: sampled rows"
+            assert np.array_equal(nxt.cpu().numpy(), en), f"config {cfg} step {t}: next observations"
+            codes |= set(er[:, -1].astype(int).tolist())
+            # the kept observation differs from the post-reset one the ring holds (so the test can tell them apart)
+            kept = (er[:, -1] == 1) | (er[:, -1] == 2)
+            if kept.any():
+                assert (en[kept] != ring_np[(slots[kept] + n) % cap, :B + 5]).any(axis=1).mean() > 0.5
+        assert {0, 1, 2} <= codes and (3 in codes or t_rows > 4000), codes
+        # no terminal ring: every truncated row is marked 3, next observations are the next rows'
+        s.ring_attach_terminal(None, 0)
+        s.ring_sample(7, rows, nxt)
+        torch.cuda.synchronize()
+        er, en, slots = oracle.ring_sample(ring_np, cap, total, n, B, A, 7, ns)
+        assert np.array_equal(rows.cpu().numpy(), er) and np.array_equal(nxt.cpu().numpy(), en)
+        assert not (er[:, -1] == 2).any()
+        with pytest.raises(fn_error()):
+            s.ring_attach_terminal(term, n - 1)
+        s.close(); r.close(); m.close()
+
+
+def fn_error():
+    import paper_2606_15846_b200 as fn
+    return fn.FlashNavError
+
+
 def test_acceleration_limits(pu):
     # NEXT-3 (reading G2): command limited to the previous applied velocity +- a_max dt.
     from harness import workloads as W

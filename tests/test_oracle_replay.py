@@ -63,10 +63,10 @@ def test_terminal_observations_against_a_dictionary_model(oracle_lib):
     # PAPER.md:86 "Observations before reset are retained as next observations in replay, while reset observations are
     # returned to the collector."  The oracle keeps them in a small second ring (fno_terminal_save) and the sampler
     # hands them out as the next observation of done rows.  Pinned against plain Python bookkeeping: a dictionary
-    # from the global row id to the observation the step left behind, a FIFO of the ids whose observation is kept.
+    # from the global row id to the observation the step left behind, and per kept id the index of the first entry
+    # written after the step it belongs to (a batch of entries is given up as soon as a later write reuses one of them).
     # Every value written anywhere is unique, so a wrong row, a wrong entry or a stale entry shows.  Covers: ring wrap,
     # terminal-ring wrap (entries lost), envs reset without a finished episode, a reset called twice, codes 1 / 2 / 3.
-    import collections
     n, B, A, cap, t_cap = 5, 3, 2, 23, 7
     row, obs = B + 5 + A + 2, B + 5
     rng = np.random.default_rng(3)
@@ -75,7 +75,9 @@ def test_terminal_observations_against_a_dictionary_model(oracle_lib):
     uniq = iter(range(1, 10 ** 6))
     new_obs = lambda: np.array([next(uniq) for _ in range(obs)], np.float32)
     left_behind = {}                                              # row id -> the observation the step left (pre-reset)
-    alive = collections.OrderedDict()                             # row ids whose terminal observation is kept, oldest first
+    kept_at = {}                                                  # row id -> entries written when its step ended
+    written = 0                                                   # entries written so far
+    alive = lambda g: g in kept_at and written <= kept_at[g] + t_cap
     was_reset = set()                                             # row ids whose env was reset right after the row
     total = 0
     for e in range(n):                                            # the first observation (a reset of all envs): pending rows
@@ -94,6 +96,8 @@ def test_terminal_observations_against_a_dictionary_model(oracle_lib):
             left_behind[total + e] = o
         total += n
         head = total % cap
+        store.step_ended()
+        batch = written
         lst = [e for e in range(n) if code[e] != 0]
         if t % 4 == 1:
             lst.append(int(rng.integers(0, n)))                   # an env reset although its episode goes on (or twice)
@@ -102,10 +106,9 @@ def test_terminal_observations_against_a_dictionary_model(oracle_lib):
             oracle_lib.terminal_save(ring, cap, total, n, B, A, lst, store)
             for e in lst:                                         # the model, in list order
                 g = total - n + e
-                if code[e] != 0 and g not in alive:
-                    alive[g] = True
-                    if len(alive) > t_cap:
-                        alive.popitem(last=False)
+                if code[e] != 0 and not alive(g):
+                    kept_at[g] = batch
+                    written += 1
             for e in lst:                                         # the reset writes the reset observation
                 ring[(head + e) % cap, :obs] = new_obs()
                 was_reset.add(total - n + e)
@@ -120,7 +123,7 @@ def test_terminal_observations_against_a_dictionary_model(oracle_lib):
             want_next = ring[(slot + n) % cap, :obs]
             c = want_row[-1]
             if c != 0:
-                if g in alive:
+                if alive(g):
                     want_next = left_behind[g]
                 elif c == 2:
                     want_row[-1] = 3
@@ -133,4 +136,4 @@ def test_terminal_observations_against_a_dictionary_model(oracle_lib):
         rows0, nxt0, _ = oracle_lib.ring_sample(ring, cap, total, n, B, A, 100 + t, 64)
         assert np.array_equal(nxt0, ring[(slots + n) % cap, :obs])
         assert not (rows0[:, -1] == 2).any() and np.array_equal(rows0[:, -1] == 3, ring[slots, -1] == 2)
-    assert seen_codes == {0, 1, 2, 3} and store.head.value > 3 * t_cap
+    assert seen_codes == {0, 1, 2, 3} and store.head.value == written > 3 * t_cap

@@ -263,6 +263,12 @@ def run_ours(args):
     if wl.ring_capacity and args.ring:
         ring = torch.zeros(wl.ring_capacity * sim.ring_row_floats(), device="cuda")
         sim.ring_attach(ring, wl.ring_capacity)
+        if args.terminal:
+            # pre-reset observations kept as next observations; an eighth of the ring's rows as entries
+            # (C5: 12 % of the envs end per step)
+            term_rows = max(n, wl.ring_capacity // 8)
+            term = torch.zeros(term_rows * (B + 5), device="cuda")
+            sim.ring_attach_terminal(term, term_rows)
     sim.reset(states, mask, seeds[tape_len], ranges, gobs)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")     # > 126 MB L2
 
@@ -522,6 +528,7 @@ def run_ours(args):
                "dtype": "f64", "data": "synthetic",
                "config": config_dict(args.config, wl),
                "launch": {"l2": "flushed between timed steps", "ring_attached": bool(ring is not None),
+                          "terminal_observations_kept": bool(ring is not None and args.terminal),
                           "fused_reset": bool(fused_active), "split_step": bool(split_step), "coarse_level": bool(coarse_active),
                           "prepared_resets": float(c1["resets_prepared"] - c0["resets_prepared"]) / max(1, c1["envs_reset"] - c0["envs_reset"])},
                "protocol": {"repetitions": R, "value": "median over repetitions", "value_iqr": [float(np.percentile(rep_values, 25)), float(np.percentile(rep_values, 75))],
@@ -643,6 +650,7 @@ def main():
     ap.add_argument("--coarse", type=int, default=-1, choices=[-1, 0, 1],
                     help="coarse level in the production beam kernels: -1 = the library's choice")
     ap.add_argument("--ring", type=int, default=1, help="attach the replay ring when the config has one (C5)")
+    ap.add_argument("--terminal", type=int, default=1, help="with the ring: keep pre-reset observations (fn_ring_attach_terminal)")
     args = ap.parse_args()
     if args.impl == "reference":
         # the counts the caller gave are honoured (same accounting as our arm); without flags a bounded sample:

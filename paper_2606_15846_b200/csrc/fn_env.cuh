@@ -594,7 +594,15 @@ __global__ void __launch_bounds__(256) terminal_save_kernel(TerminalSaveArgs a) 
         entry = __shfl_sync(0xffffffffu, entry, 0);
         const float* src = a.ring + ((head + e) % a.cap) * (unsigned long long)a.row;
         float* dst = a.td.term + entry * (unsigned long long)a.obs;
-        for (int q = lane; q < a.obs; q += 32) dst[q] = src[q];
+        int q = lane;
+        for (; q + 224 < a.obs; q += 256) {                        // eight independent 128-byte loads in flight per warp
+            float v[8];
+#pragma unroll
+            for (int u = 0; u < 8; ++u) v[u] = __ldg(src + q + 32 * u);
+#pragma unroll
+            for (int u = 0; u < 8; ++u) dst[q + 32 * u] = v[u];
+        }
+        for (; q < a.obs; q += 32) dst[q] = __ldg(src + q);
         if (lane == 0) { a.td.id[entry] = g; a.td.start[entry] = batch_start; a.td.idx[c] = (int)entry; }
     }
 }

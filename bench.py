@@ -548,7 +548,8 @@ def run_ours(args):
                "ms_per_step_p50": float(np.median(per_step_ms)), "ms_per_step_p90": float(np.percentile(per_step_ms, 90)),
                "features": feat, "replay_sample": sample, "paper_fixed_step_query": paper_query, "roofline": roofline, "cpu_baseline": cpu, "clocks": clocks,
                # per step: env step (or its motion half), beam kernel, [ring_advance unless split], then fn_reset = one fused kernel or reset + beam kernel
-               "gpu_launches": (2 + (1 if ring is not None and not split_step else 0) + (1 if fused_active else 2)) * K * R}
+               "gpu_launches": (2 + (1 if ring is not None and not split_step else 0) + (1 if fused_active else 2)
+                                + (1 if ring is not None and args.terminal else 0)) * K * R}
 
     if rank == 0:
         # HBM view of the whole step ("report HBM GB/s separately for C5"): state planes in / out,

@@ -715,6 +715,14 @@ static int launch_features(fn_sim* s, const int* list, const int* count_dev, boo
     return FN_OK;
 }
 
+// evaluation is not training: between fn_eval_begin and fn_eval_end no call touches the replay ring, its
+// head or the terminal observations
+struct RingOff {
+    fn_sim* s; float* keep;
+    explicit RingOff(fn_sim* s_) : s(s_), keep(s_->ring) { if (s->eval_mode) s->ring = nullptr; }
+    ~RingOff() { s->ring = keep; }
+};
+
 static ResetArgs reset_args(fn_sim* s, float* states, const int* list, const int* count, const int* list_par_dev,
                             const uint64_t* seeds, float* out_goal_obs) {
     ResetArgs a;
@@ -762,12 +770,7 @@ extern "C" int fn_step(fn_sim* s, float* states, const float* actions, float dt,
         return fail(FN_ERR_INVALID_ARG, "fn_step: NULL argument");
     if (!std::isfinite(dt) || dt < 0.0f) return fail(FN_ERR_INVALID_ARG, "fn_step: dt must be finite and >= 0");
     if (int rc0 = sensors_unchanged(s)) return rc0;
-    // evaluation steps are not training transitions: they never touch the replay ring or its head
-    struct RingOff {
-        fn_sim* s; float* keep;
-        explicit RingOff(fn_sim* s_) : s(s_), keep(s_->ring) { if (s->eval_mode) s->ring = nullptr; }
-        ~RingOff() { s->ring = keep; }
-    } ring_off(s);
+    RingOff ring_off(s);
     EnvArgs a;
     a.map = s->map->dev; a.robot = robot_dev(s->robot, s->map); a.task = task_dev(s->task);
     a.n = s->n; a.dt = dt; a.states = states; a.actions = actions; a.reset_mask = reset_mask;
@@ -840,6 +843,7 @@ extern "C" int fn_reset(fn_sim* s, float* states, const uint8_t* mask, const uin
     if (int rc0 = sensors_unchanged(s)) return rc0;
     if (!mask && !s->done_avail)
         return fail(FN_ERR_INVALID_ARG, "fn_reset: mask_dev == NULL needs a preceding fn_step (its done list is used once)");
+    RingOff ring_off(s);
     const int* list = mask ? s->d_list : s->d_done_list;
     const int* count = mask ? s->d_count : s->d_done_count;
     if (!mask) s->done_avail = 0;
@@ -903,6 +907,7 @@ extern "C" int fn_reset(fn_sim* s, float* states, const uint8_t* mask, const uin
 extern "C" int fn_observe_all(fn_sim* s, const float* states, float* out_ranges, float* out_goal_obs) {
     if (!s || !states || !out_ranges) return fail(FN_ERR_INVALID_ARG, "fn_observe_all: NULL argument");
     if (int rc0 = sensors_unchanged(s)) return rc0;
+    RingOff ring_off(s);
     PoseArgs a;
     a.map = s->map->dev; a.robot = robot_dev(s->robot, s->map); a.n = s->n; a.states = states;
     a.out_goal_obs = out_goal_obs; a.poses = s->d_poses; a.beam_task_counter = s->d_task_counter;

@@ -1052,6 +1052,10 @@ def test_ring_untouched_by_evaluation_and_capacity_rule(pu):
     for t in range(6):
         buf.mask.zero_()
         s.step(est, actions[3 + t], float(wl.dt), buf.mask, er, buf.col, eg)
+        if t == 2:                                                # resets and full recomputes in between are evaluation too
+            buf.mask.fill_(1)
+            s.reset(est.clone(), buf.mask, seeds[9], torch.empty_like(er), torch.empty_like(eg))
+            s.observe_all(est, torch.empty_like(er))
     s.eval_end()
     torch.cuda.synchronize()
     assert torch.equal(ring, before), "evaluation wrote into the replay ring"

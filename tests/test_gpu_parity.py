@@ -727,11 +727,14 @@ def test_prepared_reset_equals_the_plain_reset(pu):
     import torch
     from harness import workloads as W
     cases = ((2, 4096, 40, False, True), (3, 4096, 12, True, True), (1, 4000, 12, True, True),
+             (2, 4097, 9, True, True),                            # with a step limit of 3: every env ends at once, twice
              (1, 64, 40, True, False),                            # too few beams to hide a reset under: dropped
              (5, 512, 6, False, False))                           # map read through L2: no such kernel
     for cfg, n, steps, with_ring, expect_used in cases:
         wl = W.make_workload(cfg, n_envs=n)
         wl.forced_reset_frac = 0.03
+        if n == 4097:
+            wl.max_episode_steps = 3
         B, A = wl.n_beams, wl.action_dim
         actions = torch.from_numpy(W.action_tape(wl, steps, 5)).cuda()
         seeds = torch.from_numpy(W.seed_tape(wl, steps + 2, 5).view(np.int64)).cuda()
@@ -783,6 +786,8 @@ def test_prepared_reset_equals_the_plain_reset(pu):
             assert used == 0
         else:
             assert 0.5 * (c1["envs_reset"] - n) <= used < c1["envs_reset"] - n, (used, c1)
+            if n == 4097:
+                assert c1["envs_reset"] > 3 * n                   # the list was the whole batch at least twice
 
 
 def test_clearance_features_against_the_oracle(pu):

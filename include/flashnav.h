@@ -214,6 +214,37 @@ int fn_eval_begin(fn_sim* sim, float* states_dev, int n_cases, int step_limit, f
 int fn_eval_result(fn_sim* sim, uint8_t* outcome_host, int32_t* steps_host, float* return_host, int* n_running);
 int fn_eval_end(fn_sim* sim);
 
+/* ---- fn_observe_all without any allocation: ranges and goal observations of n_envs poses, no fn_sim -----------
+ * For code that may not allocate device memory where it calls us.  Two kinds of caller are meant: (1) a process in
+ * which a framework's pool (PyTorch's or JAX's allocator, an inference server) has already claimed all device
+ * memory, so that a cudaMalloc from a third-party library fails or has to be routed through that pool; (2) a
+ * control or serving loop with a latency bound, where cudaMalloc / cudaFree are ruled out because they synchronise
+ * the whole device and stall every other stream.  fn_sim_create allocates per-sim buffers (poses, lists, counters);
+ * this entry point needs no sim.  Its only working memory -- one sensing pose per env and sensor, between its two
+ * kernels, plus the beam kernel's task and ray counters -- is a fixed array compiled into the library
+ * (FN_NOALLOC_MAX_ENVS poses of 96 bytes + 256 bytes, about 0.75 MiB).  That array exists on every device that
+ * loads the library, from load until the process exits, used or not.  The call makes no cudaMalloc, cudaFree or
+ * other allocating call; it enqueues the same two kernels as fn_observe_all ("Full batch") on
+ * cuda_stream and returns without synchronising, and its outputs are bit-identical to fn_observe_all's.
+ *   map, robot:       handles made earlier, where allocating was still allowed (fn_map_create / fn_robot_create
+ *                     upload the packed map and the tables); read only.  The robot's sensors all count:
+ *                     n_envs x sensors <= FN_NOALLOC_MAX_ENVS.
+ *   states_dev:       [8][N] fp32 planes as for fn_step (x, y, psi and the goal g_x, g_y are read).
+ *   out_ranges_dev:   [N][B] fp32; out_goal_obs_dev: [2][N] fp32 or NULL.  All three are the caller's device memory.
+ * First call on each device: looks up the array's address on that device (cudaGetSymbolAddress) and raises the
+ * beam kernels' shared-memory limit, once, under a lock.  Make that first call at start-up, on the device it is
+ * for and BEFORE any stream capture begins; later calls only launch.
+ * Shared state: every call on a device uses the same array, whatever map, robot or stream it is given, and the
+ * array keeps what the last call left (the task counter is cleared by the first kernel of each call, the poses are
+ * rewritten before they are read, the ray counter just runs on).  Two calls that can overlap on the GPU -- different
+ * streams without an event between them, or two host threads -- overwrite each other's poses: order them.
+ * Errors: FN_ERR_INVALID_ARG (NULL argument, n_envs <= 0, n_envs x sensors > FN_NOALLOC_MAX_ENVS: the message says
+ * so and names fn_sim_create + fn_observe_all as the way for larger batches), FN_ERR_UNSUPPORTED (beam table larger
+ * than shared memory, n_envs x B >= 2^31), FN_ERR_CUDA. */
+enum { FN_NOALLOC_MAX_ENVS = 8192 };
+int fn_observe_noalloc(const fn_map* map, const fn_robot* robot, int n_envs, const float* states_dev,
+                       float* out_ranges_dev, float* out_goal_obs_dev, void* cuda_stream);
+
 /* ---- comparison only (not on the product path): the PAPER'S range query, "fixed-step samples along
  * each beam ... queried in distance blocks, and beams with a detected obstacle are removed from subsequent
  * blocks" (blockwise != 0), or its ablation baseline that evaluates all samples (blockwise == 0).

@@ -5,7 +5,8 @@ marshalling only; every step of the hot path runs in the library's CUDA kernels.
 device memory and the stream.  There is no CPU fallback: a missing library or device raises.
 """
 from ._binding import (FlashNavError, Map, Robot, Sim, DRIVE_DIFF, DRIVE_OMNI, N_COUNTERS, COUNTER_NAMES,
-                       load_library, measure_peak, library_path, EXPORTED_SYMBOLS)
+                       load_library, measure_peak, library_path, EXPORTED_SYMBOLS, observe_noalloc, NOALLOC_MAX_ENVS)
 
 __all__ = ["FlashNavError", "Map", "Robot", "Sim", "DRIVE_DIFF", "DRIVE_OMNI", "N_COUNTERS",
-           "COUNTER_NAMES", "load_library", "measure_peak", "library_path", "EXPORTED_SYMBOLS"]
+           "COUNTER_NAMES", "load_library", "measure_peak", "library_path", "EXPORTED_SYMBOLS",
+           "observe_noalloc", "NOALLOC_MAX_ENVS"]

@@ -18,7 +18,7 @@ COUNTER_NAMES = ("rays_cast", "map_words_loaded", "envs_reset", "reset_failures"
 EXPORTED_SYMBOLS = (
     "fn_map_create", "fn_map_set_regions", "fn_map_destroy", "fn_robot_create", "fn_robot_create_union", "fn_robot_set_sensor", "fn_robot_add_sensor", "fn_robot_set_acc_limits",
     "fn_robot_destroy", "fn_task_default", "fn_sim_create", "fn_sim_destroy", "fn_sim_set_stream", "fn_step", "fn_reset",
-    "fn_sim_bind_aux", "fn_sim_bind_features", "fn_ring_attach", "fn_ring_attach_terminal", "fn_ring_sample", "fn_ranges_fixed_step", "fn_eval_begin", "fn_eval_result", "fn_eval_end", "fn_observe_all", "fn_get_counters", "fn_sim_count_words",
+    "fn_sim_bind_aux", "fn_sim_bind_features", "fn_ring_attach", "fn_ring_attach_terminal", "fn_ring_sample", "fn_ranges_fixed_step", "fn_eval_begin", "fn_eval_result", "fn_eval_end", "fn_observe_all", "fn_observe_noalloc", "fn_get_counters", "fn_sim_count_words",
     "fn_sim_episode_state", "fn_sim_beam_config", "fn_sim_set_fused_reset", "fn_sim_set_split_step", "fn_sim_set_coarse", "fn_sim_prepare_reset", "fn_sim_profile", "fn_sim_profile_read", "fn_step_host", "fn_step_host_begin", "fn_step_host_end", "fn_measure_peak", "fn_last_error", "fn_version")
 
 
@@ -67,6 +67,7 @@ def load_library():
         "fn_ring_attach_terminal": [vp, vp, u64],
         "fn_ring_sample": [vp, u64, i32, vp, vp],
         "fn_observe_all": [vp, vp, vp, vp],
+        "fn_observe_noalloc": [vp, vp, i32, vp, vp, vp, vp],
         "fn_eval_begin": [vp, vp, i32, i32, vp, vp],
         "fn_eval_result": [vp, vp, vp, vp, vp],
         "fn_eval_end": [vp],
@@ -434,6 +435,27 @@ class Sim:
             self.close()
         except Exception:
             pass
+
+
+NOALLOC_MAX_ENVS = 8192   # FN_NOALLOC_MAX_ENVS of include/flashnav.h
+
+
+def observe_noalloc(map_: Map, robot: Robot, n_envs: int, states, out_ranges, out_goal_obs=None, stream=None):
+    """fn_observe_noalloc: what Sim.observe_all computes (ranges [N, B] and, optionally, goal obs [2, N] of the poses
+    in `states` [8, N]), for callers that may not allocate device memory at the point of the call -- all of it already
+    belongs to a framework's memory pool, or a latency bound forbids the device-wide stall of cudaMalloc.  Needs no Sim:
+    the poses between its two kernels live in a fixed ~0.75 MiB array inside the library, so n_envs x sensors is limited
+    to NOALLOC_MAX_ENVS (beyond it the call raises and names Sim.observe_all).  Every call on a device shares that
+    array: calls that could overlap on the GPU (two streams, two threads) must be ordered by the caller.  The first call
+    on a device does a one-time address lookup; make it at start-up, before any stream capture.  Enqueues on `stream`
+    (default: torch's current stream) and does not synchronise."""
+    import torch
+    n, B = int(n_envs), robot.B
+    st = torch.cuda.current_stream() if stream is None else stream
+    _check(load_library().fn_observe_noalloc(
+        map_._h, robot._h, n, _dev_ptr(states, torch.float32, 8 * n, "states"),
+        _dev_ptr(out_ranges, torch.float32, n * B, "out_ranges"), _dev_ptr(out_goal_obs, torch.float32, 2 * n, "out_goal_obs"),
+        C.c_void_p(st.cuda_stream)), "fn_observe_noalloc")
 
 
 def measure_peak(kind: int) -> float:

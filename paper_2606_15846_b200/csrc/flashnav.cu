@@ -6,6 +6,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <type_traits>
 #include <vector>
@@ -1264,3 +1265,109 @@ extern "C" int fn_step_host_end(fn_sim* s, int slot) {
     return FN_OK;
 }
 
+
+// ------------------------------------------------------------------------------------------ fn_observe_noalloc
+// fn_observe_all for callers that must not allocate device memory (include/flashnav.h says who they are).  The two
+// kernels are the ones fn_observe_all launches -- pose_from_state_kernel, then the production beam kernel -- and
+// what a sim would hold for them between the two launches lives in ONE statically sized device array instead:
+//   bytes [0, 64)    the beam kernel's counters (kNCounters x u64; only "rays cast" is touched here)
+//   bytes [128, 132) the beam kernel's dynamic task counter
+//   bytes [256, ...) the sensing poses, FN_NOALLOC_MAX_ENVS x BeamPose
+// The array is part of the loaded module: every device that loads libflashnav.so carries it (~0.75 MiB) until the
+// process exits, whether or not this entry point is ever called.
+constexpr size_t kNoallocHead = 256;
+constexpr size_t kNoallocBytes = kNoallocHead + (size_t)FN_NOALLOC_MAX_ENVS * sizeof(BeamPose);
+static_assert(kNCounters * sizeof(unsigned long long) <= 128 && kNoallocHead % alignof(BeamPose) == 0, "scratch layout");
+static __device__ __align__(256) unsigned char g_noalloc_scratch[kNoallocBytes];
+
+// In host code `g_noalloc_scratch` is only a handle for the symbol, never a device address: the address on a given
+// device comes from cudaGetSymbolAddress with that device current, and differs from device to device.
+constexpr int kNoallocMaxDevices = 64;
+struct NoallocDevice {
+    unsigned char* scratch;          // device address of g_noalloc_scratch on this device, NULL = not set up yet
+    int num_sms, max_optin;
+};
+static NoallocDevice g_noalloc_dev[kNoallocMaxDevices];
+static std::mutex g_noalloc_mutex;
+
+// once per device, with that device current (the caller holds g_noalloc_mutex)
+static int noalloc_setup(int dev, NoallocDevice* d) {
+    unsigned char* p = nullptr;
+    FN_CUDA(cudaGetSymbolAddress((void**)&p, g_noalloc_scratch));
+    if (!p) return fail(FN_ERR_CUDA, "fn_observe_noalloc: cudaGetSymbolAddress returned no address");
+    FN_CUDA(cudaDeviceGetAttribute(&d->num_sms, cudaDevAttrMultiProcessorCount, dev));
+    FN_CUDA(cudaDeviceGetAttribute(&d->max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+    // raise the beam kernels' dynamic shared-memory limit to the device's opt-in maximum (what fn_sim_create does
+    // for the sims; a function attribute, no memory involved)
+    int unused = 0;
+    FN_CUDA((beam_config<true, false>(0, d->max_optin, &unused)));
+    FN_CUDA((beam_config<true, true>(0, d->max_optin, &unused)));
+    FN_CUDA((beam_config<false, false>(0, d->max_optin, &unused)));
+    FN_CUDA((beam_config<false, true>(0, d->max_optin, &unused)));
+    d->scratch = p;
+    return FN_OK;
+}
+
+extern "C" int fn_observe_noalloc(const fn_map* map, const fn_robot* robot, int n, const float* states,
+                                  float* out_ranges, float* out_goal_obs, void* stream) {
+    if (!map || !robot || !states || !out_ranges) return fail(FN_ERR_INVALID_ARG, "fn_observe_noalloc: NULL argument");
+    if (n <= 0) return fail(FN_ERR_INVALID_ARG, "fn_observe_noalloc: n_envs must be > 0");
+    const int n_sensors = (int)robot->sensors.size();
+    if ((long long)n * n_sensors > (long long)FN_NOALLOC_MAX_ENVS)
+        return fail(FN_ERR_INVALID_ARG, "fn_observe_noalloc: n_envs x sensors = %lld is beyond the static scratch of "
+                    "FN_NOALLOC_MAX_ENVS = %d poses (use fn_sim_create + fn_observe_all for larger batches)",
+                    (long long)n * n_sensors, (int)FN_NOALLOC_MAX_ENVS);
+    if ((long long)n * robot->B >= (1ll << 31)) return fail(FN_ERR_UNSUPPORTED, "fn_observe_noalloc: n_envs * B must be < 2^31");
+    int dev = 0;
+    FN_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kNoallocMaxDevices) return fail(FN_ERR_UNSUPPORTED, "fn_observe_noalloc: device ordinal %d not supported", dev);
+    NoallocDevice d;
+    {
+        std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+        if (!g_noalloc_dev[dev].scratch)
+            if (int rc = noalloc_setup(dev, &g_noalloc_dev[dev])) return rc;
+        d = g_noalloc_dev[dev];
+    }
+    // A sim on the host stack that owns nothing: the scratch pointers go into the static array, everything a caller
+    // could bind (ring, hit cells, features, coarse level) stays off, so launch_beams picks the production kernel
+    // fn_observe_all runs for a sim without instruments.
+    fn_sim shell;
+    std::memset(&shell, 0, sizeof(shell));
+    shell.map = map; shell.robot = robot; shell.n = n; shell.stream = (cudaStream_t)stream;
+    shell.num_sms = d.num_sms; shell.n_sensors = n_sensors;
+    shell.d_counters = reinterpret_cast<unsigned long long*>(d.scratch);
+    shell.d_task_counter = reinterpret_cast<unsigned*>(d.scratch + 128);
+    shell.d_poses = reinterpret_cast<BeamPose*>(d.scratch + kNoallocHead);
+    {   // the beam launch configuration, by the rule of fn_sim_create (map staged in shared memory where it fits)
+        const size_t tab = (size_t)robot->B * sizeof(double2);
+        const size_t with_map = tab + map->n_words * sizeof(uint32_t);
+        const double Tc = (double)robot->rmax / (double)map->res;
+        const int Smin = 32 * ((map->dev.strideR < map->dev.strideC) ? map->dev.strideR : map->dev.strideC);
+        const size_t rowBits = (size_t)(map->H + 2 * kLineGuard) * map->dev.strideR * 32;
+        const size_t colBits = (size_t)(map->W + 2 * kLineGuard) * map->dev.strideC * 32;
+        shell.use_smem = with_map + 8192 <= (size_t)d.max_optin && Tc + 34.0 < 0.5 * (double)Smin &&
+                         rowBits < (1u << 20) && colBits < (1u << 20);
+        shell.beam_smem = shell.use_smem ? with_map : tab;
+        if (shell.beam_smem > (size_t)d.max_optin)
+            return fail(FN_ERR_UNSUPPORTED, "fn_observe_noalloc: beam table does not fit in shared memory (B too large)");
+        int bps = 0, bps2 = 0;
+        if (shell.use_smem) {
+            FN_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, beam_kernel<true, false>, kBeamThreads, shell.beam_smem));
+            FN_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps2, beam_kernel<true, true>, kBeamThreads, shell.beam_smem));
+        } else {
+            FN_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, beam_kernel<false, false>, kBeamThreads, shell.beam_smem));
+            FN_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps2, beam_kernel<false, true>, kBeamThreads, shell.beam_smem));
+        }
+        if (bps2 < bps) bps = bps2;
+        if (bps < 1) bps = 1;
+        shell.beam_grid = d.num_sms * bps;
+    }
+    // What must start from zero: the task counter (the pose kernel zeroes it, as for fn_observe_all).  The counters
+    // only ever accumulate and nobody reads them; the poses of all n envs are rewritten before the beam kernel reads.
+    PoseArgs a;
+    a.map = map->dev; a.robot = robot_dev(robot, map); a.n = n; a.states = states;
+    a.out_goal_obs = out_goal_obs; a.poses = shell.d_poses; a.beam_task_counter = shell.d_task_counter;
+    pose_from_state_kernel<<<(n + 255) / 256, 256, 0, shell.stream>>>(a);
+    FN_CUDA(cudaGetLastError());
+    return launch_beams(&shell, nullptr, nullptr, out_ranges);
+}

@@ -1,0 +1,128 @@
+"""fn_observe_noalloc -- the observation recompute for callers that cannot allocate device memory.
+
+Who that is: a process whose device memory already belongs, all of it, to a framework's pool (a cudaMalloc from
+inside a library then fails, or bypasses the pool's accounting), and a loop with a latency bound, where the
+device-wide stall of cudaMalloc / cudaFree is not acceptable.  fn_sim_create allocates per-sim buffers; this entry
+point takes only a map, a robot and the caller's input / output tensors, and keeps the poses between its two kernels
+in a fixed array inside the library (FN_NOALLOC_MAX_ENVS poses, ~0.75 MiB per device).
+
+Checked here: its ranges and goal observations against fn_observe_all's (the existing path: a sim with its own
+buffers) -- bit for bit, which is the bar the other GPU tests set between two launches of the same beam kernel on the
+same poses -- on two calls IN A ROW that differ in batch size and poses, so that what the first call leaves in the
+shared array (poses of envs the second call does not have, a used-up task counter) would show; that the pair of calls
+leaves the free device memory where it was; and that a batch beyond the limit is refused with a message that says so.
+
+This file sorts after every other test file on purpose (pytest -x stops at the first failure: a failure here must not
+hide the parity tests), and needs nothing from them: it passes alone in a fresh process as well as after them.
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def env():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2606_15846_b200 import build
+    build.build()
+    import paper_2606_15846_b200 as fn
+    return fn
+
+
+def _states(wl, n, seed):
+    """[8, n] fp32 planes: random poses over the map (some in occupied cells or on the border: the kernels have a
+    rule for those too), zero velocities, random goals."""
+    import torch
+    from harness import workloads as W
+    st = np.zeros((8, n), np.float32)
+    st[0:3] = W.random_poses(wl, n, seed)
+    st[6:8] = W.random_poses(wl, n, seed + 1)[0:2]
+    return torch.from_numpy(st).cuda()
+
+
+def _reference(fn, m, r, wl, states, n):
+    """The existing path: a sim (which allocates) and fn_observe_all."""
+    import torch
+    s = fn.Sim(m, r, n)
+    ranges = torch.full((n, r.B), -1.0, device="cuda")
+    gobs = torch.full((2, n), -1.0, device="cuda")
+    s.observe_all(states, ranges, gobs)
+    torch.cuda.synchronize()
+    s.close()
+    return ranges, gobs
+
+
+@pytest.mark.parametrize("cfg,n_first,n_second", [(2, 4096, 1000), (1, 64, 33), (4, 300, 301)])
+def test_two_calls_in_a_row_equal_observe_all(env, cfg, n_first, n_second):
+    # cfg 2: BASELINE.json configs[1]'s map and robot (map staged in shared memory), cfg 1 the small case,
+    # cfg 4 a map that is read through L2
+    import torch
+    fn = env
+    from harness import workloads as W
+    wl = W.make_workload(cfg, n_envs=n_first)
+    m = fn.Map(wl.occ, float(wl.resolution))
+    r = fn.Robot(wl.footprint, wl.beam_angles, float(wl.max_range), wl.drive, wl.vel_limits)
+    B = r.B
+    calls = [(n_first, _states(wl, n_first, 11)), (n_second, _states(wl, n_second, 23))]
+    expected = [_reference(fn, m, r, wl, st, n) for n, st in calls]
+    outs = [(torch.full((n, B), -2.0, device="cuda"), torch.full((2, n), -2.0, device="cuda")) for n, _ in calls]
+    # the first call on this device (if this file runs alone) does the one-time set-up; memory is compared after it
+    fn.observe_noalloc(m, r, calls[0][0], calls[0][1], outs[0][0], outs[0][1])
+    torch.cuda.synchronize()
+    free_before = torch.cuda.mem_get_info()[0]
+    outs[0][0].fill_(-2.0); outs[0][1].fill_(-2.0)
+    for (n, st), (ranges, gobs) in zip(calls, outs):              # two calls, back to back on one stream, no sync between
+        fn.observe_noalloc(m, r, n, st, ranges, gobs)
+    torch.cuda.synchronize()
+    assert torch.cuda.mem_get_info()[0] == free_before, "fn_observe_noalloc changed the free device memory"
+    for k, ((n, _), (ranges, gobs), (eranges, egobs)) in enumerate(zip(calls, outs, expected)):
+        assert torch.isfinite(ranges).all() and (ranges >= 0).all() and (ranges <= float(wl.max_range)).all()
+        if not torch.equal(ranges, eranges):
+            bad = (ranges != eranges).nonzero()[0].tolist()
+            raise AssertionError(f"call {k} (n = {n}): env {bad[0]} beam {bad[1]}: {ranges[bad[0], bad[1]].item()!r} "
+                                 f"vs fn_observe_all's {eranges[bad[0], bad[1]].item()!r}")
+        assert torch.equal(gobs, egobs), f"call {k}: goal observations differ from fn_observe_all's"
+    # the goal observation is optional
+    only_ranges = torch.full((n_second, B), -2.0, device="cuda")
+    fn.observe_noalloc(m, r, n_second, calls[1][1], only_ranges)
+    torch.cuda.synchronize()
+    assert torch.equal(only_ranges, expected[1][0])
+    r.close(); m.close()
+
+
+def test_batches_beyond_the_static_scratch_are_refused(env):
+    import torch
+    fn = env
+    from harness import workloads as W
+    wl = W.make_workload(1)
+    m = fn.Map(wl.occ, float(wl.resolution))
+    r = fn.Robot(wl.footprint, wl.beam_angles, float(wl.max_range), wl.drive, wl.vel_limits)
+    n = fn.NOALLOC_MAX_ENVS + 1
+    st = _states(wl, n, 5)
+    ranges = torch.full((n, r.B), -2.0, device="cuda")
+    with pytest.raises(fn.FlashNavError, match="FN_NOALLOC_MAX_ENVS"):
+        fn.observe_noalloc(m, r, n, st, ranges)
+    torch.cuda.synchronize()
+    assert (ranges == -2.0).all(), "a refused call must not launch anything"
+    # exactly at the limit it runs
+    n = fn.NOALLOC_MAX_ENVS
+    ranges = torch.full((n, r.B), -2.0, device="cuda")
+    st = _states(wl, n, 6)
+    fn.observe_noalloc(m, r, n, st, ranges)
+    eranges, _ = _reference(fn, m, r, wl, st, n)
+    assert torch.equal(ranges, eranges)
+    # a second sensor doubles the poses per env: half the limit still fits, one env more does not
+    r.add_sensor(W.beam_table(40, 120.0), 3.0, 0.1, 0.0, 0.5)
+    half = fn.NOALLOC_MAX_ENVS // 2
+    st = _states(wl, half + 1, 7)
+    with pytest.raises(fn.FlashNavError, match="FN_NOALLOC_MAX_ENVS"):
+        fn.observe_noalloc(m, r, half + 1, st, torch.empty(half + 1, r.B, device="cuda"))
+    st = _states(wl, half, 8)
+    ranges = torch.full((half, r.B), -2.0, device="cuda")
+    fn.observe_noalloc(m, r, half, st, ranges)
+    eranges, _ = _reference(fn, m, r, wl, st, half)
+    assert torch.equal(ranges, eranges)
+    r.close(); m.close()

@@ -279,8 +279,18 @@ int fn_sim_set_coarse(fn_sim* sim, int enable, int* active_out);
  * Results are bit-identical with and without the announcement (tested).  The announcement serves one fn_step; it is
  * a hint and is dropped -- fn_reset then does the whole reset -- when the sim has no such kernel (map read through
  * L2, several sensors, instruments bound, coarse level, evaluation mode), when fn_reset is called with a mask or
- * other seeds, or when fn_map_set_regions / fn_robot_set_sensor ran in between.  seeds_dev [N] is READ DURING
- * fn_step and must hold the same values until fn_reset.  seeds_dev = NULL withdraws an announcement.
+ * other seeds, or when fn_map_set_regions / fn_robot_set_sensor ran in between.  seeds_dev = NULL withdraws an
+ * announcement.
+ * CONTRACT (not checkable by the library): seeds_dev [N] is READ DURING fn_step, and fn_reset recognises the
+ * announcement by the ADDRESS of its seeds argument.  The buffer must hold the same values from fn_step until
+ * fn_reset has been enqueued behind it; a buffer rewritten in place in between (one persistent seeds array refilled
+ * every step) silently yields resets drawn from the values it held during fn_step, which then differ from the
+ * un-announced path's (tests/test_gpu_parity.py pins this behaviour).  Refill before fn_sim_prepare_reset, or
+ * alternate two buffers.
+ * The fn_reset that applies a prepared reset starts under the tail of the preceding work in the stream, but writes
+ * nothing of the caller's -- states, ranges, goal observations -- before that work has completed: a kernel the caller
+ * enqueues between fn_step and fn_reset to read the pre-reset observation is safe, with or without programmatic
+ * dependent launch.
  * Errors: FN_ERR_INVALID_ARG (NULL sim), FN_ERR_OOM / FN_ERR_CUDA (first call: the sim's buffers, 177 bytes per env). */
 int fn_sim_prepare_reset(fn_sim* sim, const uint64_t* seeds_dev);
 

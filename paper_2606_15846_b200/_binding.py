@@ -386,7 +386,13 @@ class Sim:
 
     def prepare_reset(self, seeds):
         """Announce the seeds of the reset(mask=None) that follows the NEXT step(): that step then also prepares the
-        reset of the envs it reports done (same results, the reset's latency leaves the critical path).  None withdraws."""
+        reset of the envs it reports done (same results, the reset's latency leaves the critical path).  None withdraws.
+
+        CONTRACT: the values in `seeds` are read DURING the next step(), and reset() recognises the announcement by the
+        tensor's ADDRESS.  Do not write into this tensor between that step() and its reset(): a tensor refilled in place
+        in between yields resets drawn from the old values, silently (the library cannot see the write; this binding
+        only keeps the tensor alive).  With one persistent seeds tensor per loop, refill it BEFORE prepare_reset(), or
+        alternate between two tensors."""
         import torch
         if seeds is not None and seeds.dtype not in (torch.int64, torch.uint64):
             raise FlashNavError("seeds must be a 64-bit integer tensor")

@@ -925,6 +925,7 @@ extern "C" int fn_observe_all(fn_sim* s, const float* states, float* out_ranges,
 extern "C" int fn_ranges_fixed_step(fn_sim* s, const float* states, float delta_m, int blockwise, float* out_ranges) {
     if (!s || !states || !out_ranges) return fail(FN_ERR_INVALID_ARG, "fn_ranges_fixed_step: NULL argument");
     if (!(delta_m > 0.0f) || !std::isfinite(delta_m)) return fail(FN_ERR_INVALID_ARG, "fn_ranges_fixed_step: delta must be > 0");
+    if (int rc0 = sensors_unchanged(s)) return rc0;              // (the pose kernel writes one pose per LIVE sensor)
     if (s->n_sensors != 1) return fail(FN_ERR_UNSUPPORTED, "fn_ranges_fixed_step: comparison query, single-sensor robots only");
     PoseArgs a;
     a.map = s->map->dev; a.robot = robot_dev(s->robot, s->map); a.n = s->n; a.states = states;
@@ -994,6 +995,7 @@ extern "C" int fn_sim_bind_aux(fn_sim* s, int32_t* hit, float* reward) {
 
 extern "C" int fn_sim_bind_features(fn_sim* s, int n_sectors, float* out_z) {
     if (!s) return fail(FN_ERR_INVALID_ARG, "fn_sim_bind_features: NULL sim");
+    if (out_z) if (int rc0 = sensors_unchanged(s)) return rc0;   // (B below is the live robot's row length)
     if (out_z && s->n_sensors != 1) return fail(FN_ERR_UNSUPPORTED, "fn_sim_bind_features: single-sensor robots only");
     if (out_z && (n_sectors < 1 || n_sectors > s->robot->B))
         return fail(FN_ERR_INVALID_ARG, "fn_sim_bind_features: n_sectors must be in 1..B");
@@ -1145,15 +1147,15 @@ extern "C" int fn_step_host(fn_sim* s, float* states, const float* actions, floa
     if (!s || !states || !actions || !mask || !out_ranges || !out_collision || !out_goal_obs)
         return fail(FN_ERR_INVALID_ARG, "fn_step_host: NULL argument");
     const size_t n = (size_t)s->n, B = (size_t)s->robot->B, A = s->robot->drive == FN_DRIVE_DIFF ? 2 : 3;
-    if (!s->stg_states) {
-        FN_CUDA(cudaMalloc(&s->stg_states, 8 * n * sizeof(float)));
-        FN_CUDA(cudaMalloc(&s->stg_actions, n * A * sizeof(float)));
-        FN_CUDA(cudaMalloc(&s->stg_ranges, n * B * sizeof(float)));
-        FN_CUDA(cudaMalloc(&s->stg_gobs, 2 * n * sizeof(float)));
-        FN_CUDA(cudaMalloc(&s->stg_mask, n));
-        FN_CUDA(cudaMalloc(&s->stg_col, n));
-        FN_CUDA(cudaMalloc(&s->stg_seeds, n * sizeof(unsigned long long)));
-    }
+    // each staging buffer on its own: the pipelined entry points share stg_states (pipe_alloc) and allocate none of
+    // the others, and an allocation that failed half way must be completed by the next call, not skipped
+    if (!s->stg_states) FN_CUDA(cudaMalloc(&s->stg_states, 8 * n * sizeof(float)));
+    if (!s->stg_actions) FN_CUDA(cudaMalloc(&s->stg_actions, n * A * sizeof(float)));
+    if (!s->stg_ranges) FN_CUDA(cudaMalloc(&s->stg_ranges, n * B * sizeof(float)));
+    if (!s->stg_gobs) FN_CUDA(cudaMalloc(&s->stg_gobs, 2 * n * sizeof(float)));
+    if (!s->stg_mask) FN_CUDA(cudaMalloc(&s->stg_mask, n));
+    if (!s->stg_col) FN_CUDA(cudaMalloc(&s->stg_col, n));
+    if (!s->stg_seeds) FN_CUDA(cudaMalloc(&s->stg_seeds, n * sizeof(unsigned long long)));
     cudaStream_t st = s->stream;
     FN_CUDA(cudaMemcpyAsync(s->stg_states, states, 8 * n * sizeof(float), cudaMemcpyHostToDevice, st));
     FN_CUDA(cudaMemcpyAsync(s->stg_actions, actions, n * A * sizeof(float), cudaMemcpyHostToDevice, st));

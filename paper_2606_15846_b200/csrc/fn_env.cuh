@@ -801,19 +801,38 @@ __device__ __forceinline__ void reset_env(const ResetArgs& a, const MapDev& mp, 
 }
 
 // The stores of reset_env for env e from a prepared reset (one thread): a = the arguments of the fn_reset call.
-// _early: what the step no longer touches once its outcome warps have finished (states, episode bookkeeping, goal
-// observation, counters); _late: what it uses until it completes (the sensing pose its beams are cast from, the ring
-// head).  The prepared values are read past L1 (written by a kernel that may still be running).
+// _early: what belongs to the SIM and the step no longer touches once its outcome warps have finished (episode
+// bookkeeping, counters); _late: what the step uses until it completes (the sensing pose its beams are cast from, the
+// ring head) and everything that is the CALLER'S -- state planes and goal observation: fn_step hands them out as the
+// pre-reset observation, so a kernel of the caller between fn_step and fn_reset may still be reading them when this
+// kernel becomes resident (a reader that releases its dependents early); they are loaded before the dependency wait
+// (HeldState) and stored after it.  The prepared values are read past L1 (written by a kernel that may still be running).
 __device__ __forceinline__ void reset_apply_early(const ResetArgs& a, const PreparedReset& pr, const int e) {
-    const int n = a.n;
-#pragma unroll
-    for (int k = 0; k < 8; ++k) a.states[k * n + e] = __ldcg(pr.states + k * n + e);
     a.d_prev[e] = __ldcg(pr.d_prev + e);
     a.ep_step[e] = 0;
-    if (a.out_goal_obs) { a.out_goal_obs[e] = __ldcg(pr.goal_obs + e); a.out_goal_obs[n + e] = __ldcg(pr.goal_obs + n + e); }
     atomicAdd(&a.counters[kResets], 1ull);
     atomicAdd(&a.counters[kResetsPrepared], 1ull);
     if (__ldcg(pr.fail + e)) atomicAdd(&a.counters[kResetFail], 1ull);
+}
+struct HeldState {                       // prepared state planes and goal observation read before they may be stored
+    int e;                               // -1: none
+    float st[8], g[2];
+};
+__device__ __forceinline__ HeldState reset_state_held(const ResetArgs& a, const PreparedReset& pr, const int e) {
+    HeldState h;
+    h.e = e;
+    const int n = a.n;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) h.st[k] = __ldcg(pr.states + k * n + e);
+    h.g[0] = __ldcg(pr.goal_obs + e); h.g[1] = __ldcg(pr.goal_obs + n + e);
+    return h;
+}
+__device__ __forceinline__ void reset_state_store(const ResetArgs& a, const HeldState& h) {
+    if (h.e < 0) return;
+    const int n = a.n;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) a.states[k * n + h.e] = h.st[k];
+    if (a.out_goal_obs) { a.out_goal_obs[h.e] = h.g[0]; a.out_goal_obs[n + h.e] = h.g[1]; }
 }
 struct HeldPose {                        // a prepared sensing pose read before it may be stored
     int e;                               // -1: none

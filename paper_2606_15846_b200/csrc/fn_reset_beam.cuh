@@ -119,7 +119,10 @@ __global__ void __launch_bounds__(kFusedThreads, 2) reset_beam_kernel(const __gr
 // and the prepared poses -- is complete since the step's outcome warps finished (tens of us earlier; they count
 // themselves in end->outcomes_done).  So the work is done BEFORE the dependency wait, under the step kernel's tail:
 // the ranges are held in registers, and only the stores wait for the step to complete (it writes the terminal
-// observation into the same rows, reads the sensing poses the copies replace, and advances the ring head).  The
+// observation into the same rows, reads the sensing poses the copies replace, and advances the ring head).  Nothing
+// of the CALLER'S is written before the wait either -- ranges, state planes, goal observation: whatever the caller
+// launched between fn_step and fn_reset to read the pre-reset observation completes first (only the sim's own
+// episode bookkeeping and counters, which no one else can see before the stream reaches them, go early).  The
 // CTAs arrive in the order of their index over ~8 us, as the step's CTAs leave (measured with globaltimer stamps).  Waiting for a flag of the kernel BEFORE this one needs no co-residency: the step's
 // warps never wait for anything.
 constexpr unsigned kCopyFirstCta = 48u;
@@ -163,13 +166,15 @@ __global__ void __launch_bounds__(kBeamThreads, 2) prepared_reset_kernel(const _
     held.store = false;
     HeldPose hp;                                                   // (the first group's: longer lists copy the rest after the wait)
     hp.e = -1;
+    HeldState hs;                                                  // the caller's arrays are written after the wait only
+    hs.e = -1;
     if (service) {
         for (unsigned g = g0; g < ngroups; g += gridDim.x) {
             const unsigned k = (g << 3) + lane;
             if (lane < 8u && k < count) {
                 const int e = __ldcg(rlist + k);
                 reset_apply_early(ra, pr, e);
-                if (g == g0) hp = reset_pose_held(ra, pr, e);
+                if (g == g0) { hp = reset_pose_held(ra, pr, e); hs = reset_state_held(ra, pr, e); }
             }
         }
     } else {
@@ -189,9 +194,14 @@ __global__ void __launch_bounds__(kBeamThreads, 2) prepared_reset_kernel(const _
     fast_store_held(a, held, ring_head);
     if (service) {
         reset_pose_store(ra, hp);
+        reset_state_store(ra, hs);
         for (unsigned g = g0; g < ngroups; g += gridDim.x) {
             const unsigned k = (g << 3) + lane;
-            if (lane < 8u && k < count) reset_apply_late(ra, pr, rlist[k], g != g0);
+            if (lane < 8u && k < count) {
+                const int e = rlist[k];
+                if (g != g0) reset_state_store(ra, reset_state_held(ra, pr, e));
+                reset_apply_late(ra, pr, e, g != g0);
+            }
         }
     }
     // what a long list leaves over, shared by all warps in the usual way

@@ -357,7 +357,9 @@ def test_several_sensors_against_the_oracle(pu):
             big = torch.zeros(n, r.B, device="cuda")              # (sized for the new row, so that the library decides)
             for call in (lambda: s.step(buf.states, actions[0], float(wl.dt), buf.mask, big, buf.col, buf.gobs),
                          lambda: s.reset(buf.states, buf.mask, seeds[0], big, buf.gobs),
-                         lambda: s.observe_all(buf.states, big)):
+                         lambda: s.observe_all(buf.states, big),
+                         lambda: s.ranges_fixed_step(buf.states, 0.025, True, big),
+                         lambda: s.bind_features(4, torch.zeros(n, 4, device="cuda"))):
                 with pytest.raises(fn.FlashNavError, match="sensors changed"):
                     call()
             torch.cuda.synchronize()
@@ -620,6 +622,44 @@ def test_step_host_equals_the_device_calls(pu):
     s.close(); r.close(); m.close()
 
 
+def test_step_host_after_the_pipelined_form_on_one_sim(pu):
+    # The two host entry points share one staging buffer (the states) and each has others of its own: a sim that has
+    # served fn_step_host_begin / _end must still serve fn_step_host (it answered FN_ERR_CUDA: copies to buffers it
+    # had skipped allocating), and the other way round.  Sim A: pipelined step 0, fn_step_host step 1, pipelined
+    # step 2; sim B: fn_step_host for all three.  Outputs must agree bit for bit.
+    import torch
+    from harness import workloads as W
+    wl = W.make_workload(1, n_envs=96)
+    n, B, A = wl.n_envs, wl.n_beams, wl.action_dim
+    act = W.action_tape(wl, 3, 4)
+    seeds = W.seed_tape(wl, 4, 4).view(np.int64)
+    outs = {}
+    for name in ("A", "B"):
+        m, r, s = pu.make_sim(wl, n)
+        dev = pu.Buffers(n, B, A)
+        dev.mask.fill_(1)
+        s.reset(dev.states, dev.mask, torch.from_numpy(seeds[0]).cuda(), dev.ranges, dev.gobs)
+        torch.cuda.synchronize()
+        hs = dev.states.cpu().pin_memory()
+        hr, hg = torch.zeros(n, B).pin_memory(), torch.zeros(2, n).pin_memory()
+        hm, hc = torch.zeros(n, dtype=torch.uint8).pin_memory(), torch.zeros(n, dtype=torch.uint8).pin_memory()
+        got = []
+        for t in range(3):
+            ha, hq = torch.from_numpy(act[t]).pin_memory(), torch.from_numpy(seeds[t + 1]).pin_memory()
+            hm.zero_()
+            if name == "A" and t != 1:
+                s.step_host_begin(0, hs, ha, float(wl.dt), hm, hq, hs, hr, hc, hg)
+                s.step_host_end(0)
+            else:
+                s.step_host(hs, ha, float(wl.dt), hm, hq, hr, hc, hg)
+            got.append([x.numpy().copy() for x in (hs, hr, hg, hm, hc)])
+        outs[name] = got
+        s.close(); r.close(); m.close()
+    for t in range(3):
+        for a, b in zip(outs["A"][t], outs["B"][t]):
+            assert np.array_equal(a, b), f"step {t}"
+
+
 def test_split_step_equals_the_single_env_step_kernel(pu):
     # fn_step either runs one env-step kernel, the ring-advance kernel and the beam kernel, or (default) a
     # motion kernel and a beam kernel whose last warps compute collision / goal / reward / done for the envs
@@ -788,6 +828,45 @@ def test_prepared_reset_equals_the_plain_reset(pu):
             assert 0.5 * (c1["envs_reset"] - n) <= used < c1["envs_reset"] - n, (used, c1)
             if n == 4097:
                 assert c1["envs_reset"] > 3 * n                   # the list was the whole batch at least twice
+
+
+def test_prepared_reset_takes_the_seed_values_of_the_step(pu):
+    # The contract of fn_sim_prepare_reset, pinned from its sharp side: the announced buffer is READ DURING fn_step,
+    # and the library recognises the announcement at fn_reset by the buffer's address.  A caller that keeps one seeds
+    # tensor and rewrites it in place between fn_step and fn_reset therefore gets the resets drawn from the values the
+    # buffer held during the step -- not from the new ones, and unlike the un-announced path.  (Header, binding
+    # docstring and README say so: announce a buffer that stays untouched until fn_reset, e.g. two alternating ones.)
+    import torch
+    from harness import workloads as W
+    n = 4096
+    wl = W.make_workload(2, n_envs=n)
+    wl.forced_reset_frac = 0.05
+    B, A = wl.n_beams, wl.action_dim
+    actions = torch.from_numpy(W.action_tape(wl, 1, 3)).cuda()
+    tape = torch.from_numpy(W.seed_tape(wl, 3, 3).view(np.int64)).cuda()
+    forced = torch.from_numpy(W.forced_reset_tape(wl, 1, 3)).cuda()
+    res = {}
+    for name in ("announced, refilled in place", "plain, old seeds", "plain, new seeds"):
+        m, r, s = pu.make_sim(wl, n)
+        buf = pu.Buffers(n, B, A)
+        buf.mask.fill_(1)
+        s.reset(buf.states, buf.mask, tape[0], buf.ranges, buf.gobs)
+        buf.mask.copy_(forced[0])
+        live = tape[1].clone()                                    # the caller's one persistent seeds tensor
+        if name.startswith("announced"):
+            s.prepare_reset(live)
+        s.step(buf.states, actions[0], float(wl.dt), buf.mask, buf.ranges, buf.col, buf.gobs)
+        if name != "plain, old seeds":
+            live.copy_(tape[2])                                   # rewritten between fn_step and fn_reset
+        s.reset(buf.states, None, live, buf.ranges, buf.gobs)
+        torch.cuda.synchronize()
+        res[name] = (buf.states.clone(), buf.ranges.clone(), buf.gobs.clone(), s.counters())
+        s.close(); r.close(); m.close()
+    a, old, new = res["announced, refilled in place"], res["plain, old seeds"], res["plain, new seeds"]
+    assert a[3]["resets_prepared"] > 0.03 * n and old[3]["resets_prepared"] == 0
+    for k in range(3):
+        assert torch.equal(a[k], old[k]), "a prepared reset uses the seed values the buffer held during fn_step"
+    assert not torch.equal(a[0], new[0])
 
 
 def test_clearance_features_against_the_oracle(pu):

@@ -18,7 +18,6 @@ from __future__ import annotations
 import argparse
 import json
 import os
-import subprocess
 import sys
 import threading
 import time
@@ -547,8 +546,12 @@ def run_ours(args):
                                       "beam_reset": prof["beam_reset"][0] / K},
                "ms_per_step_p50": float(np.median(per_step_ms)), "ms_per_step_p90": float(np.percentile(per_step_ms, 90)),
                "features": feat, "replay_sample": sample, "paper_fixed_step_query": paper_query, "roofline": roofline, "cpu_baseline": cpu, "clocks": clocks,
-               # per step: env step (or its motion half), beam kernel, [ring_advance unless split], then fn_reset = one fused kernel or reset + beam kernel
-               "gpu_launches": (2 + (1 if ring is not None and not split_step else 0) + (1 if fused_active else 2)
+               # per step: env step (or its motion half), beam kernel, [ring_advance unless split], [terminal_save with a
+               # terminal ring], then fn_reset = ONE kernel when the step prepared the resets (prepared_reset_kernel; read
+               # off the resets_prepared counter of the timed region, not assumed) or when the fused reset serves the done
+               # list, else reset kernel + beam kernel
+               "gpu_launches": (2 + (1 if ring is not None and not split_step else 0)
+                                + (1 if (c1["resets_prepared"] > c0["resets_prepared"] or fused_active) else 2)
                                 + (1 if ring is not None and args.terminal else 0)) * K * R}
 
     if rank == 0:
@@ -614,7 +617,10 @@ def run_ours(args):
         d2h = 8 * n * 4 + n * B * 4 + 2 * n * 4 + n + n
         d2h_pipe = d2h
         h2d_pipe = n * A * 4 + n + n * 8                         # the states stay on the device between steps
+        # e2e.value: since round 2 the PIPELINED public calls (round 1 reported the serial fn_step_host here, which has
+        # been e2e.serial since; BASELINE.md and DESIGN.md 10 state the change) -- compare round 1's e2e.value with e2e.serial
         out["e2e"] = {"value": world * n * Ke / float(te[1]), "unit": UNIT, "h2d_bytes_per_step": h2d_pipe, "d2h_bytes_per_step": d2h_pipe,
+                      "definition": "pipelined (fn_step_host_begin / _end); round 1's e2e.value is e2e.serial here",
                       "steps": Ke, "note": "fn_step_host_begin / _end over two slots: pinned host buffers; per step H2D of actions, mask "
                                            "and seeds, fn_step + fn_reset, D2H of states, ranges, flags and goal obs on a copy stream "
                                            "that overlaps the next step's kernels; every step's outputs are awaited",

@@ -74,7 +74,7 @@ def check_observation(wl, rep, x, y, psi, g_ranges, g_hit, env_idx=None, tag="ob
     ok = amb == 0
     rep.add("beams", ok.size)
     rep.add("beams_ambiguous", (~ok).sum())
-    bad_hit = ok & (g_hit != hit)
+    bad_hit = ok & (g_hit != hit) if g_hit is not None else np.zeros_like(ok)    # (the production kernel gives no hit cells)
     bad_r = ok & (np.abs(g_ranges.astype(np.float64) - r.astype(np.float64)) > TOL_RANGE)
     if bad_hit.any() or bad_r.any():
         e, b = np.nonzero(bad_hit | bad_r)
@@ -82,7 +82,7 @@ def check_observation(wl, rep, x, y, psi, g_ranges, g_hit, env_idx=None, tag="ob
         raise AssertionError(
             f"{tag}: {bad_hit.sum()} hit-cell and {bad_r.sum()} range mismatches outside near-ties; first: env "
             f"{(env_idx[e[k]] if env_idx is not None else e[k])} beam {b[k]} pose=({x[e[k]]!r},{y[e[k]]!r},{psi[e[k]]!r}) "
-            f"gpu r={g_ranges[e[k], b[k]]!r} hit={g_hit[e[k], b[k]]} oracle r={r[e[k], b[k]]!r} hit={hit[e[k], b[k]]}")
+            f"gpu r={g_ranges[e[k], b[k]]!r} hit={g_hit[e[k], b[k]] if g_hit is not None else None} oracle r={r[e[k], b[k]]!r} hit={hit[e[k], b[k]]}")
     # ambiguous beams must still be sane
     assert np.all(np.isfinite(g_ranges)) and g_ranges.min() >= 0 and g_ranges.max() <= float(wl.max_range) + 1e-6
 
@@ -253,6 +253,116 @@ def run_parity(wl, steps, n=None, subset=None, seed=0, forced=None, check_every=
     rep.add("rays_cast", cnt["rays_cast"])
     assert cnt["oob_window_loads"] == 0, "the instrumented beam kernel read a window outside the packed map"
     assert cnt["reset_failures"] == rep.c.get("reset_failures", 0) or check_every > 1
+    s.close(); r.close(); m.close()
+    assert_ambiguity_bounds(rep)
+    return rep
+
+
+def run_production_parity(wl, steps, n=None, subset=None, seed=0, full_steps=(0, 1, 2), ring=False):
+    """The launch sequence bench.py TIMES, held against the oracle directly: no hit cells bound (so fn_step runs the
+    production step kernel, not the instrumented one), the reset seeds announced before every step
+    (fn_sim_prepare_reset), fn_reset(mask = NULL) of the step's done list.  Everything the production kernels return
+    is compared with the oracle at the usual tolerances -- state planes, collision flags, goal obs, done, reward,
+    reset states, and the RANGES (of `subset` envs per step, of all envs on `full_steps`); hit cells are the one thing
+    these kernels cannot give.  Asserts that the prepared path served resets where the sim has it."""
+    n = wl.n_envs if n is None else n
+    wl.n_envs = n
+    B, A = wl.n_beams, wl.action_dim
+    comp = getattr(wl, "components", None)
+    m, r, s = make_sim(wl, n)
+    buf = Buffers(n, B, A)
+    s.bind_aux(None, buf.reward)                                        # the reward is an output, not an instrument
+    ring_t = None
+    if ring:
+        cap = 3 * n + 5
+        ring_t = torch.zeros(cap * s.ring_row_floats(), device="cuda")
+        s.ring_attach(ring_t, cap)
+    actions = torch.from_numpy(W.action_tape(wl, steps, seed)).cuda()
+    seeds_np = W.seed_tape(wl, steps + 1, seed)
+    seeds_t = torch.from_numpy(seeds_np.view(np.int64)).cuda()
+    forced_np = W.forced_reset_tape(wl, steps, seed)
+    rng = np.random.default_rng(seed + 99)
+    sel = np.arange(n) if subset is None or subset >= n else np.sort(rng.choice(n, subset, replace=False))
+    rep = Report()
+    sensor = getattr(wl, "sensor", None)
+
+    def check_reset(mask_np, seeds_row, pre, d_prev0, ep0, keep_r, tag):
+        post = buf.states.cpu().numpy()
+        ref = pre.copy()
+        d_prev, ep = d_prev0.copy(), ep0.copy()
+        amb, failed = oracle.reset(wl.occ, wl.resolution, wl.footprint, wl.regions, wl.goal_dist_min,
+                                   wl.goal_dist_max, mask_np, seeds_row, ref, d_prev, ep, components=comp)
+        okm = (mask_np != 0) & (amb == 0)
+        rep.add("resets", (mask_np != 0).sum())
+        rep.add("resets_ambiguous", ((mask_np != 0) & (amb != 0)).sum())
+        assert np.array_equal(post[:, mask_np == 0], pre[:, mask_np == 0]), f"{tag}: reset touched other envs"
+        if not np.array_equal(post[:, okm], ref[:, okm]):
+            e = np.nonzero(okm & np.any(post != ref, axis=0))[0][0]
+            raise AssertionError(f"{tag}: reset state differs for env {e}: gpu {post[:, e]} oracle {ref[:, e]}")
+        gd, ge = s.episode_state()
+        assert np.array_equal(ge[okm], ep[okm]) and np.allclose(gd[okm], d_prev[okm], atol=1e-5)
+        rg = buf.ranges.cpu().numpy()
+        assert np.array_equal(rg[mask_np == 0], keep_r[mask_np == 0]), f"{tag}: recompute touched other rows"
+        idx = np.nonzero(okm)[0]
+        if subset is not None and idx.size > subset:
+            idx = idx[:subset]
+        if idx.size:
+            check_observation(wl, rep, post[0, idx], post[1, idx], post[2, idx], rg[idx], None, idx, tag + "/recompute")
+            g = buf.gobs.cpu().numpy()
+            og = oracle.goal_obs(post[0, idx], post[1, idx], post[2, idx], post[6, idx], post[7, idx])
+            assert np.all(close_state(g[0, idx], og[0])) and np.all(ang_diff(g[1, idx], og[1]) <= 1e-5)
+
+    pre = buf.states.cpu().numpy()
+    d0, e0 = s.episode_state()
+    buf.mask.fill_(1)
+    s.reset(buf.states, buf.mask, seeds_t[0], buf.ranges, buf.gobs)
+    torch.cuda.synchronize()
+    check_reset(np.ones(n, np.uint8), seeds_np[0], pre, d0, e0, buf.ranges.cpu().numpy(), "initial reset")
+
+    for t in range(steps):
+        pre = buf.states.cpu().numpy()
+        d_prev0, ep0 = s.episode_state()
+        buf.mask.copy_(torch.from_numpy(forced_np[t]))
+        s.prepare_reset(seeds_t[t + 1])                                 # what bench.py does
+        s.step(buf.states, actions[t], float(wl.dt), buf.mask, buf.ranges, buf.col, buf.gobs)
+        torch.cuda.synchronize()
+        done = buf.mask.cpu().numpy()
+        post = buf.states.cpu().numpy()
+        ref = oracle.motion(wl.drive, wl.vel_limits, wl.dt, pre, actions[t].cpu().numpy(), acc=getattr(wl, "acc_limits", None))
+        for p in (0, 1, 3, 4, 5, 6, 7):
+            assert np.all(close_state(post[p], ref[p])), f"step {t}: state plane {p}"
+        assert np.all(ang_diff(post[2], ref[2]) <= TOL_STATE * np.maximum(1, np.abs(ref[2]))), f"step {t}: psi"
+        x, y, psi = post[0], post[1], post[2]
+        flag, camb = oracle.collision(wl.occ, wl.resolution, wl.footprint, x, y, psi, components=comp)
+        gcol = buf.col.cpu().numpy()
+        okc = camb == 0
+        rep.add("collision_checks", n)
+        rep.add("collision_ambiguous", (~okc).sum())
+        assert np.array_equal(gcol[okc], flag[okc]), f"step {t}: collision flags"
+        og = oracle.goal_obs(x, y, psi, post[6], post[7])
+        g = buf.gobs.cpu().numpy()
+        assert np.all(close_state(g[0], og[0])), f"step {t}: goal distance"
+        assert np.all(ang_diff(g[1], og[1])[og[0] > 1e-3] <= 1e-5), f"step {t}: goal direction"
+        d_prev, ep = d_prev0.copy(), ep0.copy()
+        tie = (np.abs(og[0].astype(np.float64) - float(wl.goal_tol)) < 1e-5) | ~okc
+        rep.add("done_checks", n)
+        rep.add("done_ambiguous", tie.sum())
+        rew, odone = oracle.reward_done(og[0], flag, forced_np[t], d_prev, ep, float(wl.goal_tol), wl.max_episode_steps,
+                                        float(wl.r_success), float(wl.r_collision), float(wl.c_progress))
+        assert np.array_equal(done[~tie], odone[~tie]), f"step {t}: done flags"
+        assert np.allclose(buf.reward.cpu().numpy()[~tie], rew[~tie], atol=1e-4), f"step {t}: reward"
+        selt = np.arange(n) if t in full_steps else sel
+        rg = buf.ranges.cpu().numpy()
+        check_observation(wl, rep, x[selt], y[selt], psi[selt], rg[selt], None, selt, f"step {t} (production kernel)")
+        # the reset of the step's done list, prepared by the step where the sim has that path
+        d1, e1 = s.episode_state()
+        s.reset(buf.states, None, seeds_t[t + 1], buf.ranges, buf.gobs)
+        torch.cuda.synchronize()
+        check_reset(done, seeds_np[t + 1], post, d1, e1, rg, f"step {t} reset")
+    rep.add("steps", steps)
+    cnt = s.counters()
+    rep.add("resets_prepared", cnt["resets_prepared"])
+    rep.add("rays_cast", cnt["rays_cast"])
     s.close(); r.close(); m.close()
     assert_ambiguity_bounds(rep)
     return rep

@@ -396,6 +396,44 @@ def test_long_trajectories_c2_and_c5(pu):
     assert rep.c["steps"] == 500
 
 
+def test_production_launch_sequence_against_the_oracle(pu):
+    # What bench.py times, held against the oracle with no GPU kernel in between: no hit cells bound (fn_step runs the
+    # production step kernel step_beam_kernel<1,0,0,1>, not the instrumented one), reset seeds announced before every
+    # step, fn_reset(mask = NULL) served by prepared_reset_kernel.  States, collision, goal obs, done, reward, reset
+    # states and RANGES against the oracle at the usual tolerances: C2's full batch over 50 steps (all beams on steps
+    # 0-2, 192 envs' beams on every step), C3's full batch (union-free nonconvex footprint, omni drive), and C5 at
+    # 16 384 envs with the ring attached (map read through L2: production beam kernel, no prepared resets).
+    from harness import workloads as W
+    wl = W.make_workload(2)
+    wl.forced_reset_frac = 0.02
+    rep = pu.run_production_parity(wl, steps=50, subset=192)
+    print(rep)
+    assert rep.c["resets_prepared"] > 0.5 * (rep.c["resets"] - wl.n_envs) > 0, rep
+    assert rep.c["beams"] >= 3 * wl.n_envs * wl.n_beams
+    wl = W.make_workload(3)
+    rep = pu.run_production_parity(wl, steps=8, subset=128, full_steps=(0,))
+    print(rep)
+    assert rep.c["resets_prepared"] > 0, rep
+    wl = W.make_workload(5, n_envs=16384)
+    rep = pu.run_production_parity(wl, steps=6, subset=96, full_steps=(), ring=True)
+    print(rep)
+    assert rep.c["resets_prepared"] == 0 and rep.c["resets"] > wl.n_envs
+
+
+def test_prepared_reset_without_its_head_start(pu, monkeypatch):
+    # prepared_reset_kernel works under the step kernel's tail once the step's outcome warps have reported in; if they
+    # have not within its patience (a debugger, a time-sliced context) it waits for the whole step instead and does
+    # the same work afterwards -- no guard that could kill the context.  FLASHNAV_PREP_SPIN=0 (read at fn_sim_create)
+    # forces that branch: the production sequence must still agree with the oracle, resets prepared.
+    from harness import workloads as W
+    monkeypatch.setenv("FLASHNAV_PREP_SPIN", "0")
+    wl = W.make_workload(2)
+    wl.forced_reset_frac = 0.03
+    rep = pu.run_production_parity(wl, steps=6, subset=96, full_steps=(0,))
+    print(rep)
+    assert rep.c["resets_prepared"] > 0.5 * (rep.c["resets"] - wl.n_envs) > 0, rep
+
+
 def test_full_size_sampled_c3_c4(pu):
     # BASELINE.json's full batch sizes in the launch configuration bench.py times; beams of a fixed random
     # subset of envs against the oracle, everything per-env (motion, collision, goal obs, reward/done) in full.

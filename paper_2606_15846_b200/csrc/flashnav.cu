@@ -128,6 +128,8 @@ struct fn_sim {
     unsigned prep_map_ver, prep_robot_ver;
     PreparedReset d_prep;
     int* d_prep_epstep;
+    unsigned prep_spin;              // polls (64 ns apart) prepared_reset_kernel grants the step's outcome warps before it
+                                     // falls back to waiting for the whole step; FLASHNAV_PREP_SPIN overrides (tests: 0)
     // the coarse level in the production beam kernels (one CTA of 1024 threads per SM, fine + coarse copies staged)
     bool coarse_ok, coarse_on, split_ok_c;
     size_t beam_smem_c, split_smem_c;
@@ -462,6 +464,8 @@ extern "C" int fn_sim_create(const fn_map* map, const fn_robot* robot, int n, co
     std::memset(s, 0, sizeof(*s));
     s->map = map; s->robot = robot; s->n = n; s->stream = (cudaStream_t)stream;
     if (task) s->task = *task; else fn_task_default(&s->task);
+    s->prep_spin = 1u << 16;                                       // ~4 ms; the flag is normally up before the kernel starts
+    if (const char* v = std::getenv("FLASHNAV_PREP_SPIN")) s->prep_spin = (unsigned)std::strtoul(v, nullptr, 10);
     if (!(s->task.goal_dist_min_m >= 0.0f) || !(s->task.goal_dist_max_m >= s->task.goal_dist_min_m)) {
         delete s;
         return fail(FN_ERR_INVALID_ARG, "fn_sim_create: goal distance range must satisfy 0 <= min <= max");
@@ -883,7 +887,7 @@ extern "C" int fn_reset(fn_sim* s, float* states, const uint8_t* mask, const uin
         BeamArgs b = beam_args(s, list, count, out_ranges, false, true);
         b.poses = s->d_prep.poses;
         FN_CUDA(launch_pdl(prepared_reset_kernel, dim3(s->prep_grid), dim3(kBeamThreads), s->beam_smem, s->stream, a, b, s->d_prep,
-                           (const StepEnd*)s->d_step_end, (unsigned)s->split_grid));
+                           (const StepEnd*)s->d_step_end, (unsigned)s->split_grid, s->prep_spin));
         if (s->prof) { FN_CUDA(cudaEventRecord(e2, s->stream)); FN_CUDA(cudaEventRecord(e3, s->stream)); }
     } else if (fused) {
         // one launch: every CTA resets its share of the list from its shared copy of the map, then casts

@@ -797,11 +797,13 @@ __device__ __forceinline__ void stage_beam_constants(const BeamArgs& a, double2*
         if (stage) for (int i = (int)(map_bytes >> 2); i < mapWords; ++i) s_map[i] = __ldg(a.map.row + i);   // < 16 bytes
     }
     // phase 0 completes when the armed byte count has arrived
+    // (try_wait gives up after a system-dependent time and is simply asked again: the copies were issued by this CTA
+    // from addresses the host checked, so they complete -- or fault on their own; a bound on the polls could only
+    // misfire under a debugger or a time-sliced context, and there is nothing sensible to do without the map)
     uint32_t done = 0;
-    for (int it = 0; it < (1 << 24) && !done; ++it)
+    while (!done)
         asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], 0;\n\tselp.u32 %0, 1, 0, p;\n\t}"
                      : "=r"(done) : "r"(mb) : "memory");
-    if (!done) __trap();                                           // (never: a lost copy must not hang the device)
 }
 
 // The warps of the (persistent) grid take their tasks in two parts.  Beams differ in length by an order of

@@ -127,7 +127,8 @@ __global__ void __launch_bounds__(kFusedThreads, 2) reset_beam_kernel(const __gr
 // warps never wait for anything.
 constexpr unsigned kCopyFirstCta = 48u;
 __global__ void __launch_bounds__(kBeamThreads, 2) prepared_reset_kernel(const __grid_constant__ ResetArgs ra, const __grid_constant__ BeamArgs a,
-                                                                        const PreparedReset pr, const StepEnd* end, const unsigned n_outcome_warps) {
+                                                                        const PreparedReset pr, const StepEnd* end, const unsigned n_outcome_warps,
+                                                                        const unsigned max_spin) {
     extern __shared__ __align__(16) uint8_t smem_raw[];
     const int B = a.robot.B;
     const int mapWords = (a.map.H + 2 * kLineGuard) * a.map.strideR + (a.map.W + 2 * kLineGuard) * a.map.strideC;
@@ -136,15 +137,23 @@ __global__ void __launch_bounds__(kBeamThreads, 2) prepared_reset_kernel(const _
     __shared__ __align__(8) unsigned long long s_mbar;
     __shared__ __align__(16) FastShared<kBeamThreads / 32> s_fast;
     stage_beam_constants(a, s_tab, s_map, mapWords, true, &s_mbar);
-    if (threadIdx.x == 0) {                                        // the step's outcome warps have all finished?
+    // The step's outcome warps have all finished?  They do tens of us before this kernel starts; should the flag not
+    // arrive within max_spin polls all the same (a debugger, a time-sliced or preempted context), the CTA gives up the
+    // head start instead of the process: it waits for the step to COMPLETE first -- list, poses and flags are then
+    // final by definition -- and does the same work behind the wait.  No guard that can fire, same results.
+    __shared__ int s_early;
+    if (threadIdx.x == 0) {
         const volatile unsigned* flag = &end->outcomes_done;
-        for (int it = 0; *flag < n_outcome_warps; ++it) {
-            if (it > (1 << 22)) __trap();                          // (never: they finish tens of us before this kernel starts)
+        int ok = max_spin != 0u && *flag >= n_outcome_warps;      // (max_spin = 0: never take the head start -- tests)
+        for (unsigned it = 1; it < max_spin && !ok; ++it) {
             __nanosleep(64);
+            ok = *flag >= n_outcome_warps;
         }
+        s_early = ok;
         __threadfence();
     }
     __syncthreads();
+    if (!s_early) griddep_wait();
     // (read past L1: these words were written while this SM may have held older copies of their lines)
     const int q = __ldcg(&end->par_used);
     const int* rlist = ra.list + (size_t)q * ra.n;

@@ -659,6 +659,15 @@ def main():
     ap.add_argument("--ring", type=int, default=1, help="attach the replay ring when the config has one (C5)")
     ap.add_argument("--terminal", type=int, default=1, help="with the ring: keep pre-reset observations (fn_ring_attach_terminal)")
     args = ap.parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # started by hand without torchrun: launch the ranks ourselves (one process per GPU, replicas only -- there is
+        # no per-step collective; NCCL serves the barrier and the max over ranks of the timing)
+        import socket
+        with socket.socket() as sk:
+            sk.bind(("127.0.0.1", 0))
+            port = sk.getsockname()[1]
+        os.execv(sys.executable, [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+                                  "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:])
     if args.impl == "reference":
         # the counts the caller gave are honoured (same accounting as our arm); without flags a bounded sample:
         # a C2 step takes ~0.9 s on one core

@@ -10,7 +10,8 @@ Checked here: its ranges and goal observations against fn_observe_all's (the exi
 buffers) -- bit for bit, which is the bar the other GPU tests set between two launches of the same beam kernel on the
 same poses -- on two calls IN A ROW that differ in batch size and poses, so that what the first call leaves in the
 shared array (poses of envs the second call does not have, a used-up task counter) would show; that the pair of calls
-leaves the free device memory where it was; and that a batch beyond the limit is refused with a message that says so.
+leaves the free device memory where it was; that a batch beyond the limit is refused with a message that says so; and,
+for a sample of envs, its ranges and goal observations against the CPU oracle directly.
 
 This file sorts after every other test file on purpose (pytest -x stops at the first failure: a failure here must not
 hide the parity tests), and needs nothing from them: it passes alone in a fresh process as well as after them.
@@ -85,6 +86,21 @@ def test_two_calls_in_a_row_equal_observe_all(env, cfg, n_first, n_second):
             raise AssertionError(f"call {k} (n = {n}): env {bad[0]} beam {bad[1]}: {ranges[bad[0], bad[1]].item()!r} "
                                  f"vs fn_observe_all's {eranges[bad[0], bad[1]].item()!r}")
         assert torch.equal(gobs, egobs), f"call {k}: goal observations differ from fn_observe_all's"
+    # ... and against the oracle itself (ranges of 48 envs of the second call at the usual 1e-4 m outside the oracle's
+    # near-tie class, goal observations of all): the entry point stands on its own, not only on fn_observe_all
+    import oracle
+    oracle.build()
+    n, st = calls[1]
+    stn = st.cpu().numpy()
+    idx = np.arange(0, n, max(1, n // 48))[:48]
+    ro, _, amb = oracle.ranges(wl.occ, wl.resolution, wl.beam_angles, wl.max_range, stn[0, idx], stn[1, idx], stn[2, idx])
+    got = outs[1][0].cpu().numpy()[idx]
+    ok = amb == 0
+    assert ok.mean() > 0.99
+    assert np.abs(got.astype(np.float64) - ro.astype(np.float64))[ok].max() <= 1e-4
+    og = oracle.goal_obs(stn[0], stn[1], stn[2], stn[6], stn[7])
+    gg = outs[1][1].cpu().numpy()
+    assert np.all(np.abs(gg[0] - og[0]) <= 1e-5 * np.maximum(1.0, np.abs(og[0])))
     # the goal observation is optional
     only_ranges = torch.full((n_second, B), -2.0, device="cuda")
     fn.observe_noalloc(m, r, n_second, calls[1][1], only_ranges)
